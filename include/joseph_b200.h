@@ -1,0 +1,132 @@
+/*
+ * joseph_b200.h -- C ABI of libjoseph_b200.so: Joseph's ray-driven 3-D forward projection and its
+ * exact adjoint for PET on one NVIDIA B200 (sm_100a), non-TOF and TOF, sinogram and listmode, plus a
+ * listmode OSEM driver.  After arxiv 2212.12519 ("parallelproj"); citations are PAPER.md:<line>.
+ *
+ * The calls follow the paper's problem statement (section 2.2): the low-level
+ * projectors take "a list of coordinates representing the start and end point of the rays", are
+ * agnostic to scanner geometry, exist in non-TOF and TOF mode, with TOF sinogram ("all available TOF
+ * bins along a ray") and TOF listmode ("one specific TOF bin") variants, and the back projections are
+ * "the exact adjoint of the forward projections".
+ *
+ * Conventions (readings A1-A14 are listed in DESIGN.md)
+ *   image   f[i0][i1][i2], float32, C order, axis 2 fastest.  n = dims, voxsize v (mm), origin o =
+ *           world coordinate (mm) of the CENTRE of voxel [0][0][0].
+ *   LOR j   runs from s_j = (xs,ys,zs)[j] to e_j = (xe,ye,ze)[j] (world mm), float32, SoA.
+ *   Joseph principal axis p = argmax_a |e_a - s_a| (ties: lowest a, decided on the
+ *           exact differences); for every voxel-centre plane x_p = o_p + i v_p crossed by the closed
+ *           segment [s,e]: bilinear interpolation of the four nearest neighbours of the crossing
+ *           point (voxels outside the image count as zero); sum over planes times
+ *           cf = v_p |e-s| / |e_p - s_p|.  A zero-length LOR projects to 0.
+ *   TOF one weight per crossed plane, evaluated at the crossing point, whose
+ *           signed distance from the LOR midpoint (positive towards e) is tau:
+ *             w(tau,c) = 1/2 [ erf(clamp(c+W/2-tau, -m, m)/(sigma sqrt2))
+ *                            - erf(clamp(c-W/2-tau, -m, m)/(sigma sqrt2)) ],  m = n_sigmas*sigma,
+ *           W = tofbin_width, c = centre of the TOF bin: a Gaussian truncated at +-n_sigmas sigma,
+ *           integrated over the bin, not renormalised.  Sinogram bin k = 0..n_tofbins-1 has
+ *           c_k = (k - (n_tofbins-1)/2) W + center_offset; listmode bin `it` (signed int16) has
+ *           c = it*W + center_offset.
+ *
+ * Memory   Unless a name ends in _host, ALL data pointers are DEVICE pointers owned by the caller
+ *           (e.g. torch tensors); jp_geom / jp_tof / jp_lors structs themselves are read on the host
+ *           at call time.  Inputs are const.  The library does not keep pointers after a call
+ *           returns, except inside a jp_plan (which owns only its own device buffers).
+ * Streams  Every call is asynchronous on the CUDA stream `stream` (a cudaStream_t passed as void*,
+ *           NULL = legacy default stream) and never synchronises the device, except the _host calls,
+ *           which return after their result is in host memory.
+ * Scratch  Some calls use stream-ordered scratch (cudaMallocAsync/cudaFreeAsync on `stream`).
+ * Errors   Return 0 on success.  Negative = error, nothing (more) enqueued:
+ *             JP_ERR_POINTER (-1) null pointer where data is required
+ *             JP_ERR_SIZE    (-2) n < 0, a dim <= 0, voxsize <= 0, n_tofbins < 1 (or > JP_MAX_TOFBINS),
+ *                                 sigma <= 0, tofbin_width <= 0, n_sigmas <= 0, n_subsets < 1 ...
+ *             JP_ERR_CUDA    (-3) a CUDA runtime call failed; text via jp_last_error()
+ *             JP_ERR_PLAN    (-4) invalid plan handle
+ *           n == 0 LORs is a successful no-op.  No exceptions or C++ types cross this boundary.
+ */
+#ifndef JOSEPH_B200_H
+#define JOSEPH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JP_OK 0
+#define JP_ERR_POINTER (-1)
+#define JP_ERR_SIZE (-2)
+#define JP_ERR_CUDA (-3)
+#define JP_ERR_PLAN (-4)
+
+#define JP_MAX_TOFBINS 64
+
+/* image geometry shared by all calls (host struct) */
+typedef struct jp_geom {
+    int32_t n[3];     /* voxels along axes 0,1,2 (axis 2 fastest in memory) */
+    float origin[3];  /* world mm of the centre of voxel [0][0][0] */
+    float voxsize[3]; /* mm, > 0, may be anisotropic */
+} jp_geom;
+
+/* TOF parameters (host struct), all lengths in mm (x = c t / 2) */
+typedef struct jp_tof {
+    float tofbin_width_mm;  /* W  > 0 */
+    float sigma_tof_mm;     /* sigma > 0 (FWHM / 2.3548) */
+    float n_sigmas;         /* truncation, PAPER.md:78 uses 3 */
+    int32_t n_tofbins;      /* sinogram bins per LOR (ignored by the listmode calls) */
+    float center_offset_mm; /* shift of the bin centres along the LOR, normally 0 */
+} jp_tof;
+
+/* LOR end points, struct of arrays, float32, world mm; each array has n elements (device) */
+typedef struct jp_lors {
+    const float *xs, *ys, *zs; /* start points */
+    const float *xe, *ye, *ze; /* end points */
+    int64_t n;
+} jp_lors;
+
+/* ---- non-TOF ---------------------------------------------------------------------- */
+/* p[j] = line integral of img along LOR j.  OVERWRITES p[0..n).  img: n[0]*n[1]*n[2] floats. */
+int jp_fwd(const jp_lors *lors, const float *img, const jp_geom *geom, float *p, void *stream);
+/* img += A^T y, the exact adjoint of jp_fwd (atomic adds PAPER.md:46).
+   ACCUMULATES into img (the caller zeroes it when a plain back projection is wanted). */
+int jp_back(const jp_lors *lors, const float *y, const jp_geom *geom, float *img, void *stream);
+
+/* ---- TOF sinogram: all n_tofbins bins of every LOR ------------------------------ */
+/* p[j*n_tofbins + k], bin fastest.  OVERWRITES p. */
+int jp_fwd_tof_sino(const jp_lors *lors, const float *img, const jp_geom *geom, const jp_tof *tof,
+                    float *p, void *stream);
+/* img += A_tof^T y, y[j*n_tofbins + k].  ACCUMULATES. */
+int jp_back_tof_sino(const jp_lors *lors, const float *y, const jp_geom *geom, const jp_tof *tof,
+                     float *img, void *stream);
+
+/* ---- TOF listmode: only the TOF bin tofbin[j] of event j --------------------------- */
+int jp_fwd_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *img, const jp_geom *geom,
+                  const jp_tof *tof, float *p, void *stream);
+int jp_back_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *y, const jp_geom *geom,
+                   const jp_tof *tof, float *img, void *stream);
+
+/* ---- diagnostics --------------------------------------------------------------------------------- */
+/* principal_axis[j] in {0,1,2} ("principal direction"); bit-exact against the oracle. */
+int jp_classify(const jp_lors *lors, uint8_t *principal_axis, void *stream);
+
+/* ---- listmode OSEM (Hudson & Larkin, PAPER.md:193 ref. 39) ------------------- */
+/* n_iter iterations over n_subsets subsets, subset m = events {e : e mod n_subsets == m}, in order:
+ *   ybar_e = (A_tof x)_e;  r_e = 1/ybar_e if ybar_e > 1e-9 else 0;  b = A_m^T r;
+ *   x <- x * b * n_subsets / sens  where sens > 0, else 0.
+ * img: in = start image, out = result.  sens: sensitivity image (device).  workspace: device buffer of
+ * at least jp_lm_osem_workspace_bytes() bytes.  All on `stream`, no host synchronisation. */
+size_t jp_lm_osem_workspace_bytes(int64_t n_events, const jp_geom *geom, int n_subsets);
+int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
+               const float *sens, float *img, int n_subsets, int n_iter, void *workspace,
+               size_t workspace_bytes, void *stream);
+
+/* ---- misc ----------------------------------------------------------------------------------------- */
+/* text of the last CUDA error seen by the calling thread ("" if none); valid until the next call */
+const char *jp_last_error(void);
+/* library version, e.g. 100 = 0.1.0 */
+int jp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JOSEPH_B200_H */

@@ -1,0 +1,253 @@
+"""Thin ctypes binding over libjoseph_b200.so -- same names as include/joseph_b200.h.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of the library.  PyTorch
+is used for device memory and streams.  There is NO CPU fallback: if the library is missing or a
+tensor is not on a CUDA device the call raises.
+
+LOR end points are passed as two float32 CUDA tensors of shape (3, n) (row a = coordinate a of all
+LORs: the SoA layout of the C ABI) or as any tensors whose rows are contiguous.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libjoseph_b200.so")
+_lib = None
+
+JP_MAX_TOFBINS = 64
+
+
+class JosephError(RuntimeError):
+    pass
+
+
+class jp_geom(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("origin", C.c_float * 3), ("voxsize", C.c_float * 3)]
+
+
+class jp_tof(C.Structure):
+    _fields_ = [("tofbin_width_mm", C.c_float), ("sigma_tof_mm", C.c_float), ("n_sigmas", C.c_float),
+                ("n_tofbins", C.c_int32), ("center_offset_mm", C.c_float)]
+
+
+class jp_lors(C.Structure):
+    _fields_ = [("xs", C.c_void_p), ("ys", C.c_void_p), ("zs", C.c_void_p),
+                ("xe", C.c_void_p), ("ye", C.c_void_p), ("ze", C.c_void_p), ("n", C.c_int64)]
+
+
+# every symbol include/joseph_b200.h declares (tests/test_abi.py checks header <-> library <-> this list)
+EXPORTS = {
+    "jp_fwd": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p, C.c_void_p]),
+    "jp_back": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p, C.c_void_p]),
+    "jp_fwd_tof_sino": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
+                                  C.c_void_p, C.c_void_p]),
+    "jp_back_tof_sino": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
+                                   C.c_void_p, C.c_void_p]),
+    "jp_fwd_tof_lm": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom),
+                                C.POINTER(jp_tof), C.c_void_p, C.c_void_p]),
+    "jp_back_tof_lm": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom),
+                                 C.POINTER(jp_tof), C.c_void_p, C.c_void_p]),
+    "jp_classify": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p]),
+    "jp_lm_osem_workspace_bytes": (C.c_size_t, [C.c_int64, C.POINTER(jp_geom), C.c_int]),
+    "jp_lm_osem": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
+                             C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "jp_last_error": (C.c_char_p, []),
+    "jp_version": (C.c_int, []),
+}
+
+
+def load():
+    """dlopen the library (works without a GPU; compute calls need one).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise JosephError(f"{LIB_PATH} not found: build it with `python -m paper_2212_12519_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in EXPORTS.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        msg = load().jp_last_error().decode()
+        raise JosephError(f"{what} failed with code {rc}: {msg}")
+
+
+def _stream(stream) -> C.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype, what: str) -> torch.Tensor:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise JosephError(f"{what} must be a CUDA tensor (no CPU fallback)")
+    if t.dtype != dtype:
+        raise JosephError(f"{what} must be {dtype}, got {t.dtype}")
+    return t
+
+
+def make_geom(n, origin, voxsize) -> jp_geom:
+    g = jp_geom()
+    for a in range(3):
+        g.n[a] = int(n[a])
+        g.origin[a] = float(origin[a])
+        g.voxsize[a] = float(voxsize[a])
+    return g
+
+
+def make_tof(tofbin_width, sigma_tof, n_sigmas=3.0, n_tofbins=1, center_offset=0.0) -> jp_tof:
+    return jp_tof(float(tofbin_width), float(sigma_tof), float(n_sigmas), int(n_tofbins), float(center_offset))
+
+
+def make_lors(xstart: torch.Tensor, xend: torch.Tensor):
+    """(3, n) float32 CUDA tensors -> jp_lors (plus the tensors to keep alive)."""
+    _dev(xstart, torch.float32, "xstart")
+    _dev(xend, torch.float32, "xend")
+    if xstart.ndim != 2 or xstart.shape[0] != 3 or xend.shape != xstart.shape:
+        raise JosephError("xstart / xend must both have shape (3, n)")
+    rows = []
+    for t in (xstart, xend):
+        for a in range(3):
+            row = t[a]
+            if not row.is_contiguous():
+                row = row.contiguous()
+            rows.append(row)
+    l = jp_lors(*[r.data_ptr() for r in rows], int(xstart.shape[1]))
+    return l, rows
+
+
+def _img(img: torch.Tensor) -> torch.Tensor:
+    _dev(img, torch.float32, "img")
+    if img.ndim != 3 or not img.is_contiguous():
+        raise JosephError("img must be a contiguous 3-D tensor (C order, axis 2 fastest)")
+    return img
+
+
+def jp_version() -> int:
+    return int(load().jp_version())
+
+
+def jp_classify(xstart, xend, stream=None) -> torch.Tensor:
+    l, keep = make_lors(xstart, xend)
+    out = torch.empty(l.n, dtype=torch.uint8, device=xstart.device)
+    _check(load().jp_classify(C.byref(l), out.data_ptr(), _stream(stream)), "jp_classify")
+    return out
+
+
+def jp_fwd(xstart, xend, img, origin, voxsize, out=None, stream=None) -> torch.Tensor:
+    l, keep = make_lors(xstart, xend)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    if out is None:
+        out = torch.empty(l.n, dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == l.n and out.is_contiguous()
+    _check(load().jp_fwd(C.byref(l), img.data_ptr(), C.byref(g), out.data_ptr(), _stream(stream)), "jp_fwd")
+    return out
+
+
+def jp_back(xstart, xend, y, n, origin, voxsize, img=None, stream=None) -> torch.Tensor:
+    """img += A^T y (a zero image is made when img is None)."""
+    l, keep = make_lors(xstart, xend)
+    _dev(y, torch.float32, "y")
+    assert y.numel() == l.n and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(tuple(int(x) for x in n), dtype=torch.float32, device=y.device)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back(C.byref(l), y.data_ptr(), C.byref(g), img.data_ptr(), _stream(stream)), "jp_back")
+    return img
+
+
+def jp_fwd_tof_sino(xstart, xend, img, origin, voxsize, tof: jp_tof, out=None, stream=None) -> torch.Tensor:
+    l, keep = make_lors(xstart, xend)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    if out is None:
+        out = torch.empty((l.n, tof.n_tofbins), dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == l.n * tof.n_tofbins and out.is_contiguous()
+    _check(load().jp_fwd_tof_sino(C.byref(l), img.data_ptr(), C.byref(g), C.byref(tof), out.data_ptr(),
+                                  _stream(stream)), "jp_fwd_tof_sino")
+    return out
+
+
+def jp_back_tof_sino(xstart, xend, y, n, origin, voxsize, tof: jp_tof, img=None, stream=None) -> torch.Tensor:
+    l, keep = make_lors(xstart, xend)
+    _dev(y, torch.float32, "y")
+    assert y.numel() == l.n * tof.n_tofbins and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(tuple(int(x) for x in n), dtype=torch.float32, device=y.device)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_tof_sino(C.byref(l), y.data_ptr(), C.byref(g), C.byref(tof), img.data_ptr(),
+                                   _stream(stream)), "jp_back_tof_sino")
+    return img
+
+
+def _bins(tofbin, n):
+    _dev(tofbin, torch.int16, "tofbin")
+    assert tofbin.numel() == n and tofbin.is_contiguous()
+    return tofbin
+
+
+def jp_fwd_tof_lm(xstart, xend, tofbin, img, origin, voxsize, tof: jp_tof, out=None, stream=None) -> torch.Tensor:
+    l, keep = make_lors(xstart, xend)
+    tofbin = _bins(tofbin, l.n)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    if out is None:
+        out = torch.empty(l.n, dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == l.n and out.is_contiguous()
+    _check(load().jp_fwd_tof_lm(C.byref(l), tofbin.data_ptr(), img.data_ptr(), C.byref(g), C.byref(tof),
+                                out.data_ptr(), _stream(stream)), "jp_fwd_tof_lm")
+    return out
+
+
+def jp_back_tof_lm(xstart, xend, tofbin, y, n, origin, voxsize, tof: jp_tof, img=None, stream=None) -> torch.Tensor:
+    l, keep = make_lors(xstart, xend)
+    tofbin = _bins(tofbin, l.n)
+    _dev(y, torch.float32, "y")
+    assert y.numel() == l.n and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(tuple(int(x) for x in n), dtype=torch.float32, device=y.device)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_tof_lm(C.byref(l), tofbin.data_ptr(), y.data_ptr(), C.byref(g), C.byref(tof),
+                                 img.data_ptr(), _stream(stream)), "jp_back_tof_lm")
+    return img
+
+
+def jp_lm_osem_workspace_bytes(n_events: int, n, n_subsets: int) -> int:
+    g = make_geom(n, (0, 0, 0), (1, 1, 1))
+    return int(load().jp_lm_osem_workspace_bytes(int(n_events), C.byref(g), int(n_subsets)))
+
+
+def jp_lm_osem(xstart, xend, tofbin, sens, img, origin, voxsize, tof: jp_tof, n_subsets: int, n_iter: int,
+               workspace=None, stream=None) -> torch.Tensor:
+    """Listmode OSEM in place on ``img`` (start image in, result out); returns img."""
+    l, keep = make_lors(xstart, xend)
+    tofbin = _bins(tofbin, l.n)
+    img = _img(img)
+    sens = _img(sens)
+    assert sens.shape == img.shape
+    g = make_geom(img.shape, origin, voxsize)
+    need = jp_lm_osem_workspace_bytes(l.n, img.shape, n_subsets)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=img.device)
+    assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= need
+    _check(load().jp_lm_osem(C.byref(l), tofbin.data_ptr(), C.byref(g), C.byref(tof), sens.data_ptr(),
+                             img.data_ptr(), int(n_subsets), int(n_iter), workspace.data_ptr(),
+                             workspace.numel() * workspace.element_size(), _stream(stream)), "jp_lm_osem")
+    return img

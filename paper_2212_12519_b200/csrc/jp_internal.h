@@ -1,0 +1,37 @@
+// jp_internal.h -- launcher declarations shared by the translation units of libjoseph_b200.so
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "jp_ray.cuh"
+
+namespace jp {
+
+// LOR index of work item c is j = first + c * stride (c = 0..count-1); per-LOR inputs/outputs
+// (p, y, tofbin) are indexed by j when `compact` is false and by c when it is true.
+struct Range {
+    int64_t first, stride, count;
+    bool compact;
+};
+
+cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_t st);
+
+cudaError_t launch_fwd(const Lors &l, Range rg, const float *img, const Geom &g, float *p, cudaStream_t st);
+cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, float *img, cudaStream_t st);
+
+cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const Geom &g, const Tof &t,
+                                float *p, cudaStream_t st);
+cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t,
+                                 float *img, cudaStream_t st);
+
+// lm_mode: 0 = p = A x;  1 = p = (A x > 1e-9) ? 1/(A x) : 0   (OSEM ratio fused into the epilogue)
+cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *img, const Geom &g,
+                              const Tof &t, float *p, int lm_mode, cudaStream_t st);
+cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
+                               const Tof &t, float *img, cudaStream_t st);
+
+// x = sens > 0 ? x * b * scale / sens : 0;  b = 0   (OSEM multiplicative update, clears b for the next subset)
+cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scale, int64_t nvox, cudaStream_t st);
+
+} // namespace jp

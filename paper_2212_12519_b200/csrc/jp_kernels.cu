@@ -1,0 +1,288 @@
+// jp_kernels.cu -- generic (unplanned) Joseph kernels: one thread walks one LOR plane by plane.
+//
+// These are the reference-grade CUDA kernels of the library: they accept any LOR list in any order
+// and need no scratch memory.  The planned / sorted kernels (jp_planned.cu) are measured against
+// them.  PAPER.md:33 (Joseph), :35/:78 (TOF kernel), :43 (sinogram vs listmode TOF), :44/:46
+// (exact adjoint via atomic adds).
+#include "jp_internal.h"
+
+namespace jp {
+
+constexpr int kBlock = 128;
+
+__device__ __forceinline__ int64_t lor_index(const Range &rg, int64_t c) { return rg.first + c * rg.stride; }
+__device__ __forceinline__ int64_t io_index(const Range &rg, int64_t c) { return rg.compact ? c : lor_index(rg, c); }
+
+// ---- principal axis only (diagnostic; bit-exact against the oracle) --------------------------------
+__global__ void k_classify(Lors l, int64_t n, uint8_t *__restrict__ axis)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const double d0 = (double)l.xe[j] - (double)l.xs[j];
+    const double d1 = (double)l.ye[j] - (double)l.ys[j];
+    const double d2 = (double)l.ze[j] - (double)l.zs[j];
+    axis[j] = (uint8_t)principal_axis(d0, d1, d2);
+}
+
+// ---- non-TOF ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlock) k_fwd(Lors l, Range rg, const float *__restrict__ img, Geom g,
+                                                float *__restrict__ p)
+{
+    const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
+    if (c >= rg.count) return;
+    Ray r;
+    ray_setup<false>(l, lor_index(rg, c), g, 0.f, 0.f, 0.f, r);
+    float acc = 0.f;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        acc += plane_value(img, r, k, cl);
+    }
+    p[io_index(rg, c)] = r.cf * acc;
+}
+
+__global__ void __launch_bounds__(kBlock) k_back(Lors l, Range rg, const float *__restrict__ y, Geom g,
+                                                 float *__restrict__ img)
+{
+    const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
+    if (c >= rg.count) return;
+    Ray r;
+    ray_setup<false>(l, lor_index(rg, c), g, 0.f, 0.f, 0.f, r);
+    if (r.nk == 0) return;
+    const float x = r.cf * y[io_index(rg, c)];
+    if (x == 0.f) return;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        plane_scatter(img, r, k, cl, x);
+    }
+}
+
+// ---- TOF sinogram ---------------------------------------------------------------------------------------
+// All bins of one LOR are accumulated by one thread while it walks the planes.  The
+// per-thread bin accumulators live in shared memory, bin-major with a padded row (conflict free),
+// and the block's [kBlock][nbins] output tile -- contiguous in global memory -- is written (or, for
+// the adjoint, read) fully coalesced.
+struct BinWindow {
+    int klo, khi;
+    float x_lo; // position of the lower edge of bin klo relative to tau
+};
+
+__device__ __forceinline__ BinWindow bin_window(const Tof &t, const TofK &tk, float inv_w, float cb, float tau)
+{
+    // bins k with [c_k - W/2, c_k + W/2] meeting [tau - m, tau + m]; k = round(tau'/W + cb)
+    BinWindow b;
+    b.klo = max(0, (int)floorf((tau - tk.lim) * inv_w + cb + 0.5f));
+    b.khi = min(t.nbins - 1, (int)floorf((tau + tk.lim) * inv_w + cb + 0.5f));
+    b.x_lo = ((float)b.klo - cb) * t.width - tk.half_w - tau;
+    return b;
+}
+
+__global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, const float *__restrict__ img, Geom g,
+                                                         Tof t, float *__restrict__ p)
+{
+    extern __shared__ float acc[]; // [nbins][kBlock + 1]
+    constexpr int ld = kBlock + 1;
+    const int tid = threadIdx.x;
+    const int64_t j0 = blockIdx.x * (int64_t)kBlock;
+    const int64_t j = j0 + tid;
+    for (int kb = 0; kb < t.nbins; ++kb) acc[kb * ld + tid] = 0.f;
+    if (j < n) {
+        const TofK tk = make_tofk(t);
+        const float cb = 0.5f * (float)(t.nbins - 1);
+        const float inv_w = 1.f / t.width;
+        const float reach = cb * t.width + tk.half_w + tk.lim;
+        Ray r;
+        ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
+        for (int k = 0; k < r.nk; ++k) {
+            const Cell cl = plane_cell(r, k);
+            const float val = r.cf * plane_value(img, r, k, cl);
+            const float tau = fmaf(r.dtau, (float)k, r.tau0);
+            const BinWindow bw = bin_window(t, tk, inv_w, cb, tau);
+            float x = bw.x_lo;
+            float e_lo = edge_erf(tk, x);
+            for (int kb = bw.klo; kb <= bw.khi; ++kb) {
+                x += t.width;
+                const float e_hi = edge_erf(tk, x);
+                acc[kb * ld + tid] += val * (0.5f * (e_hi - e_lo));
+                e_lo = e_hi;
+            }
+        }
+    }
+    __syncthreads();
+    const int nvalid = (int)min((int64_t)kBlock, n - j0);
+    float *out = p + j0 * t.nbins;
+    for (int x = tid; x < nvalid * t.nbins; x += kBlock) {
+        const int lor = x / t.nbins, kb = x - lor * t.nbins;
+        out[x] = acc[kb * ld + lor];
+    }
+}
+
+__global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, const float *__restrict__ y, Geom g,
+                                                          Tof t, float *__restrict__ img)
+{
+    extern __shared__ float ysm[]; // [nbins][kBlock + 1]
+    constexpr int ld = kBlock + 1;
+    const int tid = threadIdx.x;
+    const int64_t j0 = blockIdx.x * (int64_t)kBlock;
+    const int64_t j = j0 + tid;
+    const int nvalid = (int)min((int64_t)kBlock, n - j0);
+    const float *in = y + j0 * t.nbins;
+    for (int x = tid; x < nvalid * t.nbins; x += kBlock) {
+        const int lor = x / t.nbins, kb = x - lor * t.nbins;
+        ysm[kb * ld + lor] = in[x];
+    }
+    __syncthreads();
+    if (j >= n) return;
+    const TofK tk = make_tofk(t);
+    const float cb = 0.5f * (float)(t.nbins - 1);
+    const float inv_w = 1.f / t.width;
+    const float reach = cb * t.width + tk.half_w + tk.lim;
+    Ray r;
+    ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+        const BinWindow bw = bin_window(t, tk, inv_w, cb, tau);
+        float x = bw.x_lo;
+        float e_lo = edge_erf(tk, x);
+        float s = 0.f;
+        for (int kb = bw.klo; kb <= bw.khi; ++kb) {
+            x += t.width;
+            const float e_hi = edge_erf(tk, x);
+            s = fmaf(ysm[kb * ld + tid], 0.5f * (e_hi - e_lo), s);
+            e_lo = e_hi;
+        }
+        if (s != 0.f) plane_scatter(img, r, k, cl, r.cf * s);
+    }
+}
+
+// ---- TOF listmode ---------------------------------------------------------------------------------------
+// Only the planes inside the truncated kernel of the event's own bin are visited.
+template <int LM_MODE>
+__global__ void __launch_bounds__(kBlock) k_fwd_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
+                                                       const float *__restrict__ img, Geom g, Tof t,
+                                                       float *__restrict__ p)
+{
+    const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
+    if (c >= rg.count) return;
+    const int64_t j = lor_index(rg, c);
+    const TofK tk = make_tofk(t);
+    const float centre = (float)tofbin[j] * t.width;
+    const float reach = tk.half_w + tk.lim;
+    Ray r;
+    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    float acc = 0.f;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+        acc = fmaf(plane_value(img, r, k, cl), tof_weight(tk, tau, centre), acc);
+    }
+    float out = r.cf * acc;
+    if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
+    p[io_index(rg, c)] = out;
+}
+
+__global__ void __launch_bounds__(kBlock) k_back_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
+                                                        const float *__restrict__ y, Geom g, Tof t,
+                                                        float *__restrict__ img)
+{
+    const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
+    if (c >= rg.count) return;
+    const int64_t j = lor_index(rg, c);
+    const float yj = y[io_index(rg, c)];
+    if (yj == 0.f) return;
+    const TofK tk = make_tofk(t);
+    const float centre = (float)tofbin[j] * t.width;
+    const float reach = tk.half_w + tk.lim;
+    Ray r;
+    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    const float x = r.cf * yj;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+        const float w = tof_weight(tk, tau, centre);
+        if (w != 0.f) plane_scatter(img, r, k, cl, x * w);
+    }
+}
+
+// ---- OSEM element-wise update ---------------------------------------------------------------------------
+__global__ void k_osem_update(float *__restrict__ x, float *__restrict__ b, const float *__restrict__ sens,
+                              float scale, int64_t nvox)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= nvox) return;
+    const float s = sens[i];
+    x[i] = (s > 0.f) ? x[i] * b[i] * scale / s : 0.f;
+    b[i] = 0.f;
+}
+
+// ---- launchers --------------------------------------------------------------------------------------------
+static inline unsigned grid_for(int64_t n, int block) { return (unsigned)((n + block - 1) / block); }
+
+cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_classify<<<grid_for(n, 256), 256, 0, st>>>(l, n, axis);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fwd(const Lors &l, Range rg, const float *img, const Geom &g, float *p, cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    k_fwd<<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, rg, img, g, p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, float *img, cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    k_back<<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, rg, y, g, img);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const Geom &g, const Tof &t, float *p,
+                                cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    if (rg.first != 0 || rg.stride != 1) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)t.nbins * (kBlock + 1) * sizeof(float);
+    k_fwd_tof_sino<<<grid_for(rg.count, kBlock), kBlock, smem, st>>>(l, rg.count, img, g, t, p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t, float *img,
+                                 cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    if (rg.first != 0 || rg.stride != 1) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)t.nbins * (kBlock + 1) * sizeof(float);
+    k_back_tof_sino<<<grid_for(rg.count, kBlock), kBlock, smem, st>>>(l, rg.count, y, g, t, img);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *img, const Geom &g,
+                              const Tof &t, float *p, int lm_mode, cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    if (lm_mode == 1)
+        k_fwd_tof_lm<1><<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, tofbin, rg, img, g, t, p);
+    else
+        k_fwd_tof_lm<0><<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, tofbin, rg, img, g, t, p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
+                               const Tof &t, float *img, cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    k_back_tof_lm<<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, tofbin, rg, y, g, t, img);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scale, int64_t nvox, cudaStream_t st)
+{
+    if (nvox == 0) return cudaSuccess;
+    k_osem_update<<<grid_for(nvox, 256), 256, 0, st>>>(x, b, sens, scale, nvox);
+    return cudaGetLastError();
+}
+
+} // namespace jp

@@ -1,0 +1,228 @@
+// jp_ray.cuh -- per-LOR set-up shared by all Joseph kernels (device code only).
+//
+// PAPER.md:33 (section 2.1): "the algorithm first determines the principal direction in the image
+// that is most parallel to the ray and then steps through the image volume plane by plane along this
+// principal direction.  In every plane, the intersection point between the ray and the plane is
+// calculated ..."  The crossing point is an affine function of the plane index, so the whole set-up
+// (principal axis, plane range, affine coefficients, incidence-angle factor, TOF coordinate) is done
+// ONCE per LOR in float64 -- every discrete decision (axis, tie, first/last plane of the closed
+// segment) is then exact -- and the per-plane hot loop evaluates one float32 FMA per coordinate.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace jp {
+
+struct Geom {
+    int n[3];
+    float o[3];
+    float v[3];
+};
+
+struct Tof {
+    float width;      // W, TOF bin width (mm)
+    float sigma;      // sigma (mm)
+    float nsig;       // truncation in sigmas
+    int nbins;        // sinogram bins
+    float coff;       // centre offset (mm)
+};
+
+struct Lors {
+    const float *xs, *ys, *zs, *xe, *ye, *ze;
+};
+
+// Everything the plane loop needs.  Plane index i = i0 + k, k = 0..nk-1.
+struct Ray {
+    int p;            // principal axis
+    int i0, nk;       // first plane, number of planes (0: nothing to do)
+    float a1, b1;     // u_q1(k) = a1 + b1 k   (voxel units along q1)
+    float a2, b2;     // u_q2(k) = a2 + b2 k
+    float cf;         // v_p |d| / |d_p|
+    float tau0, dtau; // tau(k) = tau0 + dtau k  (mm from the LOR midpoint, + towards e, minus centre offset)
+    int n1, n2;       // image dims along q1, q2
+    int sp, s1, s2;   // element strides of p, q1, q2
+};
+
+__device__ __forceinline__ int principal_axis(double d0, double d1, double d2)
+{
+    // argmax |d_a| on the exact differences, ties -> lowest index (reading A3)
+    double a0 = fabs(d0), a1 = fabs(d1), a2 = fabs(d2);
+    int p = 0;
+    double m = a0;
+    if (a1 > m) { p = 1; m = a1; }
+    if (a2 > m) { p = 2; }
+    return p;
+}
+
+// The plane range is clipped to the planes whose crossing point has -1 < u_q < n_q for both in-plane
+// axes (all other planes contribute exactly zero: their four neighbours are outside the image).
+// WITH_TOF: also fill tau0/dtau and clip to the planes with tau_lo <= tau <= tau_hi (outside that
+// window every TOF weight the caller needs is exactly zero: the kernel is truncated).
+// Both clips are conservative (rounded outwards); they are optimisations, not decisions.
+template <bool WITH_TOF>
+__device__ __forceinline__ void ray_setup(const Lors &l, int64_t j, const Geom &g, float coff,
+                                          float tau_lo, float tau_hi, Ray &r)
+{
+    const double s[3] = {(double)l.xs[j], (double)l.ys[j], (double)l.zs[j]};
+    const double e[3] = {(double)l.xe[j], (double)l.ye[j], (double)l.ze[j]};
+    const double d[3] = {e[0] - s[0], e[1] - s[1], e[2] - s[2]}; // exact
+    r.nk = 0;
+    r.i0 = 0;
+    r.p = principal_axis(d[0], d[1], d[2]);
+    const int p = r.p;
+    const int q1 = (p == 0) ? 1 : 0;
+    const int q2 = (p == 2) ? 1 : 2;
+    r.n1 = g.n[q1];
+    r.n2 = g.n[q2];
+    const int st[3] = {g.n[1] * g.n[2], g.n[2], 1};
+    r.sp = st[p];
+    r.s1 = st[q1];
+    r.s2 = st[q2];
+    r.a1 = r.b1 = r.a2 = r.b2 = r.cf = r.tau0 = r.dtau = 0.f;
+    if (d[0] == 0.0 && d[1] == 0.0 && d[2] == 0.0) return; // reading A1
+
+    const double op = (double)g.o[p], vp = (double)g.v[p];
+    // ---- closed segment rule (reading A4): planes with min(s_p,e_p) <= o_p + i v_p <= max(s_p,e_p)
+    const double lo = fmin(s[p], e[p]), hi = fmax(s[p], e[p]);
+    const double np1 = (double)(g.n[p] - 1);
+    double flo = ceil((lo - op) / vp), fhi = floor((hi - op) / vp);
+    flo = fmin(fmax(flo, 0.0), np1 + 1.0);
+    fhi = fmin(fmax(fhi, -1.0), np1);
+    int ilo = (int)flo, ihi = (int)fhi;
+    // exact fix-up of the rounded divisions
+    if (ilo > 0 && op + (double)(ilo - 1) * vp >= lo) --ilo;
+    if (ilo <= g.n[p] - 1 && op + (double)ilo * vp < lo) ++ilo;
+    if (ihi < g.n[p] - 1 && op + (double)(ihi + 1) * vp <= hi) ++ihi;
+    if (ihi >= 0 && op + (double)ihi * vp > hi) --ihi;
+
+    // ---- crossing point in voxel units: u_q(i) = A_q + B_q i
+    const double inv_dp = 1.0 / d[p];
+    double A[2], B[2];
+    const int q[2] = {q1, q2};
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        const double ratio = d[q[c]] * inv_dp;
+        const double ivq = 1.0 / (double)g.v[q[c]];
+        B[c] = ratio * vp * ivq;
+        A[c] = (s[q[c]] - (double)g.o[q[c]] + (op - s[p]) * ratio) * ivq;
+        // conservative clip to -1 < u < n_q
+        const double nq = (double)g.n[q[c]];
+        if (B[c] == 0.0) {
+            if (A[c] <= -1.0 || A[c] >= nq) ihi = ilo - 1;
+        } else {
+            double ia = (-1.0 - A[c]) / B[c], ib = (nq - A[c]) / B[c];
+            double imin = fmin(ia, ib), imax = fmax(ia, ib);
+            imin = fmin(fmax(floor(imin), -1.0), np1 + 1.0);
+            imax = fmin(fmax(ceil(imax), -1.0), np1 + 1.0);
+            ilo = max(ilo, (int)imin);
+            ihi = min(ihi, (int)imax);
+        }
+    }
+    const double L = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    double tau0 = 0.0, dtau = 0.0;
+    if (WITH_TOF) {
+        // tau(i) = (t_i - 1/2) L - coff, t_i = (o_p + i v_p - s_p)/d_p   (reading A8)
+        dtau = vp * inv_dp * L;
+        tau0 = ((op - s[p]) * inv_dp - 0.5) * L - (double)coff;
+        double ia = ((double)tau_lo - tau0) / dtau, ib = ((double)tau_hi - tau0) / dtau;
+        double imin = fmin(ia, ib), imax = fmax(ia, ib);
+        imin = fmin(fmax(floor(imin), -1.0), np1 + 1.0);
+        imax = fmin(fmax(ceil(imax), -1.0), np1 + 1.0);
+        ilo = max(ilo, (int)imin);
+        ihi = min(ihi, (int)imax);
+    }
+    if (ihi < ilo) return;
+    r.i0 = ilo;
+    r.nk = ihi - ilo + 1;
+    r.a1 = (float)(A[0] + B[0] * (double)ilo);
+    r.b1 = (float)B[0];
+    r.a2 = (float)(A[1] + B[1] * (double)ilo);
+    r.b2 = (float)B[1];
+    r.cf = (float)(vp * L * fabs(inv_dp));
+    if (WITH_TOF) {
+        r.tau0 = (float)(tau0 + dtau * (double)ilo);
+        r.dtau = (float)dtau;
+    }
+}
+
+// One crossed plane: integer cell and bilinear weights of the crossing point.
+struct Cell {
+    int k1, k2;
+    float w1, w2; // fractions along q1, q2
+};
+
+__device__ __forceinline__ Cell plane_cell(const Ray &r, int k)
+{
+    const float fk = (float)k;
+    const float u1 = fmaf(r.b1, fk, r.a1);
+    const float u2 = fmaf(r.b2, fk, r.a2);
+    const float f1 = floorf(u1), f2 = floorf(u2);
+    Cell c;
+    c.k1 = (int)f1;
+    c.k2 = (int)f2;
+    c.w1 = u1 - f1;
+    c.w2 = u2 - f2;
+    return c;
+}
+
+// bilinear interpolation of the four nearest neighbours, zero outside the image (reading A5)
+__device__ __forceinline__ float plane_value(const float *__restrict__ img, const Ray &r, int k, const Cell &c)
+{
+    const float *ptr = img + (int64_t)(r.i0 + k) * r.sp + (int64_t)c.k1 * r.s1 + (int64_t)c.k2 * r.s2;
+    const bool in1a = (unsigned)c.k1 < (unsigned)r.n1, in1b = (unsigned)(c.k1 + 1) < (unsigned)r.n1;
+    const bool in2a = (unsigned)c.k2 < (unsigned)r.n2, in2b = (unsigned)(c.k2 + 1) < (unsigned)r.n2;
+    const float v00 = (in1a && in2a) ? __ldg(ptr) : 0.f;
+    const float v01 = (in1a && in2b) ? __ldg(ptr + r.s2) : 0.f;
+    const float v10 = (in1b && in2a) ? __ldg(ptr + r.s1) : 0.f;
+    const float v11 = (in1b && in2b) ? __ldg(ptr + r.s1 + r.s2) : 0.f;
+    const float lo = fmaf(c.w2, v01 - v00, v00);
+    const float hi = fmaf(c.w2, v11 - v10, v10);
+    return fmaf(c.w1, hi - lo, lo);
+}
+
+// adjoint of plane_value: img[...] += w x  with atomic adds
+__device__ __forceinline__ void plane_scatter(float *__restrict__ img, const Ray &r, int k, const Cell &c, float x)
+{
+    float *ptr = img + (int64_t)(r.i0 + k) * r.sp + (int64_t)c.k1 * r.s1 + (int64_t)c.k2 * r.s2;
+    const bool in1a = (unsigned)c.k1 < (unsigned)r.n1, in1b = (unsigned)(c.k1 + 1) < (unsigned)r.n1;
+    const bool in2a = (unsigned)c.k2 < (unsigned)r.n2, in2b = (unsigned)(c.k2 + 1) < (unsigned)r.n2;
+    const float xa = x * (1.f - c.w1), xb = x * c.w1;
+    const float m2 = 1.f - c.w2;
+    if (in1a && in2a) atomicAdd(ptr, xa * m2);
+    if (in1a && in2b) atomicAdd(ptr + r.s2, xa * c.w2);
+    if (in1b && in2a) atomicAdd(ptr + r.s1, xb * m2);
+    if (in1b && in2b) atomicAdd(ptr + r.s1 + r.s2, xb * c.w2);
+}
+
+// ---- TOF kernel (reading A10) -----------------------------------------------------
+// erf of a clamped bin edge: E(x) = erf(clamp(x, -m, m) * isc), isc = 1/(sigma sqrt 2)
+struct TofK {
+    float half_w; // W/2
+    float lim;    // n_sigmas * sigma
+    float isc;    // 1/(sigma sqrt2)
+    float width;
+};
+
+__device__ __forceinline__ TofK make_tofk(const Tof &t)
+{
+    TofK k;
+    k.half_w = 0.5f * t.width;
+    k.lim = t.nsig * t.sigma;
+    k.isc = (float)(1.0 / ((double)t.sigma * 1.4142135623730951));
+    k.width = t.width;
+    return k;
+}
+
+__device__ __forceinline__ float edge_erf(const TofK &k, float x)
+{
+    return erff(fminf(fmaxf(x, -k.lim), k.lim) * k.isc);
+}
+
+// weight of the bin centred at c seen from tau
+__device__ __forceinline__ float tof_weight(const TofK &k, float tau, float c)
+{
+    const float m = c - tau;
+    return 0.5f * (edge_erf(k, m + k.half_w) - edge_erf(k, m - k.half_w));
+}
+
+} // namespace jp

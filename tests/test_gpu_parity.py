@@ -1,0 +1,237 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) against the float64 oracle,
+element by element, on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+
+  forward      rel-L2 <= 1e-5  and  max abs <= 1e-4 * max|oracle|
+  back         per-voxel max abs <= 1e-4 * max|oracle|   (atomic summation order)
+  adjointness  GPU relative gap <= 1e-4
+  principal axis / counts: bit-exact
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2212_12519_b200 import binding as jp
+from paper_2212_12519_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FWD_REL_L2 = 1e-5
+MAX_ABS = 1e-4
+ADJ_GAP = 1e-4
+
+
+def assert_fwd(gpu: torch.Tensor, ref: np.ndarray):
+    g = gpu.detach().cpu().numpy().astype(np.float64).reshape(ref.shape)
+    assert np.isfinite(g).all()
+    den = np.linalg.norm(ref)
+    rel = np.linalg.norm(g - ref) / den if den > 0 else np.linalg.norm(g)
+    mx = np.abs(g - ref).max() if ref.size else 0.0
+    scale = np.abs(ref).max() if ref.size else 1.0
+    assert rel <= FWD_REL_L2, f"forward rel-L2 {rel:.3e}"
+    assert mx <= MAX_ABS * scale, f"forward max abs {mx:.3e} vs {MAX_ABS * scale:.3e}"
+    return rel, mx / scale
+
+
+def assert_back(gpu: torch.Tensor, ref: np.ndarray):
+    g = gpu.detach().cpu().numpy().astype(np.float64)
+    assert np.isfinite(g).all()
+    mx = np.abs(g - ref).max()
+    scale = np.abs(ref).max()
+    assert mx <= MAX_ABS * scale, f"back max abs {mx:.3e} vs {MAX_ABS * scale:.3e}"
+    return mx / scale
+
+
+def adj_gap(Ax, y, x, Aty):
+    a = float((Ax.double() * y.double()).sum())
+    b = float((x.double() * Aty.double()).sum())
+    return abs(a - b) / abs(a)
+
+
+def dev(a, device):
+    return torch.as_tensor(a).to(device).contiguous()
+
+
+# ---- config 0: the full small case ---------------------------------------------------------------------
+def test_config0_nontof(cuda_device):
+    c = inputs.config0()
+    g = c["geom"]
+    xs, xe = dev(c["xstart"], cuda_device), dev(c["xend"], cuda_device)
+    img, y = dev(c["img"], cuda_device), dev(c["y"], cuda_device)
+    # principal axis: bit exact
+    ax = jp.jp_classify(xs, xe).cpu().numpy()
+    assert np.array_equal(ax, oracle.classify(c["xstart"], c["xend"], g.n, g.origin, g.voxsize))
+    p = jp.jp_fwd(xs, xe, img, g.origin, g.voxsize)
+    assert p.shape == (50_000,)
+    assert_fwd(p, oracle.fwd(c["xstart"], c["xend"], c["img"], g.origin, g.voxsize))
+    b = jp.jp_back(xs, xe, y, g.n, g.origin, g.voxsize)
+    assert_back(b, oracle.back(c["xstart"], c["xend"], c["y"], g.n, g.origin, g.voxsize))
+    assert adj_gap(p, y, img, b) <= ADJ_GAP
+    # ACCUMULATE semantics
+    b2 = jp.jp_back(xs, xe, y, g.n, g.origin, g.voxsize, img=torch.full_like(b, 3.0))
+    assert torch.allclose(b2 - 3.0, b, rtol=1e-4, atol=1e-3)
+
+
+def test_config0_tof(cuda_device):
+    """config-0 LORs with a TOF model scaled to the 128 mm image (all three principal axes occur)"""
+    c = inputs.config0(n_lors=20_000)
+    g = c["geom"]
+    rng = np.random.default_rng(5)
+    tofp = inputs.TofParams(tofbin_width=9.0, sigma_tof=7.0, n_sigmas=3.0, n_tofbins=27)
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    xs, xe = dev(c["xstart"], cuda_device), dev(c["xend"], cuda_device)
+    img = dev(c["img"], cuda_device)
+    # sinogram
+    p = jp.jp_fwd_tof_sino(xs, xe, img, g.origin, g.voxsize, tof)
+    assert_fwd(p, oracle.fwd_tof_sino(c["xstart"], c["xend"], c["img"], g.origin, g.voxsize, *args))
+    y = rng.uniform(0, 1, (20_000, 27)).astype(np.float32)
+    b = jp.jp_back_tof_sino(xs, xe, dev(y, cuda_device), g.n, g.origin, g.voxsize, tof)
+    assert_back(b, oracle.back_tof_sino(c["xstart"], c["xend"], y, g.n, g.origin, g.voxsize, *args))
+    assert adj_gap(p, dev(y, cuda_device), img, b) <= ADJ_GAP
+    # listmode
+    it = rng.integers(-13, 14, 20_000).astype(np.int16)
+    pl = jp.jp_fwd_tof_lm(xs, xe, dev(it, cuda_device), img, g.origin, g.voxsize, tof)
+    assert_fwd(pl, oracle.fwd_tof_lm(c["xstart"], c["xend"], it, c["img"], g.origin, g.voxsize, *args[:3]))
+    yl = rng.uniform(0.5, 2, 20_000).astype(np.float32)
+    bl = jp.jp_back_tof_lm(xs, xe, dev(it, cuda_device), dev(yl, cuda_device), g.n, g.origin, g.voxsize, tof)
+    assert_back(bl, oracle.back_tof_lm(c["xstart"], c["xend"], it, yl, g.n, g.origin, g.voxsize, *args[:3]))
+    assert adj_gap(pl, dev(yl, cuda_device), img, bl) <= ADJ_GAP
+
+
+# ---- slices of configs 1-3 on the scanner geometry (several tiles + ragged tail) ----------------------
+@pytest.fixture(scope="module")
+def scanner():
+    g = inputs.GEOM_SCANNER
+    return g, inputs.phantom()
+
+
+def _sino_slice(views, radial):
+    xs, xe = inputs.sinogram_lors(views=views, radial=radial)
+    return xs, xe
+
+
+def test_config1_slice_nontof(cuda_device, scanner):
+    """views 0, 64 (exact 45 degree ties) and 100, radial offsets incl. the degenerate r=+-128 and a miss"""
+    g, ph = scanner
+    radial = [-128, -70, -64, -33, -20, -1, 0, 1, 7, 31, 50, 64, 65, 128]
+    xs, xe = _sino_slice([0, 64, 100], radial)
+    n = xs.shape[1]
+    assert n == 3 * len(radial) * 2304
+    # ragged tail: drop a few LORs so n is not a multiple of the block size
+    xs, xe = xs[:, : n - 37].contiguous(), xe[:, : n - 37].contiguous()
+    n -= 37
+    xsd, xed, imgd = xs.to(cuda_device), xe.to(cuda_device), dev(ph, cuda_device)
+    ax = jp.jp_classify(xsd, xed).cpu().numpy()
+    ax_ref = oracle.classify(xs.numpy(), xe.numpy(), g.n, g.origin, g.voxsize)
+    assert np.array_equal(ax, ax_ref)
+    p = jp.jp_fwd(xsd, xed, imgd, g.origin, g.voxsize)
+    ref = oracle.fwd(xs.numpy(), xe.numpy(), ph, g.origin, g.voxsize)
+    assert (ref > 0).mean() > 0.3
+    assert_fwd(p, ref)
+    y = inputs.uniform_values(n, 0.0, 1.0, seed=11)
+    b = jp.jp_back(xsd, xed, y.to(cuda_device), g.n, g.origin, g.voxsize)
+    assert_back(b, oracle.back(xs.numpy(), xe.numpy(), y.numpy(), g.n, g.origin, g.voxsize))
+    assert adj_gap(p, y.to(cuda_device), imgd, b) <= ADJ_GAP
+
+
+def test_config2_slice_tof_sino(cuda_device, scanner):
+    g, ph = scanner
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    xs, xe = _sino_slice([64, 240], [-40, -3, 0, 25, 64])
+    # every 7th ring pair keeps the oracle fast while spanning many blocks
+    xs, xe = xs[:, ::7].contiguous(), xe[:, ::7].contiguous()
+    n = xs.shape[1]
+    xsd, xed, imgd = xs.to(cuda_device), xe.to(cuda_device), dev(ph, cuda_device)
+    p = jp.jp_fwd_tof_sino(xsd, xed, imgd, g.origin, g.voxsize, tof)
+    ref = oracle.fwd_tof_sino(xs.numpy(), xe.numpy(), ph, g.origin, g.voxsize, *args)
+    assert_fwd(p, ref)
+    # T1 on the GPU result: bins sum to erf(3/sqrt2) x non-TOF
+    pn = jp.jp_fwd(xsd, xed, imgd, g.origin, g.voxsize)
+    assert torch.allclose(p.sum(1), 0.99730020393674 * pn, rtol=2e-5, atol=1e-3)
+    y = inputs.uniform_values((n, 29), 0.0, 1.0, seed=12)
+    b = jp.jp_back_tof_sino(xsd, xed, y.to(cuda_device), g.n, g.origin, g.voxsize, tof)
+    assert_back(b, oracle.back_tof_sino(xs.numpy(), xe.numpy(), y.numpy(), g.n, g.origin, g.voxsize, *args))
+    assert adj_gap(p, y.to(cuda_device), imgd, b) <= ADJ_GAP
+
+
+@pytest.fixture(scope="module")
+def events(scanner):
+    g, ph = scanner
+    xs, xe, tb = inputs.listmode_events(300_011, seed=inputs.BASE_SEED + 3, img=ph, chunk=1_000_000)
+    return xs, xe, tb
+
+
+def test_config3_slice_tof_lm(cuda_device, scanner, events):
+    g, ph = scanner
+    xs, xe, tb = events
+    n = xs.shape[1]
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    xsd, xed, tbd, imgd = xs.to(cuda_device), xe.to(cuda_device), tb.to(cuda_device), dev(ph, cuda_device)
+    p = jp.jp_fwd_tof_lm(xsd, xed, tbd, imgd, g.origin, g.voxsize, tof)
+    ref = oracle.fwd_tof_lm(xs.numpy(), xe.numpy(), tb.numpy(), ph, g.origin, g.voxsize, *args)
+    assert (ref > 0).mean() > 0.95
+    assert_fwd(p, ref)
+    y = inputs.uniform_values(n, 0.5, 2.0, seed=13)
+    b = jp.jp_back_tof_lm(xsd, xed, tbd, y.to(cuda_device), g.n, g.origin, g.voxsize, tof)
+    assert_back(b, oracle.back_tof_lm(xs.numpy(), xe.numpy(), tb.numpy(), y.numpy(), g.n, g.origin, g.voxsize, *args))
+    assert adj_gap(p, y.to(cuda_device), imgd, b) <= ADJ_GAP
+    # T3 on the GPU: listmode == sinogram column
+    sub = slice(0, 5000)
+    ps = jp.jp_fwd_tof_sino(xsd[:, sub].contiguous(), xed[:, sub].contiguous(), imgd, g.origin, g.voxsize, tof)
+    col = ps[torch.arange(5000, device=cuda_device), (tbd[sub].long() + 14)]
+    assert torch.allclose(col, p[sub], rtol=2e-5, atol=1e-4)
+
+
+def test_config4_small_osem(cuda_device, scanner, events):
+    """listmode OSEM on a reduced problem: 300k events, 5 subsets, 2 iterations, vs the float64 oracle"""
+    g, ph = scanner
+    xs, xe, tb = events
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    # sensitivity: non-TOF back projection of ones over a coarse set of sinogram LORs
+    sx, se = inputs.sinogram_lors(views=range(0, 256, 8), radial=range(-64, 65, 4))
+    sx, se = sx[:, ::5].contiguous(), se[:, ::5].contiguous()
+    sens64 = oracle.back(sx.numpy(), se.numpy(), np.ones(sx.shape[1]), g.n, g.origin, g.voxsize)
+    sens32 = sens64.astype(np.float32)
+    x0 = np.ones(g.n, dtype=np.float32)
+    ref = oracle.lm_osem(xs.numpy(), xe.numpy(), tb.numpy(), sens32.astype(np.float64), x0, g.origin, g.voxsize,
+                         *args, n_subsets=5, n_iter=2)
+    img = dev(x0, cuda_device).clone()
+    jp.jp_lm_osem(xs.to(cuda_device), xe.to(cuda_device), tb.to(cuda_device), dev(sens32, cuda_device), img,
+                  g.origin, g.voxsize, tof, n_subsets=5, n_iter=2)
+    got = img.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.abs(got - ref).max() / np.abs(ref).max()
+    assert rel <= 1e-4, f"OSEM rel-L2 {rel:.3e}"
+    assert mx <= 1e-3, f"OSEM max abs / max {mx:.3e}"
+
+
+# ---- edge cases ----------------------------------------------------------------------------------------
+def test_edge_cases(cuda_device):
+    g = inputs.GEOM_SMALL
+    img = torch.rand(g.n, device=cuda_device)
+    empty = torch.zeros((3, 0), device=cuda_device)
+    assert jp.jp_fwd(empty, empty, img, g.origin, g.voxsize).numel() == 0
+    b = jp.jp_back(empty, empty, torch.zeros(0, device=cuda_device), g.n, g.origin, g.voxsize)
+    assert float(b.abs().max()) == 0.0
+    # zero-length LOR, LOR missing the image, LOR ending inside the image
+    xs = torch.tensor([[1.0, 500.0, 3.0], [1.0, 500.0, 2.0], [1.0, 500.0, 1.0]], device=cuda_device)
+    xe = torch.tensor([[1.0, 600.0, 90.0], [1.0, 510.0, 5.0], [1.0, 505.0, 2.0]], device=cuda_device)
+    p = jp.jp_fwd(xs, xe, img, g.origin, g.voxsize)
+    ref = oracle.fwd(xs.cpu().numpy(), xe.cpu().numpy(), img.cpu().numpy(), g.origin, g.voxsize)
+    assert p[0] == 0 and p[1] == 0 and torch.isfinite(p).all()
+    assert abs(float(p[2]) - ref[2]) <= 1e-5 * abs(ref[2])
+    # error codes: bad sizes raise
+    with pytest.raises(jp.JosephError):
+        jp.jp_fwd(xs, xe, img, g.origin, (0.0, 1.0, 1.0))
+    with pytest.raises(jp.JosephError):
+        jp.jp_fwd_tof_sino(xs, xe, img, g.origin, g.voxsize, jp.make_tof(17.0, -1.0, 3.0, 29))
+    with pytest.raises(jp.JosephError):
+        jp.jp_fwd(xs.cpu(), xe.cpu(), img, g.origin, g.voxsize)   # no CPU fallback
