@@ -109,6 +109,11 @@ int jp_back_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *y, c
 /* principal_axis[j] in {0,1,2} ("principal direction"); bit-exact against the oracle. */
 int jp_classify(const jp_lors *lors, uint8_t *principal_axis, void *stream);
 
+/* total[0] += number of (LOR, plane) pairs the projectors visit for these LORs: planes of the principal
+   axis crossed by the closed segment whose crossing point has at least one of its four neighbours
+   inside the image (the "plane-steps" the roofline is quoted in).  total: device uint64, caller-zeroed. */
+int jp_plane_steps(const jp_lors *lors, const jp_geom *geom, unsigned long long *total, void *stream);
+
 /* ---- listmode OSEM (Hudson & Larkin, PAPER.md:193 ref. 39) ------------------- */
 /* n_iter iterations over n_subsets subsets, subset m = events {e : e mod n_subsets == m}, in order:
  *   ybar_e = (A_tof x)_e;  r_e = 1/ybar_e if ybar_e > 1e-9 else 0;  b = A_m^T r;
@@ -119,6 +124,14 @@ size_t jp_lm_osem_workspace_bytes(int64_t n_events, const jp_geom *geom, int n_s
 int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
                const float *sens, float *img, int n_subsets, int n_iter, void *workspace,
                size_t workspace_bytes, void *stream);
+
+/* ---- hybrid mode: HOST pointers in and out ---------------------------------------- */
+/* Same semantics as jp_fwd / jp_back, but every pointer (inside lors_host too) is a HOST pointer.  The
+ * LOR list is streamed through the current CUDA device in chunks on two internal streams (copies
+ * overlap kernels when the host memory is page-locked).  Allocates and frees its own device staging.
+ * Returns after the result is in host memory.  jp_back_host ACCUMULATES into img_host. */
+int jp_fwd_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, float *p_host);
+int jp_back_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, float *img_host);
 
 /* ---- misc ----------------------------------------------------------------------------------------- */
 /* text of the last CUDA error seen by the calling thread ("" if none); valid until the next call */

@@ -52,9 +52,12 @@ EXPORTS = {
     "jp_back_tof_lm": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom),
                                  C.POINTER(jp_tof), C.c_void_p, C.c_void_p]),
     "jp_classify": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p]),
+    "jp_plane_steps": (C.c_int, [C.POINTER(jp_lors), C.POINTER(jp_geom), C.c_void_p, C.c_void_p]),
     "jp_lm_osem_workspace_bytes": (C.c_size_t, [C.c_int64, C.POINTER(jp_geom), C.c_int]),
     "jp_lm_osem": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
                              C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
+    "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
     "jp_version": (C.c_int, []),
 }
@@ -142,6 +145,15 @@ def jp_classify(xstart, xend, stream=None) -> torch.Tensor:
     out = torch.empty(l.n, dtype=torch.uint8, device=xstart.device)
     _check(load().jp_classify(C.byref(l), out.data_ptr(), _stream(stream)), "jp_classify")
     return out
+
+
+def jp_plane_steps(xstart, xend, n, origin, voxsize, stream=None) -> int:
+    """number of (LOR, plane) pairs the projectors visit (synchronises to return a Python int)"""
+    l, keep = make_lors(xstart, xend)
+    g = make_geom(n, origin, voxsize)
+    total = torch.zeros(1, dtype=torch.int64, device=xstart.device)
+    _check(load().jp_plane_steps(C.byref(l), C.byref(g), total.data_ptr(), _stream(stream)), "jp_plane_steps")
+    return int(total.item())
 
 
 def jp_fwd(xstart, xend, img, origin, voxsize, out=None, stream=None) -> torch.Tensor:
@@ -250,4 +262,37 @@ def jp_lm_osem(xstart, xend, tofbin, sens, img, origin, voxsize, tof: jp_tof, n_
     _check(load().jp_lm_osem(C.byref(l), tofbin.data_ptr(), C.byref(g), C.byref(tof), sens.data_ptr(),
                              img.data_ptr(), int(n_subsets), int(n_iter), workspace.data_ptr(),
                              workspace.numel() * workspace.element_size(), _stream(stream)), "jp_lm_osem")
+    return img
+
+
+# ---- hybrid mode: host tensors in and out -------------------------------------------------------
+def _host_lors(xstart: torch.Tensor, xend: torch.Tensor):
+    for t in (xstart, xend):
+        if t.is_cuda or t.dtype != torch.float32 or t.ndim != 2 or t.shape[0] != 3:
+            raise JosephError("host end points must be CPU float32 tensors of shape (3, n)")
+    rows = [t[a] if t[a].is_contiguous() else t[a].contiguous() for t in (xstart, xend) for a in range(3)]
+    return jp_lors(*[r.data_ptr() for r in rows], int(xstart.shape[1])), rows
+
+
+def jp_fwd_host(xstart, xend, img, origin, voxsize, out=None) -> torch.Tensor:
+    """CPU tensors in, CPU tensor out; the projection itself runs on the current CUDA device."""
+    l, keep = _host_lors(xstart, xend)
+    if img.is_cuda or img.dtype != torch.float32 or not img.is_contiguous():
+        raise JosephError("img must be a contiguous CPU float32 tensor")
+    g = make_geom(img.shape, origin, voxsize)
+    if out is None:
+        out = torch.empty(l.n, dtype=torch.float32)
+    assert not out.is_cuda and out.numel() == l.n and out.is_contiguous()
+    _check(load().jp_fwd_host(C.byref(l), img.data_ptr(), C.byref(g), out.data_ptr()), "jp_fwd_host")
+    return out
+
+
+def jp_back_host(xstart, xend, y, img, origin, voxsize) -> torch.Tensor:
+    """img (CPU, float32) += A^T y, computed on the current CUDA device."""
+    l, keep = _host_lors(xstart, xend)
+    if img.is_cuda or img.dtype != torch.float32 or not img.is_contiguous():
+        raise JosephError("img must be a contiguous CPU float32 tensor")
+    assert not y.is_cuda and y.dtype == torch.float32 and y.numel() == l.n and y.is_contiguous()
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_host(C.byref(l), y.data_ptr(), C.byref(g), img.data_ptr()), "jp_back_host")
     return img

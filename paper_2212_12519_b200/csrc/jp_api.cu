@@ -6,19 +6,24 @@
 #include "../../include/joseph_b200.h"
 #include "jp_internal.h"
 
+namespace jp {
+thread_local char g_err_buf[512] = "";
+char *err_buf() { return g_err_buf; }
+} // namespace jp
+
 namespace {
 
-thread_local char g_err[512] = "";
+#define g_err jp::g_err_buf
 
 int fail_cuda(cudaError_t e, const char *where)
 {
-    snprintf(g_err, sizeof(g_err), "%s: %s (%s)", where, cudaGetErrorString(e), cudaGetErrorName(e));
+    snprintf(g_err, 512, "%s: %s (%s)", where, cudaGetErrorString(e), cudaGetErrorName(e));
     return JP_ERR_CUDA;
 }
 
 int fail(int code, const char *msg)
 {
-    snprintf(g_err, sizeof(g_err), "%s", msg);
+    snprintf(g_err, 512, "%s", msg);
     return code;
 }
 
@@ -92,6 +97,18 @@ int jp_classify(const jp_lors *lors, uint8_t *principal_axis, void *stream)
     JP_TRY(check_lors(lors, l));
     if (lors->n > 0 && !principal_axis) return fail(JP_ERR_POINTER, "principal_axis is NULL");
     JP_CUDA(jp::launch_classify(l, lors->n, principal_axis, (cudaStream_t)stream), "jp_classify");
+    return JP_OK;
+}
+
+int jp_plane_steps(const jp_lors *lors, const jp_geom *geom, unsigned long long *total, void *stream)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    JP_TRY(check_lors(lors, l));
+    JP_TRY(check_geom(geom, g));
+    if (!total) return fail(JP_ERR_POINTER, "total is NULL");
+    JP_CUDA(jp::launch_plane_steps(l, lors->n, g, total, (cudaStream_t)stream), "jp_plane_steps");
     return JP_OK;
 }
 

@@ -10,12 +10,17 @@ namespace jp {
 
 // LOR index of work item c is j = first + c * stride (c = 0..count-1); per-LOR inputs/outputs
 // (p, y, tofbin) are indexed by j when `compact` is false and by c when it is true.
+// per-thread error text returned by jp_last_error() (512 bytes)
+char *err_buf();
+
 struct Range {
     int64_t first, stride, count;
     bool compact;
 };
 
 cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_t st);
+
+cudaError_t launch_plane_steps(const Lors &l, int64_t n, const Geom &g, unsigned long long *total, cudaStream_t st);
 
 cudaError_t launch_fwd(const Lors &l, Range rg, const float *img, const Geom &g, float *p, cudaStream_t st);
 cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, float *img, cudaStream_t st);

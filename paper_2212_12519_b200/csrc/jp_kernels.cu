@@ -24,6 +24,19 @@ __global__ void k_classify(Lors l, int64_t n, uint8_t *__restrict__ axis)
     axis[j] = (uint8_t)principal_axis(d0, d1, d2);
 }
 
+__global__ void k_plane_steps(Lors l, int64_t n, Geom g, unsigned long long *__restrict__ total)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    unsigned long long nk = 0;
+    if (j < n) {
+        Ray r;
+        ray_setup<false>(l, j, g, 0.f, 0.f, 0.f, r);
+        nk = (unsigned long long)r.nk;
+    }
+    for (int o = 16; o > 0; o >>= 1) nk += __shfl_xor_sync(0xffffffffu, nk, o);
+    if ((threadIdx.x & 31) == 0 && nk) atomicAdd(total, nk);
+}
+
 // ---- non-TOF ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlock) k_fwd(Lors l, Range rg, const float *__restrict__ img, Geom g,
                                                 float *__restrict__ p)
@@ -222,6 +235,13 @@ cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_
 {
     if (n == 0) return cudaSuccess;
     k_classify<<<grid_for(n, 256), 256, 0, st>>>(l, n, axis);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_plane_steps(const Lors &l, int64_t n, const Geom &g, unsigned long long *total, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_plane_steps<<<grid_for(n, 256), 256, 0, st>>>(l, n, g, total);
     return cudaGetLastError();
 }
 
