@@ -120,7 +120,7 @@ int jp_fwd(const jp_lors *lors, const float *img, const jp_geom *geom, float *p,
     JP_TRY(check_lors(lors, l));
     JP_TRY(check_geom(geom, g));
     if (!img || (lors->n > 0 && !p)) return fail(JP_ERR_POINTER, "img or p is NULL");
-    JP_CUDA(jp::launch_fwd(l, whole(lors->n), img, g, p, (cudaStream_t)stream), "jp_fwd");
+    JP_CUDA(jp::launch_fwd_tile(l, lors->n, img, g, p, (cudaStream_t)stream), "jp_fwd");
     return JP_OK;
 }
 
@@ -132,7 +132,7 @@ int jp_back(const jp_lors *lors, const float *y, const jp_geom *geom, float *img
     JP_TRY(check_lors(lors, l));
     JP_TRY(check_geom(geom, g));
     if (!img || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "img or y is NULL");
-    JP_CUDA(jp::launch_back(l, whole(lors->n), y, g, img, (cudaStream_t)stream), "jp_back");
+    JP_CUDA(jp::launch_back_tile(l, lors->n, y, g, img, (cudaStream_t)stream), "jp_back");
     return JP_OK;
 }
 

@@ -101,7 +101,7 @@ int jp_fwd_host(const jp_lors *lors_host, const float *img_host, const jp_geom *
         const int64_t m = std::min(chunk, n - c0);
         jp::Lors l;
         if ((e = stage_coords(lors_host, c0, m, hp.coord[s], chunk, hp.st[s], l)) != cudaSuccess) break;
-        if ((e = jp::launch_fwd(l, jp::Range{0, 1, m, false}, hp.img, g, hp.val[s], hp.st[s])) != cudaSuccess) break;
+        if ((e = jp::launch_fwd_tile(l, m, hp.img, g, hp.val[s], hp.st[s])) != cudaSuccess) break;
         if ((e = cudaMemcpyAsync(p_host + c0, hp.val[s], sizeof(float) * m, cudaMemcpyDeviceToHost, hp.st[s])) != cudaSuccess) break;
     }
     for (int k = 0; k < kStreams; ++k) {
@@ -134,7 +134,7 @@ int jp_back_host(const jp_lors *lors_host, const float *y_host, const jp_geom *g
         jp::Lors l;
         if ((e = stage_coords(lors_host, c0, m, hp.coord[s], chunk, hp.st[s], l)) != cudaSuccess) break;
         if ((e = cudaMemcpyAsync(hp.val[s], y_host + c0, sizeof(float) * m, cudaMemcpyHostToDevice, hp.st[s])) != cudaSuccess) break;
-        if ((e = jp::launch_back(l, jp::Range{0, 1, m, false}, hp.val[s], g, hp.img, hp.st[s])) != cudaSuccess) break;
+        if ((e = jp::launch_back_tile(l, m, hp.val[s], g, hp.img, hp.st[s])) != cudaSuccess) break;
     }
     for (int k = 0; k < kStreams; ++k) {
         cudaError_t e2 = cudaStreamSynchronize(hp.st[k]);

@@ -25,6 +25,10 @@ cudaError_t launch_plane_steps(const Lors &l, int64_t n, const Geom &g, unsigned
 cudaError_t launch_fwd(const Lors &l, Range rg, const float *img, const Geom &g, float *p, cudaStream_t st);
 cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, float *img, cudaStream_t st);
 
+// tiled non-TOF kernels (jp_tile.cu): track tiles through shared memory, everything else per LOR
+cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st);
+cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st);
+
 cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const Geom &g, const Tof &t,
                                 float *p, cudaStream_t st);
 cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t,
