@@ -8,11 +8,13 @@
 // Joseph's bilinear interpolation factorises:
 //
 //   forward   C[i][z] = (1-w1(i)) f[i,k1(i),z] + w1(i) f[i,k1(i)+1,z]      built once per tile in shared
-//             p_j     = cf_j * sum_i lerp_z(C[i][.], u2_j(i))               memory, 2 LDS + ~13 instr/step
+//             p_j     = cf_j * sum_i lerp_z(C[i][.], u2_j(i))               memory as (value, slope) pairs:
+//                                                                          one 64-bit LDS + 7 FP32 per step
 //   adjoint   C[i][z] += cf_j y_j * hat(u2_j(i) - z)                        native int32 shared atomics on a
-//             img[i,k1,z] += (1-w1) C[i][z];  img[i,k1+1,z] += w1 C[i][z]   fixed-point tile, then coalesced REDs
+//             img[i,k1,z] += (1-w1) C[i][z];  img[i,k1+1,z] += w1 C[i][z]   fixed-point tile, then 128-bit REDs
 //
-// Planes are processed in chunks of 64 rows, so shared memory is 64 x (n2+4) x 4 B whatever the image.
+// Planes are processed in chunks of `rows_cap` rows (shared memory = rows_cap x P x 8 or 4 bytes; the
+// row pitch P is a template parameter so that the unrolled plane loop addresses rows with immediates).
 // Tiles that are not tracks (ragged tail, principal axis z, unsorted lists) take the generic per-LOR
 // path in the same launch.  No plan, no scratch memory, results in caller order.
 #include "jp_internal.h"
@@ -24,19 +26,27 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kPerThread = 3;
 constexpr int kTile = kThreads * kPerThread;
-constexpr int kChunk = 64;
-constexpr float kMagic = 12582912.f;   // 1.5 * 2^23: (x + kMagic) rounds x to the nearest integer
+constexpr float kMagic = 12582912.f;   // 1.5 * 2^23: fadd_rd(x, kMagic) holds floor(x) in the low mantissa bits
 constexpr int kMagicI = 0x4B400000;    // bit pattern of kMagic
-constexpr int kPad = 2;                // zero columns on both sides of a shared-memory row
+constexpr int kPad = 4;                // padding columns left of z = 0 in a shared-memory row
+constexpr int kPadR = 4;               // columns needed right of z = n2 - 1
 
 // shared per-tile track description, written by thread 0
 struct Track {
-    int p;          // principal axis (0 or 1); -1: not a track tile
+    int p;          // principal axis (0 or 1)
     int I0, I1;     // plane range of the track (closed segment rule and q1 clip); empty if I1 < I0
     float a1, b1;   // u_q1(i) = a1 + b1 (i - I0)
     double inv_dp;  // 1 / d_p
     double ops;     // o_p - s_p
     float R;        // 1 + (d_q1/d_p)^2
+};
+
+// q1 cell of one plane of the track (shared by the whole tile): element offsets of the two image rows
+// (i, k1, z = 0) and (i, k1 + 1, z = 0), -1 when the row lies outside the image (reading A5), and the
+// two q1 weights
+struct __align__(16) RowInfo {
+    int base_a, base_b;
+    float wa, wb;
 };
 
 __device__ __forceinline__ bool same_bits(float a, float b) { return __float_as_uint(a) == __float_as_uint(b); }
@@ -86,10 +96,29 @@ __device__ void track_setup(const Geom &g, float xs, float ys, float xe, float y
     t.R = (float)(1.0 + ratio * ratio);
 }
 
-// per-LOR axial part: u2(i) = a2h + 0.5 + b2 (i - i0), planes [i0, i1], incidence factor cf
+__device__ __forceinline__ RowInfo row_info(const Geom &g, const Track &t, int i)
+{
+    const int q1 = 1 - t.p;
+    const int st[2] = {g.n[1] * g.n[2], g.n[2]};
+    const float u1 = fmaf(t.b1, (float)(i - t.I0), t.a1);
+    const float f1 = floorf(u1);
+    const int k1 = (int)f1;
+    const float w1 = u1 - f1;
+    const bool in_a = (unsigned)k1 < (unsigned)g.n[q1];
+    const bool in_b = (unsigned)(k1 + 1) < (unsigned)g.n[q1];
+    const int base = i * st[t.p] + k1 * st[q1];
+    RowInfo r;
+    r.base_a = in_a ? base : -1;
+    r.base_b = in_b ? base + st[q1] : -1;
+    r.wa = in_a ? 1.f - w1 : 0.f;
+    r.wb = in_b ? w1 : 0.f;
+    return r;
+}
+
+// per-LOR axial part: u2(i) = a2 + b2 (i - i0), planes [i0, i1], incidence factor cf
 struct ZRay {
     int i0, i1;
-    float a2h, b2, cf;
+    float a2, b2, cf;
 };
 
 __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs, float ze)
@@ -117,18 +146,18 @@ __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs,
         ihi = min(ihi, (int)imax);
     }
     z.b2 = Bf;
-    z.a2h = (float)(A + B * (double)ilo - 0.5);
-    // trim: the rounded index must stay inside the padded row: -2 <= round(u2 - 1/2) <= n2
-    const float hmin = -2.4f, hmax = n2 + 0.4f;
+    z.a2 = (float)(A + B * (double)ilo);
+    // trim: floor(u2) must stay inside the padded row: -2 <= floor(u2) <= n2 (planes trimmed away have
+    // all four neighbours outside the image and contribute exactly zero)
+    const float umin = -1.9f, umax = n2 + 0.9f;
     while (ilo <= ihi) {
-        const float h = z.a2h;
-        if (h > hmin && h < hmax) break;
+        if (z.a2 > umin && z.a2 < umax) break;
         ++ilo;
-        z.a2h = (float)(A + B * (double)ilo - 0.5);
+        z.a2 = (float)(A + B * (double)ilo);
     }
     while (ilo <= ihi) {
-        const float h = fmaf(z.b2, (float)(ihi - ilo), z.a2h);
-        if (h > hmin && h < hmax) break;
+        const float u = fmaf(z.b2, (float)(ihi - ilo), z.a2);
+        if (u > umin && u < umax) break;
         --ihi;
     }
     z.i0 = ilo;
@@ -179,39 +208,48 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
     return __syncthreads_and(ok) != 0;
 }
 
-// row r of the chunk: q1 cell of plane i (shared by the whole tile)
-struct RowCell {
-    int base;     // element offset of (i, k1, z=0)
-    float w1;
-    bool in_a, in_b;
-};
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ RowCell row_cell(const Geom &g, const Track &t, int i)
+template <int OFF>
+__device__ __forceinline__ float2 lds_pair(uint32_t addr)
 {
-    const int q1 = 1 - t.p;
-    const int st[2] = {g.n[1] * g.n[2], g.n[2]};
-    const float u1 = fmaf(t.b1, (float)(i - t.I0), t.a1);
-    const float f1 = floorf(u1);
-    const int k1 = (int)f1;
-    RowCell c;
-    c.w1 = u1 - f1;
-    c.in_a = (unsigned)k1 < (unsigned)g.n[q1];
-    c.in_b = (unsigned)(k1 + 1) < (unsigned)g.n[q1];
-    c.base = i * st[t.p] + k1 * st[q1];
-    return c;
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(addr), "n"(OFF) : "memory");
+    return v;
+}
+
+template <int OFF>
+__device__ __forceinline__ void reds_add(uint32_t addr, int q)
+{
+    asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(q) : "memory");
 }
 
 } // namespace
 
 // ---- forward ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g,
-                                                       float *__restrict__ p)
+// One plane step of one LOR against the (value, slope) rows in shared memory: 4 FP32 for the
+// axial cell (FFMA, FADD.RM, FADD, FADD), one address LEA, one LDS.64, 2 FP32 to accumulate.
+#define JP_FWD_STEP(K, A2K)                                                    \
+    {                                                                          \
+        const float u = fmaf(b2, fk, A2K);                                     \
+        const float tt = __fadd_rd(u, kMagic);                                 \
+        const float w = u - (tt - kMagic);                                     \
+        const float2 v = lds_pair<(K) * P * 8>(row + (__float_as_uint(tt) << 3)); \
+        acc0 += v.x;                                                           \
+        acc1 = fmaf(w, v.y, acc1);                                             \
+    }
+
+template <int P>
+__global__ void __launch_bounds__(kThreads, 4)
+    k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
+               float *__restrict__ p)
 {
-    extern __shared__ float C[]; // [kChunk][ld]
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                      // [rows_cap][P]
+    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(float2)); // [max(n0,n1)]
     __shared__ Track trk;
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kTile;
-    const int ld = g.n[2] + 2 * kPad;
 
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
@@ -237,33 +275,87 @@ __global__ void __launch_bounds__(kThreads) k_fwd_tile(Lors l, int64_t n, const 
         for (int m = 0; m < kPerThread; ++m) p[j0 + m * kThreads + tid] = 0.f;
         return;
     }
+    const int n2 = g.n[2];
+    // q1 cells of all planes of the track; constant zero columns of the shared rows
+    for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
+    {
+        const int ncl = kPad - 1, ncr = P - (n2 + kPad);
+        for (int e = tid; e < rows_cap * (ncl + ncr); e += kThreads) {
+            const int r = e / (ncl + ncr), c = e - r * (ncl + ncr);
+            C2[r * P + (c < ncl ? c : n2 + kPad + (c - ncl))] = make_float2(0.f, 0.f);
+        }
+    }
     ZRay zr[kPerThread];
-    float acc[kPerThread];
+    float acc0[kPerThread], acc1[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
         zr[m] = z_setup(g, t, zs[m], ze[m]);
-        acc[m] = 0.f;
+        acc0[m] = 0.f;
+        acc1[m] = 0.f;
     }
     const int warp = tid >> 5, lane = tid & 31;
-    const int s1 = (t.p == 0) ? g.n[2] : g.n[1] * g.n[2];
+    const uint32_t c2_base = smem_addr(C2) + kPad * 8u - ((uint32_t)kMagicI << 3);
+    __syncthreads();
 
-    for (int c0 = t.I0; c0 <= t.I1; c0 += kChunk) {
-        const int rows = min(kChunk, t.I1 - c0 + 1);
-        // ---- build C: one warp per row, lanes along z (coalesced image reads)
-        for (int r = warp; r < rows; r += kThreads / 32) {
-            const RowCell rc = row_cell(g, t, c0 + r);
-            const float wa = 1.f - rc.w1, wb = rc.w1;
-            const float *ra = img + (rc.in_a ? rc.base : 0);
-            const float *rb = img + (rc.in_b ? rc.base + s1 : 0);
-            for (int zc = lane; zc < ld; zc += 32) {
-                const int z = zc - kPad;
-                float v = 0.f;
-                if ((unsigned)z < (unsigned)g.n[2]) {
-                    const float fa = rc.in_a ? __ldg(ra + z) : 0.f; // neighbours outside the image count as zero
-                    const float fb = rc.in_b ? __ldg(rb + z) : 0.f;
-                    v = fmaf(wb, fb, wa * fa);
+    for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
+        const int rows = min(rows_cap, t.I1 - c0 + 1);
+        // ---- build the (value, slope) rows: C[z] = wa f[i,k1,z] + wb f[i,k1+1,z], pair = (C[z], C[z+1]-C[z])
+        if (vec_ok) {
+            const int G = n2 >> 2, total = rows * G;
+            const float invG = 1.f / (float)G;
+            for (int e0 = warp * 32; e0 < total; e0 += kThreads) {
+                const int e = e0 + lane;
+                const bool act = e < total;
+                int r = (int)(((float)e + 0.5f) * invG);
+                int gq = e - r * G;
+                if (gq < 0) { --r; gq += G; }
+                if (gq >= G) { ++r; gq -= G; }
+                float c[4] = {0.f, 0.f, 0.f, 0.f};
+                RowInfo ri;
+                ri.base_a = ri.base_b = -1;
+                ri.wa = ri.wb = 0.f;
+                if (act) {
+                    ri = rinfo[c0 - t.I0 + r];
+                    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+                    if (ri.base_a >= 0) a = __ldg(reinterpret_cast<const float4 *>(img + ri.base_a) + gq);
+                    if (ri.base_b >= 0) b = __ldg(reinterpret_cast<const float4 *>(img + ri.base_b) + gq);
+                    c[0] = fmaf(ri.wb, b.x, ri.wa * a.x);
+                    c[1] = fmaf(ri.wb, b.y, ri.wa * a.y);
+                    c[2] = fmaf(ri.wb, b.z, ri.wa * a.z);
+                    c[3] = fmaf(ri.wb, b.w, ri.wa * a.w);
                 }
-                C[r * ld + zc] = v;
+                float c4 = __shfl_down_sync(0xffffffffu, c[0], 1);
+                if (gq == G - 1) {
+                    c4 = 0.f; // z = n2 lies outside the image
+                } else if (lane == 31 && act) { // the neighbour group belongs to another warp
+                    const float fa = (ri.base_a >= 0) ? __ldg(img + ri.base_a + 4 * gq + 4) : 0.f;
+                    const float fb = (ri.base_b >= 0) ? __ldg(img + ri.base_b + 4 * gq + 4) : 0.f;
+                    c4 = fmaf(ri.wb, fb, ri.wa * fa);
+                }
+                if (act) {
+                    float4 *dst = reinterpret_cast<float4 *>(C2 + r * P + kPad + 4 * gq);
+                    dst[0] = make_float4(c[0], c[1] - c[0], c[1], c[2] - c[1]);
+                    dst[1] = make_float4(c[2], c[3] - c[2], c[3], c4 - c[3]);
+                    if (gq == 0) C2[r * P + kPad - 1] = make_float2(0.f, c[0]);
+                }
+            }
+        } else {
+            const int ld = n2 + 1; // columns z = -1 .. n2-1
+            for (int e = tid; e < rows * ld; e += kThreads) {
+                const int r = e / ld, z = e - r * ld - 1;
+                const RowInfo ri = rinfo[c0 - t.I0 + r];
+                float v0 = 0.f, v1 = 0.f;
+                if (z >= 0) {
+                    const float fa = (ri.base_a >= 0) ? __ldg(img + ri.base_a + z) : 0.f;
+                    const float fb = (ri.base_b >= 0) ? __ldg(img + ri.base_b + z) : 0.f;
+                    v0 = fmaf(ri.wb, fb, ri.wa * fa);
+                }
+                if (z + 1 < n2) {
+                    const float fa = (ri.base_a >= 0) ? __ldg(img + ri.base_a + z + 1) : 0.f;
+                    const float fb = (ri.base_b >= 0) ? __ldg(img + ri.base_b + z + 1) : 0.f;
+                    v1 = fmaf(ri.wb, fb, ri.wa * fa);
+                }
+                C2[r * P + kPad + z] = make_float2(v0, v1 - v0);
             }
         }
         __syncthreads();
@@ -272,44 +364,72 @@ __global__ void __launch_bounds__(kThreads) k_fwd_tile(Lors l, int64_t n, const 
         for (int m = 0; m < kPerThread; ++m) {
             const int ib = max(zr[m].i0, c0), ie = min(zr[m].i1, c0 + rows - 1);
             if (ib > ie) continue;
+            const int nst = ie - ib + 1;
+            const float b2 = zr[m].b2, a2_0 = zr[m].a2;
+            const float a2_1 = fmaf(b2, 1.f, a2_0), a2_2 = fmaf(b2, 2.f, a2_0), a2_3 = fmaf(b2, 3.f, a2_0);
             float fk = (float)(ib - zr[m].i0);
-            int off = (ib - c0) * ld + kPad - kMagicI;
-            const float a2h = zr[m].a2h, b2 = zr[m].b2;
-            float a = acc[m];
-#pragma unroll 4
-            for (int i = ib; i <= ie; ++i) {
-                const float h = fmaf(b2, fk, a2h);   // u2 - 1/2
-                const float tt = h + kMagic;           // integer part in the low mantissa bits
-                const float w = (h - (tt - kMagic)) + 0.5f;
-                const int idx = __float_as_int(tt) + off;
-                const float v0 = C[idx], v1 = C[idx + 1];
-                a += fmaf(w, v1 - v0, v0);
-                fk += 1.f;
-                off += ld;
+            uint32_t row = c2_base + (uint32_t)((ib - c0) * P) * 8u;
+            float a0 = acc0[m], a1 = acc1[m];
+            {
+                float acc0 = a0, acc1 = a1;
+#pragma unroll 1
+                for (int it = nst >> 2; it > 0; --it) {
+                    JP_FWD_STEP(0, a2_0)
+                    JP_FWD_STEP(1, a2_1)
+                    JP_FWD_STEP(2, a2_2)
+                    JP_FWD_STEP(3, a2_3)
+                    fk += 4.f;
+                    row += 4u * P * 8u;
+                }
+#pragma unroll 1
+                for (int it = nst & 3; it > 0; --it) {
+                    JP_FWD_STEP(0, a2_0)
+                    fk += 1.f;
+                    row += P * 8u;
+                }
+                a0 = acc0;
+                a1 = acc1;
             }
-            acc[m] = a;
+            acc0[m] = a0;
+            acc1[m] = a1;
         }
         __syncthreads();
     }
 #pragma unroll
-    for (int m = 0; m < kPerThread; ++m) p[j0 + m * kThreads + tid] = zr[m].cf * acc[m];
+    for (int m = 0; m < kPerThread; ++m) p[j0 + m * kThreads + tid] = zr[m].cf * (acc0[m] + acc1[m]);
 }
+#undef JP_FWD_STEP
 
 // ---- back ------------------------------------------------------------------------------------------------
 // Fixed-point staging: contributions are rounded to multiples of 1/S and summed with native int32
 // shared-memory atomics (ATOMS.ADD; float shared atomics are CAS loops on sm_100).  S is chosen per
 // tile from X = max_j |cf_j y_j| so that neither a single contribution (|c S| < 2^22, the range of the
-// magic-number rounding) nor a whole bin (at most one contribution per LOR and plane: |sum| <= 768 X S
-// < 2^31) can overflow.  Rounding error per contribution <= X 768 / 2^32 = 1.8e-7 X.
-__global__ void __launch_bounds__(kThreads) k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g,
-                                                        float *__restrict__ img)
+// magic-number rounding) nor a whole bin (at most two contributions per LOR and plane: |sum| <= 2 x 768 X S
+// < 2^31) can overflow.  Rounding error per contribution <= X 768 / 2^31 = 3.6e-7 X.
+// Per step the two bins get q1 = round(S x w) and q0 = round(S x) - q1 (their sum is exact).
+#define JP_BACK_STEP(K, A2K)                                                   \
+    {                                                                          \
+        const float u = fmaf(b2, fk, A2K);                                     \
+        const float tt = __fadd_rd(u, kMagic);                                 \
+        const float w = u - (tt - kMagic);                                     \
+        const uint32_t a = row + (__float_as_uint(tt) << 2);                   \
+        const int bits = __float_as_int(fmaf(xm, w, kMagic));                  \
+        reds_add<(K) * P * 4>(a, qxm - bits);                                  \
+        reds_add<(K) * P * 4 + 4>(a, bits - kMagicI);                          \
+    }
+
+template <int P>
+__global__ void __launch_bounds__(kThreads, 4)
+    k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
+                float *__restrict__ img)
 {
-    extern __shared__ int Ci[]; // [kChunk][ld]
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int *Ci = reinterpret_cast<int *>(smem_raw);                                        // [rows_cap][P]
+    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(int)); // [max(n0,n1)]
     __shared__ Track trk;
     __shared__ float red[kThreads / 32];
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kTile;
-    const int ld = g.n[2] + 2 * kPad;
 
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
@@ -331,6 +451,7 @@ __global__ void __launch_bounds__(kThreads) k_back_tile(Lors l, int64_t n, const
     __syncthreads();
     const Track t = trk;
     if (t.I1 < t.I0) return;
+    const int n2 = g.n[2];
 
     ZRay zr[kPerThread];
     float x[kPerThread];
@@ -344,99 +465,179 @@ __global__ void __launch_bounds__(kThreads) k_back_tile(Lors l, int64_t n, const
     // block max of |x|
     for (int o = 16; o > 0; o >>= 1) xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
     if ((tid & 31) == 0) red[tid >> 5] = xmax;
-    for (int e = tid; e < kChunk * ld; e += kThreads) Ci[e] = 0;
+    for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
+    {
+        int4 *z4 = reinterpret_cast<int4 *>(Ci);
+        for (int e = tid; e < rows_cap * (P / 4); e += kThreads) z4[e] = make_int4(0, 0, 0, 0);
+    }
     __syncthreads();
     xmax = red[0];
 #pragma unroll
     for (int w = 1; w < kThreads / 32; ++w) xmax = fmaxf(xmax, red[w]);
     if (!(xmax > 0.f) || !(xmax < 3.0e38f)) return; // nothing to add (or non-finite input: undefined, skip)
-    // S: |c S| <= 2^22 - 2 and 768 |c S| < 2^31  ->  |c S| <= 2^31 / 768 - 1
-    const float lim = fminf(4194302.f, 2147483648.f / (float)kTile - 1.f);
+    // S: |c S| <= 2^22 - 2 and 2 x 768 |c S| < 2^31
+    const float lim = fminf(4194302.f, 2147483648.f / (float)(2 * kTile) - 1.f);
     const float S = lim / xmax, invS = xmax / lim;
+    int qx[kPerThread];
 #pragma unroll
-    for (int m = 0; m < kPerThread; ++m) x[m] *= S;
+    for (int m = 0; m < kPerThread; ++m) {
+        x[m] *= S;
+        qx[m] = __float2int_rn(x[m]) + kMagicI;
+    }
 
     const int warp = tid >> 5, lane = tid & 31;
-    const int s1 = (t.p == 0) ? g.n[2] : g.n[1] * g.n[2];
+    const uint32_t ci_base = smem_addr(Ci) + kPad * 4u - ((uint32_t)kMagicI << 2);
 
-    for (int c0 = t.I0; c0 <= t.I1; c0 += kChunk) {
-        const int rows = min(kChunk, t.I1 - c0 + 1);
+    for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
+        const int rows = min(rows_cap, t.I1 - c0 + 1);
         // ---- scatter along z into the fixed-point tile
 #pragma unroll
         for (int m = 0; m < kPerThread; ++m) {
             const int ib = max(zr[m].i0, c0), ie = min(zr[m].i1, c0 + rows - 1);
             if (ib > ie || x[m] == 0.f) continue;
+            const int nst = ie - ib + 1;
+            const float b2 = zr[m].b2, a2_0 = zr[m].a2, xm = x[m];
+            const int qxm = qx[m];
+            const float a2_1 = fmaf(b2, 1.f, a2_0), a2_2 = fmaf(b2, 2.f, a2_0), a2_3 = fmaf(b2, 3.f, a2_0);
             float fk = (float)(ib - zr[m].i0);
-            int off = (ib - c0) * ld + kPad - kMagicI;
-            const float a2h = zr[m].a2h, b2 = zr[m].b2, xm = x[m];
-#pragma unroll 4
-            for (int i = ib; i <= ie; ++i) {
-                const float h = fmaf(b2, fk, a2h);
-                const float tt = h + kMagic;
-                const float w = (h - (tt - kMagic)) + 0.5f;
-                const int idx = __float_as_int(tt) + off;
-                const int q1 = __float_as_int(fmaf(xm, w, kMagic)) - kMagicI;
-                const int q0 = __float_as_int(fmaf(xm, 1.f - w, kMagic)) - kMagicI;
-                atomicAdd(&Ci[idx], q0);
-                atomicAdd(&Ci[idx + 1], q1);
+            uint32_t row = ci_base + (uint32_t)((ib - c0) * P) * 4u;
+#pragma unroll 1
+            for (int it = nst >> 2; it > 0; --it) {
+                JP_BACK_STEP(0, a2_0)
+                JP_BACK_STEP(1, a2_1)
+                JP_BACK_STEP(2, a2_2)
+                JP_BACK_STEP(3, a2_3)
+                fk += 4.f;
+                row += 4u * P * 4u;
+            }
+#pragma unroll 1
+            for (int it = nst & 3; it > 0; --it) {
+                JP_BACK_STEP(0, a2_0)
                 fk += 1.f;
-                off += ld;
+                row += P * 4u;
             }
         }
         __syncthreads();
-        // ---- flush: spread every row over its two q1 neighbours with coalesced REDs, and clear it
-        for (int r = warp; r < rows; r += kThreads / 32) {
-            const RowCell rc = row_cell(g, t, c0 + r);
-            const float wa = (1.f - rc.w1) * invS, wb = rc.w1 * invS;
-            float *ra = img + (rc.in_a ? rc.base : 0);
-            float *rb = img + (rc.in_b ? rc.base + s1 : 0);
-            for (int zc = lane; zc < ld; zc += 32) {
-                const int q = Ci[r * ld + zc];
-                if (q == 0) continue;
-                Ci[r * ld + zc] = 0;
-                const int z = zc - kPad;
-                if ((unsigned)z < (unsigned)g.n[2]) {
-                    const float v = (float)q;
-                    if (rc.in_a) atomicAdd(ra + z, wa * v);
-                    if (rc.in_b) atomicAdd(rb + z, wb * v);
+        // ---- flush: spread every row over its two q1 neighbours with REDs, and clear it
+        if (vec_ok) {
+            const int G = n2 >> 2, total = rows * G;
+            const float invG = 1.f / (float)G;
+            for (int e = tid; e < total; e += kThreads) {
+                int r = (int)(((float)e + 0.5f) * invG);
+                int gq = e - r * G;
+                if (gq < 0) { --r; gq += G; }
+                if (gq >= G) { ++r; gq -= G; }
+                int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
+                const int4 q = *src;
+                if ((q.x | q.y | q.z | q.w) == 0) continue;
+                *src = make_int4(0, 0, 0, 0);
+                const RowInfo ri = rinfo[c0 - t.I0 + r];
+                const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
+                if (ri.base_a >= 0) {
+                    const float s = ri.wa * invS;
+                    atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq, make_float4(s * v.x, s * v.y, s * v.z, s * v.w));
                 }
+                if (ri.base_b >= 0) {
+                    const float s = ri.wb * invS;
+                    atomicAdd(reinterpret_cast<float4 *>(img + ri.base_b) + gq, make_float4(s * v.x, s * v.y, s * v.z, s * v.w));
+                }
+            }
+        } else {
+            for (int e = tid; e < rows * n2; e += kThreads) {
+                const int r = e / n2, z = e - r * n2;
+                const int q = Ci[r * P + kPad + z];
+                if (q == 0) continue;
+                Ci[r * P + kPad + z] = 0;
+                const RowInfo ri = rinfo[c0 - t.I0 + r];
+                const float v = (float)q * invS;
+                if (ri.base_a >= 0) atomicAdd(img + ri.base_a + z, ri.wa * v);
+                if (ri.base_b >= 0) atomicAdd(img + ri.base_b + z, ri.wb * v);
             }
         }
         __syncthreads();
     }
+    (void)warp;
+    (void)lane;
 }
+#undef JP_BACK_STEP
 
 // ---- launchers ----------------------------------------------------------------------------------------------
-static inline size_t tile_smem(const Geom &g) { return (size_t)kChunk * (g.n[2] + 2 * kPad) * sizeof(float); }
+namespace {
+
+constexpr size_t kSmemBudget = 54 * 1024; // per CTA: four CTAs per SM
+
+struct TileCfg {
+    int P;        // row pitch (0: image too wide along z for the tiled kernels)
+    int rows_cap; // rows per chunk
+    size_t smem;
+    int vec_ok;
+};
+
+TileCfg tile_cfg(const Geom &g, const void *img, size_t elem)
+{
+    TileCfg c{};
+    const int need = g.n[2] + kPad + kPadR;
+    const int pitches[] = {40, 72, 104, 136, 200, 264};
+    for (int P : pitches)
+        if (need <= P) { c.P = P; break; }
+    if (!c.P) return c;
+    const int np = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
+    const size_t rinfo = (size_t)np * sizeof(RowInfo);
+    const size_t row = (size_t)c.P * elem;
+    size_t rows = rinfo + row <= kSmemBudget ? (kSmemBudget - rinfo) / row : 0;
+    if (rows < 8) { c.P = 0; return c; }
+    if (rows > (size_t)np) rows = (size_t)np;
+    c.rows_cap = (int)rows;
+    c.smem = rows * row + rinfo;
+    c.vec_ok = (g.n[2] % 4 == 0) && ((uintptr_t)img % 16 == 0);
+    return c;
+}
+
+template <typename K>
+cudaError_t set_smem(K kernel, size_t smem)
+{
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
+}
+
+} // namespace
+
+#define JP_DISPATCH_P(CFG, ...)                    \
+    switch ((CFG).P) {                             \
+    case 40: { constexpr int P = 40; __VA_ARGS__; } break;   \
+    case 72: { constexpr int P = 72; __VA_ARGS__; } break;   \
+    case 104: { constexpr int P = 104; __VA_ARGS__; } break; \
+    case 136: { constexpr int P = 136; __VA_ARGS__; } break; \
+    case 200: { constexpr int P = 200; __VA_ARGS__; } break; \
+    case 264: { constexpr int P = 264; __VA_ARGS__; } break; \
+    default: return cudaErrorInvalidValue;         \
+    }
 
 cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
-    const size_t smem = tile_smem(g);
-    static thread_local size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_fwd_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const TileCfg c = tile_cfg(g, img, sizeof(float2));
+    if (!c.P) return launch_fwd(l, Range{0, 1, n, false}, img, g, p, st);
+    const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
+    JP_DISPATCH_P(c, {
+        cudaError_t e = set_smem(k_fwd_tile<P>, c.smem);
         if (e != cudaSuccess) return e;
-        configured = smem;
-    }
-    k_fwd_tile<<<(unsigned)((n + kTile - 1) / kTile), kThreads, smem, st>>>(l, n, img, g, p);
+        k_fwd_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok, p);
+    })
     return cudaGetLastError();
 }
 
 cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
-    const size_t smem = tile_smem(g);
-    static thread_local size_t configured = 0;
-    if (smem > 48 * 1024 && smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_back_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const TileCfg c = tile_cfg(g, img, sizeof(int));
+    if (!c.P) return launch_back(l, Range{0, 1, n, false}, y, g, img, st);
+    const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
+    JP_DISPATCH_P(c, {
+        cudaError_t e = set_smem(k_back_tile<P>, c.smem);
         if (e != cudaSuccess) return e;
-        configured = smem;
-    }
-    k_back_tile<<<(unsigned)((n + kTile - 1) / kTile), kThreads, smem, st>>>(l, n, y, g, img);
+        k_back_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok, img);
+    })
     return cudaGetLastError();
 }
-
-size_t tile_smem_bytes(const Geom &g) { return tile_smem(g); }
 
 } // namespace jp
