@@ -197,18 +197,45 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
     bool ok = (j0 + kTile <= n);
     if (ok) {
         const double dmax = fmax(fabs((double)xe0 - (double)xs0), fabs((double)ye0 - (double)ys0));
-        ok = dmax > 0.0;
+        // all loads first (no short-circuit: twelve independent loads in flight), then compare bits
+        uint32_t diff = 0;
 #pragma unroll
         for (int m = 0; m < kPerThread; ++m) {
             const int64_t j = j0 + m * kThreads + threadIdx.x;
-            ok = ok && same_bits(l.xs[j], xs0) && same_bits(l.ys[j], ys0) && same_bits(l.xe[j], xe0) &&
-                 same_bits(l.ye[j], ye0) && (fabs((double)ze[m] - (double)zs[m]) <= dmax);
+            diff |= (__float_as_uint(l.xs[j]) ^ __float_as_uint(xs0)) | (__float_as_uint(l.ys[j]) ^ __float_as_uint(ys0)) |
+                    (__float_as_uint(l.xe[j]) ^ __float_as_uint(xe0)) | (__float_as_uint(l.ye[j]) ^ __float_as_uint(ye0));
+            ok = ok && (fabs((double)ze[m] - (double)zs[m]) <= dmax);
         }
+        ok = ok && (diff == 0) && (dmax > 0.0);
     }
     return __syncthreads_and(ok) != 0;
 }
 
 __device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+#ifndef JP_PREFETCH_DIST
+#define JP_PREFETCH_DIST 592
+#endif
+#ifndef JP_RB
+#define JP_RB 2
+#endif
+#ifndef JP_MINB
+#define JP_MINB 4
+#endif
+
+// pull the end points of the tile that starts at LOR jt into L2 (one 128-byte line per thread): the CTA
+// that will work on it finds them there instead of waiting for HBM
+__device__ __forceinline__ void prefetch_tile(const Lors &l, int64_t n, int64_t jt)
+{
+    if (JP_PREFETCH_DIST == 0 || jt + kTile > n) return;
+    const int tid = threadIdx.x;
+    constexpr int kLines = kTile * 4 / 128; // lines per coordinate array
+    if (tid < 6 * kLines) {
+        const int a = tid / kLines, ln = tid - a * kLines;
+        const float *base = (a == 0) ? l.xs : (a == 1) ? l.ys : (a == 2) ? l.zs : (a == 3) ? l.xe : (a == 4) ? l.ye : l.ze;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(base + jt + ln * 32));
+    }
+}
 
 template <int OFF>
 __device__ __forceinline__ float2 lds_pair(uint32_t addr)
@@ -240,7 +267,7 @@ __device__ __forceinline__ void reds_add(uint32_t addr, int q)
     }
 
 template <int P>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, JP_MINB)
     k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
                float *__restrict__ p)
 {
@@ -251,6 +278,7 @@ __global__ void __launch_bounds__(kThreads, 4)
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kTile;
 
+    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
@@ -301,42 +329,47 @@ __global__ void __launch_bounds__(kThreads, 4)
         const int rows = min(rows_cap, t.I1 - c0 + 1);
         // ---- build the (value, slope) rows: C[z] = wa f[i,k1,z] + wb f[i,k1+1,z], pair = (C[z], C[z+1]-C[z])
         if (vec_ok) {
-            const int G = n2 >> 2, total = rows * G;
-            const float invG = 1.f / (float)G;
-            for (int e0 = warp * 32; e0 < total; e0 += kThreads) {
-                const int e = e0 + lane;
-                const bool act = e < total;
-                int r = (int)(((float)e + 0.5f) * invG);
-                int gq = e - r * G;
-                if (gq < 0) { --r; gq += G; }
-                if (gq >= G) { ++r; gq -= G; }
-                float c[4] = {0.f, 0.f, 0.f, 0.f};
-                RowInfo ri;
-                ri.base_a = ri.base_b = -1;
-                ri.wa = ri.wb = 0.f;
-                if (act) {
-                    ri = rinfo[c0 - t.I0 + r];
-                    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-                    if (ri.base_a >= 0) a = __ldg(reinterpret_cast<const float4 *>(img + ri.base_a) + gq);
-                    if (ri.base_b >= 0) b = __ldg(reinterpret_cast<const float4 *>(img + ri.base_b) + gq);
-                    c[0] = fmaf(ri.wb, b.x, ri.wa * a.x);
-                    c[1] = fmaf(ri.wb, b.y, ri.wa * a.y);
-                    c[2] = fmaf(ri.wb, b.z, ri.wa * a.z);
-                    c[3] = fmaf(ri.wb, b.w, ri.wa * a.w);
-                }
-                float c4 = __shfl_down_sync(0xffffffffu, c[0], 1);
-                if (gq == G - 1) {
-                    c4 = 0.f; // z = n2 lies outside the image
-                } else if (lane == 31 && act) { // the neighbour group belongs to another warp
-                    const float fa = (ri.base_a >= 0) ? __ldg(img + ri.base_a + 4 * gq + 4) : 0.f;
-                    const float fb = (ri.base_b >= 0) ? __ldg(img + ri.base_b + 4 * gq + 4) : 0.f;
-                    c4 = fmaf(ri.wb, fb, ri.wa * fa);
-                }
-                if (act) {
-                    float4 *dst = reinterpret_cast<float4 *>(C2 + r * P + kPad + 4 * gq);
-                    dst[0] = make_float4(c[0], c[1] - c[0], c[1], c[2] - c[1]);
-                    dst[1] = make_float4(c[2], c[3] - c[2], c[3], c4 - c[3]);
-                    if (gq == 0) C2[r * P + kPad - 1] = make_float2(0.f, c[0]);
+            // one warp per row, lanes along z in groups of four voxels; kRB rows in flight per warp
+            const int G = n2 >> 2;
+            constexpr int kRB = JP_RB, kNW = kThreads / 32;
+            for (int g0 = 0; g0 < G; g0 += 32) {
+                const int gq = g0 + lane;
+                const bool act = gq < G;
+                for (int r0 = warp; r0 < rows; r0 += kRB * kNW) {
+                    float4 a[kRB], b[kRB];
+#pragma unroll
+                    for (int u = 0; u < kRB; ++u) {
+                        const int r = r0 + u * kNW;
+                        a[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        b[u] = a[u];
+                        if (r < rows && act) {
+                            const RowInfo ri = rinfo[c0 - t.I0 + r];
+                            if (ri.base_a >= 0) a[u] = __ldg(reinterpret_cast<const float4 *>(img + ri.base_a) + gq);
+                            if (ri.base_b >= 0) b[u] = __ldg(reinterpret_cast<const float4 *>(img + ri.base_b) + gq);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < kRB; ++u) {
+                        const int r = r0 + u * kNW;
+                        if (r >= rows) break; // warp-uniform
+                        const RowInfo ri = rinfo[c0 - t.I0 + r];
+                        const float c0v = fmaf(ri.wb, b[u].x, ri.wa * a[u].x), c1v = fmaf(ri.wb, b[u].y, ri.wa * a[u].y);
+                        const float c2v = fmaf(ri.wb, b[u].z, ri.wa * a[u].z), c3v = fmaf(ri.wb, b[u].w, ri.wa * a[u].w);
+                        float c4v = __shfl_down_sync(0xffffffffu, c0v, 1);
+                        if (gq >= G - 1) {
+                            c4v = 0.f; // z = n2 lies outside the image
+                        } else if (lane == 31) { // the neighbour group is in the next pass
+                            const float fa = (ri.base_a >= 0) ? __ldg(img + ri.base_a + 4 * gq + 4) : 0.f;
+                            const float fb = (ri.base_b >= 0) ? __ldg(img + ri.base_b + 4 * gq + 4) : 0.f;
+                            c4v = fmaf(ri.wb, fb, ri.wa * fa);
+                        }
+                        if (act) {
+                            float4 *dst = reinterpret_cast<float4 *>(C2 + r * P + kPad + 4 * gq);
+                            dst[0] = make_float4(c0v, c1v - c0v, c1v, c2v - c1v);
+                            dst[1] = make_float4(c2v, c3v - c2v, c3v, c4v - c3v);
+                            if (gq == 0) C2[r * P + kPad - 1] = make_float2(0.f, c0v);
+                        }
+                    }
                 }
             }
         } else {
@@ -419,7 +452,7 @@ __global__ void __launch_bounds__(kThreads, 4)
     }
 
 template <int P>
-__global__ void __launch_bounds__(kThreads, 4)
+__global__ void __launch_bounds__(kThreads, JP_MINB)
     k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
                 float *__restrict__ img)
 {
@@ -431,6 +464,7 @@ __global__ void __launch_bounds__(kThreads, 4)
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kTile;
 
+    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
@@ -520,26 +554,22 @@ __global__ void __launch_bounds__(kThreads, 4)
         __syncthreads();
         // ---- flush: spread every row over its two q1 neighbours with REDs, and clear it
         if (vec_ok) {
-            const int G = n2 >> 2, total = rows * G;
-            const float invG = 1.f / (float)G;
-            for (int e = tid; e < total; e += kThreads) {
-                int r = (int)(((float)e + 0.5f) * invG);
-                int gq = e - r * G;
-                if (gq < 0) { --r; gq += G; }
-                if (gq >= G) { ++r; gq -= G; }
-                int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
-                const int4 q = *src;
-                if ((q.x | q.y | q.z | q.w) == 0) continue;
-                *src = make_int4(0, 0, 0, 0);
+            const int G = n2 >> 2;
+            for (int r = warp; r < rows; r += kThreads / 32) {
                 const RowInfo ri = rinfo[c0 - t.I0 + r];
-                const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
-                if (ri.base_a >= 0) {
-                    const float s = ri.wa * invS;
-                    atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq, make_float4(s * v.x, s * v.y, s * v.z, s * v.w));
-                }
-                if (ri.base_b >= 0) {
-                    const float s = ri.wb * invS;
-                    atomicAdd(reinterpret_cast<float4 *>(img + ri.base_b) + gq, make_float4(s * v.x, s * v.y, s * v.z, s * v.w));
+                const float sa = ri.wa * invS, sb = ri.wb * invS;
+                for (int gq = lane; gq < G; gq += 32) {
+                    int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
+                    const int4 q = *src;
+                    if ((q.x | q.y | q.z | q.w) == 0) continue;
+                    *src = make_int4(0, 0, 0, 0);
+                    const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
+                    if (ri.base_a >= 0)
+                        atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq,
+                                  make_float4(sa * v.x, sa * v.y, sa * v.z, sa * v.w));
+                    if (ri.base_b >= 0)
+                        atomicAdd(reinterpret_cast<float4 *>(img + ri.base_b) + gq,
+                                  make_float4(sb * v.x, sb * v.y, sb * v.z, sb * v.w));
                 }
             }
         } else {
@@ -556,15 +586,16 @@ __global__ void __launch_bounds__(kThreads, 4)
         }
         __syncthreads();
     }
-    (void)warp;
-    (void)lane;
 }
 #undef JP_BACK_STEP
 
 // ---- launchers ----------------------------------------------------------------------------------------------
 namespace {
 
-constexpr size_t kSmemBudget = 54 * 1024; // per CTA: four CTAs per SM
+#ifndef JP_SMEM_KB
+#define JP_SMEM_KB 54
+#endif
+constexpr size_t kSmemBudget = JP_SMEM_KB * 1024; // per CTA: four CTAs per SM
 
 struct TileCfg {
     int P;        // row pitch (0: image too wide along z for the tiled kernels)
