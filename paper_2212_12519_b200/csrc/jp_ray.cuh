@@ -43,6 +43,26 @@ struct Ray {
     int sp, s1, s2;   // element strides of p, q1, q2
 };
 
+// 1/x and sqrt(x) in double from a float32 seed and Newton steps (relative error ~1e-16): the double
+// precision division and square root of the CUDA library are 30-40 instruction routines, and the
+// set-up needs neither correct rounding (its results are rounded to float32) nor exactness (every
+// discrete decision is re-checked with exact products).
+__device__ __forceinline__ double drcp(double x)
+{
+    double r = (double)(1.f / (float)x);
+    r = fma(r, fma(-x, r, 1.0), r);
+    r = fma(r, fma(-x, r, 1.0), r);
+    return r;
+}
+
+__device__ __forceinline__ double dsqrt_pos(double x) // x > 0
+{
+    double r = (double)rsqrtf((float)x); // ~ 1/sqrt(x)
+    r = r * fma(-0.5 * x * r, r, 1.5);
+    r = r * fma(-0.5 * x * r, r, 1.5);
+    return x * r;
+}
+
 __device__ __forceinline__ int principal_axis(double d0, double d1, double d2)
 {
     // argmax |d_a| on the exact differences, ties -> lowest index (reading A3)
@@ -85,32 +105,38 @@ __device__ __forceinline__ void ray_setup(const Lors &l, int64_t j, const Geom &
     // ---- closed segment rule (reading A4): planes with min(s_p,e_p) <= o_p + i v_p <= max(s_p,e_p)
     const double lo = fmin(s[p], e[p]), hi = fmax(s[p], e[p]);
     const double np1 = (double)(g.n[p] - 1);
-    double flo = ceil((lo - op) / vp), fhi = floor((hi - op) / vp);
-    flo = fmin(fmax(flo, 0.0), np1 + 1.0);
-    fhi = fmin(fmax(fhi, -1.0), np1);
-    int ilo = (int)flo, ihi = (int)fhi;
-    // exact fix-up of the rounded divisions
-    if (ilo > 0 && op + (double)(ilo - 1) * vp >= lo) --ilo;
-    if (ilo <= g.n[p] - 1 && op + (double)ilo * vp < lo) ++ilo;
-    if (ihi < g.n[p] - 1 && op + (double)(ihi + 1) * vp <= hi) ++ihi;
-    if (ihi >= 0 && op + (double)ihi * vp > hi) --ihi;
+    int ilo = 0, ihi = g.n[p] - 1;
+    if (!(lo <= op && hi >= op + np1 * vp)) { // an end point inside the image slab (rare)
+        const double ivp = drcp(vp);
+        double flo = ceil((lo - op) * ivp), fhi = floor((hi - op) * ivp);
+        flo = fmin(fmax(flo, 0.0), np1 + 1.0);
+        fhi = fmin(fmax(fhi, -1.0), np1);
+        ilo = (int)flo;
+        ihi = (int)fhi;
+        // exact fix-up of the rounded quotients
+        if (ilo > 0 && op + (double)(ilo - 1) * vp >= lo) --ilo;
+        if (ilo <= g.n[p] - 1 && op + (double)ilo * vp < lo) ++ilo;
+        if (ihi < g.n[p] - 1 && op + (double)(ihi + 1) * vp <= hi) ++ihi;
+        if (ihi >= 0 && op + (double)ihi * vp > hi) --ihi;
+    }
 
     // ---- crossing point in voxel units: u_q(i) = A_q + B_q i
-    const double inv_dp = 1.0 / d[p];
+    const double inv_dp = drcp(d[p]);
     double A[2], B[2];
     const int q[2] = {q1, q2};
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
         const double ratio = d[q[c]] * inv_dp;
-        const double ivq = 1.0 / (double)g.v[q[c]];
+        const double ivq = drcp((double)g.v[q[c]]);
         B[c] = ratio * vp * ivq;
         A[c] = (s[q[c]] - (double)g.o[q[c]] + (op - s[p]) * ratio) * ivq;
         // conservative clip to -1 < u < n_q
         const double nq = (double)g.n[q[c]];
-        if (B[c] == 0.0) {
+        if (fabs(B[c]) < 1e-12) { // u_q moves by less than 1e-9 voxel over the whole image
             if (A[c] <= -1.0 || A[c] >= nq) ihi = ilo - 1;
         } else {
-            double ia = (-1.0 - A[c]) / B[c], ib = (nq - A[c]) / B[c];
+            const double ivb = drcp(B[c]);
+            double ia = (-1.0 - A[c]) * ivb, ib = (nq - A[c]) * ivb;
             double imin = fmin(ia, ib), imax = fmax(ia, ib);
             imin = fmin(fmax(floor(imin), -1.0), np1 + 1.0);
             imax = fmin(fmax(ceil(imax), -1.0), np1 + 1.0);
@@ -118,13 +144,14 @@ __device__ __forceinline__ void ray_setup(const Lors &l, int64_t j, const Geom &
             ihi = min(ihi, (int)imax);
         }
     }
-    const double L = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    const double L = dsqrt_pos(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
     double tau0 = 0.0, dtau = 0.0;
     if (WITH_TOF) {
         // tau(i) = (t_i - 1/2) L - coff, t_i = (o_p + i v_p - s_p)/d_p   (reading A8)
         dtau = vp * inv_dp * L;
         tau0 = ((op - s[p]) * inv_dp - 0.5) * L - (double)coff;
-        double ia = ((double)tau_lo - tau0) / dtau, ib = ((double)tau_hi - tau0) / dtau;
+        const double ivt = drcp(dtau);
+        double ia = ((double)tau_lo - tau0) * ivt, ib = ((double)tau_hi - tau0) * ivt;
         double imin = fmin(ia, ib), imax = fmax(ia, ib);
         imin = fmin(fmax(floor(imin), -1.0), np1 + 1.0);
         imax = fmin(fmax(ceil(imax), -1.0), np1 + 1.0);

@@ -63,24 +63,30 @@ __device__ void track_setup(const Geom &g, float xs, float ys, float xe, float y
     const double sp = s[p], ep = s[p] + d[p];
     const double lo = fmin(sp, ep), hi = fmax(sp, ep);
     const double np1 = (double)(g.n[p] - 1);
-    double flo = ceil((lo - op) / vp), fhi = floor((hi - op) / vp);
-    flo = fmin(fmax(flo, 0.0), np1 + 1.0);
-    fhi = fmin(fmax(fhi, -1.0), np1);
-    int ilo = (int)flo, ihi = (int)fhi;
-    if (ilo > 0 && op + (double)(ilo - 1) * vp >= lo) --ilo;
-    if (ilo <= g.n[p] - 1 && op + (double)ilo * vp < lo) ++ilo;
-    if (ihi < g.n[p] - 1 && op + (double)(ihi + 1) * vp <= hi) ++ihi;
-    if (ihi >= 0 && op + (double)ihi * vp > hi) --ihi;
-    const double inv_dp = 1.0 / d[p];
+    int ilo = 0, ihi = g.n[p] - 1;
+    if (!(lo <= op && hi >= op + np1 * vp)) { // an end point inside the image slab: closed segment rule (A4)
+        const double ivp = drcp(vp);
+        double flo = ceil((lo - op) * ivp), fhi = floor((hi - op) * ivp);
+        flo = fmin(fmax(flo, 0.0), np1 + 1.0);
+        fhi = fmin(fmax(fhi, -1.0), np1);
+        ilo = (int)flo;
+        ihi = (int)fhi;
+        if (ilo > 0 && op + (double)(ilo - 1) * vp >= lo) --ilo;
+        if (ilo <= g.n[p] - 1 && op + (double)ilo * vp < lo) ++ilo;
+        if (ihi < g.n[p] - 1 && op + (double)(ihi + 1) * vp <= hi) ++ihi;
+        if (ihi >= 0 && op + (double)ihi * vp > hi) --ihi;
+    }
+    const double inv_dp = drcp(d[p]);
     const double ratio = d[q1] * inv_dp;
-    const double ivq = 1.0 / (double)g.v[q1];
+    const double ivq = drcp((double)g.v[q1]);
     const double B = ratio * vp * ivq;
     const double A = (s[q1] - (double)g.o[q1] + (op - sp) * ratio) * ivq;
     const double nq = (double)g.n[q1];
-    if (B == 0.0) {
+    if (fabs(B) < 1e-12) { // u_q1 moves by less than 1e-9 voxel over the whole image
         if (A <= -1.0 || A >= nq) ihi = ilo - 1;
     } else {
-        const double ia = (-1.0 - A) / B, ib = (nq - A) / B;
+        const double ivb = drcp(B);
+        const double ia = (-1.0 - A) * ivb, ib = (nq - A) * ivb;
         double imin = fmin(ia, ib), imax = fmax(ia, ib);
         imin = fmin(fmax(floor(imin), -1.0), np1 + 1.0);
         imax = fmin(fmax(ceil(imax), -1.0), np1 + 1.0);
@@ -127,7 +133,7 @@ __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs,
     const double dz = (double)ze - (double)zs;
     const double rz = dz * t.inv_dp;
     const double vp = (double)g.v[t.p];
-    const double iv2 = 1.0 / (double)g.v[2];
+    const double iv2 = drcp((double)g.v[2]);
     const double B = rz * vp * iv2;
     const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2;
     const float rzf = (float)rz;
