@@ -147,7 +147,12 @@ int jp_fwd_tof_sino(const jp_lors *lors, const float *img, const jp_geom *geom, 
     JP_TRY(check_geom(geom, g));
     JP_TRY(check_tof(tof, true, t));
     if (!img || (lors->n > 0 && !p)) return fail(JP_ERR_POINTER, "img or p is NULL");
-    JP_CUDA(jp::launch_fwd_tof_sino(l, whole(lors->n), img, g, t, p, (cudaStream_t)stream), "jp_fwd_tof_sino");
+    if (lors->n == 0) return JP_OK;
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_fwd_tof_sino (table)");
+    const cudaError_t e = jp::launch_fwd_tof_sino(l, whole(lors->n), img, g, t, lut, p, (cudaStream_t)stream);
+    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
+    JP_CUDA(e, "jp_fwd_tof_sino");
     return JP_OK;
 }
 
@@ -162,7 +167,12 @@ int jp_back_tof_sino(const jp_lors *lors, const float *y, const jp_geom *geom, c
     JP_TRY(check_geom(geom, g));
     JP_TRY(check_tof(tof, true, t));
     if (!img || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "img or y is NULL");
-    JP_CUDA(jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, img, (cudaStream_t)stream), "jp_back_tof_sino");
+    if (lors->n == 0) return JP_OK;
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_back_tof_sino (table)");
+    const cudaError_t e = jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, lut, img, (cudaStream_t)stream);
+    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
+    JP_CUDA(e, "jp_back_tof_sino");
     return JP_OK;
 }
 
@@ -177,7 +187,12 @@ int jp_fwd_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *img, 
     JP_TRY(check_geom(geom, g));
     JP_TRY(check_tof(tof, false, t));
     if (!img || (lors->n > 0 && (!p || !tofbin))) return fail(JP_ERR_POINTER, "img, p or tofbin is NULL");
-    JP_CUDA(jp::launch_fwd_tof_lm(l, tofbin, whole(lors->n), img, g, t, p, 0, (cudaStream_t)stream), "jp_fwd_tof_lm");
+    if (lors->n == 0) return JP_OK;
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_fwd_tof_lm (table)");
+    const cudaError_t e = jp::launch_fwd_tof_lm(l, tofbin, whole(lors->n), img, g, t, lut, p, 0, (cudaStream_t)stream);
+    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
+    JP_CUDA(e, "jp_fwd_tof_lm");
     return JP_OK;
 }
 
@@ -192,7 +207,12 @@ int jp_back_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *y, c
     JP_TRY(check_geom(geom, g));
     JP_TRY(check_tof(tof, false, t));
     if (!img || (lors->n > 0 && (!y || !tofbin))) return fail(JP_ERR_POINTER, "img, y or tofbin is NULL");
-    JP_CUDA(jp::launch_back_tof_lm(l, tofbin, whole(lors->n), y, g, t, img, (cudaStream_t)stream), "jp_back_tof_lm");
+    if (lors->n == 0) return JP_OK;
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_back_tof_lm (table)");
+    const cudaError_t e = jp::launch_back_tof_lm(l, tofbin, whole(lors->n), y, g, t, lut, img, (cudaStream_t)stream);
+    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
+    JP_CUDA(e, "jp_back_tof_lm");
     return JP_OK;
 }
 
@@ -226,15 +246,20 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
     float *b = (float *)workspace;
     float *r = b + ((nvox + 31) / 32) * 32;
     JP_CUDA(cudaMemsetAsync(b, 0, (size_t)nvox * sizeof(float), st), "jp_lm_osem memset");
-    for (int it = 0; it < n_iter; ++it) {
-        for (int m = 0; m < n_subsets; ++m) {
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_lm_osem (table)");
+    cudaError_t e = cudaSuccess;
+    for (int it = 0; it < n_iter && e == cudaSuccess; ++it) {
+        for (int m = 0; m < n_subsets && e == cudaSuccess; ++m) {
             const int64_t count = (n > m) ? (n - m + n_subsets - 1) / n_subsets : 0;
             const jp::Range rg{m, n_subsets, count, true};
-            JP_CUDA(jp::launch_fwd_tof_lm(l, tofbin, rg, img, g, t, r, 1, st), "jp_lm_osem fwd");
-            JP_CUDA(jp::launch_back_tof_lm(l, tofbin, rg, r, g, t, b, st), "jp_lm_osem back");
-            JP_CUDA(jp::launch_osem_update(img, b, sens, (float)n_subsets, nvox, st), "jp_lm_osem update");
+            e = jp::launch_fwd_tof_lm(l, tofbin, rg, img, g, t, lut, r, 1, st);
+            if (e == cudaSuccess) e = jp::launch_back_tof_lm(l, tofbin, rg, r, g, t, lut, b, st);
+            if (e == cudaSuccess) e = jp::launch_osem_update(img, b, sens, (float)n_subsets, nvox, st);
         }
     }
+    jp::tof_lut_destroy(&lut, st);
+    JP_CUDA(e, "jp_lm_osem");
     return JP_OK;
 }
 

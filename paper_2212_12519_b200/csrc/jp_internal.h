@@ -29,16 +29,20 @@ cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, 
 cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st);
 cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st);
 
+// table of the TOF edge function (jp_tof_lut.cu): stream-ordered device scratch, one per call
+cudaError_t tof_lut_create(const Tof &t, cudaStream_t st, TofLut *out);
+void tof_lut_destroy(TofLut *lut, cudaStream_t st);
+
 cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const Geom &g, const Tof &t,
-                                float *p, cudaStream_t st);
+                                const TofLut &lut, float *p, cudaStream_t st);
 cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t,
-                                 float *img, cudaStream_t st);
+                                 const TofLut &lut, float *img, cudaStream_t st);
 
 // lm_mode: 0 = p = A x;  1 = p = (A x > 1e-9) ? 1/(A x) : 0   (OSEM ratio fused into the epilogue)
 cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *img, const Geom &g,
-                              const Tof &t, float *p, int lm_mode, cudaStream_t st);
+                              const Tof &t, const TofLut &lut, float *p, int lm_mode, cudaStream_t st);
 cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
-                               const Tof &t, float *img, cudaStream_t st);
+                               const Tof &t, const TofLut &lut, float *img, cudaStream_t st);
 
 // x = sens > 0 ? x * b * scale / sens : 0;  b = 0   (OSEM multiplicative update, clears b for the next subset)
 cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scale, int64_t nvox, cudaStream_t st);

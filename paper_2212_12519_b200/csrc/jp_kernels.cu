@@ -79,42 +79,46 @@ struct BinWindow {
     float x_lo; // position of the lower edge of bin klo relative to tau
 };
 
-__device__ __forceinline__ BinWindow bin_window(const Tof &t, const TofK &tk, float inv_w, float cb, float tau)
+__device__ __forceinline__ BinWindow bin_window(const Tof &t, float lim, float inv_w, float cb, float tau)
 {
     // bins k with [c_k - W/2, c_k + W/2] meeting [tau - m, tau + m]; k = round(tau'/W + cb)
     BinWindow b;
-    b.klo = max(0, (int)floorf((tau - tk.lim) * inv_w + cb + 0.5f));
-    b.khi = min(t.nbins - 1, (int)floorf((tau + tk.lim) * inv_w + cb + 0.5f));
-    b.x_lo = ((float)b.klo - cb) * t.width - tk.half_w - tau;
+    b.klo = max(0, (int)floorf((tau - lim) * inv_w + cb + 0.5f));
+    b.khi = min(t.nbins - 1, (int)floorf((tau + lim) * inv_w + cb + 0.5f));
+    b.x_lo = ((float)b.klo - cb) * t.width - 0.5f * t.width - tau;
     return b;
 }
 
 __global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, const float *__restrict__ img, Geom g,
-                                                         Tof t, float *__restrict__ p)
+                                                         Tof t, TofLut lut, float *__restrict__ p)
 {
-    extern __shared__ float acc[]; // [nbins][kBlock + 1]
+    extern __shared__ __align__(16) float acc[]; // [nbins][kBlock + 1], then the edge-function table
     constexpr int ld = kBlock + 1;
+    float2 *lut_sm = reinterpret_cast<float2 *>(acc + ((t.nbins * ld + 3) & ~3));
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kBlock;
     const int64_t j = j0 + tid;
     for (int kb = 0; kb < t.nbins; ++kb) acc[kb * ld + tid] = 0.f;
+    lut_load(lut, lut_sm);
+    __syncthreads();
+    const uint32_t lb = lut_base(lut_sm);
     if (j < n) {
-        const TofK tk = make_tofk(t);
+        const float lim = t.nsig * t.sigma;
         const float cb = 0.5f * (float)(t.nbins - 1);
         const float inv_w = 1.f / t.width;
-        const float reach = cb * t.width + tk.half_w + tk.lim;
+        const float reach = cb * t.width + 0.5f * t.width + lim;
         Ray r;
         ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
         for (int k = 0; k < r.nk; ++k) {
             const Cell cl = plane_cell(r, k);
             const float val = r.cf * plane_value(img, r, k, cl);
             const float tau = fmaf(r.dtau, (float)k, r.tau0);
-            const BinWindow bw = bin_window(t, tk, inv_w, cb, tau);
+            const BinWindow bw = bin_window(t, lim, inv_w, cb, tau);
             float x = bw.x_lo;
-            float e_lo = edge_erf(tk, x);
+            float e_lo = lut_E(lb, lut.inv_h, x);
             for (int kb = bw.klo; kb <= bw.khi; ++kb) {
                 x += t.width;
-                const float e_hi = edge_erf(tk, x);
+                const float e_hi = lut_E(lb, lut.inv_h, x);
                 acc[kb * ld + tid] += val * (0.5f * (e_hi - e_lo));
                 e_lo = e_hi;
             }
@@ -130,10 +134,12 @@ __global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, cons
 }
 
 __global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, const float *__restrict__ y, Geom g,
-                                                          Tof t, float *__restrict__ img)
+                                                          Tof t, TofLut lut, float *__restrict__ img)
 {
-    extern __shared__ float ysm[]; // [nbins][kBlock + 1]
+    extern __shared__ __align__(16) float ysm[]; // [nbins][kBlock + 1], then the edge-function table
     constexpr int ld = kBlock + 1;
+    float2 *lut_sm = reinterpret_cast<float2 *>(ysm + ((t.nbins * ld + 3) & ~3));
+    lut_load(lut, lut_sm);
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kBlock;
     const int64_t j = j0 + tid;
@@ -145,22 +151,23 @@ __global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, con
     }
     __syncthreads();
     if (j >= n) return;
-    const TofK tk = make_tofk(t);
+    const uint32_t lb = lut_base(lut_sm);
+    const float lim = t.nsig * t.sigma;
     const float cb = 0.5f * (float)(t.nbins - 1);
     const float inv_w = 1.f / t.width;
-    const float reach = cb * t.width + tk.half_w + tk.lim;
+    const float reach = cb * t.width + 0.5f * t.width + lim;
     Ray r;
     ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        const BinWindow bw = bin_window(t, tk, inv_w, cb, tau);
+        const BinWindow bw = bin_window(t, lim, inv_w, cb, tau);
         float x = bw.x_lo;
-        float e_lo = edge_erf(tk, x);
+        float e_lo = lut_E(lb, lut.inv_h, x);
         float s = 0.f;
         for (int kb = bw.klo; kb <= bw.khi; ++kb) {
             x += t.width;
-            const float e_hi = edge_erf(tk, x);
+            const float e_hi = lut_E(lb, lut.inv_h, x);
             s = fmaf(ysm[kb * ld + tid], 0.5f * (e_hi - e_lo), s);
             e_lo = e_hi;
         }
@@ -173,21 +180,25 @@ __global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, con
 template <int LM_MODE>
 __global__ void __launch_bounds__(kBlock) k_fwd_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
                                                        const float *__restrict__ img, Geom g, Tof t,
-                                                       float *__restrict__ p)
+                                                       TofLut lut, float *__restrict__ p)
 {
+    extern __shared__ __align__(16) float2 lut_sm[];
+    lut_load(lut, lut_sm);
+    __syncthreads();
+    const uint32_t lb = lut_base(lut_sm);
     const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
     if (c >= rg.count) return;
     const int64_t j = lor_index(rg, c);
-    const TofK tk = make_tofk(t);
+    const float half_w = 0.5f * t.width;
     const float centre = (float)tofbin[j] * t.width;
-    const float reach = tk.half_w + tk.lim;
+    const float reach = half_w + t.nsig * t.sigma;
     Ray r;
     ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
     float acc = 0.f;
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        acc = fmaf(plane_value(img, r, k, cl), tof_weight(tk, tau, centre), acc);
+        acc = fmaf(plane_value(img, r, k, cl), tof_weight(lb, lut.inv_h, half_w, tau, centre), acc);
     }
     float out = r.cf * acc;
     if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
@@ -196,23 +207,27 @@ __global__ void __launch_bounds__(kBlock) k_fwd_tof_lm(Lors l, const int16_t *__
 
 __global__ void __launch_bounds__(kBlock) k_back_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
                                                         const float *__restrict__ y, Geom g, Tof t,
-                                                        float *__restrict__ img)
+                                                        TofLut lut, float *__restrict__ img)
 {
+    extern __shared__ __align__(16) float2 lut_sm[];
+    lut_load(lut, lut_sm);
+    __syncthreads();
+    const uint32_t lb = lut_base(lut_sm);
     const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
     if (c >= rg.count) return;
     const int64_t j = lor_index(rg, c);
     const float yj = y[io_index(rg, c)];
     if (yj == 0.f) return;
-    const TofK tk = make_tofk(t);
+    const float half_w = 0.5f * t.width;
     const float centre = (float)tofbin[j] * t.width;
-    const float reach = tk.half_w + tk.lim;
+    const float reach = half_w + t.nsig * t.sigma;
     Ray r;
     ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
     const float x = r.cf * yj;
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        const float w = tof_weight(tk, tau, centre);
+        const float w = tof_weight(lb, lut.inv_h, half_w, tau, centre);
         if (w != 0.f) plane_scatter(img, r, k, cl, x * w);
     }
 }
@@ -259,42 +274,53 @@ cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, 
     return cudaGetLastError();
 }
 
-cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const Geom &g, const Tof &t, float *p,
-                                cudaStream_t st)
+static inline size_t sino_smem(const Tof &t)
+{
+    return (size_t)((t.nbins * (kBlock + 1) + 3) & ~3) * sizeof(float) + (size_t)kLutN * sizeof(float2);
+}
+
+cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const Geom &g, const Tof &t,
+                                const TofLut &lut, float *p, cudaStream_t st)
 {
     if (rg.count == 0) return cudaSuccess;
     if (rg.first != 0 || rg.stride != 1) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)t.nbins * (kBlock + 1) * sizeof(float);
-    k_fwd_tof_sino<<<grid_for(rg.count, kBlock), kBlock, smem, st>>>(l, rg.count, img, g, t, p);
+    const size_t smem = sino_smem(t);
+    cudaError_t e = cudaFuncSetAttribute(k_fwd_tof_sino, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_fwd_tof_sino<<<grid_for(rg.count, kBlock), kBlock, smem, st>>>(l, rg.count, img, g, t, lut, p);
     return cudaGetLastError();
 }
 
-cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t, float *img,
-                                 cudaStream_t st)
+cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t,
+                                 const TofLut &lut, float *img, cudaStream_t st)
 {
     if (rg.count == 0) return cudaSuccess;
     if (rg.first != 0 || rg.stride != 1) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)t.nbins * (kBlock + 1) * sizeof(float);
-    k_back_tof_sino<<<grid_for(rg.count, kBlock), kBlock, smem, st>>>(l, rg.count, y, g, t, img);
+    const size_t smem = sino_smem(t);
+    cudaError_t e = cudaFuncSetAttribute(k_back_tof_sino, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_back_tof_sino<<<grid_for(rg.count, kBlock), kBlock, smem, st>>>(l, rg.count, y, g, t, lut, img);
     return cudaGetLastError();
 }
+
+constexpr size_t kLutBytes = (size_t)kLutN * sizeof(float2);
 
 cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *img, const Geom &g,
-                              const Tof &t, float *p, int lm_mode, cudaStream_t st)
+                              const Tof &t, const TofLut &lut, float *p, int lm_mode, cudaStream_t st)
 {
     if (rg.count == 0) return cudaSuccess;
     if (lm_mode == 1)
-        k_fwd_tof_lm<1><<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, tofbin, rg, img, g, t, p);
+        k_fwd_tof_lm<1><<<grid_for(rg.count, kBlock), kBlock, kLutBytes, st>>>(l, tofbin, rg, img, g, t, lut, p);
     else
-        k_fwd_tof_lm<0><<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, tofbin, rg, img, g, t, p);
+        k_fwd_tof_lm<0><<<grid_for(rg.count, kBlock), kBlock, kLutBytes, st>>>(l, tofbin, rg, img, g, t, lut, p);
     return cudaGetLastError();
 }
 
 cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
-                               const Tof &t, float *img, cudaStream_t st)
+                               const Tof &t, const TofLut &lut, float *img, cudaStream_t st)
 {
     if (rg.count == 0) return cudaSuccess;
-    k_back_tof_lm<<<grid_for(rg.count, kBlock), kBlock, 0, st>>>(l, tofbin, rg, y, g, t, img);
+    k_back_tof_lm<<<grid_for(rg.count, kBlock), kBlock, kLutBytes, st>>>(l, tofbin, rg, y, g, t, lut, img);
     return cudaGetLastError();
 }
 

@@ -26,8 +26,6 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kPerThread = 3;
 constexpr int kTile = kThreads * kPerThread;
-constexpr float kMagic = 12582912.f;   // 1.5 * 2^23: fadd_rd(x, kMagic) holds floor(x) in the low mantissa bits
-constexpr int kMagicI = 0x4B400000;    // bit pattern of kMagic
 constexpr int kPad = 4;                // padding columns left of z = 0 in a shared-memory row
 constexpr int kPadR = 4;               // columns needed right of z = n2 - 1
 
@@ -217,8 +215,6 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
     return __syncthreads_and(ok) != 0;
 }
 
-__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
 #ifndef JP_PREFETCH_DIST
 #define JP_PREFETCH_DIST 592
 #endif
@@ -241,14 +237,6 @@ __device__ __forceinline__ void prefetch_tile(const Lors &l, int64_t n, int64_t 
         const float *base = (a == 0) ? l.xs : (a == 1) ? l.ys : (a == 2) ? l.zs : (a == 3) ? l.xe : (a == 4) ? l.ye : l.ze;
         asm volatile("prefetch.global.L2 [%0];" ::"l"(base + jt + ln * 32));
     }
-}
-
-template <int OFF>
-__device__ __forceinline__ float2 lds_pair(uint32_t addr)
-{
-    float2 v;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(addr), "n"(OFF) : "memory");
-    return v;
 }
 
 template <int OFF>
