@@ -125,6 +125,34 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
                const float *sens, float *img, int n_subsets, int n_iter, void *workspace,
                size_t workspace_bytes, void *stream);
 
+/* ---- listmode plan: sorted events (set-up; BASELINE.json north_star (b)) ---------------- */
+/* Listmode events arrive in acquisition order, which makes the image access of the projectors random
+ * (PAPER.md:88); the paper names pre-sorting the events as the remedy.  A plan is that
+ * sort, done once per event list: the events of every OSEM subset (subset m = {e : e mod n_subsets == m},
+ * the rule of jp_lm_osem) are ordered by principal axis, transaxial line, plane and axial position of
+ * their TOF bin, and a sorted copy of the end points / TOF bins is kept on the device together with the
+ * permutation.  Planned calls compute exactly what the unplanned calls compute (same arithmetic per
+ * event; only the order of the floating-point sums of the back projection changes) and take / return
+ * per-event arrays in CALLER order.
+ *   events, tofbin: device arrays, only read during jp_lm_plan_create (not kept).
+ *   The plan owns its device buffers (26 + 4 bytes per event) until jp_lm_plan_destroy.
+ *   jp_lm_plan_create is asynchronous on `stream` except for its device allocations (cudaMalloc);
+ *   n_subsets in 1..255, fewer than 2^31 events.  subset = -1 in the calls below means all events. */
+typedef struct jp_plan jp_plan;
+int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
+                      int n_subsets, void *stream, jp_plan **plan);
+int jp_lm_plan_destroy(jp_plan *plan);
+/* number of events of a subset (subset = -1: all); -1 for an invalid plan or subset */
+int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset);
+/* p[e] for the events e of the subset (other entries of p are left untouched); p has n entries */
+int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream);
+/* img += A_subset^T y, y has n entries in caller order.  ACCUMULATES. */
+int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream);
+/* jp_lm_osem on the plan's events, subsets and geometry */
+size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan);
+int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
+                       size_t workspace_bytes, void *stream);
+
 /* ---- hybrid mode: HOST pointers in and out ---------------------------------------- */
 /* Same semantics as jp_fwd / jp_back, but every pointer (inside lors_host too) is a HOST pointer.  The
  * LOR list is streamed through the current CUDA device in chunks on two internal streams (copies

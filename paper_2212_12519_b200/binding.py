@@ -56,6 +56,15 @@ EXPORTS = {
     "jp_lm_osem_workspace_bytes": (C.c_size_t, [C.c_int64, C.POINTER(jp_geom), C.c_int]),
     "jp_lm_osem": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
                              C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "jp_lm_plan_create": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_int,
+                                    C.c_void_p, C.POINTER(C.c_void_p)]),
+    "jp_lm_plan_destroy": (C.c_int, [C.c_void_p]),
+    "jp_lm_plan_subset_count": (C.c_int64, [C.c_void_p, C.c_int]),
+    "jp_fwd_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_back_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_lm_osem_planned_workspace_bytes": (C.c_size_t, [C.c_void_p]),
+    "jp_lm_osem_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_size_t,
+                                     C.c_void_p]),
     "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
@@ -262,6 +271,76 @@ def jp_lm_osem(xstart, xend, tofbin, sens, img, origin, voxsize, tof: jp_tof, n_
     _check(load().jp_lm_osem(C.byref(l), tofbin.data_ptr(), C.byref(g), C.byref(tof), sens.data_ptr(),
                              img.data_ptr(), int(n_subsets), int(n_iter), workspace.data_ptr(),
                              workspace.numel() * workspace.element_size(), _stream(stream)), "jp_lm_osem")
+    return img
+
+
+# ---- listmode plan (sorted events) ----------------------------------------------------------------------------
+class LmPlan:
+    """Owner of a jp_plan handle (the sort is done by jp_lm_plan_create; this class only holds the handle)."""
+
+    def __init__(self, xstart, xend, tofbin, n, origin, voxsize, tof: jp_tof, n_subsets: int = 1, stream=None):
+        l, keep = make_lors(xstart, xend)
+        tofbin = _bins(tofbin, l.n)
+        self.n = int(l.n)
+        self.shape = tuple(int(x) for x in n)
+        self.n_subsets = int(n_subsets)
+        self.device = xstart.device
+        g = make_geom(self.shape, origin, voxsize)
+        h = C.c_void_p()
+        _check(load().jp_lm_plan_create(C.byref(l), tofbin.data_ptr(), C.byref(g), C.byref(tof), int(n_subsets),
+                                        _stream(stream), C.byref(h)), "jp_lm_plan_create")
+        self.handle = h
+
+    def subset_count(self, subset: int = -1) -> int:
+        return int(load().jp_lm_plan_subset_count(self.handle, int(subset)))
+
+    def destroy(self):
+        if self.handle is not None and self.handle.value:
+            _check(load().jp_lm_plan_destroy(self.handle), "jp_lm_plan_destroy")
+        self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def jp_fwd_tof_lm_planned(plan: LmPlan, img, subset: int = -1, out=None, stream=None) -> torch.Tensor:
+    img = _img(img)
+    assert tuple(img.shape) == plan.shape
+    if out is None:
+        out = torch.zeros(plan.n, dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == plan.n and out.is_contiguous()
+    _check(load().jp_fwd_tof_lm_planned(plan.handle, int(subset), img.data_ptr(), out.data_ptr(), _stream(stream)),
+           "jp_fwd_tof_lm_planned")
+    return out
+
+
+def jp_back_tof_lm_planned(plan: LmPlan, y, subset: int = -1, img=None, stream=None) -> torch.Tensor:
+    _dev(y, torch.float32, "y")
+    assert y.numel() == plan.n and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(plan.shape, dtype=torch.float32, device=y.device)
+    img = _img(img)
+    assert tuple(img.shape) == plan.shape
+    _check(load().jp_back_tof_lm_planned(plan.handle, int(subset), y.data_ptr(), img.data_ptr(), _stream(stream)),
+           "jp_back_tof_lm_planned")
+    return img
+
+
+def jp_lm_osem_planned(plan: LmPlan, sens, img, n_iter: int, workspace=None, stream=None) -> torch.Tensor:
+    img = _img(img)
+    sens = _img(sens)
+    assert tuple(img.shape) == plan.shape and sens.shape == img.shape
+    need = int(load().jp_lm_osem_planned_workspace_bytes(plan.handle))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=img.device)
+    assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= need
+    _check(load().jp_lm_osem_planned(plan.handle, sens.data_ptr(), img.data_ptr(), int(n_iter), workspace.data_ptr(),
+                                     workspace.numel() * workspace.element_size(), _stream(stream)),
+           "jp_lm_osem_planned")
     return img
 
 

@@ -69,7 +69,7 @@ int check_lors(const jp_lors *l, jp::Lors &out)
     return JP_OK;
 }
 
-inline jp::Range whole(int64_t n) { return jp::Range{0, 1, n, false}; }
+inline jp::Range whole(int64_t n) { return jp::Range{0, 1, n, false, nullptr}; }
 
 #define JP_TRY(expr)                  \
     do {                              \
@@ -252,7 +252,7 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
     for (int it = 0; it < n_iter && e == cudaSuccess; ++it) {
         for (int m = 0; m < n_subsets && e == cudaSuccess; ++m) {
             const int64_t count = (n > m) ? (n - m + n_subsets - 1) / n_subsets : 0;
-            const jp::Range rg{m, n_subsets, count, true};
+            const jp::Range rg{m, n_subsets, count, true, nullptr};
             e = jp::launch_fwd_tof_lm(l, tofbin, rg, img, g, t, lut, r, 1, st);
             if (e == cudaSuccess) e = jp::launch_back_tof_lm(l, tofbin, rg, r, g, t, lut, b, st);
             if (e == cudaSuccess) e = jp::launch_osem_update(img, b, sens, (float)n_subsets, nvox, st);
@@ -260,6 +260,144 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
     }
     jp::tof_lut_destroy(&lut, st);
     JP_CUDA(e, "jp_lm_osem");
+    return JP_OK;
+}
+
+
+// ---- listmode plan ------------------------------------------------------------------------------------------
+struct jp_plan {
+    jp::LmPlan *lm;
+};
+
+int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
+                      int n_subsets, void *stream, jp_plan **plan)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_lors(events, l));
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, false, t));
+    if (!plan) return fail(JP_ERR_POINTER, "plan is NULL");
+    *plan = nullptr;
+    if (n_subsets < 1 || n_subsets > 255) return fail(JP_ERR_SIZE, "n_subsets must be in 1..255");
+    if (events->n >= ((int64_t)1 << 31)) return fail(JP_ERR_SIZE, "a plan holds fewer than 2^31 events");
+    if (events->n > 0 && !tofbin) return fail(JP_ERR_POINTER, "tofbin is NULL");
+    jp::LmPlan *lm = nullptr;
+    JP_CUDA(jp::lm_plan_create(l, tofbin, events->n, g, t, n_subsets, (cudaStream_t)stream, &lm), "jp_lm_plan_create");
+    jp_plan *pl = new jp_plan;
+    pl->lm = lm;
+    *plan = pl;
+    return JP_OK;
+}
+
+int jp_lm_plan_destroy(jp_plan *plan)
+{
+    g_err[0] = 0;
+    if (!plan) return JP_OK;
+    if (!plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    jp::lm_plan_destroy(plan->lm);
+    plan->lm = nullptr;
+    delete plan;
+    return JP_OK;
+}
+
+int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset)
+{
+    if (!plan || !plan->lm) return -1;
+    jp::Lors l;
+    const int16_t *tb;
+    jp::Range rg;
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return -1;
+    jp::lm_plan_view(plan->lm, subset, true, &l, &tb, &rg);
+    return rg.count;
+}
+
+int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    jp::Lors l;
+    const int16_t *tb;
+    jp::Range rg;
+    jp::lm_plan_view(plan->lm, subset, false, &l, &tb, &rg);
+    if (rg.count == 0) return JP_OK;
+    if (!img || !p) return fail(JP_ERR_POINTER, "img or p is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const jp::Tof &t = jp::lm_plan_tof(plan->lm);
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_fwd_tof_lm_planned (table)");
+    const cudaError_t e = jp::launch_fwd_tof_lm(l, tb, rg, img, jp::lm_plan_geom(plan->lm), t, lut, p, 0, st);
+    jp::tof_lut_destroy(&lut, st);
+    JP_CUDA(e, "jp_fwd_tof_lm_planned");
+    return JP_OK;
+}
+
+int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    jp::Lors l;
+    const int16_t *tb;
+    jp::Range rg;
+    jp::lm_plan_view(plan->lm, subset, false, &l, &tb, &rg);
+    if (rg.count == 0) return JP_OK;
+    if (!img || !y) return fail(JP_ERR_POINTER, "img or y is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const jp::Tof &t = jp::lm_plan_tof(plan->lm);
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_back_tof_lm_planned (table)");
+    const cudaError_t e = jp::launch_back_tof_lm(l, tb, rg, y, jp::lm_plan_geom(plan->lm), t, lut, img, st);
+    jp::tof_lut_destroy(&lut, st);
+    JP_CUDA(e, "jp_back_tof_lm_planned");
+    return JP_OK;
+}
+
+size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan)
+{
+    if (!plan || !plan->lm) return 0;
+    const jp::Geom &g = jp::lm_plan_geom(plan->lm);
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    const int64_t n = jp::lm_plan_n(plan->lm);
+    const int ns = jp::lm_plan_subsets(plan->lm);
+    return (size_t)(nvox + (n + ns - 1) / ns + 64) * sizeof(float);
+}
+
+int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
+                       size_t workspace_bytes, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
+    if (!sens || !img || !workspace) return fail(JP_ERR_POINTER, "NULL argument");
+    if (workspace_bytes < jp_lm_osem_planned_workspace_bytes(plan)) return fail(JP_ERR_SIZE, "workspace too small");
+    cudaStream_t st = (cudaStream_t)stream;
+    const jp::Geom &g = jp::lm_plan_geom(plan->lm);
+    const jp::Tof &t = jp::lm_plan_tof(plan->lm);
+    const int ns = jp::lm_plan_subsets(plan->lm);
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    float *b = (float *)workspace;
+    float *r = b + ((nvox + 31) / 32) * 32;
+    JP_CUDA(cudaMemsetAsync(b, 0, (size_t)nvox * sizeof(float), st), "jp_lm_osem_planned memset");
+    jp::TofLut lut{};
+    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_lm_osem_planned (table)");
+    cudaError_t e = cudaSuccess;
+    for (int it = 0; it < n_iter && e == cudaSuccess; ++it) {
+        for (int m = 0; m < ns && e == cudaSuccess; ++m) {
+            jp::Lors l;
+            const int16_t *tb;
+            jp::Range rg;
+            jp::lm_plan_view(plan->lm, m, true, &l, &tb, &rg); // r is indexed in sorted order: no permutation
+            e = jp::launch_fwd_tof_lm(l, tb, rg, img, g, t, lut, r, 1, st);
+            if (e == cudaSuccess) e = jp::launch_back_tof_lm(l, tb, rg, r, g, t, lut, b, st);
+            if (e == cudaSuccess) e = jp::launch_osem_update(img, b, sens, (float)ns, nvox, st);
+        }
+    }
+    jp::tof_lut_destroy(&lut, st);
+    JP_CUDA(e, "jp_lm_osem_planned");
     return JP_OK;
 }
 

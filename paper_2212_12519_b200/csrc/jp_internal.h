@@ -16,6 +16,7 @@ char *err_buf();
 struct Range {
     int64_t first, stride, count;
     bool compact;
+    const int *perm = nullptr; // if set (and not compact): per-LOR inputs/outputs are indexed by perm[j]
 };
 
 cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_t st);
@@ -43,6 +44,17 @@ cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, co
                               const Tof &t, const TofLut &lut, float *p, int lm_mode, cudaStream_t st);
 cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
                                const Tof &t, const TofLut &lut, float *img, cudaStream_t st);
+
+// listmode plan (jp_plan.cu)
+struct LmPlan;
+cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
+                           int n_subsets, cudaStream_t st, LmPlan **out);
+void lm_plan_destroy(LmPlan *pl);
+int64_t lm_plan_n(const LmPlan *pl);
+int lm_plan_subsets(const LmPlan *pl);
+const Geom &lm_plan_geom(const LmPlan *pl);
+const Tof &lm_plan_tof(const LmPlan *pl);
+void lm_plan_view(const LmPlan *pl, int m, bool compact, Lors *l, const int16_t **tb, Range *rg);
 
 // x = sens > 0 ? x * b * scale / sens : 0;  b = 0   (OSEM multiplicative update, clears b for the next subset)
 cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scale, int64_t nvox, cudaStream_t st);

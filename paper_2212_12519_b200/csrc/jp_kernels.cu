@@ -11,7 +11,12 @@ namespace jp {
 constexpr int kBlock = 128;
 
 __device__ __forceinline__ int64_t lor_index(const Range &rg, int64_t c) { return rg.first + c * rg.stride; }
-__device__ __forceinline__ int64_t io_index(const Range &rg, int64_t c) { return rg.compact ? c : lor_index(rg, c); }
+__device__ __forceinline__ int64_t io_index(const Range &rg, int64_t c)
+{
+    if (rg.compact) return c;
+    const int64_t j = lor_index(rg, c);
+    return rg.perm ? (int64_t)rg.perm[j] : j;
+}
 
 // ---- principal axis only (diagnostic; bit-exact against the oracle) --------------------------------
 __global__ void k_classify(Lors l, int64_t n, uint8_t *__restrict__ axis)

@@ -1,0 +1,192 @@
+// jp_plan.cu -- listmode plan: the events of every OSEM subset, reordered so that neighbouring threads
+// walk nearby voxels (BASELINE.json north_star: "LORs sorted or binned by principal axis and direction
+// so neighbouring threads walk nearby voxels"; the paper names pre-sorting of listmode events as the way
+// to speed up the projections).
+//
+// Events arrive in acquisition order (random access).  The image is stored with the axial
+// axis fastest, so a warp's four gathers per plane touch few 128-byte lines only when its lanes sit on
+// the same transaxial line (same plane, same row) -- and its lanes stay converged only when their TOF
+// windows cover the same planes.  The sort key, most significant field first:
+//
+//   subset (e mod n_subsets) | principal axis | transaxial slope d_q1/d_p (11 bits) | transaxial
+//   intercept at the image centre plane (11 bits) | plane of the TOF bin centre (6 bits) | axial
+//   position of the TOF bin centre (6 bits)
+//
+// It is purely geometric (no scanner model): crystal-snapped events of one crystal pair get the same
+// slope/intercept cell, continuous events get neighbours.  The plan owns a sorted SoA copy of the end
+// points and TOF bins (coalesced loads) and the permutation (results are returned in caller order).
+// The sort itself is CUB's device radix sort (a library primitive used for set-up); key generation,
+// gather and all projections are this library's kernels.
+#include <cub/device/device_radix_sort.cuh>
+
+#include "jp_internal.h"
+
+namespace jp {
+
+__global__ void k_lm_keys(Lors l, const int16_t *__restrict__ tofbin, int64_t n, Geom g, Tof t, int n_subsets,
+                          unsigned long long *__restrict__ keys, int *__restrict__ idx)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const float s[3] = {l.xs[j], l.ys[j], l.zs[j]};
+    const float e[3] = {l.xe[j], l.ye[j], l.ze[j]};
+    const double d0 = (double)e[0] - (double)s[0], d1 = (double)e[1] - (double)s[1], d2 = (double)e[2] - (double)s[2];
+    const int p = principal_axis(d0, d1, d2);
+    const float d[3] = {(float)d0, (float)d1, (float)d2};
+    unsigned long long key = (unsigned long long)(j % n_subsets) << 36 | (unsigned long long)p << 34;
+    const float L = sqrtf(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    if (L > 0.f) {
+        const int q1 = (p == 0) ? 1 : 0, q2 = (p == 2) ? 1 : 2;
+        const float inv_dp = 1.f / d[p];
+        // transaxial line in slope / intercept form (the same for both orientations of the event)
+        const float slope = d[q1] * inv_dp; // in [-1, 1]
+        const float cp = g.o[p] + 0.5f * (float)(g.n[p] - 1) * g.v[p];
+        const float cq = g.o[q1] + 0.5f * (float)(g.n[q1] - 1) * g.v[q1];
+        const float icpt = s[q1] + (cp - s[p]) * slope - cq;              // mm from the image centre
+        const float half = 0.75f * (float)g.n[q1] * g.v[q1];              // covers the image with margin
+        const int ks = min(2047, max(0, (int)((slope + 1.f) * 1023.5f)));
+        const int ki = min(2047, max(0, (int)((icpt / half + 1.f) * 1023.5f)));
+        // TOF bin centre: tau_c mm from the midpoint towards e
+        const float tau_c = (float)tofbin[j] * t.width + t.coff;
+        const float f = 0.5f + tau_c / L;
+        const float xc = s[p] + f * d[p], zc = s[q2] + f * d[q2];
+        const int kp = min(63, max(0, (int)((xc - g.o[p]) / (g.v[p] * (float)g.n[p]) * 64.f)));
+        const int kz = min(63, max(0, (int)((zc - g.o[q2]) / (g.v[q2] * (float)g.n[q2]) * 64.f)));
+        key |= (unsigned long long)ks << 23 | (unsigned long long)ki << 12 | (unsigned long long)kp << 6 |
+               (unsigned long long)kz;
+    }
+    keys[j] = key;
+    idx[j] = (int)j;
+}
+
+__global__ void k_lm_gather(Lors l, const int16_t *__restrict__ tofbin, const int *__restrict__ perm, int64_t n,
+                            float *__restrict__ xs, float *__restrict__ ys, float *__restrict__ zs,
+                            float *__restrict__ xe, float *__restrict__ ye, float *__restrict__ ze,
+                            int16_t *__restrict__ tb)
+{
+    const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c >= n) return;
+    const int j = perm[c];
+    xs[c] = l.xs[j];
+    ys[c] = l.ys[j];
+    zs[c] = l.zs[j];
+    xe[c] = l.xe[j];
+    ye[c] = l.ye[j];
+    ze[c] = l.ze[j];
+    tb[c] = tofbin[j];
+}
+
+struct LmPlan {
+    int64_t n = 0;
+    int n_subsets = 1;
+    Geom g{};
+    Tof t{};
+    float *coord = nullptr; // 6 arrays of n floats: xs ys zs xe ye ze, sorted
+    int16_t *tb = nullptr;  // sorted TOF bins
+    int *perm = nullptr;    // sorted position -> caller index
+};
+
+static int bits_for(int v)
+{
+    int b = 0;
+    while ((1 << b) < v) ++b;
+    return b;
+}
+
+cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
+                           int n_subsets, cudaStream_t st, LmPlan **out)
+{
+    LmPlan *pl = new LmPlan;
+    pl->n = n;
+    pl->n_subsets = n_subsets;
+    pl->g = g;
+    pl->t = t;
+    *out = pl;
+    if (n == 0) return cudaSuccess;
+    cudaError_t e;
+    unsigned long long *keys = nullptr, *keys2 = nullptr;
+    int *idx = nullptr;
+    void *tmp = nullptr;
+    size_t tmp_bytes = 0;
+#define JP_PLAN_TRY(x)                  \
+    do {                                \
+        e = (x);                        \
+        if (e != cudaSuccess) goto fail; \
+    } while (0)
+    JP_PLAN_TRY(cudaMalloc((void **)&pl->coord, sizeof(float) * 6 * (size_t)n));
+    JP_PLAN_TRY(cudaMalloc((void **)&pl->tb, sizeof(int16_t) * (size_t)n));
+    JP_PLAN_TRY(cudaMalloc((void **)&pl->perm, sizeof(int) * (size_t)n));
+    JP_PLAN_TRY(cudaMallocAsync((void **)&keys, sizeof(unsigned long long) * (size_t)n, st));
+    JP_PLAN_TRY(cudaMallocAsync((void **)&keys2, sizeof(unsigned long long) * (size_t)n, st));
+    JP_PLAN_TRY(cudaMallocAsync((void **)&idx, sizeof(int) * (size_t)n, st));
+    {
+        const unsigned grid = (unsigned)((n + 255) / 256);
+        k_lm_keys<<<grid, 256, 0, st>>>(l, tofbin, n, g, t, n_subsets, keys, idx);
+        JP_PLAN_TRY(cudaGetLastError());
+        const int end_bit = 36 + bits_for(n_subsets);
+        JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
+        JP_PLAN_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
+        JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
+        float *c = pl->coord;
+        k_lm_gather<<<grid, 256, 0, st>>>(l, tofbin, pl->perm, n, c, c + n, c + 2 * n, c + 3 * n, c + 4 * n, c + 5 * n,
+                                           pl->tb);
+        JP_PLAN_TRY(cudaGetLastError());
+    }
+    cudaFreeAsync(tmp, st);
+    cudaFreeAsync(idx, st);
+    cudaFreeAsync(keys2, st);
+    cudaFreeAsync(keys, st);
+    return cudaSuccess;
+fail:
+    if (tmp) cudaFreeAsync(tmp, st);
+    if (idx) cudaFreeAsync(idx, st);
+    if (keys2) cudaFreeAsync(keys2, st);
+    if (keys) cudaFreeAsync(keys, st);
+    lm_plan_destroy(pl);
+    *out = nullptr;
+    return e;
+#undef JP_PLAN_TRY
+}
+
+void lm_plan_destroy(LmPlan *pl)
+{
+    if (!pl) return;
+    cudaFree(pl->coord);
+    cudaFree(pl->tb);
+    cudaFree(pl->perm);
+    delete pl;
+}
+
+int64_t lm_plan_n(const LmPlan *pl) { return pl->n; }
+int lm_plan_subsets(const LmPlan *pl) { return pl->n_subsets; }
+const Geom &lm_plan_geom(const LmPlan *pl) { return pl->g; }
+const Tof &lm_plan_tof(const LmPlan *pl) { return pl->t; }
+
+// sorted events of subset m (m < 0: all subsets) as a LOR list + range; per-event inputs / outputs are
+// addressed through the permutation (caller order) unless `compact`
+void lm_plan_view(const LmPlan *pl, int m, bool compact, Lors *l, const int16_t **tb, Range *rg)
+{
+    const int64_t n = pl->n;
+    const float *c = pl->coord;
+    l->xs = c;
+    l->ys = c + n;
+    l->zs = c + 2 * n;
+    l->xe = c + 3 * n;
+    l->ye = c + 4 * n;
+    l->ze = c + 5 * n;
+    *tb = pl->tb;
+    int64_t first = 0, count = n;
+    if (m >= 0) {
+        const int ns = pl->n_subsets;
+        // subset k holds the events {e : e mod ns == k}: ceil((n - k) / ns) of them, stored in subset order
+        for (int k = 0; k < m; ++k) first += (n > k) ? (n - k + ns - 1) / ns : 0;
+        count = (n > m) ? (n - m + ns - 1) / ns : 0;
+    }
+    rg->first = first;
+    rg->stride = 1;
+    rg->count = count;
+    rg->compact = compact;
+    rg->perm = compact ? nullptr : pl->perm;
+}
+
+} // namespace jp

@@ -641,7 +641,7 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
 {
     if (n == 0) return cudaSuccess;
     const TileCfg c = tile_cfg(g, img, sizeof(float2));
-    if (!c.P) return launch_fwd(l, Range{0, 1, n, false}, img, g, p, st);
+    if (!c.P) return launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
     JP_DISPATCH_P(c, {
         cudaError_t e = set_smem(k_fwd_tile<P>, c.smem);
@@ -655,7 +655,7 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
 {
     if (n == 0) return cudaSuccess;
     const TileCfg c = tile_cfg(g, img, sizeof(int));
-    if (!c.P) return launch_back(l, Range{0, 1, n, false}, y, g, img, st);
+    if (!c.P) return launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
     JP_DISPATCH_P(c, {
         cudaError_t e = set_smem(k_back_tile<P>, c.smem);

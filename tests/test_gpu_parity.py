@@ -213,6 +213,65 @@ def test_config4_small_osem(cuda_device, scanner, events):
     assert mx <= 1e-3, f"OSEM max abs / max {mx:.3e}"
 
 
+def test_config3_plan_sorted_events(cuda_device, scanner, events):
+    """the listmode plan (sorted events) computes what the unplanned calls compute, in caller order"""
+    g, ph = scanner
+    xs, xe, tb = events
+    n = xs.shape[1]
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    xsd, xed, tbd, imgd = xs.to(cuda_device), xe.to(cuda_device), tb.to(cuda_device), dev(ph, cuda_device)
+    plan = jp.LmPlan(xsd, xed, tbd, g.n, g.origin, g.voxsize, tof, n_subsets=7)
+    # counts: bit exact
+    counts = [plan.subset_count(m) for m in range(7)]
+    assert counts == [len(range(m, n, 7)) for m in range(7)] and plan.subset_count(-1) == n
+    p_ref = jp.jp_fwd_tof_lm(xsd, xed, tbd, imgd, g.origin, g.voxsize, tof)
+    p_all = jp.jp_fwd_tof_lm_planned(plan, imgd)
+    assert torch.equal(p_all, p_ref)          # same arithmetic per event, only the order differs
+    # one subset: only its events are written
+    p_sub = jp.jp_fwd_tof_lm_planned(plan, imgd, subset=3, out=torch.full((n,), -1.0, device=cuda_device))
+    mask = torch.zeros(n, dtype=torch.bool, device=cuda_device)
+    mask[3::7] = True
+    assert torch.equal(p_sub[mask], p_ref[mask]) and bool((p_sub[~mask] == -1.0).all())
+    # adjoint: subsets add up to the whole, and the whole matches the oracle
+    y = inputs.uniform_values(n, 0.5, 2.0, seed=13).to(cuda_device)
+    b_all = jp.jp_back_tof_lm_planned(plan, y)
+    b_sum = torch.zeros_like(b_all)
+    for m in range(7):
+        jp.jp_back_tof_lm_planned(plan, y, subset=m, img=b_sum)
+    ref = oracle.back_tof_lm(xs.numpy(), xe.numpy(), tb.numpy(), y.cpu().numpy(), g.n, g.origin, g.voxsize, *args)
+    assert_back(b_all, ref)
+    assert_back(b_sum, ref)
+    assert adj_gap(p_all, y, imgd, b_all) <= ADJ_GAP
+    plan.destroy()
+
+
+def test_config4_small_osem_planned(cuda_device, scanner, events):
+    g, ph = scanner
+    xs, xe, tb = events
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    sx, se = inputs.sinogram_lors(views=range(0, 256, 8), radial=range(-64, 65, 4))
+    sx, se = sx[:, ::5].contiguous(), se[:, ::5].contiguous()
+    sens32 = oracle.back(sx.numpy(), se.numpy(), np.ones(sx.shape[1]), g.n, g.origin, g.voxsize).astype(np.float32)
+    x0 = np.ones(g.n, dtype=np.float32)
+    ref = oracle.lm_osem(xs.numpy(), xe.numpy(), tb.numpy(), sens32.astype(np.float64), x0, g.origin, g.voxsize,
+                         *args, n_subsets=5, n_iter=2)
+    plan = jp.LmPlan(xs.to(cuda_device), xe.to(cuda_device), tb.to(cuda_device), g.n, g.origin, g.voxsize, tof,
+                     n_subsets=5)
+    img = dev(x0, cuda_device).clone()
+    jp.jp_lm_osem_planned(plan, dev(sens32, cuda_device), img, n_iter=2)
+    got = img.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.abs(got - ref).max() / np.abs(ref).max()
+    assert rel <= 1e-4, f"OSEM rel-L2 {rel:.3e}"
+    assert mx <= 1e-3, f"OSEM max abs / max {mx:.3e}"
+    plan.destroy()
+
+
 # ---- edge cases ----------------------------------------------------------------------------------------
 def test_edge_cases(cuda_device):
     g = inputs.GEOM_SMALL
