@@ -83,6 +83,71 @@ inline jp::Range whole(int64_t n) { return jp::Range{0, 1, n, false, nullptr}; }
         if (e__ != cudaSuccess) return fail_cuda(e__, where); \
     } while (0)
 
+// stream-ordered scratch of one TOF call: the edge-function table and a zero-padded image
+struct TofCtx {
+    jp::TofLut lut{};
+    float *pimg = nullptr;
+    cudaStream_t st = nullptr;
+    ~TofCtx()
+    {
+        jp::tof_lut_destroy(&lut, st);
+        jp::padded_destroy(pimg, st);
+    }
+};
+
+// mode 0: pimg = padded copy of img (forward); 1: pimg = zero accumulator (back)
+static int tof_ctx_init(TofCtx &c, const jp::Tof &t, const jp::Geom &g, const float *img, int mode, cudaStream_t st,
+                        const char *where)
+{
+    c.st = st;
+    if (jp::padded_voxels(g) >= ((int64_t)1 << 31)) return fail(JP_ERR_SIZE, "padded image has >= 2^31 voxels");
+    JP_CUDA(jp::tof_lut_create(t, st, &c.lut), where);
+    JP_CUDA(jp::padded_create(img, g, mode == 1, st, &c.pimg), where);
+    return JP_OK;
+}
+
+static int lm_fwd(const jp::Lors &l, const int16_t *tb, const jp::Range &rg, const float *img, const jp::Geom &g,
+                  const jp::Tof &t, float *p, cudaStream_t st, const char *where)
+{
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, img, 0, st, where));
+    JP_CUDA(jp::launch_fwd_tof_lm(l, tb, rg, c.pimg, g, t, c.lut, p, 0, st), where);
+    return JP_OK;
+}
+
+static int lm_back(const jp::Lors &l, const int16_t *tb, const jp::Range &rg, const float *y, const jp::Geom &g,
+                   const jp::Tof &t, float *img, cudaStream_t st, const char *where)
+{
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, nullptr, 1, st, where));
+    JP_CUDA(jp::launch_back_tof_lm(l, tb, rg, y, g, t, c.lut, c.pimg, st), where);
+    JP_CUDA(jp::padded_add_to(c.pimg, g, img, st), where);
+    return JP_OK;
+}
+
+// OSEM subset loop on padded copies of x and b (allocated here, stream-ordered); r = per-event ratios
+template <typename View>
+static int lm_osem_loop(View view, int n_subsets, int n_iter, const jp::Geom &g, const jp::Tof &t, const float *sens,
+                        float *img, float *r, cudaStream_t st, const char *where)
+{
+    TofCtx cx, cb; // cx.pimg = padded x, cb.pimg = padded b
+    JP_TRY(tof_ctx_init(cx, t, g, img, 0, st, where));
+    cb.st = st;
+    JP_CUDA(jp::padded_create(nullptr, g, true, st, &cb.pimg), where);
+    for (int it = 0; it < n_iter; ++it) {
+        for (int m = 0; m < n_subsets; ++m) {
+            jp::Lors l;
+            const int16_t *tb;
+            jp::Range rg;
+            view(m, &l, &tb, &rg);
+            JP_CUDA(jp::launch_fwd_tof_lm(l, tb, rg, cx.pimg, g, t, cx.lut, r, 1, st), where);
+            JP_CUDA(jp::launch_back_tof_lm(l, tb, rg, r, g, t, cx.lut, cb.pimg, st), where);
+            JP_CUDA(jp::launch_osem_update_padded(img, cx.pimg, cb.pimg, sens, (float)n_subsets, g, st), where);
+        }
+    }
+    return JP_OK;
+}
+
 } // namespace
 
 extern "C" {
@@ -148,11 +213,10 @@ int jp_fwd_tof_sino(const jp_lors *lors, const float *img, const jp_geom *geom, 
     JP_TRY(check_tof(tof, true, t));
     if (!img || (lors->n > 0 && !p)) return fail(JP_ERR_POINTER, "img or p is NULL");
     if (lors->n == 0) return JP_OK;
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_fwd_tof_sino (table)");
-    const cudaError_t e = jp::launch_fwd_tof_sino(l, whole(lors->n), img, g, t, lut, p, (cudaStream_t)stream);
-    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
-    JP_CUDA(e, "jp_fwd_tof_sino");
+    cudaStream_t st = (cudaStream_t)stream;
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, img, 0, st, "jp_fwd_tof_sino (scratch)"));
+    JP_CUDA(jp::launch_fwd_tof_sino(l, whole(lors->n), c.pimg, g, t, c.lut, p, st), "jp_fwd_tof_sino");
     return JP_OK;
 }
 
@@ -168,11 +232,11 @@ int jp_back_tof_sino(const jp_lors *lors, const float *y, const jp_geom *geom, c
     JP_TRY(check_tof(tof, true, t));
     if (!img || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "img or y is NULL");
     if (lors->n == 0) return JP_OK;
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_back_tof_sino (table)");
-    const cudaError_t e = jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, lut, img, (cudaStream_t)stream);
-    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
-    JP_CUDA(e, "jp_back_tof_sino");
+    cudaStream_t st = (cudaStream_t)stream;
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, nullptr, 1, st, "jp_back_tof_sino (scratch)"));
+    JP_CUDA(jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, c.lut, c.pimg, st), "jp_back_tof_sino");
+    JP_CUDA(jp::padded_add_to(c.pimg, g, img, st), "jp_back_tof_sino (unpad)");
     return JP_OK;
 }
 
@@ -188,12 +252,7 @@ int jp_fwd_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *img, 
     JP_TRY(check_tof(tof, false, t));
     if (!img || (lors->n > 0 && (!p || !tofbin))) return fail(JP_ERR_POINTER, "img, p or tofbin is NULL");
     if (lors->n == 0) return JP_OK;
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_fwd_tof_lm (table)");
-    const cudaError_t e = jp::launch_fwd_tof_lm(l, tofbin, whole(lors->n), img, g, t, lut, p, 0, (cudaStream_t)stream);
-    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
-    JP_CUDA(e, "jp_fwd_tof_lm");
-    return JP_OK;
+    return lm_fwd(l, tofbin, whole(lors->n), img, g, t, p, (cudaStream_t)stream, "jp_fwd_tof_lm");
 }
 
 int jp_back_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *y, const jp_geom *geom,
@@ -208,12 +267,7 @@ int jp_back_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *y, c
     JP_TRY(check_tof(tof, false, t));
     if (!img || (lors->n > 0 && (!y || !tofbin))) return fail(JP_ERR_POINTER, "img, y or tofbin is NULL");
     if (lors->n == 0) return JP_OK;
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, (cudaStream_t)stream, &lut), "jp_back_tof_lm (table)");
-    const cudaError_t e = jp::launch_back_tof_lm(l, tofbin, whole(lors->n), y, g, t, lut, img, (cudaStream_t)stream);
-    jp::tof_lut_destroy(&lut, (cudaStream_t)stream);
-    JP_CUDA(e, "jp_back_tof_lm");
-    return JP_OK;
+    return lm_back(l, tofbin, whole(lors->n), y, g, t, img, (cudaStream_t)stream, "jp_back_tof_lm");
 }
 
 // workspace layout: [b: nvox floats][r: ceil(n_events / n_subsets) floats]
@@ -245,21 +299,14 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
     const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
     float *b = (float *)workspace;
     float *r = b + ((nvox + 31) / 32) * 32;
-    JP_CUDA(cudaMemsetAsync(b, 0, (size_t)nvox * sizeof(float), st), "jp_lm_osem memset");
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_lm_osem (table)");
-    cudaError_t e = cudaSuccess;
-    for (int it = 0; it < n_iter && e == cudaSuccess; ++it) {
-        for (int m = 0; m < n_subsets && e == cudaSuccess; ++m) {
-            const int64_t count = (n > m) ? (n - m + n_subsets - 1) / n_subsets : 0;
-            const jp::Range rg{m, n_subsets, count, true, nullptr};
-            e = jp::launch_fwd_tof_lm(l, tofbin, rg, img, g, t, lut, r, 1, st);
-            if (e == cudaSuccess) e = jp::launch_back_tof_lm(l, tofbin, rg, r, g, t, lut, b, st);
-            if (e == cudaSuccess) e = jp::launch_osem_update(img, b, sens, (float)n_subsets, nvox, st);
-        }
-    }
-    jp::tof_lut_destroy(&lut, st);
-    JP_CUDA(e, "jp_lm_osem");
+    (void)b;
+    auto view = [&](int m, jp::Lors *lo, const int16_t **tb, jp::Range *rg) {
+        *lo = l;
+        *tb = tofbin;
+        const int64_t count = (n > m) ? (n - m + n_subsets - 1) / n_subsets : 0;
+        *rg = jp::Range{m, n_subsets, count, true, nullptr};
+    };
+    JP_TRY(lm_osem_loop(view, n_subsets, n_iter, g, t, sens, img, r, st, "jp_lm_osem"));
     return JP_OK;
 }
 
@@ -325,14 +372,8 @@ int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, flo
     jp::lm_plan_view(plan->lm, subset, false, &l, &tb, &rg);
     if (rg.count == 0) return JP_OK;
     if (!img || !p) return fail(JP_ERR_POINTER, "img or p is NULL");
-    cudaStream_t st = (cudaStream_t)stream;
-    const jp::Tof &t = jp::lm_plan_tof(plan->lm);
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_fwd_tof_lm_planned (table)");
-    const cudaError_t e = jp::launch_fwd_tof_lm(l, tb, rg, img, jp::lm_plan_geom(plan->lm), t, lut, p, 0, st);
-    jp::tof_lut_destroy(&lut, st);
-    JP_CUDA(e, "jp_fwd_tof_lm_planned");
-    return JP_OK;
+    return lm_fwd(l, tb, rg, img, jp::lm_plan_geom(plan->lm), jp::lm_plan_tof(plan->lm), p, (cudaStream_t)stream,
+                  "jp_fwd_tof_lm_planned");
 }
 
 int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream)
@@ -346,14 +387,8 @@ int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, floa
     jp::lm_plan_view(plan->lm, subset, false, &l, &tb, &rg);
     if (rg.count == 0) return JP_OK;
     if (!img || !y) return fail(JP_ERR_POINTER, "img or y is NULL");
-    cudaStream_t st = (cudaStream_t)stream;
-    const jp::Tof &t = jp::lm_plan_tof(plan->lm);
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_back_tof_lm_planned (table)");
-    const cudaError_t e = jp::launch_back_tof_lm(l, tb, rg, y, jp::lm_plan_geom(plan->lm), t, lut, img, st);
-    jp::tof_lut_destroy(&lut, st);
-    JP_CUDA(e, "jp_back_tof_lm_planned");
-    return JP_OK;
+    return lm_back(l, tb, rg, y, jp::lm_plan_geom(plan->lm), jp::lm_plan_tof(plan->lm), img, (cudaStream_t)stream,
+                   "jp_back_tof_lm_planned");
 }
 
 size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan)
@@ -381,23 +416,11 @@ int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n
     const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
     float *b = (float *)workspace;
     float *r = b + ((nvox + 31) / 32) * 32;
-    JP_CUDA(cudaMemsetAsync(b, 0, (size_t)nvox * sizeof(float), st), "jp_lm_osem_planned memset");
-    jp::TofLut lut{};
-    JP_CUDA(jp::tof_lut_create(t, st, &lut), "jp_lm_osem_planned (table)");
-    cudaError_t e = cudaSuccess;
-    for (int it = 0; it < n_iter && e == cudaSuccess; ++it) {
-        for (int m = 0; m < ns && e == cudaSuccess; ++m) {
-            jp::Lors l;
-            const int16_t *tb;
-            jp::Range rg;
-            jp::lm_plan_view(plan->lm, m, true, &l, &tb, &rg); // r is indexed in sorted order: no permutation
-            e = jp::launch_fwd_tof_lm(l, tb, rg, img, g, t, lut, r, 1, st);
-            if (e == cudaSuccess) e = jp::launch_back_tof_lm(l, tb, rg, r, g, t, lut, b, st);
-            if (e == cudaSuccess) e = jp::launch_osem_update(img, b, sens, (float)ns, nvox, st);
-        }
-    }
-    jp::tof_lut_destroy(&lut, st);
-    JP_CUDA(e, "jp_lm_osem_planned");
+    (void)b;
+    auto view = [&](int m, jp::Lors *lo, const int16_t **tb, jp::Range *rg) {
+        jp::lm_plan_view(plan->lm, m, true, lo, tb, rg); // r is indexed in sorted order: no permutation
+    };
+    JP_TRY(lm_osem_loop(view, ns, n_iter, g, t, sens, img, r, st, "jp_lm_osem_planned"));
     return JP_OK;
 }
 

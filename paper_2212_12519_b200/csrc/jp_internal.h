@@ -45,6 +45,14 @@ cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, co
 cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
                                const Tof &t, const TofLut &lut, float *img, cudaStream_t st);
 
+// zero-padded image copies for the per-LOR kernels (jp_pad.cu)
+int64_t padded_voxels(const Geom &g);
+cudaError_t padded_create(const float *img, const Geom &g, bool zero_only, cudaStream_t st, float **out);
+cudaError_t padded_add_to(const float *pimg, const Geom &g, float *img, cudaStream_t st);
+void padded_destroy(float *p, cudaStream_t st);
+cudaError_t launch_osem_update_padded(float *x, float *px, float *pb, const float *sens, float scale, const Geom &g,
+                                      cudaStream_t st);
+
 // listmode plan (jp_plan.cu)
 struct LmPlan;
 cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,

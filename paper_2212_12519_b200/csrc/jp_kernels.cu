@@ -9,6 +9,7 @@
 namespace jp {
 
 constexpr int kBlock = 128;
+constexpr int kLmBlock = 256;
 
 __device__ __forceinline__ int64_t lor_index(const Range &rg, int64_t c) { return rg.first + c * rg.stride; }
 __device__ __forceinline__ int64_t io_index(const Range &rg, int64_t c)
@@ -78,7 +79,7 @@ __global__ void __launch_bounds__(kBlock) k_back(Lors l, Range rg, const float *
 // All bins of one LOR are accumulated by one thread while it walks the planes.  The
 // per-thread bin accumulators live in shared memory, bin-major with a padded row (conflict free),
 // and the block's [kBlock][nbins] output tile -- contiguous in global memory -- is written (or, for
-// the adjoint, read) fully coalesced.
+// the adjoint, read) fully coalesced.  The image is the zero-padded copy (no bounds tests, PRay).
 struct BinWindow {
     int klo, khi;
     float x_lo; // position of the lower edge of bin klo relative to tau
@@ -94,7 +95,7 @@ __device__ __forceinline__ BinWindow bin_window(const Tof &t, float lim, float i
     return b;
 }
 
-__global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, const float *__restrict__ img, Geom g,
+__global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, const float *__restrict__ pimg, Geom g,
                                                          Tof t, TofLut lut, float *__restrict__ p)
 {
     extern __shared__ __align__(16) float acc[]; // [nbins][kBlock + 1], then the edge-function table
@@ -114,10 +115,13 @@ __global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, cons
         const float reach = cb * t.width + 0.5f * t.width + lim;
         Ray r;
         ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
-        for (int k = 0; k < r.nk; ++k) {
-            const Cell cl = plane_cell(r, k);
-            const float val = r.cf * plane_value(img, r, k, cl);
-            const float tau = fmaf(r.dtau, (float)k, r.tau0);
+        const PRay q = pray_from(r, g);
+        float fk = 0.f;
+        int po = q.off;
+        for (int k = 0; k < q.nk; ++k) {
+            const PCell cl = pray_cell(q, fk, po);
+            const float val = q.cf * pray_value(pimg, q, cl);
+            const float tau = fmaf(q.dtau, fk, q.tau0);
             const BinWindow bw = bin_window(t, lim, inv_w, cb, tau);
             float x = bw.x_lo;
             float e_lo = lut_E(lb, lut.inv_h, x);
@@ -127,6 +131,8 @@ __global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, cons
                 acc[kb * ld + tid] += val * (0.5f * (e_hi - e_lo));
                 e_lo = e_hi;
             }
+            fk += 1.f;
+            po += q.sp;
         }
     }
     __syncthreads();
@@ -139,7 +145,7 @@ __global__ void __launch_bounds__(kBlock) k_fwd_tof_sino(Lors l, int64_t n, cons
 }
 
 __global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, const float *__restrict__ y, Geom g,
-                                                          Tof t, TofLut lut, float *__restrict__ img)
+                                                          Tof t, TofLut lut, float *__restrict__ pimg)
 {
     extern __shared__ __align__(16) float ysm[]; // [nbins][kBlock + 1], then the edge-function table
     constexpr int ld = kBlock + 1;
@@ -163,9 +169,12 @@ __global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, con
     const float reach = cb * t.width + 0.5f * t.width + lim;
     Ray r;
     ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
-    for (int k = 0; k < r.nk; ++k) {
-        const Cell cl = plane_cell(r, k);
-        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+    const PRay q = pray_from(r, g);
+    float fk = 0.f;
+    int po = q.off;
+    for (int k = 0; k < q.nk; ++k) {
+        const PCell cl = pray_cell(q, fk, po);
+        const float tau = fmaf(q.dtau, fk, q.tau0);
         const BinWindow bw = bin_window(t, lim, inv_w, cb, tau);
         float x = bw.x_lo;
         float e_lo = lut_E(lb, lut.inv_h, x);
@@ -176,22 +185,24 @@ __global__ void __launch_bounds__(kBlock) k_back_tof_sino(Lors l, int64_t n, con
             s = fmaf(ysm[kb * ld + tid], 0.5f * (e_hi - e_lo), s);
             e_lo = e_hi;
         }
-        if (s != 0.f) plane_scatter(img, r, k, cl, r.cf * s);
+        if (s != 0.f) pray_scatter(pimg, q, cl, q.cf * s);
+        fk += 1.f;
+        po += q.sp;
     }
 }
 
 // ---- TOF listmode ---------------------------------------------------------------------------------------
 // Only the planes inside the truncated kernel of the event's own bin are visited.
 template <int LM_MODE>
-__global__ void __launch_bounds__(kBlock) k_fwd_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
-                                                       const float *__restrict__ img, Geom g, Tof t,
-                                                       TofLut lut, float *__restrict__ p)
+__global__ void __launch_bounds__(kLmBlock) k_fwd_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
+                                                         const float *__restrict__ pimg, Geom g, Tof t,
+                                                         TofLut lut, float *__restrict__ p)
 {
     extern __shared__ __align__(16) float2 lut_sm[];
     lut_load(lut, lut_sm);
     __syncthreads();
     const uint32_t lb = lut_base(lut_sm);
-    const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
+    const int64_t c = blockIdx.x * (int64_t)kLmBlock + threadIdx.x;
     if (c >= rg.count) return;
     const int64_t j = lor_index(rg, c);
     const float half_w = 0.5f * t.width;
@@ -199,26 +210,30 @@ __global__ void __launch_bounds__(kBlock) k_fwd_tof_lm(Lors l, const int16_t *__
     const float reach = half_w + t.nsig * t.sigma;
     Ray r;
     ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
-    float acc = 0.f;
-    for (int k = 0; k < r.nk; ++k) {
-        const Cell cl = plane_cell(r, k);
-        const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        acc = fmaf(plane_value(img, r, k, cl), tof_weight(lb, lut.inv_h, half_w, tau, centre), acc);
+    const PRay q = pray_from(r, g);
+    float acc = 0.f, fk = 0.f;
+    int po = q.off;
+    for (int k = 0; k < q.nk; ++k) {
+        const PCell cl = pray_cell(q, fk, po);
+        const float tau = fmaf(q.dtau, fk, q.tau0);
+        acc = fmaf(pray_value(pimg, q, cl), tof_weight(lb, lut.inv_h, half_w, tau, centre), acc);
+        fk += 1.f;
+        po += q.sp;
     }
-    float out = r.cf * acc;
+    float out = q.cf * acc;
     if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
     p[io_index(rg, c)] = out;
 }
 
-__global__ void __launch_bounds__(kBlock) k_back_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
-                                                        const float *__restrict__ y, Geom g, Tof t,
-                                                        TofLut lut, float *__restrict__ img)
+__global__ void __launch_bounds__(kLmBlock) k_back_tof_lm(Lors l, const int16_t *__restrict__ tofbin, Range rg,
+                                                          const float *__restrict__ y, Geom g, Tof t,
+                                                          TofLut lut, float *__restrict__ pimg)
 {
     extern __shared__ __align__(16) float2 lut_sm[];
     lut_load(lut, lut_sm);
     __syncthreads();
     const uint32_t lb = lut_base(lut_sm);
-    const int64_t c = blockIdx.x * (int64_t)kBlock + threadIdx.x;
+    const int64_t c = blockIdx.x * (int64_t)kLmBlock + threadIdx.x;
     if (c >= rg.count) return;
     const int64_t j = lor_index(rg, c);
     const float yj = y[io_index(rg, c)];
@@ -228,12 +243,17 @@ __global__ void __launch_bounds__(kBlock) k_back_tof_lm(Lors l, const int16_t *_
     const float reach = half_w + t.nsig * t.sigma;
     Ray r;
     ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
-    const float x = r.cf * yj;
-    for (int k = 0; k < r.nk; ++k) {
-        const Cell cl = plane_cell(r, k);
-        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+    const PRay q = pray_from(r, g);
+    const float x = q.cf * yj;
+    float fk = 0.f;
+    int po = q.off;
+    for (int k = 0; k < q.nk; ++k) {
+        const PCell cl = pray_cell(q, fk, po);
+        const float tau = fmaf(q.dtau, fk, q.tau0);
         const float w = tof_weight(lb, lut.inv_h, half_w, tau, centre);
-        if (w != 0.f) plane_scatter(img, r, k, cl, x * w);
+        if (w != 0.f) pray_scatter(pimg, q, cl, x * w);
+        fk += 1.f;
+        po += q.sp;
     }
 }
 
@@ -315,9 +335,9 @@ cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, co
 {
     if (rg.count == 0) return cudaSuccess;
     if (lm_mode == 1)
-        k_fwd_tof_lm<1><<<grid_for(rg.count, kBlock), kBlock, kLutBytes, st>>>(l, tofbin, rg, img, g, t, lut, p);
+        k_fwd_tof_lm<1><<<grid_for(rg.count, kLmBlock), kLmBlock, kLutBytes, st>>>(l, tofbin, rg, img, g, t, lut, p);
     else
-        k_fwd_tof_lm<0><<<grid_for(rg.count, kBlock), kBlock, kLutBytes, st>>>(l, tofbin, rg, img, g, t, lut, p);
+        k_fwd_tof_lm<0><<<grid_for(rg.count, kLmBlock), kLmBlock, kLutBytes, st>>>(l, tofbin, rg, img, g, t, lut, p);
     return cudaGetLastError();
 }
 
@@ -325,7 +345,7 @@ cudaError_t launch_back_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, c
                                const Tof &t, const TofLut &lut, float *img, cudaStream_t st)
 {
     if (rg.count == 0) return cudaSuccess;
-    k_back_tof_lm<<<grid_for(rg.count, kBlock), kBlock, kLutBytes, st>>>(l, tofbin, rg, y, g, t, lut, img);
+    k_back_tof_lm<<<grid_for(rg.count, kLmBlock), kLmBlock, kLutBytes, st>>>(l, tofbin, rg, y, g, t, lut, img);
     return cudaGetLastError();
 }
 

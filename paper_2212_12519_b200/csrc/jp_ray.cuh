@@ -272,4 +272,95 @@ __device__ __forceinline__ float tof_weight(uint32_t base, float inv_h, float ha
     return 0.5f * (lut_E(base, inv_h, x + half_w) - lut_E(base, inv_h, x - half_w));
 }
 
+// ---- padded image: the per-LOR kernels without boundary tests ----------------------------------------
+// Reading A5 (neighbours outside the image count as zero) is zero padding.  The per-LOR kernels work on
+// a copy of the image with kImgPad zero voxels on every side (jp_pad.cu), so the four neighbour loads /
+// atomic adds of a plane need no bounds predicates.  PRay is Ray for that copy: the plane range is
+// trimmed (evaluating the end planes with the same float32 FMA as the loop) so that
+// -kImgPad <= floor(u_q) and floor(u_q) + 1 <= n_q + kImgPad - 1 on every visited plane -- planes
+// trimmed away have all four neighbours outside the image and contribute exactly zero.
+constexpr int kImgPad = 2;
+
+struct PRay {
+    int nk;           // planes to visit (0: nothing to do)
+    int off;          // element offset of (first plane, k1 = 0, k2 = 0) in the padded image, biased for the
+                      // magic-number floor: off + bits(t1) * s1 + bits(t2) * s2 addresses the cell
+    int sp, s1, s2;   // padded element strides of p, q1, q2
+    float a1, b1, a2, b2, cf, tau0, dtau;
+};
+
+__device__ __forceinline__ PRay pray_from(const Ray &r, const Geom &g)
+{
+    PRay q;
+    const int pn1 = g.n[1] + 2 * kImgPad, pn2 = g.n[2] + 2 * kImgPad;
+    const int st[3] = {pn1 * pn2, pn2, 1};
+    const int p = r.p, q1 = (p == 0) ? 1 : 0, q2 = (p == 2) ? 1 : 2;
+    q.sp = st[p];
+    q.s1 = st[q1];
+    q.s2 = st[q2];
+    q.b1 = r.b1;
+    q.b2 = r.b2;
+    q.cf = r.cf;
+    q.dtau = r.dtau;
+    // trim both ends against the padded range
+    const float lo = -(float)kImgPad + 0.1f;
+    const float hi1 = (float)(r.n1 + kImgPad - 1) - 0.1f, hi2 = (float)(r.n2 + kImgPad - 1) - 0.1f;
+    int k0 = 0, k1 = r.nk - 1;
+    while (k0 <= k1) {
+        const float u1 = fmaf(r.b1, (float)k0, r.a1), u2 = fmaf(r.b2, (float)k0, r.a2);
+        if (u1 > lo && u1 < hi1 && u2 > lo && u2 < hi2) break;
+        ++k0;
+    }
+    while (k0 <= k1) {
+        const float u1 = fmaf(r.b1, (float)k1, r.a1), u2 = fmaf(r.b2, (float)k1, r.a2);
+        if (u1 > lo && u1 < hi1 && u2 > lo && u2 < hi2) break;
+        --k1;
+    }
+    q.nk = k1 - k0 + 1;
+    // rebase the affine coefficients to the first kept plane (one extra float32 rounding)
+    q.a1 = fmaf(r.b1, (float)k0, r.a1);
+    q.a2 = fmaf(r.b2, (float)k0, r.a2);
+    q.tau0 = fmaf(r.dtau, (float)k0, r.tau0);
+    q.off = (int)((uint32_t)((r.i0 + k0 + kImgPad) * q.sp + kImgPad * (q.s1 + q.s2)) -
+                  (uint32_t)kMagicI * (uint32_t)q.s1 - (uint32_t)kMagicI * (uint32_t)q.s2); // wraps by design
+    return q;
+}
+
+// one plane of a PRay: cell offset and bilinear fractions (FMA pipe only: the floor is a round-down add)
+struct PCell {
+    int off;
+    float w1, w2;
+};
+
+__device__ __forceinline__ PCell pray_cell(const PRay &q, float fk, int plane_off)
+{
+    const float u1 = fmaf(q.b1, fk, q.a1), u2 = fmaf(q.b2, fk, q.a2);
+    const float t1 = __fadd_rd(u1, kMagic), t2 = __fadd_rd(u2, kMagic);
+    PCell c;
+    c.w1 = u1 - (t1 - kMagic);
+    c.w2 = u2 - (t2 - kMagic);
+    c.off = (int)((uint32_t)plane_off + __float_as_uint(t1) * (uint32_t)q.s1 + __float_as_uint(t2) * (uint32_t)q.s2);
+    return c;
+}
+
+__device__ __forceinline__ float pray_value(const float *__restrict__ pimg, const PRay &q, const PCell &c)
+{
+    const float *ptr = pimg + c.off;
+    const float v00 = __ldg(ptr), v01 = __ldg(ptr + q.s2), v10 = __ldg(ptr + q.s1), v11 = __ldg(ptr + q.s1 + q.s2);
+    const float lo = fmaf(c.w2, v01 - v00, v00);
+    const float hi = fmaf(c.w2, v11 - v10, v10);
+    return fmaf(c.w1, hi - lo, lo);
+}
+
+__device__ __forceinline__ void pray_scatter(float *__restrict__ pimg, const PRay &q, const PCell &c, float x)
+{
+    float *ptr = pimg + c.off;
+    const float xa = x * (1.f - c.w1), xb = x * c.w1;
+    const float m2 = 1.f - c.w2;
+    atomicAdd(ptr, xa * m2);
+    atomicAdd(ptr + q.s2, xa * c.w2);
+    atomicAdd(ptr + q.s1, xb * m2);
+    atomicAdd(ptr + q.s1 + q.s2, xb * c.w2);
+}
+
 } // namespace jp
