@@ -1,19 +1,21 @@
 #!/usr/bin/env python
-"""bench.py -- headline benchmark of the B200-native Joseph projector.
+"""bench.py -- benchmark of the B200-native Joseph projector.
 
-    python bench.py --gpus N --steps K --warmup W [--impl reference]
+    python bench.py --gpus N --steps K --warmup W [--config {1,2,3,4}] [--impl reference]
 
-A "step" is one pass of the hot path over one batch of synthetic input: the non-TOF forward
-projection of the phantom over all 151,584,768 sinogram LORs of BASELINE.json configs[1], followed
-by the exact adjoint back projection of a U[0,1) sinogram (image zero-fill included).
-`value` = LORs per second through that fwd+back pair (the paper reports fwd+back sums),
-inputs resident in HBM.  `e2e` is the same pair through the host-buffer C-ABI calls
-(jp_fwd_host / jp_back_host) with host<->device copies inside the timed region.
+A "step" is one pass of the hot path over one batch of synthetic input.  The default workload is
+BASELINE.json configs[1] (the configuration the headline LORs/s is quoted on): the non-TOF forward
+projection of the phantom over all 151,584,768 sinogram LORs followed by the exact adjoint back projection
+of a U[0,1) sinogram (image zero-fill included).  `value` = LORs per second through that fwd+back pair
+(the paper reports fwd+back sums), inputs resident in HBM.  `e2e` is the same pair through the
+host-buffer C-ABI calls (jp_fwd_host / jp_back_host) with host<->device copies inside the timed region.
+The default run also times configs[2], [3] and [4] briefly and reports them under "other_configs"
+(BASELINE.json metric: LORs/s fwd, back and TOF-LM events/s, each with its roofline fraction);
+`--config C` makes configs[C] the timed workload of the line instead (used for the ncu captures in profiles/).
 
-N > 1 (torchrun): LORs are independent units; every rank projects its own full
-configs[1] sinogram of its own frame (weak scaling), no data-path collective; timing is the max over
-ranks.  `--impl reference` times the float64 CPU oracle (oracle/) on a bounded sample of the same
-workload on the host cores.
+N > 1 (torchrun): LORs are independent units; every rank projects its own full frame (weak
+scaling), no data-path collective; timing is the max over ranks.  `--impl reference` times the float64 CPU
+oracle (oracle/) on a bounded sample of the same workload on the host cores.
 """
 from __future__ import annotations
 
@@ -33,15 +35,34 @@ sys.path.insert(0, ROOT)
 
 from paper_2212_12519_b200 import inputs  # noqa: E402
 
-METRIC = "LORs/s (non-TOF sinogram fwd+back pair)"
-UNIT = "LORs/s"
-WORKLOAD = ("configs[1]: non-TOF sinogram fwd+back, 151584768 LORs (257 radial x 256 views x 48x48 ring pairs), "
-            "image 200x200x96 @ 2 mm (cylinder + 10 hot spheres)")
+G = inputs.GEOM_SCANNER
+NVOX = int(np.prod(G.n))
+TOFP = inputs.TofParams()
+TOF_ARGS = (TOFP.tofbin_width, TOFP.sigma_tof, TOFP.n_sigmas, TOFP.n_tofbins)
+
 # FP32 lane-instructions per plane-step of the minimal formulation
-LANE_INSTR_FWD = 11.0
-LANE_INSTR_BACK = 12.0
+LANE = {"fwd": 11.0, "back": 12.0, "lm": 40.0, "sino": 112.0}
 FP32_LANES_PER_SM = 128
 N_SM = 148
+
+SPEC = {
+    1: dict(metric="LORs/s (non-TOF sinogram fwd+back pair)", unit="LORs/s",
+            workload="configs[1]: non-TOF sinogram fwd+back, 151584768 LORs (257 radial x 256 views x 48x48 ring "
+                     "pairs), image 200x200x96 @ 2 mm (cylinder + 10 hot spheres)",
+            l2="inputs (4.2 GB of end points + values per step) exceed the 126 MB L2; no flush"),
+    2: dict(metric="LORs/s (TOF sinogram fwd+back pair, 29 TOF bins per LOR)", unit="LORs/s",
+            workload="configs[2]: TOF sinogram fwd+back, one OSEM subset = 16 views x 257 radial x 2304 ring pairs "
+                     "= 9474048 LORs x 29 TOF bins of 17 mm, sigma 13.6 mm, 3 sigma; same scanner and phantom",
+            l2="inputs (227 MB of end points + 1.1 GB of TOF sinogram per direction) exceed the 126 MB L2; no flush"),
+    3: dict(metric="events/s (TOF listmode fwd+back pair)", unit="events/s",
+            workload="configs[3]: TOF listmode fwd+back, 40000000 events sampled from the phantom (crystal-snapped "
+                     "end points, int16 TOF bin), sorted once by the listmode plan; results in caller order",
+            l2="inputs (1.04 GB of sorted events + 0.32 GB of per-event values per step) exceed the 126 MB L2; no flush"),
+    4: dict(metric="events/s (TOF listmode OSEM, one full iteration of 20 subsets)", unit="events/s",
+            workload="configs[4]: listmode OSEM on the configs[3] events, 20 subsets, sens = non-TOF A^T 1 over all "
+                     "configs[1] LORs; one step = one full iteration (20 x (fwd, ratio, back, update))",
+            l2="every iteration streams all 1.04 GB of sorted events; no flush"),
+}
 
 
 def measured_peaks():
@@ -102,60 +123,290 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-# ---- oracle legs ----------------------------------------------------------------------------------------------
-def oracle_sample():
-    """bounded sample of configs[1]: 17 views (incl. a 45 degree tie view) x all 257 radial x every 2nd ring pair"""
-    views = sorted(set(range(5, 256, 16)) | {64})
-    xs, xe = inputs.sinogram_lors(views=views)
-    xs, xe = xs[:, ::2].contiguous().numpy(), xe[:, ::2].contiguous().numpy()
-    desc = ("views {5,21,...,245} and 64 x 257 radial x every 2nd of the 2304 ring pairs = %d LORs of configs[1] "
-            "(fwd + back, float64, OpenMP)" % xs.shape[1])
-    return xs, xe, desc
-
-
-def time_oracle(steps: int, warmup: int):
+# ---- oracle legs (cpu_baseline and --impl reference): the float64 oracle on a bounded sample ------------------
+def time_oracle(config: int, steps: int, warmup: int):
+    """(units in the sample, mean fwd s, mean back s, cores, description); for config 4 fwd_s = whole iteration"""
     import oracle
     oracle.build()
-    g = inputs.GEOM_SCANNER
     ph = inputs.phantom().astype(np.float64)
-    xs, xe, desc = oracle_sample()
-    n = xs.shape[1]
-    y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 101).numpy().astype(np.float64)
+    if config == 1:
+        # 17 views (incl. a 45 degree tie view) x all 257 radial x every 2nd ring pair
+        views = sorted(set(range(5, 256, 16)) | {64})
+        xs, xe = inputs.sinogram_lors(views=views)
+        xs, xe = xs[:, ::2].contiguous().numpy(), xe[:, ::2].contiguous().numpy()
+        n = xs.shape[1]
+        desc = ("views {5,21,...,245} and 64 x 257 radial x every 2nd of the 2304 ring pairs = %d LORs of configs[1] "
+                "(fwd + back, float64, OpenMP)" % n)
+        y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 101).numpy().astype(np.float64)
+        f = lambda: oracle.fwd(xs, xe, ph, G.origin, G.voxsize)
+        b = lambda: oracle.back(xs, xe, y, G.n, G.origin, G.voxsize)
+    elif config == 2:
+        xs, xe = inputs.sinogram_lors(views=inputs.SUBSET_VIEWS)
+        xs, xe = xs[:, ::24].contiguous().numpy(), xe[:, ::24].contiguous().numpy()
+        n = xs.shape[1]
+        desc = ("every 24th LOR of the configs[2] subset = %d LORs x 29 TOF bins (fwd + back, float64, OpenMP)" % n)
+        y = inputs.uniform_values((n, 29), 0.0, 1.0, seed=inputs.BASE_SEED + 102).numpy().astype(np.float64)
+        f = lambda: oracle.fwd_tof_sino(xs, xe, ph, G.origin, G.voxsize, *TOF_ARGS)
+        b = lambda: oracle.back_tof_sino(xs, xe, y, G.n, G.origin, G.voxsize, *TOF_ARGS)
+    else:
+        n = 1_000_000
+        xs, xe, tb = inputs.listmode_events(n, img=inputs.phantom(), chunk=2_000_000)
+        xs, xe, tb = xs.numpy(), xe.numpy(), tb.numpy()
+        if config == 3:
+            desc = "1000000 events of the configs[3] model (CPU-seeded) (fwd + back, float64, OpenMP)"
+            y = inputs.uniform_values(n, 0.5, 2.0, seed=inputs.BASE_SEED + 103).numpy().astype(np.float64)
+            f = lambda: oracle.fwd_tof_lm(xs, xe, tb, ph, G.origin, G.voxsize, *TOF_ARGS[:3])
+            b = lambda: oracle.back_tof_lm(xs, xe, tb, y, G.n, G.origin, G.voxsize, *TOF_ARGS[:3])
+        else:
+            desc = ("one OSEM iteration (20 subsets) on 1000000 events of the configs[3] model, sens = ones "
+                    "(float64, OpenMP)")
+            sens = np.ones(G.n)
+            f = lambda: oracle.lm_osem(xs, xe, tb, sens, np.ones(G.n, dtype=np.float32), G.origin, G.voxsize,
+                                       *TOF_ARGS[:3], n_subsets=20, n_iter=1)
+            b = lambda: None
     times = []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
-        oracle.fwd(xs, xe, ph, g.origin, g.voxsize)
+        f()
         t1 = time.perf_counter()
-        oracle.back(xs, xe, y, g.n, g.origin, g.voxsize)
+        b()
         t2 = time.perf_counter()
         if it >= warmup:
             times.append((t1 - t0, t2 - t1))
     tf = float(np.mean([t[0] for t in times]))
-    tb = float(np.mean([t[1] for t in times]))
-    return dict(n=n, fwd_s=tf, back_s=tb, cores=oracle.num_threads(), sample=desc)
+    tb_ = float(np.mean([t[1] for t in times]))
+    return dict(n=n, fwd_s=tf, back_s=tb_, cores=oracle.num_threads(), sample=desc)
+
+
+def cpu_baseline_dict(config: int, r: dict):
+    t = r["fwd_s"] + r["back_s"]
+    d = {"value": r["n"] / t, "unit": SPEC[config]["unit"], "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+    if config != 4:
+        d["fwd_per_s"] = r["n"] / r["fwd_s"]
+        d["back_per_s"] = r["n"] / r["back_s"]
+    return d
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    r = time_oracle(args.steps, args.warmup)
+    c = args.config
+    r = time_oracle(c, args.steps, args.warmup)
     t = r["fwd_s"] + r["back_s"]
     val = r["n"] / t
     line = {
-        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "sample_per_step": r["sample"]},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
-                         "fwd_lors_per_s": r["n"] / r["fwd_s"], "back_lors_per_s": r["n"] / r["back_s"]},
-        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "impl": "reference", "metric": SPEC[c]["metric"], "value": val, "unit": SPEC[c]["unit"], "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": SPEC[c]["workload"], "sample_per_step": r["sample"]},
+        "cpu_baseline": cpu_baseline_dict(c, r),
+        "e2e": {"value": val, "unit": SPEC[c]["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
-# ---- the CUDA arm ---------------------------------------------------------------------------------------------
+# ---- the CUDA arm: one Workload per BASELINE.json config -------------------------------------------------------
+class Workload:
+    """set-up (untimed) of configs[c] on `dev`; step(ev) enqueues one pass on the current stream and records
+    the events ev[0] (start), ev[1] (forward done), ev[2] (back done) when given."""
+
+    def __init__(self, c: int, jp, dev, rank: int):
+        self.c, self.jp, self.dev = c, jp, dev
+        self.stream = torch.cuda.current_stream()
+        self.tof = jp.make_tof(*TOF_ARGS)
+        self.img = torch.from_numpy(inputs.phantom(seed=inputs.BASE_SEED + 1 + 1000 * rank)).to(dev)
+        self.bimg = torch.zeros(G.n, dtype=torch.float32, device=dev)
+        self.plan = None
+        self.plan_s = None
+        if c in (1, 2):
+            self.xs, self.xe = inputs.sinogram_lors(views=None if c == 1 else inputs.SUBSET_VIEWS, device=dev)
+            self.n = self.xs.shape[1]
+            shape = self.n if c == 1 else (self.n, TOFP.n_tofbins)
+            self.y = inputs.uniform_values(shape, 0.0, 1.0, seed=inputs.BASE_SEED + 100 + c + rank, device=dev)
+            self.p = torch.empty(shape, dtype=torch.float32, device=dev)
+            self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
+            self.kinds = ("fwd", "back") if c == 1 else ("sino", "sino")
+            self.launches = 2
+            self.hbm_bytes = (self.n * 28 + NVOX * 4) if c == 1 else (self.n * (24 + 4 * TOFP.n_tofbins) + NVOX * 4)
+        else:
+            nev = int(os.environ.get("JP_BENCH_EVENTS", "40000000"))
+            self.xs, self.xe, self.tb = inputs.listmode_events(nev, seed=inputs.BASE_SEED + 3 + rank, device=dev,
+                                                               img=inputs.phantom())
+            self.n = self.xs.shape[1]
+            self.plane_steps = jp.jp_plane_steps_tof_lm(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            self.plan = jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof, n_subsets=20)
+            torch.cuda.synchronize()
+            self.plan_s = time.perf_counter() - t0
+            self.kinds = ("lm", "lm")
+            self.hbm_bytes = self.n * 30 + NVOX * 4
+            if c == 3:
+                self.y = inputs.uniform_values(self.n, 0.5, 2.0, seed=inputs.BASE_SEED + 103 + rank, device=dev)
+                self.p = torch.empty(self.n, dtype=torch.float32, device=dev)
+                self.launches = 2 + 3        # + pad / zero-fill of the padded accumulator / unpad-add
+            else:
+                self.sens = torch.ones(G.n, dtype=torch.float32, device=dev)   # replaced by A^T 1 in setup_sens()
+                self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
+                self.launches = 3 * 20 + 2
+
+    def setup_sens(self):
+        """configs[4]: sens = non-TOF back projection of ones over all configs[1] LORs (one-time, untimed)"""
+        sx, se = inputs.sinogram_lors(device=self.dev)
+        self.sens.zero_()
+        self.jp.jp_back(sx, se, torch.ones(sx.shape[1], device=self.dev), G.n, G.origin, G.voxsize, img=self.sens)
+        torch.cuda.synchronize()
+
+    def step(self, ev=None):
+        jp, c, s = self.jp, self.c, self.stream
+        if ev:
+            ev[0].record(s)
+        if c == 1:
+            jp.jp_fwd(self.xs, self.xe, self.img, G.origin, G.voxsize, out=self.p)
+        elif c == 2:
+            jp.jp_fwd_tof_sino(self.xs, self.xe, self.img, G.origin, G.voxsize, self.tof, out=self.p)
+        elif c == 3:
+            jp.jp_fwd_tof_lm_planned(self.plan, self.img, out=self.p)
+        else:
+            jp.jp_lm_osem_planned(self.plan, self.sens, self.x, n_iter=1)
+        if ev:
+            ev[1].record(s)
+        if c != 4:
+            self.bimg.zero_()
+        if c == 1:
+            jp.jp_back(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
+        elif c == 2:
+            jp.jp_back_tof_sino(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, self.tof, img=self.bimg)
+        elif c == 3:
+            jp.jp_back_tof_lm_planned(self.plan, self.y, img=self.bimg)
+        if ev:
+            ev[2].record(s)
+
+    def checksum(self):
+        if self.c == 4:
+            return float(self.x.double().sum())
+        p = self.p.reshape(-1)
+        return float(p[:: max(1, p.numel() // 4096)].double().sum()) + float(self.bimg.double().sum())
+
+    # ---- end to end with HOST buffers: H2D of the step's inputs, the calls, D2H of the results, all timed ------
+    def e2e_setup(self):
+        jp, c = self.jp, self.c
+        pin = lambda t: t.cpu().pin_memory()
+        if c == 1:
+            self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
+                          p=torch.empty(self.n, dtype=torch.float32).pin_memory(),
+                          b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
+            self.e2e_api = "jp_fwd_host + jp_back_host (pinned host tensors)"
+            self.h2d, self.d2h = 2 * 24 * self.n + 4 * self.n + 2 * 4 * NVOX, 4 * self.n + 4 * NVOX
+        elif c == 2:
+            self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
+                          p=torch.empty_like(self.p, device="cpu").pin_memory(),
+                          b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
+            self.e2e_api = "pinned host -> device copies, jp_fwd_tof_sino + jp_back_tof_sino, device -> pinned host"
+            self.h2d = 24 * self.n + 4 * self.y.numel() + 4 * NVOX
+            self.d2h = 4 * self.p.numel() + 4 * NVOX
+        elif c == 3:
+            self.h = dict(xs=pin(self.xs), xe=pin(self.xe), tb=pin(self.tb), y=pin(self.y), img=pin(self.img),
+                          p=torch.empty(self.n, dtype=torch.float32).pin_memory(),
+                          b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
+            self.e2e_api = ("pinned host -> device copies of the events, jp_lm_plan_create, jp_fwd_tof_lm_planned + "
+                            "jp_back_tof_lm_planned, device -> pinned host")
+            self.h2d = 26 * self.n + 4 * self.n + 4 * NVOX
+            self.d2h = 4 * self.n + 4 * NVOX
+        else:
+            self.h = dict(xs=pin(self.xs), xe=pin(self.xe), tb=pin(self.tb), sens=pin(self.sens),
+                          x=torch.ones(G.n, dtype=torch.float32).pin_memory(),
+                          xo=torch.empty(G.n, dtype=torch.float32).pin_memory())
+            self.e2e_api = ("pinned host -> device copies of the events and sens, jp_lm_plan_create, "
+                            "jp_lm_osem_planned (1 iteration), image device -> pinned host")
+            self.h2d = 26 * self.n + 2 * 4 * NVOX
+            self.d2h = 4 * NVOX
+
+    def e2e_step(self):
+        jp, c, h = self.jp, self.c, self.h
+        if c == 1:
+            jp.jp_fwd_host(h["xs"], h["xe"], h["img"], G.origin, G.voxsize, out=h["p"])
+            h["b"].zero_()
+            jp.jp_back_host(h["xs"], h["xe"], h["y"], h["b"], G.origin, G.voxsize)
+            return
+        self.xs.copy_(h["xs"], non_blocking=True)
+        self.xe.copy_(h["xe"], non_blocking=True)
+        if c == 2:
+            self.img.copy_(h["img"], non_blocking=True)
+            self.y.copy_(h["y"], non_blocking=True)
+            self.step()
+        else:
+            self.tb.copy_(h["tb"], non_blocking=True)
+            plan = self.jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof, n_subsets=20)
+            old, self.plan = self.plan, plan
+            if c == 3:
+                self.img.copy_(h["img"], non_blocking=True)
+                self.y.copy_(h["y"], non_blocking=True)
+            else:
+                self.sens.copy_(h["sens"], non_blocking=True)
+                self.x.copy_(h["x"], non_blocking=True)
+            self.step()
+            torch.cuda.synchronize()
+            self.plan = old
+            plan.destroy()
+        if c == 4:
+            h["xo"].copy_(self.x, non_blocking=True)
+        else:
+            h["p"].copy_(self.p, non_blocking=True)
+            h["b"].copy_(self.bimg, non_blocking=True)
+        torch.cuda.synchronize()
+
+
+def measure(w: Workload, steps: int, warmup: int, barrier, sampler=None):
+    """warm-up, then `steps` timed steps between CUDA events on the launching stream"""
+    for _ in range(warmup):
+        w.step()
+    barrier()
+    if sampler:
+        sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e_beg.record(w.stream)
+    for k in range(steps):
+        w.step(evs[k])
+    e_end.record(w.stream)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = e_beg.elapsed_time(e_end)
+    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    back_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))   # includes the image zero-fill
+    return total_ms, fwd_ms, back_ms, clocks
+
+
+def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
+    peaks, peak_src = measured_peaks()
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
+    kf, kb = w.kinds
+    names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_fwd_tof_sino", "k_back_tof_sino"),
+             3: ("k_fwd_tof_lm", "k_back_tof_lm"), 4: ("k_fwd_tof_lm + k_back_tof_lm", "")}[w.c]
+    src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
+    if w.c == 4:
+        lane = 2 * LANE["lm"]
+        achieved = lane * w.plane_steps / (fwd_ms * 1e-3)
+        return {"bound": "alu", "kernel": names[0], "achieved": achieved / 1e12, "peak": alu_peak / 1e12,
+                "unit": "T lane-instr/s (FP32)", "frac": achieved / alu_peak, "traffic": None, "peak_source": src,
+                "plane_steps_per_iteration": w.plane_steps, "lane_instr_per_plane_step": lane,
+                "hbm_bound_frac": 2 * w.hbm_bytes / (fwd_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9)}
+    dom = "back" if back_ms >= fwd_ms else "fwd"
+    dom_ms = max(back_ms, fwd_ms)
+    lane = LANE[kb] if dom == "back" else LANE[kf]
+    achieved = lane * w.plane_steps / (dom_ms * 1e-3)
+    per = lambda ms, k: {"ms": ms, "per_s": w.n / ms * 1e3, "frac_alu": LANE[k] * w.plane_steps / (ms * 1e-3) / alu_peak}
+    return {"bound": "alu", "kernel": names[1] if dom == "back" else names[0], "achieved": achieved / 1e12,
+            "peak": alu_peak / 1e12, "unit": "T lane-instr/s (FP32)", "frac": achieved / alu_peak, "traffic": None,
+            "peak_source": src, "plane_steps_per_launch": w.plane_steps, "lane_instr_per_plane_step": lane,
+            "fwd": per(fwd_ms, kf), "back": per(back_ms, kb),
+            "hbm_bound_frac": w.hbm_bytes / (dom_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9)}
+
+
 def run_ours(args):
     from paper_2212_12519_b200 import binding as jp
     import torch.distributed as dist
@@ -171,132 +422,87 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     jp.load()
 
-    g = inputs.GEOM_SCANNER
-    # frame `rank`: same scanner, its own phantom and sinogram values (weak scaling, no exchange)
-    img = torch.from_numpy(inputs.phantom(seed=inputs.BASE_SEED + 1 + 1000 * rank)).to(dev)
-    xs, xe = inputs.sinogram_lors(device=dev)
-    n = xs.shape[1]
-    y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 101 + rank, device=dev)
-    p = torch.empty(n, dtype=torch.float32, device=dev)
-    bimg = torch.zeros(g.n, dtype=torch.float32, device=dev)
-    plane_steps = jp.jp_plane_steps(xs, xe, g.n, g.origin, g.voxsize)
-    stream = torch.cuda.current_stream()
-
-    def step(ev=None):
-        if ev:
-            ev[0].record(stream)
-        jp.jp_fwd(xs, xe, img, g.origin, g.voxsize, out=p)
-        if ev:
-            ev[1].record(stream)
-        bimg.zero_()
-        jp.jp_back(xs, xe, y, g.n, g.origin, g.voxsize, img=bimg)
-        if ev:
-            ev[2].record(stream)
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    e_beg = torch.cuda.Event(enable_timing=True)
-    e_end = torch.cuda.Event(enable_timing=True)
-    e_beg.record(stream)
-    for k in range(args.steps):
-        step(evs[k])
-    e_end.record(stream)
-    barrier()
-    clocks = sampler.stop() if rank == 0 else None
-    total_ms = e_beg.elapsed_time(e_end)
-    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-    back_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))   # includes the image zero-fill
-    checksum = float(p[:: max(1, n // 4096)].double().sum()) + float(bimg.double().sum())
+    c = args.config
+    w = Workload(c, jp, dev, rank)
+    if c == 4:
+        w.setup_sens()
+    total_ms, fwd_ms, back_ms, clocks = measure(w, args.steps, args.warmup, barrier,
+                                                ClockSampler(local) if rank == 0 else None)
+    checksum = w.checksum()
 
-    # ---- end to end through the host-buffer C ABI (pinned host tensors; H2D + kernels + D2H timed) --------
-    e2e = None
+    e2e_s = None
     if not args.no_e2e:
-        hxs, hxe = xs.cpu().pin_memory(), xe.cpu().pin_memory()
-        hy, himg = y.cpu().pin_memory(), img.cpu().pin_memory()
-        hp = torch.empty(n, dtype=torch.float32).pin_memory()
-        hb = torch.zeros(g.n, dtype=torch.float32).pin_memory()
-
-        def e2e_step():
-            jp.jp_fwd_host(hxs, hxe, himg, g.origin, g.voxsize, out=hp)
-            hb.zero_()
-            jp.jp_back_host(hxs, hxe, hy, hb, g.origin, g.voxsize)
-
-        e2e_step()
+        w.e2e_setup()
+        w.e2e_step()
         barrier()
         t0 = time.perf_counter()
         ne2e = max(1, min(args.steps, 3))
         for _ in range(ne2e):
-            e2e_step()
+            w.e2e_step()
         barrier()
         e2e_s = (time.perf_counter() - t0) / ne2e
-        nvox = int(np.prod(g.n))
-        e2e = {"s_per_step": e2e_s,
-               "h2d": 2 * 24 * n + 4 * n + 2 * 4 * nvox, "d2h": 4 * n + 4 * nvox,
-               "check": float((hp[:: max(1, n // 4096)].double().sum()))}
-        del hxs, hxe, hy, hp
+        w.h = None
 
     if world > 1:
-        t = torch.tensor([total_ms, fwd_ms, back_ms, e2e["s_per_step"] if e2e else 0.0], device=dev, dtype=torch.float64)
+        t = torch.tensor([total_ms, fwd_ms, back_ms, e2e_s or 0.0], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms, fwd_ms, back_ms = float(t[0]), float(t[1]), float(t[2])
-        if e2e:
-            e2e["s_per_step"] = float(t[3])
+        if e2e_s is not None:
+            e2e_s = float(t[3])
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     ms_per_step = total_ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
-    peaks, peak_src = measured_peaks()
-    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-    alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
-    dom = "back" if back_ms >= fwd_ms else "fwd"
-    dom_ms = max(back_ms, fwd_ms)
-    lane = LANE_INSTR_BACK if dom == "back" else LANE_INSTR_FWD
-    achieved = lane * plane_steps / (dom_ms * 1e-3)
-    hbm_bytes = n * 28 + int(np.prod(g.n)) * 4
-    roofline = {
-        "bound": "alu", "kernel": "k_back" if dom == "back" else "k_fwd",
-        "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "T lane-instr/s (FP32)",
-        "frac": achieved / alu_peak, "traffic": None,
-        "peak_source": f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})",
-        "plane_steps_per_launch": plane_steps, "lane_instr_per_plane_step": lane,
-        "fwd": {"ms": fwd_ms, "lors_per_s": n / fwd_ms * 1e3, "frac_alu": LANE_INSTR_FWD * plane_steps / (fwd_ms * 1e-3) / alu_peak},
-        "back": {"ms": back_ms, "lors_per_s": n / back_ms * 1e3, "frac_alu": LANE_INSTR_BACK * plane_steps / (back_ms * 1e-3) / alu_peak},
-        "hbm_bound_frac": hbm_bytes / (dom_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9),
-    }
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "lors_per_gpu": n, "l2": "inputs (4.2 GB of end points + values per step) exceed the 126 MB L2; no flush",
+        "metric": SPEC[c]["metric"], "value": world * w.n / (ms_per_step * 1e-3), "unit": SPEC[c]["unit"],
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": SPEC[c]["workload"], "units_per_gpu": w.n, "l2": SPEC[c]["l2"],
                    "parallelism": f"frames{world}" if world > 1 else "single"},
-        "gpu_launches": 2 * args.steps,
+        "gpu_launches": w.launches * args.steps,
         "clocks": clocks,
-        "roofline": roofline,
+        "roofline": roofline_dict(w, fwd_ms, back_ms),
         "checksum": checksum,
     }
-    if e2e:
-        line["e2e"] = {"value": world * n / e2e["s_per_step"], "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
-                       "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e["s_per_step"] * 1e3,
-                       "api": "jp_fwd_host + jp_back_host (pinned host tensors)"}
+    if w.plan_s is not None:
+        line["config"]["plan_s"] = w.plan_s
+    if c == 4:
+        line["s_per_iteration"] = ms_per_step * 1e-3
+    if e2e_s is not None:
+        line["e2e"] = {"value": world * w.n / e2e_s, "unit": SPEC[c]["unit"], "h2d_bytes_per_step": w.h2d,
+                       "d2h_bytes_per_step": w.d2h, "ms_per_step": e2e_s * 1e3, "api": w.e2e_api}
     if world == 1 and not args.no_cpu_baseline:
-        r = time_oracle(1, 0)
-        t = r["fwd_s"] + r["back_s"]
-        line["cpu_baseline"] = {"value": r["n"] / t, "unit": UNIT, "cores": r["cores"], "kind": "oracle",
-                                "sample": r["sample"], "fwd_lors_per_s": r["n"] / r["fwd_s"],
-                                "back_lors_per_s": r["n"] / r["back_s"]}
+        line["cpu_baseline"] = cpu_baseline_dict(c, time_oracle(c, 1, 0))
+    # ---- the other configs, briefly (single GPU, default workload only) -----------------------------------
+    if world == 1 and c == 1 and not args.no_other:
+        del w
+        torch.cuda.empty_cache()
+        other = {}
+        for oc in (2, 3, 4):
+            ow = Workload(oc, jp, dev, rank)
+            if oc == 4:
+                ow.setup_sens()
+            t_ms, f_ms, b_ms, _ = measure(ow, 3, 3, barrier)
+            r = roofline_dict(ow, f_ms, b_ms)
+            d = {"units": ow.n, "ms_per_step": t_ms / 3, "per_s": ow.n / (t_ms / 3 * 1e-3), "unit": SPEC[oc]["unit"],
+                 "plane_steps": ow.plane_steps, "frac_alu": r["frac"]}
+            if oc == 4:
+                d["s_per_iteration"] = t_ms / 3 * 1e-3
+            else:
+                d["fwd"], d["back"] = r["fwd"], r["back"]
+            if ow.plan_s is not None:
+                d["plan_s"] = ow.plan_s
+            other[f"configs[{oc}]"] = d
+            del ow
+            torch.cuda.empty_cache()
+        line["other_configs"] = other
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -308,8 +514,10 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3, 4])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other", action="store_true", help="skip the brief configs[2..4] runs of the default line")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

@@ -113,6 +113,11 @@ int jp_classify(const jp_lors *lors, uint8_t *principal_axis, void *stream);
    axis crossed by the closed segment whose crossing point has at least one of its four neighbours
    inside the image (the "plane-steps" the roofline is quoted in).  total: device uint64, caller-zeroed. */
 int jp_plane_steps(const jp_lors *lors, const jp_geom *geom, unsigned long long *total, void *stream);
+/* the same count for the TOF listmode projectors ("only affected by a few voxels"): only
+   the planes whose crossing point lies inside the truncated TOF kernel of the event's own bin,
+   |tau - c| <= n_sigmas sigma + W/2, are visited. */
+int jp_plane_steps_tof_lm(const jp_lors *lors, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
+                          unsigned long long *total, void *stream);
 
 /* ---- listmode OSEM (Hudson & Larkin, PAPER.md:193 ref. 39) ------------------- */
 /* n_iter iterations over n_subsets subsets, subset m = events {e : e mod n_subsets == m}, in order:

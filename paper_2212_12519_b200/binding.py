@@ -53,6 +53,8 @@ EXPORTS = {
                                  C.POINTER(jp_tof), C.c_void_p, C.c_void_p]),
     "jp_classify": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p]),
     "jp_plane_steps": (C.c_int, [C.POINTER(jp_lors), C.POINTER(jp_geom), C.c_void_p, C.c_void_p]),
+    "jp_plane_steps_tof_lm": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
+                                        C.c_void_p, C.c_void_p]),
     "jp_lm_osem_workspace_bytes": (C.c_size_t, [C.c_int64, C.POINTER(jp_geom), C.c_int]),
     "jp_lm_osem": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
                              C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]),
@@ -162,6 +164,17 @@ def jp_plane_steps(xstart, xend, n, origin, voxsize, stream=None) -> int:
     g = make_geom(n, origin, voxsize)
     total = torch.zeros(1, dtype=torch.int64, device=xstart.device)
     _check(load().jp_plane_steps(C.byref(l), C.byref(g), total.data_ptr(), _stream(stream)), "jp_plane_steps")
+    return int(total.item())
+
+
+def jp_plane_steps_tof_lm(xstart, xend, tofbin, n, origin, voxsize, tof: jp_tof, stream=None) -> int:
+    """number of (event, plane) pairs the TOF listmode projectors visit (synchronises)"""
+    l, keep = make_lors(xstart, xend)
+    tofbin = _bins(tofbin, l.n)
+    g = make_geom(n, origin, voxsize)
+    total = torch.zeros(1, dtype=torch.int64, device=xstart.device)
+    _check(load().jp_plane_steps_tof_lm(C.byref(l), tofbin.data_ptr(), C.byref(g), C.byref(tof), total.data_ptr(),
+                                        _stream(stream)), "jp_plane_steps_tof_lm")
     return int(total.item())
 
 

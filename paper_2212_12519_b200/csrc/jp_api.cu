@@ -177,6 +177,22 @@ int jp_plane_steps(const jp_lors *lors, const jp_geom *geom, unsigned long long 
     return JP_OK;
 }
 
+int jp_plane_steps_tof_lm(const jp_lors *lors, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
+                          unsigned long long *total, void *stream)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_lors(lors, l));
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, false, t));
+    if (!total || (lors->n > 0 && !tofbin)) return fail(JP_ERR_POINTER, "total or tofbin is NULL");
+    JP_CUDA(jp::launch_plane_steps_tof_lm(l, tofbin, lors->n, g, t, total, (cudaStream_t)stream),
+            "jp_plane_steps_tof_lm");
+    return JP_OK;
+}
+
 int jp_fwd(const jp_lors *lors, const float *img, const jp_geom *geom, float *p, void *stream)
 {
     g_err[0] = 0;

@@ -23,6 +23,9 @@ cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_
 
 cudaError_t launch_plane_steps(const Lors &l, int64_t n, const Geom &g, unsigned long long *total, cudaStream_t st);
 
+cudaError_t launch_plane_steps_tof_lm(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
+                                      unsigned long long *total, cudaStream_t st);
+
 cudaError_t launch_fwd(const Lors &l, Range rg, const float *img, const Geom &g, float *p, cudaStream_t st);
 cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, float *img, cudaStream_t st);
 

@@ -43,6 +43,23 @@ __global__ void k_plane_steps(Lors l, int64_t n, Geom g, unsigned long long *__r
     if ((threadIdx.x & 31) == 0 && nk) atomicAdd(total, nk);
 }
 
+// plane-steps of the TOF listmode projectors: planes inside the truncated kernel of the event's own bin
+__global__ void k_plane_steps_tof_lm(Lors l, const int16_t *__restrict__ tofbin, int64_t n, Geom g, Tof t,
+                                     unsigned long long *__restrict__ total)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    unsigned long long nk = 0;
+    if (j < n) {
+        const float centre = (float)tofbin[j] * t.width;
+        const float reach = 0.5f * t.width + t.nsig * t.sigma;
+        Ray r;
+        ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+        nk = (unsigned long long)r.nk;
+    }
+    for (int o = 16; o > 0; o >>= 1) nk += __shfl_xor_sync(0xffffffffu, nk, o);
+    if ((threadIdx.x & 31) == 0 && nk) atomicAdd(total, nk);
+}
+
 // ---- non-TOF ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlock) k_fwd(Lors l, Range rg, const float *__restrict__ img, Geom g,
                                                 float *__restrict__ p)
@@ -282,6 +299,14 @@ cudaError_t launch_plane_steps(const Lors &l, int64_t n, const Geom &g, unsigned
 {
     if (n == 0) return cudaSuccess;
     k_plane_steps<<<grid_for(n, 256), 256, 0, st>>>(l, n, g, total);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_plane_steps_tof_lm(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
+                                      unsigned long long *total, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_plane_steps_tof_lm<<<grid_for(n, 256), 256, 0, st>>>(l, tofbin, n, g, t, total);
     return cudaGetLastError();
 }
 

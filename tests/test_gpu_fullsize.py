@@ -1,0 +1,175 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The oracle cannot run 151.6 M LORs / 40 M events in seconds, so (task statement, parity bar):
+  forward   the full-size launch is compared with the oracle on SAMPLED outputs (seeded random LORs plus
+            whole tracks that contain the 45 degree tie views and the degenerate r = +-128 LORs);
+  back      the full-size launch gets a sinogram that is zero outside a sampled subset S of the LORs, so
+            its result is the oracle's back projection of the LORs of S alone -- compared voxel by voxel;
+            plus a property that holds at any size: <A x, y> = <x, A^T y> with the dense y;
+  counts    LOR / event / subset counts and the principal axis of every sampled LOR: bit exact.
+Tolerances are BASELINE.json north_star's (see test_gpu_parity.py).
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2212_12519_b200 import binding as jp
+from paper_2212_12519_b200 import inputs
+from test_gpu_parity import ADJ_GAP, adj_gap, assert_back, assert_fwd
+
+pytestmark = pytest.mark.gpu
+
+G = inputs.GEOM_SCANNER
+TOFP = inputs.TofParams()
+TOF_ARGS = (TOFP.tofbin_width, TOFP.sigma_tof, TOFP.n_sigmas, TOFP.n_tofbins)
+
+
+def _tof():
+    return jp.make_tof(TOFP.tofbin_width, TOFP.sigma_tof, TOFP.n_sigmas, TOFP.n_tofbins)
+
+
+def _sample(n, k, seed, extra=()):
+    rng = np.random.default_rng(seed)
+    idx = np.unique(np.concatenate([rng.integers(0, n, k)] + [np.asarray(e, dtype=np.int64) for e in extra]))
+    return torch.from_numpy(idx)
+
+
+def _track(v_index, r, n_views_total=inputs.N_VIEWS):
+    """all 2304 ring pairs of sinogram bin (view position v_index in the list, radial offset r)"""
+    base = (v_index * inputs.N_RADIAL + (r + 128)) * 2304
+    return np.arange(base, base + 2304)
+
+
+@pytest.fixture(scope="module")
+def phantom_dev(cuda_device):
+    ph = inputs.phantom()
+    return ph, torch.from_numpy(ph).to(cuda_device)
+
+
+def test_config1_full_nontof(cuda_device, phantom_dev):
+    ph, imgd = phantom_dev
+    xs, xe = inputs.sinogram_lors(device=cuda_device)
+    n = xs.shape[1]
+    assert n == 151_584_768                                               # LOR count: bit exact
+    # sample: 150k random LORs + tie view 64 (r = 0, 17), view 192 (r = -5), rim (r = 64), degenerate r = 128
+    extra = [_track(64, 0), _track(64, 17), _track(192, -5), _track(10, 64), _track(3, 128), _track(255, -128)]
+    idx = _sample(n, 150_000, 1, extra).to(cuda_device)
+    sxs, sxe = xs[:, idx].contiguous(), xe[:, idx].contiguous()
+    hxs, hxe = sxs.cpu().numpy(), sxe.cpu().numpy()
+
+    ax = jp.jp_classify(xs, xe)
+    assert np.array_equal(ax[idx].cpu().numpy(), oracle.classify(hxs, hxe, G.n, G.origin, G.voxsize))
+    del ax
+    p = jp.jp_fwd(xs, xe, imgd, G.origin, G.voxsize)
+    ref = oracle.fwd(hxs, hxe, ph, G.origin, G.voxsize)
+    assert (ref > 0).mean() > 0.2          # 44 % of configs[1] LORs reach the image, fewer the phantom
+    assert_fwd(p[idx], ref)
+
+    # back: the full launch with y supported on the sample only
+    y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 101, device=cuda_device)
+    ys = torch.zeros_like(y)
+    ys[idx] = y[idx]
+    b = jp.jp_back(xs, xe, ys, G.n, G.origin, G.voxsize)
+    assert_back(b, oracle.back(hxs, hxe, ys[idx].cpu().numpy(), G.n, G.origin, G.voxsize))
+    del ys, b
+    # adjointness of the full-size pair with the dense y
+    bd = jp.jp_back(xs, xe, y, G.n, G.origin, G.voxsize)
+    assert adj_gap(p, y, imgd, bd) <= ADJ_GAP
+    # the sensitivity image of configs[4] is this operator applied to ones: sum(A^T 1) = sum(A 1)
+    ones_img = torch.ones_like(imgd)
+    p1 = jp.jp_fwd(xs, xe, ones_img, G.origin, G.voxsize)
+    sens = jp.jp_back(xs, xe, torch.ones_like(y), G.n, G.origin, G.voxsize)
+    gap = abs(float(p1.double().sum()) - float(sens.double().sum())) / float(p1.double().sum())
+    assert gap <= ADJ_GAP
+
+
+def test_config2_full_tof_sino(cuda_device, phantom_dev):
+    ph, imgd = phantom_dev
+    xs, xe = inputs.sinogram_lors(views=inputs.SUBSET_VIEWS, device=cuda_device)
+    n = xs.shape[1]
+    assert n == 9_474_048
+    # view 64 is the 5th view of the subset (tie view), view 192 the 13th
+    extra = [_track(4, 0)[::9], _track(12, 30)[::9], _track(0, 64)[::9]]
+    idx = _sample(n, 12_000, 2, extra).to(cuda_device)
+    hxs, hxe = xs[:, idx].cpu().numpy(), xe[:, idx].cpu().numpy()
+    tof = _tof()
+    p = jp.jp_fwd_tof_sino(xs, xe, imgd, G.origin, G.voxsize, tof)
+    assert p.shape == (n, 29)
+    ref = oracle.fwd_tof_sino(hxs, hxe, ph, G.origin, G.voxsize, *TOF_ARGS)
+    assert_fwd(p[idx], ref)
+    # T1 at full size: bins sum to erf(3/sqrt2) x non-TOF for every LOR (phantom radius 150 mm < 205 mm)
+    pn = jp.jp_fwd(xs, xe, imgd, G.origin, G.voxsize)
+    assert torch.allclose(p.sum(1), 0.99730020393674 * pn, rtol=3e-5, atol=2e-3)
+    y = inputs.uniform_values((n, 29), 0.0, 1.0, seed=inputs.BASE_SEED + 102, device=cuda_device)
+    ys = torch.zeros_like(y)
+    ys[idx] = y[idx]
+    b = jp.jp_back_tof_sino(xs, xe, ys, G.n, G.origin, G.voxsize, tof)
+    assert_back(b, oracle.back_tof_sino(hxs, hxe, ys[idx].cpu().numpy(), G.n, G.origin, G.voxsize, *TOF_ARGS))
+    bd = jp.jp_back_tof_sino(xs, xe, y, G.n, G.origin, G.voxsize, tof)
+    assert adj_gap(p, y, imgd, bd) <= ADJ_GAP
+
+
+@pytest.fixture(scope="module")
+def events_full(cuda_device):
+    xs, xe, tb = inputs.listmode_events(40_000_000, device=cuda_device, img=inputs.phantom())
+    return xs, xe, tb
+
+
+def test_config3_full_tof_lm(cuda_device, phantom_dev, events_full):
+    ph, imgd = phantom_dev
+    xs, xe, tb = events_full
+    n = xs.shape[1]
+    assert n == 40_000_000 and tb.dtype == torch.int16
+    idx = _sample(n, 120_000, 3).to(cuda_device)
+    hxs, hxe, htb = xs[:, idx].cpu().numpy(), xe[:, idx].cpu().numpy(), tb[idx].cpu().numpy()
+    tof = _tof()
+    ref = oracle.fwd_tof_lm(hxs, hxe, htb, ph, G.origin, G.voxsize, *TOF_ARGS[:3])
+    y = inputs.uniform_values(n, 0.5, 2.0, seed=inputs.BASE_SEED + 103, device=cuda_device)
+    ys = torch.zeros_like(y)
+    ys[idx] = y[idx]
+    bref = oracle.back_tof_lm(hxs, hxe, htb, ys[idx].cpu().numpy(), G.n, G.origin, G.voxsize, *TOF_ARGS[:3])
+    # unplanned calls (acquisition order)
+    p = jp.jp_fwd_tof_lm(xs, xe, tb, imgd, G.origin, G.voxsize, tof)
+    assert_fwd(p[idx], ref)
+    assert_back(jp.jp_back_tof_lm(xs, xe, tb, ys, G.n, G.origin, G.voxsize, tof), bref)
+    # planned calls (sorted events, the configuration bench.py times), results in caller order
+    plan = jp.LmPlan(xs, xe, tb, G.n, G.origin, G.voxsize, tof, n_subsets=20)
+    assert [plan.subset_count(m) for m in range(20)] == [2_000_000] * 20 and plan.subset_count(-1) == n
+    pp = jp.jp_fwd_tof_lm_planned(plan, imgd)
+    assert_fwd(pp[idx], ref)
+    assert_back(jp.jp_back_tof_lm_planned(plan, ys), bref)
+    bd = jp.jp_back_tof_lm_planned(plan, y)
+    assert adj_gap(pp, y, imgd, bd) <= ADJ_GAP
+    plan.destroy()
+
+
+def test_config4_osem_full_image(cuda_device, phantom_dev, events_full):
+    """configs[4] geometry (200x200x96 image, 20 subsets, 3 iterations, sens = non-TOF A^T 1 over all 151.6 M
+    configs[1] LORs) on the first JP_OSEM_EVENTS events (default 4 M; 40000000 = the full config, about
+    ten minutes of oracle time on 16 cores) against the float64 oracle OSEM."""
+    ph, imgd = phantom_dev
+    nev = int(os.environ.get("JP_OSEM_EVENTS", "4000000"))
+    xs, xe, tb = (t[..., :nev].contiguous() for t in events_full)
+    sx, se = inputs.sinogram_lors(device=cuda_device)
+    sens = jp.jp_back(sx, se, torch.ones(sx.shape[1], device=cuda_device), G.n, G.origin, G.voxsize)
+    del sx, se
+    tof = _tof()
+    x = torch.ones(G.n, device=cuda_device)
+    plan = jp.LmPlan(xs, xe, tb, G.n, G.origin, G.voxsize, tof, n_subsets=20)
+    jp.jp_lm_osem_planned(plan, sens, x, n_iter=3)
+    x2 = torch.ones(G.n, device=cuda_device)
+    jp.jp_lm_osem(xs, xe, tb, sens, x2, G.origin, G.voxsize, tof, n_subsets=20, n_iter=3)
+    sens32 = sens.cpu().numpy()
+    ref = oracle.lm_osem(xs.cpu().numpy(), xe.cpu().numpy(), tb.cpu().numpy(), sens32.astype(np.float64),
+                         np.ones(G.n, dtype=np.float32), G.origin, G.voxsize, *TOF_ARGS[:3], n_subsets=20, n_iter=3)
+    for got in (x, x2):
+        g = got.cpu().numpy().astype(np.float64)
+        assert np.isfinite(g).all()
+        rel = np.linalg.norm(g - ref) / np.linalg.norm(ref)
+        mx = np.abs(g - ref).max() / np.abs(ref).max()
+        assert rel <= 1e-4, f"OSEM rel-L2 {rel:.3e}"
+        assert mx <= 1e-3, f"OSEM max abs / max {mx:.3e}"
+    plan.destroy()
