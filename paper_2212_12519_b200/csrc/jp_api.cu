@@ -377,19 +377,76 @@ int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset)
     return rg.count;
 }
 
+// ---- planned calls: quad image, axis by axis (jp_quad.cu) --------------------------------------------------------
+namespace {
+
+struct PlanCtx {
+    jp::LmPlan *lm;
+    jp::Lors l;
+    const int16_t *tb;
+    jp::Range all;          // the whole sorted list (perm set)
+    int ns;
+    jp::Geom g;
+    jp::Tof t;
+    explicit PlanCtx(const jp_plan *plan) : lm(plan->lm)
+    {
+        jp::lm_plan_view(lm, -1, false, &l, &tb, &all);
+        ns = jp::lm_plan_subsets(lm);
+        g = jp::lm_plan_geom(lm);
+        t = jp::lm_plan_tof(lm);
+    }
+    // run of (subset m, axis a); compact: per-event arrays indexed from the start of subset m
+    jp::Range seg(int m, int a, bool compact) const
+    {
+        int64_t first, count, sfirst, dummy;
+        jp::lm_plan_segment(lm, m, a, &first, &count);
+        jp::lm_plan_segment(lm, m, 0, &sfirst, &dummy);
+        jp::Range rg{first, 1, count, compact, compact ? nullptr : all.perm};
+        rg.io_off = first - sfirst;
+        return rg;
+    }
+    bool has_axis2(int subset) const
+    {
+        for (int m = 0; m < ns; ++m)
+            if (subset < 0 || m == subset) {
+                int64_t f, c;
+                jp::lm_plan_segment(lm, m, 2, &f, &c);
+                if (c) return true;
+            }
+        return false;
+    }
+};
+
+} // namespace
+
 int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream)
 {
     g_err[0] = 0;
     if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
     if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
-    jp::Lors l;
-    const int16_t *tb;
-    jp::Range rg;
-    jp::lm_plan_view(plan->lm, subset, false, &l, &tb, &rg);
-    if (rg.count == 0) return JP_OK;
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
     if (!img || !p) return fail(JP_ERR_POINTER, "img or p is NULL");
-    return lm_fwd(l, tb, rg, img, jp::lm_plan_geom(plan->lm), jp::lm_plan_tof(plan->lm), p, (cudaStream_t)stream,
-                  "jp_fwd_tof_lm_planned");
+    const char *where = "jp_fwd_tof_lm_planned";
+    cudaStream_t st = (cudaStream_t)stream;
+    PlanCtx c(plan);
+    TofCtx tc;
+    tc.st = st;
+    JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
+    float4 *q[2];
+    JP_CUDA(jp::lm_plan_quad(c.lm, 0, &q[0]), where);
+    JP_CUDA(jp::lm_plan_quad(c.lm, 1, &q[1]), where);
+    JP_CUDA(jp::launch_quad_build(img, c.g, q[0], q[1], st), where);
+    for (int a = 0; a < 2; ++a)
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), q[a], c.g, c.t, tc.lut, p, 0, st), where);
+    if (c.has_axis2(subset)) { // principal axis z: per-LOR kernels on the padded scalar image
+        JP_CUDA(jp::padded_create(img, c.g, false, st, &tc.pimg), where);
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_CUDA(jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, false), tc.pimg, c.g, c.t, tc.lut, p, 0, st), where);
+    }
+    return JP_OK;
 }
 
 int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream)
@@ -397,14 +454,32 @@ int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, floa
     g_err[0] = 0;
     if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
     if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
-    jp::Lors l;
-    const int16_t *tb;
-    jp::Range rg;
-    jp::lm_plan_view(plan->lm, subset, false, &l, &tb, &rg);
-    if (rg.count == 0) return JP_OK;
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
     if (!img || !y) return fail(JP_ERR_POINTER, "img or y is NULL");
-    return lm_back(l, tb, rg, y, jp::lm_plan_geom(plan->lm), jp::lm_plan_tof(plan->lm), img, (cudaStream_t)stream,
-                   "jp_back_tof_lm_planned");
+    const char *where = "jp_back_tof_lm_planned";
+    cudaStream_t st = (cudaStream_t)stream;
+    PlanCtx c(plan);
+    TofCtx tc;
+    tc.st = st;
+    JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
+    float4 *b[2];
+    const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+    for (int a = 0; a < 2; ++a) {
+        JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
+        JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), y, c.g, c.t, tc.lut, b[a], st), where);
+    }
+    JP_CUDA(jp::launch_quad_merge(b[0], b[1], c.g, img, st), where);
+    if (c.has_axis2(subset)) {
+        JP_CUDA(jp::padded_create(nullptr, c.g, true, st, &tc.pimg), where);
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_CUDA(jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, false), y, c.g, c.t, tc.lut, tc.pimg, st), where);
+        JP_CUDA(jp::padded_add_to(tc.pimg, c.g, img, st), where);
+    }
+    return JP_OK;
 }
 
 size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan)
@@ -425,18 +500,48 @@ int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n
     if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
     if (!sens || !img || !workspace) return fail(JP_ERR_POINTER, "NULL argument");
     if (workspace_bytes < jp_lm_osem_planned_workspace_bytes(plan)) return fail(JP_ERR_SIZE, "workspace too small");
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    const char *where = "jp_lm_osem_planned";
     cudaStream_t st = (cudaStream_t)stream;
-    const jp::Geom &g = jp::lm_plan_geom(plan->lm);
-    const jp::Tof &t = jp::lm_plan_tof(plan->lm);
-    const int ns = jp::lm_plan_subsets(plan->lm);
-    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
-    float *b = (float *)workspace;
-    float *r = b + ((nvox + 31) / 32) * 32;
-    (void)b;
-    auto view = [&](int m, jp::Lors *lo, const int16_t **tb, jp::Range *rg) {
-        jp::lm_plan_view(plan->lm, m, true, lo, tb, rg); // r is indexed in sorted order: no permutation
-    };
-    JP_TRY(lm_osem_loop(view, ns, n_iter, g, t, sens, img, r, st, "jp_lm_osem_planned"));
+    PlanCtx c(plan);
+    const int64_t nvox = (int64_t)c.g.n[0] * c.g.n[1] * c.g.n[2];
+    float *bz = (float *)workspace;              // image-sized accumulator of the principal-axis-z events
+    float *r = bz + ((nvox + 31) / 32) * 32;     // per-event ratios of one subset, in sorted order
+    TofCtx tc;
+    tc.st = st;
+    JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
+    float4 *q[2], *b[2];
+    const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+    for (int a = 0; a < 2; ++a) {
+        JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
+        JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
+    }
+    const bool z_events = c.has_axis2(-1);
+    if (z_events) JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
+    // per subset: fwd (ratio fused) and back axis by axis on the quad arrays, then the multiplicative update
+    for (int it = 0; it < n_iter; ++it) {
+        for (int m = 0; m < c.ns; ++m) {
+            JP_CUDA(jp::launch_quad_build(img, c.g, q[0], q[1], st), where);
+            for (int a = 0; a < 2; ++a)
+                JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, r, 1, st), where);
+            for (int a = 0; a < 2; ++a) {
+                JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
+                JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st), where);
+            }
+            if (z_events) {
+                float *px = nullptr, *pb = nullptr;
+                JP_CUDA(jp::padded_create(img, c.g, false, st, &px), where);
+                cudaError_t e = jp::padded_create(nullptr, c.g, true, st, &pb);
+                if (e == cudaSuccess) e = jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, true), px, c.g, c.t, tc.lut, r, 1, st);
+                if (e == cudaSuccess) e = jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, true), r, c.g, c.t, tc.lut, pb, st);
+                if (e == cudaSuccess) e = jp::padded_add_to(pb, c.g, bz, st);
+                jp::padded_destroy(px, st);
+                jp::padded_destroy(pb, st);
+                JP_CUDA(e, where);
+            }
+            JP_CUDA(jp::launch_quad_osem_update(img, b[0], b[1], z_events ? bz : nullptr, sens, (float)c.ns, c.g, st), where);
+        }
+    }
     return JP_OK;
 }
 

@@ -17,6 +17,7 @@ struct Range {
     int64_t first, stride, count;
     bool compact;
     const int *perm = nullptr; // if set (and not compact): per-LOR inputs/outputs are indexed by perm[j]
+    int64_t io_off = 0;        // compact: per-LOR inputs/outputs are indexed by c + io_off
 };
 
 cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_t st);
@@ -56,6 +57,17 @@ void padded_destroy(float *p, cudaStream_t st);
 cudaError_t launch_osem_update_padded(float *x, float *px, float *pb, const float *sens, float scale, const Geom &g,
                                       cudaStream_t st);
 
+// quad image / accumulators and the TOF listmode kernels on them (jp_quad.cu); q0: q1 = axis 1 (principal
+// axis 0), q1: q1 = axis 0 (principal axis 1); each array has padded_voxels(g) float4 elements
+cudaError_t launch_quad_build(const float *img, const Geom &g, float4 *q0, float4 *q1, cudaStream_t st);
+cudaError_t launch_quad_merge(const float4 *b0, const float4 *b1, const Geom &g, float *img, cudaStream_t st);
+cudaError_t launch_quad_osem_update(float *x, const float4 *b0, const float4 *b1, float *extra, const float *sens,
+                                    float scale, const Geom &g, cudaStream_t st);
+cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float4 *q, const Geom &g,
+                                   const Tof &t, const TofLut &lut, float *p, int lm_mode, cudaStream_t st);
+cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
+
 // listmode plan (jp_plan.cu)
 struct LmPlan;
 cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
@@ -66,6 +78,10 @@ int lm_plan_subsets(const LmPlan *pl);
 const Geom &lm_plan_geom(const LmPlan *pl);
 const Tof &lm_plan_tof(const LmPlan *pl);
 void lm_plan_view(const LmPlan *pl, int m, bool compact, Lors *l, const int16_t **tb, Range *rg);
+// events of subset m with principal axis a (a contiguous run of the sorted list): first index and count
+void lm_plan_segment(const LmPlan *pl, int m, int a, int64_t *first, int64_t *count);
+// persistent quad scratch of the plan (allocated on first use): which = 0,1: Q0,Q1; 2,3: B0,B1
+cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
 
 // x = sens > 0 ? x * b * scale / sens : 0;  b = 0   (OSEM multiplicative update, clears b for the next subset)
 cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scale, int64_t nvox, cudaStream_t st);

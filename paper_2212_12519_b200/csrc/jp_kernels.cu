@@ -14,7 +14,7 @@ constexpr int kLmBlock = 256;
 __device__ __forceinline__ int64_t lor_index(const Range &rg, int64_t c) { return rg.first + c * rg.stride; }
 __device__ __forceinline__ int64_t io_index(const Range &rg, int64_t c)
 {
-    if (rg.compact) return c;
+    if (rg.compact) return c + rg.io_off;
     const int64_t j = lor_index(rg, c);
     return rg.perm ? (int64_t)rg.perm[j] : j;
 }

@@ -19,15 +19,21 @@
 // gather and all projections are this library's kernels.
 #include <cub/device/device_radix_sort.cuh>
 
+#include <vector>
+
 #include "jp_internal.h"
 
 namespace jp {
 
 __global__ void k_lm_keys(Lors l, const int16_t *__restrict__ tofbin, int64_t n, Geom g, Tof t, int n_subsets,
-                          unsigned long long *__restrict__ keys, int *__restrict__ idx)
+                          unsigned long long *__restrict__ keys, int *__restrict__ idx, int *__restrict__ counts)
 {
+    // events per (subset, principal axis): block-level counters, then one global atomic per non-empty counter
+    extern __shared__ int cnt_sm[]; // [n_subsets][4]
+    for (int i = threadIdx.x; i < n_subsets * 4; i += blockDim.x) cnt_sm[i] = 0;
+    __syncthreads();
     const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (j >= n) return;
+    if (j < n) {
     const float s[3] = {l.xs[j], l.ys[j], l.zs[j]};
     const float e[3] = {l.xe[j], l.ye[j], l.ze[j]};
     const double d0 = (double)e[0] - (double)s[0], d1 = (double)e[1] - (double)s[1], d2 = (double)e[2] - (double)s[2];
@@ -57,6 +63,11 @@ __global__ void k_lm_keys(Lors l, const int16_t *__restrict__ tofbin, int64_t n,
     }
     keys[j] = key;
     idx[j] = (int)j;
+    atomicAdd(&cnt_sm[(int)(j % n_subsets) * 4 + p], 1);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n_subsets * 4; i += blockDim.x)
+        if (cnt_sm[i]) atomicAdd(&counts[i], cnt_sm[i]);
 }
 
 __global__ void k_lm_gather(Lors l, const int16_t *__restrict__ tofbin, const int *__restrict__ perm, int64_t n,
@@ -84,6 +95,8 @@ struct LmPlan {
     float *coord = nullptr; // 6 arrays of n floats: xs ys zs xe ye ze, sorted
     int16_t *tb = nullptr;  // sorted TOF bins
     int *perm = nullptr;    // sorted position -> caller index
+    std::vector<int64_t> seg_first, seg_count; // [n_subsets][4]: run of (subset, principal axis) in the sorted list
+    float4 *quad[4] = {nullptr, nullptr, nullptr, nullptr}; // Q0, Q1, B0, B1 (allocated on first use)
 };
 
 static int bits_for(int v)
@@ -102,10 +115,12 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
     pl->g = g;
     pl->t = t;
     *out = pl;
+    pl->seg_first.assign((size_t)n_subsets * 4, 0);
+    pl->seg_count.assign((size_t)n_subsets * 4, 0);
     if (n == 0) return cudaSuccess;
     cudaError_t e;
     unsigned long long *keys = nullptr, *keys2 = nullptr;
-    int *idx = nullptr;
+    int *idx = nullptr, *counts = nullptr;
     void *tmp = nullptr;
     size_t tmp_bytes = 0;
 #define JP_PLAN_TRY(x)                  \
@@ -119,10 +134,23 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
     JP_PLAN_TRY(cudaMallocAsync((void **)&keys, sizeof(unsigned long long) * (size_t)n, st));
     JP_PLAN_TRY(cudaMallocAsync((void **)&keys2, sizeof(unsigned long long) * (size_t)n, st));
     JP_PLAN_TRY(cudaMallocAsync((void **)&idx, sizeof(int) * (size_t)n, st));
+    JP_PLAN_TRY(cudaMallocAsync((void **)&counts, sizeof(int) * (size_t)n_subsets * 4, st));
+    JP_PLAN_TRY(cudaMemsetAsync(counts, 0, sizeof(int) * (size_t)n_subsets * 4, st));
     {
         const unsigned grid = (unsigned)((n + 255) / 256);
-        k_lm_keys<<<grid, 256, 0, st>>>(l, tofbin, n, g, t, n_subsets, keys, idx);
+        k_lm_keys<<<grid, 256, sizeof(int) * (size_t)n_subsets * 4, st>>>(l, tofbin, n, g, t, n_subsets, keys, idx, counts);
         JP_PLAN_TRY(cudaGetLastError());
+        {   // the sorted list is ordered by (subset, axis, ...): turn the counts into runs (host, synchronises)
+            std::vector<int> h((size_t)n_subsets * 4);
+            JP_PLAN_TRY(cudaMemcpyAsync(h.data(), counts, sizeof(int) * h.size(), cudaMemcpyDeviceToHost, st));
+            JP_PLAN_TRY(cudaStreamSynchronize(st));
+            int64_t at = 0;
+            for (size_t i = 0; i < h.size(); ++i) {
+                pl->seg_first[i] = at;
+                pl->seg_count[i] = h[i];
+                at += h[i];
+            }
+        }
         const int end_bit = 36 + bits_for(n_subsets);
         JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
         JP_PLAN_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
@@ -133,12 +161,14 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
         JP_PLAN_TRY(cudaGetLastError());
     }
     cudaFreeAsync(tmp, st);
+    cudaFreeAsync(counts, st);
     cudaFreeAsync(idx, st);
     cudaFreeAsync(keys2, st);
     cudaFreeAsync(keys, st);
     return cudaSuccess;
 fail:
     if (tmp) cudaFreeAsync(tmp, st);
+    if (counts) cudaFreeAsync(counts, st);
     if (idx) cudaFreeAsync(idx, st);
     if (keys2) cudaFreeAsync(keys2, st);
     if (keys) cudaFreeAsync(keys, st);
@@ -154,7 +184,24 @@ void lm_plan_destroy(LmPlan *pl)
     cudaFree(pl->coord);
     cudaFree(pl->tb);
     cudaFree(pl->perm);
+    for (float4 *q : pl->quad) cudaFree(q);
     delete pl;
+}
+
+void lm_plan_segment(const LmPlan *pl, int m, int a, int64_t *first, int64_t *count)
+{
+    *first = pl->seg_first[(size_t)m * 4 + a];
+    *count = pl->seg_count[(size_t)m * 4 + a];
+}
+
+cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out)
+{
+    if (!pl->quad[which]) {
+        cudaError_t e = cudaMalloc((void **)&pl->quad[which], sizeof(float4) * (size_t)padded_voxels(pl->g));
+        if (e != cudaSuccess) return e;
+    }
+    *out = pl->quad[which];
+    return cudaSuccess;
 }
 
 int64_t lm_plan_n(const LmPlan *pl) { return pl->n; }
