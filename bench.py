@@ -385,8 +385,8 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
     kf, kb = w.kinds
-    names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_fwd_tof_sino", "k_back_tof_sino"),
-             3: ("k_fwd_tof_lm", "k_back_tof_lm"), 4: ("k_fwd_tof_lm + k_back_tof_lm", "")}[w.c]
+    names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
+             3: ("k_fwd_tof_lm_quad", "k_back_tof_lm_quad"), 4: ("k_fwd_tof_lm_quad + k_back_tof_lm_quad", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
     if w.c == 4:
         lane = 2 * LANE["lm"]

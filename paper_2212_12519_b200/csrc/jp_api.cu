@@ -232,7 +232,10 @@ int jp_fwd_tof_sino(const jp_lors *lors, const float *img, const jp_geom *geom, 
     cudaStream_t st = (cudaStream_t)stream;
     TofCtx c;
     JP_TRY(tof_ctx_init(c, t, g, img, 0, st, "jp_fwd_tof_sino (scratch)"));
-    JP_CUDA(jp::launch_fwd_tof_sino(l, whole(lors->n), c.pimg, g, t, c.lut, p, st), "jp_fwd_tof_sino");
+    cudaError_t e = jp::launch_tof_sino_win(false, l, lors->n, c.pimg, nullptr, g, t, p, nullptr, st);
+    if (e == cudaErrorNotSupported) // TOF window wider than the compiled register windows: generic kernel
+        e = jp::launch_fwd_tof_sino(l, whole(lors->n), c.pimg, g, t, c.lut, p, st);
+    JP_CUDA(e, "jp_fwd_tof_sino");
     return JP_OK;
 }
 
@@ -251,7 +254,10 @@ int jp_back_tof_sino(const jp_lors *lors, const float *y, const jp_geom *geom, c
     cudaStream_t st = (cudaStream_t)stream;
     TofCtx c;
     JP_TRY(tof_ctx_init(c, t, g, nullptr, 1, st, "jp_back_tof_sino (scratch)"));
-    JP_CUDA(jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, c.lut, c.pimg, st), "jp_back_tof_sino");
+    cudaError_t e = jp::launch_tof_sino_win(true, l, lors->n, nullptr, c.pimg, g, t, nullptr, y, st);
+    if (e == cudaErrorNotSupported)
+        e = jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, c.lut, c.pimg, st);
+    JP_CUDA(e, "jp_back_tof_sino");
     JP_CUDA(jp::padded_add_to(c.pimg, g, img, st), "jp_back_tof_sino (unpad)");
     return JP_OK;
 }

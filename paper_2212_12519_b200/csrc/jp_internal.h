@@ -43,6 +43,10 @@ cudaError_t launch_fwd_tof_sino(const Lors &l, Range rg, const float *img, const
 cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const Geom &g, const Tof &t,
                                  const TofLut &lut, float *img, cudaStream_t st);
 
+// sliding-window TOF sinogram kernels (jp_tof_sino.cu); cudaErrorNotSupported: window wider than compiled
+cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g,
+                                const Tof &t, float *p, const float *y, cudaStream_t st);
+
 // lm_mode: 0 = p = A x;  1 = p = (A x > 1e-9) ? 1/(A x) : 0   (OSEM ratio fused into the epilogue)
 cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *img, const Geom &g,
                               const Tof &t, const TofLut &lut, float *p, int lm_mode, cudaStream_t st);

@@ -1,0 +1,308 @@
+// jp_tof_sino.cu -- TOF sinogram forward / back projection with a sliding register window of TOF bins:
+// the kernels behind jp_fwd_tof_sino / jp_back_tof_sino.
+//
+// in sinogram mode every plane step contributes to ALL TOF bins along the ray; PAPER.md:35,
+// :78: the weight of a bin is the Gaussian integrated over the bin (difference of two error functions),
+// truncated at n_sigmas.  In bin coordinates s = tau / W + (n_tofbins - 1) / 2 (bin k centred at s = k) the
+// weight of bin k is G(k - s),
+//
+//     G(x) = 1/2 [E((x + 1/2) W) - E((x - 1/2) W)],   E(y) = erf(clamp(y, -m, m) / (sigma sqrt2)),
+//
+// with support |x| < R = m / W + 1/2: at most ceil(2R) consecutive bins starting at base = ceil(s - R).
+// Two facts shape the kernels:
+//   * with phi = base - (s - R) in [0, 1), the arguments of ALL bins of the window are n + phi - R: one row
+//     of a table T[phi][n] = G(n + phi - R) (512 rows, (value, slope) pairs, built in float64) gives every
+//     weight of the step with NBW/2 128-bit shared-memory loads and NBW FMAs -- instead of one edge-function
+//     look-up per bin edge;
+//   * s is monotone along the ray (the planes are walked in the direction of increasing tau), so base never
+//     decreases: the NBW bins of the window are accumulated in REGISTERS and a bin is written (forward) /
+//     its y value read (back) exactly once, when the window slides past it.
+// Persistent CTAs (one table copy per CTA) loop over blocks of 256 consecutive LORs; the block's
+// [256][n_tofbins] tile is staged through shared memory so that global reads / writes are coalesced, and
+// blocks whose LORs all miss the image skip the walk (forward: zero fill; back: y is not even read).
+// Images are the zero-padded copies of jp_pad.cu (PRay).
+#include "jp_internal.h"
+
+namespace jp {
+
+namespace {
+
+constexpr int kSBlock = 256;
+constexpr int kSLd = kSBlock + 1;
+constexpr int kGK = 512; // table rows per unit of phi
+#ifndef JP_SINO_MINB
+#define JP_SINO_MINB 4
+#endif
+
+__global__ void k_tof_gtab(float2 *tab, int nbw, double R, double W, double m, double isc)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (kGK + 2) * nbw) return;
+    const int r = e / nbw, n = e - r * nbw;
+    auto E = [&](double y) { return erf(fmin(fmax(y, -m), m) * isc); };
+    auto G = [&](double x) { return 0.5 * (E((x + 0.5) * W) - E((x - 0.5) * W)); };
+    const double x0 = (double)n + (double)r / (double)kGK - R;
+    const double g0 = G(x0), g1 = G(x0 + 1.0 / (double)kGK);
+    tab[e] = make_float2((float)g0, (float)(g1 - g0));
+}
+
+struct GTab {
+    const float2 *tab; // device, (kGK + 2) rows of NBW (value, slope) pairs
+    float cbR;         // (n_tofbins - 1) / 2 - R
+    float inv_w;       // 1 / W
+};
+
+template <int OFF>
+__device__ __forceinline__ float4 lds_quad(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                 : "r"(addr), "n"(OFF)
+                 : "memory");
+    return v;
+}
+
+// weights of the NBW window bins from one table row: w[n] = T[n] + f D[n]
+template <int NBW, int N>
+__device__ __forceinline__ void load_weights(uint32_t row, float f, float (&w)[NBW])
+{
+    if constexpr (N < NBW) {
+        const float4 v = lds_quad<N * 8>(row);
+        w[N] = fmaf(f, v.y, v.x);
+        w[N + 1] = fmaf(f, v.w, v.z);
+        load_weights<NBW, N + 2>(row, f, w);
+    }
+}
+
+// the walk of one LOR; FWD: a[] accumulates value x weight per window bin, flushed into acc (shared, [bin][kSLd]);
+// BACK: yv[] holds the y values of the window bins (from ysm), the step's sum is scattered with atomic adds
+// S2ONE: the q2 axis is the contiguous image axis (principal axis x or y), neighbours along q2 are 4 bytes apart
+template <int NBW, bool BACK, bool S2ONE>
+__device__ __forceinline__ void walk(const PRay &q, const GTab &gt, uint32_t tab_addr, float *__restrict__ stage,
+                                     int nbins, const float *__restrict__ pimg_r, float *__restrict__ pimg_w)
+{
+    const int tid = threadIdx.x;
+    const float ds = q.dtau * gt.inv_w;
+    const float sR0 = fmaf(q.tau0, gt.inv_w, gt.cbR);
+    // walk in the direction of increasing s
+    float fk = 0.f, dfk = 1.f;
+    int po = q.off, dpo = q.sp;
+    if (ds < 0.f) {
+        fk = (float)(q.nk - 1);
+        dfk = -1.f;
+        po = q.off + (q.nk - 1) * q.sp;
+        dpo = -q.sp;
+    }
+    float sR = fmaf(ds, fk, sR0);
+    float basef = __fadd_ru(sR, kMagic) - kMagic; // ceil(s - R)
+    int base = (int)basef;
+    float a[NBW];
+#pragma unroll
+    for (int n = 0; n < NBW; ++n) {
+        if (BACK)
+            a[n] = ((unsigned)(base + n) < (unsigned)nbins) ? stage[(base + n) * kSLd + tid] : 0.f;
+        else
+            a[n] = 0.f;
+    }
+    const int s2 = S2ONE ? 1 : q.s2;
+    PCell cl = pray_cell(q, fk, po);
+    for (int it = 0; it < q.nk; ++it) {
+        sR = fmaf(ds, fk, sR0);
+        const float cur = __fadd_ru(sR, kMagic) - kMagic;
+#pragma unroll 1
+        while (cur > basef) { // slide the window by one bin (false for NaN)
+            if (BACK) {
+#pragma unroll
+                for (int n = 0; n + 1 < NBW; ++n) a[n] = a[n + 1];
+                a[NBW - 1] = ((unsigned)(base + NBW) < (unsigned)nbins) ? stage[(base + NBW) * kSLd + tid] : 0.f;
+            } else {
+                if ((unsigned)base < (unsigned)nbins) stage[base * kSLd + tid] = q.cf * a[0];
+#pragma unroll
+                for (int n = 0; n + 1 < NBW; ++n) a[n] = a[n + 1];
+                a[NBW - 1] = 0.f;
+            }
+            basef += 1.f;
+            ++base;
+        }
+        const float tk = (cur - sR) * (float)kGK;
+        const float tt = __fadd_rd(tk, kMagic);
+        const float f = tk - (tt - kMagic);
+        const uint32_t row = tab_addr + __float_as_uint(tt) * (uint32_t)(NBW * 8);
+        float w[NBW];
+        load_weights<NBW, 0>(row, f, w);
+        fk += dfk;
+        po += dpo;
+        if (BACK) {
+            float s = 0.f;
+#pragma unroll
+            for (int n = 0; n < NBW; ++n) s = fmaf(a[n], w[n], s);
+            if (s != 0.f) {
+                const float x = q.cf * s;
+                float *p0 = pimg_w + cl.off, *p1 = p0 + q.s1;
+                const float xa = x * (1.f - cl.w1), xb = x * cl.w1, m2 = 1.f - cl.w2;
+                atomicAdd(p0, xa * m2);
+                atomicAdd(p0 + s2, xa * cl.w2);
+                atomicAdd(p1, xb * m2);
+                atomicAdd(p1 + s2, xb * cl.w2);
+            }
+            cl = pray_cell(q, fk, po);
+        } else {
+            const float *p0 = pimg_r + cl.off, *p1 = p0 + q.s1;
+            const float v00 = __ldg(p0), v01 = __ldg(p0 + s2), v10 = __ldg(p1), v11 = __ldg(p1 + s2);
+            const float lo = fmaf(cl.w2, v01 - v00, v00), hi = fmaf(cl.w2, v11 - v10, v10);
+            const float val = fmaf(cl.w1, hi - lo, lo);
+#pragma unroll
+            for (int n = 0; n < NBW; ++n) a[n] = fmaf(val, w[n], a[n]);
+            cl = pray_cell(q, fk, po);
+        }
+    }
+    if (!BACK) {
+#pragma unroll
+        for (int n = 0; n < NBW; ++n)
+            if ((unsigned)(base + n) < (unsigned)nbins) stage[(base + n) * kSLd + tid] = q.cf * a[n];
+    }
+}
+
+template <int NBW, bool BACK>
+__global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
+    k_tof_sino_win(Lors l, int64_t n, int64_t nblocks, const float *__restrict__ pimg_r, float *__restrict__ pimg_w,
+                   Geom g, Tof t, GTab gt, float *__restrict__ p, const float *__restrict__ y)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *tab = reinterpret_cast<float2 *>(smem_raw);                                       // [(kGK + 2)][NBW]
+    float *stage = reinterpret_cast<float *>(smem_raw + (size_t)(kGK + 2) * NBW * sizeof(float2)); // [nbins][kSLd]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nbins = t.nbins;
+    for (int i = tid; i < (kGK + 2) * NBW; i += kSBlock) tab[i] = __ldg(gt.tab + i);
+    if (!BACK)
+        for (int i = tid; i < nbins * kSLd; i += kSBlock) stage[i] = 0.f;
+    const uint32_t tab_addr = smem_addr(tab) - (uint32_t)kMagicI * (uint32_t)(NBW * 8);
+    const float lim = t.nsig * t.sigma;
+    const float reach = 0.5f * (float)(nbins - 1) * t.width + 0.5f * t.width + lim;
+    __syncthreads();
+
+    for (int64_t blk = blockIdx.x; blk < nblocks; blk += gridDim.x) {
+        const int64_t j0 = blk * kSBlock, j = j0 + tid;
+        const int nvalid = (int)min((int64_t)kSBlock, n - j0);
+        PRay q;
+        q.nk = 0;
+        if (j < n) {
+            Ray r;
+            ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
+            q = pray_from(r, g);
+        }
+        const bool any = __syncthreads_or(q.nk > 0) != 0;
+        if (!any) {
+            if (!BACK) { // the whole block misses the image: zeros
+                float *out = p + j0 * nbins;
+                const int tot = nvalid * nbins;
+                if (nvalid == kSBlock && (((uintptr_t)out) & 15) == 0) {
+                    float4 *o4 = reinterpret_cast<float4 *>(out);
+                    for (int x = tid; x < tot / 4; x += kSBlock) o4[x] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int x = (tot & ~3) + tid; x < tot; x += kSBlock) out[x] = 0.f;
+                } else {
+                    for (int x = tid; x < tot; x += kSBlock) out[x] = 0.f;
+                }
+            }
+            continue;
+        }
+        if (BACK) { // stage y[j0 .. j0 + nvalid)[nbins]: one warp per LOR, lanes along the bins
+            const float *in = y + j0 * nbins;
+            for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
+                for (int kb = lane; kb < nbins; kb += 32) stage[kb * kSLd + lor] = in[lor * nbins + kb];
+            __syncthreads();
+        }
+        if (q.nk > 0) {
+            if (q.s2 == 1)
+                walk<NBW, BACK, true>(q, gt, tab_addr, stage, nbins, pimg_r, pimg_w);
+            else
+                walk<NBW, BACK, false>(q, gt, tab_addr, stage, nbins, pimg_r, pimg_w);
+        }
+        __syncthreads();
+        if (!BACK) { // write the tile (and clear it for the next block)
+            float *out = p + j0 * nbins;
+            for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
+                for (int kb = lane; kb < nbins; kb += 32) {
+                    out[lor * nbins + kb] = stage[kb * kSLd + lor];
+                    stage[kb * kSLd + lor] = 0.f;
+                }
+            __syncthreads();
+        }
+    }
+}
+
+int window_bins(const Tof &t, double *R_out)
+{
+    const double m = (double)t.nsig * (double)t.sigma;
+    const double R = m / (double)t.width + 0.5;
+    *R_out = R;
+    const int nb = (int)ceil(2.0 * R);
+    const int sizes[] = {4, 6, 8, 12};
+    for (int s : sizes)
+        if (nb <= s) return s;
+    return 0;
+}
+
+size_t win_smem(int nbw, int nbins) { return (size_t)(kGK + 2) * nbw * sizeof(float2) + (size_t)nbins * kSLd * sizeof(float); }
+
+template <int NBW, bool BACK>
+cudaError_t launch_win(const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g, const Tof &t,
+                       const GTab &gt, float *p, const float *y, cudaStream_t st)
+{
+    const size_t smem = win_smem(NBW, t.nbins);
+    auto kern = k_tof_sino_win<NBW, BACK>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int dev = 0, nsm = 0, per_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kSBlock, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorInvalidConfiguration;
+    const int64_t nblocks = (n + kSBlock - 1) / kSBlock;
+    const int64_t cap = (int64_t)nsm * per_sm;
+    const unsigned grid = (unsigned)(nblocks < cap ? nblocks : cap);
+    kern<<<grid, kSBlock, smem, st>>>(l, n, nblocks, pimg_r, pimg_w, g, t, gt, p, y);
+    return cudaGetLastError();
+}
+
+} // namespace
+
+// returns cudaErrorNotSupported when the TOF window is wider than the compiled sizes or the tile does not fit
+// in shared memory (the caller then uses the generic kernels of jp_kernels.cu)
+cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g,
+                                const Tof &t, float *p, const float *y, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    double R;
+    const int nbw = window_bins(t, &R);
+    if (!nbw || win_smem(nbw, t.nbins) > 72 * 1024) return cudaErrorNotSupported;
+    float2 *tab = nullptr;
+    const int ne = (kGK + 2) * nbw;
+    cudaError_t e = cudaMallocAsync((void **)&tab, sizeof(float2) * ne, st);
+    if (e != cudaSuccess) return e;
+    const double m = (double)t.nsig * (double)t.sigma;
+    k_tof_gtab<<<(ne + 255) / 256, 256, 0, st>>>(tab, nbw, R, (double)t.width, m, 1.0 / ((double)t.sigma * 1.4142135623730951));
+    e = cudaGetLastError();
+    GTab gt{tab, (float)(0.5 * (double)(t.nbins - 1) - R), 1.f / t.width};
+    if (e == cudaSuccess) {
+#define JP_WIN(NB)                                                                                           \
+    case NB:                                                                                                 \
+        e = back ? launch_win<NB, true>(l, n, pimg_r, pimg_w, g, t, gt, p, y, st)                             \
+                 : launch_win<NB, false>(l, n, pimg_r, pimg_w, g, t, gt, p, y, st);                           \
+        break;
+        switch (nbw) {
+            JP_WIN(4)
+            JP_WIN(6)
+            JP_WIN(8)
+            JP_WIN(12)
+        default: e = cudaErrorNotSupported;
+        }
+#undef JP_WIN
+    }
+    cudaFreeAsync(tab, st);
+    return e;
+}
+
+} // namespace jp

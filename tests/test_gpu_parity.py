@@ -99,6 +99,28 @@ def test_config0_tof(cuda_device):
     assert adj_gap(pl, dev(yl, cuda_device), img, bl) <= ADJ_GAP
 
 
+@pytest.mark.parametrize("width,nbins,coff", [(20.0, 13, 0.0), (9.0, 27, 2.5), (6.0, 41, 0.0), (4.0, 61, -1.0),
+                                              (2.5, 63, 0.0)])
+def test_tof_sino_window_sizes(cuda_device, width, nbins, coff):
+    """TOF sinogram kernels for every compiled register-window size (4, 6, 8, 12 bins) and the generic fallback
+    (window of 18 bins), with a centre offset, all three principal axes and a ragged tail"""
+    c = inputs.config0(n_lors=6_007)
+    g = c["geom"]
+    sigma, nsig = 7.0, 3.0
+    tof = jp.make_tof(width, sigma, nsig, nbins, coff)
+    xs, xe = dev(c["xstart"], cuda_device), dev(c["xend"], cuda_device)
+    img = dev(c["img"], cuda_device)
+    p = jp.jp_fwd_tof_sino(xs, xe, img, g.origin, g.voxsize, tof)
+    ref = oracle.fwd_tof_sino(c["xstart"], c["xend"], c["img"], g.origin, g.voxsize, width, sigma, nsig, nbins,
+                              center_offset=coff)
+    assert_fwd(p, ref)
+    y = np.random.default_rng(int(width * 10)).uniform(-0.5, 1, (6_007, nbins)).astype(np.float32)
+    b = jp.jp_back_tof_sino(xs, xe, dev(y, cuda_device), g.n, g.origin, g.voxsize, tof)
+    assert_back(b, oracle.back_tof_sino(c["xstart"], c["xend"], y, g.n, g.origin, g.voxsize, width, sigma, nsig, nbins,
+                                        center_offset=coff))
+    assert adj_gap(p, dev(y, cuda_device), img, b) <= ADJ_GAP
+
+
 # ---- slices of configs 1-3 on the scanner geometry (several tiles + ragged tail) ----------------------
 @pytest.fixture(scope="module")
 def scanner():
