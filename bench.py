@@ -238,7 +238,8 @@ class Workload:
             self.plane_steps = jp.jp_plane_steps_tof_lm(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            self.plan = jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof, n_subsets=20)
+            self.plan = jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof,
+                                  n_subsets=1 if c == 3 else 20)   # configs[3] has no subsets: one sorted list
             torch.cuda.synchronize()
             self.plan_s = time.perf_counter() - t0
             self.kinds = ("lm", "lm")
@@ -246,7 +247,7 @@ class Workload:
             if c == 3:
                 self.y = inputs.uniform_values(self.n, 0.5, 2.0, seed=inputs.BASE_SEED + 103 + rank, device=dev)
                 self.p = torch.empty(self.n, dtype=torch.float32, device=dev)
-                self.launches = 2 + 3        # + pad / zero-fill of the padded accumulator / unpad-add
+                self.launches = 2 * 2 + 2    # fwd + back line-tile kernels per principal axis (x, y) + their TOF tables
             else:
                 self.sens = torch.ones(G.n, dtype=torch.float32, device=dev)   # replaced by A^T 1 in setup_sens()
                 self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
@@ -386,7 +387,7 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
     kf, kb = w.kinds
     names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
-             3: ("k_fwd_tof_lm_quad", "k_back_tof_lm_quad"), 4: ("k_fwd_tof_lm_quad + k_back_tof_lm_quad", "")}[w.c]
+             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_fwd_tof_lm_quad + k_back_tof_lm_quad", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
     if w.c == 4:
         lane = 2 * LANE["lm"]

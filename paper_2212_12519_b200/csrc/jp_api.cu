@@ -1,6 +1,7 @@
 // jp_api.cu -- the extern "C" boundary of libjoseph_b200.so (see include/joseph_b200.h).
 // Argument validation, error text, and dispatch to the kernel launchers; no arithmetic here.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "../../include/joseph_b200.h"
@@ -386,6 +387,17 @@ int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset)
 // ---- planned calls: quad image, axis by axis (jp_quad.cu) --------------------------------------------------------
 namespace {
 
+// line tiles (jp_lm_tile.cu) pay when the sorted events come in long runs on one transaxial line (crystal-snapped
+// events, all subsets together: ~2500 per run for configs[3]); short runs (one OSEM subset of 20: ~120) are
+// faster on the quad image.  JP_LM_TILE=0/1 overrides the rule (debugging, tests).
+bool lm_tiles_wanted(const jp::LmPlan *lm)
+{
+    const char *e = getenv("JP_LM_TILE");
+    if (e && (e[0] == '0' || e[0] == '1')) return e[0] == '1';
+    const int64_t runs = jp::lm_plan_runs(lm);
+    return runs > 0 && jp::lm_plan_n(lm) / runs >= 512;
+}
+
 struct PlanCtx {
     jp::LmPlan *lm;
     jp::Lors l;
@@ -441,11 +453,17 @@ int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, flo
     float4 *q[2];
     JP_CUDA(jp::lm_plan_quad(c.lm, 0, &q[0]), where);
     JP_CUDA(jp::lm_plan_quad(c.lm, 1, &q[1]), where);
-    JP_CUDA(jp::launch_quad_build(img, c.g, q[0], q[1], st), where);
+    const bool tiles = lm_tiles_wanted(c.lm);
+    if (!tiles) JP_CUDA(jp::launch_quad_build(img, c.g, q[0], q[1], st), where);
     for (int a = 0; a < 2; ++a)
         for (int m = 0; m < c.ns; ++m)
-            if (subset < 0 || m == subset)
-                JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), q[a], c.g, c.t, tc.lut, p, 0, st), where);
+            if (subset < 0 || m == subset) {
+                const jp::Range rg = c.seg(m, a, false);
+                if (tiles)
+                    JP_CUDA(jp::launch_fwd_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, img, c.g, c.t, p, 0, st), where);
+                else
+                    JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, rg, q[a], c.g, c.t, tc.lut, p, 0, st), where);
+            }
     if (c.has_axis2(subset)) { // principal axis z: per-LOR kernels on the padded scalar image
         JP_CUDA(jp::padded_create(img, c.g, false, st, &tc.pimg), where);
         for (int m = 0; m < c.ns; ++m)
@@ -468,16 +486,25 @@ int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, floa
     TofCtx tc;
     tc.st = st;
     JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
-    float4 *b[2];
-    const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
-    for (int a = 0; a < 2; ++a) {
-        JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
-        JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
-        for (int m = 0; m < c.ns; ++m)
-            if (subset < 0 || m == subset)
-                JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), y, c.g, c.t, tc.lut, b[a], st), where);
+    if (lm_tiles_wanted(c.lm)) {
+        for (int a = 0; a < 2; ++a)
+            for (int m = 0; m < c.ns; ++m)
+                if (subset < 0 || m == subset) {
+                    const jp::Range rg = c.seg(m, a, false);
+                    JP_CUDA(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, y, c.g, c.t, img, st), where);
+                }
+    } else {
+        float4 *b[2];
+        const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+        for (int a = 0; a < 2; ++a) {
+            JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
+            JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
+            for (int m = 0; m < c.ns; ++m)
+                if (subset < 0 || m == subset)
+                    JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), y, c.g, c.t, tc.lut, b[a], st), where);
+        }
+        JP_CUDA(jp::launch_quad_merge(b[0], b[1], c.g, img, st), where);
     }
-    JP_CUDA(jp::launch_quad_merge(b[0], b[1], c.g, img, st), where);
     if (c.has_axis2(subset)) {
         JP_CUDA(jp::padded_create(nullptr, c.g, true, st, &tc.pimg), where);
         for (int m = 0; m < c.ns; ++m)

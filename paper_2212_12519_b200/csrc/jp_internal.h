@@ -72,12 +72,23 @@ cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range r
 cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
                                     const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
 
+// TOF listmode on line tiles (jp_lm_tile.cu): events [first, first + count) of a SORTED list; outputs / inputs at
+// perm[e] (perm != null) or io_off + e - first; cudaErrorNotSupported: image too wide for the tiled kernels
+cudaError_t launch_fwd_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t first, int64_t count, const int *perm,
+                                   int64_t io_off, const float *img, const Geom &g, const Tof &t, float *p, int lm_mode,
+                                   cudaStream_t st);
+
+cudaError_t launch_back_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t first, int64_t count, const int *perm,
+                                    int64_t io_off, const float *y, const Geom &g, const Tof &t, float *img,
+                                    cudaStream_t st);
+
 // listmode plan (jp_plan.cu)
 struct LmPlan;
 cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
                            int n_subsets, cudaStream_t st, LmPlan **out);
 void lm_plan_destroy(LmPlan *pl);
 int64_t lm_plan_n(const LmPlan *pl);
+int64_t lm_plan_runs(const LmPlan *pl); // runs of sorted events sharing their transaxial line
 int lm_plan_subsets(const LmPlan *pl);
 const Geom &lm_plan_geom(const LmPlan *pl);
 const Tof &lm_plan_tof(const LmPlan *pl);

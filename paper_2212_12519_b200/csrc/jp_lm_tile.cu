@@ -1,0 +1,725 @@
+// jp_lm_tile.cu -- TOF listmode forward / back projection on LINE TILES: the planned listmode calls over a
+// sorted event list whose runs of events share their transaxial line.
+//
+// A ring scanner snaps events to crystal centres, so after the plan's sort (jp_plan.cu) thousands of events
+// of configs[3] share the same transaxial projection (same crystal pair, any ring pair, any TOF bin, either
+// orientation).  For such a run the q1 half of Joseph's bilinear interpolation is common to
+// all its events, exactly as for the ring pairs of one sinogram bin (jp_tile.cu):
+//
+//   forward   C[i][z] = (1-w1(i)) f[i,k1(i),z] + w1(i) f[i,k1(i)+1,z]   rows built once per run in shared memory;
+//             p_e     = cf_e sum_{i in TOF window of e} G_e(i) lerp_z(C[i][.], u2_e(i))
+//   adjoint   C[i][z] += cf_e y_e G_e(i) hat(u2_e(i) - z)  (fixed-point shared atomics), then each row is
+//             spread over its two image rows with 128-bit REDs: one global atomic per (plane, 4 voxels) of the
+//             run instead of one per event and plane (north_star: shared-memory tile staging)
+//
+// G_e(i) is the TOF weight of the event's own bin, from a float64-built table of
+// G(x) = 1/2 [E((x + 1/2) W) - E((x - 1/2) W)] over x = |c - tau| / W (reading A10).
+// A CTA takes 768 consecutive sorted events, finds the runs inside them (bit-exact comparison of the
+// canonically ordered transaxial end points) and processes run after run; an event given as (e, s) instead of
+// (s, e) is walked in the canonical orientation with its axial end points swapped and its TOF centre negated
+// (the kernel is even).  Runs shorter than kMinRun, and events whose principal axis is z, take the per-LOR path.
+#include "jp_tile_common.cuh"
+
+namespace jp {
+
+using namespace tile;
+
+namespace {
+
+#ifndef JP_LMT_MINB
+#define JP_LMT_MINB 4
+#endif
+constexpr int kG1K = 512;   // table intervals per TOF bin width
+constexpr int kMinRun = 48; // shorter runs are not worth a row build
+
+__global__ void k_tof_g1tab(float2 *tab, int n, double W, double m, double isc)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    auto E = [&](double y) { return erf(fmin(fmax(y, -m), m) * isc); };
+    auto G = [&](double x) { return 0.5 * (E((x + 0.5) * W) - E((x - 0.5) * W)); };
+    const double g0 = G((double)k / kG1K), g1 = G((double)(k + 1) / kG1K);
+    tab[k] = make_float2((float)g0, (float)(g1 - g0));
+}
+
+struct G1Tab {
+    const float2 *tab; // device, n entries; entry k = (G(k / kG1K), G((k+1) / kG1K) - G(k / kG1K)); zero beyond R
+    int n;
+    float scale; // kG1K / W: mm -> table units
+    float xmax;  // n - 1.5
+};
+
+// canonical orientation of the transaxial end points: start = the lexicographically smaller (x, y)
+__device__ __forceinline__ bool is_swapped(float xs, float ys, float xe, float ye)
+{
+    return !((xs < xe) || (xs == xe && ys <= ye));
+}
+
+// weight of the event's bin at table position xs (table units, any sign)
+__device__ __forceinline__ float g1_weight(uint32_t gbase, float xmax, float xs)
+{
+    const float xa = fminf(fabsf(xs), xmax);
+    const float tt = __fadd_rd(xa, kMagic);
+    const float f = xa - (tt - kMagic);
+    const float2 v = lds_pair<0>(gbase + (__float_as_uint(tt) << 3));
+    return fmaf(f, v.y, v.x);
+}
+
+// per-event axial + TOF part on track t (canonical orientation)
+struct LmRay {
+    int i0, i1;     // planes inside the image along z AND inside the TOF window of the event's bin
+    float a2, b2;   // u2(i) = a2 + b2 (i - i0)
+    float cf;
+    float x0, dx;   // table position of plane i: x0 + dx (i - i0)
+};
+
+struct LineExtra {
+    double Rd;      // 1 + (d_q1 / d_p)^2
+};
+
+__device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double Rd, float zs, float ze, float centre,
+                                          float reach, float scale)
+{
+    LmRay z;
+    const double dz = (double)ze - (double)zs;
+    const double rz = dz * t.inv_dp;
+    const double vp = (double)g.v[t.p];
+    const double iv2 = drcp((double)g.v[2]);
+    const double B = rz * vp * iv2;
+    const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2;
+    const double Ln = dsqrt_pos(Rd + rz * rz);   // L / |d_p|
+    z.cf = (float)(vp * Ln);
+    // tau(i) = ((ops + i vp) inv_dp - 1/2) L,  L = Ln / |inv_dp|
+    const double L = Ln * fabs(drcp(t.inv_dp));
+    const double dtau = vp * t.inv_dp * L;
+    const double tau_at0 = (t.ops * t.inv_dp - 0.5) * L;
+    int ilo = t.I0, ihi = t.I1;
+    {   // TOF window: |tau(i) - centre| <= reach, rounded outwards
+        const double ivt = drcp(dtau);
+        const double ia = ((double)centre - (double)reach - tau_at0) * ivt, ib = ((double)centre + (double)reach - tau_at0) * ivt;
+        const double np = (double)g.n[t.p];
+        const double imin = fmin(fmax(floor(fmin(ia, ib)), -1.0), np), imax = fmin(fmax(ceil(fmax(ia, ib)), -1.0), np);
+        ilo = max(ilo, (int)imin);
+        ihi = min(ihi, (int)imax);
+    }
+    const float Af = (float)A, Bf = (float)B, n2 = (float)g.n[2];
+    if (Bf == 0.f) {
+        if (Af <= -1.f || Af >= n2) ihi = ilo - 1;
+    } else {
+        const float inv = 1.f / Bf;
+        const float ia = (-1.f - Af) * inv, ib = (n2 - Af) * inv;
+        const float imin = fminf(fmaxf(floorf(fminf(ia, ib)) - 1.f, -1.f), (float)g.n[t.p]);
+        const float imax = fminf(fmaxf(ceilf(fmaxf(ia, ib)) + 1.f, -1.f), (float)g.n[t.p]);
+        ilo = max(ilo, (int)imin);
+        ihi = min(ihi, (int)imax);
+    }
+    z.b2 = Bf;
+    z.a2 = (float)(A + B * (double)ilo);
+    const float umin = -1.9f, umax = n2 + 0.9f;
+    while (ilo <= ihi) {
+        if (z.a2 > umin && z.a2 < umax) break;
+        ++ilo;
+        z.a2 = (float)(A + B * (double)ilo);
+    }
+    while (ilo <= ihi) {
+        const float u = fmaf(z.b2, (float)(ihi - ilo), z.a2);
+        if (u > umin && u < umax) break;
+        --ihi;
+    }
+    z.i0 = ilo;
+    z.i1 = ihi;
+    z.x0 = (float)(((double)centre - (tau_at0 + dtau * (double)ilo)) * (double)scale);
+    z.dx = (float)(-dtau * (double)scale);
+    return z;
+}
+
+// per-LOR path (short runs, principal axis z): same arithmetic as jp_kernels.cu on the unpadded image
+__device__ __forceinline__ float generic_fwd_lm(const Lors &l, int64_t j, float centre, float reach, const Geom &g,
+                                                const Tof &t, const float *__restrict__ img, uint32_t gbase,
+                                                const G1Tab &gt)
+{
+    Ray r;
+    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    float acc = 0.f;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+        acc = fmaf(plane_value(img, r, k, cl), g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale), acc);
+    }
+    return r.cf * acc;
+}
+
+__device__ __forceinline__ void generic_back_lm(const Lors &l, int64_t j, float centre, float reach, float y, const Geom &g,
+                                                const Tof &t, float *__restrict__ img, uint32_t gbase, const G1Tab &gt)
+{
+    Ray r;
+    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    const float x = r.cf * y;
+    if (r.nk == 0 || x == 0.f) return;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        const float tau = fmaf(r.dtau, (float)k, r.tau0);
+        const float w = g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale);
+        if (w != 0.f) plane_scatter(img, r, k, cl, x * w);
+    }
+}
+
+// shared bookkeeping of a CTA
+struct TileState {
+    Track trk;
+    LineExtra ex;
+    int nruns;
+    int imin, imax;
+    unsigned short starts[kTile + 1];
+};
+
+// runs of events with identical canonical transaxial end points among the CTA's nev events; canon = smem scratch
+// of kTile uint4 (may alias the row buffer).  All threads; ends with a barrier.
+__device__ __forceinline__ void find_runs(TileState &S, uint4 *canon, const uint4 (&mine)[kPerThread], int nev)
+{
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) canon[m * kThreads + tid] = mine[m];
+    __syncthreads();
+    if (tid < 32) {
+        int n = 0;
+        for (int b0 = 0; b0 < nev; b0 += 32) {
+            const int pos = b0 + tid;
+            bool flag = false;
+            if (pos < nev) {
+                if (pos == 0) {
+                    flag = true;
+                } else {
+                    const uint4 a = canon[pos], b = canon[pos - 1];
+                    flag = (a.x != b.x) | (a.y != b.y) | (a.z != b.z) | (a.w != b.w);
+                }
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, flag);
+            if (flag) S.starts[n + __popc(bal & ((1u << tid) - 1u))] = (unsigned short)pos;
+            n += __popc(bal);
+        }
+        if (tid == 0) {
+            S.starts[n] = (unsigned short)nev;
+            S.nruns = n;
+        }
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ int64_t out_index(const int *__restrict__ perm, int64_t io_off, int64_t first, int64_t e)
+{
+    return perm ? (int64_t)perm[e] : (e - first) + io_off;
+}
+
+} // namespace
+
+// ---- forward ------------------------------------------------------------------------------------------------
+#define JP_LM_FWD_STEP(K, A2K, X0K)                                             \
+    {                                                                           \
+        const float u = fmaf(b2, fk, A2K);                                      \
+        const float tt = __fadd_rd(u, kMagic);                                  \
+        const float w = u - (tt - kMagic);                                      \
+        const float2 v = lds_pair<(K) * P * 8>(row + (__float_as_uint(tt) << 3)); \
+        const float wt = g1_weight(gbase, xmax, fmaf(dx, fk, X0K));             \
+        acc = fmaf(fmaf(w, v.y, v.x), wt, acc);                                 \
+    }
+
+template <int P, int LM_MODE>
+__global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
+    k_fwd_tof_lm_tile(Lors l, const int16_t *__restrict__ tofbin, int64_t first, int64_t count,
+                      const int *__restrict__ perm, int64_t io_off, const float *__restrict__ img, Geom g, Tof t,
+                      G1Tab gt, int rows_cap, int vec_ok, float *__restrict__ p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                             // [rows_cap][P]
+    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(float2)); // [max(n0,n1)]
+    const int np = max(g.n[0], g.n[1]);
+    float2 *g1 = reinterpret_cast<float2 *>(rinfo + np);                                           // [gt.n]
+    __shared__ TileState S;
+    const int tid = threadIdx.x;
+    const int64_t c0 = first + blockIdx.x * (int64_t)kTile;
+    const int nev = (int)min((int64_t)kTile, first + count - c0);
+    const float reach = 0.5f * t.width + t.nsig * t.sigma;
+
+    for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
+    const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
+    const float xmax = gt.xmax;
+
+    // ---- canonical transaxial end points of the CTA's events -> runs
+    {
+        uint4 canon[kPerThread];
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            const int pos = m * kThreads + tid;
+            canon[m] = make_uint4(0xffffffffu, pos, 0, 0); // invalid slots never match
+            if (pos < nev) {
+                const int64_t e = c0 + pos;
+                float xs = l.xs[e], ys = l.ys[e], xe = l.xe[e], ye = l.ye[e];
+                const double dx = (double)xe - (double)xs, dy = (double)ye - (double)ys;
+                const double dz = (double)l.ze[e] - (double)l.zs[e];
+                if (is_swapped(xs, ys, xe, ye)) {
+                    float tmp = xs; xs = xe; xe = tmp;
+                    tmp = ys; ys = ye; ye = tmp;
+                }
+                canon[m] = (principal_axis(dx, dy, dz) != 2)
+                               ? make_uint4(__float_as_uint(xs), __float_as_uint(ys), __float_as_uint(xe), __float_as_uint(ye))
+                               : make_uint4(0xffffffffu, pos, 1, 0); // principal axis z: a run of one
+            }
+        }
+        find_runs(S, reinterpret_cast<uint4 *>(C2), canon, nev);
+    }
+    const int nruns = S.nruns;
+    // constant zero columns of the shared rows (after the scratch use of C2)
+    {
+        const int ncl = kPad - 1, ncr = P - (g.n[2] + kPad);
+        for (int e = tid; e < rows_cap * (ncl + ncr); e += kThreads) {
+            const int r = e / (ncl + ncr), c = e - r * (ncl + ncr);
+            C2[r * P + (c < ncl ? c : g.n[2] + kPad + (c - ncl))] = make_float2(0.f, 0.f);
+        }
+    }
+    const uint32_t c2_base = smem_addr(C2) + kPad * 8u - ((uint32_t)kMagicI << 3);
+    const int n2 = g.n[2];
+
+    for (int k = 0; k < nruns; ++k) {
+        const int ra = S.starts[k], rb = S.starts[k + 1];
+        bool active[kPerThread]; // the run's events are dealt to the threads: event ra + m kThreads + tid
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) active[m] = ra + m * kThreads + tid < rb;
+        if (rb - ra < kMinRun) { // per-LOR path (also every event whose principal axis is z: runs of one)
+#pragma unroll 1
+            for (int m = 0; m < kPerThread; ++m)
+                if (active[m]) {
+                    const int64_t e = c0 + ra + m * kThreads + tid;
+                    const float c = (float)tofbin[e] * t.width;
+                    float out = generic_fwd_lm(l, e, c, reach, g, t, img, gbase, gt);
+                    if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
+                    p[out_index(perm, io_off, first, e)] = out;
+                }
+            continue;
+        }
+        // ---- the run's track (thread owning its first event)
+        if (tid == 0) {
+                const int64_t e = c0 + ra;
+                float xs = l.xs[e], ys = l.ys[e], xe = l.xe[e], ye = l.ye[e];
+                if (is_swapped(xs, ys, xe, ye)) {
+                    float tmp = xs; xs = xe; xe = tmp;
+                    tmp = ys; ys = ye; ye = tmp;
+                }
+                track_setup(g, xs, ys, xe, ye, S.trk);
+                const double dxy[2] = {(double)xe - (double)xs, (double)ye - (double)ys};
+                const double ratio = dxy[1 - S.trk.p] * S.trk.inv_dp;
+                S.ex.Rd = 1.0 + ratio * ratio;
+                S.imin = 0x7fffffff;
+                S.imax = -1;
+            }
+        __syncthreads();
+        const Track trk = S.trk;
+        LmRay zr[kPerThread];
+        float acc_[kPerThread];
+        if (trk.I1 >= trk.I0) {
+            const double Rd = S.ex.Rd;
+            int lo = 0x7fffffff, hi = -1;
+#pragma unroll
+            for (int m = 0; m < kPerThread; ++m) {
+                acc_[m] = 0.f;
+                zr[m].i0 = 0;
+                zr[m].i1 = -1;
+                if (active[m]) {
+                    const int64_t e = c0 + ra + m * kThreads + tid;
+                    float zs = l.zs[e], ze = l.ze[e];
+                    float centre = fmaf((float)tofbin[e], t.width, t.coff); // bin centre on the canonical tau axis
+                    if (is_swapped(l.xs[e], l.ys[e], l.xe[e], l.ye[e])) {   // (e, s): walk it as (s, e), mirrored
+                        const float tmp = zs; zs = ze; ze = tmp;
+                        centre = -centre;
+                    }
+                    zr[m] = lm_setup(g, trk, Rd, zs, ze, centre, reach, gt.scale);
+                    if (zr[m].i1 >= zr[m].i0) {
+                        lo = min(lo, zr[m].i0);
+                        hi = max(hi, zr[m].i1);
+                    }
+                }
+            }
+            if (hi >= lo) {
+                atomicMin(&S.imin, lo);
+                atomicMax(&S.imax, hi);
+            }
+            for (int r = tid; r <= trk.I1 - trk.I0; r += kThreads) rinfo[r] = row_info(g, trk, trk.I0 + r);
+        }
+        __syncthreads();
+        if (trk.I1 >= trk.I0) {
+            const int I0 = S.imin, I1 = S.imax;
+            for (int cc = I0; cc <= I1; cc += rows_cap) {
+                const int rows = min(rows_cap, I1 - cc + 1);
+                build_rows<P>(C2, rinfo, img, trk, cc, rows, n2, vec_ok);
+                __syncthreads();
+#pragma unroll
+                for (int m = 0; m < kPerThread; ++m) {
+                    const int ib = max(zr[m].i0, cc), ie = min(zr[m].i1, cc + rows - 1);
+                    if (ib > ie) continue;
+                    const int nst = ie - ib + 1;
+                    const float b2 = zr[m].b2, a2_0 = zr[m].a2, dx = zr[m].dx, x0_0 = zr[m].x0;
+                    const float a2_1 = fmaf(b2, 1.f, a2_0), x0_1 = fmaf(dx, 1.f, x0_0);
+                    float fk = (float)(ib - zr[m].i0);
+                    uint32_t row = c2_base + (uint32_t)((ib - cc) * P) * 8u;
+                    float acc = acc_[m];
+#pragma unroll 1
+                    for (int it = nst >> 1; it > 0; --it) {
+                        JP_LM_FWD_STEP(0, a2_0, x0_0)
+                        JP_LM_FWD_STEP(1, a2_1, x0_1)
+                        fk += 2.f;
+                        row += 2u * P * 8u;
+                    }
+                    if (nst & 1) JP_LM_FWD_STEP(0, a2_0, x0_0)
+                    acc_[m] = acc;
+                }
+                __syncthreads();
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m)
+            if (active[m]) {
+                float out = (trk.I1 >= trk.I0) ? zr[m].cf * acc_[m] : 0.f;
+                if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
+                p[out_index(perm, io_off, first, c0 + ra + m * kThreads + tid)] = out;
+            }
+        __syncthreads(); // S.trk is rewritten by the next run
+    }
+}
+#undef JP_LM_FWD_STEP
+
+// ---- back ------------------------------------------------------------------------------------------------------
+// Fixed-point staging as in jp_tile.cu (native int32 shared atomics; scale from max |cf y| over the run: the TOF
+// weight is <= 1, a bin receives at most two contributions per event and plane, a run has at most kTile events).
+template <int OFF>
+__device__ __forceinline__ void reds_add_lm(uint32_t addr, int q)
+{
+    asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(q) : "memory");
+}
+
+#define JP_LM_BACK_STEP(K, A2K, X0K)                                            \
+    {                                                                           \
+        const float u = fmaf(b2, fk, A2K);                                      \
+        const float tt = __fadd_rd(u, kMagic);                                  \
+        const float w = u - (tt - kMagic);                                      \
+        const uint32_t a = row + (__float_as_uint(tt) << 2);                    \
+        const float xw = xm * g1_weight(gbase, xmax, fmaf(dx, fk, X0K));        \
+        const int qxw = __float_as_int(xw + kMagic);                            \
+        const int bits = __float_as_int(fmaf(xw, w, kMagic));                   \
+        reds_add_lm<(K) * P * 4>(a, qxw - bits);                                \
+        reds_add_lm<(K) * P * 4 + 4>(a, bits - kMagicI);                        \
+    }
+
+template <int P>
+__global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
+    k_back_tof_lm_tile(Lors l, const int16_t *__restrict__ tofbin, int64_t first, int64_t count,
+                       const int *__restrict__ perm, int64_t io_off, const float *__restrict__ y, Geom g, Tof t,
+                       G1Tab gt, int rows_cap, int vec_ok, float *__restrict__ img)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int *Ci = reinterpret_cast<int *>(smem_raw);                                                 // [rows_cap][P]
+    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(int)); // [max(n0,n1)]
+    const int np = max(g.n[0], g.n[1]);
+    float2 *g1 = reinterpret_cast<float2 *>(rinfo + np);                                         // [gt.n]
+    __shared__ TileState S;
+    __shared__ float red[kThreads / 32];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int64_t c0 = first + blockIdx.x * (int64_t)kTile;
+    const int nev = (int)min((int64_t)kTile, first + count - c0);
+    const float reach = 0.5f * t.width + t.nsig * t.sigma;
+
+    for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
+    const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
+    const float xmax = gt.xmax;
+    {
+        uint4 canon[kPerThread];
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            const int pos = m * kThreads + tid;
+            canon[m] = make_uint4(0xffffffffu, pos, 0, 0);
+            if (pos < nev) {
+                const int64_t e = c0 + pos;
+                float xs = l.xs[e], ys = l.ys[e], xe = l.xe[e], ye = l.ye[e];
+                const double dx = (double)xe - (double)xs, dy = (double)ye - (double)ys;
+                const double dz = (double)l.ze[e] - (double)l.zs[e];
+                if (is_swapped(xs, ys, xe, ye)) {
+                    float tmp = xs; xs = xe; xe = tmp;
+                    tmp = ys; ys = ye; ye = tmp;
+                }
+                canon[m] = (principal_axis(dx, dy, dz) != 2)
+                               ? make_uint4(__float_as_uint(xs), __float_as_uint(ys), __float_as_uint(xe), __float_as_uint(ye))
+                               : make_uint4(0xffffffffu, pos, 1, 0);
+            }
+        }
+        find_runs(S, reinterpret_cast<uint4 *>(Ci), canon, nev);
+    }
+    const int nruns = S.nruns;
+    {
+        int4 *z4 = reinterpret_cast<int4 *>(Ci);
+        for (int e = tid; e < rows_cap * (P / 4); e += kThreads) z4[e] = make_int4(0, 0, 0, 0);
+    }
+    const uint32_t ci_base = smem_addr(Ci) + kPad * 4u - ((uint32_t)kMagicI << 2);
+    const int n2 = g.n[2];
+    __syncthreads();
+
+    for (int k = 0; k < nruns; ++k) {
+        const int ra = S.starts[k], rb = S.starts[k + 1];
+        bool active[kPerThread];
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) active[m] = ra + m * kThreads + tid < rb;
+        if (rb - ra < kMinRun) {
+#pragma unroll 1
+            for (int m = 0; m < kPerThread; ++m)
+                if (active[m]) {
+                    const int64_t e = c0 + ra + m * kThreads + tid;
+                    const float yv = y[out_index(perm, io_off, first, e)];
+                    if (yv != 0.f) generic_back_lm(l, e, (float)tofbin[e] * t.width, reach, yv, g, t, img, gbase, gt);
+                }
+            continue;
+        }
+        if (tid == 0) {
+            const int64_t e = c0 + ra;
+            float xs = l.xs[e], ys = l.ys[e], xe = l.xe[e], ye = l.ye[e];
+            if (is_swapped(xs, ys, xe, ye)) {
+                float tmp = xs; xs = xe; xe = tmp;
+                tmp = ys; ys = ye; ye = tmp;
+            }
+            track_setup(g, xs, ys, xe, ye, S.trk);
+            const double dxy[2] = {(double)xe - (double)xs, (double)ye - (double)ys};
+            const double ratio = dxy[1 - S.trk.p] * S.trk.inv_dp;
+            S.ex.Rd = 1.0 + ratio * ratio;
+            S.imin = 0x7fffffff;
+            S.imax = -1;
+        }
+        __syncthreads();
+        const Track trk = S.trk;
+        if (trk.I1 < trk.I0) {
+            __syncthreads();
+            continue;
+        }
+        LmRay zr[kPerThread];
+        float x[kPerThread];
+        float xm_ = 0.f;
+        {
+            const double Rd = S.ex.Rd;
+            int lo = 0x7fffffff, hi = -1;
+#pragma unroll
+            for (int m = 0; m < kPerThread; ++m) {
+                x[m] = 0.f;
+                zr[m].i0 = 0;
+                zr[m].i1 = -1;
+                if (active[m]) {
+                    const int64_t e = c0 + ra + m * kThreads + tid;
+                    float zs = l.zs[e], ze = l.ze[e];
+                    float centre = fmaf((float)tofbin[e], t.width, t.coff);
+                    if (is_swapped(l.xs[e], l.ys[e], l.xe[e], l.ye[e])) {
+                        const float tmp = zs; zs = ze; ze = tmp;
+                        centre = -centre;
+                    }
+                    zr[m] = lm_setup(g, trk, Rd, zs, ze, centre, reach, gt.scale);
+                    x[m] = zr[m].cf * y[out_index(perm, io_off, first, e)];
+                    if (zr[m].i1 >= zr[m].i0 && x[m] != 0.f) {
+                        lo = min(lo, zr[m].i0);
+                        hi = max(hi, zr[m].i1);
+                        xm_ = fmaxf(xm_, fabsf(x[m]));
+                    } else {
+                        zr[m].i1 = zr[m].i0 - 1;
+                    }
+                }
+            }
+            if (hi >= lo) {
+                atomicMin(&S.imin, lo);
+                atomicMax(&S.imax, hi);
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) xm_ = fmaxf(xm_, __shfl_xor_sync(0xffffffffu, xm_, o));
+        if (lane == 0) red[warp] = xm_;
+        for (int r = tid; r <= trk.I1 - trk.I0; r += kThreads) rinfo[r] = row_info(g, trk, trk.I0 + r);
+        __syncthreads();
+        xm_ = red[0];
+#pragma unroll
+        for (int w = 1; w < kThreads / 32; ++w) xm_ = fmaxf(xm_, red[w]);
+        const int I0 = S.imin, I1 = S.imax;
+        if (xm_ > 0.f && xm_ < 3.0e38f && I1 >= I0) {
+            const float lim = fminf(4194302.f, 2147483648.f / (float)(2 * kTile) - 1.f);
+            const float Sc = lim / xm_, invS = xm_ / lim;
+            for (int cc = I0; cc <= I1; cc += rows_cap) {
+                const int rows = min(rows_cap, I1 - cc + 1);
+#pragma unroll
+                for (int m = 0; m < kPerThread; ++m) {
+                    const int ib = max(zr[m].i0, cc), ie = min(zr[m].i1, cc + rows - 1);
+                    if (ib > ie) continue;
+                    const int nst = ie - ib + 1;
+                    const float b2 = zr[m].b2, a2_0 = zr[m].a2, dx = zr[m].dx, x0_0 = zr[m].x0, xm = x[m] * Sc;
+                    const float a2_1 = fmaf(b2, 1.f, a2_0), x0_1 = fmaf(dx, 1.f, x0_0);
+                    float fk = (float)(ib - zr[m].i0);
+                    uint32_t row = ci_base + (uint32_t)((ib - cc) * P) * 4u;
+#pragma unroll 1
+                    for (int it = nst >> 1; it > 0; --it) {
+                        JP_LM_BACK_STEP(0, a2_0, x0_0)
+                        JP_LM_BACK_STEP(1, a2_1, x0_1)
+                        fk += 2.f;
+                        row += 2u * P * 4u;
+                    }
+                    if (nst & 1) JP_LM_BACK_STEP(0, a2_0, x0_0)
+                }
+                __syncthreads();
+                // ---- flush: spread every row over its two q1 neighbours with REDs, and clear it
+                if (vec_ok) {
+                    const int G = n2 >> 2;
+                    for (int r = warp; r < rows; r += kThreads / 32) {
+                        const RowInfo ri = rinfo[cc - trk.I0 + r];
+                        const float sa = ri.wa * invS, sb = ri.wb * invS;
+                        for (int gq = lane; gq < G; gq += 32) {
+                            int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
+                            const int4 q = *src;
+                            if ((q.x | q.y | q.z | q.w) == 0) continue;
+                            *src = make_int4(0, 0, 0, 0);
+                            const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
+                            if (ri.base_a >= 0)
+                                atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq,
+                                          make_float4(sa * v.x, sa * v.y, sa * v.z, sa * v.w));
+                            if (ri.base_b >= 0)
+                                atomicAdd(reinterpret_cast<float4 *>(img + ri.base_b) + gq,
+                                          make_float4(sb * v.x, sb * v.y, sb * v.z, sb * v.w));
+                        }
+                    }
+                } else {
+                    for (int e = tid; e < rows * n2; e += kThreads) {
+                        const int r = e / n2, z = e - r * n2;
+                        const int q = Ci[r * P + kPad + z];
+                        if (q == 0) continue;
+                        Ci[r * P + kPad + z] = 0;
+                        const RowInfo ri = rinfo[cc - trk.I0 + r];
+                        const float v = (float)q * invS;
+                        if (ri.base_a >= 0) atomicAdd(img + ri.base_a + z, ri.wa * v);
+                        if (ri.base_b >= 0) atomicAdd(img + ri.base_b + z, ri.wb * v);
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        __syncthreads(); // S.trk / red are rewritten by the next run
+    }
+}
+#undef JP_LM_BACK_STEP
+
+// ---- launchers ----------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kSmemBudget = 54 * 1024;
+
+struct LmTileCfg {
+    int P, rows_cap, vec_ok, g1n;
+    size_t smem;
+};
+
+// elem: bytes per row element (8: forward pairs, 4: back fixed point)
+LmTileCfg lm_tile_cfg(const Geom &g, const Tof &t, const void *img, size_t elem)
+{
+    LmTileCfg c{};
+    const int need = g.n[2] + kPad + kPadR;
+    const int pitches[] = {40, 72, 104, 136, 200, 264};
+    for (int P : pitches)
+        if (need <= P) { c.P = P; break; }
+    if (!c.P) return c;
+    const double R = (double)t.nsig * (double)t.sigma / (double)t.width + 0.5;
+    c.g1n = (int)ceil(R * kG1K) + 3;
+    const int np = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
+    const size_t fixed = (size_t)np * sizeof(RowInfo) + (size_t)c.g1n * sizeof(float2);
+    const size_t row = (size_t)c.P * elem;
+    size_t rows = fixed + row <= kSmemBudget ? (kSmemBudget - fixed) / row : 0;
+    if (rows * row < (size_t)kTile * sizeof(uint4) || rows < 8) { c.P = 0; return c; } // also the run-detection scratch
+    if (rows > (size_t)np) rows = (size_t)np;
+    if (rows * row < (size_t)kTile * sizeof(uint4)) rows = ((size_t)kTile * sizeof(uint4) + row - 1) / row;
+    c.rows_cap = (int)rows;
+    c.smem = rows * row + fixed;
+    c.vec_ok = (g.n[2] % 4 == 0) && ((uintptr_t)img % 16 == 0);
+    return c;
+}
+
+cudaError_t g1tab_create(const Tof &t, int n, cudaStream_t st, G1Tab *out)
+{
+    float2 *tab = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&tab, sizeof(float2) * n, st);
+    if (e != cudaSuccess) return e;
+    const double m = (double)t.nsig * (double)t.sigma;
+    k_tof_g1tab<<<(n + 255) / 256, 256, 0, st>>>(tab, n, (double)t.width, m, 1.0 / ((double)t.sigma * 1.4142135623730951));
+    e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        cudaFreeAsync(tab, st);
+        return e;
+    }
+    out->tab = tab;
+    out->n = n;
+    out->scale = (float)((double)kG1K / (double)t.width);
+    out->xmax = (float)n - 1.5f;
+    return cudaSuccess;
+}
+
+} // namespace
+
+#define JP_LM_DISPATCH_P(CFG, ...)                           \
+    switch ((CFG).P) {                                       \
+    case 40: { constexpr int P = 40; __VA_ARGS__; } break;   \
+    case 72: { constexpr int P = 72; __VA_ARGS__; } break;   \
+    case 104: { constexpr int P = 104; __VA_ARGS__; } break; \
+    case 136: { constexpr int P = 136; __VA_ARGS__; } break; \
+    case 200: { constexpr int P = 200; __VA_ARGS__; } break; \
+    case 264: { constexpr int P = 264; __VA_ARGS__; } break; \
+    default: return cudaErrorNotSupported;                   \
+    }
+
+// events [first, first + count) of the sorted list l / tofbin; outputs p[perm[e]] (perm != null) or
+// p[io_off + e - first].  cudaErrorNotSupported: image too wide for the tiled kernel.
+cudaError_t launch_fwd_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t first, int64_t count, const int *perm,
+                                   int64_t io_off, const float *img, const Geom &g, const Tof &t, float *p, int lm_mode,
+                                   cudaStream_t st)
+{
+    if (count == 0) return cudaSuccess;
+    const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(float2));
+    if (!c.P) return cudaErrorNotSupported;
+    G1Tab gt;
+    cudaError_t e = g1tab_create(t, c.g1n, st, &gt);
+    if (e != cudaSuccess) return e;
+    const unsigned grid = (unsigned)((count + kTile - 1) / kTile);
+    JP_LM_DISPATCH_P(c, {
+        if (lm_mode == 1) {
+            e = cudaFuncSetAttribute(k_fwd_tof_lm_tile<P, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
+            if (e == cudaSuccess)
+                k_fwd_tof_lm_tile<P, 1><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, img, g, t, gt,
+                                                                        c.rows_cap, c.vec_ok, p);
+        } else {
+            e = cudaFuncSetAttribute(k_fwd_tof_lm_tile<P, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
+            if (e == cudaSuccess)
+                k_fwd_tof_lm_tile<P, 0><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, img, g, t, gt,
+                                                                        c.rows_cap, c.vec_ok, p);
+        }
+    })
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaFreeAsync((void *)gt.tab, st);
+    return e;
+}
+
+cudaError_t launch_back_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t first, int64_t count, const int *perm,
+                                    int64_t io_off, const float *y, const Geom &g, const Tof &t, float *img,
+                                    cudaStream_t st)
+{
+    if (count == 0) return cudaSuccess;
+    const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(int));
+    if (!c.P) return cudaErrorNotSupported;
+    G1Tab gt;
+    cudaError_t e = g1tab_create(t, c.g1n, st, &gt);
+    if (e != cudaSuccess) return e;
+    const unsigned grid = (unsigned)((count + kTile - 1) / kTile);
+    JP_LM_DISPATCH_P(c, {
+        e = cudaFuncSetAttribute(k_back_tof_lm_tile<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
+        if (e == cudaSuccess)
+            k_back_tof_lm_tile<P><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, y, g, t, gt,
+                                                                  c.rows_cap, c.vec_ok, img);
+    })
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaFreeAsync((void *)gt.tab, st);
+    return e;
+}
+
+} // namespace jp

@@ -9,8 +9,8 @@
 // windows cover the same planes.  The sort key, most significant field first:
 //
 //   subset (e mod n_subsets) | principal axis | transaxial slope d_q1/d_p (11 bits) | transaxial
-//   intercept at the image centre plane (11 bits) | plane of the TOF bin centre (6 bits) | axial
-//   position of the TOF bin centre (6 bits)
+//   intercept at the image centre plane (11 bits) | hash of the transaxial end points (20 bits) | plane of
+//   the TOF bin centre (6 bits) | axial position of the TOF bin centre (6 bits)
 //
 // It is purely geometric (no scanner model): crystal-snapped events of one crystal pair get the same
 // slope/intercept cell, continuous events get neighbours.  The plan owns a sorted SoA copy of the end
@@ -39,7 +39,7 @@ __global__ void k_lm_keys(Lors l, const int16_t *__restrict__ tofbin, int64_t n,
     const double d0 = (double)e[0] - (double)s[0], d1 = (double)e[1] - (double)s[1], d2 = (double)e[2] - (double)s[2];
     const int p = principal_axis(d0, d1, d2);
     const float d[3] = {(float)d0, (float)d1, (float)d2};
-    unsigned long long key = (unsigned long long)(j % n_subsets) << 36 | (unsigned long long)p << 34;
+    unsigned long long key = (unsigned long long)(j % n_subsets) << 56 | (unsigned long long)p << 54;
     const float L = sqrtf(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
     if (L > 0.f) {
         const int q1 = (p == 0) ? 1 : 0, q2 = (p == 2) ? 1 : 2;
@@ -58,8 +58,19 @@ __global__ void k_lm_keys(Lors l, const int16_t *__restrict__ tofbin, int64_t n,
         const float xc = s[p] + f * d[p], zc = s[q2] + f * d[q2];
         const int kp = min(63, max(0, (int)((xc - g.o[p]) / (g.v[p] * (float)g.n[p]) * 64.f)));
         const int kz = min(63, max(0, (int)((zc - g.o[q2]) / (g.v[q2] * (float)g.n[q2]) * 64.f)));
-        key |= (unsigned long long)ks << 23 | (unsigned long long)ki << 12 | (unsigned long long)kp << 6 |
-               (unsigned long long)kz;
+        // 20-bit hash of the canonically ordered transaxial end points: events of one crystal pair (either
+        // orientation) that share a slope / intercept cell with another pair still form ONE contiguous run
+        // (the line tiles of jp_lm_tile.cu need that; a hash collision only costs a tile its coherence)
+        const bool sw = !((s[0] < e[0]) || (s[0] == e[0] && s[1] <= e[1]));
+        const unsigned ax = __float_as_uint(sw ? e[0] : s[0]), ay = __float_as_uint(sw ? e[1] : s[1]);
+        const unsigned bx = __float_as_uint(sw ? s[0] : e[0]), by = __float_as_uint(sw ? s[1] : e[1]);
+        unsigned h = ax * 0x9E3779B1u;
+        h = (h ^ (h >> 15) ^ ay) * 0x85EBCA77u;
+        h = (h ^ (h >> 13) ^ bx) * 0xC2B2AE3Du;
+        h = (h ^ (h >> 16) ^ by) * 0x27D4EB2Fu;
+        h ^= h >> 15;
+        key |= (unsigned long long)ks << 43 | (unsigned long long)ki << 32 | (unsigned long long)(h & 0xFFFFFu) << 12 |
+               (unsigned long long)kp << 6 | (unsigned long long)kz;
     }
     keys[j] = key;
     idx[j] = (int)j;
@@ -87,8 +98,28 @@ __global__ void k_lm_gather(Lors l, const int16_t *__restrict__ tofbin, const in
     tb[c] = tofbin[j];
 }
 
+// number of runs of consecutive sorted events with the same (canonically ordered) transaxial end points
+__global__ void k_lm_count_runs(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ xe,
+                                const float *__restrict__ ye, int64_t n, unsigned long long *__restrict__ runs)
+{
+    const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    bool flag = false;
+    if (c < n) {
+        flag = (c == 0);
+        if (!flag) {
+            float a[4] = {xs[c], ys[c], xe[c], ye[c]}, b[4] = {xs[c - 1], ys[c - 1], xe[c - 1], ye[c - 1]};
+            if (!((a[0] < a[2]) || (a[0] == a[2] && a[1] <= a[3]))) { float t = a[0]; a[0] = a[2]; a[2] = t; t = a[1]; a[1] = a[3]; a[3] = t; }
+            if (!((b[0] < b[2]) || (b[0] == b[2] && b[1] <= b[3]))) { float t = b[0]; b[0] = b[2]; b[2] = t; t = b[1]; b[1] = b[3]; b[3] = t; }
+            flag = (a[0] != b[0]) || (a[1] != b[1]) || (a[2] != b[2]) || (a[3] != b[3]);
+        }
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, flag);
+    if ((threadIdx.x & 31) == 0 && bal) atomicAdd(runs, (unsigned long long)__popc(bal));
+}
+
 struct LmPlan {
     int64_t n = 0;
+    int64_t n_runs = 0;     // runs of events sharing their transaxial line in the sorted list
     int n_subsets = 1;
     Geom g{};
     Tof t{};
@@ -151,7 +182,7 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
                 at += h[i];
             }
         }
-        const int end_bit = 36 + bits_for(n_subsets);
+        const int end_bit = 56 + bits_for(n_subsets);
         JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
         JP_PLAN_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
         JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
@@ -159,6 +190,16 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
         k_lm_gather<<<grid, 256, 0, st>>>(l, tofbin, pl->perm, n, c, c + n, c + 2 * n, c + 3 * n, c + 4 * n, c + 5 * n,
                                            pl->tb);
         JP_PLAN_TRY(cudaGetLastError());
+        {   // run statistics of the sorted list: decides between line tiles and the quad kernels
+            unsigned long long *runs = reinterpret_cast<unsigned long long *>(keys); // scratch, keys are dead
+            unsigned long long h = 0;
+            JP_PLAN_TRY(cudaMemsetAsync(runs, 0, sizeof(unsigned long long), st));
+            k_lm_count_runs<<<grid, 256, 0, st>>>(c, c + n, c + 3 * n, c + 4 * n, n, runs);
+            JP_PLAN_TRY(cudaGetLastError());
+            JP_PLAN_TRY(cudaMemcpyAsync(&h, runs, sizeof(h), cudaMemcpyDeviceToHost, st));
+            JP_PLAN_TRY(cudaStreamSynchronize(st));
+            pl->n_runs = (int64_t)h;
+        }
     }
     cudaFreeAsync(tmp, st);
     cudaFreeAsync(counts, st);
@@ -205,6 +246,7 @@ cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out)
 }
 
 int64_t lm_plan_n(const LmPlan *pl) { return pl->n; }
+int64_t lm_plan_runs(const LmPlan *pl) { return pl->n_runs; }
 int lm_plan_subsets(const LmPlan *pl) { return pl->n_subsets; }
 const Geom &lm_plan_geom(const LmPlan *pl) { return pl->g; }
 const Tof &lm_plan_tof(const LmPlan *pl) { return pl->t; }

@@ -269,6 +269,46 @@ def test_config3_plan_sorted_events(cuda_device, scanner, events):
     plan.destroy()
 
 
+def _line_events(seed=21):
+    """events that share few transaxial lines (long runs for the line tiles): all 2304 ring pairs of 22 sinogram
+    bins, a third of them given as (e, s) instead of (s, e), random TOF bins, shuffled"""
+    xs, xe = inputs.sinogram_lors(views=[3, 64, 100, 192, 200], radial=[-30, -5, 0, 17])
+    xs2, xe2 = inputs.sinogram_lors(views=[77], radial=[-64, 31])     # grazing / partly outside
+    xs, xe = torch.cat([xs, xs2], 1), torch.cat([xe, xe2], 1)
+    n = xs.shape[1]
+    rng = np.random.default_rng(seed)
+    keep = rng.permutation(n)[: n - 101]                                # ragged
+    xs, xe = xs[:, keep].numpy().copy(), xe[:, keep].numpy().copy()
+    n = xs.shape[1]
+    swap = rng.random(n) < 0.33
+    xs[:, swap], xe[:, swap] = xe[:, swap].copy(), xs[:, swap].copy()
+    tb = rng.integers(-12, 13, n).astype(np.int16)
+    return xs, xe, tb
+
+
+@pytest.mark.parametrize("n_subsets", [1, 3])
+def test_lm_line_tiles(cuda_device, scanner, n_subsets, monkeypatch):
+    """planned TOF listmode projectors on line tiles (runs of events sharing a transaxial line) vs the oracle"""
+    monkeypatch.setenv("JP_LM_TILE", "1")
+    g, ph = scanner
+    xs, xe, tb = _line_events()
+    n = xs.shape[1]
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins, 1.5)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    xsd, xed, tbd, imgd = dev(xs, cuda_device), dev(xe, cuda_device), dev(tb, cuda_device), dev(ph, cuda_device)
+    plan = jp.LmPlan(xsd, xed, tbd, g.n, g.origin, g.voxsize, tof, n_subsets=n_subsets)
+    p = jp.jp_fwd_tof_lm_planned(plan, imgd)
+    ref = oracle.fwd_tof_lm(xs, xe, tb, ph, g.origin, g.voxsize, *args, center_offset=1.5)
+    assert (ref > 0).mean() > 0.5
+    assert_fwd(p, ref)
+    y = inputs.uniform_values(n, 0.5, 2.0, seed=14).to(cuda_device)
+    b = jp.jp_back_tof_lm_planned(plan, y)
+    assert_back(b, oracle.back_tof_lm(xs, xe, tb, y.cpu().numpy(), g.n, g.origin, g.voxsize, *args, center_offset=1.5))
+    assert adj_gap(p, y, imgd, b) <= ADJ_GAP
+    plan.destroy()
+
+
 def test_config4_small_osem_planned(cuda_device, scanner, events):
     g, ph = scanner
     xs, xe, tb = events
