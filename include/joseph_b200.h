@@ -158,6 +158,20 @@ size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan);
 int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
                        size_t workspace_bytes, void *stream);
 
+/* ---- image-based resolution model -------------------------------- */
+/* out = G in: 3-D Gaussian of standard deviation sigma_mm (mm; FWHM = 2 sqrt(2 ln 2) sigma; the paper uses
+ * 4.5 mm FWHM), taps exp(-(k v_a)^2 / (2 sigma^2)) for |k| <= ceil(n_sigmas sigma / v_a), normalised per axis,
+ * zero outside the image (so G is symmetric: the same call serves "before forward" and "after back").
+ * in / out: device, geom->n voxels, C order; in may equal out.  Asynchronous on `stream`; scratch is
+ * stream-ordered.  JP_ERR_SIZE: sigma_mm <= 0, n_sigmas <= 0 or a kernel radius > 16 voxels. */
+int jp_gauss3d(const float *in, float *out, const jp_geom *geom, float sigma_mm, float n_sigmas, void *stream);
+
+/* jp_lm_osem_planned with the resolution model in every subset (reading R3): ybar = A (G x), b = G (A^T r),
+ * x <- x b n_subsets / sens; `sens` is the caller's (it should hold G A^T 1).  Workspace as for
+ * jp_lm_osem_planned. */
+int jp_lm_osem_planned_res(const jp_plan *plan, const float *sens, float *img, int n_iter, float res_sigma_mm,
+                           float res_n_sigmas, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- hybrid mode: HOST pointers in and out ---------------------------------------- */
 /* Same semantics as jp_fwd / jp_back, but every pointer (inside lors_host too) is a HOST pointer.  The
  * LOR list is streamed through the current CUDA device in chunks on two internal streams (copies

@@ -67,6 +67,9 @@ EXPORTS = {
     "jp_lm_osem_planned_workspace_bytes": (C.c_size_t, [C.c_void_p]),
     "jp_lm_osem_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_size_t,
                                      C.c_void_p]),
+    "jp_lm_osem_planned_res": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_float, C.c_float, C.c_void_p,
+                                         C.c_size_t, C.c_void_p]),
+    "jp_gauss3d": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_float, C.c_float, C.c_void_p]),
     "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
@@ -355,6 +358,36 @@ def jp_lm_osem_planned(plan: LmPlan, sens, img, n_iter: int, workspace=None, str
                                      workspace.numel() * workspace.element_size(), _stream(stream)),
            "jp_lm_osem_planned")
     return img
+
+
+def jp_lm_osem_planned_res(plan: LmPlan, sens, img, n_iter: int, res_sigma_mm: float, res_n_sigmas: float = 3.0,
+                           workspace=None, stream=None) -> torch.Tensor:
+    """listmode OSEM with the image-based resolution model in every subset"""
+    img = _img(img)
+    sens = _img(sens)
+    assert tuple(img.shape) == plan.shape and sens.shape == img.shape
+    need = int(load().jp_lm_osem_planned_workspace_bytes(plan.handle))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=img.device)
+    assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= need
+    _check(load().jp_lm_osem_planned_res(plan.handle, sens.data_ptr(), img.data_ptr(), int(n_iter), float(res_sigma_mm),
+                                         float(res_n_sigmas), workspace.data_ptr(),
+                                         workspace.numel() * workspace.element_size(), _stream(stream)),
+           "jp_lm_osem_planned_res")
+    return img
+
+
+def jp_gauss3d(img, voxsize, sigma_mm: float, n_sigmas: float = 3.0, out=None, stream=None) -> torch.Tensor:
+    """out = G img: the image-based resolution model (3-D Gaussian, zero boundary); out may be img"""
+    img = _img(img)
+    g = make_geom(img.shape, (0.0, 0.0, 0.0), voxsize)
+    if out is None:
+        out = torch.empty_like(img)
+    _dev(out, torch.float32, "out")
+    assert out.shape == img.shape and out.is_contiguous()
+    _check(load().jp_gauss3d(img.data_ptr(), out.data_ptr(), C.byref(g), float(sigma_mm), float(n_sigmas),
+                             _stream(stream)), "jp_gauss3d")
+    return out
 
 
 # ---- hybrid mode: host tensors in and out (PAPER.md:61) -------------------------------------------------------

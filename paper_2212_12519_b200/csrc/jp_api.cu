@@ -525,10 +525,11 @@ size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan)
     return (size_t)(nvox + (n + ns - 1) / ns + 64) * sizeof(float);
 }
 
-int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
-                       size_t workspace_bytes, void *stream)
+static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *img, int n_iter, float res_sigma,
+                                float res_nsig, void *workspace, size_t workspace_bytes, void *stream)
 {
     g_err[0] = 0;
+    const bool res = res_sigma > 0.f;
     if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
     if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
     if (!sens || !img || !workspace) return fail(JP_ERR_POINTER, "NULL argument");
@@ -551,10 +552,29 @@ int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n
     }
     const bool z_events = c.has_axis2(-1);
     if (z_events) JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
+    // resolution model: xb = G x feeds the forward projection, G folds the back projection (stream-ordered scratch)
+    struct Scratch {
+        float *p = nullptr;
+        cudaStream_t st = nullptr;
+        ~Scratch() { if (p) cudaFreeAsync(p, st); }
+    } sc;
+    float *xb = nullptr, *bb = nullptr, *tmp = nullptr;
+    if (res) {
+        sc.st = st;
+        JP_CUDA(cudaMallocAsync((void **)&sc.p, sizeof(float) * 3 * (size_t)nvox, st), where);
+        xb = sc.p;
+        bb = sc.p + nvox;
+        tmp = sc.p + 2 * nvox;
+    }
     // per subset: fwd (ratio fused) and back axis by axis on the quad arrays, then the multiplicative update
     for (int it = 0; it < n_iter; ++it) {
         for (int m = 0; m < c.ns; ++m) {
-            JP_CUDA(jp::launch_quad_build(img, c.g, q[0], q[1], st), where);
+            const float *xin = img;
+            if (res) {
+                JP_CUDA(jp::launch_gauss3d(img, xb, tmp, c.g, res_sigma, res_nsig, st), where);
+                xin = xb;
+            }
+            JP_CUDA(jp::launch_quad_build(xin, c.g, q[0], q[1], st), where);
             for (int a = 0; a < 2; ++a)
                 JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, r, 1, st), where);
             for (int a = 0; a < 2; ++a) {
@@ -563,7 +583,7 @@ int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n
             }
             if (z_events) {
                 float *px = nullptr, *pb = nullptr;
-                JP_CUDA(jp::padded_create(img, c.g, false, st, &px), where);
+                JP_CUDA(jp::padded_create(xin, c.g, false, st, &px), where);
                 cudaError_t e = jp::padded_create(nullptr, c.g, true, st, &pb);
                 if (e == cudaSuccess) e = jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, true), px, c.g, c.t, tc.lut, r, 1, st);
                 if (e == cudaSuccess) e = jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, true), r, c.g, c.t, tc.lut, pb, st);
@@ -572,9 +592,48 @@ int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n
                 jp::padded_destroy(pb, st);
                 JP_CUDA(e, where);
             }
-            JP_CUDA(jp::launch_quad_osem_update(img, b[0], b[1], z_events ? bz : nullptr, sens, (float)c.ns, c.g, st), where);
+            if (!res) {
+                JP_CUDA(jp::launch_quad_osem_update(img, b[0], b[1], z_events ? bz : nullptr, sens, (float)c.ns, c.g, st), where);
+            } else {
+                JP_CUDA(cudaMemsetAsync(bb, 0, sizeof(float) * (size_t)nvox, st), where);
+                JP_CUDA(jp::launch_quad_merge(b[0], b[1], c.g, bb, st), where);
+                if (z_events) JP_CUDA(jp::launch_add_clear(bb, bz, nvox, st), where);
+                JP_CUDA(jp::launch_gauss3d(bb, bb, tmp, c.g, res_sigma, res_nsig, st), where);
+                JP_CUDA(jp::launch_osem_update(img, bb, sens, (float)c.ns, nvox, st), where);
+            }
         }
     }
+    return JP_OK;
+}
+
+int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
+                       size_t workspace_bytes, void *stream)
+{
+    return lm_osem_planned_impl(plan, sens, img, n_iter, 0.f, 0.f, workspace, workspace_bytes, stream);
+}
+
+int jp_lm_osem_planned_res(const jp_plan *plan, const float *sens, float *img, int n_iter, float res_sigma_mm,
+                           float res_n_sigmas, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!(res_sigma_mm > 0.f) || !(res_n_sigmas > 0.f)) return fail(JP_ERR_SIZE, "res_sigma_mm <= 0 or res_n_sigmas <= 0");
+    return lm_osem_planned_impl(plan, sens, img, n_iter, res_sigma_mm, res_n_sigmas, workspace, workspace_bytes, stream);
+}
+
+int jp_gauss3d(const float *in, float *out, const jp_geom *geom, float sigma_mm, float n_sigmas, void *stream)
+{
+    g_err[0] = 0;
+    jp::Geom g;
+    JP_TRY(check_geom(geom, g));
+    if (!in || !out) return fail(JP_ERR_POINTER, "in or out is NULL");
+    if (!(sigma_mm > 0.f) || !(n_sigmas > 0.f)) return fail(JP_ERR_SIZE, "sigma_mm <= 0 or n_sigmas <= 0");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    float *tmp = nullptr;
+    JP_CUDA(cudaMallocAsync((void **)&tmp, sizeof(float) * (size_t)nvox, st), "jp_gauss3d (scratch)");
+    const cudaError_t e = jp::launch_gauss3d(in, out, tmp, g, sigma_mm, n_sigmas, st);
+    cudaFreeAsync(tmp, st);
+    if (e == cudaErrorInvalidValue) return fail(JP_ERR_SIZE, "Gaussian kernel radius > 16 voxels");
+    JP_CUDA(e, "jp_gauss3d");
     return JP_OK;
 }
 

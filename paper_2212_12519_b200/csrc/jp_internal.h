@@ -98,6 +98,11 @@ void lm_plan_segment(const LmPlan *pl, int m, int a, int64_t *first, int64_t *co
 // persistent quad scratch of the plan (allocated on first use): which = 0,1: Q0,Q1; 2,3: B0,B1
 cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
 
+// resolution model (jp_gauss.cu): out = G in, three separable passes; tmp = nvox floats of scratch; in may alias out
+cudaError_t launch_gauss3d(const float *in, float *out, float *tmp, const Geom &g, float sigma_mm, float nsig,
+                           cudaStream_t st);
+cudaError_t launch_add_clear(float *a, float *b, int64_t n, cudaStream_t st); // a += b; b = 0
+
 // x = sens > 0 ? x * b * scale / sens : 0;  b = 0   (OSEM multiplicative update, clears b for the next subset)
 cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scale, int64_t nvox, cudaStream_t st);
 

@@ -334,6 +334,43 @@ def test_config4_small_osem_planned(cuda_device, scanner, events):
     plan.destroy()
 
 
+def test_resolution_model(cuda_device, scanner, events):
+    """image-based resolution model: jp_gauss3d vs the oracle's plain 3-D sum, and OSEM with it"""
+    g, ph = scanner
+    sig = oracle.fwhm_to_sigma(4.5)
+    # anisotropic voxels, odd sizes (several blocks + ragged tail), in-place call
+    rng = np.random.default_rng(8)
+    x = rng.random((37, 21, 45)).astype(np.float32)
+    vox = (2.0, 1.5, 2.78)
+    ref = oracle.gauss3d(x, vox, sig)
+    got = jp.jp_gauss3d(dev(x, cuda_device), vox, sig)
+    assert np.abs(got.cpu().numpy() - ref).max() <= 2e-6 * np.abs(ref).max()
+    xi = dev(x, cuda_device).clone()
+    jp.jp_gauss3d(xi, vox, sig, out=xi)
+    assert torch.equal(xi, got)
+    # OSEM with the model: 5 subsets x 1 iteration on the scanner geometry
+    xs, xe, tb = events
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    sx, se = inputs.sinogram_lors(views=range(0, 256, 8), radial=range(-64, 65, 4))
+    sx, se = sx[:, ::5].contiguous(), se[:, ::5].contiguous()
+    sens = oracle.gauss3d(oracle.back(sx.numpy(), se.numpy(), np.ones(sx.shape[1]), g.n, g.origin, g.voxsize),
+                          g.voxsize, sig).astype(np.float32)
+    x0 = np.ones(g.n, dtype=np.float32)
+    ref = oracle.lm_osem_res(xs.numpy(), xe.numpy(), tb.numpy(), sens.astype(np.float64), x0, g.origin, g.voxsize,
+                             *args, n_subsets=5, n_iter=1, res_sigma_mm=sig)
+    plan = jp.LmPlan(xs.to(cuda_device), xe.to(cuda_device), tb.to(cuda_device), g.n, g.origin, g.voxsize, tof,
+                     n_subsets=5)
+    img = dev(x0, cuda_device).clone()
+    jp.jp_lm_osem_planned_res(plan, dev(sens, cuda_device), img, n_iter=1, res_sigma_mm=sig)
+    gotx = img.cpu().numpy().astype(np.float64)
+    assert np.isfinite(gotx).all()
+    assert np.linalg.norm(gotx - ref) / np.linalg.norm(ref) <= 1e-4
+    assert np.abs(gotx - ref).max() <= 1e-3 * np.abs(ref).max()
+    plan.destroy()
+
+
 # ---- edge cases ----------------------------------------------------------------------------------------
 def test_edge_cases(cuda_device):
     g = inputs.GEOM_SMALL
