@@ -285,6 +285,37 @@ class Workload:
         if ev:
             ev[2].record(s)
 
+    def time_nontof_listmode(self, reps=3):
+        """NON-TOF fwd / back over the configs[3] events, unsorted (jp_fwd /
+        jp_back on the acquisition order) and through the plan (sorted, line tiles); ms per call"""
+        jp, s = self.jp, self.stream
+        out = {}
+        y = self.y
+        p = torch.empty(self.n, dtype=torch.float32, device=self.dev)
+        calls = {
+            "unsorted": (lambda: jp.jp_fwd(self.xs, self.xe, self.img, G.origin, G.voxsize, out=p),
+                         lambda: jp.jp_back(self.xs, self.xe, y, G.n, G.origin, G.voxsize, img=self.bimg)),
+            "planned": (lambda: jp.jp_fwd_lm_planned(self.plan, self.img, out=p),
+                        lambda: jp.jp_back_lm_planned(self.plan, y, img=self.bimg)),
+        }
+        for name, (f, b) in calls.items():
+            f(); self.bimg.zero_(); b()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            ev[0].record(s)
+            for _ in range(reps):
+                f()
+            ev[1].record(s)
+            for _ in range(reps):
+                self.bimg.zero_()
+                b()
+            ev[2].record(s)
+            torch.cuda.synchronize()
+            fm, bm = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+            out[name] = {"fwd_ms": fm, "back_ms": bm, "fwd_events_per_s": self.n / fm * 1e3,
+                         "back_events_per_s": self.n / bm * 1e3}
+        out["plane_steps"] = self.jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
+        return out
+
     def time_osem_with_resolution_model(self, iters=2):
         """the same OSEM iteration with the 4.5 mm FWHM image-based resolution model
          in every subset (2 x 20 Gaussian smoothings per iteration); seconds per iteration"""
@@ -486,6 +517,8 @@ def run_ours(args):
     }
     if w.plan_s is not None:
         line["config"]["plan_s"] = w.plan_s
+    if c == 3:
+        line["nontof_listmode"] = w.time_nontof_listmode()
     if c == 4:
         line["s_per_iteration"] = ms_per_step * 1e-3
         line["s_per_iteration_with_resolution_model"] = w.time_osem_with_resolution_model()
@@ -512,6 +545,8 @@ def run_ours(args):
                 d["s_per_iteration_with_resolution_model"] = ow.time_osem_with_resolution_model()
             else:
                 d["fwd"], d["back"] = r["fwd"], r["back"]
+            if oc == 3:
+                d["nontof_listmode"] = ow.time_nontof_listmode()
             if ow.plan_s is not None:
                 d["plan_s"] = ow.plan_s
             other[f"configs[{oc}]"] = d

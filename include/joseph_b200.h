@@ -154,6 +154,12 @@ int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, flo
 /* img += A_subset^T y, y has n entries in caller order.  ACCUMULATES. */
 int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream);
 /* jp_lm_osem on the plan's events, subsets and geometry */
+/* NON-TOF projections of the plan's events (the paper's second listmode workload: every plane
+ * of each event's LOR, the TOF bins of the plan are ignored).  Arguments, order of results (caller order) and
+ * subset selection as for jp_fwd_tof_lm_planned / jp_back_tof_lm_planned; jp_back_lm_planned ACCUMULATES. */
+int jp_fwd_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream);
+int jp_back_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream);
+
 size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan);
 int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
                        size_t workspace_bytes, void *stream);

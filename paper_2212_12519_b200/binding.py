@@ -64,6 +64,8 @@ EXPORTS = {
     "jp_lm_plan_subset_count": (C.c_int64, [C.c_void_p, C.c_int]),
     "jp_fwd_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_back_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_fwd_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_back_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_lm_osem_planned_workspace_bytes": (C.c_size_t, [C.c_void_p]),
     "jp_lm_osem_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_size_t,
                                      C.c_void_p]),
@@ -343,6 +345,32 @@ def jp_back_tof_lm_planned(plan: LmPlan, y, subset: int = -1, img=None, stream=N
     assert tuple(img.shape) == plan.shape
     _check(load().jp_back_tof_lm_planned(plan.handle, int(subset), y.data_ptr(), img.data_ptr(), _stream(stream)),
            "jp_back_tof_lm_planned")
+    return img
+
+
+def jp_fwd_lm_planned(plan: LmPlan, img, subset: int = -1, out=None, stream=None) -> torch.Tensor:
+    """NON-TOF forward projection of the plan's events, results in caller order"""
+    img = _img(img)
+    assert tuple(img.shape) == plan.shape
+    if out is None:
+        out = torch.zeros(plan.n, dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == plan.n and out.is_contiguous()
+    _check(load().jp_fwd_lm_planned(plan.handle, int(subset), img.data_ptr(), out.data_ptr(), _stream(stream)),
+           "jp_fwd_lm_planned")
+    return out
+
+
+def jp_back_lm_planned(plan: LmPlan, y, subset: int = -1, img=None, stream=None) -> torch.Tensor:
+    """NON-TOF back projection of per-event values over the plan's events; ACCUMULATES into img"""
+    _dev(y, torch.float32, "y")
+    assert y.numel() == plan.n and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(plan.shape, dtype=torch.float32, device=y.device)
+    img = _img(img)
+    assert tuple(img.shape) == plan.shape
+    _check(load().jp_back_lm_planned(plan.handle, int(subset), y.data_ptr(), img.data_ptr(), _stream(stream)),
+           "jp_back_lm_planned")
     return img
 
 

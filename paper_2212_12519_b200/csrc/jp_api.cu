@@ -515,6 +515,55 @@ int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, floa
     return JP_OK;
 }
 
+// ---- non-TOF listmode over the plan's sorted events ----------------------
+int jp_fwd_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    if (!img || !p) return fail(JP_ERR_POINTER, "img or p is NULL");
+    const char *where = "jp_fwd_lm_planned";
+    cudaStream_t st = (cudaStream_t)stream;
+    PlanCtx c(plan);
+    const bool tiles = lm_tiles_wanted(c.lm);
+    for (int a = 0; a < 3; ++a)
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset) {
+                const jp::Range rg = c.seg(m, a, false);
+                cudaError_t e = cudaErrorNotSupported;
+                if (tiles && a < 2)
+                    e = jp::launch_fwd_tof_lm_tile(c.l, nullptr, rg.first, rg.count, rg.perm, 0, img, c.g, c.t, p, 0, st);
+                if (e == cudaErrorNotSupported) e = jp::launch_fwd(c.l, rg, img, c.g, p, st);
+                JP_CUDA(e, where);
+            }
+    return JP_OK;
+}
+
+int jp_back_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    if (!img || !y) return fail(JP_ERR_POINTER, "img or y is NULL");
+    const char *where = "jp_back_lm_planned";
+    cudaStream_t st = (cudaStream_t)stream;
+    PlanCtx c(plan);
+    const bool tiles = lm_tiles_wanted(c.lm);
+    for (int a = 0; a < 3; ++a)
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset) {
+                const jp::Range rg = c.seg(m, a, false);
+                cudaError_t e = cudaErrorNotSupported;
+                if (tiles && a < 2)
+                    e = jp::launch_back_tof_lm_tile(c.l, nullptr, rg.first, rg.count, rg.perm, 0, y, c.g, c.t, img, st);
+                if (e == cudaErrorNotSupported) e = jp::launch_back(c.l, rg, y, c.g, img, st);
+                JP_CUDA(e, where);
+            }
+    return JP_OK;
+}
+
 size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan)
 {
     if (!plan || !plan->lm) return 0;

@@ -77,6 +77,7 @@ struct LineExtra {
     double Rd;      // 1 + (d_q1 / d_p)^2
 };
 
+template <bool TOF>
 __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double Rd, float zs, float ze, float centre,
                                           float reach, float scale)
 {
@@ -94,7 +95,7 @@ __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double 
     const double dtau = vp * t.inv_dp * L;
     const double tau_at0 = (t.ops * t.inv_dp - 0.5) * L;
     int ilo = t.I0, ihi = t.I1;
-    {   // TOF window: |tau(i) - centre| <= reach, rounded outwards
+    if (TOF) { // TOF window: |tau(i) - centre| <= reach, rounded outwards
         const double ivt = drcp(dtau);
         const double ia = ((double)centre - (double)reach - tau_at0) * ivt, ib = ((double)centre + (double)reach - tau_at0) * ivt;
         const double np = (double)g.n[t.p];
@@ -128,38 +129,41 @@ __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double 
     }
     z.i0 = ilo;
     z.i1 = ihi;
-    z.x0 = (float)(((double)centre - (tau_at0 + dtau * (double)ilo)) * (double)scale);
-    z.dx = (float)(-dtau * (double)scale);
+    z.x0 = TOF ? (float)(((double)centre - (tau_at0 + dtau * (double)ilo)) * (double)scale) : 0.f;
+    z.dx = TOF ? (float)(-dtau * (double)scale) : 0.f;
     return z;
 }
 
 // per-LOR path (short runs, principal axis z): same arithmetic as jp_kernels.cu on the unpadded image
+template <bool TOF>
 __device__ __forceinline__ float generic_fwd_lm(const Lors &l, int64_t j, float centre, float reach, const Geom &g,
                                                 const Tof &t, const float *__restrict__ img, uint32_t gbase,
                                                 const G1Tab &gt)
 {
     Ray r;
-    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    ray_setup<TOF>(l, j, g, t.coff, centre - reach, centre + reach, r);
     float acc = 0.f;
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        acc = fmaf(plane_value(img, r, k, cl), g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale), acc);
+        const float w = TOF ? g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale) : 1.f;
+        acc = fmaf(plane_value(img, r, k, cl), w, acc);
     }
     return r.cf * acc;
 }
 
+template <bool TOF>
 __device__ __forceinline__ void generic_back_lm(const Lors &l, int64_t j, float centre, float reach, float y, const Geom &g,
                                                 const Tof &t, float *__restrict__ img, uint32_t gbase, const G1Tab &gt)
 {
     Ray r;
-    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    ray_setup<TOF>(l, j, g, t.coff, centre - reach, centre + reach, r);
     const float x = r.cf * y;
     if (r.nk == 0 || x == 0.f) return;
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        const float w = g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale);
+        const float w = TOF ? g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale) : 1.f;
         if (w != 0.f) plane_scatter(img, r, k, cl, x * w);
     }
 }
@@ -220,11 +224,11 @@ __device__ __forceinline__ int64_t out_index(const int *__restrict__ perm, int64
         const float tt = __fadd_rd(u, kMagic);                                  \
         const float w = u - (tt - kMagic);                                      \
         const float2 v = lds_pair<(K) * P * 8>(row + (__float_as_uint(tt) << 3)); \
-        const float wt = g1_weight(gbase, xmax, fmaf(dx, fk, X0K));             \
+        const float wt = TOF ? g1_weight(gbase, xmax, fmaf(dx, fk, X0K)) : 1.f; \
         acc = fmaf(fmaf(w, v.y, v.x), wt, acc);                                 \
     }
 
-template <int P, int LM_MODE>
+template <int P, int LM_MODE, bool TOF>
 __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
     k_fwd_tof_lm_tile(Lors l, const int16_t *__restrict__ tofbin, int64_t first, int64_t count,
                       const int *__restrict__ perm, int64_t io_off, const float *__restrict__ img, Geom g, Tof t,
@@ -241,7 +245,8 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
     const int nev = (int)min((int64_t)kTile, first + count - c0);
     const float reach = 0.5f * t.width + t.nsig * t.sigma;
 
-    for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
+    if (TOF)
+        for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
     const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
     const float xmax = gt.xmax;
 
@@ -290,8 +295,8 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
             for (int m = 0; m < kPerThread; ++m)
                 if (active[m]) {
                     const int64_t e = c0 + ra + m * kThreads + tid;
-                    const float c = (float)tofbin[e] * t.width;
-                    float out = generic_fwd_lm(l, e, c, reach, g, t, img, gbase, gt);
+                    const float c = TOF ? (float)tofbin[e] * t.width : 0.f;
+                    float out = generic_fwd_lm<TOF>(l, e, c, reach, g, t, img, gbase, gt);
                     if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
                     p[out_index(perm, io_off, first, e)] = out;
                 }
@@ -327,12 +332,12 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                 if (active[m]) {
                     const int64_t e = c0 + ra + m * kThreads + tid;
                     float zs = l.zs[e], ze = l.ze[e];
-                    float centre = fmaf((float)tofbin[e], t.width, t.coff); // bin centre on the canonical tau axis
+                    float centre = TOF ? fmaf((float)tofbin[e], t.width, t.coff) : 0.f; // bin centre on the canonical tau axis
                     if (is_swapped(l.xs[e], l.ys[e], l.xe[e], l.ye[e])) {   // (e, s): walk it as (s, e), mirrored
                         const float tmp = zs; zs = ze; ze = tmp;
                         centre = -centre;
                     }
-                    zr[m] = lm_setup(g, trk, Rd, zs, ze, centre, reach, gt.scale);
+                    zr[m] = lm_setup<TOF>(g, trk, Rd, zs, ze, centre, reach, gt.scale);
                     if (zr[m].i1 >= zr[m].i0) {
                         lo = min(lo, zr[m].i0);
                         hi = max(hi, zr[m].i1);
@@ -402,14 +407,14 @@ __device__ __forceinline__ void reds_add_lm(uint32_t addr, int q)
         const float tt = __fadd_rd(u, kMagic);                                  \
         const float w = u - (tt - kMagic);                                      \
         const uint32_t a = row + (__float_as_uint(tt) << 2);                    \
-        const float xw = xm * g1_weight(gbase, xmax, fmaf(dx, fk, X0K));        \
+        const float xw = TOF ? xm * g1_weight(gbase, xmax, fmaf(dx, fk, X0K)) : xm; \
         const int qxw = __float_as_int(xw + kMagic);                            \
         const int bits = __float_as_int(fmaf(xw, w, kMagic));                   \
         reds_add_lm<(K) * P * 4>(a, qxw - bits);                                \
         reds_add_lm<(K) * P * 4 + 4>(a, bits - kMagicI);                        \
     }
 
-template <int P>
+template <int P, bool TOF>
 __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
     k_back_tof_lm_tile(Lors l, const int16_t *__restrict__ tofbin, int64_t first, int64_t count,
                        const int *__restrict__ perm, int64_t io_off, const float *__restrict__ y, Geom g, Tof t,
@@ -427,7 +432,8 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
     const int nev = (int)min((int64_t)kTile, first + count - c0);
     const float reach = 0.5f * t.width + t.nsig * t.sigma;
 
-    for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
+    if (TOF)
+        for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
     const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
     const float xmax = gt.xmax;
     {
@@ -472,7 +478,8 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                 if (active[m]) {
                     const int64_t e = c0 + ra + m * kThreads + tid;
                     const float yv = y[out_index(perm, io_off, first, e)];
-                    if (yv != 0.f) generic_back_lm(l, e, (float)tofbin[e] * t.width, reach, yv, g, t, img, gbase, gt);
+                    if (yv != 0.f)
+                        generic_back_lm<TOF>(l, e, TOF ? (float)tofbin[e] * t.width : 0.f, reach, yv, g, t, img, gbase, gt);
                 }
             continue;
         }
@@ -510,12 +517,12 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                 if (active[m]) {
                     const int64_t e = c0 + ra + m * kThreads + tid;
                     float zs = l.zs[e], ze = l.ze[e];
-                    float centre = fmaf((float)tofbin[e], t.width, t.coff);
+                    float centre = TOF ? fmaf((float)tofbin[e], t.width, t.coff) : 0.f;
                     if (is_swapped(l.xs[e], l.ys[e], l.xe[e], l.ye[e])) {
                         const float tmp = zs; zs = ze; ze = tmp;
                         centre = -centre;
                     }
-                    zr[m] = lm_setup(g, trk, Rd, zs, ze, centre, reach, gt.scale);
+                    zr[m] = lm_setup<TOF>(g, trk, Rd, zs, ze, centre, reach, gt.scale);
                     x[m] = zr[m].cf * y[out_index(perm, io_off, first, e)];
                     if (zr[m].i1 >= zr[m].i0 && x[m] != 0.f) {
                         lo = min(lo, zr[m].i0);
@@ -671,54 +678,67 @@ cudaError_t g1tab_create(const Tof &t, int n, cudaStream_t st, G1Tab *out)
 
 // events [first, first + count) of the sorted list l / tofbin; outputs p[perm[e]] (perm != null) or
 // p[io_off + e - first].  cudaErrorNotSupported: image too wide for the tiled kernel.
+// tofbin == nullptr: NON-TOF listmode (every plane of the LOR, weight 1; t is ignored)
 cudaError_t launch_fwd_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t first, int64_t count, const int *perm,
-                                   int64_t io_off, const float *img, const Geom &g, const Tof &t, float *p, int lm_mode,
+                                   int64_t io_off, const float *img, const Geom &g, const Tof &t_in, float *p, int lm_mode,
                                    cudaStream_t st)
 {
     if (count == 0) return cudaSuccess;
+    const bool tof = tofbin != nullptr;
+    const Tof t = tof ? t_in : Tof{1.f, 1.f, 1.f, 1, 0.f};
     const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(float2));
     if (!c.P) return cudaErrorNotSupported;
-    G1Tab gt;
-    cudaError_t e = g1tab_create(t, c.g1n, st, &gt);
+    G1Tab gt{};
+    cudaError_t e = tof ? g1tab_create(t, c.g1n, st, &gt) : cudaSuccess;
     if (e != cudaSuccess) return e;
     const unsigned grid = (unsigned)((count + kTile - 1) / kTile);
+#define JP_LM_LAUNCH_FWD(MODE, TOFF)                                                                                   \
+    {                                                                                                                  \
+        e = cudaFuncSetAttribute(k_fwd_tof_lm_tile<P, MODE, TOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
+                                 (int)kSmemBudget);                                                                    \
+        if (e == cudaSuccess)                                                                                          \
+            k_fwd_tof_lm_tile<P, MODE, TOFF><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, img, \
+                                                                             g, t, gt, c.rows_cap, c.vec_ok, p);       \
+    }
     JP_LM_DISPATCH_P(c, {
-        if (lm_mode == 1) {
-            e = cudaFuncSetAttribute(k_fwd_tof_lm_tile<P, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
-            if (e == cudaSuccess)
-                k_fwd_tof_lm_tile<P, 1><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, img, g, t, gt,
-                                                                        c.rows_cap, c.vec_ok, p);
-        } else {
-            e = cudaFuncSetAttribute(k_fwd_tof_lm_tile<P, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
-            if (e == cudaSuccess)
-                k_fwd_tof_lm_tile<P, 0><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, img, g, t, gt,
-                                                                        c.rows_cap, c.vec_ok, p);
-        }
+        if (!tof) JP_LM_LAUNCH_FWD(0, false)
+        else if (lm_mode == 1) JP_LM_LAUNCH_FWD(1, true)
+        else JP_LM_LAUNCH_FWD(0, true)
     })
+#undef JP_LM_LAUNCH_FWD
     if (e == cudaSuccess) e = cudaGetLastError();
-    cudaFreeAsync((void *)gt.tab, st);
+    if (gt.tab) cudaFreeAsync((void *)gt.tab, st);
     return e;
 }
 
 cudaError_t launch_back_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t first, int64_t count, const int *perm,
-                                    int64_t io_off, const float *y, const Geom &g, const Tof &t, float *img,
+                                    int64_t io_off, const float *y, const Geom &g, const Tof &t_in, float *img,
                                     cudaStream_t st)
 {
     if (count == 0) return cudaSuccess;
+    const bool tof = tofbin != nullptr;
+    const Tof t = tof ? t_in : Tof{1.f, 1.f, 1.f, 1, 0.f};
     const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(int));
     if (!c.P) return cudaErrorNotSupported;
-    G1Tab gt;
-    cudaError_t e = g1tab_create(t, c.g1n, st, &gt);
+    G1Tab gt{};
+    cudaError_t e = tof ? g1tab_create(t, c.g1n, st, &gt) : cudaSuccess;
     if (e != cudaSuccess) return e;
     const unsigned grid = (unsigned)((count + kTile - 1) / kTile);
+#define JP_LM_LAUNCH_BACK(TOFF)                                                                                         \
+    {                                                                                                                   \
+        e = cudaFuncSetAttribute(k_back_tof_lm_tile<P, TOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                                 (int)kSmemBudget);                                                                     \
+        if (e == cudaSuccess)                                                                                           \
+            k_back_tof_lm_tile<P, TOFF><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, y, g, t, \
+                                                                        gt, c.rows_cap, c.vec_ok, img);                 \
+    }
     JP_LM_DISPATCH_P(c, {
-        e = cudaFuncSetAttribute(k_back_tof_lm_tile<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
-        if (e == cudaSuccess)
-            k_back_tof_lm_tile<P><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, y, g, t, gt,
-                                                                  c.rows_cap, c.vec_ok, img);
+        if (tof) JP_LM_LAUNCH_BACK(true)
+        else JP_LM_LAUNCH_BACK(false)
     })
+#undef JP_LM_LAUNCH_BACK
     if (e == cudaSuccess) e = cudaGetLastError();
-    cudaFreeAsync((void *)gt.tab, st);
+    if (gt.tab) cudaFreeAsync((void *)gt.tab, st);
     return e;
 }
 

@@ -334,6 +334,36 @@ def test_config4_small_osem_planned(cuda_device, scanner, events):
     plan.destroy()
 
 
+@pytest.mark.parametrize("tile", ["1", "0"])
+def test_nontof_listmode_planned(cuda_device, scanner, events, tile, monkeypatch):
+    """non-TOF projections of listmode events: unsorted through jp_fwd /
+    jp_back, and through the plan (line tiles forced on / off) -- all against the oracle, in caller order"""
+    monkeypatch.setenv("JP_LM_TILE", tile)
+    g, ph = scanner
+    if tile == "1":
+        xs, xe, tb = _line_events(seed=22)
+    else:
+        xs, xe, tb = (t.numpy() for t in events)
+        xs, xe, tb = xs[:, :100_003], xe[:, :100_003], tb[:100_003]
+    n = xs.shape[1]
+    tof = jp.make_tof(17.0, 13.6, 3.0, 29)
+    xsd, xed, imgd = dev(xs, cuda_device), dev(xe, cuda_device), dev(ph, cuda_device)
+    ref = oracle.fwd(xs, xe, ph, g.origin, g.voxsize)
+    assert_fwd(jp.jp_fwd(xsd, xed, imgd, g.origin, g.voxsize), ref)
+    plan = jp.LmPlan(xsd, xed, dev(tb, cuda_device), g.n, g.origin, g.voxsize, tof, n_subsets=2)
+    p = jp.jp_fwd_lm_planned(plan, imgd)
+    assert_fwd(p, ref)
+    y = inputs.uniform_values(n, 0.5, 2.0, seed=15).to(cuda_device)
+    bref = oracle.back(xs, xe, y.cpu().numpy(), g.n, g.origin, g.voxsize)
+    b = jp.jp_back_lm_planned(plan, y)
+    assert_back(b, bref)
+    b2 = jp.jp_back_lm_planned(plan, y, subset=0)
+    jp.jp_back_lm_planned(plan, y, subset=1, img=b2)
+    assert_back(b2, bref)
+    assert adj_gap(p, y, imgd, b) <= ADJ_GAP
+    plan.destroy()
+
+
 def test_resolution_model(cuda_device, scanner, events):
     """image-based resolution model: jp_gauss3d vs the oracle's plain 3-D sum, and OSEM with it"""
     g, ph = scanner
