@@ -244,3 +244,59 @@ def lm_osem_res(xstart, xend, tofbin, sens, img0, origin, voxsize, tofbin_width,
                                    _dptr(sens), _dptr(img), C.c_int(int(n_subsets)), C.c_int(int(n_iter)),
                                    C.c_double(float(res_sigma_mm)), C.c_double(float(res_n_sigmas))), "lm_osem_res")
     return img
+
+
+# ---- TOF sinogram OSEM with multiplicative factors and additive contamination ----------
+# "the projection work required for an OSEM subset update [37]-[39]"; sinogram OSEM
+# keeps "the complete image volume, the emission sinogram, the forward projection and the contamination
+# sinogram" on the GPU.  The paper gives no formula; this is OSEM (Hudson & Larkin, PAPER.md:193 ref. 39) for the
+# usual PET model  ybar = mult * (A x) + contam  (mult: attenuation x normalisation per LOR, the same for every
+# TOF bin; contam: randoms + scatter per LOR and bin).  Readings (S1-S3):
+#   S1  subset m = LORs [subset_offsets[m], subset_offsets[m+1]) of the caller's list (the caller arranges the
+#       list subset-major; for a ring scanner a subset is every n_subsets-th view), in order;
+#   S2  r[j,k] = mult[j] y[j,k] / ybar[j,k] if ybar[j,k] > 1e-9 else 0   (the guard of A14);
+#   S3  x <- x * (A_m^T r) / sens_m  where sens_m > 0, else 0;  sens_m = A_m^T (mult (x) 1_bins).
+# Written with numpy on top of the pinned projector calls, in that order, nothing fused.
+def sino_sens_tof(xstart, xend, subset_offsets, mult, n, origin, voxsize, tofbin_width, sigma_tof, n_sigmas,
+                  n_tofbins, center_offset=0.0):
+    """sens[m] = A_m^T (mult broadcast over the TOF bins): float64 [n_subsets, n0, n1, n2]"""
+    off = [int(o) for o in subset_offsets]
+    xs, xe = np.asarray(xstart), np.asarray(xend)
+    out = np.zeros((len(off) - 1,) + tuple(int(a) for a in n), dtype=np.float64)
+    for m in range(len(off) - 1):
+        a, b = off[m], off[m + 1]
+        if b > a:
+            ones = np.repeat(np.asarray(mult, dtype=np.float64)[a:b, None], int(n_tofbins), axis=1)
+            out[m] = back_tof_sino(xs[:, a:b], xe[:, a:b], ones, n, origin, voxsize, tofbin_width, sigma_tof,
+                                   n_sigmas, n_tofbins, center_offset)
+    return out
+
+
+def sino_osem_tof(xstart, xend, subset_offsets, y, mult, contam, sens, img0, origin, voxsize, tofbin_width,
+                  sigma_tof, n_sigmas, n_tofbins, n_iter, center_offset=0.0):
+    """TOF sinogram OSEM (readings S1-S3).  y, contam: [n, n_tofbins]; mult: [n]; sens: [n_subsets, n0, n1, n2].
+    Returns the final float64 image."""
+    off = [int(o) for o in subset_offsets]
+    xs, xe = np.asarray(xstart), np.asarray(xend)
+    x = np.array(img0, dtype=np.float64, order="C", copy=True)
+    y = np.asarray(y, dtype=np.float64)
+    mult = np.asarray(mult, dtype=np.float64)
+    contam = np.asarray(contam, dtype=np.float64)
+    sens = np.asarray(sens, dtype=np.float64)
+    for _ in range(int(n_iter)):
+        for m in range(len(off) - 1):
+            a, b = off[m], off[m + 1]
+            if b > a:
+                p = fwd_tof_sino(xs[:, a:b], xe[:, a:b], x, origin, voxsize, tofbin_width, sigma_tof, n_sigmas,
+                                 n_tofbins, center_offset)
+                ybar = mult[a:b, None] * p + contam[a:b]
+                r = np.zeros_like(ybar)
+                ok = ybar > 1e-9
+                r[ok] = (mult[a:b, None] * y[a:b])[ok] / ybar[ok]
+                bp = back_tof_sino(xs[:, a:b], xe[:, a:b], r, x.shape, origin, voxsize, tofbin_width, sigma_tof,
+                                   n_sigmas, n_tofbins, center_offset)
+            else:
+                bp = np.zeros_like(x)
+            pos = sens[m] > 0.0
+            x = np.where(pos, x * bp / np.where(pos, sens[m], 1.0), 0.0)
+    return x
