@@ -85,7 +85,7 @@ __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double 
     const double dz = (double)ze - (double)zs;
     const double rz = dz * t.inv_dp;
     const double vp = (double)g.v[t.p];
-    const double iv2 = drcp((double)g.v[2]);
+    const double iv2 = t.iv2;
     const double B = rz * vp * iv2;
     const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2;
     const double Ln = dsqrt_pos(Rd + rz * rz);   // L / |d_p|

@@ -17,6 +17,8 @@
 // row pitch P is a template parameter so that the unrolled plane loop addresses rows with immediates).
 // Tiles that are not tracks (ragged tail, principal axis z, unsorted lists) take the generic per-LOR
 // path in the same launch.  No plan, no scratch memory, results in caller order.
+#include <cstdlib>
+
 #include "jp_tile_common.cuh"
 
 namespace jp {
@@ -50,9 +52,66 @@ __device__ __forceinline__ void generic_back(const Lors &l, int64_t j, const Geo
     }
 }
 
+
+// ---- lane mapping (a performance hint only: any bijection of the tile's LORs onto the threads is correct) ------
+// Which LOR a lane works on decides how many shared-memory wavefronts a plane step costs.  In a sinogram the LORs
+// of a track form a grid (rows: one axial end point fixed, columns: the other one varies; ring pairs of configs[1]:
+// 16 rows x 48 columns per tile).  With consecutive LORs on consecutive lanes a half-warp spans up to 22 axial
+// cells at the far side of the image: the 64-bit row loads of the forward kernel then take 2.93 wavefronts
+// instead of 2 (profiles/r01_v3: 1.08e9 wavefronts), and the two atomics of the adjoint 4.2 (lanes less than a
+// cell apart collide on one address, lanes more than 32 cells apart on one bank).
+//   forward: a half-warp takes a block of 2 rows x 8 columns (at most 11 cells wide: conflict-free);
+//   adjoint: a half-warp takes a 16-long grid diagonal (lanes exactly one row pitch apart: no equal addresses),
+//            the second half-warp the neighbouring diagonal.
+// The row length L of the grid is read off the data: the first LOR whose zs or ze changes while the other one
+// has been constant so far.  No grid (L = 0): identity mapping.
+__device__ __forceinline__ int detect_row_length(const Lors &l, int64_t j0, int64_t n, int *sh /* 2 ints */)
+{
+    const int tid = threadIdx.x;
+    if (tid < 2) sh[tid] = kThreads;
+    __syncthreads();
+    if (j0 + kTile <= n) {
+        const float zs0 = l.zs[j0], ze0 = l.ze[j0];
+        const bool ds = !same_bits(l.zs[j0 + tid], zs0), de = !same_bits(l.ze[j0 + tid], ze0);
+        const unsigned bs = __ballot_sync(0xffffffffu, ds), be = __ballot_sync(0xffffffffu, de);
+        if ((tid & 31) == 0) {
+            if (bs) atomicMin(&sh[0], (tid & ~31) + __ffs(bs) - 1);
+            if (be) atomicMin(&sh[1], (tid & ~31) + __ffs(be) - 1);
+        }
+    }
+    __syncthreads();
+    const int Ls = sh[0], Le = sh[1];
+    int L = 0;
+    if (Ls == 1 && Le < kThreads) L = Le;       // zs runs along a row, ze is the row's constant
+    else if (Le == 1 && Ls < kThreads) L = Ls;  // the other way round
+    return L;
+}
+
+// forward: half-warp h of the tile <- rows (2 rp, 2 rp + 1) x columns [8 cg, 8 cg + 8)
+__device__ __forceinline__ int map_fwd(int idx, int L)
+{
+    if (L < 8 || (L & 7) || (kTile % (2 * L))) return idx;
+    const int h = idx >> 4, l16 = idx & 15, C = L >> 3;
+    const int rp = h / C, cg = h - rp * C;
+    return rp * 2 * L + (l16 >> 3) * L + cg * 8 + (l16 & 7);
+}
+
+// adjoint: warp w of the tile <- rows [16 rb, 16 rb + 16), two neighbouring diagonals (columns wrap)
+__device__ __forceinline__ int map_back(int idx, int L)
+{
+    if (L < 2 || (L & 1) || (kTile % (16 * L))) return idx;
+    const int w = idx >> 5, l32 = idx & 31, d = l32 & 15, s = l32 >> 4, half = L >> 1;
+    const int rb = w / half, c2 = w - rb * half;
+    int col = 2 * c2 + s + d;
+    col -= (col >= L) ? L : 0;
+    col -= (col >= L) ? L : 0;
+    return (rb * 16 + d) * L + col;
+}
+
 // is this tile a track?  all 768 LORs valid, identical transaxial end points, principal axis x or y
-__device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t n, const float (&zs)[kPerThread],
-                                              const float (&ze)[kPerThread], float xs0, float ys0, float xe0, float ye0)
+__device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t n, const int (&jm)[kPerThread],
+                                              const float (&zs)[kPerThread], const float (&ze)[kPerThread], float xs0,
+                                              float ys0, float xe0, float ye0)
 {
     bool ok = (j0 + kTile <= n);
     if (ok) {
@@ -61,7 +120,7 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
         uint32_t diff = 0;
 #pragma unroll
         for (int m = 0; m < kPerThread; ++m) {
-            const int64_t j = j0 + m * kThreads + threadIdx.x;
+            const int64_t j = j0 + jm[m];
             diff |= (__float_as_uint(l.xs[j]) ^ __float_as_uint(xs0)) | (__float_as_uint(l.ys[j]) ^ __float_as_uint(ys0)) |
                     (__float_as_uint(l.xe[j]) ^ __float_as_uint(xe0)) | (__float_as_uint(l.ye[j]) ^ __float_as_uint(ye0));
             ok = ok && (fabs((double)ze[m] - (double)zs[m]) <= dmax);
@@ -77,6 +136,10 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
 #ifndef JP_MINB
 #define JP_MINB 4
 #endif
+#ifndef JP_FWD_UNROLL
+#define JP_FWD_UNROLL 8
+#endif
+
 
 // pull the end points of the tile that starts at LOR jt into L2 (one 128-byte line per thread): the CTA
 // that will work on it finds them there instead of waiting for HBM
@@ -101,40 +164,43 @@ __device__ __forceinline__ void reds_add(uint32_t addr, int q)
 } // namespace
 
 // ---- forward ------------------------------------------------------------------------------------------
-// One plane step of one LOR against the (value, slope) rows in shared memory: 4 FP32 for the
-// axial cell (FFMA, FADD.RM, FADD, FADD), one address LEA, one LDS.64, 2 FP32 to accumulate.
+// One plane step of one LOR against the (intercept, slope) rows in shared memory (build_rows<P, true>): the
+// shifted axial coordinate u = u2 - kc (FFMA), its floor in the mantissa of u + magic (FADD.RM), one address LEA,
+// one LDS.64, and value = intercept + u slope accumulated in two FP32 instructions -- no fractional part.
 #define JP_FWD_STEP(K, A2K)                                                    \
     {                                                                          \
         const float u = fmaf(b2, fk, A2K);                                     \
         const float tt = __fadd_rd(u, kMagic);                                 \
-        const float w = u - (tt - kMagic);                                     \
         const float2 v = lds_pair<(K) * P * 8>(row + (__float_as_uint(tt) << 3)); \
         acc0 += v.x;                                                           \
-        acc1 = fmaf(w, v.y, acc1);                                             \
+        acc1 = fmaf(u, v.y, acc1);                                             \
     }
 
 template <int P>
 __global__ void __launch_bounds__(kThreads, JP_MINB)
     k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
-               float *__restrict__ p)
+               int lane_map, float *__restrict__ p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                      // [rows_cap][P]
     RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(float2)); // [max(n0,n1)]
     __shared__ Track trk;
+    __shared__ int sh_len[2];
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kTile;
 
     prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
+    int jm[kPerThread];
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
-        const int64_t j = j0 + m * kThreads + tid;
+        jm[m] = m * kThreads + tid;
+        const int64_t j = j0 + jm[m];
         zs[m] = (j < n) ? l.zs[j] : 0.f;
         ze[m] = (j < n) ? l.ze[j] : 0.f;
     }
     const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (!tile_is_track(l, j0, n, zs, ze, xs0, ys0, xe0, ye0)) {
+    if (!tile_is_track(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
 #pragma unroll 1
         for (int m = 0; m < kPerThread; ++m) {
             const int64_t j = j0 + m * kThreads + tid;
@@ -150,7 +216,19 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
         for (int m = 0; m < kPerThread; ++m) p[j0 + m * kThreads + tid] = 0.f;
         return;
     }
+    // the tile does work: choose the lane mapping and fetch the axial end points again (from L1) in that order
+    const int L = lane_map ? detect_row_length(l, j0, n, sh_len) : 0;
+    if (L) {
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            jm[m] = map_fwd(m * kThreads + tid, L);
+            zs[m] = l.zs[j0 + jm[m]];
+            ze[m] = l.ze[j0 + jm[m]];
+        }
+    }
     const int n2 = g.n[2];
+    const int kci = n2 >> 1;          // axial shift of the (intercept, slope) rows
+    const float kc = (float)kci;
     // q1 cells of all planes of the track; constant zero columns of the shared rows
     for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
     {
@@ -164,16 +242,16 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
     float acc0[kPerThread], acc1[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
-        zr[m] = z_setup(g, t, zs[m], ze[m]);
+        zr[m] = z_setup(g, t, zs[m], ze[m], (double)kci);
         acc0[m] = 0.f;
         acc1[m] = 0.f;
     }
-    const uint32_t c2_base = smem_addr(C2) + kPad * 8u - ((uint32_t)kMagicI << 3);
+    const uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
     __syncthreads();
 
     for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
         const int rows = min(rows_cap, t.I1 - c0 + 1);
-        build_rows<P>(C2, rinfo, img, t, c0, rows, n2, vec_ok);
+        build_rows<P, true>(C2, rinfo, img, t, c0, rows, n2, vec_ok, kc);
         __syncthreads();
         // ---- consume: every LOR walks its planes of this chunk, interpolating along z only
 #pragma unroll
@@ -188,8 +266,28 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
             float a0 = acc0[m], a1 = acc1[m];
             {
                 float acc0 = a0, acc1 = a1;
+                int left = nst;
+#if JP_FWD_UNROLL == 8
+                const float a2_4 = fmaf(b2, 4.f, a2_0), a2_5 = fmaf(b2, 5.f, a2_0), a2_6 = fmaf(b2, 6.f, a2_0),
+                            a2_7 = fmaf(b2, 7.f, a2_0);
 #pragma unroll 1
-                for (int it = nst >> 2; it > 0; --it) {
+                for (; left >= 8; left -= 8) {
+                    JP_FWD_STEP(0, a2_0)
+                    JP_FWD_STEP(1, a2_1)
+                    JP_FWD_STEP(2, a2_2)
+                    JP_FWD_STEP(3, a2_3)
+                    JP_FWD_STEP(4, a2_4)
+                    JP_FWD_STEP(5, a2_5)
+                    JP_FWD_STEP(6, a2_6)
+                    JP_FWD_STEP(7, a2_7)
+                    fk += 8.f;
+                    row += 8u * P * 8u;
+                }
+                if (left >= 4) {
+#else
+#pragma unroll 1
+                for (; left >= 4; left -= 4) {
+#endif
                     JP_FWD_STEP(0, a2_0)
                     JP_FWD_STEP(1, a2_1)
                     JP_FWD_STEP(2, a2_2)
@@ -198,7 +296,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
                     row += 4u * P * 8u;
                 }
 #pragma unroll 1
-                for (int it = nst & 3; it > 0; --it) {
+                for (int it = left & 3; it > 0; --it) {
                     JP_FWD_STEP(0, a2_0)
                     fk += 1.f;
                     row += P * 8u;
@@ -212,7 +310,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
         __syncthreads();
     }
 #pragma unroll
-    for (int m = 0; m < kPerThread; ++m) p[j0 + m * kThreads + tid] = zr[m].cf * (acc0[m] + acc1[m]);
+    for (int m = 0; m < kPerThread; ++m) p[j0 + map_fwd(m * kThreads + tid, L)] = zr[m].cf * (acc0[m] + acc1[m]);
 }
 #undef JP_FWD_STEP
 
@@ -237,26 +335,29 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
 template <int P>
 __global__ void __launch_bounds__(kThreads, JP_MINB)
     k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
-                float *__restrict__ img)
+                int lane_map, float *__restrict__ img)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int *Ci = reinterpret_cast<int *>(smem_raw);                                        // [rows_cap][P]
     RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(int)); // [max(n0,n1)]
     __shared__ Track trk;
     __shared__ float red[kThreads / 32];
+    __shared__ int sh_len[2];
     const int tid = threadIdx.x;
     const int64_t j0 = blockIdx.x * (int64_t)kTile;
 
     prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
+    int jm[kPerThread];
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
-        const int64_t j = j0 + m * kThreads + tid;
+        jm[m] = m * kThreads + tid;
+        const int64_t j = j0 + jm[m];
         zs[m] = (j < n) ? l.zs[j] : 0.f;
         ze[m] = (j < n) ? l.ze[j] : 0.f;
     }
     const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (!tile_is_track(l, j0, n, zs, ze, xs0, ys0, xe0, ye0)) {
+    if (!tile_is_track(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
 #pragma unroll 1
         for (int m = 0; m < kPerThread; ++m) {
             const int64_t j = j0 + m * kThreads + tid;
@@ -268,6 +369,15 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
     __syncthreads();
     const Track t = trk;
     if (t.I1 < t.I0) return;
+    const int L = lane_map ? detect_row_length(l, j0, n, sh_len) : 0;
+    if (L) {
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            jm[m] = map_back(m * kThreads + tid, L);
+            zs[m] = l.zs[j0 + jm[m]];
+            ze[m] = l.ze[j0 + jm[m]];
+        }
+    }
     const int n2 = g.n[2];
 
     ZRay zr[kPerThread];
@@ -276,7 +386,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
         zr[m] = z_setup(g, t, zs[m], ze[m]);
-        x[m] = zr[m].cf * y[j0 + m * kThreads + tid];
+        x[m] = zr[m].cf * y[j0 + jm[m]];
         if (zr[m].i1 >= zr[m].i0) xmax = fmaxf(xmax, fabsf(x[m]));
     }
     // block max of |x|
@@ -380,6 +490,13 @@ namespace {
 #endif
 constexpr size_t kSmemBudget = JP_SMEM_KB * 1024; // per CTA: four CTAs per SM
 
+// JP_LANE_MAP=0 in the environment switches the lane mapping off (A/B measurements; results are the same)
+int lane_map_on()
+{
+    const char *e = getenv("JP_LANE_MAP");
+    return !(e && e[0] == '0');
+}
+
 struct TileCfg {
     int P;        // row pitch (0: image too wide along z for the tiled kernels)
     int rows_cap; // rows per chunk
@@ -435,7 +552,7 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
     JP_DISPATCH_P(c, {
         cudaError_t e = set_smem(k_fwd_tile<P>, c.smem);
         if (e != cudaSuccess) return e;
-        k_fwd_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok, p);
+        k_fwd_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok, lane_map_on(), p);
     })
     return cudaGetLastError();
 }
@@ -449,7 +566,7 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
     JP_DISPATCH_P(c, {
         cudaError_t e = set_smem(k_back_tile<P>, c.smem);
         if (e != cudaSuccess) return e;
-        k_back_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok, img);
+        k_back_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok, lane_map_on(), img);
     })
     return cudaGetLastError();
 }

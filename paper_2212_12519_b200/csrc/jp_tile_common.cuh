@@ -26,6 +26,7 @@ struct Track {
     double inv_dp;  // 1 / d_p
     double ops;     // o_p - s_p
     float R;        // 1 + (d_q1/d_p)^2
+    double iv2;     // 1 / v_2 (axial voxel size), the same for every LOR of the tile
 };
 
 // q1 cell of one plane of the track (shared by the whole tile): element offsets of the two image rows
@@ -87,6 +88,7 @@ static __device__ void track_setup(const Geom &g, float xs, float ys, float xe, 
     t.inv_dp = inv_dp;
     t.ops = op - sp;
     t.R = (float)(1.0 + ratio * ratio);
+    t.iv2 = drcp((double)g.v[2]);
 }
 
 __device__ __forceinline__ RowInfo row_info(const Geom &g, const Track &t, int i)
@@ -114,25 +116,27 @@ struct ZRay {
     float a2, b2, cf;
 };
 
-__device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs, float ze)
+// kc: the returned a2 is u2 - kc (kc an integer-valued shift, 0 for the (value, slope) kernels)
+__device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs, float ze, double kc = 0.0)
 {
     ZRay z;
     const double dz = (double)ze - (double)zs;
     const double rz = dz * t.inv_dp;
     const double vp = (double)g.v[t.p];
-    const double iv2 = drcp((double)g.v[2]);
+    const double iv2 = t.iv2;
     const double B = rz * vp * iv2;
-    const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2;
+    const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2 - kc;
     const float rzf = (float)rz;
     z.cf = g.v[t.p] * sqrtf(fmaf(rzf, rzf, t.R));
     // clip to -1 < u2 < n2 (float32 estimate widened by one plane, then trimmed against the padded row)
     int ilo = t.I0, ihi = t.I1;
-    const float Af = (float)A, Bf = (float)B, n2 = (float)g.n[2];
+    const float kcf = (float)kc;
+    const float Af = (float)A, Bf = (float)B, lo = -1.f - kcf, hi = (float)g.n[2] - kcf;
     if (Bf == 0.f) {
-        if (Af <= -1.f || Af >= n2) ihi = ilo - 1;
+        if (Af <= lo || Af >= hi) ihi = ilo - 1;
     } else {
         const float inv = 1.f / Bf;
-        const float ia = (-1.f - Af) * inv, ib = (n2 - Af) * inv;
+        const float ia = (lo - Af) * inv, ib = (hi - Af) * inv;
         const float imin = fminf(fmaxf(floorf(fminf(ia, ib)) - 1.f, -1.f), (float)g.n[t.p]);
         const float imax = fminf(fmaxf(ceilf(fmaxf(ia, ib)) + 1.f, -1.f), (float)g.n[t.p]);
         ilo = max(ilo, (int)imin);
@@ -142,7 +146,7 @@ __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs,
     z.a2 = (float)(A + B * (double)ilo);
     // trim: floor(u2) must stay inside the padded row: -2 <= floor(u2) <= n2 (planes trimmed away have
     // all four neighbours outside the image and contribute exactly zero)
-    const float umin = -1.9f, umax = n2 + 0.9f;
+    const float umin = lo - 0.9f, umax = hi + 0.9f;
     while (ilo <= ihi) {
         if (z.a2 > umin && z.a2 < umax) break;
         ++ilo;
@@ -160,10 +164,14 @@ __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs,
 
 // ---- (value, slope) rows of planes [c0, c0 + rows) of track t:  C[z] = wa f[i,k1,z] + wb f[i,k1+1,z],
 // pair = (C[z], C[z+1] - C[z]), columns z = -1 .. n2-1 at C2[r * P + kPad + z]  (all threads of the CTA)
-template <int P>
+// ICPT: store (intercept, slope) instead of (value, slope): pair(z) = (C[z] - (z - kc) D[z], D[z]), D[z] = C[z+1] - C[z],
+// so that the interpolant at axial coordinate u (cell z = floor(u)) is  pair.x + (u - kc) pair.y  with no
+// fractional part needed; kc (an integer, the middle of the axial range) keeps |u - kc| small.
+template <int P, bool ICPT = false>
 __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, const float *__restrict__ img, const Track &t,
-                                           int c0, int rows, int n2, int vec_ok)
+                                           int c0, int rows, int n2, int vec_ok, float kc = 0.f)
 {
+    auto mk = [&](float v, float d, float zrel) { return ICPT ? make_float2(fmaf(-zrel, d, v), d) : make_float2(v, d); };
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
         if (vec_ok) {
             // one warp per row, lanes along z in groups of four voxels; kRB rows in flight per warp
@@ -202,9 +210,12 @@ __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, con
                         }
                         if (act) {
                             float4 *dst = reinterpret_cast<float4 *>(C2 + r * P + kPad + 4 * gq);
-                            dst[0] = make_float4(c0v, c1v - c0v, c1v, c2v - c1v);
-                            dst[1] = make_float4(c2v, c3v - c2v, c3v, c4v - c3v);
-                            if (gq == 0) C2[r * P + kPad - 1] = make_float2(0.f, c0v);
+                            const float z0 = (float)(4 * gq) - kc;
+                            const float2 e0 = mk(c0v, c1v - c0v, z0), e1 = mk(c1v, c2v - c1v, z0 + 1.f);
+                            const float2 e2 = mk(c2v, c3v - c2v, z0 + 2.f), e3 = mk(c3v, c4v - c3v, z0 + 3.f);
+                            dst[0] = make_float4(e0.x, e0.y, e1.x, e1.y);
+                            dst[1] = make_float4(e2.x, e2.y, e3.x, e3.y);
+                            if (gq == 0) C2[r * P + kPad - 1] = mk(0.f, c0v, -1.f - kc);
                         }
                     }
                 }
@@ -225,7 +236,7 @@ __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, con
                     const float fb = (ri.base_b >= 0) ? __ldg(img + ri.base_b + z + 1) : 0.f;
                     v1 = fmaf(ri.wb, fb, ri.wa * fa);
                 }
-                C2[r * P + kPad + z] = make_float2(v0, v1 - v0);
+                C2[r * P + kPad + z] = mk(v0, v1 - v0, (float)z - kc);
             }
         }
 }
