@@ -178,6 +178,30 @@ int jp_gauss3d(const float *in, float *out, const jp_geom *geom, float sigma_mm,
 int jp_lm_osem_planned_res(const jp_plan *plan, const float *sens, float *img, int n_iter, float res_sigma_mm,
                            float res_n_sigmas, void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- TOF sinogram OSEM with multiplicative factors and additive contamination -------- */
+/* PAPER.md:80 ("the projection work required for an OSEM subset update"), :118 (sinogram OSEM keeps "the complete
+ * image volume, the emission sinogram, the forward projection and the contamination sinogram" on the GPU).  Model
+ *     ybar[j][k] = mult[j] (A x)[j][k] + contam[j][k]
+ * (mult: attenuation x normalisation per LOR; contam: randoms + scatter per LOR and TOF bin).  Readings S1-S3:
+ *   S1  subset m = LORs [subset_offsets[m], subset_offsets[m+1]) of `lors` (the caller arranges the list subset-major,
+ *       e.g. every n_subsets-th view of a ring scanner), m = 0..n_subsets-1 in order;
+ *   S2  r[j][k] = mult[j] y[j][k] / ybar[j][k]  if ybar[j][k] > 1e-9 else 0;
+ *   S3  x <- x (A_m^T r) / sens_m  where sens_m > 0, else 0;   sens_m = A_m^T (mult (x) 1_bins).
+ * subset_offsets: HOST array of n_subsets + 1 non-decreasing offsets in [0, lors->n].  y, contam: device,
+ * [lors->n][n_tofbins]; mult: device [lors->n]; mult or contam may be NULL (= 1, = 0).  sens: device
+ * [n_subsets][n0*n1*n2].  img: in = start image, out = result.  workspace: device, at least
+ * jp_sino_osem_tof_workspace_bytes() bytes (the ratio sinogram of the largest subset).  The forward projection
+ * writes the ratio directly (fused epilogue); everything is asynchronous on `stream`, no host synchronisation. */
+size_t jp_sino_osem_tof_workspace_bytes(const int64_t *subset_offsets, int n_subsets, int64_t n, const jp_tof *tof);
+/* sens[m] = A_m^T (mult (x) 1_bins) for every subset; OVERWRITES sens.  workspace may be NULL unless the TOF
+ * kernel is wider than the fused kernels support (then as for jp_sino_osem_tof). */
+int jp_sino_sens_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *mult,
+                     const jp_geom *geom, const jp_tof *tof, float *sens, void *workspace, size_t workspace_bytes,
+                     void *stream);
+int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *y,
+                     const float *mult, const float *contam, const float *sens, const jp_geom *geom, const jp_tof *tof,
+                     float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- hybrid mode: HOST pointers in and out ---------------------------------------- */
 /* Same semantics as jp_fwd / jp_back, but every pointer (inside lors_host too) is a HOST pointer.  The
  * LOR list is streamed through the current CUDA device in chunks on two internal streams (copies

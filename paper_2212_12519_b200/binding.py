@@ -72,6 +72,12 @@ EXPORTS = {
     "jp_lm_osem_planned_res": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_float, C.c_float, C.c_void_p,
                                          C.c_size_t, C.c_void_p]),
     "jp_gauss3d": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_float, C.c_float, C.c_void_p]),
+    "jp_sino_osem_tof_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int64, C.POINTER(jp_tof)]),
+    "jp_sino_sens_tof": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_int, C.c_void_p, C.POINTER(jp_geom),
+                                   C.POINTER(jp_tof), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "jp_sino_osem_tof": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                   C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p, C.c_int, C.c_void_p,
+                                   C.c_size_t, C.c_void_p]),
     "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
@@ -419,6 +425,63 @@ def jp_gauss3d(img, voxsize, sigma_mm: float, n_sigmas: float = 3.0, out=None, s
 
 
 # ---- hybrid mode: host tensors in and out -------------------------------------------------------
+# ---- TOF sinogram OSEM (multiplicative factors + additive contamination) -----------------------------------------
+def _offsets(subset_offsets):
+    off = (C.c_int64 * len(subset_offsets))(*[int(o) for o in subset_offsets])
+    return off, len(subset_offsets) - 1
+
+
+def _opt(t, numel, what):
+    if t is None:
+        return None
+    _dev(t, torch.float32, what)
+    assert t.numel() == numel and t.is_contiguous(), what
+    return t.data_ptr()
+
+
+def jp_sino_osem_tof_workspace_bytes(subset_offsets, n: int, tof: jp_tof) -> int:
+    off, ns = _offsets(subset_offsets)
+    return int(load().jp_sino_osem_tof_workspace_bytes(off, ns, int(n), C.byref(tof)))
+
+
+def jp_sino_sens_tof(xstart, xend, subset_offsets, mult, n, origin, voxsize, tof: jp_tof, out=None, workspace=None,
+                     stream=None) -> torch.Tensor:
+    """sens[m] = A_m^T (mult x 1_bins) for every subset: float32 [n_subsets, n0, n1, n2] (overwritten)"""
+    l, keep = make_lors(xstart, xend)
+    off, ns = _offsets(subset_offsets)
+    shape = tuple(int(x) for x in n)
+    if out is None:
+        out = torch.empty((ns,) + shape, dtype=torch.float32, device=xstart.device)
+    _dev(out, torch.float32, "sens")
+    assert out.shape == (ns,) + shape and out.is_contiguous()
+    g = make_geom(shape, origin, voxsize)
+    wp, wb = (workspace.data_ptr(), workspace.numel() * workspace.element_size()) if workspace is not None else (None, 0)
+    _check(load().jp_sino_sens_tof(C.byref(l), off, ns, _opt(mult, l.n, "mult"), C.byref(g), C.byref(tof),
+                                   out.data_ptr(), wp, wb, _stream(stream)), "jp_sino_sens_tof")
+    return out
+
+
+def jp_sino_osem_tof(xstart, xend, subset_offsets, y, mult, contam, sens, img, origin, voxsize, tof: jp_tof,
+                     n_iter: int, workspace=None, stream=None) -> torch.Tensor:
+    """TOF sinogram OSEM in place on ``img`` (start image in, result out); returns img."""
+    l, keep = make_lors(xstart, xend)
+    off, ns = _offsets(subset_offsets)
+    img = _img(img)
+    _dev(sens, torch.float32, "sens")
+    assert sens.shape == (ns,) + tuple(img.shape) and sens.is_contiguous()
+    g = make_geom(img.shape, origin, voxsize)
+    nb = int(tof.n_tofbins)
+    need = int(load().jp_sino_osem_tof_workspace_bytes(off, ns, int(l.n), C.byref(tof)))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=img.device)
+    assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= need
+    _check(load().jp_sino_osem_tof(C.byref(l), off, ns, _opt(y, l.n * nb, "y"), _opt(mult, l.n, "mult"),
+                                   _opt(contam, l.n * nb, "contam"), sens.data_ptr(), C.byref(g), C.byref(tof),
+                                   img.data_ptr(), int(n_iter), workspace.data_ptr(),
+                                   workspace.numel() * workspace.element_size(), _stream(stream)), "jp_sino_osem_tof")
+    return img
+
+
 def _host_lors(xstart: torch.Tensor, xend: torch.Tensor):
     for t in (xstart, xend):
         if t.is_cuda or t.dtype != torch.float32 or t.ndim != 2 or t.shape[0] != 3:

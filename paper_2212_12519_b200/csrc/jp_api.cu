@@ -686,4 +686,124 @@ int jp_gauss3d(const float *in, float *out, const jp_geom *geom, float sigma_mm,
     return JP_OK;
 }
 
+// ---- TOF sinogram OSEM -------------------------------------------------------------------
+static int check_subsets(const int64_t *off, int n_subsets, int64_t n, int64_t *max_count)
+{
+    if (!off) return fail(JP_ERR_POINTER, "subset_offsets is NULL");
+    if (n_subsets < 1) return fail(JP_ERR_SIZE, "n_subsets < 1");
+    int64_t mx = 0;
+    if (off[0] < 0 || off[n_subsets] > n) return fail(JP_ERR_SIZE, "subset_offsets outside [0, n]");
+    for (int m = 0; m < n_subsets; ++m) {
+        if (off[m + 1] < off[m]) return fail(JP_ERR_SIZE, "subset_offsets not non-decreasing");
+        if (off[m + 1] - off[m] > mx) mx = off[m + 1] - off[m];
+    }
+    *max_count = mx;
+    return JP_OK;
+}
+
+static jp::Lors lors_at(const jp::Lors &l, int64_t a)
+{
+    return jp::Lors{l.xs + a, l.ys + a, l.zs + a, l.xe + a, l.ye + a, l.ze + a};
+}
+
+size_t jp_sino_osem_tof_workspace_bytes(const int64_t *subset_offsets, int n_subsets, int64_t n, const jp_tof *tof)
+{
+    int64_t mx = 0;
+    if (!tof || tof->n_tofbins < 1 || check_subsets(subset_offsets, n_subsets, n, &mx) != JP_OK) return 0;
+    return (size_t)(mx * tof->n_tofbins + 64) * sizeof(float);
+}
+
+int jp_sino_sens_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *mult,
+                     const jp_geom *geom, const jp_tof *tof, float *sens, void *workspace, size_t workspace_bytes,
+                     void *stream)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_lors(lors, l));
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    int64_t mx = 0;
+    JP_TRY(check_subsets(subset_offsets, n_subsets, lors->n, &mx));
+    if (!sens) return fail(JP_ERR_POINTER, "sens is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    JP_CUDA(cudaMemsetAsync(sens, 0, sizeof(float) * (size_t)nvox * n_subsets, st), "jp_sino_sens_tof (zero)");
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, nullptr, 1, st, "jp_sino_sens_tof (scratch)"));
+    jp::SinoEpi epi;
+    epi.mult_bcast = mult;
+    epi.ones_bcast = mult ? 0 : 1;
+    for (int m = 0; m < n_subsets; ++m) {
+        const int64_t a = subset_offsets[m], cnt = subset_offsets[m + 1] - a;
+        if (cnt == 0) continue;
+        jp::SinoEpi e = epi;
+        if (mult) e.mult_bcast = mult + a;
+        cudaError_t rc = jp::launch_tof_sino_win(true, lors_at(l, a), cnt, nullptr, c.pimg, g, t, nullptr, nullptr, st, &e);
+        if (rc == cudaErrorNotSupported) { // generic kernels: expand mult over the bins in the workspace first
+            if (!workspace || workspace_bytes < (size_t)(cnt * t.nbins) * sizeof(float))
+                return fail(JP_ERR_SIZE, "jp_sino_sens_tof: workspace needed (TOF window wider than the fused kernels)");
+            float *r = (float *)workspace;
+            rc = jp::launch_sino_bcast(r, mult ? mult + a : nullptr, cnt, t.nbins, st);
+            if (rc == cudaSuccess) rc = jp::launch_back_tof_sino(lors_at(l, a), whole(cnt), r, g, t, c.lut, c.pimg, st);
+        }
+        JP_CUDA(rc, "jp_sino_sens_tof");
+        JP_CUDA(jp::padded_add_to(c.pimg, g, sens + (size_t)m * nvox, st), "jp_sino_sens_tof (unpad)");
+        JP_CUDA(cudaMemsetAsync(c.pimg, 0, sizeof(float) * (size_t)jp::padded_voxels(g), st), "jp_sino_sens_tof (clear)");
+    }
+    return JP_OK;
+}
+
+int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *y,
+                     const float *mult, const float *contam, const float *sens, const jp_geom *geom, const jp_tof *tof,
+                     float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_lors(lors, l));
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    int64_t mx = 0;
+    JP_TRY(check_subsets(subset_offsets, n_subsets, lors->n, &mx));
+    if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
+    if (!sens || !img || !workspace || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "NULL argument");
+    if (workspace_bytes < jp_sino_osem_tof_workspace_bytes(subset_offsets, n_subsets, lors->n, tof))
+        return fail(JP_ERR_SIZE, "workspace too small");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    const int nb = t.nbins;
+    float *r = (float *)workspace;
+    TofCtx cx, cb; // cx.pimg = padded x, cb.pimg = padded b
+    JP_TRY(tof_ctx_init(cx, t, g, img, 0, st, "jp_sino_osem_tof (scratch)"));
+    cb.st = st;
+    JP_CUDA(jp::padded_create(nullptr, g, true, st, &cb.pimg), "jp_sino_osem_tof (scratch)");
+    for (int it = 0; it < n_iter; ++it) {
+        for (int m = 0; m < n_subsets; ++m) {
+            const int64_t a = subset_offsets[m], cnt = subset_offsets[m + 1] - a;
+            if (cnt > 0) {
+                const jp::Lors ls = lors_at(l, a);
+                jp::SinoEpi e;
+                e.y_em = y + (size_t)a * nb;
+                e.mult = mult ? mult + a : nullptr;
+                e.contam = contam ? contam + (size_t)a * nb : nullptr;
+                cudaError_t rc = jp::launch_tof_sino_win(false, ls, cnt, cx.pimg, nullptr, g, t, r, nullptr, st, &e);
+                if (rc == cudaErrorNotSupported) {
+                    rc = jp::launch_fwd_tof_sino(ls, whole(cnt), cx.pimg, g, t, cx.lut, r, st);
+                    if (rc == cudaSuccess) rc = jp::launch_sino_ratio(r, e.y_em, e.mult, e.contam, cnt, nb, st);
+                }
+                JP_CUDA(rc, "jp_sino_osem_tof (forward)");
+                rc = jp::launch_tof_sino_win(true, ls, cnt, nullptr, cb.pimg, g, t, nullptr, r, st);
+                if (rc == cudaErrorNotSupported) rc = jp::launch_back_tof_sino(ls, whole(cnt), r, g, t, cx.lut, cb.pimg, st);
+                JP_CUDA(rc, "jp_sino_osem_tof (back)");
+            }
+            JP_CUDA(jp::launch_osem_update_padded(img, cx.pimg, cb.pimg, sens + (size_t)m * nvox, 1.f, g, st),
+                    "jp_sino_osem_tof (update)");
+        }
+    }
+    return JP_OK;
+}
+
 } // extern "C"

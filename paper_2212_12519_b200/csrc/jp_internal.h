@@ -44,8 +44,27 @@ cudaError_t launch_back_tof_sino(const Lors &l, Range rg, const float *y, const 
                                  const TofLut &lut, float *img, cudaStream_t st);
 
 // sliding-window TOF sinogram kernels (jp_tof_sino.cu); cudaErrorNotSupported: window wider than compiled
+// optional fused stages of the sliding-window kernels (all pointers may be null = plain projection):
+//   forward, y_em set: the OSEM ratio  r = mult y_em / (mult p + contam) if that > 1e-9 else 0  is written
+//                      instead of p (reading S2; mult per LOR, contam per LOR and bin, either may be null);
+//   back, mult_bcast set: the value of every bin of LOR j is mult_bcast[j] (sensitivity image A^T (mult x 1)),
+//                      y is not read.
+struct SinoEpi {
+    const float *y_em = nullptr;
+    const float *mult = nullptr;
+    const float *contam = nullptr;
+    const float *mult_bcast = nullptr;
+    int ones_bcast = 0; // back: every bin of every LOR is 1 (sensitivity without multiplicative factors)
+};
+
 cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g,
-                                const Tof &t, float *p, const float *y, cudaStream_t st);
+                                const Tof &t, float *p, const float *y, cudaStream_t st, const SinoEpi *epi = nullptr);
+
+// r <- mult y / (mult r + contam) (reading S2) and r <- mult broadcast over the bins: the unfused stages used
+// with the generic TOF sinogram kernels
+cudaError_t launch_sino_ratio(float *r, const float *y, const float *mult, const float *contam, int64_t n, int nbins,
+                              cudaStream_t st);
+cudaError_t launch_sino_bcast(float *r, const float *mult, int64_t n, int nbins, cudaStream_t st);
 
 // lm_mode: 0 = p = A x;  1 = p = (A x > 1e-9) ? 1/(A x) : 0   (OSEM ratio fused into the epilogue)
 cudaError_t launch_fwd_tof_lm(const Lors &l, const int16_t *tofbin, Range rg, const float *img, const Geom &g,

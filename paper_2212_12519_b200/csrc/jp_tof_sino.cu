@@ -167,7 +167,7 @@ __device__ __forceinline__ void walk(const PRay &q, const GTab &gt, uint32_t tab
 template <int NBW, bool BACK>
 __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
     k_tof_sino_win(Lors l, int64_t n, int64_t nblocks, const float *__restrict__ pimg_r, float *__restrict__ pimg_w,
-                   Geom g, Tof t, GTab gt, float *__restrict__ p, const float *__restrict__ y)
+                   Geom g, Tof t, GTab gt, float *__restrict__ p, const float *__restrict__ y, SinoEpi epi)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);                                       // [(kGK + 2)][NBW]
@@ -208,9 +208,14 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
             continue;
         }
         if (BACK) { // stage y[j0 .. j0 + nvalid)[nbins]: one warp per LOR, lanes along the bins
-            const float *in = y + j0 * nbins;
-            for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
-                for (int kb = lane; kb < nbins; kb += 32) stage[kb * kSLd + lor] = in[lor * nbins + kb];
+            if (epi.mult_bcast || epi.ones_bcast) {
+                const float v = (tid < nvalid) ? (epi.mult_bcast ? epi.mult_bcast[j0 + tid] : 1.f) : 0.f;
+                for (int kb = 0; kb < nbins; ++kb) stage[kb * kSLd + tid] = v;
+            } else {
+                const float *in = y + j0 * nbins;
+                for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
+                    for (int kb = lane; kb < nbins; kb += 32) stage[kb * kSLd + lor] = in[lor * nbins + kb];
+            }
             __syncthreads();
         }
         if (q.nk > 0) {
@@ -222,11 +227,25 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
         __syncthreads();
         if (!BACK) { // write the tile (and clear it for the next block)
             float *out = p + j0 * nbins;
-            for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
-                for (int kb = lane; kb < nbins; kb += 32) {
-                    out[lor * nbins + kb] = stage[kb * kSLd + lor];
-                    stage[kb * kSLd + lor] = 0.f;
+            if (epi.y_em) { // OSEM ratio instead of the projection (reading S2)
+                const float *ye = epi.y_em + j0 * nbins;
+                const float *ct = epi.contam ? epi.contam + j0 * nbins : nullptr;
+                for (int lor = warp; lor < nvalid; lor += kSBlock / 32) {
+                    const float mj = epi.mult ? epi.mult[j0 + lor] : 1.f;
+                    for (int kb = lane; kb < nbins; kb += 32) {
+                        const int x = lor * nbins + kb;
+                        const float yb = fmaf(mj, stage[kb * kSLd + lor], ct ? ct[x] : 0.f);
+                        out[x] = (yb > 1e-9f) ? mj * ye[x] / yb : 0.f;
+                        stage[kb * kSLd + lor] = 0.f;
+                    }
                 }
+            } else {
+                for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
+                    for (int kb = lane; kb < nbins; kb += 32) {
+                        out[lor * nbins + kb] = stage[kb * kSLd + lor];
+                        stage[kb * kSLd + lor] = 0.f;
+                    }
+            }
             __syncthreads();
         }
     }
@@ -248,7 +267,7 @@ size_t win_smem(int nbw, int nbins) { return (size_t)(kGK + 2) * nbw * sizeof(fl
 
 template <int NBW, bool BACK>
 cudaError_t launch_win(const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g, const Tof &t,
-                       const GTab &gt, float *p, const float *y, cudaStream_t st)
+                       const GTab &gt, float *p, const float *y, const SinoEpi &epi, cudaStream_t st)
 {
     const size_t smem = win_smem(NBW, t.nbins);
     auto kern = k_tof_sino_win<NBW, BACK>;
@@ -263,7 +282,7 @@ cudaError_t launch_win(const Lors &l, int64_t n, const float *pimg_r, float *pim
     const int64_t nblocks = (n + kSBlock - 1) / kSBlock;
     const int64_t cap = (int64_t)nsm * per_sm;
     const unsigned grid = (unsigned)(nblocks < cap ? nblocks : cap);
-    kern<<<grid, kSBlock, smem, st>>>(l, n, nblocks, pimg_r, pimg_w, g, t, gt, p, y);
+    kern<<<grid, kSBlock, smem, st>>>(l, n, nblocks, pimg_r, pimg_w, g, t, gt, p, y, epi);
     return cudaGetLastError();
 }
 
@@ -272,8 +291,9 @@ cudaError_t launch_win(const Lors &l, int64_t n, const float *pimg_r, float *pim
 // returns cudaErrorNotSupported when the TOF window is wider than the compiled sizes or the tile does not fit
 // in shared memory (the caller then uses the generic kernels of jp_kernels.cu)
 cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g,
-                                const Tof &t, float *p, const float *y, cudaStream_t st)
+                                const Tof &t, float *p, const float *y, cudaStream_t st, const SinoEpi *epi_in)
 {
+    const SinoEpi epi = epi_in ? *epi_in : SinoEpi{};
     if (n == 0) return cudaSuccess;
     double R;
     const int nbw = window_bins(t, &R);
@@ -289,8 +309,8 @@ cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float
     if (e == cudaSuccess) {
 #define JP_WIN(NB)                                                                                           \
     case NB:                                                                                                 \
-        e = back ? launch_win<NB, true>(l, n, pimg_r, pimg_w, g, t, gt, p, y, st)                             \
-                 : launch_win<NB, false>(l, n, pimg_r, pimg_w, g, t, gt, p, y, st);                           \
+        e = back ? launch_win<NB, true>(l, n, pimg_r, pimg_w, g, t, gt, p, y, epi, st)                             \
+                 : launch_win<NB, false>(l, n, pimg_r, pimg_w, g, t, gt, p, y, epi, st);                           \
         break;
         switch (nbw) {
             JP_WIN(4)
@@ -303,6 +323,40 @@ cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float
     }
     cudaFreeAsync(tab, st);
     return e;
+}
+
+// ---- unfused stages for the generic TOF sinogram kernels (TOF window wider than the compiled register windows) ----
+namespace {
+__global__ void k_sino_ratio(float *__restrict__ r, const float *__restrict__ y, const float *__restrict__ mult,
+                             const float *__restrict__ contam, int64_t n, int nbins)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n * nbins) return;
+    const float mj = mult ? mult[i / nbins] : 1.f;
+    const float yb = fmaf(mj, r[i], contam ? contam[i] : 0.f);
+    r[i] = (yb > 1e-9f) ? mj * y[i] / yb : 0.f;
+}
+__global__ void k_sino_bcast(float *__restrict__ r, const float *__restrict__ mult, int64_t n, int nbins)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n * nbins) return;
+    r[i] = mult ? mult[i / nbins] : 1.f;
+}
+} // namespace
+
+cudaError_t launch_sino_ratio(float *r, const float *y, const float *mult, const float *contam, int64_t n, int nbins,
+                              cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_sino_ratio<<<(unsigned)((n * nbins + 255) / 256), 256, 0, st>>>(r, y, mult, contam, n, nbins);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sino_bcast(float *r, const float *mult, int64_t n, int nbins, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_sino_bcast<<<(unsigned)((n * nbins + 255) / 256), 256, 0, st>>>(r, mult, n, nbins);
+    return cudaGetLastError();
 }
 
 } // namespace jp
