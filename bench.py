@@ -58,6 +58,11 @@ SPEC = {
             workload="configs[3]: TOF listmode fwd+back, 40000000 events sampled from the phantom (crystal-snapped "
                      "end points, int16 TOF bin), sorted once by the listmode plan; results in caller order",
             l2="inputs (1.04 GB of sorted events + 0.32 GB of per-event values per step) exceed the 126 MB L2; no flush"),
+    5: dict(metric="LORs/s (TOF sinogram OSEM with mult / contam, one full iteration of 16 subsets)", unit="LORs/s",
+            workload="SURVEY 8(f) row 3: TOF sinogram OSEM on the full configs[1] sinogram x 29 TOF bins (151584768 LORs, "
+                     "17.6 GB emission + 17.6 GB contamination sinograms resident in HBM), 16 subsets of 16 views (the "
+                     "configs[2] subset structure), multiplicative factors per LOR; one step = one full iteration",
+            l2="every iteration streams 3.6 GB of end points and 35 GB of sinograms; no flush"),
     4: dict(metric="events/s (TOF listmode OSEM, one full iteration of 20 subsets)", unit="events/s",
             workload="configs[4]: listmode OSEM on the configs[3] events, 20 subsets, sens = non-TOF A^T 1 over all "
                      "configs[1] LORs; one step = one full iteration (20 x (fwd, ratio, back, update))",
@@ -140,6 +145,18 @@ def time_oracle(config: int, steps: int, warmup: int):
         y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 101).numpy().astype(np.float64)
         f = lambda: oracle.fwd(xs, xe, ph, G.origin, G.voxsize)
         b = lambda: oracle.back(xs, xe, y, G.n, G.origin, G.voxsize)
+    elif config == 5:
+        xs, xe = inputs.sinogram_lors(views=inputs.SUBSET_VIEWS)
+        xs, xe = xs[:, ::24].contiguous().numpy(), xe[:, ::24].contiguous().numpy()
+        n = xs.shape[1]
+        desc = ("one OSEM subset update (fwd, ratio, back, image update) with mult and contam on every 24th LOR of one "
+                "16-view subset = %d LORs x 29 TOF bins (float64, numpy + OpenMP projectors)" % n)
+        rng = np.random.default_rng(5)
+        y5, m5, c5 = rng.random((n, 29)), rng.uniform(0.2, 1.0, n), np.full((n, 29), 0.05)
+        s5 = np.ones((1,) + tuple(G.n))
+        f = lambda: oracle.sino_osem_tof(xs, xe, [0, n], y5, m5, c5, s5, np.ones(G.n), G.origin, G.voxsize, *TOF_ARGS,
+                                         n_iter=1)
+        b = lambda: None
     elif config == 2:
         xs, xe = inputs.sinogram_lors(views=inputs.SUBSET_VIEWS)
         xs, xe = xs[:, ::24].contiguous().numpy(), xe[:, ::24].contiguous().numpy()
@@ -181,7 +198,7 @@ def time_oracle(config: int, steps: int, warmup: int):
 def cpu_baseline_dict(config: int, r: dict):
     t = r["fwd_s"] + r["back_s"]
     d = {"value": r["n"] / t, "unit": SPEC[config]["unit"], "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
-    if config != 4:
+    if config < 4:
         d["fwd_per_s"] = r["n"] / r["fwd_s"]
         d["back_per_s"] = r["n"] / r["back_s"]
     return d
@@ -220,7 +237,26 @@ class Workload:
         self.bimg = torch.zeros(G.n, dtype=torch.float32, device=dev)
         self.plan = None
         self.plan_s = None
-        if c in (1, 2):
+        if c == 5:
+            nsub = 16
+            order = [m + nsub * k for m in range(nsub) for k in range(inputs.N_VIEWS // nsub)]   # subset-major views
+            self.xs, self.xe = inputs.sinogram_lors(views=order, device=dev)
+            self.n = self.xs.shape[1]
+            per = self.n // nsub
+            self.off = [m * per for m in range(nsub + 1)]
+            nb = TOFP.n_tofbins
+            self.y = inputs.uniform_values((self.n, nb), 0.0, 1.0, seed=inputs.BASE_SEED + 105 + rank, device=dev)
+            self.contam = torch.full((self.n, nb), 0.05, dtype=torch.float32, device=dev)
+            self.mult = inputs.uniform_values(self.n, 0.2, 1.0, seed=inputs.BASE_SEED + 205 + rank, device=dev)
+            self.ws = torch.empty(jp.jp_sino_osem_tof_workspace_bytes(self.off, self.n, self.tof), dtype=torch.uint8,
+                                  device=dev)
+            self.sens = jp.jp_sino_sens_tof(self.xs, self.xe, self.off, self.mult, G.n, G.origin, G.voxsize, self.tof)
+            self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
+            self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
+            self.kinds = ("sino", "sino")
+            self.launches = nsub * 3 + 4
+            self.hbm_bytes = self.n * (24 + 4 + 4 * 4 * nb) // 2   # per direction: end points, y + contam in, r out / r in
+        elif c in (1, 2):
             self.xs, self.xe = inputs.sinogram_lors(views=None if c == 1 else inputs.SUBSET_VIEWS, device=dev)
             self.n = self.xs.shape[1]
             shape = self.n if c == 1 else (self.n, TOFP.n_tofbins)
@@ -270,11 +306,14 @@ class Workload:
             jp.jp_fwd_tof_sino(self.xs, self.xe, self.img, G.origin, G.voxsize, self.tof, out=self.p)
         elif c == 3:
             jp.jp_fwd_tof_lm_planned(self.plan, self.img, out=self.p)
+        elif c == 5:
+            jp.jp_sino_osem_tof(self.xs, self.xe, self.off, self.y, self.mult, self.contam, self.sens, self.x, G.origin,
+                                G.voxsize, self.tof, n_iter=1, workspace=self.ws)
         else:
             jp.jp_lm_osem_planned(self.plan, self.sens, self.x, n_iter=1)
         if ev:
             ev[1].record(s)
-        if c != 4:
+        if c < 4:
             self.bimg.zero_()
         if c == 1:
             jp.jp_back(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
@@ -329,7 +368,7 @@ class Workload:
         return e0.elapsed_time(e1) * 1e-3 / iters
 
     def checksum(self):
-        if self.c == 4:
+        if self.c >= 4:
             return float(self.x.double().sum())
         p = self.p.reshape(-1)
         return float(p[:: max(1, p.numel() // 4096)].double().sum()) + float(self.bimg.double().sum())
@@ -430,10 +469,11 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
     kf, kb = w.kinds
     names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
-             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_fwd_tof_lm_quad + k_back_tof_lm_quad", "")}[w.c]
+             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_fwd_tof_lm_quad + k_back_tof_lm_quad", ""),
+             5: ("k_tof_sino_win<6,fwd+ratio> + k_tof_sino_win<6,back>", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
-    if w.c == 4:
-        lane = 2 * LANE["lm"]
+    if w.c in (4, 5):
+        lane = 2 * LANE["lm" if w.c == 4 else "sino"]
         achieved = lane * w.plane_steps / (fwd_ms * 1e-3)
         return {"bound": "alu", "kernel": names[0], "achieved": achieved / 1e12, "peak": alu_peak / 1e12,
                 "unit": "T lane-instr/s (FP32)", "frac": achieved / alu_peak, "traffic": None, "peak_source": src,
@@ -480,7 +520,7 @@ def run_ours(args):
     checksum = w.checksum()
 
     e2e_s = None
-    if not args.no_e2e:
+    if not args.no_e2e and c != 5:   # configs 5 keeps 40 GB of sinograms resident by design: no host leg
         w.e2e_setup()
         w.e2e_step()
         barrier()
@@ -519,8 +559,9 @@ def run_ours(args):
         line["config"]["plan_s"] = w.plan_s
     if c == 3:
         line["nontof_listmode"] = w.time_nontof_listmode()
-    if c == 4:
+    if c >= 4:
         line["s_per_iteration"] = ms_per_step * 1e-3
+    if c == 4:
         line["s_per_iteration_with_resolution_model"] = w.time_osem_with_resolution_model()
     if e2e_s is not None:
         line["e2e"] = {"value": world * w.n / e2e_s, "unit": SPEC[c]["unit"], "h2d_bytes_per_step": w.h2d,
@@ -532,7 +573,7 @@ def run_ours(args):
         del w
         torch.cuda.empty_cache()
         other = {}
-        for oc in (2, 3, 4):
+        for oc in (2, 3, 4, 5):
             ow = Workload(oc, jp, dev, rank)
             if oc == 4:
                 ow.setup_sens()
@@ -540,7 +581,9 @@ def run_ours(args):
             r = roofline_dict(ow, f_ms, b_ms)
             d = {"units": ow.n, "ms_per_step": t_ms / 3, "per_s": ow.n / (t_ms / 3 * 1e-3), "unit": SPEC[oc]["unit"],
                  "plane_steps": ow.plane_steps, "frac_alu": r["frac"]}
-            if oc == 4:
+            if oc == 5:
+                d["s_per_iteration"] = t_ms / 3 * 1e-3
+            elif oc == 4:
                 d["s_per_iteration"] = t_ms / 3 * 1e-3
                 d["s_per_iteration_with_resolution_model"] = ow.time_osem_with_resolution_model()
             else:
@@ -549,7 +592,7 @@ def run_ours(args):
                 d["nontof_listmode"] = ow.time_nontof_listmode()
             if ow.plan_s is not None:
                 d["plan_s"] = ow.plan_s
-            other[f"configs[{oc}]"] = d
+            other[f"configs[{oc}]" if oc < 5 else "sino_osem_8f3"] = d
             del ow
             torch.cuda.empty_cache()
         line["other_configs"] = other
@@ -564,7 +607,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3, 4])
+    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the brief configs[2..4] runs of the default line")
