@@ -39,11 +39,11 @@ __global__ void k_tof_g1tab(float2 *tab, int n, double W, double m, double isc)
     auto E = [&](double y) { return erf(fmin(fmax(y, -m), m) * isc); };
     auto G = [&](double x) { return 0.5 * (E((x + 0.5) * W) - E((x - 0.5) * W)); };
     const double g0 = G((double)k / kG1K), g1 = G((double)(k + 1) / kG1K);
-    tab[k] = make_float2((float)g0, (float)(g1 - g0));
+    tab[k] = make_float2((float)(g0 - (double)k * (g1 - g0)), (float)(g1 - g0)); // (intercept, slope): G(x) = .x + x .y
 }
 
 struct G1Tab {
-    const float2 *tab; // device, n entries; entry k = (G(k / kG1K), G((k+1) / kG1K) - G(k / kG1K)); zero beyond R
+    const float2 *tab; // device, n entries; entry k = (intercept, slope) of G on [k, k+1] / kG1K; zero beyond R
     int n;
     float scale; // kG1K / W: mm -> table units
     float xmax;  // n - 1.5
@@ -60,9 +60,8 @@ __device__ __forceinline__ float g1_weight(uint32_t gbase, float xmax, float xs)
 {
     const float xa = fminf(fabsf(xs), xmax);
     const float tt = __fadd_rd(xa, kMagic);
-    const float f = xa - (tt - kMagic);
     const float2 v = lds_pair<0>(gbase + (__float_as_uint(tt) << 3));
-    return fmaf(f, v.y, v.x);
+    return fmaf(xa, v.y, v.x);
 }
 
 // per-event axial + TOF part on track t (canonical orientation)
@@ -79,7 +78,7 @@ struct LineExtra {
 
 template <bool TOF>
 __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double Rd, float zs, float ze, float centre,
-                                          float reach, float scale)
+                                          float reach, float scale, double kc = 0.0) // kc: a2 is u2 - kc
 {
     LmRay z;
     const double dz = (double)ze - (double)zs;
@@ -87,7 +86,7 @@ __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double 
     const double vp = (double)g.v[t.p];
     const double iv2 = t.iv2;
     const double B = rz * vp * iv2;
-    const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2;
+    const double A = ((double)zs - (double)g.o[2] + t.ops * rz) * iv2 - kc;
     const double Ln = dsqrt_pos(Rd + rz * rz);   // L / |d_p|
     z.cf = (float)(vp * Ln);
     // tau(i) = ((ops + i vp) inv_dp - 1/2) L,  L = Ln / |inv_dp|
@@ -103,12 +102,13 @@ __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double 
         ilo = max(ilo, (int)imin);
         ihi = min(ihi, (int)imax);
     }
-    const float Af = (float)A, Bf = (float)B, n2 = (float)g.n[2];
+    const float kcf = (float)kc;
+    const float Af = (float)A, Bf = (float)B, ulo = -1.f - kcf, uhi = (float)g.n[2] - kcf;
     if (Bf == 0.f) {
-        if (Af <= -1.f || Af >= n2) ihi = ilo - 1;
+        if (Af <= ulo || Af >= uhi) ihi = ilo - 1;
     } else {
         const float inv = 1.f / Bf;
-        const float ia = (-1.f - Af) * inv, ib = (n2 - Af) * inv;
+        const float ia = (ulo - Af) * inv, ib = (uhi - Af) * inv;
         const float imin = fminf(fmaxf(floorf(fminf(ia, ib)) - 1.f, -1.f), (float)g.n[t.p]);
         const float imax = fminf(fmaxf(ceilf(fmaxf(ia, ib)) + 1.f, -1.f), (float)g.n[t.p]);
         ilo = max(ilo, (int)imin);
@@ -116,7 +116,7 @@ __device__ __forceinline__ LmRay lm_setup(const Geom &g, const Track &t, double 
     }
     z.b2 = Bf;
     z.a2 = (float)(A + B * (double)ilo);
-    const float umin = -1.9f, umax = n2 + 0.9f;
+    const float umin = ulo - 0.9f, umax = uhi + 0.9f;
     while (ilo <= ihi) {
         if (z.a2 > umin && z.a2 < umax) break;
         ++ilo;
@@ -222,10 +222,9 @@ __device__ __forceinline__ int64_t out_index(const int *__restrict__ perm, int64
     {                                                                           \
         const float u = fmaf(b2, fk, A2K);                                      \
         const float tt = __fadd_rd(u, kMagic);                                  \
-        const float w = u - (tt - kMagic);                                      \
         const float2 v = lds_pair<(K) * P * 8>(row + (__float_as_uint(tt) << 3)); \
         const float wt = TOF ? g1_weight(gbase, xmax, fmaf(dx, fk, X0K)) : 1.f; \
-        acc = fmaf(fmaf(w, v.y, v.x), wt, acc);                                 \
+        acc = fmaf(fmaf(u, v.y, v.x), wt, acc);                                 \
     }
 
 template <int P, int LM_MODE, bool TOF>
@@ -282,8 +281,9 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
             C2[r * P + (c < ncl ? c : g.n[2] + kPad + (c - ncl))] = make_float2(0.f, 0.f);
         }
     }
-    const uint32_t c2_base = smem_addr(C2) + kPad * 8u - ((uint32_t)kMagicI << 3);
     const int n2 = g.n[2];
+    const int kci = n2 >> 1; // axial shift of the (intercept, slope) rows (build_rows<P, true>)
+    const uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
 
     for (int k = 0; k < nruns; ++k) {
         const int ra = S.starts[k], rb = S.starts[k + 1];
@@ -337,7 +337,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                         const float tmp = zs; zs = ze; ze = tmp;
                         centre = -centre;
                     }
-                    zr[m] = lm_setup<TOF>(g, trk, Rd, zs, ze, centre, reach, gt.scale);
+                    zr[m] = lm_setup<TOF>(g, trk, Rd, zs, ze, centre, reach, gt.scale, (double)kci);
                     if (zr[m].i1 >= zr[m].i0) {
                         lo = min(lo, zr[m].i0);
                         hi = max(hi, zr[m].i1);
@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
             const int I0 = S.imin, I1 = S.imax;
             for (int cc = I0; cc <= I1; cc += rows_cap) {
                 const int rows = min(rows_cap, I1 - cc + 1);
-                build_rows<P>(C2, rinfo, img, trk, cc, rows, n2, vec_ok);
+                build_rows<P, true>(C2, rinfo, img, trk, cc, rows, n2, vec_ok, (float)kci);
                 __syncthreads();
 #pragma unroll
                 for (int m = 0; m < kPerThread; ++m) {
