@@ -164,6 +164,17 @@ size_t jp_lm_osem_planned_workspace_bytes(const jp_plan *plan);
 int jp_lm_osem_planned(const jp_plan *plan, const float *sens, float *img, int n_iter, void *workspace,
                        size_t workspace_bytes, void *stream);
 
+/* ---- the two halves of one listmode OSEM subset update (multi-GPU) ---------------------------- */
+/* Events are independent units: every GPU holds a plan over its own shard of the event list (shards that start at
+ * a multiple of n_subsets keep "subset = e mod n_subsets") and the whole image.  Per subset each GPU computes
+ *     b = A_m^T r,  r_e = 1/(A x)_e if (A x)_e > 1e-9 else 0        (jp_lm_osem_planned_backratio, OVERWRITES b)
+ * over its events, the caller sums b over the GPUs (one all-reduce of n0*n1*n2 floats, the only exchange step),
+ * and every GPU applies   x <- x b scale / sens  where sens > 0, else 0;  b <- 0    (jp_osem_update).
+ * With one GPU the pair is jp_lm_osem_planned's subset update.  workspace as for jp_lm_osem_planned. */
+int jp_lm_osem_planned_backratio(const jp_plan *plan, int subset, const float *x, float *b, void *workspace,
+                                 size_t workspace_bytes, void *stream);
+int jp_osem_update(float *x, float *b, const float *sens, float scale, const jp_geom *geom, void *stream);
+
 /* ---- image-based resolution model -------------------------------- */
 /* out = G in: 3-D Gaussian of standard deviation sigma_mm (mm; FWHM = 2 sqrt(2 ln 2) sigma; the paper uses
  * 4.5 mm FWHM), taps exp(-(k v_a)^2 / (2 sigma^2)) for |k| <= ceil(n_sigmas sigma / v_a), normalised per axis,

@@ -71,6 +71,9 @@ EXPORTS = {
                                      C.c_void_p]),
     "jp_lm_osem_planned_res": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_float, C.c_float, C.c_void_p,
                                          C.c_size_t, C.c_void_p]),
+    "jp_lm_osem_planned_backratio": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
+                                               C.c_void_p]),
+    "jp_osem_update": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.POINTER(jp_geom), C.c_void_p]),
     "jp_gauss3d": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_float, C.c_float, C.c_void_p]),
     "jp_sino_osem_tof_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int64, C.POINTER(jp_tof)]),
     "jp_sino_sens_tof": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_int, C.c_void_p, C.POINTER(jp_geom),
@@ -409,6 +412,32 @@ def jp_lm_osem_planned_res(plan: LmPlan, sens, img, n_iter: int, res_sigma_mm: f
                                          workspace.numel() * workspace.element_size(), _stream(stream)),
            "jp_lm_osem_planned_res")
     return img
+
+
+def jp_lm_osem_planned_backratio(plan: LmPlan, subset: int, x, out=None, workspace=None, stream=None) -> torch.Tensor:
+    """b = A_m^T (1 / (A_m x)) over the plan's events of one subset (overwrites ``out``): the projection half of an
+    OSEM subset update; sum b over the GPUs, then jp_osem_update."""
+    x = _img(x)
+    if out is None:
+        out = torch.empty_like(x)
+    out = _img(out)
+    need = int(load().jp_lm_osem_planned_workspace_bytes(plan.handle))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=x.device)
+    _check(load().jp_lm_osem_planned_backratio(plan.handle, int(subset), x.data_ptr(), out.data_ptr(),
+                                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                               _stream(stream)), "jp_lm_osem_planned_backratio")
+    return out
+
+
+def jp_osem_update(x, b, sens, scale: float, voxsize=(1.0, 1.0, 1.0), stream=None) -> torch.Tensor:
+    """x <- x b scale / sens where sens > 0, else 0; b <- 0.  In place; returns x."""
+    x, b, sens = _img(x), _img(b), _img(sens)
+    assert x.shape == b.shape == sens.shape
+    g = make_geom(x.shape, (0.0, 0.0, 0.0), voxsize)
+    _check(load().jp_osem_update(x.data_ptr(), b.data_ptr(), sens.data_ptr(), float(scale), C.byref(g),
+                                 _stream(stream)), "jp_osem_update")
+    return x
 
 
 def jp_gauss3d(img, voxsize, sigma_mm: float, n_sigmas: float = 3.0, out=None, stream=None) -> torch.Tensor:

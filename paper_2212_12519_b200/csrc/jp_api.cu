@@ -806,4 +806,63 @@ int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_s
     return JP_OK;
 }
 
+// ---- pieces of one OSEM subset update, for callers that exchange b between the two halves (multi-GPU) ----------
+int jp_lm_osem_planned_backratio(const jp_plan *plan, int subset, const float *x, float *b, void *workspace,
+                                 size_t workspace_bytes, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset < 0 || subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    if (!x || !b || !workspace) return fail(JP_ERR_POINTER, "NULL argument");
+    if (workspace_bytes < jp_lm_osem_planned_workspace_bytes(plan)) return fail(JP_ERR_SIZE, "workspace too small");
+    const char *where = "jp_lm_osem_planned_backratio";
+    cudaStream_t st = (cudaStream_t)stream;
+    PlanCtx c(plan);
+    const int64_t nvox = (int64_t)c.g.n[0] * c.g.n[1] * c.g.n[2];
+    JP_CUDA(cudaMemsetAsync(b, 0, sizeof(float) * (size_t)nvox, st), where);
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    float *r = (float *)workspace + ((nvox + 31) / 32) * 32; // per-event ratios of the subset, in sorted order
+    TofCtx tc;
+    tc.st = st;
+    JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
+    float4 *q[2], *qb[2];
+    const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+    for (int a = 0; a < 2; ++a) {
+        JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
+        JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &qb[a]), where);
+    }
+    const int m = subset;
+    JP_CUDA(jp::launch_quad_build(x, c.g, q[0], q[1], st), where);
+    for (int a = 0; a < 2; ++a)
+        JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, r, 1, st), where);
+    for (int a = 0; a < 2; ++a) {
+        JP_CUDA(cudaMemsetAsync(qb[a], 0, qbytes, st), where);
+        JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, qb[a], st), where);
+    }
+    JP_CUDA(jp::launch_quad_merge(qb[0], qb[1], c.g, b, st), where);
+    if (c.has_axis2(m)) {
+        float *px = nullptr, *pb = nullptr;
+        JP_CUDA(jp::padded_create(x, c.g, false, st, &px), where);
+        cudaError_t e = jp::padded_create(nullptr, c.g, true, st, &pb);
+        if (e == cudaSuccess) e = jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, true), px, c.g, c.t, tc.lut, r, 1, st);
+        if (e == cudaSuccess) e = jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, true), r, c.g, c.t, tc.lut, pb, st);
+        if (e == cudaSuccess) e = jp::padded_add_to(pb, c.g, b, st);
+        jp::padded_destroy(px, st);
+        jp::padded_destroy(pb, st);
+        JP_CUDA(e, where);
+    }
+    return JP_OK;
+}
+
+int jp_osem_update(float *x, float *b, const float *sens, float scale, const jp_geom *geom, void *stream)
+{
+    g_err[0] = 0;
+    jp::Geom g;
+    JP_TRY(check_geom(geom, g));
+    if (!x || !b || !sens) return fail(JP_ERR_POINTER, "NULL argument");
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    JP_CUDA(jp::launch_osem_update(x, b, sens, scale, nvox, (cudaStream_t)stream), "jp_osem_update");
+    return JP_OK;
+}
+
 } // extern "C"

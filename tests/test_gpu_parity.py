@@ -334,6 +334,56 @@ def test_config4_small_osem_planned(cuda_device, scanner, events):
     plan.destroy()
 
 
+def test_osem_over_event_shards(cuda_device, scanner, events):
+    """the multi-GPU OSEM driver (multi_gpu.lm_osem_sharded) on ONE GPU: the event list is cut into
+    the shards two and three ranks would hold (multi_gpu.shard_events), each shard gets its own plan, the per-shard
+    images b are summed where the all-reduce would sum them (sequentially, nothing waits on anything), and the
+    result must be the oracle's OSEM over the whole list.  world_size-2 gloo runs of the same driver: tests/
+    test_sharding_gloo.py."""
+    from paper_2212_12519_b200 import multi_gpu
+    g, ph = scanner
+    xs, xe, tb = events
+    n = xs.shape[1]
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
+    ns = 5
+    sx, se = inputs.sinogram_lors(views=range(0, 256, 8), radial=range(-64, 65, 4))
+    sx, se = sx[:, ::5].contiguous(), se[:, ::5].contiguous()
+    sens32 = oracle.back(sx.numpy(), se.numpy(), np.ones(sx.shape[1]), g.n, g.origin, g.voxsize).astype(np.float32)
+    x0 = np.ones(g.n, dtype=np.float32)
+    ref = oracle.lm_osem(xs.numpy(), xe.numpy(), tb.numpy(), sens32.astype(np.float64), x0, g.origin, g.voxsize,
+                         *args, n_subsets=ns, n_iter=2)
+    sens = dev(sens32, cuda_device)
+    for world in (1, 2, 3):
+        plans = []
+        for r in range(world):
+            lo, hi = multi_gpu.shard_events(n, r, world, ns)
+            plans.append(jp.LmPlan(xs[:, lo:hi].contiguous().to(cuda_device), xe[:, lo:hi].contiguous().to(cuda_device),
+                                   tb[lo:hi].contiguous().to(cuda_device), g.n, g.origin, g.voxsize, tof, n_subsets=ns))
+        shard_ops = [multi_gpu.CudaOps(jp, plan=pl) for pl in plans]
+
+        class AllRanks:      # what the ranks + the all-reduce compute together, one rank after the other
+            def backratio(self, m, x, b):
+                b.zero_()
+                part = torch.empty_like(b)
+                for o in shard_ops:
+                    o.backratio(m, x, part)
+                    b += part            # the all-reduce(sum) of the driver, stood in for on one device
+
+            def update(self, x, b, sens_, scale):
+                shard_ops[0].update(x, b, sens_, scale)
+
+        x = dev(x0, cuda_device).clone()
+        multi_gpu.lm_osem_sharded(AllRanks(), sens, x, ns, 2)
+        got = x.cpu().numpy().astype(np.float64)
+        rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+        mx = np.abs(got - ref).max() / np.abs(ref).max()
+        assert rel <= 1e-4 and mx <= 1e-3, (world, rel, mx)
+        for pl in plans:
+            pl.destroy()
+
+
 @pytest.mark.parametrize("tile", ["1", "0"])
 def test_nontof_listmode_planned(cuda_device, scanner, events, tile, monkeypatch):
     """non-TOF projections of listmode events: unsorted through jp_fwd /
