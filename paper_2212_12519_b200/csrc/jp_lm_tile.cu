@@ -613,7 +613,13 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
 // ---- launchers ----------------------------------------------------------------------------------------------
 namespace {
 
-constexpr size_t kSmemBudget = 54 * 1024;
+#ifndef JP_LMT_SMEM_KB_FWD
+#define JP_LMT_SMEM_KB_FWD 54
+#endif
+#ifndef JP_LMT_SMEM_KB_BACK
+#define JP_LMT_SMEM_KB_BACK 44
+#endif
+constexpr size_t kSmemMax = 64 * 1024;
 
 struct LmTileCfg {
     int P, rows_cap, vec_ok, g1n;
@@ -621,7 +627,7 @@ struct LmTileCfg {
 };
 
 // elem: bytes per row element (8: forward pairs, 4: back fixed point)
-LmTileCfg lm_tile_cfg(const Geom &g, const Tof &t, const void *img, size_t elem)
+LmTileCfg lm_tile_cfg(const Geom &g, const Tof &t, const void *img, size_t elem, size_t kSmemBudget)
 {
     LmTileCfg c{};
     const int need = g.n[2] + kPad + kPadR;
@@ -634,6 +640,7 @@ LmTileCfg lm_tile_cfg(const Geom &g, const Tof &t, const void *img, size_t elem)
     const int np = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
     const size_t fixed = (size_t)np * sizeof(RowInfo) + (size_t)c.g1n * sizeof(float2);
     const size_t row = (size_t)c.P * elem;
+    if (kSmemBudget > kSmemMax) kSmemBudget = kSmemMax;
     size_t rows = fixed + row <= kSmemBudget ? (kSmemBudget - fixed) / row : 0;
     if (rows * row < (size_t)kTile * sizeof(uint4) || rows < 8) { c.P = 0; return c; } // also the run-detection scratch
     if (rows > (size_t)np) rows = (size_t)np;
@@ -686,7 +693,7 @@ cudaError_t launch_fwd_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t
     if (count == 0) return cudaSuccess;
     const bool tof = tofbin != nullptr;
     const Tof t = tof ? t_in : Tof{1.f, 1.f, 1.f, 1, 0.f};
-    const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(float2));
+    const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(float2), JP_LMT_SMEM_KB_FWD * 1024);
     if (!c.P) return cudaErrorNotSupported;
     G1Tab gt{};
     cudaError_t e = tof ? g1tab_create(t, c.g1n, st, &gt) : cudaSuccess;
@@ -695,7 +702,7 @@ cudaError_t launch_fwd_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_t
 #define JP_LM_LAUNCH_FWD(MODE, TOFF)                                                                                   \
     {                                                                                                                  \
         e = cudaFuncSetAttribute(k_fwd_tof_lm_tile<P, MODE, TOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
-                                 (int)kSmemBudget);                                                                    \
+                                 (int)kSmemMax);                                                                    \
         if (e == cudaSuccess)                                                                                          \
             k_fwd_tof_lm_tile<P, MODE, TOFF><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, img, \
                                                                              g, t, gt, c.rows_cap, c.vec_ok, p);       \
@@ -718,7 +725,7 @@ cudaError_t launch_back_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_
     if (count == 0) return cudaSuccess;
     const bool tof = tofbin != nullptr;
     const Tof t = tof ? t_in : Tof{1.f, 1.f, 1.f, 1, 0.f};
-    const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(int));
+    const LmTileCfg c = lm_tile_cfg(g, t, img, sizeof(int), JP_LMT_SMEM_KB_BACK * 1024);
     if (!c.P) return cudaErrorNotSupported;
     G1Tab gt{};
     cudaError_t e = tof ? g1tab_create(t, c.g1n, st, &gt) : cudaSuccess;
@@ -727,7 +734,7 @@ cudaError_t launch_back_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_
 #define JP_LM_LAUNCH_BACK(TOFF)                                                                                         \
     {                                                                                                                   \
         e = cudaFuncSetAttribute(k_back_tof_lm_tile<P, TOFF>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
-                                 (int)kSmemBudget);                                                                     \
+                                 (int)kSmemMax);                                                                     \
         if (e == cudaSuccess)                                                                                           \
             k_back_tof_lm_tile<P, TOFF><<<grid, kThreads, c.smem, st>>>(l, tofbin, first, count, perm, io_off, y, g, t, \
                                                                         gt, c.rows_cap, c.vec_ok, img);                 \

@@ -21,6 +21,10 @@
 
 #include "jp_tile_common.cuh"
 
+#ifndef JP_BACK_MAP
+#define JP_BACK_MAP 0
+#endif // adjoint lane mapping: which neighbouring diagonal the second half-warp takes
+
 namespace jp {
 
 using namespace tile;
@@ -102,7 +106,7 @@ __device__ __forceinline__ int map_back(int idx, int L)
     if (L < 2 || (L & 1) || (kTile % (16 * L))) return idx;
     const int w = idx >> 5, l32 = idx & 31, d = l32 & 15, s = l32 >> 4, half = L >> 1;
     const int rb = w / half, c2 = w - rb * half;
-    int col = 2 * c2 + s + d;
+    int col = JP_BACK_MAP ? 2 * c2 + 1 - s + d : 2 * c2 + s + d;
     col -= (col >= L) ? L : 0;
     col -= (col >= L) ? L : 0;
     return (rb * 16 + d) * L + col;
@@ -133,8 +137,14 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
 #ifndef JP_PREFETCH_DIST
 #define JP_PREFETCH_DIST 592
 #endif
-#ifndef JP_MINB
-#define JP_MINB 4
+#ifndef JP_RB_TILE
+#define JP_RB_TILE 1 // image rows in flight per warp while building the shared rows (measured: 1 beats 2 and 4)
+#endif
+#ifndef JP_MINB_FWD
+#define JP_MINB_FWD 4
+#endif
+#ifndef JP_MINB_BACK
+#define JP_MINB_BACK 5
 #endif
 #ifndef JP_FWD_UNROLL
 #define JP_FWD_UNROLL 8
@@ -177,7 +187,7 @@ __device__ __forceinline__ void reds_add(uint32_t addr, int q)
     }
 
 template <int P>
-__global__ void __launch_bounds__(kThreads, JP_MINB)
+__global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
     k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
                int lane_map, float *__restrict__ p)
 {
@@ -251,7 +261,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
 
     for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
         const int rows = min(rows_cap, t.I1 - c0 + 1);
-        build_rows<P, true>(C2, rinfo, img, t, c0, rows, n2, vec_ok, kc);
+        build_rows<P, true, JP_RB_TILE>(C2, rinfo, img, t, c0, rows, n2, vec_ok, kc);
         __syncthreads();
         // ---- consume: every LOR walks its planes of this chunk, interpolating along z only
 #pragma unroll
@@ -333,7 +343,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
     }
 
 template <int P>
-__global__ void __launch_bounds__(kThreads, JP_MINB)
+__global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
     k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
                 int lane_map, float *__restrict__ img)
 {
@@ -485,10 +495,15 @@ __global__ void __launch_bounds__(kThreads, JP_MINB)
 // ---- launchers ----------------------------------------------------------------------------------------------
 namespace {
 
-#ifndef JP_SMEM_KB
-#define JP_SMEM_KB 54
+// Shared memory per CTA.  Measured on configs[1] (sweep 20..54 KB): the smaller the tile buffer the larger the L1 that
+// serves the end-point and image-row loads, down to ~36 KB where the extra row chunks start to cost more.
+#ifndef JP_SMEM_KB_FWD
+#define JP_SMEM_KB_FWD 36
 #endif
-constexpr size_t kSmemBudget = JP_SMEM_KB * 1024; // per CTA: four CTAs per SM
+#ifndef JP_SMEM_KB_BACK
+#define JP_SMEM_KB_BACK 28
+#endif
+constexpr size_t kSmemMax = 100 * 1024; // wide images: at least 24 rows per chunk, up to this much
 
 // JP_LANE_MAP=0 in the environment switches the lane mapping off (A/B measurements; results are the same)
 int lane_map_on()
@@ -504,7 +519,7 @@ struct TileCfg {
     int vec_ok;
 };
 
-TileCfg tile_cfg(const Geom &g, const void *img, size_t elem)
+TileCfg tile_cfg(const Geom &g, const void *img, size_t elem, size_t budget)
 {
     TileCfg c{};
     const int need = g.n[2] + kPad + kPadR;
@@ -515,7 +530,9 @@ TileCfg tile_cfg(const Geom &g, const void *img, size_t elem)
     const int np = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
     const size_t rinfo = (size_t)np * sizeof(RowInfo);
     const size_t row = (size_t)c.P * elem;
-    size_t rows = rinfo + row <= kSmemBudget ? (kSmemBudget - rinfo) / row : 0;
+    if (budget < rinfo + 24 * row) budget = rinfo + 24 * row;
+    if (budget > kSmemMax) budget = kSmemMax;
+    size_t rows = rinfo + row <= budget ? (budget - rinfo) / row : 0;
     if (rows < 8) { c.P = 0; return c; }
     if (rows > (size_t)np) rows = (size_t)np;
     c.rows_cap = (int)rows;
@@ -527,7 +544,7 @@ TileCfg tile_cfg(const Geom &g, const void *img, size_t elem)
 template <typename K>
 cudaError_t set_smem(K kernel, size_t smem)
 {
-    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBudget);
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
 }
 
 } // namespace
@@ -546,7 +563,7 @@ cudaError_t set_smem(K kernel, size_t smem)
 cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
-    const TileCfg c = tile_cfg(g, img, sizeof(float2));
+    const TileCfg c = tile_cfg(g, img, sizeof(float2), JP_SMEM_KB_FWD * 1024);
     if (!c.P) return launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
     JP_DISPATCH_P(c, {
@@ -560,7 +577,7 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
 cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
-    const TileCfg c = tile_cfg(g, img, sizeof(int));
+    const TileCfg c = tile_cfg(g, img, sizeof(int), JP_SMEM_KB_BACK * 1024);
     if (!c.P) return launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
     JP_DISPATCH_P(c, {

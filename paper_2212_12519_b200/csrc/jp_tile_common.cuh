@@ -167,7 +167,7 @@ __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs,
 // ICPT: store (intercept, slope) instead of (value, slope): pair(z) = (C[z] - (z - kc) D[z], D[z]), D[z] = C[z+1] - C[z],
 // so that the interpolant at axial coordinate u (cell z = floor(u)) is  pair.x + (u - kc) pair.y  with no
 // fractional part needed; kc (an integer, the middle of the axial range) keeps |u - kc| small.
-template <int P, bool ICPT = false>
+template <int P, bool ICPT = false, int RB = JP_RB>
 __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, const float *__restrict__ img, const Track &t,
                                            int c0, int rows, int n2, int vec_ok, float kc = 0.f)
 {
@@ -176,7 +176,7 @@ __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, con
         if (vec_ok) {
             // one warp per row, lanes along z in groups of four voxels; kRB rows in flight per warp
             const int G = n2 >> 2;
-            constexpr int kRB = JP_RB, kNW = kThreads / 32;
+            constexpr int kRB = RB, kNW = kThreads / 32;
             for (int g0 = 0; g0 < G; g0 += 32) {
                 const int gq = g0 + lane;
                 const bool act = gq < G;
