@@ -173,3 +173,35 @@ def test_config4_osem_full_image(cuda_device, phantom_dev, events_full):
         assert rel <= 1e-4, f"OSEM rel-L2 {rel:.3e}"
         assert mx <= 1e-3, f"OSEM max abs / max {mx:.3e}"
     plan.destroy()
+
+
+def test_sino_osem_full_subset(cuda_device, phantom_dev):
+    """SURVEY.md 8(f) row 3 at the size and launch configuration bench.py --config 5 times per subset (9,474,048 LORs
+    x 29 bins, fused ratio epilogue): the emission sinogram is zero outside a sampled set S of LORs, so the ratio is
+    zero there and the update is the oracle's update over the LORs of S alone (mult and contam are dense)."""
+    ph, imgd = phantom_dev
+    xs, xe = inputs.sinogram_lors(views=inputs.SUBSET_VIEWS, device=cuda_device)
+    n = xs.shape[1]
+    extra = [_track(4, 0)[::9], _track(12, 30)[::9]]
+    idx = _sample(n, 10_000, 5, extra).to(cuda_device)
+    hxs, hxe = xs[:, idx].cpu().numpy(), xe[:, idx].cpu().numpy()
+    tof = _tof()
+    y = torch.zeros((n, 29), dtype=torch.float32, device=cuda_device)
+    y[idx] = inputs.uniform_values((idx.numel(), 29), 0.0, 3.0, seed=inputs.BASE_SEED + 305, device=cuda_device)
+    mult = inputs.uniform_values(n, 0.2, 1.0, seed=inputs.BASE_SEED + 306, device=cuda_device)
+    contam = inputs.uniform_values((n, 29), 0.01, 0.1, seed=inputs.BASE_SEED + 307, device=cuda_device)
+    sens = torch.ones((1,) + tuple(G.n), dtype=torch.float32, device=cuda_device)
+    x0 = ph + np.float32(0.1)
+    x = torch.from_numpy(x0).to(cuda_device)
+    jp.jp_sino_osem_tof(xs, xe, [0, n], y, mult, contam, sens, x, G.origin, G.voxsize, tof, n_iter=1)
+    k = idx.numel()
+    ref = oracle.sino_osem_tof(hxs, hxe, [0, k], y[idx].cpu().numpy(), mult[idx].cpu().numpy(),
+                               contam[idx].cpu().numpy(), np.ones((1,) + tuple(G.n)), x0, G.origin, G.voxsize,
+                               *TOF_ARGS, n_iter=1)
+    assert_back(x, ref)
+    # and a dense run: finite, non-negative, zero where the start image is zero
+    y = inputs.uniform_values((n, 29), 0.0, 1.0, seed=inputs.BASE_SEED + 308, device=cuda_device)
+    x = imgd.clone()
+    jp.jp_sino_osem_tof(xs, xe, [0, n], y, mult, contam, sens, x, G.origin, G.voxsize, tof, n_iter=1)
+    assert torch.isfinite(x).all() and float(x.min()) >= 0.0
+    assert float(x[imgd == 0].abs().max()) == 0.0
