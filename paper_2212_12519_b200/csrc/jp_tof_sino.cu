@@ -29,7 +29,10 @@ namespace {
 
 constexpr int kSBlock = 256;
 constexpr int kSLd = kSBlock + 1;
-constexpr int kGK = 512; // table rows per unit of phi
+#ifndef JP_SINO_GK
+#define JP_SINO_GK 512
+#endif
+constexpr int kGK = JP_SINO_GK; // table rows per unit of phi
 #ifndef JP_SINO_MINB
 #define JP_SINO_MINB 4
 #endif
