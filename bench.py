@@ -44,6 +44,11 @@ TOF_ARGS = (TOFP.tofbin_width, TOFP.sigma_tof, TOFP.n_sigmas, TOFP.n_tofbins)
 LANE = {"fwd": 11.0, "back": 12.0, "lm": 40.0, "sino": 112.0}
 FP32_LANES_PER_SM = 128
 N_SM = 148
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one `ncu --set full` capture
+# summarised in profiles/r01_v5_ncu_full.txt (bytes; listmode: one launch = the events of one principal axis)
+TRAFFIC = {(1, "fwd"): 3.953511e9 + 1.070194e9, (1, "back"): 4.103912e9 + 0.580913e9,
+           (2, "fwd"): 0.379303e9 + 1.154710e9, (2, "back"): 0.758793e9 + 0.056787e9,
+           (3, "fwd"): 1.311510e9 + 0.887897e9, (3, "back"): 2.396905e9 + 0.162793e9}
 
 SPEC = {
     1: dict(metric="LORs/s (non-TOF sinogram fwd+back pair)", unit="LORs/s",
@@ -485,7 +490,9 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     achieved = lane * w.plane_steps / (dom_ms * 1e-3)
     per = lambda ms, k: {"ms": ms, "per_s": w.n / ms * 1e3, "frac_alu": LANE[k] * w.plane_steps / (ms * 1e-3) / alu_peak}
     return {"bound": "alu", "kernel": names[1] if dom == "back" else names[0], "achieved": achieved / 1e12,
-            "peak": alu_peak / 1e12, "unit": "T lane-instr/s (FP32)", "frac": achieved / alu_peak, "traffic": None,
+            "peak": alu_peak / 1e12, "unit": "T lane-instr/s (FP32)", "frac": achieved / alu_peak,
+            "traffic": TRAFFIC.get((w.c, dom)), "traffic_source": "profiles/r01_v5_ncu_full.txt (bytes per launch)",
+            "algorithmic_bytes_per_launch": w.hbm_bytes,
             "peak_source": src, "plane_steps_per_launch": w.plane_steps, "lane_instr_per_plane_step": lane,
             "fwd": per(fwd_ms, kf), "back": per(back_ms, kb),
             "hbm_bound_frac": w.hbm_bytes / (dom_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9)}

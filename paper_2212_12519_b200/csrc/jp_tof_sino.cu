@@ -196,6 +196,20 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
             q = pray_from(r, g);
         }
         const bool any = __syncthreads_or(q.nk > 0) != 0;
+        // pull into L2 what the block will read at its end (forward: the emission / contamination tile of the OSEM
+        // ratio) or what the next block of this CTA reads at its start (back: its y tile), one 128-byte line per thread
+        if (!BACK && any && epi.y_em) {
+            const int64_t o = j0 * nbins + (int64_t)tid * 32;
+            if (o < (j0 + nvalid) * nbins) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(epi.y_em + o));
+                if (epi.contam) asm volatile("prefetch.global.L2 [%0];" ::"l"(epi.contam + o));
+            }
+        }
+        if (BACK && y && blk + gridDim.x < nblocks) {
+            const int64_t jn = (blk + gridDim.x) * kSBlock;
+            const int64_t o = jn * nbins + (int64_t)tid * 32;
+            if (o < min(n, jn + kSBlock) * nbins) asm volatile("prefetch.global.L2 [%0];" ::"l"(y + o));
+        }
         if (!any) {
             if (!BACK) { // the whole block misses the image: zeros
                 float *out = p + j0 * nbins;
