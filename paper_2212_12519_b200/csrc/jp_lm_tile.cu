@@ -169,12 +169,18 @@ __device__ __forceinline__ void generic_back_lm(const Lors &l, int64_t j, float 
 }
 
 // shared bookkeeping of a CTA
+constexpr int kMaxLong = (kTile + kMinRun - 1) / kMinRun; // long runs (>= kMinRun events) of a window: slot = start / kMinRun
+
 struct TileState {
-    Track trk;
+    Track trk;      // adjoint kernel: the current run's track
     LineExtra ex;
     int nruns;
     int imin, imax;
     unsigned short starts[kTile + 1];
+    // forward kernel: the tracks of ALL long runs of the window, set up in parallel before the run loop
+    Track trks[kMaxLong];
+    double Rds[kMaxLong];
+    int imins[kMaxLong], imaxs[kMaxLong];
 };
 
 // runs of events with identical canonical transaxial end points among the CTA's nev events; canon = smem scratch
@@ -285,6 +291,26 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
     const int kci = n2 >> 1; // axial shift of the (intercept, slope) rows (build_rows<P, true>)
     const uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
 
+    // tracks of all long runs at once (one thread per run) instead of one serial set-up + barrier per run
+    for (int k = tid; k < nruns; k += kThreads) {
+        const int ra = S.starts[k], rb = S.starts[k + 1];
+        if (rb - ra < kMinRun) continue;
+        const int slot = ra / kMinRun;
+        const int64_t e = c0 + ra;
+        float xs = l.xs[e], ys = l.ys[e], xe = l.xe[e], ye = l.ye[e];
+        if (is_swapped(xs, ys, xe, ye)) {
+            float tmp = xs; xs = xe; xe = tmp;
+            tmp = ys; ys = ye; ye = tmp;
+        }
+        track_setup(g, xs, ys, xe, ye, S.trks[slot]);
+        const double dxy[2] = {(double)xe - (double)xs, (double)ye - (double)ys};
+        const double ratio = dxy[1 - S.trks[slot].p] * S.trks[slot].inv_dp;
+        S.Rds[slot] = 1.0 + ratio * ratio;
+        S.imins[slot] = 0x7fffffff;
+        S.imaxs[slot] = -1;
+    }
+    __syncthreads();
+
     for (int k = 0; k < nruns; ++k) {
         const int ra = S.starts[k], rb = S.starts[k + 1];
         bool active[kPerThread]; // the run's events are dealt to the threads: event ra + m kThreads + tid
@@ -302,27 +328,13 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                 }
             continue;
         }
-        // ---- the run's track (thread owning its first event)
-        if (tid == 0) {
-                const int64_t e = c0 + ra;
-                float xs = l.xs[e], ys = l.ys[e], xe = l.xe[e], ye = l.ye[e];
-                if (is_swapped(xs, ys, xe, ye)) {
-                    float tmp = xs; xs = xe; xe = tmp;
-                    tmp = ys; ys = ye; ye = tmp;
-                }
-                track_setup(g, xs, ys, xe, ye, S.trk);
-                const double dxy[2] = {(double)xe - (double)xs, (double)ye - (double)ys};
-                const double ratio = dxy[1 - S.trk.p] * S.trk.inv_dp;
-                S.ex.Rd = 1.0 + ratio * ratio;
-                S.imin = 0x7fffffff;
-                S.imax = -1;
-            }
-        __syncthreads();
-        const Track trk = S.trk;
+        // ---- the run's track (set up before the loop)
+        const int slot = ra / kMinRun;
+        const Track trk = S.trks[slot];
         LmRay zr[kPerThread];
         float acc_[kPerThread];
         if (trk.I1 >= trk.I0) {
-            const double Rd = S.ex.Rd;
+            const double Rd = S.Rds[slot];
             int lo = 0x7fffffff, hi = -1;
 #pragma unroll
             for (int m = 0; m < kPerThread; ++m) {
@@ -345,14 +357,14 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                 }
             }
             if (hi >= lo) {
-                atomicMin(&S.imin, lo);
-                atomicMax(&S.imax, hi);
+                atomicMin(&S.imins[slot], lo);
+                atomicMax(&S.imaxs[slot], hi);
             }
             for (int r = tid; r <= trk.I1 - trk.I0; r += kThreads) rinfo[r] = row_info(g, trk, trk.I0 + r);
         }
         __syncthreads();
         if (trk.I1 >= trk.I0) {
-            const int I0 = S.imin, I1 = S.imax;
+            const int I0 = S.imins[slot], I1 = S.imaxs[slot];
             for (int cc = I0; cc <= I1; cc += rows_cap) {
                 const int rows = min(rows_cap, I1 - cc + 1);
                 build_rows<P, true>(C2, rinfo, img, trk, cc, rows, n2, vec_ok, (float)kci);
@@ -387,7 +399,6 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                 if (LM_MODE == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
                 p[out_index(perm, io_off, first, c0 + ra + m * kThreads + tid)] = out;
             }
-        __syncthreads(); // S.trk is rewritten by the next run
     }
 }
 #undef JP_LM_FWD_STEP
@@ -614,7 +625,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
 namespace {
 
 #ifndef JP_LMT_SMEM_KB_FWD
-#define JP_LMT_SMEM_KB_FWD 54
+#define JP_LMT_SMEM_KB_FWD 52
 #endif
 #ifndef JP_LMT_SMEM_KB_BACK
 #define JP_LMT_SMEM_KB_BACK 44
