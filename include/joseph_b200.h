@@ -220,6 +220,16 @@ int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_s
  * Returns after the result is in host memory.  jp_back_host ACCUMULATES into img_host. */
 int jp_fwd_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, float *p_host);
 int jp_back_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, float *img_host);
+/* the TOF projectors in hybrid mode (same semantics as jp_fwd/back_tof_sino and the unplanned jp_fwd/back_tof_lm;
+ * p_host / y_host: [n][n_tofbins] resp. [n]; tofbin_host: [n] int16; the back projections ACCUMULATE into img_host) */
+int jp_fwd_tof_sino_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, const jp_tof *tof,
+                         float *p_host);
+int jp_back_tof_sino_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, const jp_tof *tof,
+                          float *img_host);
+int jp_fwd_tof_lm_host(const jp_lors *lors_host, const int16_t *tofbin_host, const float *img_host, const jp_geom *geom,
+                       const jp_tof *tof, float *p_host);
+int jp_back_tof_lm_host(const jp_lors *lors_host, const int16_t *tofbin_host, const float *y_host, const jp_geom *geom,
+                        const jp_tof *tof, float *img_host);
 
 /* ---- misc ----------------------------------------------------------------------------------------- */
 /* text of the last CUDA error seen by the calling thread ("" if none); valid until the next call */

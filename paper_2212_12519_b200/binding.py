@@ -83,6 +83,12 @@ EXPORTS = {
                                    C.c_size_t, C.c_void_p]),
     "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
+    "jp_fwd_tof_sino_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p]),
+    "jp_back_tof_sino_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p]),
+    "jp_fwd_tof_lm_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
+                                     C.c_void_p]),
+    "jp_back_tof_lm_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
+                                      C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
     "jp_version": (C.c_int, []),
 }
@@ -540,4 +546,64 @@ def jp_back_host(xstart, xend, y, img, origin, voxsize) -> torch.Tensor:
     assert not y.is_cuda and y.dtype == torch.float32 and y.numel() == l.n and y.is_contiguous()
     g = make_geom(img.shape, origin, voxsize)
     _check(load().jp_back_host(C.byref(l), y.data_ptr(), C.byref(g), img.data_ptr()), "jp_back_host")
+    return img
+
+
+def _host_f32(t, what, numel=None):
+    if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise JosephError(f"{what} must be a contiguous CPU float32 tensor")
+    if numel is not None and t.numel() != numel:
+        raise JosephError(f"{what} has {t.numel()} elements, expected {numel}")
+    return t
+
+
+def _host_bins(tofbin, n):
+    if tofbin.is_cuda or tofbin.dtype != torch.int16 or not tofbin.is_contiguous() or tofbin.numel() != n:
+        raise JosephError("tofbin must be a contiguous CPU int16 tensor with one entry per event")
+    return tofbin
+
+
+def jp_fwd_tof_sino_host(xstart, xend, img, origin, voxsize, tof: jp_tof, out=None) -> torch.Tensor:
+    l, keep = _host_lors(xstart, xend)
+    img = _host_f32(img, "img")
+    if out is None:
+        out = torch.empty((l.n, int(tof.n_tofbins)), dtype=torch.float32)
+    _host_f32(out, "out", l.n * int(tof.n_tofbins))
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_fwd_tof_sino_host(C.byref(l), img.data_ptr(), C.byref(g), C.byref(tof), out.data_ptr()),
+           "jp_fwd_tof_sino_host")
+    return out
+
+
+def jp_back_tof_sino_host(xstart, xend, y, img, origin, voxsize, tof: jp_tof) -> torch.Tensor:
+    l, keep = _host_lors(xstart, xend)
+    _host_f32(y, "y", l.n * int(tof.n_tofbins))
+    img = _host_f32(img, "img")
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_tof_sino_host(C.byref(l), y.data_ptr(), C.byref(g), C.byref(tof), img.data_ptr()),
+           "jp_back_tof_sino_host")
+    return img
+
+
+def jp_fwd_tof_lm_host(xstart, xend, tofbin, img, origin, voxsize, tof: jp_tof, out=None) -> torch.Tensor:
+    l, keep = _host_lors(xstart, xend)
+    _host_bins(tofbin, l.n)
+    img = _host_f32(img, "img")
+    if out is None:
+        out = torch.empty(l.n, dtype=torch.float32)
+    _host_f32(out, "out", l.n)
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_fwd_tof_lm_host(C.byref(l), tofbin.data_ptr(), img.data_ptr(), C.byref(g), C.byref(tof),
+                                     out.data_ptr()), "jp_fwd_tof_lm_host")
+    return out
+
+
+def jp_back_tof_lm_host(xstart, xend, tofbin, y, img, origin, voxsize, tof: jp_tof) -> torch.Tensor:
+    l, keep = _host_lors(xstart, xend)
+    _host_bins(tofbin, l.n)
+    _host_f32(y, "y", l.n)
+    img = _host_f32(img, "img")
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_tof_lm_host(C.byref(l), tofbin.data_ptr(), y.data_ptr(), C.byref(g), C.byref(tof),
+                                      img.data_ptr()), "jp_back_tof_lm_host")
     return img

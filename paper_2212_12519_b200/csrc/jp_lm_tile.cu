@@ -26,6 +26,9 @@ using namespace tile;
 
 namespace {
 
+#ifndef JP_LMT_BACK_UNROLL
+#define JP_LMT_BACK_UNROLL 2
+#endif
 #ifndef JP_LMT_MINB
 #define JP_LMT_MINB 4
 #endif
@@ -571,14 +574,30 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
                     const float a2_1 = fmaf(b2, 1.f, a2_0), x0_1 = fmaf(dx, 1.f, x0_0);
                     float fk = (float)(ib - zr[m].i0);
                     uint32_t row = ci_base + (uint32_t)((ib - cc) * P) * 4u;
+                    int left = nst;
+#if JP_LMT_BACK_UNROLL == 4
+                    const float a2_2 = fmaf(b2, 2.f, a2_0), x0_2 = fmaf(dx, 2.f, x0_0);
+                    const float a2_3 = fmaf(b2, 3.f, a2_0), x0_3 = fmaf(dx, 3.f, x0_0);
 #pragma unroll 1
-                    for (int it = nst >> 1; it > 0; --it) {
+                    for (; left >= 4; left -= 4) {
+                        JP_LM_BACK_STEP(0, a2_0, x0_0)
+                        JP_LM_BACK_STEP(1, a2_1, x0_1)
+                        JP_LM_BACK_STEP(2, a2_2, x0_2)
+                        JP_LM_BACK_STEP(3, a2_3, x0_3)
+                        fk += 4.f;
+                        row += 4u * P * 4u;
+                    }
+                    if (left >= 2) {
+#else
+#pragma unroll 1
+                    for (; left >= 2; left -= 2) {
+#endif
                         JP_LM_BACK_STEP(0, a2_0, x0_0)
                         JP_LM_BACK_STEP(1, a2_1, x0_1)
                         fk += 2.f;
                         row += 2u * P * 4u;
                     }
-                    if (nst & 1) JP_LM_BACK_STEP(0, a2_0, x0_0)
+                    if (left & 1) JP_LM_BACK_STEP(0, a2_0, x0_0)
                 }
                 __syncthreads();
                 // ---- flush: spread every row over its two q1 neighbours with REDs, and clear it
