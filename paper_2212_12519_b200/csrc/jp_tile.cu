@@ -107,13 +107,60 @@ __device__ __forceinline__ int map_back(int idx, int L)
     const int w = idx >> 5, l32 = idx & 31, d = l32 & 15, s = l32 >> 4, half = L >> 1;
     const int rb = w / half, c2 = w - rb * half;
     int col = JP_BACK_MAP ? 2 * c2 + 1 - s + d : 2 * c2 + s + d;
-    col -= (col >= L) ? L : 0;
-    col -= (col >= L) ? L : 0;
+    col %= L; // columns wrap (col < L + 16)
     return (rb * 16 + d) * L + col;
 }
 
+// ---- tiles cut per track ---------------------------------------------------------------------------------------
+// A tile is 768 CONSECUTIVE LORs, so a track whose length T is not a multiple of 768 (e.g. 36 rings: 1296 ring
+// pairs) would leave every other tile straddling two tracks, i.e. on the per-LOR path.  k_track_probe reads T off
+// the head of the list (length of the first run of identical transaxial end points) and, when T > 768 is not a
+// multiple of 768, the CUT instantiation of the kernels (persistent CTAs) deals tiles per track instead:
+// track k = tile / ceil(T / 768) is cut into pieces of 768 and one shorter piece.  The list is ASSUMED to consist
+// of tracks of that length; where it does not, tile_is_track fails and the tile takes the per-LOR path as before.
+// *cut_len == 0 selects the plain instantiation (both are launched; the one not selected exits at once).
+__global__ void k_track_probe(Lors l, int64_t n, int *cut_len)
+{
+    __shared__ int first;
+    const int tid = threadIdx.x;
+    if (tid == 0) first = 0x7fffffff;
+    __syncthreads();
+    const int64_t lim = n < 8192 ? n : 8192; // tracks longer than this are treated as aligned
+    const float xs0 = l.xs[0], ys0 = l.ys[0], xe0 = l.xe[0], ye0 = l.ye[0];
+    for (int64_t j = tid; j < lim; j += blockDim.x) {
+        if (!same_bits(l.xs[j], xs0) || !same_bits(l.ys[j], ys0) || !same_bits(l.xe[j], xe0) || !same_bits(l.ye[j], ye0)) {
+            atomicMin(&first, (int)j);
+            break;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const int T = first;
+        *cut_len = (T != 0x7fffffff && T > kTile && (T % kTile) != 0) ? T : 0;
+    }
+}
+
+// first LOR and length of tile number `tile` (CUT: per track, see above); false when the list is exhausted
+template <bool CUT>
+__device__ __forceinline__ bool tile_span(int64_t tile, int64_t n, int T, int64_t &j0, int &tn)
+{
+    if (CUT) {
+        const int tpt = (T + kTile - 1) / kTile;
+        const int64_t k = tile / tpt;
+        const int t = (int)(tile - k * tpt);
+        j0 = k * (int64_t)T + (int64_t)t * kTile;
+        tn = min(kTile, T - t * kTile);
+    } else {
+        j0 = tile * (int64_t)kTile;
+        tn = kTile;
+    }
+    if (j0 >= n) return false;
+    if (j0 + tn > n) tn = (int)(n - j0);
+    return true;
+}
+
 // is this tile a track?  all 768 LORs valid, identical transaxial end points, principal axis x or y
-__device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t n, const int (&jm)[kPerThread],
+__device__ __forceinline__ bool tile_is_track_full(const Lors &l, int64_t j0, int64_t n, const int (&jm)[kPerThread],
                                               const float (&zs)[kPerThread], const float (&ze)[kPerThread], float xs0,
                                               float ys0, float xe0, float ye0)
 {
@@ -131,6 +178,29 @@ __device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int64_t
         }
         ok = ok && (diff == 0) && (dmax > 0.0);
     }
+    return __syncthreads_and(ok) != 0;
+}
+
+// is this tile a track?  all tn LORs have identical transaxial end points and principal axis x or y
+template <bool CUT>
+__device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int tn, const int (&jm)[kPerThread],
+                                              const float (&zs)[kPerThread], const float (&ze)[kPerThread], float xs0,
+                                              float ys0, float xe0, float ye0)
+{
+    const double dmax = fmax(fabs((double)xe0 - (double)xs0), fabs((double)ye0 - (double)ys0));
+    // all loads first (no short-circuit: twelve independent loads in flight), then compare bits
+    uint32_t diff = 0;
+    bool ok = (dmax > 0.0) && (CUT || tn == kTile); // plain: full tiles only, so that no slot needs a guard afterwards
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        if (jm[m] < tn) {
+            const int64_t j = j0 + jm[m];
+            diff |= (__float_as_uint(l.xs[j]) ^ __float_as_uint(xs0)) | (__float_as_uint(l.ys[j]) ^ __float_as_uint(ys0)) |
+                    (__float_as_uint(l.xe[j]) ^ __float_as_uint(xe0)) | (__float_as_uint(l.ye[j]) ^ __float_as_uint(ye0));
+            ok = ok && (fabs((double)ze[m] - (double)zs[m]) <= dmax);
+        }
+    }
+    ok = ok && (diff == 0);
     return __syncthreads_and(ok) != 0;
 }
 
@@ -189,7 +259,7 @@ __device__ __forceinline__ void reds_add(uint32_t addr, int q)
 template <int P>
 __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
     k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
-               int lane_map, float *__restrict__ p)
+               int lane_map, const int *__restrict__ cut_len, float *__restrict__ p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                      // [rows_cap][P]
@@ -210,7 +280,8 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
         ze[m] = (j < n) ? l.ze[j] : 0.f;
     }
     const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (!tile_is_track(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
+    if (cut_len && __ldg(cut_len) != 0) return; // tiles are dealt per track: the _cut kernel does this list
+    if (!tile_is_track_full(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
 #pragma unroll 1
         for (int m = 0; m < kPerThread; ++m) {
             const int64_t j = j0 + m * kThreads + tid;
@@ -322,6 +393,158 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) p[j0 + map_fwd(m * kThreads + tid, L)] = zr[m].cf * (acc0[m] + acc1[m]);
 }
+
+// ---- the same kernel with tiles dealt per track (CUT = true; see k_track_probe) -----------------------------
+template <int P, bool CUT>
+__global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
+    k_fwd_tile_cut(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
+               int lane_map, const int *__restrict__ cut_len, float *__restrict__ p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                      // [rows_cap][P]
+    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(float2)); // [max(n0,n1)]
+    __shared__ Track trk;
+    __shared__ int sh_len[2];
+    const int tid = threadIdx.x;
+    const int T = cut_len ? __ldg(cut_len) : 0;
+    if (CUT && T == 0) return; // the plain instantiation does this list (it checks after its first loads are in flight)
+  // plain: one tile per CTA; CUT: persistent CTAs over the tiles dealt per track
+  for (int64_t tile = blockIdx.x; CUT || tile == blockIdx.x; tile += gridDim.x) {
+    int64_t j0;
+    int tn;
+    if (!tile_span<CUT>(tile, n, T, j0, tn)) break;
+    if (CUT && tile != blockIdx.x) __syncthreads(); // the shared buffers of the previous tile are free
+
+    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
+    int jm[kPerThread];
+    float zs[kPerThread], ze[kPerThread];
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        jm[m] = m * kThreads + tid;
+        const int64_t j = j0 + jm[m];
+        zs[m] = (jm[m] < tn) ? l.zs[j] : 0.f;
+        ze[m] = (jm[m] < tn) ? l.ze[j] : 0.f;
+    }
+    const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
+    if (!CUT && T != 0) return; // the CUT instantiation does this list
+    if (!tile_is_track<CUT>(l, j0, tn, jm, zs, ze, xs0, ys0, xe0, ye0)) {
+#pragma unroll 1
+        for (int m = 0; m < kPerThread; ++m) {
+            const int64_t j = j0 + m * kThreads + tid;
+            if (m * kThreads + tid < tn) p[j] = generic_fwd(l, j, g, img);
+        }
+        continue;
+    }
+    if (tid == 0) track_setup(g, xs0, ys0, xe0, ye0, trk);
+    __syncthreads();
+    const Track t = trk;
+    if (t.I1 < t.I0) { // the whole track misses the image
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m)
+            if (!CUT || m * kThreads + tid < tn) p[j0 + m * kThreads + tid] = 0.f;
+        continue;
+    }
+    // the tile does work: choose the lane mapping and fetch the axial end points again (from L1) in that order
+    const int L = (lane_map && (!CUT || tn == kTile)) ? detect_row_length(l, j0, n, sh_len) : 0;
+    if (L) {
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            jm[m] = map_fwd(m * kThreads + tid, L);
+            zs[m] = l.zs[j0 + jm[m]];
+            ze[m] = l.ze[j0 + jm[m]];
+        }
+    }
+    const int n2 = g.n[2];
+    const int kci = n2 >> 1;          // axial shift of the (intercept, slope) rows
+    const float kc = (float)kci;
+    // q1 cells of all planes of the track; constant zero columns of the shared rows
+    for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
+    {
+        const int ncl = kPad - 1, ncr = P - (n2 + kPad);
+        for (int e = tid; e < rows_cap * (ncl + ncr); e += kThreads) {
+            const int r = e / (ncl + ncr), c = e - r * (ncl + ncr);
+            C2[r * P + (c < ncl ? c : n2 + kPad + (c - ncl))] = make_float2(0.f, 0.f);
+        }
+    }
+    ZRay zr[kPerThread];
+    float acc0[kPerThread], acc1[kPerThread];
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        zr[m] = z_setup(g, t, zs[m], ze[m], (double)kci);
+        if (CUT && jm[m] >= tn) zr[m].i1 = zr[m].i0 - 1; // slot beyond a short tile
+        acc0[m] = 0.f;
+        acc1[m] = 0.f;
+    }
+    const uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
+    __syncthreads();
+
+    for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
+        const int rows = min(rows_cap, t.I1 - c0 + 1);
+        build_rows<P, true, JP_RB_TILE>(C2, rinfo, img, t, c0, rows, n2, vec_ok, kc);
+        __syncthreads();
+        // ---- consume: every LOR walks its planes of this chunk, interpolating along z only
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            const int ib = max(zr[m].i0, c0), ie = min(zr[m].i1, c0 + rows - 1);
+            if (ib > ie) continue;
+            const int nst = ie - ib + 1;
+            const float b2 = zr[m].b2, a2_0 = zr[m].a2;
+            const float a2_1 = fmaf(b2, 1.f, a2_0), a2_2 = fmaf(b2, 2.f, a2_0), a2_3 = fmaf(b2, 3.f, a2_0);
+            float fk = (float)(ib - zr[m].i0);
+            uint32_t row = c2_base + (uint32_t)((ib - c0) * P) * 8u;
+            float a0 = acc0[m], a1 = acc1[m];
+            {
+                float acc0 = a0, acc1 = a1;
+                int left = nst;
+#if JP_FWD_UNROLL == 8
+                const float a2_4 = fmaf(b2, 4.f, a2_0), a2_5 = fmaf(b2, 5.f, a2_0), a2_6 = fmaf(b2, 6.f, a2_0),
+                            a2_7 = fmaf(b2, 7.f, a2_0);
+#pragma unroll 1
+                for (; left >= 8; left -= 8) {
+                    JP_FWD_STEP(0, a2_0)
+                    JP_FWD_STEP(1, a2_1)
+                    JP_FWD_STEP(2, a2_2)
+                    JP_FWD_STEP(3, a2_3)
+                    JP_FWD_STEP(4, a2_4)
+                    JP_FWD_STEP(5, a2_5)
+                    JP_FWD_STEP(6, a2_6)
+                    JP_FWD_STEP(7, a2_7)
+                    fk += 8.f;
+                    row += 8u * P * 8u;
+                }
+                if (left >= 4) {
+#else
+#pragma unroll 1
+                for (; left >= 4; left -= 4) {
+#endif
+                    JP_FWD_STEP(0, a2_0)
+                    JP_FWD_STEP(1, a2_1)
+                    JP_FWD_STEP(2, a2_2)
+                    JP_FWD_STEP(3, a2_3)
+                    fk += 4.f;
+                    row += 4u * P * 8u;
+                }
+#pragma unroll 1
+                for (int it = left & 3; it > 0; --it) {
+                    JP_FWD_STEP(0, a2_0)
+                    fk += 1.f;
+                    row += P * 8u;
+                }
+                a0 = acc0;
+                a1 = acc1;
+            }
+            acc0[m] = a0;
+            acc1[m] = a1;
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        const int jl = CUT ? jm[m] : map_fwd(m * kThreads + tid, L);
+        if (!CUT || jl < tn) p[j0 + jl] = zr[m].cf * (acc0[m] + acc1[m]);
+    }
+  }
+}
 #undef JP_FWD_STEP
 
 // ---- back ------------------------------------------------------------------------------------------------
@@ -345,7 +568,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
 template <int P>
 __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
     k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
-                int lane_map, float *__restrict__ img)
+                int lane_map, const int *__restrict__ cut_len, float *__restrict__ img)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int *Ci = reinterpret_cast<int *>(smem_raw);                                        // [rows_cap][P]
@@ -367,7 +590,8 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
         ze[m] = (j < n) ? l.ze[j] : 0.f;
     }
     const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (!tile_is_track(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
+    if (cut_len && __ldg(cut_len) != 0) return; // tiles are dealt per track: the _cut kernel does this list
+    if (!tile_is_track_full(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
 #pragma unroll 1
         for (int m = 0; m < kPerThread; ++m) {
             const int64_t j = j0 + m * kThreads + tid;
@@ -490,6 +714,165 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
         __syncthreads();
     }
 }
+
+// ---- the same kernel with tiles dealt per track (CUT = true) --------------------------------------------------
+template <int P, bool CUT>
+__global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
+    k_back_tile_cut(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
+                int lane_map, const int *__restrict__ cut_len, float *__restrict__ img)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int *Ci = reinterpret_cast<int *>(smem_raw);                                        // [rows_cap][P]
+    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(int)); // [max(n0,n1)]
+    __shared__ Track trk;
+    __shared__ float red[kThreads / 32];
+    __shared__ int sh_len[2];
+    const int tid = threadIdx.x;
+    const int T = cut_len ? __ldg(cut_len) : 0;
+    if (CUT && T == 0) return; // the plain instantiation does this list (it checks after its first loads are in flight)
+  for (int64_t tile = blockIdx.x; CUT || tile == blockIdx.x; tile += gridDim.x) {
+    int64_t j0;
+    int tn;
+    if (!tile_span<CUT>(tile, n, T, j0, tn)) break;
+    if (CUT && tile != blockIdx.x) __syncthreads(); // the shared buffers of the previous tile are free
+
+    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
+    int jm[kPerThread];
+    float zs[kPerThread], ze[kPerThread];
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        jm[m] = m * kThreads + tid;
+        const int64_t j = j0 + jm[m];
+        zs[m] = (jm[m] < tn) ? l.zs[j] : 0.f;
+        ze[m] = (jm[m] < tn) ? l.ze[j] : 0.f;
+    }
+    const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
+    if (!CUT && T != 0) return; // the CUT instantiation does this list
+    if (!tile_is_track<CUT>(l, j0, tn, jm, zs, ze, xs0, ys0, xe0, ye0)) {
+#pragma unroll 1
+        for (int m = 0; m < kPerThread; ++m) {
+            const int64_t j = j0 + m * kThreads + tid;
+            if (m * kThreads + tid < tn) generic_back(l, j, g, y[j], img);
+        }
+        continue;
+    }
+    if (tid == 0) track_setup(g, xs0, ys0, xe0, ye0, trk);
+    __syncthreads();
+    const Track t = trk;
+    if (t.I1 < t.I0) continue;
+    const int L = (lane_map && (!CUT || tn == kTile)) ? detect_row_length(l, j0, n, sh_len) : 0;
+    if (L) {
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            jm[m] = map_back(m * kThreads + tid, L);
+            zs[m] = l.zs[j0 + jm[m]];
+            ze[m] = l.ze[j0 + jm[m]];
+        }
+    }
+    const int n2 = g.n[2];
+
+    ZRay zr[kPerThread];
+    float x[kPerThread];
+    float xmax = 0.f;
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        zr[m] = z_setup(g, t, zs[m], ze[m]);
+        x[m] = (!CUT || jm[m] < tn) ? zr[m].cf * y[j0 + jm[m]] : 0.f;
+        if (CUT && jm[m] >= tn) zr[m].i1 = zr[m].i0 - 1; // slot beyond a short tile
+        if (zr[m].i1 >= zr[m].i0) xmax = fmaxf(xmax, fabsf(x[m]));
+    }
+    // block max of |x|
+    for (int o = 16; o > 0; o >>= 1) xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
+    if ((tid & 31) == 0) red[tid >> 5] = xmax;
+    for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
+    {
+        int4 *z4 = reinterpret_cast<int4 *>(Ci);
+        for (int e = tid; e < rows_cap * (P / 4); e += kThreads) z4[e] = make_int4(0, 0, 0, 0);
+    }
+    __syncthreads();
+    xmax = red[0];
+#pragma unroll
+    for (int w = 1; w < kThreads / 32; ++w) xmax = fmaxf(xmax, red[w]);
+    if (!(xmax > 0.f) || !(xmax < 3.0e38f)) continue; // nothing to add (or non-finite input: undefined, skip)
+    // S: |c S| <= 2^22 - 2 and 2 x 768 |c S| < 2^31
+    const float lim = fminf(4194302.f, 2147483648.f / (float)(2 * kTile) - 1.f);
+    const float S = lim / xmax, invS = xmax / lim;
+    int qx[kPerThread];
+#pragma unroll
+    for (int m = 0; m < kPerThread; ++m) {
+        x[m] *= S;
+        qx[m] = __float2int_rn(x[m]) + kMagicI;
+    }
+
+    const int warp = tid >> 5, lane = tid & 31;
+    const uint32_t ci_base = smem_addr(Ci) + kPad * 4u - ((uint32_t)kMagicI << 2);
+
+    for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
+        const int rows = min(rows_cap, t.I1 - c0 + 1);
+        // ---- scatter along z into the fixed-point tile
+#pragma unroll
+        for (int m = 0; m < kPerThread; ++m) {
+            const int ib = max(zr[m].i0, c0), ie = min(zr[m].i1, c0 + rows - 1);
+            if (ib > ie || x[m] == 0.f) continue;
+            const int nst = ie - ib + 1;
+            const float b2 = zr[m].b2, a2_0 = zr[m].a2, xm = x[m];
+            const int qxm = qx[m];
+            const float a2_1 = fmaf(b2, 1.f, a2_0), a2_2 = fmaf(b2, 2.f, a2_0), a2_3 = fmaf(b2, 3.f, a2_0);
+            float fk = (float)(ib - zr[m].i0);
+            uint32_t row = ci_base + (uint32_t)((ib - c0) * P) * 4u;
+#pragma unroll 1
+            for (int it = nst >> 2; it > 0; --it) {
+                JP_BACK_STEP(0, a2_0)
+                JP_BACK_STEP(1, a2_1)
+                JP_BACK_STEP(2, a2_2)
+                JP_BACK_STEP(3, a2_3)
+                fk += 4.f;
+                row += 4u * P * 4u;
+            }
+#pragma unroll 1
+            for (int it = nst & 3; it > 0; --it) {
+                JP_BACK_STEP(0, a2_0)
+                fk += 1.f;
+                row += P * 4u;
+            }
+        }
+        __syncthreads();
+        // ---- flush: spread every row over its two q1 neighbours with REDs, and clear it
+        if (vec_ok) {
+            const int G = n2 >> 2;
+            for (int r = warp; r < rows; r += kThreads / 32) {
+                const RowInfo ri = rinfo[c0 - t.I0 + r];
+                const float sa = ri.wa * invS, sb = ri.wb * invS;
+                for (int gq = lane; gq < G; gq += 32) {
+                    int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
+                    const int4 q = *src;
+                    if ((q.x | q.y | q.z | q.w) == 0) continue;
+                    *src = make_int4(0, 0, 0, 0);
+                    const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
+                    if (ri.base_a >= 0)
+                        atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq,
+                                  make_float4(sa * v.x, sa * v.y, sa * v.z, sa * v.w));
+                    if (ri.base_b >= 0)
+                        atomicAdd(reinterpret_cast<float4 *>(img + ri.base_b) + gq,
+                                  make_float4(sb * v.x, sb * v.y, sb * v.z, sb * v.w));
+                }
+            }
+        } else {
+            for (int e = tid; e < rows * n2; e += kThreads) {
+                const int r = e / n2, z = e - r * n2;
+                const int q = Ci[r * P + kPad + z];
+                if (q == 0) continue;
+                Ci[r * P + kPad + z] = 0;
+                const RowInfo ri = rinfo[c0 - t.I0 + r];
+                const float v = (float)q * invS;
+                if (ri.base_a >= 0) atomicAdd(img + ri.base_a + z, ri.wa * v);
+                if (ri.base_b >= 0) atomicAdd(img + ri.base_b + z, ri.wb * v);
+            }
+        }
+        __syncthreads();
+    }
+  }
+}
 #undef JP_BACK_STEP
 
 // ---- launchers ----------------------------------------------------------------------------------------------
@@ -560,18 +943,47 @@ cudaError_t set_smem(K kernel, size_t smem)
     default: return cudaErrorInvalidValue;         \
     }
 
+// probe of the track length (lists long enough for it to matter); *out = device int (stream-ordered scratch) or null
+static cudaError_t probe_tracks(const Lors &l, int64_t n, cudaStream_t st, int **out)
+{
+    *out = nullptr;
+    if (n < 8 * kTile) return cudaSuccess;
+    cudaError_t e = cudaMallocAsync((void **)out, sizeof(int), st);
+    if (e != cudaSuccess) return e;
+    k_track_probe<<<1, 1024, 0, st>>>(l, n, *out);
+    return cudaGetLastError();
+}
+
+static unsigned persistent_grid(int per_sm)
+{
+    int dev = 0, nsm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    return (unsigned)(nsm > 0 ? nsm * per_sm : 148 * per_sm);
+}
+
 cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
     const TileCfg c = tile_cfg(g, img, sizeof(float2), JP_SMEM_KB_FWD * 1024);
     if (!c.P) return launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
+    int *cut = nullptr;
+    cudaError_t e = probe_tracks(l, n, st, &cut);
+    if (e != cudaSuccess) return e;
     JP_DISPATCH_P(c, {
-        cudaError_t e = set_smem(k_fwd_tile<P>, c.smem);
-        if (e != cudaSuccess) return e;
-        k_fwd_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok, lane_map_on(), p);
+        e = set_smem(k_fwd_tile<P>, c.smem);
+        if (e == cudaSuccess && cut) e = set_smem(k_fwd_tile_cut<P, true>, c.smem);
+        if (e == cudaSuccess) {
+            k_fwd_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok, lane_map_on(), cut, p);
+            if (cut)
+                k_fwd_tile_cut<P, true><<<persistent_grid(JP_MINB_FWD), kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok,
+                                                                                         lane_map_on(), cut, p);
+        }
     })
-    return cudaGetLastError();
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (cut) cudaFreeAsync(cut, st);
+    return e;
 }
 
 cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st)
@@ -580,12 +992,22 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
     const TileCfg c = tile_cfg(g, img, sizeof(int), JP_SMEM_KB_BACK * 1024);
     if (!c.P) return launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
+    int *cut = nullptr;
+    cudaError_t e = probe_tracks(l, n, st, &cut);
+    if (e != cudaSuccess) return e;
     JP_DISPATCH_P(c, {
-        cudaError_t e = set_smem(k_back_tile<P>, c.smem);
-        if (e != cudaSuccess) return e;
-        k_back_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok, lane_map_on(), img);
+        e = set_smem(k_back_tile<P>, c.smem);
+        if (e == cudaSuccess && cut) e = set_smem(k_back_tile_cut<P, true>, c.smem);
+        if (e == cudaSuccess) {
+            k_back_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok, lane_map_on(), cut, img);
+            if (cut)
+                k_back_tile_cut<P, true><<<persistent_grid(JP_MINB_BACK), kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok,
+                                                                                           lane_map_on(), cut, img);
+        }
     })
-    return cudaGetLastError();
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (cut) cudaFreeAsync(cut, st);
+    return e;
 }
 
 } // namespace jp

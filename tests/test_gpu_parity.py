@@ -157,6 +157,29 @@ def test_config1_slice_nontof(cuda_device, scanner):
     assert adj_gap(p, y.to(cuda_device), imgd, b) <= ADJ_GAP
 
 
+def test_tracks_not_a_multiple_of_the_tile(cuda_device, scanner):
+    """36-ring sub-scanner: tracks of 36 x 36 = 1296 ring pairs, not a multiple of the 768-LOR tile -> the kernels
+    deal tiles per track (768 + 528); a second list whose track lengths vary (tile_is_track must fall back)"""
+    g, ph = scanner
+    xs, xe = inputs.sinogram_lors(views=[5, 64, 130], radial=range(-40, 41, 4))
+    idx = np.arange(xs.shape[1])
+    keep = ((idx // 48) % 48 < 36) & (idx % 48 < 36)
+    for variant in (0, 1):
+        k = keep.copy()
+        if variant == 1:
+            k[1296 * 3 + 100:1296 * 3 + 150] = False        # one track is 50 LORs shorter: the assumed grid slips
+        hxs, hxe = np.ascontiguousarray(xs.numpy()[:, k]), np.ascontiguousarray(xe.numpy()[:, k])
+        n = hxs.shape[1]
+        assert n > 8 * 768
+        dxs, dxe = dev(hxs, cuda_device), dev(hxe, cuda_device)
+        p = jp.jp_fwd(dxs, dxe, dev(ph, cuda_device), g.origin, g.voxsize)
+        assert_fwd(p, oracle.fwd(hxs, hxe, ph, g.origin, g.voxsize))
+        y = np.random.default_rng(variant).uniform(0, 1, n).astype(np.float32)
+        b = jp.jp_back(dxs, dxe, dev(y, cuda_device), g.n, g.origin, g.voxsize)
+        assert_back(b, oracle.back(hxs, hxe, y, g.n, g.origin, g.voxsize))
+        assert adj_gap(p, dev(y, cuda_device), dev(ph, cuda_device), b) <= ADJ_GAP
+
+
 def test_config2_slice_tof_sino(cuda_device, scanner):
     g, ph = scanner
     tofp = inputs.TofParams()
