@@ -127,12 +127,22 @@ __global__ void k_track_probe(Lors l, int64_t n, int *cut_len)
     __syncthreads();
     const int64_t lim = n < 8192 ? n : 8192; // tracks longer than this are treated as aligned
     const float xs0 = l.xs[0], ys0 = l.ys[0], xe0 = l.xe[0], ye0 = l.ye[0];
-    for (int64_t j = tid; j < lim; j += blockDim.x) {
-        if (!same_bits(l.xs[j], xs0) || !same_bits(l.ys[j], ys0) || !same_bits(l.xe[j], xe0) || !same_bits(l.ye[j], ye0)) {
-            atomicMin(&first, (int)j);
+    // 8 positions per thread, all loads independent (one round trip instead of a dependent loop)
+    uint32_t d[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        const int64_t j = (int64_t)u * blockDim.x + tid;
+        d[u] = 0;
+        if (j < lim)
+            d[u] = (__float_as_uint(l.xs[j]) ^ __float_as_uint(xs0)) | (__float_as_uint(l.ys[j]) ^ __float_as_uint(ys0)) |
+                   (__float_as_uint(l.xe[j]) ^ __float_as_uint(xe0)) | (__float_as_uint(l.ye[j]) ^ __float_as_uint(ye0));
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+        if (d[u]) {
+            atomicMin(&first, u * (int)blockDim.x + tid);
             break;
         }
-    }
     __syncthreads();
     if (tid == 0) {
         const int T = first;
@@ -948,6 +958,8 @@ static cudaError_t probe_tracks(const Lors &l, int64_t n, cudaStream_t st, int *
 {
     *out = nullptr;
     if (n < 8 * kTile) return cudaSuccess;
+    const char *env = getenv("JP_TRACK_PROBE"); // JP_TRACK_PROBE=0: assume aligned tracks (A/B measurements)
+    if (env && env[0] == '0') return cudaSuccess;
     cudaError_t e = cudaMallocAsync((void **)out, sizeof(int), st);
     if (e != cudaSuccess) return e;
     k_track_probe<<<1, 1024, 0, st>>>(l, n, *out);
