@@ -45,10 +45,10 @@ LANE = {"fwd": 11.0, "back": 12.0, "lm": 40.0, "sino": 112.0}
 FP32_LANES_PER_SM = 128
 N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one `ncu --set full` capture
-# summarised in profiles/r01_v5_ncu_full.txt (bytes; listmode: one launch = the events of one principal axis)
-TRAFFIC = {(1, "fwd"): 3.953511e9 + 1.070194e9, (1, "back"): 4.103912e9 + 0.580913e9,
-           (2, "fwd"): 0.379303e9 + 1.154710e9, (2, "back"): 0.758793e9 + 0.056787e9,
-           (3, "fwd"): 1.311510e9 + 0.887897e9, (3, "back"): 2.396905e9 + 0.162793e9}
+# summarised in profiles/r01_v6_ncu_full.txt (bytes; listmode: one launch = the events of one principal axis)
+TRAFFIC = {(1, "fwd"): 3.955821e9 + 1.071657e9, (1, "back"): 4.106105e9 + 0.588588e9,
+           (2, "fwd"): 0.378425e9 + 1.152412e9, (2, "back"): 1.441061e9 + 0.146828e9,
+           (3, "fwd"): 1.280978e9 + 0.813510e9, (3, "back"): 2.396714e9 + 0.162799e9}
 
 SPEC = {
     1: dict(metric="LORs/s (non-TOF sinogram fwd+back pair)", unit="LORs/s",
@@ -269,7 +269,7 @@ class Workload:
             self.p = torch.empty(shape, dtype=torch.float32, device=dev)
             self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
             self.kinds = ("fwd", "back") if c == 1 else ("sino", "sino")
-            self.launches = 2
+            self.launches = 6 if c == 1 else 8   # c1: (track probe, tile kernel, its per-track twin) x 2; c2: pad/unpad, 2 tables, kernel
             self.hbm_bytes = (self.n * 28 + NVOX * 4) if c == 1 else (self.n * (24 + 4 * TOFP.n_tofbins) + NVOX * 4)
         else:
             nev = int(os.environ.get("JP_BENCH_EVENTS", "40000000"))
@@ -491,7 +491,7 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     per = lambda ms, k: {"ms": ms, "per_s": w.n / ms * 1e3, "frac_alu": LANE[k] * w.plane_steps / (ms * 1e-3) / alu_peak}
     return {"bound": "alu", "kernel": names[1] if dom == "back" else names[0], "achieved": achieved / 1e12,
             "peak": alu_peak / 1e12, "unit": "T lane-instr/s (FP32)", "frac": achieved / alu_peak,
-            "traffic": TRAFFIC.get((w.c, dom)), "traffic_source": "profiles/r01_v5_ncu_full.txt (bytes per launch)",
+            "traffic": TRAFFIC.get((w.c, dom)), "traffic_source": "profiles/r01_v6_ncu_full.txt (bytes per launch)",
             "algorithmic_bytes_per_launch": w.hbm_bytes,
             "peak_source": src, "plane_steps_per_launch": w.plane_steps, "lane_instr_per_plane_step": lane,
             "fwd": per(fwd_ms, kf), "back": per(back_ms, kb),

@@ -5,8 +5,14 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 ``paper_2212_12519_b200`` and that package does not import it.
 
 The arithmetic lives in ``joseph_oracle.c`` (plain C, IEEE double, OpenMP over LORs), written from
-PAPER.md section 2.1 with the readings A1..A14 of SURVEY.md section 8(c).  This module only
-marshals numpy arrays into it.  ``build()`` compiles it with gcc.
+PAPER.md section 2.1 with the readings A1..A14 of SURVEY.md section 8(c); the image-based resolution model
+(readings R1-R3) is in the same file, the TOF sinogram OSEM with multiplicative factors and contamination (readings
+S1-S3) is written with numpy in this module on top of the C projector calls.  Otherwise this module only marshals
+numpy arrays.  ``build()`` compiles the C file with gcc.
+
+Pins: tests/test_oracle_pins.py (projectors, listmode OSEM), tests/test_oracle_resolution.py (R1-R3),
+tests/test_oracle_sino_osem.py (S1-S3).  "parity unpinned" (pure conventions the paper does not fix): A3 tie
+direction, A9 TOF index origin / sign, A14 and S1 / S3 subset rules and the 1e-9 guards.
 """
 from __future__ import annotations
 
