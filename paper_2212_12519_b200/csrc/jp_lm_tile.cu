@@ -29,8 +29,11 @@ namespace {
 #ifndef JP_LMT_BACK_UNROLL
 #define JP_LMT_BACK_UNROLL 2
 #endif
-#ifndef JP_LMT_MINB
-#define JP_LMT_MINB 4
+#ifndef JP_LMT_MINB_FWD
+#define JP_LMT_MINB_FWD 4
+#endif
+#ifndef JP_LMT_MINB_BACK
+#define JP_LMT_MINB_BACK 5
 #endif
 constexpr int kG1K = 512;   // table intervals per TOF bin width
 constexpr int kMinRun = 48; // shorter runs are not worth a row build
@@ -237,7 +240,7 @@ __device__ __forceinline__ int64_t out_index(const int *__restrict__ perm, int64
     }
 
 template <int P, int LM_MODE, bool TOF>
-__global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
+__global__ void __launch_bounds__(kThreads, JP_LMT_MINB_FWD)
     k_fwd_tof_lm_tile(Lors l, const int16_t *__restrict__ tofbin, int64_t first, int64_t count,
                       const int *__restrict__ perm, int64_t io_off, const float *__restrict__ img, Geom g, Tof t,
                       G1Tab gt, int rows_cap, int vec_ok, float *__restrict__ p)
@@ -429,7 +432,7 @@ __device__ __forceinline__ void reds_add_lm(uint32_t addr, int q)
     }
 
 template <int P, bool TOF>
-__global__ void __launch_bounds__(kThreads, JP_LMT_MINB)
+__global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
     k_back_tof_lm_tile(Lors l, const int16_t *__restrict__ tofbin, int64_t first, int64_t count,
                        const int *__restrict__ perm, int64_t io_off, const float *__restrict__ y, Geom g, Tof t,
                        G1Tab gt, int rows_cap, int vec_ok, float *__restrict__ img)
@@ -647,7 +650,7 @@ namespace {
 #define JP_LMT_SMEM_KB_FWD 52
 #endif
 #ifndef JP_LMT_SMEM_KB_BACK
-#define JP_LMT_SMEM_KB_BACK 44
+#define JP_LMT_SMEM_KB_BACK 28
 #endif
 constexpr size_t kSmemMax = 64 * 1024;
 
