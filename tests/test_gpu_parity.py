@@ -496,3 +496,35 @@ def test_edge_cases(cuda_device):
         jp.jp_fwd_tof_sino(xs, xe, img, g.origin, g.voxsize, jp.make_tof(17.0, -1.0, 3.0, 29))
     with pytest.raises(jp.JosephError):
         jp.jp_fwd(xs.cpu(), xe.cpu(), img, g.origin, g.voxsize)   # no CPU fallback
+
+
+def test_forward_projections_are_deterministic(cuda_device, scanner, events, monkeypatch):
+    """no atomics on the forward side: every forward kernel (track tiles, per-track tiles, TOF sinogram window,
+    listmode line tiles and quad gathers) must give bit-identical results from run to run -- a cheap detector of
+    shared-memory races between the phases of a tile (compute-sanitizer is not available on the test pool)"""
+    g, ph = scanner
+    img = dev(ph, cuda_device)
+    tofp = inputs.TofParams()
+    tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins)
+    xs, xe = inputs.sinogram_lors(views=[5, 64, 130], radial=range(-40, 41, 8))
+    idx = np.arange(xs.shape[1])
+    keep = torch.from_numpy(((idx // 48) % 48 < 36) & (idx % 48 < 36))
+    lists = [(xs.to(cuda_device), xe.to(cuda_device)), (xs[:, keep].contiguous().to(cuda_device), xe[:, keep].contiguous().to(cuda_device))]
+    for a, b in lists:
+        ref = jp.jp_fwd(a, b, img, g.origin, g.voxsize).clone()
+        for _ in range(3):
+            assert torch.equal(jp.jp_fwd(a, b, img, g.origin, g.voxsize), ref)
+    a, b = lists[0][0][:, :20_000].contiguous(), lists[0][1][:, :20_000].contiguous()
+    ref = jp.jp_fwd_tof_sino(a, b, img, g.origin, g.voxsize, tof).clone()
+    for _ in range(3):
+        assert torch.equal(jp.jp_fwd_tof_sino(a, b, img, g.origin, g.voxsize, tof), ref)
+    ex, ee, tb = (t.to(cuda_device) for t in events)
+    for tile in ("1", "0"):
+        monkeypatch.setenv("JP_LM_TILE", tile)
+        plan = jp.LmPlan(ex, ee, tb, g.n, g.origin, g.voxsize, tof, n_subsets=1)
+        ref = jp.jp_fwd_tof_lm_planned(plan, img).clone()
+        refn = jp.jp_fwd_lm_planned(plan, img).clone()
+        for _ in range(3):
+            assert torch.equal(jp.jp_fwd_tof_lm_planned(plan, img), ref)
+            assert torch.equal(jp.jp_fwd_lm_planned(plan, img), refn)
+        plan.destroy()
