@@ -167,6 +167,31 @@ __device__ __forceinline__ void walk(const PRay &q, const GTab &gt, uint32_t tab
     }
 }
 
+// The block's [nvalid][nbins] tile in global memory is contiguous: thread t visits elements t, t + 256, ... (fully
+// coalesced), four at a time so that four independent loads are in flight; (lor, bin) of an element advance by
+// (256 / nbins, 256 % nbins) from one visit to the next, no division in the loop.
+struct TileIdx {
+    int x, lor, kb;
+};
+__device__ __forceinline__ TileIdx tile_first(int tid, int nbins)
+{
+    TileIdx i;
+    i.x = tid;
+    i.lor = tid / nbins;
+    i.kb = tid - i.lor * nbins;
+    return i;
+}
+__device__ __forceinline__ void tile_next(TileIdx &i, int dq, int dr, int nbins)
+{
+    i.x += kSBlock;
+    i.lor += dq;
+    i.kb += dr;
+    if (i.kb >= nbins) {
+        i.kb -= nbins;
+        ++i.lor;
+    }
+}
+
 template <int NBW, bool BACK>
 __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
     k_tof_sino_win(Lors l, int64_t n, int64_t nblocks, const float *__restrict__ pimg_r, float *__restrict__ pimg_w,
@@ -175,8 +200,9 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);                                       // [(kGK + 2)][NBW]
     float *stage = reinterpret_cast<float *>(smem_raw + (size_t)(kGK + 2) * NBW * sizeof(float2)); // [nbins][kSLd]
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x;
     const int nbins = t.nbins;
+    const int dq = kSBlock / nbins, dr = kSBlock % nbins; // (lor, bin) step of the flattened tile walk
     for (int i = tid; i < (kGK + 2) * NBW; i += kSBlock) tab[i] = __ldg(gt.tab + i);
     if (!BACK)
         for (int i = tid; i < nbins * kSLd; i += kSBlock) stage[i] = 0.f;
@@ -230,8 +256,21 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
                 for (int kb = 0; kb < nbins; ++kb) stage[kb * kSLd + tid] = v;
             } else {
                 const float *in = y + j0 * nbins;
-                for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
-                    for (int kb = lane; kb < nbins; kb += 32) stage[kb * kSLd + lor] = in[lor * nbins + kb];
+                const int tot = nvalid * nbins;
+                TileIdx it = tile_first(tid, nbins);
+                while (it.x < tot) {
+                    TileIdx e[4];
+                    float v[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        e[u] = it;
+                        v[u] = (it.x < tot) ? in[it.x] : 0.f;
+                        tile_next(it, dq, dr, nbins);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (e[u].x < tot) stage[e[u].kb * kSLd + e[u].lor] = v[u];
+                }
             }
             __syncthreads();
         }
@@ -244,24 +283,39 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
         __syncthreads();
         if (!BACK) { // write the tile (and clear it for the next block)
             float *out = p + j0 * nbins;
+            const int tot = nvalid * nbins;
+            TileIdx it = tile_first(tid, nbins);
             if (epi.y_em) { // OSEM ratio instead of the projection (reading S2)
                 const float *ye = epi.y_em + j0 * nbins;
                 const float *ct = epi.contam ? epi.contam + j0 * nbins : nullptr;
-                for (int lor = warp; lor < nvalid; lor += kSBlock / 32) {
-                    const float mj = epi.mult ? epi.mult[j0 + lor] : 1.f;
-                    for (int kb = lane; kb < nbins; kb += 32) {
-                        const int x = lor * nbins + kb;
-                        const float yb = fmaf(mj, stage[kb * kSLd + lor], ct ? ct[x] : 0.f);
-                        out[x] = (yb > 1e-9f) ? mj * ye[x] / yb : 0.f;
-                        stage[kb * kSLd + lor] = 0.f;
+                while (it.x < tot) {
+                    TileIdx e[4];
+                    float yv[4], cv[4], mv[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        e[u] = it;
+                        const bool ok = it.x < tot;
+                        yv[u] = ok ? ye[it.x] : 0.f;
+                        cv[u] = (ok && ct) ? ct[it.x] : 0.f;
+                        mv[u] = (ok && epi.mult) ? epi.mult[j0 + it.lor] : 1.f;
+                        tile_next(it, dq, dr, nbins);
                     }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (e[u].x < tot) {
+                            const int sidx = e[u].kb * kSLd + e[u].lor;
+                            const float yb = fmaf(mv[u], stage[sidx], cv[u]);
+                            out[e[u].x] = (yb > 1e-9f) ? mv[u] * yv[u] / yb : 0.f;
+                            stage[sidx] = 0.f;
+                        }
                 }
             } else {
-                for (int lor = warp; lor < nvalid; lor += kSBlock / 32)
-                    for (int kb = lane; kb < nbins; kb += 32) {
-                        out[lor * nbins + kb] = stage[kb * kSLd + lor];
-                        stage[kb * kSLd + lor] = 0.f;
-                    }
+                while (it.x < tot) {
+                    const int sidx = it.kb * kSLd + it.lor;
+                    out[it.x] = stage[sidx];
+                    stage[sidx] = 0.f;
+                    tile_next(it, dq, dr, nbins);
+                }
             }
             __syncthreads();
         }
