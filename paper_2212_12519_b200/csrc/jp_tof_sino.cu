@@ -29,6 +29,9 @@ namespace {
 
 constexpr int kSBlock = 256;
 constexpr int kSLd = kSBlock + 1;
+#ifndef JP_SINO_IO
+#define JP_SINO_IO 4 // tile elements per thread in flight
+#endif
 #ifndef JP_SINO_GK
 #define JP_SINO_GK 512
 #endif
@@ -259,16 +262,16 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
                 const int tot = nvalid * nbins;
                 TileIdx it = tile_first(tid, nbins);
                 while (it.x < tot) {
-                    TileIdx e[4];
-                    float v[4];
+                    TileIdx e[JP_SINO_IO];
+                    float v[JP_SINO_IO];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
+                    for (int u = 0; u < JP_SINO_IO; ++u) {
                         e[u] = it;
                         v[u] = (it.x < tot) ? in[it.x] : 0.f;
                         tile_next(it, dq, dr, nbins);
                     }
 #pragma unroll
-                    for (int u = 0; u < 4; ++u)
+                    for (int u = 0; u < JP_SINO_IO; ++u)
                         if (e[u].x < tot) stage[e[u].kb * kSLd + e[u].lor] = v[u];
                 }
             }
@@ -289,10 +292,10 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
                 const float *ye = epi.y_em + j0 * nbins;
                 const float *ct = epi.contam ? epi.contam + j0 * nbins : nullptr;
                 while (it.x < tot) {
-                    TileIdx e[4];
-                    float yv[4], cv[4], mv[4];
+                    TileIdx e[JP_SINO_IO];
+                    float yv[JP_SINO_IO], cv[JP_SINO_IO], mv[JP_SINO_IO];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
+                    for (int u = 0; u < JP_SINO_IO; ++u) {
                         e[u] = it;
                         const bool ok = it.x < tot;
                         yv[u] = ok ? ye[it.x] : 0.f;
@@ -301,7 +304,7 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
                         tile_next(it, dq, dr, nbins);
                     }
 #pragma unroll
-                    for (int u = 0; u < 4; ++u)
+                    for (int u = 0; u < JP_SINO_IO; ++u)
                         if (e[u].x < tot) {
                             const int sidx = e[u].kb * kSLd + e[u].lor;
                             const float yb = fmaf(mv[u], stage[sidx], cv[u]);
