@@ -47,7 +47,7 @@ N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the one `ncu --set full` capture
 # summarised in profiles/r01_v6_ncu_full.txt (bytes; listmode: one launch = the events of one principal axis)
 TRAFFIC = {(1, "fwd"): 3.955821e9 + 1.071657e9, (1, "back"): 4.106105e9 + 0.588588e9,
-           (2, "fwd"): 0.378425e9 + 1.152412e9, (2, "back"): 1.441061e9 + 0.146828e9,
+           (2, "fwd"): 0.393367e9 + 1.155210e9, (2, "back"): 1.424894e9 + 0.139110e9,
            (3, "fwd"): 1.280978e9 + 0.813510e9, (3, "back"): 2.396714e9 + 0.162799e9}
 
 SPEC = {
