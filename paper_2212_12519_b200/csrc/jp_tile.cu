@@ -18,6 +18,7 @@
 // Tiles that are not tracks (ragged tail, principal axis z, unsorted lists) take the generic per-LOR
 // path in the same launch.  No plan, no scratch memory, results in caller order.
 #include <cstdlib>
+#include <mutex>
 
 #include "jp_tile_common.cuh"
 
@@ -954,16 +955,68 @@ cudaError_t set_smem(K kernel, size_t smem)
     }
 
 // probe of the track length (lists long enough for it to matter); *out = device int (stream-ordered scratch) or null
-static cudaError_t probe_tracks(const Lors &l, int64_t n, cudaStream_t st, int **out)
+// The probe result is cached per LOR list, keyed by (device, address of xs, n): repeated projections of the same
+// list (every OSEM iteration, every benchmark step) skip the probe launch, which would otherwise sit in front of the
+// tile kernel on the stream.  Only the ADDRESS is remembered, nothing is dereferenced later; a stale hit (another
+// list at the same address) can only cost speed, never correctness: both instantiations read the same int, and
+// any track length partitions the list.  Events order the int between streams: `ready` after the probe, `used`
+// after the last kernels that read it (an entry is recycled only behind that event).
+struct ProbeEntry {
+    int dev = -1;
+    const void *key = nullptr;
+    int64_t n = 0;
+    int *cut = nullptr;
+    cudaEvent_t ready = nullptr, used = nullptr;
+    unsigned long long stamp = 0;
+};
+static std::mutex g_probe_mu;
+static ProbeEntry g_probe[16];
+static unsigned long long g_probe_clock = 0;
+
+static cudaError_t probe_tracks(const Lors &l, int64_t n, cudaStream_t st, int **out, cudaEvent_t *used)
 {
     *out = nullptr;
+    *used = nullptr;
     if (n < 8 * kTile) return cudaSuccess;
     const char *env = getenv("JP_TRACK_PROBE"); // JP_TRACK_PROBE=0: assume aligned tracks (A/B measurements)
     if (env && env[0] == '0') return cudaSuccess;
-    cudaError_t e = cudaMallocAsync((void **)out, sizeof(int), st);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    k_track_probe<<<1, 1024, 0, st>>>(l, n, *out);
-    return cudaGetLastError();
+    std::lock_guard<std::mutex> lock(g_probe_mu);
+    ProbeEntry *hit = nullptr, *lru = &g_probe[0];
+    for (ProbeEntry &p : g_probe) {
+        if (p.cut && p.dev == dev && p.key == (const void *)l.xs && p.n == n) hit = &p;
+        if (p.stamp < lru->stamp) lru = &p;
+    }
+    if (hit) {
+        hit->stamp = ++g_probe_clock;
+        if ((e = cudaStreamWaitEvent(st, hit->ready, 0)) != cudaSuccess) return e;
+        // chain the users of an entry (a no-op on the same stream), so that `used` always covers all of them
+        if ((e = cudaStreamWaitEvent(st, hit->used, 0)) != cudaSuccess) return e;
+        *out = hit->cut;
+        *used = hit->used;
+        return cudaSuccess;
+    }
+    ProbeEntry &p = *lru;
+    if (!p.cut || p.dev != dev) { // first use of the slot (or another device: the old int is left to that device)
+        p = ProbeEntry{};
+        if ((e = cudaMalloc((void **)&p.cut, sizeof(int))) != cudaSuccess) return e;
+        if ((e = cudaEventCreateWithFlags(&p.ready, cudaEventDisableTiming)) != cudaSuccess) return e;
+        if ((e = cudaEventCreateWithFlags(&p.used, cudaEventDisableTiming)) != cudaSuccess) return e;
+    } else if ((e = cudaStreamWaitEvent(st, p.used, 0)) != cudaSuccess) { // kernels of the evicted list may still read it
+        return e;
+    }
+    p.dev = dev;
+    p.key = (const void *)l.xs;
+    p.n = n;
+    p.stamp = ++g_probe_clock;
+    k_track_probe<<<1, 1024, 0, st>>>(l, n, p.cut);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = cudaEventRecord(p.ready, st)) != cudaSuccess) return e;
+    *out = p.cut;
+    *used = p.used;
+    return cudaSuccess;
 }
 
 static unsigned persistent_grid(int per_sm)
@@ -981,7 +1034,8 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
     if (!c.P) return launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
     int *cut = nullptr;
-    cudaError_t e = probe_tracks(l, n, st, &cut);
+    cudaEvent_t used = nullptr;
+    cudaError_t e = probe_tracks(l, n, st, &cut, &used);
     if (e != cudaSuccess) return e;
     JP_DISPATCH_P(c, {
         e = set_smem(k_fwd_tile<P>, c.smem);
@@ -994,7 +1048,7 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
         }
     })
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (cut) cudaFreeAsync(cut, st);
+    if (used && e == cudaSuccess) e = cudaEventRecord(used, st);
     return e;
 }
 
@@ -1005,7 +1059,8 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
     if (!c.P) return launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);
     const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
     int *cut = nullptr;
-    cudaError_t e = probe_tracks(l, n, st, &cut);
+    cudaEvent_t used = nullptr;
+    cudaError_t e = probe_tracks(l, n, st, &cut, &used);
     if (e != cudaSuccess) return e;
     JP_DISPATCH_P(c, {
         e = set_smem(k_back_tile<P>, c.smem);
@@ -1018,7 +1073,7 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
         }
     })
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (cut) cudaFreeAsync(cut, st);
+    if (used && e == cudaSuccess) e = cudaEventRecord(used, st);
     return e;
 }
 
