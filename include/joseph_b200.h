@@ -29,8 +29,10 @@
  *
  * Memory   Unless a name ends in _host, ALL data pointers are DEVICE pointers owned by the caller
  *           (e.g. torch tensors); jp_geom / jp_tof / jp_lors structs themselves are read on the host
- *           at call time.  Inputs are const.  The library does not keep pointers after a call
- *           returns, except inside a jp_plan (which owns only its own device buffers).
+ *           at call time.  Inputs are const.  The library does not dereference caller pointers after a
+ *           call returns, except inside a jp_plan (which owns only its own device buffers).  jp_fwd / jp_back
+ *           remember the ADDRESS and length of up to 16 LOR lists as the key of a cached 4-byte set-up result
+ *           (track length of the list); a stale key can only cost speed, never change a result.
  * Streams  Every call is asynchronous on the CUDA stream `stream` (a cudaStream_t passed as void*,
  *           NULL = legacy default stream) and never synchronises the device, except the _host calls,
  *           which return after their result is in host memory.
