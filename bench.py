@@ -360,6 +360,35 @@ class Workload:
         out["plane_steps"] = self.jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
         return out
 
+    def time_nonaligned_tracks(self, reps=5):
+        """tracks whose length is not a multiple of the 768-LOR tile: the 36-ring sub-scanner of every 4th view of
+        configs[1] (36 x 36 = 1296 ring pairs per track, 21.3 M LORs); ms per call and plane-steps per second"""
+        jp, s = self.jp, self.stream
+        xs, xe = inputs.sinogram_lors(views=range(0, inputs.N_VIEWS, 4), device=self.dev)
+        idx = torch.arange(xs.shape[1], device=self.dev)
+        keep = ((idx // 48) % 48 < 36) & (idx % 48 < 36)
+        xs, xe = xs[:, keep].contiguous(), xe[:, keep].contiguous()
+        n = xs.shape[1]
+        y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 136, device=self.dev)
+        p = torch.empty(n, dtype=torch.float32, device=self.dev)
+        steps = jp.jp_plane_steps(xs, xe, G.n, G.origin, G.voxsize)
+        f = lambda: jp.jp_fwd(xs, xe, self.img, G.origin, G.voxsize, out=p)
+        b = lambda: jp.jp_back(xs, xe, y, G.n, G.origin, G.voxsize, img=self.bimg)
+        f(); self.bimg.zero_(); b()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record(s)
+        for _ in range(reps):
+            f()
+        ev[1].record(s)
+        for _ in range(reps):
+            self.bimg.zero_()
+            b()
+        ev[2].record(s)
+        torch.cuda.synchronize()
+        fm, bm = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        return {"lors": n, "track_length": 1296, "plane_steps": steps, "fwd_ms": fm, "back_ms": bm,
+                "fwd_plane_steps_per_s": steps / fm * 1e3, "back_plane_steps_per_s": steps / bm * 1e3}
+
     def time_osem_with_resolution_model(self, iters=2):
         """the same OSEM iteration with the 4.5 mm FWHM image-based resolution model
          in every subset (2 x 20 Gaussian smoothings per iteration); seconds per iteration"""
@@ -564,6 +593,8 @@ def run_ours(args):
     }
     if w.plan_s is not None:
         line["config"]["plan_s"] = w.plan_s
+    if c == 1 and world == 1 and not args.no_other:
+        line["nonaligned_tracks_36_rings"] = w.time_nonaligned_tracks()
     if c == 3:
         line["nontof_listmode"] = w.time_nontof_listmode()
     if c >= 4:
