@@ -65,6 +65,32 @@ def test_argument_validation_without_gpu(lib):
         >= (200 * 200 * 96 + 2_000_000) * 4
 
 
+def test_argument_validation_of_the_osem_calls_without_gpu(lib):
+    g = binding.make_geom((4, 4, 4), (0, 0, 0), (1, 1, 1))
+    t = binding.make_tof(17.0, 13.6, 3.0, 29)
+    l = binding.jp_lors(8, 8, 8, 8, 8, 8, 10)
+    P = C.c_void_p(8)
+    off_ok = (C.c_int64 * 3)(0, 4, 10)
+    off_dec = (C.c_int64 * 3)(0, 6, 4)
+    off_out = (C.c_int64 * 3)(0, 4, 11)
+    call = lambda off, ns, sens=P, ws=P, wb=1 << 20: lib.jp_sino_osem_tof(C.byref(l), off, ns, P, None, None, sens, C.byref(g),
+                                                                          C.byref(t), P, 1, ws, wb, None)
+    assert call(off_dec, 2) == -2 and b"non-decreasing" in lib.jp_last_error()
+    assert call(off_out, 2) == -2
+    assert call(off_ok, 0) == -2
+    assert call(None, 2) == -1
+    assert call(off_ok, 2, sens=None) == -1
+    assert call(off_ok, 2, wb=16) == -2 and b"workspace" in lib.jp_last_error()
+    assert lib.jp_sino_osem_tof_workspace_bytes(off_ok, 2, 10, C.byref(t)) >= 6 * 29 * 4
+    assert lib.jp_sino_osem_tof_workspace_bytes(off_dec, 2, 10, C.byref(t)) == 0
+    assert lib.jp_sino_sens_tof(C.byref(l), off_ok, 2, None, C.byref(g), C.byref(t), None, None, 0, None) == -1
+    assert lib.jp_osem_update(None, P, P, 1.0, C.byref(g), None) == -1
+    assert lib.jp_lm_osem_planned_backratio(None, 0, P, P, P, 1 << 20, None) == -4
+    assert lib.jp_fwd_tof_sino_host(None, P, C.byref(g), C.byref(t), P) == -1
+    bad = binding.make_tof(17.0, 13.6, 3.0, 0)
+    assert lib.jp_fwd_tof_sino_host(C.byref(l), P, C.byref(g), C.byref(bad), P) == -2
+
+
 def test_no_cpu_fallback():
     import torch
     x = torch.zeros((3, 4))
