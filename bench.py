@@ -524,6 +524,11 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
             "algorithmic_bytes_per_launch": w.hbm_bytes,
             "peak_source": src, "plane_steps_per_launch": w.plane_steps, "lane_instr_per_plane_step": lane,
             "fwd": per(fwd_ms, kf), "back": per(back_ms, kb),
+            # the same work counted in flops against 2 flop x lane peak (a tighter roof for the non-TOF
+            # pair: 16 / 14 flop per plane-step forward / back; the headline `frac` counts instruction slots)
+            **({"flop_based": {"peak_tflops": 2 * alu_peak / 1e12,
+                               "fwd_frac": 16.0 * w.plane_steps / (fwd_ms * 1e-3) / (2 * alu_peak),
+                               "back_frac": 14.0 * w.plane_steps / (back_ms * 1e-3) / (2 * alu_peak)}} if w.c == 1 else {}),
             "hbm_bound_frac": w.hbm_bytes / (dom_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9)}
 
 
