@@ -532,6 +532,23 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
             "hbm_bound_frac": w.hbm_bytes / (dom_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9)}
 
 
+def measure_fp32_rate(jp, dev):
+    """FFMA lane-instructions per second of jp_fma_burn (148 x 8 CTAs of 256 threads, 8 independent chains per thread),
+    best of 5 after a warm-up, CUDA events on the current stream"""
+    scratch = torch.zeros(4, dtype=torch.float32, device=dev)
+    blocks, iters = N_SM * 8, 20000
+    jp.jp_fma_burn(scratch, blocks, iters)
+    best = 0.0
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        n = jp.jp_fma_burn(scratch, blocks, iters)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, n / (e0.elapsed_time(e1) * 1e-3))
+    return best
+
+
 def run_ours(args):
     from paper_2212_12519_b200 import binding as jp
     import torch.distributed as dist
@@ -598,6 +615,10 @@ def run_ours(args):
     }
     if w.plan_s is not None:
         line["config"]["plan_s"] = w.plan_s
+    if world == 1:
+        rate = measure_fp32_rate(jp, dev)
+        line["roofline"]["fp32_ffma_measured"] = {"value": rate / 1e12, "unit": "T lane-instr/s (FP32 FFMA, jp_fma_burn)",
+                                                  "frac_of_nominal_peak": rate / (line["roofline"]["peak"] * 1e12)}
     if c == 1 and world == 1 and not args.no_other:
         line["nonaligned_tracks_36_rings"] = w.time_nonaligned_tracks()
     if c == 3:

@@ -89,6 +89,7 @@ EXPORTS = {
                                      C.c_void_p]),
     "jp_back_tof_lm_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
                                       C.c_void_p]),
+    "jp_fma_burn": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
     "jp_version": (C.c_int, []),
 }
@@ -607,3 +608,10 @@ def jp_back_tof_lm_host(xstart, xend, tofbin, y, img, origin, voxsize, tof: jp_t
     _check(load().jp_back_tof_lm_host(C.byref(l), tofbin.data_ptr(), y.data_ptr(), C.byref(g), C.byref(tof),
                                       img.data_ptr()), "jp_back_tof_lm_host")
     return img
+
+
+def jp_fma_burn(scratch: torch.Tensor, blocks: int, iters: int, stream=None) -> int:
+    """enqueue the FP32 FFMA microbenchmark; returns the number of lane-instructions (FFMAs) it executes"""
+    _dev(scratch, torch.float32, "scratch")
+    _check(load().jp_fma_burn(scratch.data_ptr(), int(blocks), int(iters), _stream(stream)), "jp_fma_burn")
+    return int(blocks) * 256 * 16 * int(iters)
