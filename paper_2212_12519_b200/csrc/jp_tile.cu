@@ -983,6 +983,9 @@ static cudaError_t probe_tracks(const Lors &l, int64_t n, cudaStream_t st, int *
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone)
+        return cudaSuccess; // inside a graph capture: no allocation, no cross-stream events -- plain tiles (always correct)
     std::lock_guard<std::mutex> lock(g_probe_mu);
     ProbeEntry *hit = nullptr, *lru = &g_probe[0];
     for (ProbeEntry &p : g_probe) {
