@@ -292,7 +292,7 @@ class Workload:
             else:
                 self.sens = torch.ones(G.n, dtype=torch.float32, device=dev)   # replaced by A^T 1 in setup_sens()
                 self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
-                self.launches = 3 * 20 + 2
+                self.launches = 4 * 20 + 1   # per subset: quad build, fused projector per axis (x, y), update
 
     def setup_sens(self):
         """configs[4]: sens = non-TOF back projection of ones over all configs[1] LORs (one-time, untimed)"""
@@ -503,7 +503,7 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
     kf, kb = w.kinds
     names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
-             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_fwd_tof_lm_quad + k_back_tof_lm_quad", ""),
+             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_osem_tof_lm_quad (forward + ratio + back per event)", ""),
              5: ("k_tof_sino_win<6,fwd+ratio> + k_tof_sino_win<6,back>", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
     if w.c in (4, 5):

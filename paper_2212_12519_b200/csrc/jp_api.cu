@@ -624,11 +624,9 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                 xin = xb;
             }
             JP_CUDA(jp::launch_quad_build(xin, c.g, q[0], q[1], st), where);
-            for (int a = 0; a < 2; ++a)
-                JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, r, 1, st), where);
-            for (int a = 0; a < 2; ++a) {
+            for (int a = 0; a < 2; ++a) { // forward, ratio and back of the subset's events in one pass per axis
                 JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
-                JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st), where);
+                JP_CUDA(jp::launch_osem_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, b[a], st), where);
             }
             if (z_events) {
                 float *px = nullptr, *pb = nullptr;
@@ -833,11 +831,9 @@ int jp_lm_osem_planned_backratio(const jp_plan *plan, int subset, const float *x
     }
     const int m = subset;
     JP_CUDA(jp::launch_quad_build(x, c.g, q[0], q[1], st), where);
-    for (int a = 0; a < 2; ++a)
-        JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, r, 1, st), where);
     for (int a = 0; a < 2; ++a) {
         JP_CUDA(cudaMemsetAsync(qb[a], 0, qbytes, st), where);
-        JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, qb[a], st), where);
+        JP_CUDA(jp::launch_osem_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, qb[a], st), where);
     }
     JP_CUDA(jp::launch_quad_merge(qb[0], qb[1], c.g, b, st), where);
     if (c.has_axis2(m)) {

@@ -91,6 +91,9 @@ cudaError_t launch_quad_osem_update(float *x, const float4 *b0, const float4 *b1
                                     float scale, const Geom &g, cudaStream_t st);
 cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float4 *q, const Geom &g,
                                    const Tof &t, const TofLut &lut, float *p, int lm_mode, cudaStream_t st);
+// forward + ratio + back of one OSEM subset in one pass (quad image in, quad accumulator out)
+cudaError_t launch_osem_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float4 *q, const Geom &g,
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
 cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
                                     const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
 

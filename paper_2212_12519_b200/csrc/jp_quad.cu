@@ -176,6 +176,52 @@ __global__ void __launch_bounds__(kQBlock) k_back_tof_lm_quad(Lors l, const int1
     }
 }
 
+
+// ---- one OSEM subset update per event in ONE pass (reading A14): ybar_e from the quad image, r_e = 1 / ybar_e, and
+// the scatter of cf r_e w along the same planes into the quad accumulator.  The event's set-up (float64) is done
+// once instead of twice, the ratio never goes through memory, and gathers (L1-bound) and atomics (L2-bound) of
+// different warps overlap in one launch.
+__global__ void __launch_bounds__(kQBlock) k_osem_tof_lm_quad(Lors l, const int16_t *__restrict__ tofbin, Range rg,
+                                                              const float4 *__restrict__ q, Geom g, Tof t, TofLut lut,
+                                                              float4 *__restrict__ b)
+{
+    extern __shared__ __align__(16) float2 lut_sm[];
+    lut_load(lut, lut_sm);
+    __syncthreads();
+    const uint32_t lb = lut_base(lut_sm);
+    const int64_t c = blockIdx.x * (int64_t)kQBlock + threadIdx.x;
+    if (c >= rg.count) return;
+    const int64_t j = rg.first + c * rg.stride;
+    const float half_w = 0.5f * t.width;
+    const float centre = (float)tofbin[j] * t.width;
+    const float reach = half_w + t.nsig * t.sigma;
+    Ray r;
+    ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
+    const PRay pr = pray_from(r, g);
+    float acc = 0.f, fk = 0.f;
+    int po = pr.off;
+    for (int k = 0; k < pr.nk; ++k) {
+        const PCell cl = pray_cell(pr, fk, po);
+        const float tau = fmaf(pr.dtau, fk, pr.tau0);
+        acc = fmaf(quad_value(q, cl), tof_weight(lb, lut.inv_h, half_w, tau, centre), acc);
+        fk += 1.f;
+        po += pr.sp;
+    }
+    const float ybar = pr.cf * acc;
+    if (!(ybar > 1e-9f)) return;
+    const float x = pr.cf * (1.f / ybar);
+    fk = 0.f;
+    po = pr.off;
+    for (int k = 0; k < pr.nk; ++k) {
+        const PCell cl = pray_cell(pr, fk, po);
+        const float tau = fmaf(pr.dtau, fk, pr.tau0);
+        const float w = tof_weight(lb, lut.inv_h, half_w, tau, centre);
+        if (w != 0.f) quad_scatter(b, cl, x * w);
+        fk += 1.f;
+        po += pr.sp;
+    }
+}
+
 // ---- launchers ------------------------------------------------------------------------------------------------
 static inline unsigned grid_for(int64_t n) { return (unsigned)((n + kQBlock - 1) / kQBlock); }
 constexpr size_t kLutBytesQ = (size_t)kLutN * sizeof(float2);
@@ -218,6 +264,14 @@ cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range 
 {
     if (rg.count == 0) return cudaSuccess;
     k_back_tof_lm_quad<<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, b);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_osem_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float4 *q, const Geom &g,
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st)
+{
+    if (rg.count == 0) return cudaSuccess;
+    k_osem_tof_lm_quad<<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, q, g, t, lut, b);
     return cudaGetLastError();
 }
 
