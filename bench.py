@@ -259,8 +259,8 @@ class Workload:
             self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
             self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
             self.kinds = ("sino", "sino")
-            self.launches = nsub * 3 + 4
-            self.hbm_bytes = self.n * (24 + 4 + 4 * 4 * nb) // 2   # per direction: end points, y + contam in, r out / r in
+            self.launches = nsub * 3     # per subset: weight table, fused forward + ratio + back kernel, image update
+            self.hbm_bytes = self.n * (24 + 4 + 2 * 4 * nb) // 2   # x 2 in the roofline dict: end points, mult, y + contam once per iteration
         elif c in (1, 2):
             self.xs, self.xe = inputs.sinogram_lors(views=None if c == 1 else inputs.SUBSET_VIEWS, device=dev)
             self.n = self.xs.shape[1]
@@ -504,7 +504,7 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     kf, kb = w.kinds
     names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
              3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_osem_tof_lm_quad (forward + ratio + back per event)", ""),
-             5: ("k_tof_sino_win<6,fwd+ratio> + k_tof_sino_win<6,back>", "")}[w.c]
+             5: ("k_tof_sino_osem<6> (forward + ratio + back per LOR block)", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
     if w.c in (4, 5):
         lane = 2 * LANE["lm" if w.c == 4 else "sino"]

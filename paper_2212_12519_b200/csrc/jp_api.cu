@@ -787,15 +787,14 @@ int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_s
                 e.y_em = y + (size_t)a * nb;
                 e.mult = mult ? mult + a : nullptr;
                 e.contam = contam ? contam + (size_t)a * nb : nullptr;
-                cudaError_t rc = jp::launch_tof_sino_win(false, ls, cnt, cx.pimg, nullptr, g, t, r, nullptr, st, &e);
+                // one fused pass (forward, ratio, back); the unfused generic kernels when the TOF window is too wide
+                cudaError_t rc = jp::launch_tof_sino_osem(ls, cnt, cx.pimg, cb.pimg, g, t, e, st);
                 if (rc == cudaErrorNotSupported) {
                     rc = jp::launch_fwd_tof_sino(ls, whole(cnt), cx.pimg, g, t, cx.lut, r, st);
                     if (rc == cudaSuccess) rc = jp::launch_sino_ratio(r, e.y_em, e.mult, e.contam, cnt, nb, st);
+                    if (rc == cudaSuccess) rc = jp::launch_back_tof_sino(ls, whole(cnt), r, g, t, cx.lut, cb.pimg, st);
                 }
-                JP_CUDA(rc, "jp_sino_osem_tof (forward)");
-                rc = jp::launch_tof_sino_win(true, ls, cnt, nullptr, cb.pimg, g, t, nullptr, r, st);
-                if (rc == cudaErrorNotSupported) rc = jp::launch_back_tof_sino(ls, whole(cnt), r, g, t, cx.lut, cb.pimg, st);
-                JP_CUDA(rc, "jp_sino_osem_tof (back)");
+                JP_CUDA(rc, "jp_sino_osem_tof (subset pass)");
             }
             JP_CUDA(jp::launch_osem_update_padded(img, cx.pimg, cb.pimg, sens + (size_t)m * nvox, 1.f, g, st),
                     "jp_sino_osem_tof (update)");

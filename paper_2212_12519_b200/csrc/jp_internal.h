@@ -63,6 +63,10 @@ struct SinoEpi {
 cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g,
                                 const Tof &t, float *p, const float *y, cudaStream_t st, const SinoEpi *epi = nullptr);
 
+// one OSEM subset pass in one kernel: pimg_w += A^T (mult y / (mult A pimg_r + contam)); epi.y_em must be set
+cudaError_t launch_tof_sino_osem(const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g, const Tof &t,
+                                 const SinoEpi &epi, cudaStream_t st);
+
 // r <- mult y / (mult r + contam) (reading S2) and r <- mult broadcast over the bins: the unfused stages used
 // with the generic TOF sinogram kernels
 cudaError_t launch_sino_ratio(float *r, const float *y, const float *mult, const float *contam, int64_t n, int nbins,

@@ -325,6 +325,92 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
     }
 }
 
+// ---- one OSEM subset update per LOR in ONE pass (readings S1-S3): forward walk into the shared tile, ratio in place
+// (mult y / (mult p + contam), emission and contamination tiles read as flat coalesced ranges), back walk out of the
+// same tile.  The ratio sinogram never goes through global memory and the float64 ray set-up is done once.
+template <int NBW>
+__global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
+    k_tof_sino_osem(Lors l, int64_t n, int64_t nblocks, const float *__restrict__ pimg_r, float *__restrict__ pimg_w,
+                    Geom g, Tof t, GTab gt, SinoEpi epi)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *tab = reinterpret_cast<float2 *>(smem_raw);                                       // [(kGK + 2)][NBW]
+    float *stage = reinterpret_cast<float *>(smem_raw + (size_t)(kGK + 2) * NBW * sizeof(float2)); // [nbins][kSLd]
+    const int tid = threadIdx.x;
+    const int nbins = t.nbins;
+    const int dq = kSBlock / nbins, dr = kSBlock % nbins;
+    for (int i = tid; i < (kGK + 2) * NBW; i += kSBlock) tab[i] = __ldg(gt.tab + i);
+    for (int i = tid; i < nbins * kSLd; i += kSBlock) stage[i] = 0.f;
+    const uint32_t tab_addr = smem_addr(tab) - (uint32_t)kMagicI * (uint32_t)(NBW * 8);
+    const float lim = t.nsig * t.sigma;
+    const float reach = 0.5f * (float)(nbins - 1) * t.width + 0.5f * t.width + lim;
+    __syncthreads();
+
+    for (int64_t blk = blockIdx.x; blk < nblocks; blk += gridDim.x) {
+        const int64_t j0 = blk * kSBlock, j = j0 + tid;
+        const int nvalid = (int)min((int64_t)kSBlock, n - j0);
+        PRay q;
+        q.nk = 0;
+        if (j < n) {
+            Ray r;
+            ray_setup<true>(l, j, g, t.coff, -reach, reach, r);
+            q = pray_from(r, g);
+        }
+        const bool any = __syncthreads_or(q.nk > 0) != 0;
+        if (!any) continue; // no LOR of the block meets the image: nothing to add
+        const int tot = nvalid * nbins;
+        { // the tiles the ratio stage will read, one 128-byte line per thread
+            const int64_t o = j0 * nbins + (int64_t)tid * 32;
+            if (o < (j0 + nvalid) * nbins) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(epi.y_em + o));
+                if (epi.contam) asm volatile("prefetch.global.L2 [%0];" ::"l"(epi.contam + o));
+            }
+        }
+        if (q.nk > 0) {
+            if (q.s2 == 1)
+                walk<NBW, false, true>(q, gt, tab_addr, stage, nbins, pimg_r, nullptr);
+            else
+                walk<NBW, false, false>(q, gt, tab_addr, stage, nbins, pimg_r, nullptr);
+        }
+        __syncthreads();
+        { // ratio in place (LORs that miss the image keep p = 0: their ratio is never walked)
+            const float *ye = epi.y_em + j0 * nbins;
+            const float *ct = epi.contam ? epi.contam + j0 * nbins : nullptr;
+            TileIdx it = tile_first(tid, nbins);
+            while (it.x < tot) {
+                TileIdx e[JP_SINO_IO];
+                float yv[JP_SINO_IO], cv[JP_SINO_IO], mv[JP_SINO_IO];
+#pragma unroll
+                for (int u = 0; u < JP_SINO_IO; ++u) {
+                    e[u] = it;
+                    const bool ok = it.x < tot;
+                    yv[u] = ok ? ye[it.x] : 0.f;
+                    cv[u] = (ok && ct) ? ct[it.x] : 0.f;
+                    mv[u] = (ok && epi.mult) ? epi.mult[j0 + it.lor] : 1.f;
+                    tile_next(it, dq, dr, nbins);
+                }
+#pragma unroll
+                for (int u = 0; u < JP_SINO_IO; ++u)
+                    if (e[u].x < tot) {
+                        const int sidx = e[u].kb * kSLd + e[u].lor;
+                        const float yb = fmaf(mv[u], stage[sidx], cv[u]);
+                        stage[sidx] = (yb > 1e-9f) ? mv[u] * yv[u] / yb : 0.f;
+                    }
+            }
+        }
+        __syncthreads();
+        if (q.nk > 0) {
+            if (q.s2 == 1)
+                walk<NBW, true, true>(q, gt, tab_addr, stage, nbins, nullptr, pimg_w);
+            else
+                walk<NBW, true, false>(q, gt, tab_addr, stage, nbins, nullptr, pimg_w);
+        }
+        __syncthreads();
+        for (int i = tid; i < nbins * kSLd; i += kSBlock) stage[i] = 0.f; // the forward walk of the next block starts from zeros
+        __syncthreads();
+    }
+}
+
 int window_bins(const Tof &t, double *R_out)
 {
     const double m = (double)t.nsig * (double)t.sigma;
@@ -394,6 +480,57 @@ cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float
         default: e = cudaErrorNotSupported;
         }
 #undef JP_WIN
+    }
+    cudaFreeAsync(tab, st);
+    return e;
+}
+
+// fused OSEM subset pass (forward + ratio + back); cudaErrorNotSupported as for launch_tof_sino_win
+namespace {
+template <int NBW>
+cudaError_t launch_osem_win(const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g, const Tof &t,
+                            const GTab &gt, const SinoEpi &epi, cudaStream_t st)
+{
+    const size_t smem = win_smem(NBW, t.nbins);
+    auto kern = k_tof_sino_osem<NBW>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int dev = 0, nsm = 0, per_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kSBlock, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorInvalidConfiguration;
+    const int64_t nblocks = (n + kSBlock - 1) / kSBlock;
+    const int64_t cap = (int64_t)nsm * per_sm;
+    kern<<<(unsigned)(nblocks < cap ? nblocks : cap), kSBlock, smem, st>>>(l, n, nblocks, pimg_r, pimg_w, g, t, gt, epi);
+    return cudaGetLastError();
+}
+} // namespace
+
+cudaError_t launch_tof_sino_osem(const Lors &l, int64_t n, const float *pimg_r, float *pimg_w, const Geom &g, const Tof &t,
+                                 const SinoEpi &epi, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    double R;
+    const int nbw = window_bins(t, &R);
+    if (!nbw || win_smem(nbw, t.nbins) > 72 * 1024) return cudaErrorNotSupported;
+    float2 *tab = nullptr;
+    const int ne = (kGK + 2) * nbw;
+    cudaError_t e = cudaMallocAsync((void **)&tab, sizeof(float2) * ne, st);
+    if (e != cudaSuccess) return e;
+    const double m = (double)t.nsig * (double)t.sigma;
+    k_tof_gtab<<<(ne + 255) / 256, 256, 0, st>>>(tab, nbw, R, (double)t.width, m, 1.0 / ((double)t.sigma * 1.4142135623730951));
+    e = cudaGetLastError();
+    GTab gt{tab, (float)(0.5 * (double)(t.nbins - 1) - R), 1.f / t.width};
+    if (e == cudaSuccess) {
+        switch (nbw) {
+        case 4: e = launch_osem_win<4>(l, n, pimg_r, pimg_w, g, t, gt, epi, st); break;
+        case 6: e = launch_osem_win<6>(l, n, pimg_r, pimg_w, g, t, gt, epi, st); break;
+        case 8: e = launch_osem_win<8>(l, n, pimg_r, pimg_w, g, t, gt, epi, st); break;
+        case 12: e = launch_osem_win<12>(l, n, pimg_r, pimg_w, g, t, gt, epi, st); break;
+        default: e = cudaErrorNotSupported;
+        }
     }
     cudaFreeAsync(tab, st);
     return e;
