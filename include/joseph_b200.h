@@ -203,8 +203,9 @@ int jp_lm_osem_planned_res(const jp_plan *plan, const float *sens, float *img, i
  * subset_offsets: HOST array of n_subsets + 1 non-decreasing offsets in [0, lors->n].  y, contam: device,
  * [lors->n][n_tofbins]; mult: device [lors->n]; mult or contam may be NULL (= 1, = 0).  sens: device
  * [n_subsets][n0*n1*n2].  img: in = start image, out = result.  workspace: device, at least
- * jp_sino_osem_tof_workspace_bytes() bytes (the ratio sinogram of the largest subset).  The forward projection
- * writes the ratio directly (fused epilogue); everything is asynchronous on `stream`, no host synchronisation. */
+ * jp_sino_osem_tof_workspace_bytes() bytes (the ratio sinogram of the largest subset; only used when the TOF kernel is
+ * wider than the fused kernel supports -- otherwise forward, ratio and back of a subset run as one kernel and the
+ * ratio never leaves the chip).  Everything is asynchronous on `stream`, no host synchronisation. */
 size_t jp_sino_osem_tof_workspace_bytes(const int64_t *subset_offsets, int n_subsets, int64_t n, const jp_tof *tof);
 /* sens[m] = A_m^T (mult (x) 1_bins) for every subset; OVERWRITES sens.  workspace may be NULL unless the TOF
  * kernel is wider than the fused kernels support (then as for jp_sino_osem_tof). */
