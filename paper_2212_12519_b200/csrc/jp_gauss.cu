@@ -6,6 +6,7 @@
 // (axis 2, 1, 0); every pass reads and writes the 15 MB image once from L2.  Taps are computed on the host in
 // float64 and travel as kernel parameters.
 #include <cmath>
+#include <cstdint>
 
 #include "jp_internal.h"
 
@@ -35,7 +36,8 @@ bool make_taps(double sigma_mm, double nsig, double v, Taps *t)
     return true;
 }
 
-// out[i] = sum_k w[k] in[i - k e_AXIS], zero outside; one thread per voxel (neighbours come from L1 / L2)
+// out[i] = sum_k w[k] in[i - k e_AXIS], zero outside; one thread per voxel (neighbours come from L1 / L2).
+// Generic pass: any image shape.
 template <int AXIS>
 __global__ void __launch_bounds__(256) k_gauss_axis(const float *__restrict__ in, float *__restrict__ out, int n0, int n1,
                                                      int n2, Taps t)
@@ -57,6 +59,69 @@ __global__ void __launch_bounds__(256) k_gauss_axis(const float *__restrict__ in
     out[i] = acc;
 }
 
+// ---- fast path (n2 a multiple of 4, 16-byte aligned images, n2 <= kGZ): two kernels instead of three passes --------
+// k_gauss_zy: a CTA takes one image plane i0 and kGY rows of it (+ halo): the axis-2 pass goes from global memory
+// into a shared tile, the axis-1 pass out of the tile -- the intermediate image never leaves the SM.
+// k_gauss_x4: axis-0 pass, four consecutive voxels of axis 2 per thread (128-bit loads, coalesced).
+constexpr int kGY = 32;  // rows per CTA
+constexpr int kGZ = 128; // largest n2 of the fast path
+
+__global__ void __launch_bounds__(256) k_gauss_zy(const float *__restrict__ in, float *__restrict__ out, int n0, int n1,
+                                                   int n2, Taps tz, Taps ty)
+{
+    extern __shared__ float tile[]; // [(kGY + 2 ry)][n2]
+    const int i0 = blockIdx.y, y0 = blockIdx.x * kGY;
+    const int ry = ty.r, rz = tz.r;
+    const int rows = kGY + 2 * ry;
+    const float *plane = in + (int64_t)i0 * n1 * n2;
+    // axis-2 pass of rows y0 - ry .. y0 + kGY + ry - 1 (zero outside the image)
+    for (int e = threadIdx.x; e < rows * n2; e += 256) {
+        const int r = e / n2, z = e - r * n2;
+        const int y = y0 - ry + r;
+        float acc = 0.f;
+        if ((unsigned)y < (unsigned)n1) {
+            const float *row = plane + (int64_t)y * n2;
+            for (int k = -rz; k <= rz; ++k) {
+                const int j = z - k;
+                if ((unsigned)j < (unsigned)n2) acc = fmaf(tz.w[k + rz], __ldg(row + j), acc);
+            }
+        }
+        tile[e] = acc;
+    }
+    __syncthreads();
+    // axis-1 pass out of the tile
+    float *oplane = out + (int64_t)i0 * n1 * n2;
+    for (int e = threadIdx.x; e < kGY * n2; e += 256) {
+        const int r = e / n2, z = e - r * n2;
+        const int y = y0 + r;
+        if (y >= n1) break;
+        float acc = 0.f;
+        for (int k = -ry; k <= ry; ++k) acc = fmaf(ty.w[k + ry], tile[(r + ry - k) * n2 + z], acc);
+        oplane[(int64_t)y * n2 + z] = acc;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_gauss_x4(const float4 *__restrict__ in, float4 *__restrict__ out, int n0,
+                                                   int plane4 /* n1 n2 / 4 */, Taps t)
+{
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= n0 * plane4) return;
+    const int i0 = i / plane4;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = -t.r; k <= t.r; ++k) {
+        const int j = i0 - k;
+        if ((unsigned)j < (unsigned)n0) {
+            const float4 v = __ldg(in + i - k * plane4);
+            const float w = t.w[k + t.r];
+            acc.x = fmaf(w, v.x, acc.x);
+            acc.y = fmaf(w, v.y, acc.y);
+            acc.z = fmaf(w, v.z, acc.z);
+            acc.w = fmaf(w, v.w, acc.w);
+        }
+    }
+    out[i] = acc;
+}
+
 } // namespace
 
 // tmp: nvox floats of scratch (may not alias in / out); in may alias out.  cudaErrorInvalidValue: radius too large
@@ -67,6 +132,19 @@ cudaError_t launch_gauss3d(const float *in, float *out, float *tmp, const Geom &
     for (int a = 0; a < 3; ++a)
         if (!make_taps((double)sigma_mm, (double)nsig, (double)g.v[a], &t[a])) return cudaErrorInvalidValue;
     const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    const bool fast = (g.n[2] % 4 == 0) && g.n[2] <= kGZ && nvox < ((int64_t)1 << 31) &&
+                      (((uintptr_t)in | (uintptr_t)out | (uintptr_t)tmp) % 16 == 0);
+    if (fast) { // in -> tmp (axes 2 and 1 in one kernel), tmp -> out (axis 0); in may alias out
+        const size_t smem = (size_t)(kGY + 2 * t[1].r) * g.n[2] * sizeof(float);
+        cudaError_t e = cudaFuncSetAttribute(k_gauss_zy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const dim3 grid((unsigned)((g.n[1] + kGY - 1) / kGY), (unsigned)g.n[0]);
+        k_gauss_zy<<<grid, 256, smem, st>>>(in, tmp, g.n[0], g.n[1], g.n[2], t[2], t[1]);
+        const int plane4 = g.n[1] * g.n[2] / 4;
+        k_gauss_x4<<<(unsigned)(((int64_t)g.n[0] * plane4 + 255) / 256), 256, 0, st>>>(
+            reinterpret_cast<const float4 *>(tmp), reinterpret_cast<float4 *>(out), g.n[0], plane4, t[0]);
+        return cudaGetLastError();
+    }
     const unsigned grid = (unsigned)((nvox + 255) / 256);
     // in -> out (axis 2), out -> tmp (axis 1), tmp -> out (axis 0); "in" is dead after the first pass
     if (in == out) {

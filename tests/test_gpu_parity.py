@@ -451,6 +451,14 @@ def test_resolution_model(cuda_device, scanner, events):
     xi = dev(x, cuda_device).clone()
     jp.jp_gauss3d(xi, vox, sig, out=xi)
     assert torch.equal(xi, got)
+    # fused two-kernel path (n2 a multiple of 4): several row tiles with a ragged last one, also in place
+    x4 = rng.random((19, 70, 44)).astype(np.float32)
+    ref4 = oracle.gauss3d(x4, vox, sig)
+    got4 = jp.jp_gauss3d(dev(x4, cuda_device), vox, sig)
+    assert np.abs(got4.cpu().numpy() - ref4).max() <= 2e-6 * np.abs(ref4).max()
+    x4i = dev(x4, cuda_device).clone()
+    jp.jp_gauss3d(x4i, vox, sig, out=x4i)
+    assert torch.equal(x4i, got4)
     # OSEM with the model: 5 subsets x 1 iteration on the scanner geometry
     xs, xe, tb = events
     tofp = inputs.TofParams()
