@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- benchmark of the B200-native Joseph projector.
 
-    python bench.py --gpus N --steps K --warmup W [--config {1,2,3,4}] [--impl reference]
+    python bench.py --gpus N --steps K --warmup W [--config {0,1,2,3,4,5}] [--check] [--impl reference]
 
 A "step" is one pass of the hot path over one batch of synthetic input.  The default workload is
 BASELINE.json configs[1] (the configuration the headline LORs/s is quoted on): the non-TOF forward
@@ -11,7 +11,10 @@ of a U[0,1) sinogram (image zero-fill included).  `value` = LORs per second thro
 host-buffer C-ABI calls (jp_fwd_host / jp_back_host) with host<->device copies inside the timed region.
 The default run also times configs[2], [3] and [4] briefly and reports them under "other_configs"
 (BASELINE.json metric: LORs/s fwd, back and TOF-LM events/s, each with its roofline fraction);
-`--config C` makes configs[C] the timed workload of the line instead (used for the ncu captures in profiles/).
+`--config C` makes configs[C] the timed workload of the line instead (used for the ncu captures in profiles/);
+`--check` adds `parity` to the line: the float64 oracle run on the FULL config (outside the timed region; configs[4]:
+40 M events x 20 subsets x 3 iterations, about ten minutes on 16 cores) against the CUDA results of the same inputs,
+with the oracle's wall time per direction (`oracle_full`).  configs[0] (50,000 LORs, 4e5 plane-steps) is launch-bound.
 
 N > 1 (torchrun): LORs are independent units; every rank projects its own full frame (weak
 scaling), no data-path collective; timing is the max over ranks.  `--impl reference` times the float64 CPU
@@ -51,6 +54,12 @@ TRAFFIC = {(1, "fwd"): 3.955821e9 + 1.071657e9, (1, "back"): 4.106105e9 + 0.5885
            (3, "fwd"): 1.280978e9 + 0.813510e9, (3, "back"): 2.396714e9 + 0.162799e9}
 
 SPEC = {
+    0: dict(metric="LORs/s (non-TOF fwd+back pair, small case)", unit="LORs/s",
+            workload="configs[0]: non-TOF fwd+back, 50000 random chords of a cylinder (r 150 mm, |z| < 40 mm), image "
+                     "32x32x16 @ 4 mm U[0,1); LAUNCH-BOUND (4.06e5 plane-steps: microseconds of work per call), a "
+                     "roofline fraction is not meaningful for it",
+            l2="inputs (1.4 MB) fit in L2: a 256 MB buffer is overwritten between timed steps (L2 flush, outside the "
+               "per-direction events)"),
     1: dict(metric="LORs/s (non-TOF sinogram fwd+back pair)", unit="LORs/s",
             workload="configs[1]: non-TOF sinogram fwd+back, 151584768 LORs (257 radial x 256 views x 48x48 ring "
                      "pairs), image 200x200x96 @ 2 mm (cylinder + 10 hot spheres)",
@@ -139,7 +148,15 @@ def time_oracle(config: int, steps: int, warmup: int):
     import oracle
     oracle.build()
     ph = inputs.phantom().astype(np.float64)
-    if config == 1:
+    if config == 0:
+        c0 = inputs.config0()
+        g0 = c0["geom"]
+        xs, xe, n = c0["xstart"], c0["xend"], c0["xstart"].shape[1]
+        desc = "the whole of configs[0]: %d LORs (fwd + back, float64, OpenMP)" % n
+        i0, y0 = c0["img"].astype(np.float64), c0["y"].astype(np.float64)
+        f = lambda: oracle.fwd(xs, xe, i0, g0.origin, g0.voxsize)
+        b = lambda: oracle.back(xs, xe, y0, g0.n, g0.origin, g0.voxsize)
+    elif config == 1:
         # 17 views (incl. a 45 degree tie view) x all 257 radial x every 2nd ring pair
         views = sorted(set(range(5, 256, 16)) | {64})
         xs, xe = inputs.sinogram_lors(views=views)
@@ -202,7 +219,8 @@ def time_oracle(config: int, steps: int, warmup: int):
 
 def cpu_baseline_dict(config: int, r: dict):
     t = r["fwd_s"] + r["back_s"]
-    d = {"value": r["n"] / t, "unit": SPEC[config]["unit"], "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+    d = {"value": r["n"] / t, "unit": SPEC[config]["unit"], "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+         "sample_kind": "bounded sample of the workload, one run (the full config is timed under --check: parity.oracle_full)"}
     if config < 4:
         d["fwd_per_s"] = r["n"] / r["fwd_s"]
         d["back_per_s"] = r["n"] / r["back_s"]
@@ -242,7 +260,23 @@ class Workload:
         self.bimg = torch.zeros(G.n, dtype=torch.float32, device=dev)
         self.plan = None
         self.plan_s = None
-        if c == 5:
+        self.g = G
+        self.flush = None
+        if c == 0:
+            c0 = inputs.config0()
+            self.g = c0["geom"]
+            self.xs, self.xe = torch.from_numpy(c0["xstart"]).to(dev), torch.from_numpy(c0["xend"]).to(dev)
+            self.img = torch.from_numpy(c0["img"]).to(dev)
+            self.y = torch.from_numpy(c0["y"]).to(dev)
+            self.n = self.xs.shape[1]
+            self.p = torch.empty(self.n, dtype=torch.float32, device=dev)
+            self.bimg = torch.zeros(self.g.n, dtype=torch.float32, device=dev)
+            self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, self.g.n, self.g.origin, self.g.voxsize)
+            self.kinds = ("fwd", "back")
+            self.launches = 2
+            self.hbm_bytes = self.n * 28 + int(np.prod(self.g.n)) * 4
+            self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+        elif c == 5:
             nsub = 16
             order = [m + nsub * k for m in range(nsub) for k in range(inputs.N_VIEWS // nsub)]   # subset-major views
             self.xs, self.xe = inputs.sinogram_lors(views=order, device=dev)
@@ -303,9 +337,13 @@ class Workload:
 
     def step(self, ev=None):
         jp, c, s = self.jp, self.c, self.stream
+        if self.flush is not None:
+            self.flush.zero_()
         if ev:
             ev[0].record(s)
-        if c == 1:
+        if c == 0:
+            jp.jp_fwd(self.xs, self.xe, self.img, self.g.origin, self.g.voxsize, out=self.p)
+        elif c == 1:
             jp.jp_fwd(self.xs, self.xe, self.img, G.origin, G.voxsize, out=self.p)
         elif c == 2:
             jp.jp_fwd_tof_sino(self.xs, self.xe, self.img, G.origin, G.voxsize, self.tof, out=self.p)
@@ -320,7 +358,9 @@ class Workload:
             ev[1].record(s)
         if c < 4:
             self.bimg.zero_()
-        if c == 1:
+        if c == 0:
+            jp.jp_back(self.xs, self.xe, self.y, self.g.n, self.g.origin, self.g.voxsize, img=self.bimg)
+        elif c == 1:
             jp.jp_back(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
         elif c == 2:
             jp.jp_back_tof_sino(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, self.tof, img=self.bimg)
@@ -411,12 +451,13 @@ class Workload:
     def e2e_setup(self):
         jp, c = self.jp, self.c
         pin = lambda t: t.cpu().pin_memory()
-        if c == 1:
+        if c in (0, 1):
+            nvox = int(np.prod(self.g.n))
             self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
                           p=torch.empty(self.n, dtype=torch.float32).pin_memory(),
-                          b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
+                          b=torch.zeros(self.g.n, dtype=torch.float32).pin_memory())
             self.e2e_api = "jp_fwd_host + jp_back_host (pinned host tensors)"
-            self.h2d, self.d2h = 2 * 24 * self.n + 4 * self.n + 2 * 4 * NVOX, 4 * self.n + 4 * NVOX
+            self.h2d, self.d2h = 2 * 24 * self.n + 4 * self.n + 2 * 4 * nvox, 4 * self.n + 4 * nvox
         elif c == 2:
             self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
                           p=torch.empty_like(self.p, device="cpu").pin_memory(),
@@ -443,10 +484,10 @@ class Workload:
 
     def e2e_step(self):
         jp, c, h = self.jp, self.c, self.h
-        if c == 1:
-            jp.jp_fwd_host(h["xs"], h["xe"], h["img"], G.origin, G.voxsize, out=h["p"])
+        if c in (0, 1):
+            jp.jp_fwd_host(h["xs"], h["xe"], h["img"], self.g.origin, self.g.voxsize, out=h["p"])
             h["b"].zero_()
-            jp.jp_back_host(h["xs"], h["xe"], h["y"], h["b"], G.origin, G.voxsize)
+            jp.jp_back_host(h["xs"], h["xe"], h["y"], h["b"], self.g.origin, self.g.voxsize)
             return
         self.xs.copy_(h["xs"], non_blocking=True)
         self.xe.copy_(h["xe"], non_blocking=True)
@@ -476,6 +517,78 @@ class Workload:
         torch.cuda.synchronize()
 
 
+# ---- --check: the float64 oracle on the FULL config against the CUDA results (outside every timed region) -----------
+def check_parity(w: Workload):
+    """parity of the workload's CUDA results against the oracle run on the whole config on the host cores:
+    forward rel-L2 and max-abs / max|oracle| over ALL outputs, back projection max-abs / max|oracle| over ALL voxels
+    with the DENSE input, the GPU adjoint gap, and the oracle's wall time per direction (`oracle_full`)"""
+    import oracle
+    oracle.build()
+    jp, c, g = w.jp, w.c, w.g
+    tol = {"fwd_rel_l2": 1e-5, "max_abs_rel": 1e-4, "adjoint_gap": 1e-4, "osem_rel_l2": 1e-4, "osem_max_abs_rel": 1e-3}
+    out = {"oracle_cores": oracle.num_threads(), "tolerances": tol}
+    f64 = lambda t: t.detach().cpu().numpy().astype(np.float64)
+
+    def cmp_fwd(got, ref):
+        d = got - ref
+        return float(np.linalg.norm(d) / np.linalg.norm(ref)), float(np.abs(d).max() / np.abs(ref).max())
+
+    if c in (0, 1, 2, 3):
+        w.step()
+        torch.cuda.synchronize()
+        xs, xe = w.xs.cpu().numpy(), w.xe.cpu().numpy()
+        img64 = f64(w.img)
+        t0 = time.perf_counter()
+        if c in (0, 1):
+            ref = oracle.fwd(xs, xe, img64, g.origin, g.voxsize)
+        elif c == 2:
+            ref = oracle.fwd_tof_sino(xs, xe, img64, g.origin, g.voxsize, *TOF_ARGS)
+        else:
+            tb = w.tb.cpu().numpy()
+            ref = oracle.fwd_tof_lm(xs, xe, tb, img64, g.origin, g.voxsize, *TOF_ARGS[:3])
+        t1 = time.perf_counter()
+        rel, mx = cmp_fwd(f64(w.p).reshape(ref.shape), ref)
+        del ref
+        y64 = f64(w.y)
+        t2 = time.perf_counter()
+        if c in (0, 1):
+            bref = oracle.back(xs, xe, y64, g.n, g.origin, g.voxsize)
+        elif c == 2:
+            bref = oracle.back_tof_sino(xs, xe, y64, g.n, g.origin, g.voxsize, *TOF_ARGS)
+        else:
+            bref = oracle.back_tof_lm(xs, xe, tb, y64, g.n, g.origin, g.voxsize, *TOF_ARGS[:3])
+        t3 = time.perf_counter()
+        bmx = float(np.abs(f64(w.bimg) - bref).max() / np.abs(bref).max())
+        a = float((w.p.double().reshape(-1) * w.y.double().reshape(-1)).sum())
+        b = float((w.img.double() * w.bimg.double()).sum())
+        out.update({"fwd_rel_l2": rel, "fwd_max_abs_rel": mx, "back_max_abs_rel": bmx, "adjoint_gap": abs(a - b) / abs(a),
+                    "units_checked": int(w.n), "back_input": "dense",
+                    "oracle_full": {"fwd_s": t1 - t0, "back_s": t3 - t2, "units": int(w.n),
+                                    "fwd_per_s": w.n / (t1 - t0), "back_per_s": w.n / (t3 - t2)}})
+        out["pass"] = bool(rel <= tol["fwd_rel_l2"] and mx <= tol["max_abs_rel"] and bmx <= tol["max_abs_rel"]
+                           and out["adjoint_gap"] <= tol["adjoint_gap"])
+    elif c == 4:
+        n_iter = 3
+        x = torch.ones(G.n, dtype=torch.float32, device=w.dev)
+        jp.jp_lm_osem_planned(w.plan, w.sens, x, n_iter=n_iter)
+        torch.cuda.synchronize()
+        xs, xe, tb = w.xs.cpu().numpy(), w.xe.cpu().numpy(), w.tb.cpu().numpy()
+        t0 = time.perf_counter()
+        ref = oracle.lm_osem(xs, xe, tb, f64(w.sens), np.ones(G.n, dtype=np.float32), G.origin, G.voxsize,
+                             *TOF_ARGS[:3], n_subsets=20, n_iter=n_iter)
+        t1 = time.perf_counter()
+        got = f64(x)
+        rel = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+        mx = float(np.abs(got - ref).max() / np.abs(ref).max())
+        out.update({"osem_rel_l2": rel, "osem_max_abs_rel": mx, "events": int(w.n), "n_subsets": 20, "n_iter": n_iter,
+                    "image_max": float(ref.max()), "image_sum": float(ref.sum()), "finite": bool(np.isfinite(got).all()),
+                    "oracle_full": {"s_per_iteration": (t1 - t0) / n_iter, "events": int(w.n)}})
+        out["pass"] = bool(rel <= tol["osem_rel_l2"] and mx <= tol["osem_max_abs_rel"] and out["finite"])
+    else:
+        out["skipped"] = "the 40 GB sinogram OSEM workload is checked per subset in tests/test_gpu_fullsize.py"
+    return out
+
+
 def measure(w: Workload, steps: int, warmup: int, barrier, sampler=None):
     """warm-up, then `steps` timed steps between CUDA events on the launching stream"""
     for _ in range(warmup):
@@ -492,9 +605,18 @@ def measure(w: Workload, steps: int, warmup: int, barrier, sampler=None):
     barrier()
     clocks = sampler.stop() if sampler else None
     total_ms = e_beg.elapsed_time(e_end)
-    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-    back_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))   # includes the image zero-fill
-    return total_ms, fwd_ms, back_ms, clocks
+    f = [e[0].elapsed_time(e[1]) for e in evs]
+    b = [e[1].elapsed_time(e[2]) for e in evs]                         # includes the image zero-fill
+    if w.flush is not None:   # the L2 flush between steps is not part of a step
+        total_ms = float(np.sum(f) + np.sum(b))
+    w.step_ms = {"fwd": f, "back": b}
+    return total_ms, float(np.mean(f)), float(np.mean(b)), clocks
+
+
+def spread(ms):
+    """median / min / max of the per-step CUDA-event times (median and min of the repetitions)"""
+    a = np.asarray(ms, dtype=np.float64)
+    return {"median_ms": float(np.median(a)), "min_ms": float(a.min()), "max_ms": float(a.max()), "n": int(a.size)}
 
 
 def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
@@ -502,7 +624,8 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
     kf, kb = w.kinds
-    names = {1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
+    names = {0: ("k_fwd_tile (per-LOR path: random chords are not tracks)", "k_back_tile (per-LOR path)"),
+             1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
              3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_osem_tof_lm_quad (forward + ratio + back per event)", ""),
              5: ("k_tof_sino_osem<6> (forward + ratio + back per LOR block)", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
@@ -583,7 +706,7 @@ def run_ours(args):
         w.e2e_step()
         barrier()
         t0 = time.perf_counter()
-        ne2e = max(1, min(args.steps, 3))
+        ne2e = max(1, min(args.steps, 10))
         for _ in range(ne2e):
             w.e2e_step()
         barrier()
@@ -611,8 +734,13 @@ def run_ours(args):
         "gpu_launches": w.launches * args.steps,
         "clocks": clocks,
         "roofline": roofline_dict(w, fwd_ms, back_ms),
+        "timing": ({"fwd": spread(w.step_ms["fwd"]), "back": spread(w.step_ms["back"])} if c < 4 else
+                   {"iteration": spread(w.step_ms["fwd"])}),
         "checksum": checksum,
     }
+    if c == 0:
+        line["roofline"]["note"] = ("launch-bound: 4.06e5 plane-steps are microseconds of work per call; the fraction "
+                                    "is reported as SURVEY.md 8(d) asks, it says nothing about the kernels")
     if w.plan_s is not None:
         line["config"]["plan_s"] = w.plan_s
     if world == 1:
@@ -632,6 +760,8 @@ def run_ours(args):
                        "d2h_bytes_per_step": w.d2h, "ms_per_step": e2e_s * 1e3, "api": w.e2e_api}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline_dict(c, time_oracle(c, 1, 0))
+    if args.check and world == 1:
+        line["parity"] = check_parity(w)
     # ---- the other configs, briefly (single GPU, default workload only) -----------------------------------
     if world == 1 and c == 1 and not args.no_other:
         del w
@@ -672,7 +802,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5])
+    ap.add_argument("--check", action="store_true",
+                    help="run the float64 oracle on the FULL config (outside the timed region) and add `parity` to the line")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the brief configs[2..4] runs of the default line")

@@ -218,6 +218,34 @@ int jp_back(const jp_lors *lors, const float *y, const jp_geom *geom, float *img
     return JP_OK;
 }
 
+// bodies of the unplanned TOF sinogram calls (also the fallback of the planned ones)
+static int sino_fwd_impl(const jp::Lors &l, int64_t n, const float *img, const jp::Geom &g, const jp::Tof &t, float *p,
+                         cudaStream_t st)
+{
+    if (n == 0) return JP_OK;
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, img, 0, st, "jp_fwd_tof_sino (scratch)"));
+    cudaError_t e = jp::launch_tof_sino_win(false, l, n, c.pimg, nullptr, g, t, p, nullptr, st);
+    if (e == cudaErrorNotSupported) // TOF window wider than the compiled register windows: generic kernel
+        e = jp::launch_fwd_tof_sino(l, whole(n), c.pimg, g, t, c.lut, p, st);
+    JP_CUDA(e, "jp_fwd_tof_sino");
+    return JP_OK;
+}
+
+static int sino_back_impl(const jp::Lors &l, int64_t n, const float *y, const jp::Geom &g, const jp::Tof &t, float *img,
+                          cudaStream_t st)
+{
+    if (n == 0) return JP_OK;
+    TofCtx c;
+    JP_TRY(tof_ctx_init(c, t, g, nullptr, 1, st, "jp_back_tof_sino (scratch)"));
+    cudaError_t e = jp::launch_tof_sino_win(true, l, n, nullptr, c.pimg, g, t, nullptr, y, st);
+    if (e == cudaErrorNotSupported)
+        e = jp::launch_back_tof_sino(l, whole(n), y, g, t, c.lut, c.pimg, st);
+    JP_CUDA(e, "jp_back_tof_sino");
+    JP_CUDA(jp::padded_add_to(c.pimg, g, img, st), "jp_back_tof_sino (unpad)");
+    return JP_OK;
+}
+
 int jp_fwd_tof_sino(const jp_lors *lors, const float *img, const jp_geom *geom, const jp_tof *tof, float *p,
                     void *stream)
 {
@@ -229,15 +257,7 @@ int jp_fwd_tof_sino(const jp_lors *lors, const float *img, const jp_geom *geom, 
     JP_TRY(check_geom(geom, g));
     JP_TRY(check_tof(tof, true, t));
     if (!img || (lors->n > 0 && !p)) return fail(JP_ERR_POINTER, "img or p is NULL");
-    if (lors->n == 0) return JP_OK;
-    cudaStream_t st = (cudaStream_t)stream;
-    TofCtx c;
-    JP_TRY(tof_ctx_init(c, t, g, img, 0, st, "jp_fwd_tof_sino (scratch)"));
-    cudaError_t e = jp::launch_tof_sino_win(false, l, lors->n, c.pimg, nullptr, g, t, p, nullptr, st);
-    if (e == cudaErrorNotSupported) // TOF window wider than the compiled register windows: generic kernel
-        e = jp::launch_fwd_tof_sino(l, whole(lors->n), c.pimg, g, t, c.lut, p, st);
-    JP_CUDA(e, "jp_fwd_tof_sino");
-    return JP_OK;
+    return sino_fwd_impl(l, lors->n, img, g, t, p, (cudaStream_t)stream);
 }
 
 int jp_back_tof_sino(const jp_lors *lors, const float *y, const jp_geom *geom, const jp_tof *tof, float *img,
@@ -251,16 +271,7 @@ int jp_back_tof_sino(const jp_lors *lors, const float *y, const jp_geom *geom, c
     JP_TRY(check_geom(geom, g));
     JP_TRY(check_tof(tof, true, t));
     if (!img || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "img or y is NULL");
-    if (lors->n == 0) return JP_OK;
-    cudaStream_t st = (cudaStream_t)stream;
-    TofCtx c;
-    JP_TRY(tof_ctx_init(c, t, g, nullptr, 1, st, "jp_back_tof_sino (scratch)"));
-    cudaError_t e = jp::launch_tof_sino_win(true, l, lors->n, nullptr, c.pimg, g, t, nullptr, y, st);
-    if (e == cudaErrorNotSupported)
-        e = jp::launch_back_tof_sino(l, whole(lors->n), y, g, t, c.lut, c.pimg, st);
-    JP_CUDA(e, "jp_back_tof_sino");
-    JP_CUDA(jp::padded_add_to(c.pimg, g, img, st), "jp_back_tof_sino (unpad)");
-    return JP_OK;
+    return sino_back_impl(l, lors->n, y, g, t, img, (cudaStream_t)stream);
 }
 
 int jp_fwd_tof_lm(const jp_lors *lors, const int16_t *tofbin, const float *img, const jp_geom *geom,
@@ -336,7 +347,8 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
 
 // ---- listmode plan ------------------------------------------------------------------------------------------
 struct jp_plan {
-    jp::LmPlan *lm;
+    jp::LmPlan *lm = nullptr;     // listmode plan (jp_lm_plan_create)
+    jp::SinoPlan *sino = nullptr; // sinogram plan (jp_sino_plan_create)
 };
 
 int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
@@ -362,16 +374,20 @@ int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geo
     return JP_OK;
 }
 
-int jp_lm_plan_destroy(jp_plan *plan)
+int jp_plan_destroy(jp_plan *plan)
 {
     g_err[0] = 0;
     if (!plan) return JP_OK;
-    if (!plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
-    jp::lm_plan_destroy(plan->lm);
+    if (!plan->lm && !plan->sino) return fail(JP_ERR_PLAN, "invalid plan");
+    if (plan->lm) jp::lm_plan_destroy(plan->lm);
+    if (plan->sino) jp::sino_plan_destroy(plan->sino);
     plan->lm = nullptr;
+    plan->sino = nullptr;
     delete plan;
     return JP_OK;
 }
+
+int jp_lm_plan_destroy(jp_plan *plan) { return jp_plan_destroy(plan); }
 
 int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset)
 {

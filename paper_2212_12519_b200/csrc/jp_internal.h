@@ -127,6 +127,36 @@ void lm_plan_segment(const LmPlan *pl, int m, int a, int64_t *first, int64_t *co
 // persistent quad scratch of the plan (allocated on first use): which = 0,1: Q0,Q1; 2,3: B0,B1
 cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
 
+// sinogram plan (jp_sino_plan.cu): a LOR list analysed once.  REGULAR = K tracks of T LORs each (a track: identical
+// transaxial end points) that all share ONE axial pattern (zs, ze)[T] -- every sinogram of a ring scanner.  A regular
+// plan keeps only the K transaxial end-point quadruples, the pattern and a lane order (pattern indices sorted by
+// |ze - zs|: LORs of equal axial tilt have identical TOF weights on every plane); any other list is kept as a copy.
+struct SinoPlan;
+struct SinoPlanView {
+    int64_t n = 0;        // LORs
+    int64_t K = 0;        // tracks (regular)
+    int T = 0;            // LORs per track (regular)
+    int regular = 0;
+    double dz_max = 0.0;  // max |ze - zs| of the pattern
+    const float4 *trk = nullptr;  // [K] (xs, ys, xe, ye)
+    const float2 *zpat = nullptr; // [T] (zs, ze)
+    const int *order = nullptr;   // [T] pattern indices sorted by |ze - zs|, then sign, then zs
+    Lors lors{};                  // irregular: the plan's own SoA copy of the list
+};
+cudaError_t sino_plan_create(const Lors &l, int64_t n, cudaStream_t st, SinoPlan **out);
+void sino_plan_destroy(SinoPlan *pl);
+SinoPlanView sino_plan_view(const SinoPlan *pl);
+// regular plan: write the end points of LORs [first, first + count) as SoA arrays into coord6 (6 x count floats)
+cudaError_t sino_plan_expand(const SinoPlanView &pv, int64_t first, int64_t count, float *coord6, cudaStream_t st, Lors *out);
+
+// TOF sinogram kernels on the track tiles of a REGULAR plan (jp_tof_sino_tile.cu), tracks [k0, k0 + nk):
+//   mode 0  p[j][:] = A x            (p, y, epi arrays are indexed by the LOR index j of the plan's list)
+//   mode 1  img_w += A^T y           (or the broadcast values of epi: sensitivity images)
+//   mode 2  img_w += A^T (mult y_em / (mult A img_r + contam))   one OSEM subset pass (epi.y_em set)
+// img_r / img_w: UNPADDED images.  cudaErrorNotSupported: TOF window wider than compiled, or image too wide.
+cudaError_t launch_tof_sino_tile(int mode, const SinoPlanView &pv, int64_t k0, int64_t nk, const float *img_r, float *img_w,
+                                 const Geom &g, const Tof &t, float *p, const float *y, const SinoEpi *epi, cudaStream_t st);
+
 // resolution model (jp_gauss.cu): out = G in, three separable passes; tmp = nvox floats of scratch; in may alias out
 cudaError_t launch_gauss3d(const float *in, float *out, float *tmp, const Geom &g, float sigma_mm, float nsig,
                            cudaStream_t st);

@@ -80,11 +80,9 @@ __device__ __forceinline__ int principal_axis(double d0, double d1, double d2)
 // window every TOF weight the caller needs is exactly zero: the kernel is truncated).
 // Both clips are conservative (rounded outwards); they are optimisations, not decisions.
 template <bool WITH_TOF>
-__device__ __forceinline__ void ray_setup(const Lors &l, int64_t j, const Geom &g, float coff,
-                                          float tau_lo, float tau_hi, Ray &r)
+__device__ __forceinline__ void ray_setup_pts(const double (&s)[3], const double (&e)[3], const Geom &g, float coff,
+                                              float tau_lo, float tau_hi, Ray &r)
 {
-    const double s[3] = {(double)l.xs[j], (double)l.ys[j], (double)l.zs[j]};
-    const double e[3] = {(double)l.xe[j], (double)l.ye[j], (double)l.ze[j]};
     const double d[3] = {e[0] - s[0], e[1] - s[1], e[2] - s[2]}; // exact
     r.nk = 0;
     r.i0 = 0;
@@ -170,6 +168,15 @@ __device__ __forceinline__ void ray_setup(const Lors &l, int64_t j, const Geom &
         r.tau0 = (float)(tau0 + dtau * (double)ilo);
         r.dtau = (float)dtau;
     }
+}
+
+template <bool WITH_TOF>
+__device__ __forceinline__ void ray_setup(const Lors &l, int64_t j, const Geom &g, float coff,
+                                          float tau_lo, float tau_hi, Ray &r)
+{
+    const double s[3] = {(double)l.xs[j], (double)l.ys[j], (double)l.zs[j]};
+    const double e[3] = {(double)l.xe[j], (double)l.ye[j], (double)l.ze[j]};
+    ray_setup_pts<WITH_TOF>(s, e, g, coff, tau_lo, tau_hi, r);
 }
 
 // One crossed plane: integer cell and bilinear weights of the crossing point.

@@ -167,16 +167,18 @@ __device__ __forceinline__ ZRay z_setup(const Geom &g, const Track &t, float zs,
 // ICPT: store (intercept, slope) instead of (value, slope): pair(z) = (C[z] - (z - kc) D[z], D[z]), D[z] = C[z+1] - C[z],
 // so that the interpolant at axial coordinate u (cell z = floor(u)) is  pair.x + (u - kc) pair.y  with no
 // fractional part needed; kc (an integer, the middle of the axial range) keeps |u - kc| small.
-template <int P, bool ICPT = false, int RB = JP_RB>
+// PT: row pitch as a template parameter (rows addressed with immediates), or 0: the pitch is the run-time value `prt`
+template <int PT, bool ICPT = false, int RB = JP_RB, int NT = kThreads>
 __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, const float *__restrict__ img, const Track &t,
-                                           int c0, int rows, int n2, int vec_ok, float kc = 0.f)
+                                           int c0, int rows, int n2, int vec_ok, float kc = 0.f, int prt = 0)
 {
+    const int P = PT > 0 ? PT : prt;
     auto mk = [&](float v, float d, float zrel) { return ICPT ? make_float2(fmaf(-zrel, d, v), d) : make_float2(v, d); };
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
         if (vec_ok) {
             // one warp per row, lanes along z in groups of four voxels; kRB rows in flight per warp
             const int G = n2 >> 2;
-            constexpr int kRB = RB, kNW = kThreads / 32;
+            constexpr int kRB = RB, kNW = NT / 32;
             for (int g0 = 0; g0 < G; g0 += 32) {
                 const int gq = g0 + lane;
                 const bool act = gq < G;
@@ -222,7 +224,7 @@ __device__ __forceinline__ void build_rows(float2 *C2, const RowInfo *rinfo, con
             }
         } else {
             const int ld = n2 + 1; // columns z = -1 .. n2-1
-            for (int e = tid; e < rows * ld; e += kThreads) {
+            for (int e = tid; e < rows * ld; e += NT) {
                 const int r = e / ld, z = e - r * ld - 1;
                 const RowInfo ri = rinfo[c0 - t.I0 + r];
                 float v0 = 0.f, v1 = 0.f;

@@ -21,9 +21,11 @@
 // [256][n_tofbins] tile is staged through shared memory so that global reads / writes are coalesced, and
 // blocks whose LORs all miss the image skip the walk (forward: zero fill; back: y is not even read).
 // Images are the zero-padded copies of jp_pad.cu (PRay).
-#include "jp_internal.h"
+#include "jp_tof_win.cuh"
 
 namespace jp {
+
+using namespace tofwin;
 
 namespace {
 
@@ -32,54 +34,9 @@ constexpr int kSLd = kSBlock + 1;
 #ifndef JP_SINO_IO
 #define JP_SINO_IO 4 // tile elements per thread in flight
 #endif
-#ifndef JP_SINO_GK
-#define JP_SINO_GK 512
-#endif
-constexpr int kGK = JP_SINO_GK; // table rows per unit of phi
 #ifndef JP_SINO_MINB
 #define JP_SINO_MINB 4
 #endif
-
-__global__ void k_tof_gtab(float2 *tab, int nbw, double R, double W, double m, double isc)
-{
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= (kGK + 2) * nbw) return;
-    const int r = e / nbw, n = e - r * nbw;
-    auto E = [&](double y) { return erf(fmin(fmax(y, -m), m) * isc); };
-    auto G = [&](double x) { return 0.5 * (E((x + 0.5) * W) - E((x - 0.5) * W)); };
-    const double x0 = (double)n + (double)r / (double)kGK - R;
-    const double g0 = G(x0), g1 = G(x0 + 1.0 / (double)kGK);
-    tab[e] = make_float2((float)g0, (float)(g1 - g0));
-}
-
-struct GTab {
-    const float2 *tab; // device, (kGK + 2) rows of NBW (value, slope) pairs
-    float cbR;         // (n_tofbins - 1) / 2 - R
-    float inv_w;       // 1 / W
-};
-
-template <int OFF>
-__device__ __forceinline__ float4 lds_quad(uint32_t addr)
-{
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
-                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                 : "r"(addr), "n"(OFF)
-                 : "memory");
-    return v;
-}
-
-// weights of the NBW window bins from one table row: w[n] = T[n] + f D[n]
-template <int NBW, int N>
-__device__ __forceinline__ void load_weights(uint32_t row, float f, float (&w)[NBW])
-{
-    if constexpr (N < NBW) {
-        const float4 v = lds_quad<N * 8>(row);
-        w[N] = fmaf(f, v.y, v.x);
-        w[N + 1] = fmaf(f, v.w, v.z);
-        load_weights<NBW, N + 2>(row, f, w);
-    }
-}
 
 // the walk of one LOR; FWD: a[] accumulates value x weight per window bin, flushed into acc (shared, [bin][kSLd]);
 // BACK: yv[] holds the y values of the window bins (from ysm), the step's sum is scattered with atomic adds
@@ -411,18 +368,6 @@ __global__ void __launch_bounds__(kSBlock, JP_SINO_MINB)
     }
 }
 
-int window_bins(const Tof &t, double *R_out)
-{
-    const double m = (double)t.nsig * (double)t.sigma;
-    const double R = m / (double)t.width + 0.5;
-    *R_out = R;
-    const int nb = (int)ceil(2.0 * R);
-    const int sizes[] = {4, 6, 8, 12};
-    for (int s : sizes)
-        if (nb <= s) return s;
-    return 0;
-}
-
 size_t win_smem(int nbw, int nbins) { return (size_t)(kGK + 2) * nbw * sizeof(float2) + (size_t)nbins * kSLd * sizeof(float); }
 
 template <int NBW, bool BACK>
@@ -456,16 +401,10 @@ cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float
     const SinoEpi epi = epi_in ? *epi_in : SinoEpi{};
     if (n == 0) return cudaSuccess;
     double R;
-    const int nbw = window_bins(t, &R);
+    int nbw = window_bins(t, &R);
     if (!nbw || win_smem(nbw, t.nbins) > 72 * 1024) return cudaErrorNotSupported;
-    float2 *tab = nullptr;
-    const int ne = (kGK + 2) * nbw;
-    cudaError_t e = cudaMallocAsync((void **)&tab, sizeof(float2) * ne, st);
-    if (e != cudaSuccess) return e;
-    const double m = (double)t.nsig * (double)t.sigma;
-    k_tof_gtab<<<(ne + 255) / 256, 256, 0, st>>>(tab, nbw, R, (double)t.width, m, 1.0 / ((double)t.sigma * 1.4142135623730951));
-    e = cudaGetLastError();
-    GTab gt{tab, (float)(0.5 * (double)(t.nbins - 1) - R), 1.f / t.width};
+    GTab gt{};
+    cudaError_t e = gtab_create(t, st, &gt, &nbw);
     if (e == cudaSuccess) {
 #define JP_WIN(NB)                                                                                           \
     case NB:                                                                                                 \
@@ -481,7 +420,7 @@ cudaError_t launch_tof_sino_win(bool back, const Lors &l, int64_t n, const float
         }
 #undef JP_WIN
     }
-    cudaFreeAsync(tab, st);
+    gtab_destroy(&gt, st);
     return e;
 }
 
@@ -513,16 +452,10 @@ cudaError_t launch_tof_sino_osem(const Lors &l, int64_t n, const float *pimg_r, 
 {
     if (n == 0) return cudaSuccess;
     double R;
-    const int nbw = window_bins(t, &R);
+    int nbw = window_bins(t, &R);
     if (!nbw || win_smem(nbw, t.nbins) > 72 * 1024) return cudaErrorNotSupported;
-    float2 *tab = nullptr;
-    const int ne = (kGK + 2) * nbw;
-    cudaError_t e = cudaMallocAsync((void **)&tab, sizeof(float2) * ne, st);
-    if (e != cudaSuccess) return e;
-    const double m = (double)t.nsig * (double)t.sigma;
-    k_tof_gtab<<<(ne + 255) / 256, 256, 0, st>>>(tab, nbw, R, (double)t.width, m, 1.0 / ((double)t.sigma * 1.4142135623730951));
-    e = cudaGetLastError();
-    GTab gt{tab, (float)(0.5 * (double)(t.nbins - 1) - R), 1.f / t.width};
+    GTab gt{};
+    cudaError_t e = gtab_create(t, st, &gt, &nbw);
     if (e == cudaSuccess) {
         switch (nbw) {
         case 4: e = launch_osem_win<4>(l, n, pimg_r, pimg_w, g, t, gt, epi, st); break;
@@ -532,7 +465,7 @@ cudaError_t launch_tof_sino_osem(const Lors &l, int64_t n, const float *pimg_r, 
         default: e = cudaErrorNotSupported;
         }
     }
-    cudaFreeAsync(tab, st);
+    gtab_destroy(&gt, st);
     return e;
 }
 
