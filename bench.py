@@ -259,6 +259,7 @@ class Workload:
         self.img = torch.from_numpy(inputs.phantom(seed=inputs.BASE_SEED + 1 + 1000 * rank)).to(dev)
         self.bimg = torch.zeros(G.n, dtype=torch.float32, device=dev)
         self.plan = None
+        self.splan = None
         self.plan_s = None
         self.g = G
         self.flush = None
@@ -289,7 +290,11 @@ class Workload:
             self.mult = inputs.uniform_values(self.n, 0.2, 1.0, seed=inputs.BASE_SEED + 205 + rank, device=dev)
             self.ws = torch.empty(jp.jp_sino_osem_tof_workspace_bytes(self.off, self.n, self.tof), dtype=torch.uint8,
                                   device=dev)
-            self.sens = jp.jp_sino_sens_tof(self.xs, self.xe, self.off, self.mult, G.n, G.origin, G.voxsize, self.tof)
+            self.make_sino_plan()
+            if self.splan is not None:
+                self.sens = jp.jp_sino_sens_tof_planned(self.splan, self.off, self.mult, G.n, G.origin, G.voxsize, self.tof)
+            else:
+                self.sens = jp.jp_sino_sens_tof(self.xs, self.xe, self.off, self.mult, G.n, G.origin, G.voxsize, self.tof)
             self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
             self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
             self.kinds = ("sino", "sino")
@@ -304,6 +309,10 @@ class Workload:
             self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
             self.kinds = ("fwd", "back") if c == 1 else ("sino", "sino")
             self.launches = 6 if c == 1 else 8   # c1: (track probe, tile kernel, its per-track twin) x 2; c2: pad/unpad, 2 tables, kernel
+            if c == 2:
+                self.make_sino_plan()
+                if self.splan is not None:
+                    self.launches = 4            # per direction: weight table + track-tile kernel
             self.hbm_bytes = (self.n * 28 + NVOX * 4) if c == 1 else (self.n * (24 + 4 * TOFP.n_tofbins) + NVOX * 4)
         else:
             nev = int(os.environ.get("JP_BENCH_EVENTS", "40000000"))
@@ -328,6 +337,18 @@ class Workload:
                 self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
                 self.launches = 4 * 20 + 1   # per subset: quad build, fused projector per axis (x, y), update
 
+    def make_sino_plan(self):
+        """sinogram plan of the workload's LOR list (set-up, timed separately: `plan_s`); JP_BENCH_UNPLANNED=1 in the
+        environment times the unplanned per-LOR kernels instead (A/B measurements)"""
+        self.splan = None
+        if os.environ.get("JP_BENCH_UNPLANNED", "0") == "1":
+            return
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        self.splan = self.jp.SinoPlan(self.xs, self.xe)
+        torch.cuda.synchronize()
+        self.plan_s = time.perf_counter() - t0
+
     def setup_sens(self):
         """configs[4]: sens = non-TOF back projection of ones over all configs[1] LORs (one-time, untimed)"""
         sx, se = inputs.sinogram_lors(device=self.dev)
@@ -346,12 +367,19 @@ class Workload:
         elif c == 1:
             jp.jp_fwd(self.xs, self.xe, self.img, G.origin, G.voxsize, out=self.p)
         elif c == 2:
-            jp.jp_fwd_tof_sino(self.xs, self.xe, self.img, G.origin, G.voxsize, self.tof, out=self.p)
+            if self.splan is not None:
+                jp.jp_fwd_tof_sino_planned(self.splan, self.img, G.origin, G.voxsize, self.tof, out=self.p)
+            else:
+                jp.jp_fwd_tof_sino(self.xs, self.xe, self.img, G.origin, G.voxsize, self.tof, out=self.p)
         elif c == 3:
             jp.jp_fwd_tof_lm_planned(self.plan, self.img, out=self.p)
         elif c == 5:
-            jp.jp_sino_osem_tof(self.xs, self.xe, self.off, self.y, self.mult, self.contam, self.sens, self.x, G.origin,
-                                G.voxsize, self.tof, n_iter=1, workspace=self.ws)
+            if self.splan is not None:
+                jp.jp_sino_osem_tof_planned(self.splan, self.off, self.y, self.mult, self.contam, self.sens, self.x,
+                                            G.origin, G.voxsize, self.tof, n_iter=1, workspace=self.ws)
+            else:
+                jp.jp_sino_osem_tof(self.xs, self.xe, self.off, self.y, self.mult, self.contam, self.sens, self.x,
+                                    G.origin, G.voxsize, self.tof, n_iter=1, workspace=self.ws)
         else:
             jp.jp_lm_osem_planned(self.plan, self.sens, self.x, n_iter=1)
         if ev:
@@ -363,7 +391,10 @@ class Workload:
         elif c == 1:
             jp.jp_back(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
         elif c == 2:
-            jp.jp_back_tof_sino(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, self.tof, img=self.bimg)
+            if self.splan is not None:
+                jp.jp_back_tof_sino_planned(self.splan, self.y, G.n, G.origin, G.voxsize, self.tof, img=self.bimg)
+            else:
+                jp.jp_back_tof_sino(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, self.tof, img=self.bimg)
         elif c == 3:
             jp.jp_back_tof_lm_planned(self.plan, self.y, img=self.bimg)
         if ev:
@@ -462,7 +493,9 @@ class Workload:
             self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
                           p=torch.empty_like(self.p, device="cpu").pin_memory(),
                           b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
-            self.e2e_api = "pinned host -> device copies, jp_fwd_tof_sino + jp_back_tof_sino, device -> pinned host"
+            self.e2e_api = ("pinned host -> device copies, jp_sino_plan_create, jp_fwd_tof_sino_planned + "
+                            "jp_back_tof_sino_planned, device -> pinned host" if self.splan is not None else
+                            "pinned host -> device copies, jp_fwd_tof_sino + jp_back_tof_sino, device -> pinned host")
             self.h2d = 24 * self.n + 4 * self.y.numel() + 4 * NVOX
             self.d2h = 4 * self.p.numel() + 4 * NVOX
         elif c == 3:
@@ -494,7 +527,14 @@ class Workload:
         if c == 2:
             self.img.copy_(h["img"], non_blocking=True)
             self.y.copy_(h["y"], non_blocking=True)
+            old = self.splan
+            if old is not None:      # the plan is part of the step: it is made from the end points just uploaded
+                self.splan = self.jp.SinoPlan(self.xs, self.xe)
             self.step()
+            if old is not None:
+                torch.cuda.synchronize()
+                self.splan.destroy()
+                self.splan = old
         else:
             self.tb.copy_(h["tb"], non_blocking=True)
             plan = self.jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof, n_subsets=20)
@@ -624,10 +664,13 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak = N_SM * FP32_LANES_PER_SM * sm_mhz * 1e6          # FP32 lane-instructions / s
     kf, kb = w.kinds
+    planned = getattr(w, "splan", None) is not None
     names = {0: ("k_fwd_tile (per-LOR path: random chords are not tracks)", "k_back_tile (per-LOR path)"),
-             1: ("k_fwd_tile", "k_back_tile"), 2: ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
+             1: ("k_fwd_tile", "k_back_tile"),
+             2: ("k_tof_sino_tile<6,fwd>", "k_tof_sino_tile<6,back>") if planned else ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
              3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_osem_tof_lm_quad (forward + ratio + back per event)", ""),
-             5: ("k_tof_sino_osem<6> (forward + ratio + back per LOR block)", "")}[w.c]
+             5: ("k_tof_sino_tile<6,osem> (forward + ratio + back per track slice)" if planned else
+                 "k_tof_sino_osem<6> (forward + ratio + back per LOR block)", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
     if w.c in (4, 5):
         lane = 2 * LANE["lm" if w.c == 4 else "sino"]

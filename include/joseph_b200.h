@@ -216,6 +216,43 @@ int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_s
                      const float *mult, const float *contam, const float *sens, const jp_geom *geom, const jp_tof *tof,
                      float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- sinogram plan: the structure of a LOR list, found once (set-up; BASELINE.json north_star (b)) ------------------ */
+/* The projectors take plain lists of LOR end points.  The lists a ring scanner produces are regular: a
+ * sinogram is K TRACKS (runs of LORs with bit-identical transaxial end points xs, ys, xe, ye: the ring pairs of one
+ * (view, radial) bin) of T LORs each, and every track has the same axial pattern (zs, ze)[T].  jp_sino_plan_create
+ * detects exactly that from the data (T = length of the first run; n a multiple of T; every block of T LORs a track
+ * with the pattern of the first) and then keeps 16 bytes per TRACK, the pattern, and a lane order (LORs of a track
+ * sorted by |ze - zs|: equal tilt = equal LOR length = identical TOF weights on every plane).  Any other list is kept
+ * as a plain copy (24 bytes per LOR) and the planned calls run the kernels of the unplanned calls on it.
+ *   lors: device arrays, only read during jp_sino_plan_create (not kept).  The plan is independent of the image
+ *   geometry and of the TOF parameters.  jp_sino_plan_create SYNCHRONISES `stream` (it reads the track length and the
+ *   regularity flag back) and allocates the plan's device buffers with cudaMalloc; destroy with jp_plan_destroy.
+ * Planned calls compute what the unplanned calls compute (same arithmetic per LOR and plane; only the order of the
+ * floating-point sums of the back projection differs), take / return per-LOR arrays in CALLER (list) order, are
+ * asynchronous on `stream` and use only stream-ordered scratch.  A plan may be used from several streams at once
+ * (it is read-only after creation). */
+int jp_sino_plan_create(const jp_lors *lors, void *stream, jp_plan **plan);
+/* n_lors; n_tracks and track_length (both 0 for a list that is not regular); any output pointer may be NULL */
+int jp_sino_plan_info(const jp_plan *plan, int64_t *n_lors, int64_t *n_tracks, int32_t *track_length);
+/* destroys a plan made by jp_sino_plan_create or jp_lm_plan_create (jp_lm_plan_destroy is the same call) */
+int jp_plan_destroy(jp_plan *plan);
+/* jp_fwd_tof_sino / jp_back_tof_sino on the plan's LORs.  On a regular plan: track tiles --
+ * the image rows of a track are interpolated along q1 once per tile in shared memory, the adjoint is staged in
+ * shared memory (fixed point; a tile whose y holds Inf / NaN takes the per-LOR float path, so non-finite values
+ * propagate as in the unplanned call) and flushed with 128-bit atomic adds. */
+int jp_fwd_tof_sino_planned(const jp_plan *plan, const float *img, const jp_geom *geom, const jp_tof *tof, float *p,
+                            void *stream);
+int jp_back_tof_sino_planned(const jp_plan *plan, const float *y, const jp_geom *geom, const jp_tof *tof, float *img,
+                             void *stream);
+/* jp_sino_sens_tof / jp_sino_osem_tof on the plan's LORs (same arguments otherwise; workspace as for the unplanned
+ * calls, only touched when the plan is not regular, a subset boundary cuts a track, or the TOF kernel is too wide) */
+int jp_sino_sens_tof_planned(const jp_plan *plan, const int64_t *subset_offsets, int n_subsets, const float *mult,
+                             const jp_geom *geom, const jp_tof *tof, float *sens, void *workspace, size_t workspace_bytes,
+                             void *stream);
+int jp_sino_osem_tof_planned(const jp_plan *plan, const int64_t *subset_offsets, int n_subsets, const float *y,
+                             const float *mult, const float *contam, const float *sens, const jp_geom *geom,
+                             const jp_tof *tof, float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- hybrid mode: HOST pointers in and out ---------------------------------------- */
 /* Same semantics as jp_fwd / jp_back, but every pointer (inside lors_host too) is a HOST pointer.  The
  * LOR list is streamed through the current CUDA device in chunks on two internal streams (copies

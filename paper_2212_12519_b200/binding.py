@@ -81,6 +81,18 @@ EXPORTS = {
     "jp_sino_osem_tof": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                    C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p, C.c_int, C.c_void_p,
                                    C.c_size_t, C.c_void_p]),
+    "jp_sino_plan_create": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(C.c_void_p)]),
+    "jp_sino_plan_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32)]),
+    "jp_plan_destroy": (C.c_int, [C.c_void_p]),
+    "jp_fwd_tof_sino_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
+                                          C.c_void_p]),
+    "jp_back_tof_sino_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
+                                           C.c_void_p]),
+    "jp_sino_sens_tof_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.POINTER(jp_geom),
+                                           C.POINTER(jp_tof), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "jp_sino_osem_tof_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p, C.c_int,
+                                           C.c_void_p, C.c_size_t, C.c_void_p]),
     "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_fwd_tof_sino_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p]),
@@ -515,6 +527,95 @@ def jp_sino_osem_tof(xstart, xend, subset_offsets, y, mult, contam, sens, img, o
                                    _opt(contam, l.n * nb, "contam"), sens.data_ptr(), C.byref(g), C.byref(tof),
                                    img.data_ptr(), int(n_iter), workspace.data_ptr(),
                                    workspace.numel() * workspace.element_size(), _stream(stream)), "jp_sino_osem_tof")
+    return img
+
+
+# ---- sinogram plan (regular LOR lists: tracks with a common axial pattern) ---------------------------------------
+class SinoPlan:
+    """Owner of a jp_plan handle made by jp_sino_plan_create (the analysis runs in the library)."""
+
+    def __init__(self, xstart, xend, stream=None):
+        l, keep = make_lors(xstart, xend)
+        self.device = xstart.device
+        h = C.c_void_p()
+        _check(load().jp_sino_plan_create(C.byref(l), _stream(stream), C.byref(h)), "jp_sino_plan_create")
+        self.handle = h
+        n, k, t = C.c_int64(), C.c_int64(), C.c_int32()
+        _check(load().jp_sino_plan_info(h, C.byref(n), C.byref(k), C.byref(t)), "jp_sino_plan_info")
+        self.n, self.n_tracks, self.track_length = int(n.value), int(k.value), int(t.value)
+
+    @property
+    def regular(self) -> bool:
+        return self.track_length > 0
+
+    def destroy(self):
+        if self.handle is not None and self.handle.value:
+            _check(load().jp_plan_destroy(self.handle), "jp_plan_destroy")
+        self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def jp_fwd_tof_sino_planned(plan: SinoPlan, img, origin, voxsize, tof: jp_tof, out=None, stream=None) -> torch.Tensor:
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    if out is None:
+        out = torch.empty((plan.n, tof.n_tofbins), dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == plan.n * tof.n_tofbins and out.is_contiguous()
+    _check(load().jp_fwd_tof_sino_planned(plan.handle, img.data_ptr(), C.byref(g), C.byref(tof), out.data_ptr(),
+                                          _stream(stream)), "jp_fwd_tof_sino_planned")
+    return out
+
+
+def jp_back_tof_sino_planned(plan: SinoPlan, y, n, origin, voxsize, tof: jp_tof, img=None, stream=None) -> torch.Tensor:
+    _dev(y, torch.float32, "y")
+    assert y.numel() == plan.n * tof.n_tofbins and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(tuple(int(x) for x in n), dtype=torch.float32, device=y.device)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_tof_sino_planned(plan.handle, y.data_ptr(), C.byref(g), C.byref(tof), img.data_ptr(),
+                                           _stream(stream)), "jp_back_tof_sino_planned")
+    return img
+
+
+def jp_sino_sens_tof_planned(plan: SinoPlan, subset_offsets, mult, n, origin, voxsize, tof: jp_tof, out=None,
+                             workspace=None, stream=None) -> torch.Tensor:
+    off, ns = _offsets(subset_offsets)
+    shape = tuple(int(x) for x in n)
+    if out is None:
+        out = torch.empty((ns,) + shape, dtype=torch.float32, device=plan.device)
+    _dev(out, torch.float32, "sens")
+    assert out.shape == (ns,) + shape and out.is_contiguous()
+    g = make_geom(shape, origin, voxsize)
+    wp, wb = (workspace.data_ptr(), workspace.numel() * workspace.element_size()) if workspace is not None else (None, 0)
+    _check(load().jp_sino_sens_tof_planned(plan.handle, off, ns, _opt(mult, plan.n, "mult"), C.byref(g), C.byref(tof),
+                                           out.data_ptr(), wp, wb, _stream(stream)), "jp_sino_sens_tof_planned")
+    return out
+
+
+def jp_sino_osem_tof_planned(plan: SinoPlan, subset_offsets, y, mult, contam, sens, img, origin, voxsize, tof: jp_tof,
+                             n_iter: int, workspace=None, stream=None) -> torch.Tensor:
+    off, ns = _offsets(subset_offsets)
+    img = _img(img)
+    _dev(sens, torch.float32, "sens")
+    assert sens.shape == (ns,) + tuple(img.shape) and sens.is_contiguous()
+    g = make_geom(img.shape, origin, voxsize)
+    nb = int(tof.n_tofbins)
+    need = int(load().jp_sino_osem_tof_workspace_bytes(off, ns, int(plan.n), C.byref(tof)))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=img.device)
+    assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= need
+    _check(load().jp_sino_osem_tof_planned(plan.handle, off, ns, _opt(y, plan.n * nb, "y"), _opt(mult, plan.n, "mult"),
+                                           _opt(contam, plan.n * nb, "contam"), sens.data_ptr(), C.byref(g),
+                                           C.byref(tof), img.data_ptr(), int(n_iter), workspace.data_ptr(),
+                                           workspace.numel() * workspace.element_size(), _stream(stream)),
+           "jp_sino_osem_tof_planned")
     return img
 
 

@@ -727,21 +727,10 @@ size_t jp_sino_osem_tof_workspace_bytes(const int64_t *subset_offsets, int n_sub
     return (size_t)(mx * tof->n_tofbins + 64) * sizeof(float);
 }
 
-int jp_sino_sens_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *mult,
-                     const jp_geom *geom, const jp_tof *tof, float *sens, void *workspace, size_t workspace_bytes,
-                     void *stream)
+static int sino_sens_impl(const jp::Lors &l, const int64_t *subset_offsets, int n_subsets, const float *mult,
+                          const jp::Geom &g, const jp::Tof &t, float *sens, void *workspace, size_t workspace_bytes,
+                          cudaStream_t st)
 {
-    g_err[0] = 0;
-    jp::Lors l;
-    jp::Geom g;
-    jp::Tof t;
-    JP_TRY(check_lors(lors, l));
-    JP_TRY(check_geom(geom, g));
-    JP_TRY(check_tof(tof, true, t));
-    int64_t mx = 0;
-    JP_TRY(check_subsets(subset_offsets, n_subsets, lors->n, &mx));
-    if (!sens) return fail(JP_ERR_POINTER, "sens is NULL");
-    cudaStream_t st = (cudaStream_t)stream;
     const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
     JP_CUDA(cudaMemsetAsync(sens, 0, sizeof(float) * (size_t)nvox * n_subsets, st), "jp_sino_sens_tof (zero)");
     TofCtx c;
@@ -769,24 +758,10 @@ int jp_sino_sens_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_s
     return JP_OK;
 }
 
-int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *y,
-                     const float *mult, const float *contam, const float *sens, const jp_geom *geom, const jp_tof *tof,
-                     float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream)
+static int sino_osem_impl(const jp::Lors &l, const int64_t *subset_offsets, int n_subsets, const float *y,
+                          const float *mult, const float *contam, const float *sens, const jp::Geom &g, const jp::Tof &t,
+                          float *img, int n_iter, void *workspace, cudaStream_t st)
 {
-    g_err[0] = 0;
-    jp::Lors l;
-    jp::Geom g;
-    jp::Tof t;
-    JP_TRY(check_lors(lors, l));
-    JP_TRY(check_geom(geom, g));
-    JP_TRY(check_tof(tof, true, t));
-    int64_t mx = 0;
-    JP_TRY(check_subsets(subset_offsets, n_subsets, lors->n, &mx));
-    if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
-    if (!sens || !img || !workspace || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "NULL argument");
-    if (workspace_bytes < jp_sino_osem_tof_workspace_bytes(subset_offsets, n_subsets, lors->n, tof))
-        return fail(JP_ERR_SIZE, "workspace too small");
-    cudaStream_t st = (cudaStream_t)stream;
     const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
     const int nb = t.nbins;
     float *r = (float *)workspace;
@@ -817,6 +792,245 @@ int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_s
         }
     }
     return JP_OK;
+}
+
+int jp_sino_sens_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *mult,
+                     const jp_geom *geom, const jp_tof *tof, float *sens, void *workspace, size_t workspace_bytes,
+                     void *stream)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_lors(lors, l));
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    int64_t mx = 0;
+    JP_TRY(check_subsets(subset_offsets, n_subsets, lors->n, &mx));
+    if (!sens) return fail(JP_ERR_POINTER, "sens is NULL");
+    return sino_sens_impl(l, subset_offsets, n_subsets, mult, g, t, sens, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+int jp_sino_osem_tof(const jp_lors *lors, const int64_t *subset_offsets, int n_subsets, const float *y,
+                     const float *mult, const float *contam, const float *sens, const jp_geom *geom, const jp_tof *tof,
+                     float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_lors(lors, l));
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    int64_t mx = 0;
+    JP_TRY(check_subsets(subset_offsets, n_subsets, lors->n, &mx));
+    if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
+    if (!sens || !img || !workspace || (lors->n > 0 && !y)) return fail(JP_ERR_POINTER, "NULL argument");
+    if (workspace_bytes < jp_sino_osem_tof_workspace_bytes(subset_offsets, n_subsets, lors->n, tof))
+        return fail(JP_ERR_SIZE, "workspace too small");
+    return sino_osem_impl(l, subset_offsets, n_subsets, y, mult, contam, sens, g, t, img, n_iter, workspace,
+                          (cudaStream_t)stream);
+}
+
+// ---- sinogram plan and the planned TOF sinogram calls (jp_sino_plan.cu, jp_tof_sino_tile.cu) ---------------------------
+int jp_sino_plan_create(const jp_lors *lors, void *stream, jp_plan **plan)
+{
+    g_err[0] = 0;
+    jp::Lors l;
+    JP_TRY(check_lors(lors, l));
+    if (!plan) return fail(JP_ERR_POINTER, "plan is NULL");
+    *plan = nullptr;
+    jp::SinoPlan *sp = nullptr;
+    JP_CUDA(jp::sino_plan_create(l, lors->n, (cudaStream_t)stream, &sp), "jp_sino_plan_create");
+    jp_plan *pl = new jp_plan;
+    pl->sino = sp;
+    *plan = pl;
+    return JP_OK;
+}
+
+int jp_sino_plan_info(const jp_plan *plan, int64_t *n_lors, int64_t *n_tracks, int32_t *track_length)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    if (n_lors) *n_lors = v.n;
+    if (n_tracks) *n_tracks = v.regular ? v.K : 0;
+    if (track_length) *track_length = v.regular ? v.T : 0;
+    return JP_OK;
+}
+
+namespace {
+
+// the LOR list of a sinogram plan as arrays: the plan's own copy (irregular) or stream-ordered scratch filled from the
+// track table and the axial pattern (regular plans on a path that needs per-LOR arrays)
+struct PlanLors {
+    jp::Lors l{};
+    float *scratch = nullptr;
+    cudaStream_t st = nullptr;
+    ~PlanLors() { if (scratch) cudaFreeAsync(scratch, st); }
+    cudaError_t init(const jp::SinoPlanView &v, cudaStream_t s)
+    {
+        st = s;
+        if (!v.regular) {
+            l = v.lors;
+            return cudaSuccess;
+        }
+        cudaError_t e = cudaMallocAsync((void **)&scratch, sizeof(float) * 6 * (size_t)v.n, s);
+        if (e != cudaSuccess) return e;
+        return jp::sino_plan_expand(v, 0, v.n, scratch, s, &l);
+    }
+};
+
+// subsets of a regular plan must consist of whole tracks for the tile kernels
+bool subsets_on_tracks(const int64_t *off, int n_subsets, int T)
+{
+    for (int m = 0; m <= n_subsets; ++m)
+        if (off[m] % T) return false;
+    return true;
+}
+
+} // namespace
+
+int jp_fwd_tof_sino_planned(const jp_plan *plan, const float *img, const jp_geom *geom, const jp_tof *tof, float *p,
+                            void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    if (!img || (v.n > 0 && !p)) return fail(JP_ERR_POINTER, "img or p is NULL");
+    if (v.n == 0) return JP_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (v.regular) {
+        const cudaError_t e = jp::launch_tof_sino_tile(0, v, 0, v.K, img, nullptr, g, t, p, nullptr, nullptr, st);
+        if (e != cudaErrorNotSupported) {
+            JP_CUDA(e, "jp_fwd_tof_sino_planned");
+            return JP_OK;
+        }
+    }
+    PlanLors pl;
+    JP_CUDA(pl.init(v, st), "jp_fwd_tof_sino_planned (LOR list)");
+    return sino_fwd_impl(pl.l, v.n, img, g, t, p, st);
+}
+
+int jp_back_tof_sino_planned(const jp_plan *plan, const float *y, const jp_geom *geom, const jp_tof *tof, float *img,
+                             void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    if (!img || (v.n > 0 && !y)) return fail(JP_ERR_POINTER, "img or y is NULL");
+    if (v.n == 0) return JP_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (v.regular) {
+        const cudaError_t e = jp::launch_tof_sino_tile(1, v, 0, v.K, nullptr, img, g, t, nullptr, y, nullptr, st);
+        if (e != cudaErrorNotSupported) {
+            JP_CUDA(e, "jp_back_tof_sino_planned");
+            return JP_OK;
+        }
+    }
+    PlanLors pl;
+    JP_CUDA(pl.init(v, st), "jp_back_tof_sino_planned (LOR list)");
+    return sino_back_impl(pl.l, v.n, y, g, t, img, st);
+}
+
+int jp_sino_sens_tof_planned(const jp_plan *plan, const int64_t *subset_offsets, int n_subsets, const float *mult,
+                             const jp_geom *geom, const jp_tof *tof, float *sens, void *workspace, size_t workspace_bytes,
+                             void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    int64_t mx = 0;
+    JP_TRY(check_subsets(subset_offsets, n_subsets, v.n, &mx));
+    if (!sens) return fail(JP_ERR_POINTER, "sens is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    if (v.regular && subsets_on_tracks(subset_offsets, n_subsets, v.T)) {
+        JP_CUDA(cudaMemsetAsync(sens, 0, sizeof(float) * (size_t)nvox * n_subsets, st), "jp_sino_sens_tof_planned (zero)");
+        jp::SinoEpi epi;
+        epi.mult_bcast = mult;
+        epi.ones_bcast = mult ? 0 : 1;
+        cudaError_t e = cudaSuccess;
+        for (int m = 0; m < n_subsets && e == cudaSuccess; ++m) {
+            const int64_t k0 = subset_offsets[m] / v.T, nk = subset_offsets[m + 1] / v.T - k0;
+            e = jp::launch_tof_sino_tile(1, v, k0, nk, nullptr, sens + (size_t)m * nvox, g, t, nullptr, nullptr, &epi, st);
+        }
+        if (e != cudaErrorNotSupported) {
+            JP_CUDA(e, "jp_sino_sens_tof_planned");
+            return JP_OK;
+        }
+    }
+    PlanLors pl;
+    JP_CUDA(pl.init(v, st), "jp_sino_sens_tof_planned (LOR list)");
+    return sino_sens_impl(pl.l, subset_offsets, n_subsets, mult, g, t, sens, workspace, workspace_bytes, st);
+}
+
+int jp_sino_osem_tof_planned(const jp_plan *plan, const int64_t *subset_offsets, int n_subsets, const float *y,
+                             const float *mult, const float *contam, const float *sens, const jp_geom *geom,
+                             const jp_tof *tof, float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    jp::Geom g;
+    jp::Tof t;
+    JP_TRY(check_geom(geom, g));
+    JP_TRY(check_tof(tof, true, t));
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    int64_t mx = 0;
+    JP_TRY(check_subsets(subset_offsets, n_subsets, v.n, &mx));
+    if (n_iter < 0) return fail(JP_ERR_SIZE, "n_iter < 0");
+    if (!sens || !img || !workspace || (v.n > 0 && !y)) return fail(JP_ERR_POINTER, "NULL argument");
+    if (workspace_bytes < jp_sino_osem_tof_workspace_bytes(subset_offsets, n_subsets, v.n, tof))
+        return fail(JP_ERR_SIZE, "workspace too small");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nvox = (int64_t)g.n[0] * g.n[1] * g.n[2];
+    double R;
+    jp::Tof tt = t;
+    if (v.regular && subsets_on_tracks(subset_offsets, n_subsets, v.T) && jp::tof_window_bins(tt, &R) > 0) {
+        // per subset: ONE fused kernel on the unpadded images (forward, ratio, back), then the multiplicative update
+        struct Scratch {
+            float *p = nullptr;
+            cudaStream_t st = nullptr;
+            ~Scratch() { if (p) cudaFreeAsync(p, st); }
+        } b;
+        b.st = st;
+        JP_CUDA(cudaMallocAsync((void **)&b.p, sizeof(float) * (size_t)nvox, st), "jp_sino_osem_tof_planned (scratch)");
+        JP_CUDA(cudaMemsetAsync(b.p, 0, sizeof(float) * (size_t)nvox, st), "jp_sino_osem_tof_planned (scratch)");
+        jp::SinoEpi epi;
+        epi.y_em = y;
+        epi.mult = mult;
+        epi.contam = contam;
+        bool unsupported = false;
+        for (int it = 0; it < n_iter && !unsupported; ++it) {
+            for (int m = 0; m < n_subsets; ++m) {
+                const int64_t k0 = subset_offsets[m] / v.T, nk = subset_offsets[m + 1] / v.T - k0;
+                const cudaError_t e = jp::launch_tof_sino_tile(2, v, k0, nk, img, b.p, g, t, nullptr, nullptr, &epi, st);
+                if (e == cudaErrorNotSupported && it == 0 && m == 0) { // nothing enqueued yet: take the unplanned path
+                    unsupported = true;
+                    break;
+                }
+                JP_CUDA(e, "jp_sino_osem_tof_planned (subset pass)");
+                JP_CUDA(jp::launch_osem_update(img, b.p, sens + (size_t)m * nvox, 1.f, nvox, st),
+                        "jp_sino_osem_tof_planned (update)");
+            }
+        }
+        if (!unsupported) return JP_OK;
+    }
+    PlanLors pl;
+    JP_CUDA(pl.init(v, st), "jp_sino_osem_tof_planned (LOR list)");
+    return sino_osem_impl(pl.l, subset_offsets, n_subsets, y, mult, contam, sens, g, t, img, n_iter, workspace, st);
 }
 
 // ---- pieces of one OSEM subset update, for callers that exchange b between the two halves (multi-GPU) ----------

@@ -131,6 +131,8 @@ cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
 // transaxial end points) that all share ONE axial pattern (zs, ze)[T] -- every sinogram of a ring scanner.  A regular
 // plan keeps only the K transaxial end-point quadruples, the pattern and a lane order (pattern indices sorted by
 // |ze - zs|: LORs of equal axial tilt have identical TOF weights on every plane); any other list is kept as a copy.
+constexpr int kSinoSlice = 384;    // LORs of a track one CTA of the tile kernels takes (jp_tof_sino_tile.cu)
+constexpr int kSinoGroupsMax = 16; // groups of equal |ze - zs| per slice that get shared TOF weight rows
 struct SinoPlan;
 struct SinoPlanView {
     int64_t n = 0;        // LORs
@@ -140,7 +142,12 @@ struct SinoPlanView {
     double dz_max = 0.0;  // max |ze - zs| of the pattern
     const float4 *trk = nullptr;  // [K] (xs, ys, xe, ye)
     const float2 *zpat = nullptr; // [T] (zs, ze)
-    const int *order = nullptr;   // [T] pattern indices sorted by |ze - zs|, then sign, then zs
+    // lane order: the pattern indices arranged in slices of kSinoSlice entries; a slice is made of whole GROUPS (LORs
+    // of equal |ze - zs|, ordered by sign and zs) wherever they fit, at most kSinoGroupsMax of them
+    const int *order = nullptr;            // [T]
+    const unsigned char *slot_grp = nullptr; // [T] group of the entry, numbered from 0 inside its slice
+    const int *slice_ng = nullptr;         // [ceil(T / kSinoSlice)] groups of the slice; 0: too many, weights per lane
+    int slice_len = kSinoSlice;
     Lors lors{};                  // irregular: the plan's own SoA copy of the list
 };
 cudaError_t sino_plan_create(const Lors &l, int64_t n, cudaStream_t st, SinoPlan **out);
@@ -156,6 +163,9 @@ cudaError_t sino_plan_expand(const SinoPlanView &pv, int64_t first, int64_t coun
 // img_r / img_w: UNPADDED images.  cudaErrorNotSupported: TOF window wider than compiled, or image too wide.
 cudaError_t launch_tof_sino_tile(int mode, const SinoPlanView &pv, int64_t k0, int64_t nk, const float *img_r, float *img_w,
                                  const Geom &g, const Tof &t, float *p, const float *y, const SinoEpi *epi, cudaStream_t st);
+
+// window bins the TOF sinogram kernels are compiled for (0: TOF kernel too wide); R = n_sigmas sigma / W + 1/2
+int tof_window_bins(const Tof &t, double *R_out);
 
 // resolution model (jp_gauss.cu): out = G in, three separable passes; tmp = nvox floats of scratch; in may alias out
 cudaError_t launch_gauss3d(const float *in, float *out, float *tmp, const Geom &g, float sigma_mm, float nsig,

@@ -94,6 +94,8 @@ struct SinoPlan {
     float4 *trk = nullptr;
     float2 *zpat = nullptr;
     int *order = nullptr;
+    unsigned char *slot_grp = nullptr;
+    int *slice_ng = nullptr;
     float *coord = nullptr;
 };
 
@@ -103,6 +105,8 @@ void sino_plan_destroy(SinoPlan *pl)
     cudaFree(pl->trk);
     cudaFree(pl->zpat);
     cudaFree(pl->order);
+    cudaFree(pl->slot_grp);
+    cudaFree(pl->slice_ng);
     cudaFree(pl->coord);
     delete pl;
 }
@@ -154,22 +158,70 @@ cudaError_t sino_plan_create(const Lors &l, int64_t n, cudaStream_t st, SinoPlan
         std::vector<float2> zp((size_t)T);
         JP_SP_TRY(cudaMemcpyAsync(zp.data(), pl->zpat, sizeof(float2) * (size_t)T, cudaMemcpyDeviceToHost, st));
         JP_SP_TRY(cudaStreamSynchronize(st));
-        // lane order: |dz| (exact in double), then the sign of dz, then zs -- a performance hint only, any
-        // permutation of 0..T-1 gives the same results
+        // ---- lane order (a performance hint only: any permutation of 0..T-1 gives the same results).
+        // Groups = pattern entries of equal |dz| (exact in double), inside a group ordered by sign of dz, then zs.
+        // Slices of kSinoSlice entries are filled with whole groups, largest first, each into the slice with the most
+        // room (a group that fits nowhere is split), so that every slice holds few groups: the tile kernels build
+        // ONE row of TOF weights per (group, plane).
         std::vector<int> ord((size_t)T);
         double dzmax = 0.0;
+        auto dz_of = [&](int i) { return (double)zp[(size_t)i].y - (double)zp[(size_t)i].x; };
         for (int i = 0; i < T; ++i) {
             ord[(size_t)i] = i;
-            dzmax = std::max(dzmax, std::fabs((double)zp[(size_t)i].y - (double)zp[(size_t)i].x));
+            dzmax = std::max(dzmax, std::fabs(dz_of(i)));
         }
         std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) {
-            const double da = (double)zp[(size_t)a].y - (double)zp[(size_t)a].x, db = (double)zp[(size_t)b].y - (double)zp[(size_t)b].x;
+            const double da = dz_of(a), db = dz_of(b);
             if (std::fabs(da) != std::fabs(db)) return std::fabs(da) < std::fabs(db);
             if ((da < 0) != (db < 0)) return da < 0;
             return zp[(size_t)a].x < zp[(size_t)b].x;
         });
-        JP_SP_TRY(cudaMemcpyAsync(pl->order, ord.data(), sizeof(int) * (size_t)T, cudaMemcpyHostToDevice, st));
-        JP_SP_TRY(cudaStreamSynchronize(st)); // ord is a host temporary
+        struct Grp { int first, count; };
+        std::vector<Grp> grps;
+        for (int i = 0; i < T;) {
+            int j = i + 1;
+            while (j < T && std::fabs(dz_of(ord[(size_t)j])) == std::fabs(dz_of(ord[(size_t)i]))) ++j;
+            grps.push_back(Grp{i, j - i});
+            i = j;
+        }
+        std::stable_sort(grps.begin(), grps.end(), [](const Grp &a, const Grp &b) { return a.count > b.count; });
+        const int nsl = (T + kSinoSlice - 1) / kSinoSlice;
+        std::vector<int> room((size_t)nsl, kSinoSlice), ngr((size_t)nsl, 0);
+        room[(size_t)nsl - 1] = T - (nsl - 1) * kSinoSlice;
+        std::vector<std::vector<int>> members((size_t)nsl);      // pattern indices per slice
+        std::vector<std::vector<unsigned char>> mgrp((size_t)nsl);
+        for (const Grp &gr : grps) {
+            int first = gr.first, left = gr.count;
+            while (left > 0) {
+                int best = 0;
+                for (int s2 = 1; s2 < nsl; ++s2)
+                    if (room[(size_t)s2] > room[(size_t)best]) best = s2;
+                const int take = std::min(left, room[(size_t)best]);
+                const int gi = ngr[(size_t)best]++;
+                for (int k = 0; k < take; ++k) {
+                    members[(size_t)best].push_back(ord[(size_t)(first + k)]);
+                    mgrp[(size_t)best].push_back((unsigned char)std::min(gi, 255));
+                }
+                room[(size_t)best] -= take;
+                first += take;
+                left -= take;
+            }
+        }
+        std::vector<int> order_h((size_t)T), ng_h((size_t)nsl);
+        std::vector<unsigned char> grp_h((size_t)T);
+        for (int s2 = 0; s2 < nsl; ++s2) {
+            ng_h[(size_t)s2] = ngr[(size_t)s2] <= kSinoGroupsMax ? ngr[(size_t)s2] : 0;
+            for (size_t k = 0; k < members[(size_t)s2].size(); ++k) {
+                order_h[(size_t)s2 * kSinoSlice + k] = members[(size_t)s2][k];
+                grp_h[(size_t)s2 * kSinoSlice + k] = mgrp[(size_t)s2][k];
+            }
+        }
+        JP_SP_TRY(cudaMalloc((void **)&pl->slot_grp, (size_t)T));
+        JP_SP_TRY(cudaMalloc((void **)&pl->slice_ng, sizeof(int) * (size_t)nsl));
+        JP_SP_TRY(cudaMemcpyAsync(pl->order, order_h.data(), sizeof(int) * (size_t)T, cudaMemcpyHostToDevice, st));
+        JP_SP_TRY(cudaMemcpyAsync(pl->slot_grp, grp_h.data(), (size_t)T, cudaMemcpyHostToDevice, st));
+        JP_SP_TRY(cudaMemcpyAsync(pl->slice_ng, ng_h.data(), sizeof(int) * (size_t)nsl, cudaMemcpyHostToDevice, st));
+        JP_SP_TRY(cudaStreamSynchronize(st)); // the vectors are host temporaries
         pl->v.K = K;
         pl->v.T = T;
         pl->v.regular = 1;
@@ -177,6 +229,8 @@ cudaError_t sino_plan_create(const Lors &l, int64_t n, cudaStream_t st, SinoPlan
         pl->v.trk = pl->trk;
         pl->v.zpat = pl->zpat;
         pl->v.order = pl->order;
+        pl->v.slot_grp = pl->slot_grp;
+        pl->v.slice_ng = pl->slice_ng;
     } else {
         JP_SP_TRY(cudaMalloc((void **)&pl->coord, sizeof(float) * 6 * (size_t)n));
         const float *src[6] = {l.xs, l.ys, l.zs, l.xe, l.ye, l.ze};

@@ -35,7 +35,7 @@ using namespace tofwin;
 
 namespace {
 
-constexpr int kTS = 384;         // threads per CTA = LORs per slice
+constexpr int kTS = kSinoSlice;  // threads per CTA = LORs per slice
 constexpr int kTSLd = kTS + 1;
 constexpr int kNW = kTS / 32;
 
@@ -55,7 +55,8 @@ struct SRay {
     float a2, b2;   // u2(r) - kc = a2 + b2 (r - r_lo)
     float a2u;      // u2(r_lo), not shifted (the fixed-point rows of the adjoint)
     float cf;
-    float sR0, ds;  // bin coordinate minus R at r_lo; increment per plane (>= 0)
+    float q0, dq;   // kGK x (bin coordinate minus R) at r_lo; increment per plane (>= 0)
+    float qr0;      // the same at walk position r = 0 (identical for all LORs of the track with the same |ze - zs|)
 };
 
 __device__ __forceinline__ SRay sino_setup(const Geom &g, const TrackX &X, float zs, float ze, const Tof &t, float cbR,
@@ -118,9 +119,10 @@ __device__ __forceinline__ SRay sino_setup(const Geom &g, const TrackX &X, float
     z.r_lo = r_lo;
     z.r_hi = r_hi;
     z.a2u = (float)(A + kc + B * (double)(ifirst + dir * r_lo));
-    const double inv_w = 1.0 / (double)t.width;
-    z.sR0 = (float)((tau0 + dtau * (double)(ifirst + dir * r_lo)) * inv_w + (double)cbR);
-    z.ds = (float)(fabs(dtau) * inv_w);
+    const double sc = (double)tofwin::kGK / (double)t.width, off = (double)cbR * (double)tofwin::kGK;
+    z.dq = (float)(fabs(dtau) * sc);
+    z.qr0 = (float)((tau0 + dtau * (double)ifirst) * sc + off);
+    z.q0 = (float)((tau0 + dtau * (double)(ifirst + dir * r_lo)) * sc + off);
     return z;
 }
 
@@ -130,20 +132,26 @@ __device__ __forceinline__ void reds_add_s(uint32_t addr, int q)
     asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(q) : "memory");
 }
 
+// TOF bin coordinates are carried scaled by kGK (table rows): q = kGK (s - R).  kMagicG = 1.5 x 2^23 x kGK: adding it
+// rounds q to a multiple of kGK, so  cq = (q + kMagicG)_ru - kMagicG = kGK ceil(s - R)  and  cq - q  is the table row.
+constexpr float kMagicG = 12582912.f * (float)kGK;
+constexpr float kGKf = (float)kGK;
+constexpr int kGMax = kSinoGroupsMax; // groups (LORs of equal |ze - zs|) per slice that get shared weight rows
+
 // TOF window of one LOR: NBW bins starting at `base`, values in registers
 template <int NBW>
 struct Win {
     float a[NBW];
-    float basef;
+    float baseq; // kGK * base
     int base;
 };
 
-// slide the window up to bin `cur` (forward: retire bins into the stage; back: fetch the y of the bins entering)
+// slide the window up to scaled bin coordinate cq (forward: retire bins into the stage; back: fetch the bins entering)
 template <int NBW, bool BACK>
-__device__ __forceinline__ void win_slide(Win<NBW> &w, float cur, float *__restrict__ stage, int slot, int nbins, float cf)
+__device__ __forceinline__ void win_slide(Win<NBW> &w, float cq, float *__restrict__ stage, int slot, int nbins, float cf)
 {
 #pragma unroll 1
-    while (cur > w.basef) { // false for NaN
+    while (cq > w.baseq) { // false for NaN
         if (BACK) {
 #pragma unroll
             for (int n = 0; n + 1 < NBW; ++n) w.a[n] = w.a[n + 1];
@@ -154,16 +162,16 @@ __device__ __forceinline__ void win_slide(Win<NBW> &w, float cur, float *__restr
             for (int n = 0; n + 1 < NBW; ++n) w.a[n] = w.a[n + 1];
             w.a[NBW - 1] = 0.f;
         }
-        w.basef += 1.f;
+        w.baseq += kGKf;
         ++w.base;
     }
 }
 
 template <int NBW, bool BACK>
-__device__ __forceinline__ void win_init(Win<NBW> &w, float sR0, const float *__restrict__ stage, int slot, int nbins)
+__device__ __forceinline__ void win_init(Win<NBW> &w, float q0, const float *__restrict__ stage, int slot, int nbins)
 {
-    w.basef = __fadd_ru(sR0, kMagic) - kMagic; // ceil(s - R)
-    w.base = (int)w.basef;
+    w.baseq = __fadd_ru(q0, kMagicG) - kMagicG; // kGK ceil(s - R)
+    w.base = (int)(w.baseq * (1.f / kGKf));
 #pragma unroll
     for (int n = 0; n < NBW; ++n)
         w.a[n] = (BACK && (unsigned)(w.base + n) < (unsigned)nbins) ? stage[(w.base + n) * kTSLd + slot] : 0.f;
@@ -177,18 +185,36 @@ __device__ __forceinline__ void win_flush(const Win<NBW> &w, float *__restrict__
         if ((unsigned)(w.base + n) < (unsigned)nbins) stage[(w.base + n) * kTSLd + slot] = cf * w.a[n];
 }
 
-// weights of the window bins on a plane with bin coordinate (minus R) sR; slides the window first
-template <int NBW, bool BACK>
-__device__ __forceinline__ void win_weights(Win<NBW> &w, float sR, uint32_t tab_addr, float *__restrict__ stage, int slot,
-                                            int nbins, float cf, float (&wt)[NBW])
+// weights of the window bins on a plane with scaled bin coordinate q, from the table; returns cq = kGK ceil(s - R)
+template <int NBW>
+__device__ __forceinline__ float tab_weights(float q, uint32_t tab_addr, float (&wt)[NBW])
 {
-    const float cur = __fadd_ru(sR, kMagic) - kMagic;
-    win_slide<NBW, BACK>(w, cur, stage, slot, nbins, cf);
-    const float tk = (cur - sR) * (float)kGK;
+    const float cq = __fadd_ru(q, kMagicG) - kMagicG;
+    const float tk = cq - q;
     const float tt = __fadd_rd(tk, kMagic);
     const float f = tk - (tt - kMagic);
     const uint32_t row = tab_addr + __float_as_uint(tt) * (uint32_t)(NBW * 8);
     load_weights<NBW, 0>(row, f, wt);
+    return cq;
+}
+
+// ---- shared weight rows: one entry per (group, plane of the chunk) = the NBW weights and cq -------------------------
+template <int NBW>
+struct WEntry {
+    static constexpr int kFloats = ((NBW + 1 + 3) / 4) * 4;
+};
+
+template <int NBW, int N>
+__device__ __forceinline__ void load_wentry(uint32_t addr, float (&v)[WEntry<NBW>::kFloats])
+{
+    if constexpr (N < WEntry<NBW>::kFloats) {
+        const float4 x = lds_quad<N * 4>(addr);
+        v[N] = x.x;
+        v[N + 1] = x.y;
+        v[N + 2] = x.z;
+        v[N + 3] = x.w;
+        load_wentry<NBW, N + 4>(addr, v);
+    }
 }
 
 // per-LOR path (any principal axis, global gathers / atomics on the unpadded image): same table, same window
@@ -201,18 +227,19 @@ __device__ __forceinline__ void generic_walk(const double (&s)[3], const double 
     ray_setup_pts<true>(s, e, g, t.coff, -reach, reach, r);
     if (r.nk == 0) return;
     const int nbins = t.nbins;
-    const float ds = r.dtau * gt.inv_w;
-    const float sR0 = fmaf(r.tau0, gt.inv_w, gt.cbR);
+    const float dq = r.dtau * gt.inv_w * kGKf;
+    const float q0 = fmaf(r.tau0, gt.inv_w, gt.cbR) * kGKf;
     int k = 0, dk = 1;
-    if (ds < 0.f) {
+    if (dq < 0.f) {
         k = r.nk - 1;
         dk = -1;
     }
     Win<NBW> w;
-    win_init<NBW, BACK>(w, fmaf(ds, (float)k, sR0), stage, slot, nbins);
+    win_init<NBW, BACK>(w, fmaf(dq, (float)k, q0), stage, slot, nbins);
     for (int it = 0; it < r.nk; ++it, k += dk) {
         float wt[NBW];
-        win_weights<NBW, BACK>(w, fmaf(ds, (float)k, sR0), tab_addr, stage, slot, nbins, r.cf, wt);
+        const float cq = tab_weights<NBW>(fmaf(dq, (float)k, q0), tab_addr, wt);
+        win_slide<NBW, BACK>(w, cq, stage, slot, nbins, r.cf);
         const Cell cl = plane_cell(r, k);
         if (BACK) {
             float sm = 0.f;
@@ -232,6 +259,8 @@ struct TileArgs {
     const float4 *trk;
     const float2 *zpat;
     const int *order;
+    const unsigned char *slot_grp; // [T] group of every entry of the lane order, numbered from 0 inside its slice
+    const int *slice_ng;           // [slices] groups of the slice (0: more than kGMax -> per-lane weights)
     int T;
     double dz_max;
     int64_t k0, nk; // tracks
@@ -252,31 +281,39 @@ struct TileArgs {
 template <int NBW, int MODE>
 __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
 {
+    constexpr int WE = WEntry<NBW>::kFloats;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nbins = A.t.nbins;
     const int np = max(A.g.n[0], A.g.n[1]);
+    const int rows_cap = A.rows_cap;
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);                                         // [(kGK + 2)][NBW]
     float *stage = reinterpret_cast<float *>(smem_raw + (size_t)(kGK + 2) * NBW * sizeof(float2)); // [nbins][kTSLd]
     RowInfo *rinfo = reinterpret_cast<RowInfo *>(stage + (((size_t)nbins * kTSLd + 3) & ~(size_t)3)); // [np], walk order
     int *kidx = reinterpret_cast<int *>(rinfo + np);                                            // [kTS]
-    unsigned char *rows_raw = reinterpret_cast<unsigned char *>(kidx + kTS);                    // float2 / int [rows_cap][P]
+    float *Wt = reinterpret_cast<float *>(kidx + kTS);                                          // [kGMax][rows_cap][WE]
+    unsigned char *rows_raw = reinterpret_cast<unsigned char *>(Wt + (size_t)kGMax * rows_cap * WE); // float2 / int [rows_cap][P]
     float2 *C2 = reinterpret_cast<float2 *>(rows_raw);
     int *Ci = reinterpret_cast<int *>(rows_raw);
     __shared__ TrackX X;
     __shared__ float red[kNW];
+    __shared__ float2 grpq[kGMax]; // per group: scaled bin coordinate at walk position 0, increment per plane
     __shared__ int flag_nonfinite;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const Geom &g = A.g;
     const Tof &t = A.t;
-    const int P = A.P, rows_cap = A.rows_cap, n2 = g.n[2];
+    const int P = A.P, n2 = g.n[2];
     for (int i = tid; i < (kGK + 2) * NBW; i += kTS) tab[i] = __ldg(A.gt.tab + i);
     for (int i = tid; i < nbins * kTSLd; i += kTS) stage[i] = 0.f;
-    const uint32_t tab_addr = smem_addr(tab) - (uint32_t)kMagicI * (uint32_t)(NBW * 8);
+    uint32_t tab_addr = smem_addr(tab) - (uint32_t)kMagicI * (uint32_t)(NBW * 8);
     const float reach = 0.5f * (float)(nbins - 1) * t.width + 0.5f * t.width + t.nsig * t.sigma;
     const int kci = n2 >> 1;
-    const uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
-    const uint32_t ci_base = smem_addr(Ci) + kPad * 4u - ((uint32_t)kMagicI << 2);
+    uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
+    uint32_t ci_base = smem_addr(Ci) + kPad * 4u - ((uint32_t)kMagicI << 2);
+    uint32_t wt_base = smem_addr(Wt);
+    // keep the biased shared-memory addresses in registers: left to itself the compiler rematerialises them (an S2R
+    // and three integer adds) inside the plane loops
+    asm volatile("" : "+r"(tab_addr), "+r"(c2_base), "+r"(ci_base), "+r"(wt_base));
     const int T = A.T;
     const int nsl = (T + kTS - 1) / kTS;
     const int64_t items = A.nk * nsl;
@@ -324,6 +361,8 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
         // ---- this thread's LOR: slot tid of the slice = entry sl * kTS + tid of the lane order
         const int kk = (tid < nv) ? __ldg(A.order + sl * kTS + tid) : -1;
         kidx[tid] = kk;
+        const int NG = generic ? 0 : __ldg(A.slice_ng + sl); // 0: weights per lane
+        const int gid = (NG > 0 && kk >= 0) ? (int)__ldg(A.slot_grp + sl * kTS + tid) : 0;
         float zs = 0.f, ze = 0.f;
         if (kk >= 0) {
             const float2 zz = __ldg(A.zpat + kk);
@@ -333,9 +372,12 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
         SRay zr;
         zr.r_lo = 0;
         zr.r_hi = -1;
-        zr.a2 = zr.b2 = zr.a2u = zr.cf = zr.sR0 = zr.ds = 0.f;
+        zr.a2 = zr.b2 = zr.a2u = zr.cf = zr.q0 = zr.dq = zr.qr0 = 0.f;
         if (!generic) {
-            if (kk >= 0) zr = sino_setup(g, X, zs, ze, t, A.gt.cbR, reach, MODE == 1 ? 0.0 : (double)kci);
+            if (kk >= 0) {
+                zr = sino_setup(g, X, zs, ze, t, A.gt.cbR, reach, (double)kci);
+                if (NG > 0) grpq[gid] = make_float2(zr.qr0, zr.dq); // the same bits from every LOR of the group
+            }
             int lo = zr.r_hi >= zr.r_lo ? zr.r_lo : 0x7fffffff, hi = zr.r_hi >= zr.r_lo ? zr.r_hi : -1;
             for (int o = 16; o > 0; o >>= 1) {
                 lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
@@ -349,8 +391,26 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
             const int nr = tr.I1 - tr.I0;
             for (int r = tid; r <= nr; r += kTS) rinfo[r] = row_info(g, tr, X.dir > 0 ? tr.I0 + r : tr.I1 - r);
         }
-        __syncthreads(); // kidx, rinfo, X.rmin / rmax
+        __syncthreads(); // kidx, rinfo, grpq, X.rmin / rmax
         const double sp[3] = {(double)X.xs, (double)X.ys, (double)zs}, ep[3] = {(double)X.xe, (double)X.ye, (double)ze};
+        const bool live = zr.r_hi >= zr.r_lo;
+        // scaled bin coordinate of the first plane: with shared weight rows the SAME float32 expression that builds the
+        // rows, so that the window a lane opens and the window the row was made for cannot differ by a rounding
+        const float q_init = NG > 0 ? fmaf(grpq[gid].y, (float)zr.r_lo, grpq[gid].x) : zr.q0;
+
+        // the weight rows of chunk [r0, r0 + rows): thread e -> (group, plane)
+        auto build_wt = [&](int r0, int rows) {
+            if (tid < NG * rows) {
+                const int gq = tid / rows, rr = tid - gq * rows;
+                const float2 gp = grpq[gq];
+                float wt[NBW];
+                const float cq = tab_weights<NBW>(fmaf(gp.y, (float)(r0 + rr), gp.x), tab_addr, wt);
+                float *dst = Wt + (size_t)(gq * rows_cap + rr) * WE;
+#pragma unroll
+                for (int n = 0; n < NBW; ++n) dst[n] = wt[n];
+                dst[NBW] = cq;
+            }
+        };
 
         // ======== forward (MODE 0, 2): walk into the window registers, retire bins into the stage =======================
         if (MODE != 1) {
@@ -366,44 +426,72 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
                     }
                 }
                 Win<NBW> w;
-                win_init<NBW, false>(w, zr.sR0, stage, tid, nbins);
+                win_init<NBW, false>(w, q_init, stage, tid, nbins);
                 const int R0 = X.rmin, R1 = X.rmax;
                 for (int r0 = R0; r0 <= R1; r0 += rows_cap) {
                     const int rows = min(rows_cap, R1 - r0 + 1);
                     __syncthreads(); // the previous chunk's rows are no longer read
                     build_rows<0, true, 1, kTS>(C2, rinfo, A.img_r, X.t, X.t.I0 + r0, rows, n2, A.vec_r, (float)kci, P);
+                    build_wt(r0, rows);
                     __syncthreads();
                     const int rb = max(zr.r_lo, r0), re = min(zr.r_hi, r0 + rows - 1);
                     if (rb <= re) {
                         float fk = (float)(rb - zr.r_lo);
                         uint32_t row = c2_base + (uint32_t)((rb - r0) * P) * 8u;
-#pragma unroll 1
-                        for (int it = re - rb + 1; it > 0; --it) {
-                            const float u = fmaf(zr.b2, fk, zr.a2);
-                            const float tt = __fadd_rd(u, kMagic);
-                            const float2 v = lds_pair<0>(row + (__float_as_uint(tt) << 3));
-                            float wt[NBW];
-                            win_weights<NBW, false>(w, fmaf(zr.ds, fk, zr.sR0), tab_addr, stage, tid, nbins, zr.cf, wt);
-                            const float val = fmaf(u, v.y, v.x);
+                        if (NG > 0) {
+                            uint32_t wrow = wt_base + (uint32_t)((gid * rows_cap + (rb - r0)) * WE) * 4u;
+#pragma unroll 2
+                            for (int it = re - rb + 1; it > 0; --it) {
+                                const float u = fmaf(zr.b2, fk, zr.a2);
+                                const float tt = __fadd_rd(u, kMagic);
+                                const float2 v = lds_pair<0>(row + (__float_as_uint(tt) << 3));
+                                float wv[WE];
+                                load_wentry<NBW, 0>(wrow, wv);
+                                win_slide<NBW, false>(w, wv[NBW], stage, tid, nbins, zr.cf);
+                                const float val = fmaf(u, v.y, v.x);
 #pragma unroll
-                            for (int n = 0; n < NBW; ++n) w.a[n] = fmaf(val, wt[n], w.a[n]);
-                            fk += 1.f;
-                            row += (uint32_t)P * 8u;
+                                for (int n = 0; n < NBW; ++n) w.a[n] = fmaf(val, wv[n], w.a[n]);
+                                fk += 1.f;
+                                row += (uint32_t)P * 8u;
+                                wrow += WE * 4u;
+                            }
+                        } else {
+#pragma unroll 1
+                            for (int it = re - rb + 1; it > 0; --it) {
+                                const float u = fmaf(zr.b2, fk, zr.a2);
+                                const float tt = __fadd_rd(u, kMagic);
+                                const float2 v = lds_pair<0>(row + (__float_as_uint(tt) << 3));
+                                float wt[NBW];
+                                const float cq = tab_weights<NBW>(fmaf(zr.dq, fk, zr.q0), tab_addr, wt);
+                                win_slide<NBW, false>(w, cq, stage, tid, nbins, zr.cf);
+                                const float val = fmaf(u, v.y, v.x);
+#pragma unroll
+                                for (int n = 0; n < NBW; ++n) w.a[n] = fmaf(val, wt[n], w.a[n]);
+                                fk += 1.f;
+                                row += (uint32_t)P * 8u;
+                            }
                         }
                     }
                 }
-                if (zr.r_hi >= zr.r_lo) win_flush<NBW>(w, stage, tid, nbins, zr.cf);
+                if (live) win_flush<NBW>(w, stage, tid, nbins, zr.cf);
             }
             __syncthreads(); // the stage holds p[slot][:] of the slice
         }
 
         // ======== forward: write the LOR rows (and clear the stage) ==========================================================
         if (MODE == 0) {
+            float *st_lo = stage + lane * kTSLd, *st_hi = stage + (lane + 32) * kTSLd; // JP_MAX_TOFBINS = 64: two halves
+            const bool lo_ok = lane < nbins, hi_ok = lane + 32 < nbins;
+#pragma unroll 4
             for (int s0 = warp; s0 < nv; s0 += kNW) {
-                const int64_t j = j0 + kidx[s0];
-                for (int b = lane; b < nbins; b += 32) {
-                    A.p[j * nbins + b] = stage[b * kTSLd + s0];
-                    stage[b * kTSLd + s0] = 0.f;
+                float *out = A.p + (j0 + kidx[s0]) * nbins + lane;
+                if (lo_ok) {
+                    out[0] = st_lo[s0];
+                    st_lo[s0] = 0.f;
+                }
+                if (hi_ok) {
+                    out[32] = st_hi[s0];
+                    st_hi[s0] = 0.f;
                 }
             }
             continue;
@@ -443,14 +531,28 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
 
         // ======== OSEM (MODE 2): the ratio in place (reading S2) =========================================================
         if (MODE == 2) {
+            const bool lo_ok = lane < nbins, hi_ok = lane + 32 < nbins;
+#pragma unroll 2
             for (int s0 = warp; s0 < nv; s0 += kNW) {
                 const int64_t j = j0 + kidx[s0];
                 const float mv = A.epi.mult ? A.epi.mult[j] : 1.f;
-                for (int b = lane; b < nbins; b += 32) {
-                    const float yv = A.epi.y_em[j * nbins + b];
-                    const float cv = A.epi.contam ? A.epi.contam[j * nbins + b] : 0.f;
-                    const float yb = fmaf(mv, stage[b * kTSLd + s0], cv);
-                    stage[b * kTSLd + s0] = (yb > 1e-9f) ? mv * yv / yb : 0.f;
+                const int64_t e = j * nbins + lane;
+                float y0 = 0.f, y1 = 0.f, c0 = 0.f, c1 = 0.f;
+                if (lo_ok) y0 = A.epi.y_em[e];
+                if (hi_ok) y1 = A.epi.y_em[e + 32];
+                if (A.epi.contam) {
+                    if (lo_ok) c0 = A.epi.contam[e];
+                    if (hi_ok) c1 = A.epi.contam[e + 32];
+                }
+                if (lo_ok) {
+                    float *sp2 = stage + lane * kTSLd + s0;
+                    const float yb = fmaf(mv, *sp2, c0);
+                    *sp2 = (yb > 1e-9f) ? mv * y0 / yb : 0.f;
+                }
+                if (hi_ok) {
+                    float *sp2 = stage + (lane + 32) * kTSLd + s0;
+                    const float yb = fmaf(mv, *sp2, c1);
+                    *sp2 = (yb > 1e-9f) ? mv * y1 / yb : 0.f;
                 }
             }
             __syncthreads();
@@ -458,11 +560,11 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
 
         // ======== back walk (MODE 1, 2) ==================================================================================
         bool use_generic = generic;
-        float S = 0.f, invS = 0.f;
+        bool any_value = true;
         if (!generic) {
-            // fixed-point scale from X = max_j cf_j max_k |value[j][k]| (the TOF weights of a step sum to <= 1)
+            // Inf / NaN anywhere in the values of a LOR that crosses the image -> per-LOR float path for the slice
             float xm = 0.f;
-            if (zr.r_hi >= zr.r_lo) {
+            if (live) {
                 bool bad = false;
                 for (int b = 0; b < nbins; ++b) {
                     const float v = fabsf(stage[b * kTSLd + tid]);
@@ -470,7 +572,6 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
                     xm = fmaxf(xm, v);
                 }
                 if (bad) atomicExch(&flag_nonfinite, 1);
-                xm *= zr.cf;
             }
             for (int o = 16; o > 0; o >>= 1) xm = fmaxf(xm, __shfl_xor_sync(0xffffffffu, xm, o));
             if (lane == 0) red[warp] = xm;
@@ -483,47 +584,91 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
             xm = red[0];
 #pragma unroll
             for (int w2 = 1; w2 < kNW; ++w2) xm = fmaxf(xm, red[w2]);
-            if (flag_nonfinite || !(xm < 3.0e38f)) {
-                use_generic = true; // propagate Inf / NaN exactly as the per-LOR adjoint does
-            } else if (xm > 0.f) {
-                const float lim = 4194302.f; // |c S| <= 2^22 - 2 and kTS |c S| < 2^31
-                S = lim / xm;
-                invS = xm / lim;
-            }
+            use_generic = flag_nonfinite != 0; // propagate Inf / NaN exactly as the per-LOR adjoint does
+            any_value = xm > 0.f;
         }
         if (use_generic) {
             if (kk >= 0) generic_walk<NBW, true>(sp, ep, g, t, A.gt, tab_addr, stage, tid, reach, nullptr, A.img_w);
-        } else if (S > 0.f && X.rmax >= X.rmin) {
-            SRay zb = zr;
-            zb.a2 = zr.a2u; // the forward rows are shifted by kc, the fixed-point rows are not
+        } else if (any_value && X.rmax >= X.rmin) {
+            // Fixed-point staging with a scale per CHUNK of planes: S = lim / Xc, Xc = max over the slice's LORs of
+            // cf x max |value| over the TOF bins whose window is open on the chunk's planes (the weights of a step sum
+            // to <= 1, so |cf sum_k w_k value_k| <= Xc).  Rounding error per contribution <= 2.4e-7 Xc.
             Win<NBW> w;
-            win_init<NBW, true>(w, zb.sR0, stage, tid, nbins);
-            const float xs_ = zb.cf * S;
+            win_init<NBW, true>(w, q_init, stage, tid, nbins);
             const int R0 = X.rmin, R1 = X.rmax;
+            const float lim = 4194302.f; // |c S| <= 2^22 - 2 and kTS |c S| < 2^31
             for (int r0 = R0; r0 <= R1; r0 += rows_cap) {
                 const int rows = min(rows_cap, R1 - r0 + 1);
-                const int rb = max(zb.r_lo, r0), re = min(zb.r_hi, r0 + rows - 1);
-                if (rb <= re) {
-                    float fk = (float)(rb - zb.r_lo);
-                    uint32_t row = ci_base + (uint32_t)((rb - r0) * P) * 4u;
-#pragma unroll 1
-                    for (int it = re - rb + 1; it > 0; --it) {
-                        const float u = fmaf(zb.b2, fk, zb.a2);
-                        const float tt = __fadd_rd(u, kMagic);
-                        const float wz = u - (tt - kMagic);
-                        const uint32_t a = row + (__float_as_uint(tt) << 2);
-                        float wt[NBW];
-                        win_weights<NBW, true>(w, fmaf(zb.ds, fk, zb.sR0), tab_addr, stage, tid, nbins, zb.cf, wt);
-                        float sm = 0.f;
+                const int rb = max(zr.r_lo, r0), re = min(zr.r_hi, r0 + rows - 1);
+                build_wt(r0, rows);
+                { // bound of this LOR's contributions in the chunk
+                    float xm = 0.f;
+                    if (rb <= re) {
+                        const float qe = fmaf(zr.dq, (float)(re - zr.r_lo), zr.q0);
+                        const int k_hi = min(nbins - 1, (int)((__fadd_ru(qe, kMagicG) - kMagicG) * (1.f / kGKf)) + NBW);
+                        for (int k = max(w.base, 0); k <= k_hi; ++k) xm = fmaxf(xm, fabsf(stage[k * kTSLd + tid]));
+                        xm *= zr.cf;
+                    }
+                    for (int o = 16; o > 0; o >>= 1) xm = fmaxf(xm, __shfl_xor_sync(0xffffffffu, xm, o));
+                    if (lane == 0) red[warp] = xm;
+                }
+                __syncthreads(); // weight rows, red; the previous chunk's flush is complete
+                float xc = red[0];
 #pragma unroll
-                        for (int n = 0; n < NBW; ++n) sm = fmaf(w.a[n], wt[n], sm);
-                        const float xw = xs_ * sm;
-                        const int qxw = __float_as_int(xw + kMagic);
-                        const int bits = __float_as_int(fmaf(xw, wz, kMagic));
-                        reds_add_s<0>(a, qxw - bits);
-                        reds_add_s<4>(a, bits - kMagicI);
-                        fk += 1.f;
-                        row += (uint32_t)P * 4u;
+                for (int w2 = 1; w2 < kNW; ++w2) xc = fmaxf(xc, red[w2]);
+                if (!(xc > 0.f)) { // nothing to add on these planes (block-uniform)
+                    __syncthreads(); // red is rewritten by the next chunk
+                    continue;
+                }
+                const float S = lim / xc, invS = xc / lim;
+                if (rb <= re) {
+                    const float xs_ = zr.cf * S;
+                    float fk = (float)(rb - zr.r_lo);
+                    uint32_t row = ci_base + (uint32_t)((rb - r0) * P) * 4u;
+                    if (NG > 0) {
+                        uint32_t wrow = wt_base + (uint32_t)((gid * rows_cap + (rb - r0)) * WE) * 4u;
+#pragma unroll 2
+                        for (int it = re - rb + 1; it > 0; --it) {
+                            const float u = fmaf(zr.b2, fk, zr.a2u);
+                            const float tt = __fadd_rd(u, kMagic);
+                            const float wz = u - (tt - kMagic);
+                            const uint32_t a = row + (__float_as_uint(tt) << 2);
+                            float wv[WE];
+                            load_wentry<NBW, 0>(wrow, wv);
+                            win_slide<NBW, true>(w, wv[NBW], stage, tid, nbins, zr.cf);
+                            float sm = 0.f;
+#pragma unroll
+                            for (int n = 0; n < NBW; ++n) sm = fmaf(w.a[n], wv[n], sm);
+                            const float xw = xs_ * sm;
+                            const int qxw = __float_as_int(xw + kMagic);
+                            const int bits = __float_as_int(fmaf(xw, wz, kMagic));
+                            reds_add_s<0>(a, qxw - bits);
+                            reds_add_s<4>(a, bits - kMagicI);
+                            fk += 1.f;
+                            row += (uint32_t)P * 4u;
+                            wrow += WE * 4u;
+                        }
+                    } else {
+#pragma unroll 1
+                        for (int it = re - rb + 1; it > 0; --it) {
+                            const float u = fmaf(zr.b2, fk, zr.a2u);
+                            const float tt = __fadd_rd(u, kMagic);
+                            const float wz = u - (tt - kMagic);
+                            const uint32_t a = row + (__float_as_uint(tt) << 2);
+                            float wt[NBW];
+                            const float cq = tab_weights<NBW>(fmaf(zr.dq, fk, zr.q0), tab_addr, wt);
+                            win_slide<NBW, true>(w, cq, stage, tid, nbins, zr.cf);
+                            float sm = 0.f;
+#pragma unroll
+                            for (int n = 0; n < NBW; ++n) sm = fmaf(w.a[n], wt[n], sm);
+                            const float xw = xs_ * sm;
+                            const int qxw = __float_as_int(xw + kMagic);
+                            const int bits = __float_as_int(fmaf(xw, wz, kMagic));
+                            reds_add_s<0>(a, qxw - bits);
+                            reds_add_s<4>(a, bits - kMagicI);
+                            fk += 1.f;
+                            row += (uint32_t)P * 4u;
+                        }
                     }
                 }
                 __syncthreads();
@@ -559,7 +704,7 @@ __global__ void __launch_bounds__(kTS, 2) k_tof_sino_tile(TileArgs A)
                         if (ri.base_b >= 0) atomicAdd(A.img_w + ri.base_b + z, ri.wb * v);
                     }
                 }
-                __syncthreads();
+                // (the barrier at the top of the next chunk, or of the next item, orders the flush against the next scatter)
             }
         }
         if (MODE == 2) { // the forward walk of the next item starts from zeros
@@ -582,20 +727,22 @@ TileCfgS tile_cfg_s(const Geom &g, int nbw, int nbins, int mode, const void *img
     for (int P : pitches)
         if (need <= P) { c.P = P; break; }
     const int np = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
+    const size_t we = (size_t)((nbw + 1 + 3) / 4) * 4;
     const size_t fixed = (size_t)(kGK + 2) * nbw * sizeof(float2) + ((((size_t)nbins * kTSLd + 3) & ~(size_t)3)) * sizeof(float) +
                          (size_t)np * sizeof(RowInfo) + (size_t)kTS * sizeof(int);
     const size_t elem = (mode == 1) ? sizeof(int) : sizeof(float2);
-    const size_t budget = 110 * 1024; // two CTAs per SM
+    const size_t wrow = (size_t)kGMax * we * sizeof(float); // weight rows of one plane
+    const size_t budget = 110 * 1024;                       // two CTAs per SM
     size_t rows = 0;
     if (c.P) {
-        const size_t row = (size_t)c.P * elem;
+        const size_t row = (size_t)c.P * elem + wrow;
         rows = fixed + 8 * row <= budget ? (budget - fixed) / row : 0;
-        if (rows > 32) rows = 32;
+        if (rows > (size_t)(kTS / kGMax)) rows = kTS / kGMax; // one thread per (group, plane) builds the weight rows
         if (rows > (size_t)np) rows = (size_t)np;
         if (rows < 8) { c.P = 0; rows = 0; }
     }
     c.rows_cap = (int)rows;
-    c.smem = fixed + rows * (size_t)c.P * elem;
+    c.smem = fixed + rows * ((size_t)c.P * elem + wrow);
     c.vec_r = (g.n[2] % 4 == 0) && ((uintptr_t)img_r % 16 == 0);
     c.vec_w = (g.n[2] % 4 == 0) && ((uintptr_t)img_w % 16 == 0);
     return c;
@@ -621,6 +768,8 @@ cudaError_t launch_tile(const TileArgs &A, size_t smem, cudaStream_t st)
 
 } // namespace
 
+int tof_window_bins(const Tof &t, double *R_out) { return window_bins(t, R_out); }
+
 cudaError_t launch_tof_sino_tile(int mode, const SinoPlanView &pv, int64_t k0, int64_t nk, const float *img_r, float *img_w,
                                  const Geom &g, const Tof &t, float *p, const float *y, const SinoEpi *epi_in, cudaStream_t st)
 {
@@ -636,7 +785,12 @@ cudaError_t launch_tof_sino_tile(int mode, const SinoPlanView &pv, int64_t k0, i
         return cudaErrorNotSupported;
     }
     TileArgs A{};
-    A.trk = pv.trk; A.zpat = pv.zpat; A.order = pv.order; A.T = pv.T; A.dz_max = pv.dz_max;
+    A.trk = pv.trk; A.zpat = pv.zpat; A.order = pv.order; A.slot_grp = pv.slot_grp; A.slice_ng = pv.slice_ng;
+    A.T = pv.T; A.dz_max = pv.dz_max;
+    if (pv.slice_len != kTS) { // the plan's slices are not ours (never happens: both come from kSinoSlice)
+        gtab_destroy(&gt, st);
+        return cudaErrorNotSupported;
+    }
     A.k0 = k0; A.nk = nk; A.img_r = img_r; A.img_w = img_w; A.g = g; A.t = t; A.gt = gt;
     A.P = c.P; A.rows_cap = c.rows_cap; A.vec_r = c.vec_r; A.vec_w = c.vec_w; A.p = p; A.y = y;
     A.epi = epi_in ? *epi_in : SinoEpi{};

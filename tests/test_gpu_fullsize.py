@@ -110,6 +110,20 @@ def test_config2_full_tof_sino(cuda_device, phantom_dev):
     assert_back(b, oracle.back_tof_sino(hxs, hxe, ys[idx].cpu().numpy(), G.n, G.origin, G.voxsize, *TOF_ARGS))
     bd = jp.jp_back_tof_sino(xs, xe, y, G.n, G.origin, G.voxsize, tof)
     assert adj_gap(p, y, imgd, bd) <= ADJ_GAP
+    # the planned calls (track tiles of the sinogram plan: the configuration bench.py times), same checks
+    plan = jp.SinoPlan(xs, xe)
+    assert plan.regular and plan.track_length == 2304 and plan.n_tracks == 16 * 257 and plan.n == n
+    pp = jp.jp_fwd_tof_sino_planned(plan, imgd, G.origin, G.voxsize, tof)
+    assert_fwd(pp[idx], ref)
+    assert torch.allclose(pp.sum(1), 0.99730020393674 * pn, rtol=3e-5, atol=2e-3)
+    assert float((pp - p).abs().max()) <= 2e-5 * float(p.abs().max())
+    del p, pn
+    b = jp.jp_back_tof_sino_planned(plan, ys, G.n, G.origin, G.voxsize, tof)
+    assert_back(b, oracle.back_tof_sino(hxs, hxe, ys[idx].cpu().numpy(), G.n, G.origin, G.voxsize, *TOF_ARGS))
+    bp = jp.jp_back_tof_sino_planned(plan, y, G.n, G.origin, G.voxsize, tof)
+    assert adj_gap(pp, y, imgd, bp) <= ADJ_GAP
+    assert float((bp - bd).abs().max()) <= 1e-4 * float(bd.abs().max())    # dense y: tile path == per-LOR path
+    plan.destroy()
 
 
 @pytest.fixture(scope="module")
@@ -199,9 +213,17 @@ def test_sino_osem_full_subset(cuda_device, phantom_dev):
                                contam[idx].cpu().numpy(), np.ones((1,) + tuple(G.n)), x0, G.origin, G.voxsize,
                                *TOF_ARGS, n_iter=1)
     assert_back(x, ref)
-    # and a dense run: finite, non-negative, zero where the start image is zero
+    plan = jp.SinoPlan(xs, xe)
+    xp = torch.from_numpy(x0).to(cuda_device)
+    jp.jp_sino_osem_tof_planned(plan, [0, n], y, mult, contam, sens, xp, G.origin, G.voxsize, tof, n_iter=1)
+    assert_back(xp, ref)
+    # and a dense run: finite, non-negative, zero where the start image is zero; planned == unplanned
     y = inputs.uniform_values((n, 29), 0.0, 1.0, seed=inputs.BASE_SEED + 308, device=cuda_device)
     x = imgd.clone()
     jp.jp_sino_osem_tof(xs, xe, [0, n], y, mult, contam, sens, x, G.origin, G.voxsize, tof, n_iter=1)
     assert torch.isfinite(x).all() and float(x.min()) >= 0.0
     assert float(x[imgd == 0].abs().max()) == 0.0
+    xp = imgd.clone()
+    jp.jp_sino_osem_tof_planned(plan, [0, n], y, mult, contam, sens, xp, G.origin, G.voxsize, tof, n_iter=1)
+    assert float((xp - x).abs().max()) <= 1e-4 * float(x.abs().max())
+    plan.destroy()
