@@ -308,11 +308,10 @@ class Workload:
             self.p = torch.empty(shape, dtype=torch.float32, device=dev)
             self.plane_steps = jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
             self.kinds = ("fwd", "back") if c == 1 else ("sino", "sino")
-            self.launches = 6 if c == 1 else 8   # c1: (track probe, tile kernel, its per-track twin) x 2; c2: pad/unpad, 2 tables, kernel
-            if c == 2:
-                self.make_sino_plan()
-                if self.splan is not None:
-                    self.launches = 4            # per direction: weight table + track-tile kernel
+            self.launches = 2 if c == 1 else 8   # unplanned: c1 one tile kernel per direction; c2: pad/unpad, 2 tables, kernel
+            self.make_sino_plan()
+            if self.splan is not None:
+                self.launches = 2 if c == 1 else 4   # c1: one track-tile kernel per direction; c2: + the weight table
             self.hbm_bytes = (self.n * 28 + NVOX * 4) if c == 1 else (self.n * (24 + 4 * TOFP.n_tofbins) + NVOX * 4)
         else:
             nev = int(os.environ.get("JP_BENCH_EVENTS", "40000000"))
@@ -365,7 +364,10 @@ class Workload:
         if c == 0:
             jp.jp_fwd(self.xs, self.xe, self.img, self.g.origin, self.g.voxsize, out=self.p)
         elif c == 1:
-            jp.jp_fwd(self.xs, self.xe, self.img, G.origin, G.voxsize, out=self.p)
+            if self.splan is not None:
+                jp.jp_fwd_planned(self.splan, self.img, G.origin, G.voxsize, out=self.p)
+            else:
+                jp.jp_fwd(self.xs, self.xe, self.img, G.origin, G.voxsize, out=self.p)
         elif c == 2:
             if self.splan is not None:
                 jp.jp_fwd_tof_sino_planned(self.splan, self.img, G.origin, G.voxsize, self.tof, out=self.p)
@@ -389,7 +391,10 @@ class Workload:
         if c == 0:
             jp.jp_back(self.xs, self.xe, self.y, self.g.n, self.g.origin, self.g.voxsize, img=self.bimg)
         elif c == 1:
-            jp.jp_back(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
+            if self.splan is not None:
+                jp.jp_back_planned(self.splan, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
+            else:
+                jp.jp_back(self.xs, self.xe, self.y, G.n, G.origin, G.voxsize, img=self.bimg)
         elif c == 2:
             if self.splan is not None:
                 jp.jp_back_tof_sino_planned(self.splan, self.y, G.n, G.origin, G.voxsize, self.tof, img=self.bimg)
@@ -443,22 +448,29 @@ class Workload:
         y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 136, device=self.dev)
         p = torch.empty(n, dtype=torch.float32, device=self.dev)
         steps = jp.jp_plane_steps(xs, xe, G.n, G.origin, G.voxsize)
-        f = lambda: jp.jp_fwd(xs, xe, self.img, G.origin, G.voxsize, out=p)
-        b = lambda: jp.jp_back(xs, xe, y, G.n, G.origin, G.voxsize, img=self.bimg)
-        f(); self.bimg.zero_(); b()
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-        ev[0].record(s)
-        for _ in range(reps):
-            f()
-        ev[1].record(s)
-        for _ in range(reps):
-            self.bimg.zero_()
-            b()
-        ev[2].record(s)
-        torch.cuda.synchronize()
-        fm, bm = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
-        return {"lors": n, "track_length": 1296, "plane_steps": steps, "fwd_ms": fm, "back_ms": bm,
-                "fwd_plane_steps_per_s": steps / fm * 1e3, "back_plane_steps_per_s": steps / bm * 1e3}
+        plan = jp.SinoPlan(xs, xe)
+        out = {"lors": n, "track_length": plan.track_length, "plane_steps": steps}
+        calls = {"planned": (lambda: jp.jp_fwd_planned(plan, self.img, G.origin, G.voxsize, out=p),
+                             lambda: jp.jp_back_planned(plan, y, G.n, G.origin, G.voxsize, img=self.bimg)),
+                 "unplanned": (lambda: jp.jp_fwd(xs, xe, self.img, G.origin, G.voxsize, out=p),
+                               lambda: jp.jp_back(xs, xe, y, G.n, G.origin, G.voxsize, img=self.bimg))}
+        for name, (f, b) in calls.items():
+            f(); self.bimg.zero_(); b()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            ev[0].record(s)
+            for _ in range(reps):
+                f()
+            ev[1].record(s)
+            for _ in range(reps):
+                self.bimg.zero_()
+                b()
+            ev[2].record(s)
+            torch.cuda.synchronize()
+            fm, bm = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+            out[name] = {"fwd_ms": fm, "back_ms": bm, "fwd_plane_steps_per_s": steps / fm * 1e3,
+                         "back_plane_steps_per_s": steps / bm * 1e3}
+        plan.destroy()
+        return out
 
     def time_osem_with_resolution_model(self, iters=2):
         """the same OSEM iteration with the 4.5 mm FWHM image-based resolution model
@@ -666,7 +678,7 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     kf, kb = w.kinds
     planned = getattr(w, "splan", None) is not None
     names = {0: ("k_fwd_tile (per-LOR path: random chords are not tracks)", "k_back_tile (per-LOR path)"),
-             1: ("k_fwd_tile", "k_back_tile"),
+             1: ("k_fwd_tile<104, plan>", "k_back_tile<104, plan>") if planned else ("k_fwd_tile<104, list>", "k_back_tile<104, list>"),
              2: ("k_tof_sino_tile<6,fwd>", "k_tof_sino_tile<6,back>") if planned else ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
              3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_osem_tof_lm_quad (forward + ratio + back per event)", ""),
              5: ("k_tof_sino_tile<6,osem> (forward + ratio + back per track slice)" if planned else

@@ -84,6 +84,8 @@ EXPORTS = {
     "jp_sino_plan_create": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(C.c_void_p)]),
     "jp_sino_plan_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32)]),
     "jp_plan_destroy": (C.c_int, [C.c_void_p]),
+    "jp_fwd_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_void_p, C.c_void_p]),
+    "jp_back_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_void_p, C.c_void_p]),
     "jp_fwd_tof_sino_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
                                           C.c_void_p]),
     "jp_back_tof_sino_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p,
@@ -558,6 +560,32 @@ class SinoPlan:
             self.destroy()
         except Exception:
             pass
+
+
+def jp_fwd_planned(plan: SinoPlan, img, origin, voxsize, out=None, stream=None) -> torch.Tensor:
+    """non-TOF forward projection of the plan's LORs (results in list order)"""
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    if out is None:
+        out = torch.empty(plan.n, dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == plan.n and out.is_contiguous()
+    _check(load().jp_fwd_planned(plan.handle, img.data_ptr(), C.byref(g), out.data_ptr(), _stream(stream)),
+           "jp_fwd_planned")
+    return out
+
+
+def jp_back_planned(plan: SinoPlan, y, n, origin, voxsize, img=None, stream=None) -> torch.Tensor:
+    """img += A^T y over the plan's LORs (a zero image is made when img is None)"""
+    _dev(y, torch.float32, "y")
+    assert y.numel() == plan.n and y.is_contiguous()
+    if img is None:
+        img = torch.zeros(tuple(int(x) for x in n), dtype=torch.float32, device=y.device)
+    img = _img(img)
+    g = make_geom(img.shape, origin, voxsize)
+    _check(load().jp_back_planned(plan.handle, y.data_ptr(), C.byref(g), img.data_ptr(), _stream(stream)),
+           "jp_back_planned")
+    return img
 
 
 def jp_fwd_tof_sino_planned(plan: SinoPlan, img, origin, voxsize, tof: jp_tof, out=None, stream=None) -> torch.Tensor:

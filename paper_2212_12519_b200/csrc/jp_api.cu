@@ -891,6 +891,53 @@ bool subsets_on_tracks(const int64_t *off, int n_subsets, int T)
 
 } // namespace
 
+// non-TOF projections of a sinogram plan's LORs: per-track tiles read the track table and the axial pattern only
+int jp_fwd_planned(const jp_plan *plan, const float *img, const jp_geom *geom, float *p, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    jp::Geom g;
+    JP_TRY(check_geom(geom, g));
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    if (!img || (v.n > 0 && !p)) return fail(JP_ERR_POINTER, "img or p is NULL");
+    if (v.n == 0) return JP_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (v.regular) {
+        const cudaError_t e = jp::launch_fwd_tile(jp::Lors{}, v.n, img, g, p, st, &v);
+        if (e != cudaErrorNotSupported) {
+            JP_CUDA(e, "jp_fwd_planned");
+            return JP_OK;
+        }
+    }
+    PlanLors pl;
+    JP_CUDA(pl.init(v, st), "jp_fwd_planned (LOR list)");
+    JP_CUDA(jp::launch_fwd_tile(pl.l, v.n, img, g, p, st), "jp_fwd_planned");
+    return JP_OK;
+}
+
+int jp_back_planned(const jp_plan *plan, const float *y, const jp_geom *geom, float *img, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->sino) return fail(JP_ERR_PLAN, "not a sinogram plan");
+    jp::Geom g;
+    JP_TRY(check_geom(geom, g));
+    const jp::SinoPlanView v = jp::sino_plan_view(plan->sino);
+    if (!img || (v.n > 0 && !y)) return fail(JP_ERR_POINTER, "img or y is NULL");
+    if (v.n == 0) return JP_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (v.regular) {
+        const cudaError_t e = jp::launch_back_tile(jp::Lors{}, v.n, y, g, img, st, &v);
+        if (e != cudaErrorNotSupported) {
+            JP_CUDA(e, "jp_back_planned");
+            return JP_OK;
+        }
+    }
+    PlanLors pl;
+    JP_CUDA(pl.init(v, st), "jp_back_planned (LOR list)");
+    JP_CUDA(jp::launch_back_tile(pl.l, v.n, y, g, img, st), "jp_back_planned");
+    return JP_OK;
+}
+
 int jp_fwd_tof_sino_planned(const jp_plan *plan, const float *img, const jp_geom *geom, const jp_tof *tof, float *p,
                             void *stream)
 {

@@ -34,8 +34,12 @@ cudaError_t launch_fwd(const Lors &l, Range rg, const float *img, const Geom &g,
 cudaError_t launch_back(const Lors &l, Range rg, const float *y, const Geom &g, float *img, cudaStream_t st);
 
 // tiled non-TOF kernels (jp_tile.cu): track tiles through shared memory, everything else per LOR
-cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st);
-cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st);
+// pv: a REGULAR sinogram plan (tiles per track, `l` is not read), or null: tiles of 768 consecutive LORs of `l`
+struct SinoPlanView;
+cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st,
+                            const SinoPlanView *pv = nullptr, int lane_map = 1);
+cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st,
+                             const SinoPlanView *pv = nullptr, int lane_map = 1);
 
 // table of the TOF edge function (jp_tof_lut.cu): stream-ordered device scratch, one per call
 cudaError_t tof_lut_create(const Tof &t, cudaStream_t st, TofLut *out);

@@ -16,10 +16,8 @@
 // Planes are processed in chunks of `rows_cap` rows (shared memory = rows_cap x P x 8 or 4 bytes; the
 // row pitch P is a template parameter so that the unrolled plane loop addresses rows with immediates).
 // Tiles that are not tracks (ragged tail, principal axis z, unsorted lists) take the generic per-LOR
-// path in the same launch.  No plan, no scratch memory, results in caller order.
-#include <cstdlib>
-#include <mutex>
-
+// path in the same launch.  No scratch memory, no state between calls, results in caller order.  With a regular
+// sinogram plan (jp_fwd_planned / jp_back_planned) tiles are dealt per track and no end-point array is read.
 #include "jp_tile_common.cuh"
 
 #ifndef JP_BACK_MAP
@@ -70,28 +68,6 @@ __device__ __forceinline__ void generic_back(const Lors &l, int64_t j, const Geo
 //            the second half-warp the neighbouring diagonal.
 // The row length L of the grid is read off the data: the first LOR whose zs or ze changes while the other one
 // has been constant so far.  No grid (L = 0): identity mapping.
-__device__ __forceinline__ int detect_row_length(const Lors &l, int64_t j0, int64_t n, int *sh /* 2 ints */)
-{
-    const int tid = threadIdx.x;
-    if (tid < 2) sh[tid] = kThreads;
-    __syncthreads();
-    if (j0 + kTile <= n) {
-        const float zs0 = l.zs[j0], ze0 = l.ze[j0];
-        const bool ds = !same_bits(l.zs[j0 + tid], zs0), de = !same_bits(l.ze[j0 + tid], ze0);
-        const unsigned bs = __ballot_sync(0xffffffffu, ds), be = __ballot_sync(0xffffffffu, de);
-        if ((tid & 31) == 0) {
-            if (bs) atomicMin(&sh[0], (tid & ~31) + __ffs(bs) - 1);
-            if (be) atomicMin(&sh[1], (tid & ~31) + __ffs(be) - 1);
-        }
-    }
-    __syncthreads();
-    const int Ls = sh[0], Le = sh[1];
-    int L = 0;
-    if (Ls == 1 && Le < kThreads) L = Le;       // zs runs along a row, ze is the row's constant
-    else if (Le == 1 && Ls < kThreads) L = Ls;  // the other way round
-    return L;
-}
-
 // forward: half-warp h of the tile <- rows (2 rp, 2 rp + 1) x columns [8 cg, 8 cg + 8)
 __device__ __forceinline__ int map_fwd(int idx, int L)
 {
@@ -112,65 +88,56 @@ __device__ __forceinline__ int map_back(int idx, int L)
     return (rb * 16 + d) * L + col;
 }
 
-// ---- tiles cut per track ---------------------------------------------------------------------------------------
-// A tile is 768 CONSECUTIVE LORs, so a track whose length T is not a multiple of 768 (e.g. 36 rings: 1296 ring
-// pairs) would leave every other tile straddling two tracks, i.e. on the per-LOR path.  k_track_probe reads T off
-// the head of the list (length of the first run of identical transaxial end points) and, when T > 768 is not a
-// multiple of 768, the CUT instantiation of the kernels (persistent CTAs) deals tiles per track instead:
-// track k = tile / ceil(T / 768) is cut into pieces of 768 and one shorter piece.  The list is ASSUMED to consist
-// of tracks of that length; where it does not, tile_is_track fails and the tile takes the per-LOR path as before.
-// *cut_len == 0 selects the plain instantiation (both are launched; the one not selected exits at once).
-__global__ void k_track_probe(Lors l, int64_t n, int *cut_len)
+// ---- where a tile's LORs come from -------------------------------------------------------------------------------
+// LIST: 768 consecutive LORs of the caller's arrays; a tile is a track if all 768 share their transaxial end points
+//       (checked at run time, bit-exactly).
+// PLAN: a regular sinogram plan (jp_sino_plan.cu): K tracks of T LORs with one axial pattern.  Tiles are dealt PER TRACK
+//       (track = tile / tpt, pieces of 768 and one shorter piece when T is not a multiple of 768, e.g. 36 rings: 1296 =
+//       768 + 528), the transaxial end points come from the track table and the axial ones from the pattern: no
+//       end-point arrays are read at all (24 bytes per LOR of HBM traffic saved) and nothing needs checking.
+struct PlanSrc {
+    const float4 *trk;  // [K] (xs, ys, xe, ye)
+    const float2 *zpat; // [T] (zs, ze)
+    int T;
+    int tpt;            // tiles per track = ceil(T / kTile)
+    double dz_max;      // max |ze - zs| of the pattern: tracks with dz_max > max(|dx|, |dy|) take the per-LOR path
+};
+
+template <bool PLAN>
+struct TileSrc {
+    const Lors &l;
+    const PlanSrc &ps;
+    int64_t j0; // first LOR of the tile in the list
+    int k0;     // PLAN: first pattern index of the tile
+    __device__ __forceinline__ float zs(int i) const { return PLAN ? __ldg(ps.zpat + k0 + i).x : l.zs[j0 + i]; }
+    __device__ __forceinline__ float ze(int i) const { return PLAN ? __ldg(ps.zpat + k0 + i).y : l.ze[j0 + i]; }
+};
+
+// row length of the tile's (zs, ze) grid, see "lane mapping" above (full tiles only)
+template <bool PLAN>
+__device__ __forceinline__ int detect_row_length(const TileSrc<PLAN> &src, int *sh /* 2 ints */)
 {
-    __shared__ int first;
     const int tid = threadIdx.x;
-    if (tid == 0) first = 0x7fffffff;
+    if (tid < 2) sh[tid] = kThreads;
     __syncthreads();
-    const int64_t lim = n < 8192 ? n : 8192; // tracks longer than this are treated as aligned
-    const float xs0 = l.xs[0], ys0 = l.ys[0], xe0 = l.xe[0], ye0 = l.ye[0];
-    // 8 positions per thread, all loads independent (one round trip instead of a dependent loop)
-    uint32_t d[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-        const int64_t j = (int64_t)u * blockDim.x + tid;
-        d[u] = 0;
-        if (j < lim)
-            d[u] = (__float_as_uint(l.xs[j]) ^ __float_as_uint(xs0)) | (__float_as_uint(l.ys[j]) ^ __float_as_uint(ys0)) |
-                   (__float_as_uint(l.xe[j]) ^ __float_as_uint(xe0)) | (__float_as_uint(l.ye[j]) ^ __float_as_uint(ye0));
-    }
-#pragma unroll
-    for (int u = 0; u < 8; ++u)
-        if (d[u]) {
-            atomicMin(&first, u * (int)blockDim.x + tid);
-            break;
+    {
+        const float zs0 = src.zs(0), ze0 = src.ze(0);
+        const bool ds = !same_bits(src.zs(tid), zs0), de = !same_bits(src.ze(tid), ze0);
+        const unsigned bs = __ballot_sync(0xffffffffu, ds), be = __ballot_sync(0xffffffffu, de);
+        if ((tid & 31) == 0) {
+            if (bs) atomicMin(&sh[0], (tid & ~31) + __ffs(bs) - 1);
+            if (be) atomicMin(&sh[1], (tid & ~31) + __ffs(be) - 1);
         }
+    }
     __syncthreads();
-    if (tid == 0) {
-        const int T = first;
-        *cut_len = (T != 0x7fffffff && T > kTile && (T % kTile) != 0) ? T : 0;
-    }
+    const int Ls = sh[0], Le = sh[1];
+    int L = 0;
+    if (Ls == 1 && Le < kThreads) L = Le;       // zs runs along a row, ze is the row's constant
+    else if (Le == 1 && Ls < kThreads) L = Ls;  // the other way round
+    return L;
 }
 
-// first LOR and length of tile number `tile` (CUT: per track, see above); false when the list is exhausted
-template <bool CUT>
-__device__ __forceinline__ bool tile_span(int64_t tile, int64_t n, int T, int64_t &j0, int &tn)
-{
-    if (CUT) {
-        const int tpt = (T + kTile - 1) / kTile;
-        const int64_t k = tile / tpt;
-        const int t = (int)(tile - k * tpt);
-        j0 = k * (int64_t)T + (int64_t)t * kTile;
-        tn = min(kTile, T - t * kTile);
-    } else {
-        j0 = tile * (int64_t)kTile;
-        tn = kTile;
-    }
-    if (j0 >= n) return false;
-    if (j0 + tn > n) tn = (int)(n - j0);
-    return true;
-}
-
-// is this tile a track?  all 768 LORs valid, identical transaxial end points, principal axis x or y
+// is this LIST tile a track?  all 768 LORs valid, identical transaxial end points, principal axis x or y
 __device__ __forceinline__ bool tile_is_track_full(const Lors &l, int64_t j0, int64_t n, const int (&jm)[kPerThread],
                                               const float (&zs)[kPerThread], const float (&ze)[kPerThread], float xs0,
                                               float ys0, float xe0, float ye0)
@@ -189,29 +156,6 @@ __device__ __forceinline__ bool tile_is_track_full(const Lors &l, int64_t j0, in
         }
         ok = ok && (diff == 0) && (dmax > 0.0);
     }
-    return __syncthreads_and(ok) != 0;
-}
-
-// is this tile a track?  all tn LORs have identical transaxial end points and principal axis x or y
-template <bool CUT>
-__device__ __forceinline__ bool tile_is_track(const Lors &l, int64_t j0, int tn, const int (&jm)[kPerThread],
-                                              const float (&zs)[kPerThread], const float (&ze)[kPerThread], float xs0,
-                                              float ys0, float xe0, float ye0)
-{
-    const double dmax = fmax(fabs((double)xe0 - (double)xs0), fabs((double)ye0 - (double)ys0));
-    // all loads first (no short-circuit: twelve independent loads in flight), then compare bits
-    uint32_t diff = 0;
-    bool ok = (dmax > 0.0) && (CUT || tn == kTile); // plain: full tiles only, so that no slot needs a guard afterwards
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        if (jm[m] < tn) {
-            const int64_t j = j0 + jm[m];
-            diff |= (__float_as_uint(l.xs[j]) ^ __float_as_uint(xs0)) | (__float_as_uint(l.ys[j]) ^ __float_as_uint(ys0)) |
-                    (__float_as_uint(l.xe[j]) ^ __float_as_uint(xe0)) | (__float_as_uint(l.ye[j]) ^ __float_as_uint(ye0));
-            ok = ok && (fabs((double)ze[m] - (double)zs[m]) <= dmax);
-        }
-    }
-    ok = ok && (diff == 0);
     return __syncthreads_and(ok) != 0;
 }
 
@@ -267,149 +211,59 @@ __device__ __forceinline__ void reds_add(uint32_t addr, int q)
         acc1 = fmaf(u, v.y, acc1);                                             \
     }
 
-template <int P>
-__global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
-    k_fwd_tile(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
-               int lane_map, const int *__restrict__ cut_len, float *__restrict__ p)
+// generic per-LOR forward / back from explicit end points (PLAN tiles on tracks that may hold principal-axis-z LORs)
+__device__ __forceinline__ float generic_fwd_pts(const double (&s)[3], const double (&e)[3], const Geom &g,
+                                                 const float *__restrict__ img)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                      // [rows_cap][P]
-    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(float2)); // [max(n0,n1)]
-    __shared__ Track trk;
-    __shared__ int sh_len[2];
-    const int tid = threadIdx.x;
-    const int64_t j0 = blockIdx.x * (int64_t)kTile;
-
-    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
-    int jm[kPerThread];
-    float zs[kPerThread], ze[kPerThread];
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        jm[m] = m * kThreads + tid;
-        const int64_t j = j0 + jm[m];
-        zs[m] = (j < n) ? l.zs[j] : 0.f;
-        ze[m] = (j < n) ? l.ze[j] : 0.f;
+    Ray r;
+    ray_setup_pts<false>(s, e, g, 0.f, 0.f, 0.f, r);
+    float acc = 0.f;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        acc += plane_value(img, r, k, cl);
     }
-    const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (cut_len && __ldg(cut_len) != 0) return; // tiles are dealt per track: the _cut kernel does this list
-    if (!tile_is_track_full(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
-#pragma unroll 1
-        for (int m = 0; m < kPerThread; ++m) {
-            const int64_t j = j0 + m * kThreads + tid;
-            if (j < n) p[j] = generic_fwd(l, j, g, img);
-        }
-        return;
-    }
-    if (tid == 0) track_setup(g, xs0, ys0, xe0, ye0, trk);
-    __syncthreads();
-    const Track t = trk;
-    if (t.I1 < t.I0) { // the whole track misses the image
-#pragma unroll
-        for (int m = 0; m < kPerThread; ++m) p[j0 + m * kThreads + tid] = 0.f;
-        return;
-    }
-    // the tile does work: choose the lane mapping and fetch the axial end points again (from L1) in that order
-    const int L = lane_map ? detect_row_length(l, j0, n, sh_len) : 0;
-    if (L) {
-#pragma unroll
-        for (int m = 0; m < kPerThread; ++m) {
-            jm[m] = map_fwd(m * kThreads + tid, L);
-            zs[m] = l.zs[j0 + jm[m]];
-            ze[m] = l.ze[j0 + jm[m]];
-        }
-    }
-    const int n2 = g.n[2];
-    const int kci = n2 >> 1;          // axial shift of the (intercept, slope) rows
-    const float kc = (float)kci;
-    // q1 cells of all planes of the track; constant zero columns of the shared rows
-    for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
-    {
-        const int ncl = kPad - 1, ncr = P - (n2 + kPad);
-        for (int e = tid; e < rows_cap * (ncl + ncr); e += kThreads) {
-            const int r = e / (ncl + ncr), c = e - r * (ncl + ncr);
-            C2[r * P + (c < ncl ? c : n2 + kPad + (c - ncl))] = make_float2(0.f, 0.f);
-        }
-    }
-    ZRay zr[kPerThread];
-    float acc0[kPerThread], acc1[kPerThread];
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        zr[m] = z_setup(g, t, zs[m], ze[m], (double)kci);
-        acc0[m] = 0.f;
-        acc1[m] = 0.f;
-    }
-    const uint32_t c2_base = smem_addr(C2) + (uint32_t)(kPad + kci) * 8u - ((uint32_t)kMagicI << 3);
-    __syncthreads();
-
-    for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
-        const int rows = min(rows_cap, t.I1 - c0 + 1);
-        build_rows<P, true, JP_RB_TILE>(C2, rinfo, img, t, c0, rows, n2, vec_ok, kc);
-        __syncthreads();
-        // ---- consume: every LOR walks its planes of this chunk, interpolating along z only
-#pragma unroll
-        for (int m = 0; m < kPerThread; ++m) {
-            const int ib = max(zr[m].i0, c0), ie = min(zr[m].i1, c0 + rows - 1);
-            if (ib > ie) continue;
-            const int nst = ie - ib + 1;
-            const float b2 = zr[m].b2, a2_0 = zr[m].a2;
-            const float a2_1 = fmaf(b2, 1.f, a2_0), a2_2 = fmaf(b2, 2.f, a2_0), a2_3 = fmaf(b2, 3.f, a2_0);
-            float fk = (float)(ib - zr[m].i0);
-            uint32_t row = c2_base + (uint32_t)((ib - c0) * P) * 8u;
-            float a0 = acc0[m], a1 = acc1[m];
-            {
-                float acc0 = a0, acc1 = a1;
-                int left = nst;
-#if JP_FWD_UNROLL == 8
-                const float a2_4 = fmaf(b2, 4.f, a2_0), a2_5 = fmaf(b2, 5.f, a2_0), a2_6 = fmaf(b2, 6.f, a2_0),
-                            a2_7 = fmaf(b2, 7.f, a2_0);
-#pragma unroll 1
-                for (; left >= 8; left -= 8) {
-                    JP_FWD_STEP(0, a2_0)
-                    JP_FWD_STEP(1, a2_1)
-                    JP_FWD_STEP(2, a2_2)
-                    JP_FWD_STEP(3, a2_3)
-                    JP_FWD_STEP(4, a2_4)
-                    JP_FWD_STEP(5, a2_5)
-                    JP_FWD_STEP(6, a2_6)
-                    JP_FWD_STEP(7, a2_7)
-                    fk += 8.f;
-                    row += 8u * P * 8u;
-                }
-                if (left >= 4) {
-#else
-#pragma unroll 1
-                for (; left >= 4; left -= 4) {
-#endif
-                    JP_FWD_STEP(0, a2_0)
-                    JP_FWD_STEP(1, a2_1)
-                    JP_FWD_STEP(2, a2_2)
-                    JP_FWD_STEP(3, a2_3)
-                    fk += 4.f;
-                    row += 4u * P * 8u;
-                }
-#pragma unroll 1
-                for (int it = left & 3; it > 0; --it) {
-                    JP_FWD_STEP(0, a2_0)
-                    fk += 1.f;
-                    row += P * 8u;
-                }
-                a0 = acc0;
-                a1 = acc1;
-            }
-            acc0[m] = a0;
-            acc1[m] = a1;
-        }
-        __syncthreads();
-    }
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) p[j0 + map_fwd(m * kThreads + tid, L)] = zr[m].cf * (acc0[m] + acc1[m]);
+    return r.cf * acc;
 }
 
-// ---- the same kernel with tiles dealt per track (CUT = true; see k_track_probe) -----------------------------
-template <int P, bool CUT>
+__device__ __forceinline__ void generic_back_pts(const double (&s)[3], const double (&e)[3], const Geom &g, float y,
+                                                 float *__restrict__ img)
+{
+    Ray r;
+    ray_setup_pts<false>(s, e, g, 0.f, 0.f, 0.f, r);
+    const float x = r.cf * y;
+    if (r.nk == 0 || x == 0.f) return;
+    for (int k = 0; k < r.nk; ++k) {
+        const Cell cl = plane_cell(r, k);
+        plane_scatter(img, r, k, cl, x);
+    }
+}
+
+// first LOR, pattern offset, length and transaxial end points of the CTA's tile; false: nothing to do
+template <bool PLAN>
+__device__ __forceinline__ bool tile_of_block(const Lors &l, const PlanSrc &ps, int64_t n, int64_t &j0, int &k0, int &tn,
+                                              float &xs0, float &ys0, float &xe0, float &ye0)
+{
+    if (PLAN) {
+        const int64_t trk = blockIdx.x / ps.tpt;
+        const int piece = (int)(blockIdx.x - trk * ps.tpt);
+        k0 = piece * kTile;
+        j0 = trk * (int64_t)ps.T + k0;
+        tn = min(kTile, ps.T - k0);
+        const float4 q = __ldg(ps.trk + trk);
+        xs0 = q.x; ys0 = q.y; xe0 = q.z; ye0 = q.w;
+    } else {
+        j0 = blockIdx.x * (int64_t)kTile;
+        k0 = 0;
+        tn = (int)min((int64_t)kTile, n - j0);
+        xs0 = l.xs[j0]; ys0 = l.ys[j0]; xe0 = l.xe[j0]; ye0 = l.ye[j0];
+    }
+    return tn > 0;
+}
+
+template <int P, bool PLAN>
 __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
-    k_fwd_tile_cut(Lors l, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
-               int lane_map, const int *__restrict__ cut_len, float *__restrict__ p)
+    k_fwd_tile(Lors l, PlanSrc ps, int64_t n, const float *__restrict__ img, Geom g, int rows_cap, int vec_ok,
+               int lane_map, float *__restrict__ p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *C2 = reinterpret_cast<float2 *>(smem_raw);                                      // [rows_cap][P]
@@ -417,34 +271,40 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
     __shared__ Track trk;
     __shared__ int sh_len[2];
     const int tid = threadIdx.x;
-    const int T = cut_len ? __ldg(cut_len) : 0;
-    if (CUT && T == 0) return; // the plain instantiation does this list (it checks after its first loads are in flight)
-  // plain: one tile per CTA; CUT: persistent CTAs over the tiles dealt per track
-  for (int64_t tile = blockIdx.x; CUT || tile == blockIdx.x; tile += gridDim.x) {
     int64_t j0;
-    int tn;
-    if (!tile_span<CUT>(tile, n, T, j0, tn)) break;
-    if (CUT && tile != blockIdx.x) __syncthreads(); // the shared buffers of the previous tile are free
-
-    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
+    int k0, tn;
+    float xs0, ys0, xe0, ye0;
+    if (!PLAN) prefetch_tile(l, n, blockIdx.x * (int64_t)kTile + (int64_t)JP_PREFETCH_DIST * kTile);
+    if (!tile_of_block<PLAN>(l, ps, n, j0, k0, tn, xs0, ys0, xe0, ye0)) return;
+    TileSrc<PLAN> src{l, ps, j0, k0};
     int jm[kPerThread];
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
         jm[m] = m * kThreads + tid;
-        const int64_t j = j0 + jm[m];
-        zs[m] = (jm[m] < tn) ? l.zs[j] : 0.f;
-        ze[m] = (jm[m] < tn) ? l.ze[j] : 0.f;
+        zs[m] = (jm[m] < tn) ? src.zs(jm[m]) : 0.f;
+        ze[m] = (jm[m] < tn) ? src.ze(jm[m]) : 0.f;
     }
-    const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (!CUT && T != 0) return; // the CUT instantiation does this list
-    if (!tile_is_track<CUT>(l, j0, tn, jm, zs, ze, xs0, ys0, xe0, ye0)) {
+    bool is_track;
+    if (PLAN) {
+        const double dmax = fmax(fabs((double)xe0 - (double)xs0), fabs((double)ye0 - (double)ys0));
+        is_track = dmax > 0.0 && ps.dz_max <= dmax; // no LOR of the track can have principal axis z
+    } else {
+        is_track = tile_is_track_full(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0);
+    }
+    if (!is_track) {
 #pragma unroll 1
         for (int m = 0; m < kPerThread; ++m) {
-            const int64_t j = j0 + m * kThreads + tid;
-            if (m * kThreads + tid < tn) p[j] = generic_fwd(l, j, g, img);
+            const int i = m * kThreads + tid;
+            if (i >= tn) continue;
+            if (PLAN) {
+                const double sp[3] = {(double)xs0, (double)ys0, (double)zs[m]}, ep[3] = {(double)xe0, (double)ye0, (double)ze[m]};
+                p[j0 + i] = generic_fwd_pts(sp, ep, g, img);
+            } else {
+                p[j0 + i] = generic_fwd(l, j0 + i, g, img);
+            }
         }
-        continue;
+        return;
     }
     if (tid == 0) track_setup(g, xs0, ys0, xe0, ye0, trk);
     __syncthreads();
@@ -452,17 +312,17 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
     if (t.I1 < t.I0) { // the whole track misses the image
 #pragma unroll
         for (int m = 0; m < kPerThread; ++m)
-            if (!CUT || m * kThreads + tid < tn) p[j0 + m * kThreads + tid] = 0.f;
-        continue;
+            if (m * kThreads + tid < tn) p[j0 + m * kThreads + tid] = 0.f;
+        return;
     }
     // the tile does work: choose the lane mapping and fetch the axial end points again (from L1) in that order
-    const int L = (lane_map && (!CUT || tn == kTile)) ? detect_row_length(l, j0, n, sh_len) : 0;
+    const int L = (lane_map && tn == kTile) ? detect_row_length<PLAN>(src, sh_len) : 0;
     if (L) {
 #pragma unroll
         for (int m = 0; m < kPerThread; ++m) {
             jm[m] = map_fwd(m * kThreads + tid, L);
-            zs[m] = l.zs[j0 + jm[m]];
-            ze[m] = l.ze[j0 + jm[m]];
+            zs[m] = src.zs(jm[m]);
+            ze[m] = src.ze(jm[m]);
         }
     }
     const int n2 = g.n[2];
@@ -482,7 +342,7 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
         zr[m] = z_setup(g, t, zs[m], ze[m], (double)kci);
-        if (CUT && jm[m] >= tn) zr[m].i1 = zr[m].i0 - 1; // slot beyond a short tile
+        if (jm[m] >= tn) zr[m].i1 = zr[m].i0 - 1; // slot beyond a short tile
         acc0[m] = 0.f;
         acc1[m] = 0.f;
     }
@@ -550,11 +410,8 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
         __syncthreads();
     }
 #pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        const int jl = CUT ? jm[m] : map_fwd(m * kThreads + tid, L);
-        if (!CUT || jl < tn) p[j0 + jl] = zr[m].cf * (acc0[m] + acc1[m]);
-    }
-  }
+    for (int m = 0; m < kPerThread; ++m)
+        if (jm[m] < tn) p[j0 + jm[m]] = zr[m].cf * (acc0[m] + acc1[m]);
 }
 #undef JP_FWD_STEP
 
@@ -565,6 +422,8 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
 // magic-number rounding) nor a whole bin (at most two contributions per LOR and plane: |sum| <= 2 x 768 X S
 // < 2^31) can overflow.  Rounding error per contribution <= X 768 / 2^31 = 3.6e-7 X.
 // Per step the two bins get q1 = round(S x w) and q0 = round(S x) - q1 (their sum is exact).
+// A tile whose y holds Inf or NaN (on a LOR that crosses the image) cannot be staged: it takes the per-LOR path with
+// float atomics, so non-finite values propagate exactly as they do for LORs that are not in a track tile.
 #define JP_BACK_STEP(K, A2K)                                                   \
     {                                                                          \
         const float u = fmaf(b2, fk, A2K);                                     \
@@ -576,10 +435,10 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_FWD)
         reds_add<(K) * P * 4 + 4>(a, bits - kMagicI);                          \
     }
 
-template <int P>
+template <int P, bool PLAN>
 __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
-    k_back_tile(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
-                int lane_map, const int *__restrict__ cut_len, float *__restrict__ img)
+    k_back_tile(Lors l, PlanSrc ps, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
+                int lane_map, float *__restrict__ img)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     int *Ci = reinterpret_cast<int *>(smem_raw);                                        // [rows_cap][P]
@@ -587,40 +446,60 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
     __shared__ Track trk;
     __shared__ float red[kThreads / 32];
     __shared__ int sh_len[2];
+    __shared__ int sh_bad;
     const int tid = threadIdx.x;
-    const int64_t j0 = blockIdx.x * (int64_t)kTile;
-
-    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
+    int64_t j0;
+    int k0, tn;
+    float xs0, ys0, xe0, ye0;
+    if (!PLAN) prefetch_tile(l, n, blockIdx.x * (int64_t)kTile + (int64_t)JP_PREFETCH_DIST * kTile);
+    if (!tile_of_block<PLAN>(l, ps, n, j0, k0, tn, xs0, ys0, xe0, ye0)) return;
+    TileSrc<PLAN> src{l, ps, j0, k0};
     int jm[kPerThread];
     float zs[kPerThread], ze[kPerThread];
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
         jm[m] = m * kThreads + tid;
-        const int64_t j = j0 + jm[m];
-        zs[m] = (j < n) ? l.zs[j] : 0.f;
-        ze[m] = (j < n) ? l.ze[j] : 0.f;
+        zs[m] = (jm[m] < tn) ? src.zs(jm[m]) : 0.f;
+        ze[m] = (jm[m] < tn) ? src.ze(jm[m]) : 0.f;
     }
-    const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (cut_len && __ldg(cut_len) != 0) return; // tiles are dealt per track: the _cut kernel does this list
-    if (!tile_is_track_full(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0)) {
+    if (tid == 0) sh_bad = 0;
+    bool is_track;
+    if (PLAN) {
+        const double dmax = fmax(fabs((double)xe0 - (double)xs0), fabs((double)ye0 - (double)ys0));
+        is_track = dmax > 0.0 && ps.dz_max <= dmax;
+    } else {
+        is_track = tile_is_track_full(l, j0, n, jm, zs, ze, xs0, ys0, xe0, ye0);
+    }
+    // per-LOR path for the whole tile (float atomics): not a track, or non-finite values (below)
+    auto per_lor = [&]() {
 #pragma unroll 1
         for (int m = 0; m < kPerThread; ++m) {
-            const int64_t j = j0 + m * kThreads + tid;
-            if (j < n) generic_back(l, j, g, y[j], img);
+            const int i = m * kThreads + tid;
+            if (i >= tn) continue;
+            if (PLAN) {
+                const float zsi = src.zs(i), zei = src.ze(i);
+                const double sp[3] = {(double)xs0, (double)ys0, (double)zsi}, ep[3] = {(double)xe0, (double)ye0, (double)zei};
+                generic_back_pts(sp, ep, g, y[j0 + i], img);
+            } else {
+                generic_back(l, j0 + i, g, y[j0 + i], img);
+            }
         }
+    };
+    if (!is_track) {
+        per_lor();
         return;
     }
     if (tid == 0) track_setup(g, xs0, ys0, xe0, ye0, trk);
     __syncthreads();
     const Track t = trk;
     if (t.I1 < t.I0) return;
-    const int L = lane_map ? detect_row_length(l, j0, n, sh_len) : 0;
+    const int L = (lane_map && tn == kTile) ? detect_row_length<PLAN>(src, sh_len) : 0;
     if (L) {
 #pragma unroll
         for (int m = 0; m < kPerThread; ++m) {
             jm[m] = map_back(m * kThreads + tid, L);
-            zs[m] = l.zs[j0 + jm[m]];
-            ze[m] = l.ze[j0 + jm[m]];
+            zs[m] = src.zs(jm[m]);
+            ze[m] = src.ze(jm[m]);
         }
     }
     const int n2 = g.n[2];
@@ -628,12 +507,19 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
     ZRay zr[kPerThread];
     float x[kPerThread];
     float xmax = 0.f;
+    bool bad = false;
 #pragma unroll
     for (int m = 0; m < kPerThread; ++m) {
         zr[m] = z_setup(g, t, zs[m], ze[m]);
-        x[m] = zr[m].cf * y[j0 + jm[m]];
-        if (zr[m].i1 >= zr[m].i0) xmax = fmaxf(xmax, fabsf(x[m]));
+        x[m] = (jm[m] < tn) ? zr[m].cf * y[j0 + jm[m]] : 0.f;
+        if (jm[m] >= tn) zr[m].i1 = zr[m].i0 - 1; // slot beyond a short tile
+        if (zr[m].i1 >= zr[m].i0) {
+            const float ax = fabsf(x[m]);
+            bad = bad || !(ax < 3.0e38f); // Inf or NaN (fmaxf would drop a NaN)
+            xmax = fmaxf(xmax, ax);
+        }
     }
+    if (bad) atomicExch(&sh_bad, 1);
     // block max of |x|
     for (int o = 16; o > 0; o >>= 1) xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
     if ((tid & 31) == 0) red[tid >> 5] = xmax;
@@ -643,10 +529,14 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
         for (int e = tid; e < rows_cap * (P / 4); e += kThreads) z4[e] = make_int4(0, 0, 0, 0);
     }
     __syncthreads();
+    if (sh_bad) { // non-finite input on a LOR that crosses the image: propagate it as the per-LOR adjoint does
+        per_lor();
+        return;
+    }
     xmax = red[0];
 #pragma unroll
     for (int w = 1; w < kThreads / 32; ++w) xmax = fmaxf(xmax, red[w]);
-    if (!(xmax > 0.f) || !(xmax < 3.0e38f)) return; // nothing to add (or non-finite input: undefined, skip)
+    if (!(xmax > 0.f)) return; // nothing to add
     // S: |c S| <= 2^22 - 2 and 2 x 768 |c S| < 2^31
     const float lim = fminf(4194302.f, 2147483648.f / (float)(2 * kTile) - 1.f);
     const float S = lim / xmax, invS = xmax / lim;
@@ -697,10 +587,10 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
                 const RowInfo ri = rinfo[c0 - t.I0 + r];
                 const float sa = ri.wa * invS, sb = ri.wb * invS;
                 for (int gq = lane; gq < G; gq += 32) {
-                    int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
-                    const int4 q = *src;
+                    int4 *src4 = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
+                    const int4 q = *src4;
                     if ((q.x | q.y | q.z | q.w) == 0) continue;
-                    *src = make_int4(0, 0, 0, 0);
+                    *src4 = make_int4(0, 0, 0, 0);
                     const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
                     if (ri.base_a >= 0)
                         atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq,
@@ -724,165 +614,6 @@ __global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
         }
         __syncthreads();
     }
-}
-
-// ---- the same kernel with tiles dealt per track (CUT = true) --------------------------------------------------
-template <int P, bool CUT>
-__global__ void __launch_bounds__(kThreads, JP_MINB_BACK)
-    k_back_tile_cut(Lors l, int64_t n, const float *__restrict__ y, Geom g, int rows_cap, int vec_ok,
-                int lane_map, const int *__restrict__ cut_len, float *__restrict__ img)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    int *Ci = reinterpret_cast<int *>(smem_raw);                                        // [rows_cap][P]
-    RowInfo *rinfo = reinterpret_cast<RowInfo *>(smem_raw + (size_t)rows_cap * P * sizeof(int)); // [max(n0,n1)]
-    __shared__ Track trk;
-    __shared__ float red[kThreads / 32];
-    __shared__ int sh_len[2];
-    const int tid = threadIdx.x;
-    const int T = cut_len ? __ldg(cut_len) : 0;
-    if (CUT && T == 0) return; // the plain instantiation does this list (it checks after its first loads are in flight)
-  for (int64_t tile = blockIdx.x; CUT || tile == blockIdx.x; tile += gridDim.x) {
-    int64_t j0;
-    int tn;
-    if (!tile_span<CUT>(tile, n, T, j0, tn)) break;
-    if (CUT && tile != blockIdx.x) __syncthreads(); // the shared buffers of the previous tile are free
-
-    prefetch_tile(l, n, j0 + (int64_t)JP_PREFETCH_DIST * kTile);
-    int jm[kPerThread];
-    float zs[kPerThread], ze[kPerThread];
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        jm[m] = m * kThreads + tid;
-        const int64_t j = j0 + jm[m];
-        zs[m] = (jm[m] < tn) ? l.zs[j] : 0.f;
-        ze[m] = (jm[m] < tn) ? l.ze[j] : 0.f;
-    }
-    const float xs0 = l.xs[j0], ys0 = l.ys[j0], xe0 = l.xe[j0], ye0 = l.ye[j0];
-    if (!CUT && T != 0) return; // the CUT instantiation does this list
-    if (!tile_is_track<CUT>(l, j0, tn, jm, zs, ze, xs0, ys0, xe0, ye0)) {
-#pragma unroll 1
-        for (int m = 0; m < kPerThread; ++m) {
-            const int64_t j = j0 + m * kThreads + tid;
-            if (m * kThreads + tid < tn) generic_back(l, j, g, y[j], img);
-        }
-        continue;
-    }
-    if (tid == 0) track_setup(g, xs0, ys0, xe0, ye0, trk);
-    __syncthreads();
-    const Track t = trk;
-    if (t.I1 < t.I0) continue;
-    const int L = (lane_map && (!CUT || tn == kTile)) ? detect_row_length(l, j0, n, sh_len) : 0;
-    if (L) {
-#pragma unroll
-        for (int m = 0; m < kPerThread; ++m) {
-            jm[m] = map_back(m * kThreads + tid, L);
-            zs[m] = l.zs[j0 + jm[m]];
-            ze[m] = l.ze[j0 + jm[m]];
-        }
-    }
-    const int n2 = g.n[2];
-
-    ZRay zr[kPerThread];
-    float x[kPerThread];
-    float xmax = 0.f;
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        zr[m] = z_setup(g, t, zs[m], ze[m]);
-        x[m] = (!CUT || jm[m] < tn) ? zr[m].cf * y[j0 + jm[m]] : 0.f;
-        if (CUT && jm[m] >= tn) zr[m].i1 = zr[m].i0 - 1; // slot beyond a short tile
-        if (zr[m].i1 >= zr[m].i0) xmax = fmaxf(xmax, fabsf(x[m]));
-    }
-    // block max of |x|
-    for (int o = 16; o > 0; o >>= 1) xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
-    if ((tid & 31) == 0) red[tid >> 5] = xmax;
-    for (int r = tid; r <= t.I1 - t.I0; r += kThreads) rinfo[r] = row_info(g, t, t.I0 + r);
-    {
-        int4 *z4 = reinterpret_cast<int4 *>(Ci);
-        for (int e = tid; e < rows_cap * (P / 4); e += kThreads) z4[e] = make_int4(0, 0, 0, 0);
-    }
-    __syncthreads();
-    xmax = red[0];
-#pragma unroll
-    for (int w = 1; w < kThreads / 32; ++w) xmax = fmaxf(xmax, red[w]);
-    if (!(xmax > 0.f) || !(xmax < 3.0e38f)) continue; // nothing to add (or non-finite input: undefined, skip)
-    // S: |c S| <= 2^22 - 2 and 2 x 768 |c S| < 2^31
-    const float lim = fminf(4194302.f, 2147483648.f / (float)(2 * kTile) - 1.f);
-    const float S = lim / xmax, invS = xmax / lim;
-    int qx[kPerThread];
-#pragma unroll
-    for (int m = 0; m < kPerThread; ++m) {
-        x[m] *= S;
-        qx[m] = __float2int_rn(x[m]) + kMagicI;
-    }
-
-    const int warp = tid >> 5, lane = tid & 31;
-    const uint32_t ci_base = smem_addr(Ci) + kPad * 4u - ((uint32_t)kMagicI << 2);
-
-    for (int c0 = t.I0; c0 <= t.I1; c0 += rows_cap) {
-        const int rows = min(rows_cap, t.I1 - c0 + 1);
-        // ---- scatter along z into the fixed-point tile
-#pragma unroll
-        for (int m = 0; m < kPerThread; ++m) {
-            const int ib = max(zr[m].i0, c0), ie = min(zr[m].i1, c0 + rows - 1);
-            if (ib > ie || x[m] == 0.f) continue;
-            const int nst = ie - ib + 1;
-            const float b2 = zr[m].b2, a2_0 = zr[m].a2, xm = x[m];
-            const int qxm = qx[m];
-            const float a2_1 = fmaf(b2, 1.f, a2_0), a2_2 = fmaf(b2, 2.f, a2_0), a2_3 = fmaf(b2, 3.f, a2_0);
-            float fk = (float)(ib - zr[m].i0);
-            uint32_t row = ci_base + (uint32_t)((ib - c0) * P) * 4u;
-#pragma unroll 1
-            for (int it = nst >> 2; it > 0; --it) {
-                JP_BACK_STEP(0, a2_0)
-                JP_BACK_STEP(1, a2_1)
-                JP_BACK_STEP(2, a2_2)
-                JP_BACK_STEP(3, a2_3)
-                fk += 4.f;
-                row += 4u * P * 4u;
-            }
-#pragma unroll 1
-            for (int it = nst & 3; it > 0; --it) {
-                JP_BACK_STEP(0, a2_0)
-                fk += 1.f;
-                row += P * 4u;
-            }
-        }
-        __syncthreads();
-        // ---- flush: spread every row over its two q1 neighbours with REDs, and clear it
-        if (vec_ok) {
-            const int G = n2 >> 2;
-            for (int r = warp; r < rows; r += kThreads / 32) {
-                const RowInfo ri = rinfo[c0 - t.I0 + r];
-                const float sa = ri.wa * invS, sb = ri.wb * invS;
-                for (int gq = lane; gq < G; gq += 32) {
-                    int4 *src = reinterpret_cast<int4 *>(Ci + r * P + kPad) + gq;
-                    const int4 q = *src;
-                    if ((q.x | q.y | q.z | q.w) == 0) continue;
-                    *src = make_int4(0, 0, 0, 0);
-                    const float4 v = make_float4((float)q.x, (float)q.y, (float)q.z, (float)q.w);
-                    if (ri.base_a >= 0)
-                        atomicAdd(reinterpret_cast<float4 *>(img + ri.base_a) + gq,
-                                  make_float4(sa * v.x, sa * v.y, sa * v.z, sa * v.w));
-                    if (ri.base_b >= 0)
-                        atomicAdd(reinterpret_cast<float4 *>(img + ri.base_b) + gq,
-                                  make_float4(sb * v.x, sb * v.y, sb * v.z, sb * v.w));
-                }
-            }
-        } else {
-            for (int e = tid; e < rows * n2; e += kThreads) {
-                const int r = e / n2, z = e - r * n2;
-                const int q = Ci[r * P + kPad + z];
-                if (q == 0) continue;
-                Ci[r * P + kPad + z] = 0;
-                const RowInfo ri = rinfo[c0 - t.I0 + r];
-                const float v = (float)q * invS;
-                if (ri.base_a >= 0) atomicAdd(img + ri.base_a + z, ri.wa * v);
-                if (ri.base_b >= 0) atomicAdd(img + ri.base_b + z, ri.wb * v);
-            }
-        }
-        __syncthreads();
-    }
-  }
 }
 #undef JP_BACK_STEP
 
@@ -898,13 +629,6 @@ namespace {
 #define JP_SMEM_KB_BACK 28
 #endif
 constexpr size_t kSmemMax = 100 * 1024; // wide images: at least 24 rows per chunk, up to this much
-
-// JP_LANE_MAP=0 in the environment switches the lane mapping off (A/B measurements; results are the same)
-int lane_map_on()
-{
-    const char *e = getenv("JP_LANE_MAP");
-    return !(e && e[0] == '0');
-}
 
 struct TileCfg {
     int P;        // row pitch (0: image too wide along z for the tiled kernels)
@@ -936,9 +660,22 @@ TileCfg tile_cfg(const Geom &g, const void *img, size_t elem, size_t budget)
 }
 
 template <typename K>
-cudaError_t set_smem(K kernel, size_t smem)
+cudaError_t set_smem(K kernel)
 {
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
+}
+
+PlanSrc plan_src(const SinoPlanView *pv)
+{
+    PlanSrc ps{};
+    if (pv && pv->regular) {
+        ps.trk = pv->trk;
+        ps.zpat = pv->zpat;
+        ps.T = pv->T;
+        ps.tpt = (pv->T + kTile - 1) / kTile;
+        ps.dz_max = pv->dz_max;
+    }
+    return ps;
 }
 
 } // namespace
@@ -954,129 +691,57 @@ cudaError_t set_smem(K kernel, size_t smem)
     default: return cudaErrorInvalidValue;         \
     }
 
-// probe of the track length (lists long enough for it to matter); *out = device int (stream-ordered scratch) or null
-// The probe result is cached per LOR list, keyed by (device, address of xs, n): repeated projections of the same
-// list (every OSEM iteration, every benchmark step) skip the probe launch, which would otherwise sit in front of the
-// tile kernel on the stream.  Only the ADDRESS is remembered, nothing is dereferenced later; a stale hit (another
-// list at the same address) can only cost speed, never correctness: both instantiations read the same int, and
-// any track length partitions the list.  Events order the int between streams: `ready` after the probe, `used`
-// after the last kernels that read it (an entry is recycled only behind that event).
-struct ProbeEntry {
-    int dev = -1;
-    const void *key = nullptr;
-    int64_t n = 0;
-    int *cut = nullptr;
-    cudaEvent_t ready = nullptr, used = nullptr;
-    unsigned long long stamp = 0;
-};
-static std::mutex g_probe_mu;
-static ProbeEntry g_probe[16];
-static unsigned long long g_probe_clock = 0;
-
-static cudaError_t probe_tracks(const Lors &l, int64_t n, cudaStream_t st, int **out, cudaEvent_t *used)
-{
-    *out = nullptr;
-    *used = nullptr;
-    if (n < 8 * kTile) return cudaSuccess;
-    const char *env = getenv("JP_TRACK_PROBE"); // JP_TRACK_PROBE=0: assume aligned tracks (A/B measurements)
-    if (env && env[0] == '0') return cudaSuccess;
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone)
-        return cudaSuccess; // inside a graph capture: no allocation, no cross-stream events -- plain tiles (always correct)
-    std::lock_guard<std::mutex> lock(g_probe_mu);
-    ProbeEntry *hit = nullptr, *lru = &g_probe[0];
-    for (ProbeEntry &p : g_probe) {
-        if (p.cut && p.dev == dev && p.key == (const void *)l.xs && p.n == n) hit = &p;
-        if (p.stamp < lru->stamp) lru = &p;
-    }
-    if (hit) {
-        hit->stamp = ++g_probe_clock;
-        if ((e = cudaStreamWaitEvent(st, hit->ready, 0)) != cudaSuccess) return e;
-        // chain the users of an entry (a no-op on the same stream), so that `used` always covers all of them
-        if ((e = cudaStreamWaitEvent(st, hit->used, 0)) != cudaSuccess) return e;
-        *out = hit->cut;
-        *used = hit->used;
-        return cudaSuccess;
-    }
-    ProbeEntry &p = *lru;
-    if (!p.cut || p.dev != dev) { // first use of the slot (or another device: the old int is left to that device)
-        p = ProbeEntry{};
-        if ((e = cudaMalloc((void **)&p.cut, sizeof(int))) != cudaSuccess) return e;
-        if ((e = cudaEventCreateWithFlags(&p.ready, cudaEventDisableTiming)) != cudaSuccess) return e;
-        if ((e = cudaEventCreateWithFlags(&p.used, cudaEventDisableTiming)) != cudaSuccess) return e;
-    } else if ((e = cudaStreamWaitEvent(st, p.used, 0)) != cudaSuccess) { // kernels of the evicted list may still read it
-        return e;
-    }
-    p.dev = dev;
-    p.key = (const void *)l.xs;
-    p.n = n;
-    p.stamp = ++g_probe_clock;
-    k_track_probe<<<1, 1024, 0, st>>>(l, n, p.cut);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    if ((e = cudaEventRecord(p.ready, st)) != cudaSuccess) return e;
-    *out = p.cut;
-    *used = p.used;
-    return cudaSuccess;
-}
-
-static unsigned persistent_grid(int per_sm)
-{
-    int dev = 0, nsm = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    return (unsigned)(nsm > 0 ? nsm * per_sm : 148 * per_sm);
-}
-
-cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st)
+// pv == null (or an irregular plan): tiles of 768 consecutive LORs of `l`; a regular plan: tiles per track, `l` unused.
+// lane_map = 0 switches the lane mapping off (a performance hint only; the results are the same)
+cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Geom &g, float *p, cudaStream_t st,
+                            const SinoPlanView *pv, int lane_map)
 {
     if (n == 0) return cudaSuccess;
+    const bool plan = pv && pv->regular;
     const TileCfg c = tile_cfg(g, img, sizeof(float2), JP_SMEM_KB_FWD * 1024);
-    if (!c.P) return launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
-    const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
-    int *cut = nullptr;
-    cudaEvent_t used = nullptr;
-    cudaError_t e = probe_tracks(l, n, st, &cut, &used);
-    if (e != cudaSuccess) return e;
+    const PlanSrc ps = plan_src(pv);
+    if (!c.P) return plan ? cudaErrorNotSupported : launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
+    const int64_t tiles = plan ? pv->K * ps.tpt : (n + kTile - 1) / kTile;
+    if (tiles >= ((int64_t)1 << 31)) return cudaErrorInvalidValue;
+    cudaError_t e = cudaSuccess;
     JP_DISPATCH_P(c, {
-        e = set_smem(k_fwd_tile<P>, c.smem);
-        if (e == cudaSuccess && cut) e = set_smem(k_fwd_tile_cut<P, true>, c.smem);
-        if (e == cudaSuccess) {
-            k_fwd_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok, lane_map_on(), cut, p);
-            if (cut)
-                k_fwd_tile_cut<P, true><<<persistent_grid(JP_MINB_FWD), kThreads, c.smem, st>>>(l, n, img, g, c.rows_cap, c.vec_ok,
-                                                                                         lane_map_on(), cut, p);
+        if (plan) {
+            e = set_smem(k_fwd_tile<P, true>);
+            if (e == cudaSuccess)
+                k_fwd_tile<P, true><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, img, g, c.rows_cap, c.vec_ok, lane_map, p);
+        } else {
+            e = set_smem(k_fwd_tile<P, false>);
+            if (e == cudaSuccess)
+                k_fwd_tile<P, false><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, img, g, c.rows_cap, c.vec_ok, lane_map, p);
         }
     })
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (used && e == cudaSuccess) e = cudaEventRecord(used, st);
     return e;
 }
 
-cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st)
+cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geom &g, float *img, cudaStream_t st,
+                             const SinoPlanView *pv, int lane_map)
 {
     if (n == 0) return cudaSuccess;
+    const bool plan = pv && pv->regular;
     const TileCfg c = tile_cfg(g, img, sizeof(int), JP_SMEM_KB_BACK * 1024);
-    if (!c.P) return launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);
-    const unsigned grid = (unsigned)((n + kTile - 1) / kTile);
-    int *cut = nullptr;
-    cudaEvent_t used = nullptr;
-    cudaError_t e = probe_tracks(l, n, st, &cut, &used);
-    if (e != cudaSuccess) return e;
+    const PlanSrc ps = plan_src(pv);
+    if (!c.P) return plan ? cudaErrorNotSupported : launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);
+    const int64_t tiles = plan ? pv->K * ps.tpt : (n + kTile - 1) / kTile;
+    if (tiles >= ((int64_t)1 << 31)) return cudaErrorInvalidValue;
+    cudaError_t e = cudaSuccess;
     JP_DISPATCH_P(c, {
-        e = set_smem(k_back_tile<P>, c.smem);
-        if (e == cudaSuccess && cut) e = set_smem(k_back_tile_cut<P, true>, c.smem);
-        if (e == cudaSuccess) {
-            k_back_tile<P><<<grid, kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok, lane_map_on(), cut, img);
-            if (cut)
-                k_back_tile_cut<P, true><<<persistent_grid(JP_MINB_BACK), kThreads, c.smem, st>>>(l, n, y, g, c.rows_cap, c.vec_ok,
-                                                                                           lane_map_on(), cut, img);
+        if (plan) {
+            e = set_smem(k_back_tile<P, true>);
+            if (e == cudaSuccess)
+                k_back_tile<P, true><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, y, g, c.rows_cap, c.vec_ok, lane_map, img);
+        } else {
+            e = set_smem(k_back_tile<P, false>);
+            if (e == cudaSuccess)
+                k_back_tile<P, false><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, y, g, c.rows_cap, c.vec_ok, lane_map, img);
         }
     })
     if (e == cudaSuccess) e = cudaGetLastError();
-    if (used && e == cudaSuccess) e = cudaEventRecord(used, st);
     return e;
 }
 
