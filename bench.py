@@ -492,30 +492,30 @@ class Workload:
 
     # ---- end to end with HOST buffers: H2D of the step's inputs, the calls, D2H of the results, all timed ------
     def e2e_setup(self):
+        """host-side copies of the step's inputs in pinned memory + the hybrid handle (jp_hybrid over this rank's GPU)"""
         jp, c = self.jp, self.c
         pin = lambda t: t.cpu().pin_memory()
+        nvox = int(np.prod(self.g.n))
+        self.hyb = jp.Hybrid([self.dev.index if self.dev.index is not None else 0]) if c < 4 else None
         if c in (0, 1):
-            nvox = int(np.prod(self.g.n))
             self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
                           p=torch.empty(self.n, dtype=torch.float32).pin_memory(),
                           b=torch.zeros(self.g.n, dtype=torch.float32).pin_memory())
-            self.e2e_api = "jp_fwd_host + jp_back_host (pinned host tensors)"
-            self.h2d, self.d2h = 2 * 24 * self.n + 4 * self.n + 2 * 4 * nvox, 4 * self.n + 4 * nvox
+            self.e2e_api = "jp_hybrid_set_lors + jp_hybrid_fwd + jp_hybrid_back (pinned host tensors; the LOR list is uploaded once per step)"
+            self.h2d, self.d2h = 24 * self.n + 4 * self.n + 4 * nvox, 4 * self.n + 4 * nvox
         elif c == 2:
             self.h = dict(xs=pin(self.xs), xe=pin(self.xe), y=pin(self.y), img=pin(self.img),
                           p=torch.empty_like(self.p, device="cpu").pin_memory(),
                           b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
-            self.e2e_api = ("pinned host -> device copies, jp_sino_plan_create, jp_fwd_tof_sino_planned + "
-                            "jp_back_tof_sino_planned, device -> pinned host" if self.splan is not None else
-                            "pinned host -> device copies, jp_fwd_tof_sino + jp_back_tof_sino, device -> pinned host")
+            self.e2e_api = "jp_hybrid_set_lors + jp_hybrid_fwd_tof_sino + jp_hybrid_back_tof_sino (pinned host tensors)"
             self.h2d = 24 * self.n + 4 * self.y.numel() + 4 * NVOX
             self.d2h = 4 * self.p.numel() + 4 * NVOX
         elif c == 3:
             self.h = dict(xs=pin(self.xs), xe=pin(self.xe), tb=pin(self.tb), y=pin(self.y), img=pin(self.img),
                           p=torch.empty(self.n, dtype=torch.float32).pin_memory(),
                           b=torch.zeros(G.n, dtype=torch.float32).pin_memory())
-            self.e2e_api = ("pinned host -> device copies of the events, jp_lm_plan_create, jp_fwd_tof_lm_planned + "
-                            "jp_back_tof_lm_planned, device -> pinned host")
+            self.e2e_api = ("jp_hybrid_set_lors (events + TOF bins, builds the listmode plan) + jp_hybrid_fwd_tof_lm + "
+                            "jp_hybrid_back_tof_lm (pinned host tensors)")
             self.h2d = 26 * self.n + 4 * self.n + 4 * NVOX
             self.d2h = 4 * self.n + 4 * NVOX
         else:
@@ -528,48 +528,49 @@ class Workload:
             self.d2h = 4 * NVOX
 
     def e2e_step(self):
-        jp, c, h = self.jp, self.c, self.h
-        if c in (0, 1):
-            jp.jp_fwd_host(h["xs"], h["xe"], h["img"], self.g.origin, self.g.voxsize, out=h["p"])
+        jp, c, h, g = self.jp, self.c, self.h, self.g
+        if c < 4:
+            hy = self.hyb
             h["b"].zero_()
-            jp.jp_back_host(h["xs"], h["xe"], h["y"], h["b"], self.g.origin, self.g.voxsize)
+            if c in (0, 1):
+                hy.set_lors(h["xs"], h["xe"])
+                hy.fwd(h["img"], g.origin, g.voxsize, out=h["p"])
+                hy.back(h["y"], h["b"], g.origin, g.voxsize)
+            elif c == 2:
+                hy.set_lors(h["xs"], h["xe"])
+                hy.fwd_tof_sino(h["img"], g.origin, g.voxsize, self.tof, out=h["p"])
+                hy.back_tof_sino(h["y"], h["b"], g.origin, g.voxsize, self.tof)
+            else:
+                hy.set_lors(h["xs"], h["xe"], h["tb"], g.n, g.origin, g.voxsize, self.tof)
+                hy.fwd_tof_lm(h["img"], out=h["p"])
+                hy.back_tof_lm(h["y"], h["b"])
             return
         self.xs.copy_(h["xs"], non_blocking=True)
         self.xe.copy_(h["xe"], non_blocking=True)
-        if c == 2:
-            self.img.copy_(h["img"], non_blocking=True)
-            self.y.copy_(h["y"], non_blocking=True)
-            old = self.splan
-            if old is not None:      # the plan is part of the step: it is made from the end points just uploaded
-                self.splan = self.jp.SinoPlan(self.xs, self.xe)
-            self.step()
-            if old is not None:
-                torch.cuda.synchronize()
-                self.splan.destroy()
-                self.splan = old
-        else:
-            self.tb.copy_(h["tb"], non_blocking=True)
-            plan = self.jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof, n_subsets=20)
-            old, self.plan = self.plan, plan
-            if c == 3:
-                self.img.copy_(h["img"], non_blocking=True)
-                self.y.copy_(h["y"], non_blocking=True)
-            else:
-                self.sens.copy_(h["sens"], non_blocking=True)
-                self.x.copy_(h["x"], non_blocking=True)
-            self.step()
-            torch.cuda.synchronize()
-            self.plan = old
-            plan.destroy()
-        if c == 4:
-            h["xo"].copy_(self.x, non_blocking=True)
-        else:
-            h["p"].copy_(self.p, non_blocking=True)
-            h["b"].copy_(self.bimg, non_blocking=True)
+        self.tb.copy_(h["tb"], non_blocking=True)
+        plan = self.jp.LmPlan(self.xs, self.xe, self.tb, G.n, G.origin, G.voxsize, self.tof, n_subsets=20)
+        old, self.plan = self.plan, plan
+        self.sens.copy_(h["sens"], non_blocking=True)
+        self.x.copy_(h["x"], non_blocking=True)
+        self.step()
+        torch.cuda.synchronize()
+        self.plan = old
+        plan.destroy()
+        h["xo"].copy_(self.x, non_blocking=True)
         torch.cuda.synchronize()
 
+    def e2e_check(self):
+        """the e2e results must be the step's results (a copy that silently failed would leave the buffers untouched)"""
+        if self.c >= 4:
+            return True
+        p, b = self.h["p"].to(self.dev).reshape(-1), self.h["b"].to(self.dev)
+        self.step()
+        torch.cuda.synchronize()
+        ok_p = float((p - self.p.reshape(-1)).abs().max()) <= 2e-5 * float(self.p.abs().max())
+        ok_b = float((b - self.bimg).abs().max()) <= 1e-4 * float(self.bimg.abs().max())
+        return bool(ok_p and ok_b)
 
-# ---- --check: the float64 oracle on the FULL config against the CUDA results (outside every timed region) -----------
+
 def check_parity(w: Workload):
     """parity of the workload's CUDA results against the oracle run on the whole config on the host cores:
     forward rel-L2 and max-abs / max|oracle| over ALL outputs, back projection max-abs / max|oracle| over ALL voxels
@@ -766,7 +767,10 @@ def run_ours(args):
             w.e2e_step()
         barrier()
         e2e_s = (time.perf_counter() - t0) / ne2e
+        e2e_ok = w.e2e_check()
         w.h = None
+        if getattr(w, "hyb", None) is not None:
+            w.hyb.destroy()
 
     if world > 1:
         t = torch.tensor([total_ms, fwd_ms, back_ms, e2e_s or 0.0], device=dev, dtype=torch.float64)
@@ -812,7 +816,8 @@ def run_ours(args):
         line["s_per_iteration_with_resolution_model"] = w.time_osem_with_resolution_model()
     if e2e_s is not None:
         line["e2e"] = {"value": world * w.n / e2e_s, "unit": SPEC[c]["unit"], "h2d_bytes_per_step": w.h2d,
-                       "d2h_bytes_per_step": w.d2h, "ms_per_step": e2e_s * 1e3, "api": w.e2e_api}
+                       "d2h_bytes_per_step": w.d2h, "ms_per_step": e2e_s * 1e3, "api": w.e2e_api,
+                       "results_match_device_step": e2e_ok}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline_dict(c, time_oracle(c, 1, 0))
     if args.check and world == 1:

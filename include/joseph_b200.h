@@ -146,12 +146,21 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
  * per-event arrays in CALLER order.
  *   events, tofbin: device arrays, only read during jp_lm_plan_create (not kept).
  *   The plan owns its device buffers (26 + 4 bytes per event) until jp_lm_plan_destroy.
- *   jp_lm_plan_create is asynchronous on `stream` except for its device allocations (cudaMalloc);
+ *   jp_lm_plan_create allocates with cudaMalloc and SYNCHRONISES `stream` twice (it reads the per-subset / per-axis
+ *   event counts and the run statistics back to the host); the planned calls are asynchronous.  A plan keeps
+ *   image-sized scratch (quad image and accumulators, allocated with cudaMalloc on the first call that needs them)
+ *   that the planned calls write: use a plan from ONE stream at a time.
  *   n_subsets in 1..255, fewer than 2^31 events.  subset = -1 in the calls below means all events. */
 typedef struct jp_plan jp_plan;
 int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
                       int n_subsets, void *stream, jp_plan **plan);
 int jp_lm_plan_destroy(jp_plan *plan);
+/* Which kernels the planned listmode projectors use: 0 = chosen from the plan's run statistics (default: line tiles
+ * when the sorted events come in runs of >= 512 on one transaxial line, else the quad image), 1 = line tiles,
+ * 2 = quad image / per-event kernels.  All paths compute the same projections (tests force each of them); images or
+ * TOF kernels too wide for the line tiles take path 2 whatever is asked.  Not to be changed while a call that uses the
+ * plan is being issued from another thread. */
+int jp_lm_plan_set_path(jp_plan *plan, int path);
 /* number of events of a subset (subset = -1: all); -1 for an invalid plan or subset */
 int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset);
 /* p[e] for the events e of the subset (other entries of p are left untouched); p has n entries */
@@ -262,15 +271,40 @@ int jp_sino_osem_tof_planned(const jp_plan *plan, const int64_t *subset_offsets,
                              const float *mult, const float *contam, const float *sens, const jp_geom *geom,
                              const jp_tof *tof, float *img, int n_iter, void *workspace, size_t workspace_bytes, void *stream);
 
-/* ---- hybrid mode: HOST pointers in and out ---------------------------------------- */
-/* Same semantics as jp_fwd / jp_back, but every pointer (inside lors_host too) is a HOST pointer.  The
- * LOR list is streamed through the current CUDA device in chunks on two internal streams (copies
- * overlap kernels when the host memory is page-locked).  Allocates and frees its own device staging.
- * Returns after the result is in host memory.  jp_back_host ACCUMULATES into img_host. */
+/* ---- hybrid mode: HOST pointers in and out, over all visible GPUs --------------------------- */
+/* "data transfer from the host to all available GPUs, execution of projection kernels on the GPUs, and transfer of
+ * the results back".  A jp_hybrid handle owns one worker per device it was created over (a host thread
+ * per call, a CUDA stream, device buffers that are KEPT between calls and freed with the handle).
+ *   devices   ordinals of the devices to use, n_devices of them; NULL = all visible devices.  A device may be listed
+ *             more than once (several workers on one GPU).
+ *   jp_hybrid_set_lors  splits the HOST LOR list into one contiguous shard per worker (cut at multiples of the list's
+ *             track length when it has one, and of 768 LORs), uploads every shard ONCE and builds the shard's plan: a
+ *             sinogram plan, or, when tofbin_host is given, a listmode plan (then geom and tof are required; they are
+ *             the geometry / TOF model of the later jp_hybrid_*_tof_lm calls).  The host arrays are not kept.
+ *   projection calls    move only what changes: the image to every GPU, the per-LOR values of each shard, the results
+ *             back.  Forward results are disjoint; a back projection sums the workers' partial images on the host in
+ *             worker order and ACCUMULATES the sum into img_host.  Same per-LOR arithmetic as the device calls.
+ * All jp_hybrid_* calls return after their result is in host memory (they synchronise their own streams only), may
+ * allocate device and pinned host memory, and do not change the calling thread's current device.  One call at a
+ * time per handle.  Page-locked host arrays make the copies faster; pageable ones work. */
+typedef struct jp_hybrid jp_hybrid;
+int jp_hybrid_create(const int *devices, int n_devices, jp_hybrid **handle);
+int jp_hybrid_destroy(jp_hybrid *handle);
+int jp_hybrid_worker_count(const jp_hybrid *handle); /* -1 for NULL */
+int jp_hybrid_set_lors(jp_hybrid *handle, const jp_lors *lors_host, const int16_t *tofbin_host /* or NULL */,
+                       const jp_geom *geom /* with tofbin_host */, const jp_tof *tof /* with tofbin_host */);
+int jp_hybrid_fwd(jp_hybrid *handle, const float *img_host, const jp_geom *geom, float *p_host);
+int jp_hybrid_back(jp_hybrid *handle, const float *y_host, const jp_geom *geom, float *img_host);
+int jp_hybrid_fwd_tof_sino(jp_hybrid *handle, const float *img_host, const jp_geom *geom, const jp_tof *tof, float *p_host);
+int jp_hybrid_back_tof_sino(jp_hybrid *handle, const float *y_host, const jp_geom *geom, const jp_tof *tof, float *img_host);
+int jp_hybrid_fwd_tof_lm(jp_hybrid *handle, const float *img_host, float *p_host);
+int jp_hybrid_back_tof_lm(jp_hybrid *handle, const float *y_host, float *img_host);
+
+/* One-shot forms (same semantics as jp_fwd / jp_back / ..., every pointer -- inside lors_host too -- a HOST pointer):
+ * each makes a handle over all visible devices, sets the list, projects and destroys the handle.  jp_back*_host
+ * ACCUMULATE into img_host.  Callers that project a list more than once should keep a handle instead. */
 int jp_fwd_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, float *p_host);
 int jp_back_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, float *img_host);
-/* the TOF projectors in hybrid mode (same semantics as jp_fwd/back_tof_sino and the unplanned jp_fwd/back_tof_lm;
- * p_host / y_host: [n][n_tofbins] resp. [n]; tofbin_host: [n] int16; the back projections ACCUMULATE into img_host) */
 int jp_fwd_tof_sino_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, const jp_tof *tof,
                          float *p_host);
 int jp_back_tof_sino_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, const jp_tof *tof,

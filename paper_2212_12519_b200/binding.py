@@ -62,6 +62,7 @@ EXPORTS = {
                                     C.c_void_p, C.POINTER(C.c_void_p)]),
     "jp_lm_plan_destroy": (C.c_int, [C.c_void_p]),
     "jp_lm_plan_subset_count": (C.c_int64, [C.c_void_p, C.c_int]),
+    "jp_lm_plan_set_path": (C.c_int, [C.c_void_p, C.c_int]),
     "jp_fwd_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_back_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_fwd_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -95,6 +96,16 @@ EXPORTS = {
     "jp_sino_osem_tof_planned": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p, C.c_int,
                                            C.c_void_p, C.c_size_t, C.c_void_p]),
+    "jp_hybrid_create": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_void_p)]),
+    "jp_hybrid_destroy": (C.c_int, [C.c_void_p]),
+    "jp_hybrid_worker_count": (C.c_int, [C.c_void_p]),
+    "jp_hybrid_set_lors": (C.c_int, [C.c_void_p, C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof)]),
+    "jp_hybrid_fwd": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
+    "jp_hybrid_back": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
+    "jp_hybrid_fwd_tof_sino": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p]),
+    "jp_hybrid_back_tof_sino": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p]),
+    "jp_hybrid_fwd_tof_lm": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_hybrid_back_tof_lm": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_fwd_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_back_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.c_void_p]),
     "jp_fwd_tof_sino_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof), C.c_void_p]),
@@ -341,6 +352,11 @@ class LmPlan:
 
     def subset_count(self, subset: int = -1) -> int:
         return int(load().jp_lm_plan_subset_count(self.handle, int(subset)))
+
+    def set_path(self, path: int):
+        """0: automatic, 1: line tiles, 2: quad image / per-event kernels (jp_lm_plan_set_path)"""
+        _check(load().jp_lm_plan_set_path(self.handle, int(path)), "jp_lm_plan_set_path")
+        return self
 
     def destroy(self):
         if self.handle is not None and self.handle.value:
@@ -653,6 +669,101 @@ def _host_lors(xstart: torch.Tensor, xend: torch.Tensor):
             raise JosephError("host end points must be CPU float32 tensors of shape (3, n)")
     rows = [t[a] if t[a].is_contiguous() else t[a].contiguous() for t in (xstart, xend) for a in range(3)]
     return jp_lors(*[r.data_ptr() for r in rows], int(xstart.shape[1])), rows
+
+
+class Hybrid:
+    """Owner of a jp_hybrid handle: host tensors in and out, the work split over the handle's devices.
+    ``devices``: list of CUDA ordinals (None: all visible; an ordinal may repeat: several workers on one GPU)."""
+
+    def __init__(self, devices=None):
+        h = C.c_void_p()
+        if devices is None:
+            rc = load().jp_hybrid_create(None, 0, C.byref(h))
+        else:
+            arr = (C.c_int * len(devices))(*[int(d) for d in devices])
+            rc = load().jp_hybrid_create(arr, len(devices), C.byref(h))
+        _check(rc, "jp_hybrid_create")
+        self.handle = h
+        self.n = 0
+        self.shape = None
+
+    @property
+    def workers(self) -> int:
+        return int(load().jp_hybrid_worker_count(self.handle))
+
+    def set_lors(self, xstart, xend, tofbin=None, n=None, origin=None, voxsize=None, tof: jp_tof = None):
+        l, keep = _host_lors(xstart, xend)
+        self.n = int(l.n)
+        if tofbin is None:
+            _check(load().jp_hybrid_set_lors(self.handle, C.byref(l), None, None, None), "jp_hybrid_set_lors")
+        else:
+            _host_bins(tofbin, l.n)
+            self.shape = tuple(int(x) for x in n)
+            g = make_geom(self.shape, origin, voxsize)
+            _check(load().jp_hybrid_set_lors(self.handle, C.byref(l), tofbin.data_ptr(), C.byref(g), C.byref(tof)),
+                   "jp_hybrid_set_lors")
+        return self
+
+    def fwd(self, img, origin, voxsize, out=None):
+        img = _host_f32(img, "img")
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float32)
+        _host_f32(out, "out", self.n)
+        g = make_geom(img.shape, origin, voxsize)
+        _check(load().jp_hybrid_fwd(self.handle, img.data_ptr(), C.byref(g), out.data_ptr()), "jp_hybrid_fwd")
+        return out
+
+    def back(self, y, img, origin, voxsize):
+        _host_f32(y, "y", self.n)
+        img = _host_f32(img, "img")
+        g = make_geom(img.shape, origin, voxsize)
+        _check(load().jp_hybrid_back(self.handle, y.data_ptr(), C.byref(g), img.data_ptr()), "jp_hybrid_back")
+        return img
+
+    def fwd_tof_sino(self, img, origin, voxsize, tof: jp_tof, out=None):
+        img = _host_f32(img, "img")
+        if out is None:
+            out = torch.empty((self.n, int(tof.n_tofbins)), dtype=torch.float32)
+        _host_f32(out, "out", self.n * int(tof.n_tofbins))
+        g = make_geom(img.shape, origin, voxsize)
+        _check(load().jp_hybrid_fwd_tof_sino(self.handle, img.data_ptr(), C.byref(g), C.byref(tof), out.data_ptr()),
+               "jp_hybrid_fwd_tof_sino")
+        return out
+
+    def back_tof_sino(self, y, img, origin, voxsize, tof: jp_tof):
+        _host_f32(y, "y", self.n * int(tof.n_tofbins))
+        img = _host_f32(img, "img")
+        g = make_geom(img.shape, origin, voxsize)
+        _check(load().jp_hybrid_back_tof_sino(self.handle, y.data_ptr(), C.byref(g), C.byref(tof), img.data_ptr()),
+               "jp_hybrid_back_tof_sino")
+        return img
+
+    def fwd_tof_lm(self, img, out=None):
+        img = _host_f32(img, "img")
+        assert tuple(img.shape) == self.shape
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float32)
+        _host_f32(out, "out", self.n)
+        _check(load().jp_hybrid_fwd_tof_lm(self.handle, img.data_ptr(), out.data_ptr()), "jp_hybrid_fwd_tof_lm")
+        return out
+
+    def back_tof_lm(self, y, img):
+        _host_f32(y, "y", self.n)
+        img = _host_f32(img, "img")
+        assert tuple(img.shape) == self.shape
+        _check(load().jp_hybrid_back_tof_lm(self.handle, y.data_ptr(), img.data_ptr()), "jp_hybrid_back_tof_lm")
+        return img
+
+    def destroy(self):
+        if self.handle is not None and self.handle.value:
+            _check(load().jp_hybrid_destroy(self.handle), "jp_hybrid_destroy")
+        self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
 
 def jp_fwd_host(xstart, xend, img, origin, voxsize, out=None) -> torch.Tensor:

@@ -389,6 +389,15 @@ int jp_plan_destroy(jp_plan *plan)
 
 int jp_lm_plan_destroy(jp_plan *plan) { return jp_plan_destroy(plan); }
 
+int jp_lm_plan_set_path(jp_plan *plan, int path)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "not a listmode plan");
+    if (path < 0 || path > 2) return fail(JP_ERR_SIZE, "path must be 0 (automatic), 1 (line tiles) or 2 (quad image)");
+    jp::lm_plan_set_path(plan->lm, path);
+    return JP_OK;
+}
+
 int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset)
 {
     if (!plan || !plan->lm) return -1;
@@ -405,11 +414,14 @@ namespace {
 
 // line tiles (jp_lm_tile.cu) pay when the sorted events come in long runs on one transaxial line (crystal-snapped
 // events, all subsets together: ~2500 per run for configs[3]); short runs (one OSEM subset of 20: ~120) are
-// faster on the quad image.  JP_LM_TILE=0/1 overrides the rule (debugging, tests).
-bool lm_tiles_wanted(const jp::LmPlan *lm)
+// faster on the quad image.  jp_lm_plan_set_path overrides the rule; images / TOF kernels the tiles cannot hold
+// always take the other paths.
+bool lm_tiles_wanted(const jp::LmPlan *lm, bool tof)
 {
-    const char *e = getenv("JP_LM_TILE");
-    if (e && (e[0] == '0' || e[0] == '1')) return e[0] == '1';
+    if (!jp::lm_tile_supported(jp::lm_plan_geom(lm), jp::lm_plan_tof(lm), tof)) return false;
+    const int path = jp::lm_plan_path(lm);
+    if (path == 1) return true;
+    if (path == 2) return false;
     const int64_t runs = jp::lm_plan_runs(lm);
     return runs > 0 && jp::lm_plan_n(lm) / runs >= 512;
 }
@@ -453,6 +465,90 @@ struct PlanCtx {
 
 } // namespace
 
+} // extern "C"
+
+// the planned TOF listmode projectors as internal calls (also used by the hybrid handle, jp_host.cu)
+namespace jp {
+
+#define JP_E(x)                           \
+    do {                                  \
+        const cudaError_t e__ = (x);      \
+        if (e__ != cudaSuccess) return e__; \
+    } while (0)
+
+cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, cudaStream_t st)
+{
+    jp_plan tmp;
+    tmp.lm = lm;
+    PlanCtx c(&tmp);
+    TofCtx tc;
+    tc.st = st;
+    JP_E(jp::tof_lut_create(c.t, st, &tc.lut));
+    float4 *q[2];
+    JP_E(jp::lm_plan_quad(c.lm, 0, &q[0]));
+    JP_E(jp::lm_plan_quad(c.lm, 1, &q[1]));
+    const bool tiles = lm_tiles_wanted(c.lm, true);
+    if (!tiles) JP_E(jp::launch_quad_build(img, c.g, q[0], q[1], st));
+    for (int a = 0; a < 2; ++a)
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset) {
+                const jp::Range rg = c.seg(m, a, false);
+                if (tiles)
+                    JP_E(jp::launch_fwd_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, img, c.g, c.t, p, 0, st));
+                else
+                    JP_E(jp::launch_fwd_tof_lm_quad(c.l, c.tb, rg, q[a], c.g, c.t, tc.lut, p, 0, st));
+            }
+    if (c.has_axis2(subset)) { // principal axis z: per-LOR kernels on the padded scalar image
+        JP_E(jp::padded_create(img, c.g, false, st, &tc.pimg));
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_E(jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, false), tc.pimg, c.g, c.t, tc.lut, p, 0, st));
+    }
+    return cudaSuccess;
+}
+
+cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img, cudaStream_t st)
+{
+    jp_plan tmp;
+    tmp.lm = lm;
+    PlanCtx c(&tmp);
+    TofCtx tc;
+    tc.st = st;
+    JP_E(jp::tof_lut_create(c.t, st, &tc.lut));
+    if (lm_tiles_wanted(c.lm, true)) {
+        for (int a = 0; a < 2; ++a)
+            for (int m = 0; m < c.ns; ++m)
+                if (subset < 0 || m == subset) {
+                    const jp::Range rg = c.seg(m, a, false);
+                    JP_E(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, y, c.g, c.t, img, st));
+                }
+    } else {
+        float4 *b[2];
+        const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+        for (int a = 0; a < 2; ++a) {
+            JP_E(jp::lm_plan_quad(c.lm, 2 + a, &b[a]));
+            JP_E(cudaMemsetAsync(b[a], 0, qbytes, st));
+            for (int m = 0; m < c.ns; ++m)
+                if (subset < 0 || m == subset)
+                    JP_E(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), y, c.g, c.t, tc.lut, b[a], st));
+        }
+        JP_E(jp::launch_quad_merge(b[0], b[1], c.g, img, st));
+    }
+    if (c.has_axis2(subset)) {
+        JP_E(jp::padded_create(nullptr, c.g, true, st, &tc.pimg));
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_E(jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, false), y, c.g, c.t, tc.lut, tc.pimg, st));
+        JP_E(jp::padded_add_to(tc.pimg, c.g, img, st));
+    }
+    return cudaSuccess;
+}
+#undef JP_E
+
+} // namespace jp
+
+extern "C" {
+
 int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream)
 {
     g_err[0] = 0;
@@ -460,32 +556,7 @@ int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, flo
     if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
     if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
     if (!img || !p) return fail(JP_ERR_POINTER, "img or p is NULL");
-    const char *where = "jp_fwd_tof_lm_planned";
-    cudaStream_t st = (cudaStream_t)stream;
-    PlanCtx c(plan);
-    TofCtx tc;
-    tc.st = st;
-    JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
-    float4 *q[2];
-    JP_CUDA(jp::lm_plan_quad(c.lm, 0, &q[0]), where);
-    JP_CUDA(jp::lm_plan_quad(c.lm, 1, &q[1]), where);
-    const bool tiles = lm_tiles_wanted(c.lm);
-    if (!tiles) JP_CUDA(jp::launch_quad_build(img, c.g, q[0], q[1], st), where);
-    for (int a = 0; a < 2; ++a)
-        for (int m = 0; m < c.ns; ++m)
-            if (subset < 0 || m == subset) {
-                const jp::Range rg = c.seg(m, a, false);
-                if (tiles)
-                    JP_CUDA(jp::launch_fwd_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, img, c.g, c.t, p, 0, st), where);
-                else
-                    JP_CUDA(jp::launch_fwd_tof_lm_quad(c.l, c.tb, rg, q[a], c.g, c.t, tc.lut, p, 0, st), where);
-            }
-    if (c.has_axis2(subset)) { // principal axis z: per-LOR kernels on the padded scalar image
-        JP_CUDA(jp::padded_create(img, c.g, false, st, &tc.pimg), where);
-        for (int m = 0; m < c.ns; ++m)
-            if (subset < 0 || m == subset)
-                JP_CUDA(jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, false), tc.pimg, c.g, c.t, tc.lut, p, 0, st), where);
-    }
+    JP_CUDA(jp::lm_plan_fwd_tof(plan->lm, subset, img, p, (cudaStream_t)stream), "jp_fwd_tof_lm_planned");
     return JP_OK;
 }
 
@@ -496,38 +567,7 @@ int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, floa
     if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
     if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
     if (!img || !y) return fail(JP_ERR_POINTER, "img or y is NULL");
-    const char *where = "jp_back_tof_lm_planned";
-    cudaStream_t st = (cudaStream_t)stream;
-    PlanCtx c(plan);
-    TofCtx tc;
-    tc.st = st;
-    JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
-    if (lm_tiles_wanted(c.lm)) {
-        for (int a = 0; a < 2; ++a)
-            for (int m = 0; m < c.ns; ++m)
-                if (subset < 0 || m == subset) {
-                    const jp::Range rg = c.seg(m, a, false);
-                    JP_CUDA(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, y, c.g, c.t, img, st), where);
-                }
-    } else {
-        float4 *b[2];
-        const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
-        for (int a = 0; a < 2; ++a) {
-            JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
-            JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
-            for (int m = 0; m < c.ns; ++m)
-                if (subset < 0 || m == subset)
-                    JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), y, c.g, c.t, tc.lut, b[a], st), where);
-        }
-        JP_CUDA(jp::launch_quad_merge(b[0], b[1], c.g, img, st), where);
-    }
-    if (c.has_axis2(subset)) {
-        JP_CUDA(jp::padded_create(nullptr, c.g, true, st, &tc.pimg), where);
-        for (int m = 0; m < c.ns; ++m)
-            if (subset < 0 || m == subset)
-                JP_CUDA(jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, false), y, c.g, c.t, tc.lut, tc.pimg, st), where);
-        JP_CUDA(jp::padded_add_to(tc.pimg, c.g, img, st), where);
-    }
+    JP_CUDA(jp::lm_plan_back_tof(plan->lm, subset, y, img, (cudaStream_t)stream), "jp_back_tof_lm_planned");
     return JP_OK;
 }
 
@@ -542,7 +582,7 @@ int jp_fwd_lm_planned(const jp_plan *plan, int subset, const float *img, float *
     const char *where = "jp_fwd_lm_planned";
     cudaStream_t st = (cudaStream_t)stream;
     PlanCtx c(plan);
-    const bool tiles = lm_tiles_wanted(c.lm);
+    const bool tiles = lm_tiles_wanted(c.lm, false);
     for (int a = 0; a < 3; ++a)
         for (int m = 0; m < c.ns; ++m)
             if (subset < 0 || m == subset) {
@@ -566,7 +606,7 @@ int jp_back_lm_planned(const jp_plan *plan, int subset, const float *y, float *i
     const char *where = "jp_back_lm_planned";
     cudaStream_t st = (cudaStream_t)stream;
     PlanCtx c(plan);
-    const bool tiles = lm_tiles_wanted(c.lm);
+    const bool tiles = lm_tiles_wanted(c.lm, false);
     for (int a = 0; a < 3; ++a)
         for (int m = 0; m < c.ns; ++m)
             if (subset < 0 || m == subset) {

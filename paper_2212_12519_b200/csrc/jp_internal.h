@@ -115,6 +115,8 @@ cudaError_t launch_back_tof_lm_tile(const Lors &l, const int16_t *tofbin, int64_
                                     int64_t io_off, const float *y, const Geom &g, const Tof &t, float *img,
                                     cudaStream_t st);
 
+bool lm_tile_supported(const Geom &g, const Tof &t, bool tof);
+
 // listmode plan (jp_plan.cu)
 struct LmPlan;
 cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, const Geom &g, const Tof &t,
@@ -123,11 +125,16 @@ void lm_plan_destroy(LmPlan *pl);
 int64_t lm_plan_n(const LmPlan *pl);
 int64_t lm_plan_runs(const LmPlan *pl); // runs of sorted events sharing their transaxial line
 int lm_plan_subsets(const LmPlan *pl);
+int lm_plan_path(const LmPlan *pl);            // 0: chosen from the run statistics, 1: line tiles, 2: quad image
+void lm_plan_set_path(LmPlan *pl, int path);
 const Geom &lm_plan_geom(const LmPlan *pl);
 const Tof &lm_plan_tof(const LmPlan *pl);
 void lm_plan_view(const LmPlan *pl, int m, bool compact, Lors *l, const int16_t **tb, Range *rg);
 // events of subset m with principal axis a (a contiguous run of the sorted list): first index and count
 void lm_plan_segment(const LmPlan *pl, int m, int a, int64_t *first, int64_t *count);
+// the planned TOF listmode projectors (jp_api.cu), subset < 0: all events; p / y in caller order
+cudaError_t lm_plan_fwd_tof(LmPlan *pl, int subset, const float *img, float *p, cudaStream_t st);
+cudaError_t lm_plan_back_tof(LmPlan *pl, int subset, const float *y, float *img, cudaStream_t st);
 // persistent quad scratch of the plan (allocated on first use): which = 0,1: Q0,Q1; 2,3: B0,B1
 cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
 

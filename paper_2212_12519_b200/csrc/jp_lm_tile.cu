@@ -182,6 +182,7 @@ struct TileState {
     LineExtra ex;
     int nruns;
     int imin, imax;
+    int bad;        // adjoint kernel: the current run holds a non-finite value on an event that crosses the image
     unsigned short starts[kTile + 1];
     // forward kernel: the tracks of ALL long runs of the window, set up in parallel before the run loop
     Track trks[kMaxLong];
@@ -513,6 +514,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
             S.ex.Rd = 1.0 + ratio * ratio;
             S.imin = 0x7fffffff;
             S.imax = -1;
+            S.bad = 0;
         }
         __syncthreads();
         const Track trk = S.trk;
@@ -523,6 +525,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
         LmRay zr[kPerThread];
         float x[kPerThread];
         float xm_ = 0.f;
+        bool bad = false;
         {
             const double Rd = S.ex.Rd;
             int lo = 0x7fffffff, hi = -1;
@@ -544,6 +547,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
                     if (zr[m].i1 >= zr[m].i0 && x[m] != 0.f) {
                         lo = min(lo, zr[m].i0);
                         hi = max(hi, zr[m].i1);
+                        bad = bad || !(fabsf(x[m]) < 3.0e38f); // Inf or NaN (fmaxf would drop a NaN)
                         xm_ = fmaxf(xm_, fabsf(x[m]));
                     } else {
                         zr[m].i1 = zr[m].i0 - 1;
@@ -554,6 +558,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
                 atomicMin(&S.imin, lo);
                 atomicMax(&S.imax, hi);
             }
+            if (bad) atomicExch(&S.bad, 1);
         }
         for (int o = 16; o > 0; o >>= 1) xm_ = fmaxf(xm_, __shfl_xor_sync(0xffffffffu, xm_, o));
         if (lane == 0) red[warp] = xm_;
@@ -563,7 +568,17 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
 #pragma unroll
         for (int w = 1; w < kThreads / 32; ++w) xm_ = fmaxf(xm_, red[w]);
         const int I0 = S.imin, I1 = S.imax;
-        if (xm_ > 0.f && xm_ < 3.0e38f && I1 >= I0) {
+        if (S.bad) { // a non-finite value cannot be staged in fixed point: the run takes the per-LOR float path, so that
+                     // Inf / NaN propagate exactly as they do for events outside a line tile
+#pragma unroll 1
+            for (int m = 0; m < kPerThread; ++m)
+                if (active[m]) {
+                    const int64_t e = c0 + ra + m * kThreads + tid;
+                    const float yv = y[out_index(perm, io_off, first, e)];
+                    if (yv != 0.f)
+                        generic_back_lm<TOF>(l, e, TOF ? (float)tofbin[e] * t.width : 0.f, reach, yv, g, t, img, gbase, gt);
+                }
+        } else if (xm_ > 0.f && I1 >= I0) {
             const float lim = fminf(4194302.f, 2147483648.f / (float)(2 * kTile) - 1.f);
             const float Sc = lim / xm_, invS = xm_ / lim;
             for (int cc = I0; cc <= I1; cc += rows_cap) {
@@ -683,6 +698,18 @@ LmTileCfg lm_tile_cfg(const Geom &g, const Tof &t, const void *img, size_t elem,
     c.vec_ok = (g.n[2] % 4 == 0) && ((uintptr_t)img % 16 == 0);
     return c;
 }
+
+} // namespace
+
+// can the line-tile kernels take this image / TOF kernel at all?  (the planned calls use the quad or per-LOR path if not)
+bool lm_tile_supported(const Geom &g, const Tof &t_in, bool tof)
+{
+    const Tof t = tof ? t_in : Tof{1.f, 1.f, 1.f, 1, 0.f};
+    return lm_tile_cfg(g, t, nullptr, sizeof(float2), JP_LMT_SMEM_KB_FWD * 1024).P != 0 &&
+           lm_tile_cfg(g, t, nullptr, sizeof(int), JP_LMT_SMEM_KB_BACK * 1024).P != 0;
+}
+
+namespace {
 
 cudaError_t g1tab_create(const Tof &t, int n, cudaStream_t st, G1Tab *out)
 {

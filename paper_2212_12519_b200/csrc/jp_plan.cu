@@ -121,6 +121,7 @@ struct LmPlan {
     int64_t n = 0;
     int64_t n_runs = 0;     // runs of events sharing their transaxial line in the sorted list
     int n_subsets = 1;
+    int path = 0;           // 0: automatic, 1: line tiles, 2: quad image (jp_lm_plan_set_path)
     Geom g{};
     Tof t{};
     float *coord = nullptr; // 6 arrays of n floats: xs ys zs xe ye ze, sorted
@@ -248,6 +249,8 @@ cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out)
 int64_t lm_plan_n(const LmPlan *pl) { return pl->n; }
 int64_t lm_plan_runs(const LmPlan *pl) { return pl->n_runs; }
 int lm_plan_subsets(const LmPlan *pl) { return pl->n_subsets; }
+int lm_plan_path(const LmPlan *pl) { return pl->path; }
+void lm_plan_set_path(LmPlan *pl, int path) { pl->path = path; }
 const Geom &lm_plan_geom(const LmPlan *pl) { return pl->g; }
 const Tof &lm_plan_tof(const LmPlan *pl) { return pl->t; }
 

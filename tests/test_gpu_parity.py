@@ -310,9 +310,9 @@ def _line_events(seed=21):
 
 
 @pytest.mark.parametrize("n_subsets", [1, 3])
-def test_lm_line_tiles(cuda_device, scanner, n_subsets, monkeypatch):
-    """planned TOF listmode projectors on line tiles (runs of events sharing a transaxial line) vs the oracle"""
-    monkeypatch.setenv("JP_LM_TILE", "1")
+def test_lm_line_tiles(cuda_device, scanner, n_subsets):
+    """planned TOF listmode projectors on line tiles (runs of events sharing a transaxial line) vs the oracle; then a
+    y with Inf / NaN: the runs that hold them take the per-LOR float path, nothing finite is lost"""
     g, ph = scanner
     xs, xe, tb = _line_events()
     n = xs.shape[1]
@@ -320,7 +320,7 @@ def test_lm_line_tiles(cuda_device, scanner, n_subsets, monkeypatch):
     tof = jp.make_tof(tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas, tofp.n_tofbins, 1.5)
     args = (tofp.tofbin_width, tofp.sigma_tof, tofp.n_sigmas)
     xsd, xed, tbd, imgd = dev(xs, cuda_device), dev(xe, cuda_device), dev(tb, cuda_device), dev(ph, cuda_device)
-    plan = jp.LmPlan(xsd, xed, tbd, g.n, g.origin, g.voxsize, tof, n_subsets=n_subsets)
+    plan = jp.LmPlan(xsd, xed, tbd, g.n, g.origin, g.voxsize, tof, n_subsets=n_subsets).set_path(1)
     p = jp.jp_fwd_tof_lm_planned(plan, imgd)
     ref = oracle.fwd_tof_lm(xs, xe, tb, ph, g.origin, g.voxsize, *args, center_offset=1.5)
     assert (ref > 0).mean() > 0.5
@@ -329,6 +329,18 @@ def test_lm_line_tiles(cuda_device, scanner, n_subsets, monkeypatch):
     b = jp.jp_back_tof_lm_planned(plan, y)
     assert_back(b, oracle.back_tof_lm(xs, xe, tb, y.cpu().numpy(), g.n, g.origin, g.voxsize, *args, center_offset=1.5))
     assert adj_gap(p, y, imgd, b) <= ADJ_GAP
+    # non-finite values on events that cross the image (chosen among the large forward values)
+    hit = np.argsort(ref)[-2000:]
+    y2 = y.cpu().numpy().copy()
+    y2[hit[0]], y2[hit[1000]] = np.inf, np.nan
+    got = jp.jp_back_tof_lm_planned(plan, dev(y2, cuda_device)).cpu().numpy()
+    y0 = y2.copy()
+    y0[~np.isfinite(y0)] = 0.0
+    ref0 = oracle.back_tof_lm(xs, xe, tb, y0, g.n, g.origin, g.voxsize, *args, center_offset=1.5)
+    refb = ~np.isfinite(oracle.back_tof_lm(xs, xe, tb, y2, g.n, g.origin, g.voxsize, *args, center_offset=1.5))
+    bad = ~np.isfinite(got)
+    assert bad.any() and not bad.all() and not (bad & ~refb).sum() > 0.01 * refb.sum()
+    assert np.abs(got[~bad] - ref0[~bad]).max() <= 1e-4 * np.abs(ref0).max()
     plan.destroy()
 
 
@@ -408,10 +420,9 @@ def test_osem_over_event_shards(cuda_device, scanner, events):
 
 
 @pytest.mark.parametrize("tile", ["1", "0"])
-def test_nontof_listmode_planned(cuda_device, scanner, events, tile, monkeypatch):
+def test_nontof_listmode_planned(cuda_device, scanner, events, tile):
     """non-TOF projections of listmode events: unsorted through jp_fwd /
     jp_back, and through the plan (line tiles forced on / off) -- all against the oracle, in caller order"""
-    monkeypatch.setenv("JP_LM_TILE", tile)
     g, ph = scanner
     if tile == "1":
         xs, xe, tb = _line_events(seed=22)
@@ -424,6 +435,7 @@ def test_nontof_listmode_planned(cuda_device, scanner, events, tile, monkeypatch
     ref = oracle.fwd(xs, xe, ph, g.origin, g.voxsize)
     assert_fwd(jp.jp_fwd(xsd, xed, imgd, g.origin, g.voxsize), ref)
     plan = jp.LmPlan(xsd, xed, dev(tb, cuda_device), g.n, g.origin, g.voxsize, tof, n_subsets=2)
+    plan.set_path(1 if tile == "1" else 2)
     p = jp.jp_fwd_lm_planned(plan, imgd)
     assert_fwd(p, ref)
     y = inputs.uniform_values(n, 0.5, 2.0, seed=15).to(cuda_device)
@@ -527,12 +539,42 @@ def test_forward_projections_are_deterministic(cuda_device, scanner, events, mon
     for _ in range(3):
         assert torch.equal(jp.jp_fwd_tof_sino(a, b, img, g.origin, g.voxsize, tof), ref)
     ex, ee, tb = (t.to(cuda_device) for t in events)
-    for tile in ("1", "0"):
-        monkeypatch.setenv("JP_LM_TILE", tile)
-        plan = jp.LmPlan(ex, ee, tb, g.n, g.origin, g.voxsize, tof, n_subsets=1)
+    for path in (1, 2):
+        plan = jp.LmPlan(ex, ee, tb, g.n, g.origin, g.voxsize, tof, n_subsets=1).set_path(path)
         ref = jp.jp_fwd_tof_lm_planned(plan, img).clone()
         refn = jp.jp_fwd_lm_planned(plan, img).clone()
         for _ in range(3):
             assert torch.equal(jp.jp_fwd_tof_lm_planned(plan, img), ref)
             assert torch.equal(jp.jp_fwd_lm_planned(plan, img), refn)
         plan.destroy()
+
+
+@pytest.mark.parametrize("case", ["wide_image", "wide_tof_kernel"])
+def test_planned_listmode_when_the_line_tiles_cannot_hold_the_problem(cuda_device, case):
+    """an image longer than the line tiles' widest shared row (n2 > 256), and a TOF kernel whose weight table does not
+    fit in shared memory: the planned TOF and non-TOF calls must take the quad / per-event path even when line tiles
+    are asked for (they used to fail with 'operation not supported'), and agree with the oracle"""
+    c = inputs.config0(n_lors=4_000)
+    if case == "wide_image":
+        g = inputs.Geometry((24, 24, 270), (4.0, 4.0, 1.0))
+        width, sigma = 9.0, 7.0
+    else:
+        g = c["geom"]
+        width, sigma = 1.0, 40.0
+    rng = np.random.default_rng(3)
+    img = rng.uniform(0, 1, g.n).astype(np.float32)
+    tb = rng.integers(-4, 5, 4_000).astype(np.int16)
+    tof = jp.make_tof(width, sigma, 3.0, 29)
+    xs, xe = c["xstart"], c["xend"]
+    xsd, xed, imgd = dev(xs, cuda_device), dev(xe, cuda_device), dev(img, cuda_device)
+    plan = jp.LmPlan(xsd, xed, dev(tb, cuda_device), g.n, g.origin, g.voxsize, tof, n_subsets=2).set_path(1)
+    p = jp.jp_fwd_tof_lm_planned(plan, imgd)
+    assert_fwd(p, oracle.fwd_tof_lm(xs, xe, tb, img, g.origin, g.voxsize, width, sigma, 3.0))
+    y = rng.uniform(0.5, 2, 4_000).astype(np.float32)
+    b = jp.jp_back_tof_lm_planned(plan, dev(y, cuda_device))
+    assert_back(b, oracle.back_tof_lm(xs, xe, tb, y, g.n, g.origin, g.voxsize, width, sigma, 3.0))
+    pn = jp.jp_fwd_lm_planned(plan, imgd)
+    assert_fwd(pn, oracle.fwd(xs, xe, img, g.origin, g.voxsize))
+    bn = jp.jp_back_lm_planned(plan, dev(y, cuda_device))
+    assert_back(bn, oracle.back(xs, xe, y, g.n, g.origin, g.voxsize))
+    plan.destroy()
