@@ -436,6 +436,28 @@ class Workload:
         out["plane_steps"] = self.jp.jp_plane_steps(self.xs, self.xe, G.n, G.origin, G.voxsize)
         return out
 
+    def time_plan_order_io(self, reps=5):
+        """configs[3] with the per-event arrays in PLAN order (jp_*_tof_lm_planned_sorted): no gather /
+        scatter through the permutation; ms per call"""
+        jp, s = self.jp, self.stream
+        ys = jp.jp_lm_plan_permute(self.plan, self.y, True)
+        ps = torch.empty(self.n, dtype=torch.float32, device=self.dev)
+        f = lambda: jp.jp_fwd_tof_lm_planned_sorted(self.plan, self.img, out=ps)
+        b = lambda: jp.jp_back_tof_lm_planned_sorted(self.plan, ys, img=self.bimg)
+        f(); self.bimg.zero_(); b()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record(s)
+        for _ in range(reps):
+            f()
+        ev[1].record(s)
+        for _ in range(reps):
+            self.bimg.zero_()
+            b()
+        ev[2].record(s)
+        torch.cuda.synchronize()
+        fm, bm = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        return {"fwd_ms": fm, "back_ms": bm, "fwd_events_per_s": self.n / fm * 1e3, "back_events_per_s": self.n / bm * 1e3}
+
     def time_nonaligned_tracks(self, reps=5):
         """tracks whose length is not a multiple of the 768-LOR tile: the 36-ring sub-scanner of every 4th view of
         configs[1] (36 x 36 = 1296 ring pairs per track, 21.3 M LORs); ms per call and plane-steps per second"""
@@ -711,6 +733,46 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
             "hbm_bound_frac": w.hbm_bytes / (dom_ms * 1e-3) / (float(peaks["hbm_gbs"]) * 1e9)}
 
 
+def run_sharded_osem(jp, dev, rank, world, barrier, steps, warmup):
+    """configs[4] with the 40 M events SHARDED over the ranks (multi_gpu.shard_events: contiguous shards
+    that start at a multiple of n_subsets), a listmode plan per rank, and per OSEM subset ONE all-reduce(sum) of the
+    15.36 MB image over NCCL (multi_gpu.lm_osem_sharded); the sensitivity image is a sharded non-TOF back projection of
+    ones over the configs[1] views of the rank + one all-reduce.  Strong scaling: the total work is fixed.
+    Returns (ms per iteration on this rank, dict)."""
+    from paper_2212_12519_b200 import multi_gpu
+    tof = jp.make_tof(*TOF_ARGS)
+    nev = int(os.environ.get("JP_BENCH_EVENTS", "40000000"))
+    n_subsets = 20
+    xs, xe, tb = inputs.listmode_events(nev, seed=inputs.BASE_SEED + 3, device=dev, img=inputs.phantom())   # same list on every rank
+    lo, hi = multi_gpu.shard_events(nev, rank, world, n_subsets)
+    xs, xe, tb = xs[:, lo:hi].contiguous(), xe[:, lo:hi].contiguous(), tb[lo:hi].contiguous()
+    plan = jp.LmPlan(xs, xe, tb, G.n, G.origin, G.voxsize, tof, n_subsets=n_subsets)
+    views = range(rank * inputs.N_VIEWS // world, (rank + 1) * inputs.N_VIEWS // world)
+    sx, se = inputs.sinogram_lors(views=views, device=dev)
+    sens = torch.empty(G.n, dtype=torch.float32, device=dev)
+    multi_gpu.back_sharded(multi_gpu.CudaOps(jp, lors=(sx, se), geom=G), torch.ones(sx.shape[1], device=dev), sens)
+    del sx, se
+    ops = multi_gpu.CudaOps(jp, plan=plan)
+    x = torch.ones(G.n, dtype=torch.float32, device=dev)
+    for _ in range(max(warmup, 1)):
+        multi_gpu.lm_osem_sharded(ops, sens, x, n_subsets, 1)
+    barrier()
+    st = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(steps):
+        multi_gpu.lm_osem_sharded(ops, sens, x, n_subsets, 1)
+    e1.record(st)
+    barrier()
+    ms = e0.elapsed_time(e1) / steps
+    info = {"events": nev, "events_on_rank0": hi - lo if rank == 0 else None, "n_subsets": n_subsets,
+            "collective": "all_reduce(sum) of the %d-voxel float32 image per OSEM subset (%d per iteration) over %s"
+                          % (NVOX, n_subsets, "NCCL" if world > 1 else "one rank (no exchange)"),
+            "image_sum": float(x.double().sum()), "finite": bool(torch.isfinite(x).all())}
+    plan.destroy()
+    return ms, info
+
+
 def measure_fp32_rate(jp, dev):
     """FFMA lane-instructions per second of jp_fma_burn (148 x 8 CTAs of 256 threads, 8 independent chains per thread),
     best of 5 after a warm-up, CUDA events on the current stream"""
@@ -749,6 +811,24 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     c = args.config
+    if c == 4 and (world > 1 or args.sharded):
+        # the 40 M events of ONE reconstruction sharded over the ranks, one all-reduce of the image per subset
+        ms, info = run_sharded_osem(jp, dev, rank, world, barrier, args.steps, args.warmup)
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t[0])
+        if rank == 0:
+            line = {"metric": SPEC[4]["metric"], "value": info["events"] / (ms * 1e-3), "unit": SPEC[4]["unit"],
+                    "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+                    "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                    "config": {"workload": SPEC[4]["workload"] + "; events sharded over the ranks (SURVEY.md 8(e))",
+                               "parallelism": f"event shards x{world}", "l2": SPEC[4]["l2"]},
+                    "gpu_launches": (4 * 20 + 1 + 20) * args.steps, "s_per_iteration": ms * 1e-3, "sharded": info}
+            print(json.dumps(line), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     w = Workload(c, jp, dev, rank)
     if c == 4:
         w.setup_sens()
@@ -772,12 +852,21 @@ def run_ours(args):
         if getattr(w, "hyb", None) is not None:
             w.hyb.destroy()
 
+    sharded = None
+    if world > 1 and c == 1 and not args.no_other:
+        # the path's one exchange step on this node: configs[4] with the events sharded over the ranks (NCCL all-reduce)
+        w_keep = w
+        ms_sh, sharded = run_sharded_osem(jp, dev, rank, world, barrier, 3, 1)
+        w = w_keep
     if world > 1:
-        t = torch.tensor([total_ms, fwd_ms, back_ms, e2e_s or 0.0], device=dev, dtype=torch.float64)
+        t = torch.tensor([total_ms, fwd_ms, back_ms, e2e_s or 0.0, ms_sh if sharded else 0.0], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms, fwd_ms, back_ms = float(t[0]), float(t[1]), float(t[2])
         if e2e_s is not None:
             e2e_s = float(t[3])
+        if sharded:
+            sharded["ms_per_iteration"] = float(t[4])
+            sharded["events_per_s"] = sharded["events"] / (float(t[4]) * 1e-3)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -802,6 +891,8 @@ def run_ours(args):
                                     "is reported as SURVEY.md 8(d) asks, it says nothing about the kernels")
     if w.plan_s is not None:
         line["config"]["plan_s"] = w.plan_s
+    if sharded:
+        line["sharded_osem"] = sharded
     if world == 1:
         rate = measure_fp32_rate(jp, dev)
         line["roofline"]["fp32_ffma_measured"] = {"value": rate / 1e12, "unit": "T lane-instr/s (FP32 FFMA, jp_fma_burn)",
@@ -810,6 +901,7 @@ def run_ours(args):
         line["nonaligned_tracks_36_rings"] = w.time_nonaligned_tracks()
     if c == 3:
         line["nontof_listmode"] = w.time_nontof_listmode()
+        line["plan_order_io"] = w.time_plan_order_io()
     if c >= 4:
         line["s_per_iteration"] = ms_per_step * 1e-3
     if c == 4:
@@ -845,6 +937,7 @@ def run_ours(args):
                 d["fwd"], d["back"] = r["fwd"], r["back"]
             if oc == 3:
                 d["nontof_listmode"] = ow.time_nontof_listmode()
+                d["plan_order_io"] = ow.time_plan_order_io()
             if ow.plan_s is not None:
                 d["plan_s"] = ow.plan_s
             other[f"configs[{oc}]" if oc < 5 else "sino_osem_8f3"] = d
@@ -865,6 +958,8 @@ def main():
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5])
     ap.add_argument("--check", action="store_true",
                     help="run the float64 oracle on the FULL config (outside the timed region) and add `parity` to the line")
+    ap.add_argument("--sharded", action="store_true",
+                    help="--config 4: run the sharded OSEM driver (multi_gpu.lm_osem_sharded) even on one GPU")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the brief configs[2..4] runs of the default line")

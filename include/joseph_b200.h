@@ -167,6 +167,14 @@ int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset);
 int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, float *p, void *stream);
 /* img += A_subset^T y, y has n entries in caller order.  ACCUMULATES. */
 int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, float *img, void *stream);
+/* The same projections with the per-event arrays in PLAN order ("pre-sorted" listmode events): entry k
+ * of p_sorted / y_sorted belongs to the event at position k of the plan's sorted list, i.e. caller event perm[k].  The
+ * planned calls above gather / scatter through the permutation on every call (one 32-byte sector per 4-byte value);
+ * callers that project a list many times (OSEM) permute once with jp_lm_plan_permute and use these.
+ * jp_lm_plan_permute: to_plan_order != 0: out[k] = in[perm[k]]; else out[perm[k]] = in[k].  in != out, n floats. */
+int jp_fwd_tof_lm_planned_sorted(const jp_plan *plan, int subset, const float *img, float *p_sorted, void *stream);
+int jp_back_tof_lm_planned_sorted(const jp_plan *plan, int subset, const float *y_sorted, float *img, void *stream);
+int jp_lm_plan_permute(const jp_plan *plan, const float *in, float *out, int to_plan_order, void *stream);
 /* jp_lm_osem on the plan's events, subsets and geometry */
 /* NON-TOF projections of the plan's events (the paper's second listmode workload: every plane
  * of each event's LOR, the TOF bins of the plan are ignored).  Arguments, order of results (caller order) and

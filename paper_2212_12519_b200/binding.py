@@ -65,6 +65,9 @@ EXPORTS = {
     "jp_lm_plan_set_path": (C.c_int, [C.c_void_p, C.c_int]),
     "jp_fwd_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_back_tof_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_fwd_tof_lm_planned_sorted": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_back_tof_lm_planned_sorted": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "jp_lm_plan_permute": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]),
     "jp_fwd_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_back_lm_planned": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "jp_lm_osem_planned_workspace_bytes": (C.c_size_t, [C.c_void_p]),
@@ -392,6 +395,42 @@ def jp_back_tof_lm_planned(plan: LmPlan, y, subset: int = -1, img=None, stream=N
     _check(load().jp_back_tof_lm_planned(plan.handle, int(subset), y.data_ptr(), img.data_ptr(), _stream(stream)),
            "jp_back_tof_lm_planned")
     return img
+
+
+def jp_fwd_tof_lm_planned_sorted(plan: LmPlan, img, subset: int = -1, out=None, stream=None) -> torch.Tensor:
+    """forward projection with the per-event results in PLAN order (see jp_lm_plan_permute)"""
+    img = _img(img)
+    assert tuple(img.shape) == plan.shape
+    if out is None:
+        out = torch.zeros(plan.n, dtype=torch.float32, device=img.device)
+    _dev(out, torch.float32, "out")
+    assert out.numel() == plan.n and out.is_contiguous()
+    _check(load().jp_fwd_tof_lm_planned_sorted(plan.handle, int(subset), img.data_ptr(), out.data_ptr(), _stream(stream)),
+           "jp_fwd_tof_lm_planned_sorted")
+    return out
+
+
+def jp_back_tof_lm_planned_sorted(plan: LmPlan, y_sorted, subset: int = -1, img=None, stream=None) -> torch.Tensor:
+    _dev(y_sorted, torch.float32, "y_sorted")
+    assert y_sorted.numel() == plan.n and y_sorted.is_contiguous()
+    if img is None:
+        img = torch.zeros(plan.shape, dtype=torch.float32, device=y_sorted.device)
+    img = _img(img)
+    assert tuple(img.shape) == plan.shape
+    _check(load().jp_back_tof_lm_planned_sorted(plan.handle, int(subset), y_sorted.data_ptr(), img.data_ptr(),
+                                                _stream(stream)), "jp_back_tof_lm_planned_sorted")
+    return img
+
+
+def jp_lm_plan_permute(plan: LmPlan, values, to_plan_order: bool, out=None, stream=None) -> torch.Tensor:
+    """per-event float32 values between caller order and plan order"""
+    _dev(values, torch.float32, "values")
+    assert values.numel() == plan.n and values.is_contiguous()
+    if out is None:
+        out = torch.empty_like(values)
+    _check(load().jp_lm_plan_permute(plan.handle, values.data_ptr(), out.data_ptr(), 1 if to_plan_order else 0,
+                                     _stream(stream)), "jp_lm_plan_permute")
+    return out
 
 
 def jp_fwd_lm_planned(plan: LmPlan, img, subset: int = -1, out=None, stream=None) -> torch.Tensor:

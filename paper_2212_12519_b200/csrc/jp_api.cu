@@ -451,6 +451,13 @@ struct PlanCtx {
         rg.io_off = first - sfirst;
         return rg;
     }
+    // the same run with per-event arrays in PLAN order (index = position in the sorted list), or in caller order
+    jp::Range seg_io(int m, int a, bool sorted_io) const
+    {
+        jp::Range rg = seg(m, a, sorted_io);
+        if (sorted_io) rg.io_off = rg.first;
+        return rg;
+    }
     bool has_axis2(int subset) const
     {
         for (int m = 0; m < ns; ++m)
@@ -476,7 +483,7 @@ namespace jp {
         if (e__ != cudaSuccess) return e__; \
     } while (0)
 
-cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, cudaStream_t st)
+cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, cudaStream_t st, bool sorted_io)
 {
     jp_plan tmp;
     tmp.lm = lm;
@@ -492,9 +499,9 @@ cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, 
     for (int a = 0; a < 2; ++a)
         for (int m = 0; m < c.ns; ++m)
             if (subset < 0 || m == subset) {
-                const jp::Range rg = c.seg(m, a, false);
+                const jp::Range rg = c.seg_io(m, a, sorted_io);
                 if (tiles)
-                    JP_E(jp::launch_fwd_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, img, c.g, c.t, p, 0, st));
+                    JP_E(jp::launch_fwd_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, rg.io_off, img, c.g, c.t, p, 0, st));
                 else
                     JP_E(jp::launch_fwd_tof_lm_quad(c.l, c.tb, rg, q[a], c.g, c.t, tc.lut, p, 0, st));
             }
@@ -502,12 +509,12 @@ cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, 
         JP_E(jp::padded_create(img, c.g, false, st, &tc.pimg));
         for (int m = 0; m < c.ns; ++m)
             if (subset < 0 || m == subset)
-                JP_E(jp::launch_fwd_tof_lm(c.l, c.tb, c.seg(m, 2, false), tc.pimg, c.g, c.t, tc.lut, p, 0, st));
+                JP_E(jp::launch_fwd_tof_lm(c.l, c.tb, c.seg_io(m, 2, sorted_io), tc.pimg, c.g, c.t, tc.lut, p, 0, st));
     }
     return cudaSuccess;
 }
 
-cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img, cudaStream_t st)
+cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img, cudaStream_t st, bool sorted_io)
 {
     jp_plan tmp;
     tmp.lm = lm;
@@ -519,8 +526,8 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
         for (int a = 0; a < 2; ++a)
             for (int m = 0; m < c.ns; ++m)
                 if (subset < 0 || m == subset) {
-                    const jp::Range rg = c.seg(m, a, false);
-                    JP_E(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, 0, y, c.g, c.t, img, st));
+                    const jp::Range rg = c.seg_io(m, a, sorted_io);
+                    JP_E(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, rg.io_off, y, c.g, c.t, img, st));
                 }
     } else {
         float4 *b[2];
@@ -530,7 +537,7 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
             JP_E(cudaMemsetAsync(b[a], 0, qbytes, st));
             for (int m = 0; m < c.ns; ++m)
                 if (subset < 0 || m == subset)
-                    JP_E(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, false), y, c.g, c.t, tc.lut, b[a], st));
+                    JP_E(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg_io(m, a, sorted_io), y, c.g, c.t, tc.lut, b[a], st));
         }
         JP_E(jp::launch_quad_merge(b[0], b[1], c.g, img, st));
     }
@@ -538,7 +545,7 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
         JP_E(jp::padded_create(nullptr, c.g, true, st, &tc.pimg));
         for (int m = 0; m < c.ns; ++m)
             if (subset < 0 || m == subset)
-                JP_E(jp::launch_back_tof_lm(c.l, c.tb, c.seg(m, 2, false), y, c.g, c.t, tc.lut, tc.pimg, st));
+                JP_E(jp::launch_back_tof_lm(c.l, c.tb, c.seg_io(m, 2, sorted_io), y, c.g, c.t, tc.lut, tc.pimg, st));
         JP_E(jp::padded_add_to(tc.pimg, c.g, img, st));
     }
     return cudaSuccess;
@@ -556,7 +563,39 @@ int jp_fwd_tof_lm_planned(const jp_plan *plan, int subset, const float *img, flo
     if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
     if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
     if (!img || !p) return fail(JP_ERR_POINTER, "img or p is NULL");
-    JP_CUDA(jp::lm_plan_fwd_tof(plan->lm, subset, img, p, (cudaStream_t)stream), "jp_fwd_tof_lm_planned");
+    JP_CUDA(jp::lm_plan_fwd_tof(plan->lm, subset, img, p, (cudaStream_t)stream, false), "jp_fwd_tof_lm_planned");
+    return JP_OK;
+}
+
+int jp_fwd_tof_lm_planned_sorted(const jp_plan *plan, int subset, const float *img, float *p_sorted, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    if (!img || !p_sorted) return fail(JP_ERR_POINTER, "img or p is NULL");
+    JP_CUDA(jp::lm_plan_fwd_tof(plan->lm, subset, img, p_sorted, (cudaStream_t)stream, true), "jp_fwd_tof_lm_planned_sorted");
+    return JP_OK;
+}
+
+int jp_back_tof_lm_planned_sorted(const jp_plan *plan, int subset, const float *y_sorted, float *img, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    if (!img || !y_sorted) return fail(JP_ERR_POINTER, "img or y is NULL");
+    JP_CUDA(jp::lm_plan_back_tof(plan->lm, subset, y_sorted, img, (cudaStream_t)stream, true), "jp_back_tof_lm_planned_sorted");
+    return JP_OK;
+}
+
+int jp_lm_plan_permute(const jp_plan *plan, const float *in, float *out, int to_plan_order, void *stream)
+{
+    g_err[0] = 0;
+    if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "invalid plan");
+    if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
+    if (!in || !out || in == out) return fail(JP_ERR_POINTER, "in / out is NULL, or in == out");
+    JP_CUDA(jp::lm_plan_permute(plan->lm, in, out, to_plan_order != 0, (cudaStream_t)stream), "jp_lm_plan_permute");
     return JP_OK;
 }
 
@@ -567,7 +606,7 @@ int jp_back_tof_lm_planned(const jp_plan *plan, int subset, const float *y, floa
     if (subset >= jp::lm_plan_subsets(plan->lm)) return fail(JP_ERR_SIZE, "subset out of range");
     if (jp::lm_plan_n(plan->lm) == 0) return JP_OK;
     if (!img || !y) return fail(JP_ERR_POINTER, "img or y is NULL");
-    JP_CUDA(jp::lm_plan_back_tof(plan->lm, subset, y, img, (cudaStream_t)stream), "jp_back_tof_lm_planned");
+    JP_CUDA(jp::lm_plan_back_tof(plan->lm, subset, y, img, (cudaStream_t)stream, false), "jp_back_tof_lm_planned");
     return JP_OK;
 }
 

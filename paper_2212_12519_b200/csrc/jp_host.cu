@@ -488,6 +488,19 @@ struct OneShot {
     ~OneShot() { jp_hybrid_destroy(h); }
 };
 
+// argument errors are reported before any device is touched
+int oneshot_check(const jp_lors *l, const jp_geom *geom, const jp_tof *tof, bool need_tof, bool sino, const void *a, const void *b)
+{
+    jp::err_buf()[0] = 0;
+    if (!l || !geom || (need_tof && !tof) || !a) return JP_ERR_POINTER;
+    jp::Geom g;
+    jp::Tof t;
+    int64_t nvox;
+    if (l->n < 0 || !geom_ok(geom, g, nvox) || (need_tof && !tof_ok(tof, sino, t))) return JP_ERR_SIZE;
+    if (l->n > 0 && (!b || !l->xs || !l->ys || !l->zs || !l->xe || !l->ye || !l->ze)) return JP_ERR_POINTER;
+    return JP_OK;
+}
+
 } // namespace
 
 extern "C" {
@@ -514,6 +527,7 @@ int jp_hybrid_back_tof_lm(jp_hybrid *h, const float *y_host, float *img_host)
 
 int jp_fwd_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, float *p_host)
 {
+    { const int rc0 = oneshot_check(lors_host, geom, nullptr, false, false, img_host, p_host); if (rc0 != JP_OK) return rc0; }
     OneShot o;
     int rc = jp_hybrid_create(nullptr, 0, &o.h);
     if (rc == JP_OK) rc = jp_hybrid_set_lors(o.h, lors_host, nullptr, nullptr, nullptr);
@@ -523,6 +537,7 @@ int jp_fwd_host(const jp_lors *lors_host, const float *img_host, const jp_geom *
 
 int jp_back_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, float *img_host)
 {
+    { const int rc0 = oneshot_check(lors_host, geom, nullptr, false, false, img_host, y_host); if (rc0 != JP_OK) return rc0; }
     OneShot o;
     int rc = jp_hybrid_create(nullptr, 0, &o.h);
     if (rc == JP_OK) rc = jp_hybrid_set_lors(o.h, lors_host, nullptr, nullptr, nullptr);
@@ -533,6 +548,7 @@ int jp_back_host(const jp_lors *lors_host, const float *y_host, const jp_geom *g
 int jp_fwd_tof_sino_host(const jp_lors *lors_host, const float *img_host, const jp_geom *geom, const jp_tof *tof,
                          float *p_host)
 {
+    { const int rc0 = oneshot_check(lors_host, geom, tof, true, true, img_host, p_host); if (rc0 != JP_OK) return rc0; }
     OneShot o;
     int rc = jp_hybrid_create(nullptr, 0, &o.h);
     if (rc == JP_OK) rc = jp_hybrid_set_lors(o.h, lors_host, nullptr, nullptr, nullptr);
@@ -543,6 +559,7 @@ int jp_fwd_tof_sino_host(const jp_lors *lors_host, const float *img_host, const 
 int jp_back_tof_sino_host(const jp_lors *lors_host, const float *y_host, const jp_geom *geom, const jp_tof *tof,
                           float *img_host)
 {
+    { const int rc0 = oneshot_check(lors_host, geom, tof, true, true, img_host, y_host); if (rc0 != JP_OK) return rc0; }
     OneShot o;
     int rc = jp_hybrid_create(nullptr, 0, &o.h);
     if (rc == JP_OK) rc = jp_hybrid_set_lors(o.h, lors_host, nullptr, nullptr, nullptr);
@@ -554,6 +571,7 @@ int jp_fwd_tof_lm_host(const jp_lors *lors_host, const int16_t *tofbin_host, con
                        const jp_tof *tof, float *p_host)
 {
     if (lors_host && lors_host->n > 0 && !tofbin_host) return JP_ERR_POINTER;
+    { const int rc0 = oneshot_check(lors_host, geom, tof, true, false, img_host, p_host); if (rc0 != JP_OK) return rc0; }
     OneShot o;
     int rc = jp_hybrid_create(nullptr, 0, &o.h);
     if (rc == JP_OK) rc = jp_hybrid_set_lors(o.h, lors_host, tofbin_host, geom, tof);
@@ -565,6 +583,7 @@ int jp_back_tof_lm_host(const jp_lors *lors_host, const int16_t *tofbin_host, co
                         const jp_tof *tof, float *img_host)
 {
     if (lors_host && lors_host->n > 0 && !tofbin_host) return JP_ERR_POINTER;
+    { const int rc0 = oneshot_check(lors_host, geom, tof, true, false, img_host, y_host); if (rc0 != JP_OK) return rc0; }
     OneShot o;
     int rc = jp_hybrid_create(nullptr, 0, &o.h);
     if (rc == JP_OK) rc = jp_hybrid_set_lors(o.h, lors_host, tofbin_host, geom, tof);

@@ -133,8 +133,11 @@ void lm_plan_view(const LmPlan *pl, int m, bool compact, Lors *l, const int16_t 
 // events of subset m with principal axis a (a contiguous run of the sorted list): first index and count
 void lm_plan_segment(const LmPlan *pl, int m, int a, int64_t *first, int64_t *count);
 // the planned TOF listmode projectors (jp_api.cu), subset < 0: all events; p / y in caller order
-cudaError_t lm_plan_fwd_tof(LmPlan *pl, int subset, const float *img, float *p, cudaStream_t st);
-cudaError_t lm_plan_back_tof(LmPlan *pl, int subset, const float *y, float *img, cudaStream_t st);
+// sorted_io: p / y are in PLAN order (index = position in the sorted list) instead of caller order
+cudaError_t lm_plan_fwd_tof(LmPlan *pl, int subset, const float *img, float *p, cudaStream_t st, bool sorted_io = false);
+cudaError_t lm_plan_back_tof(LmPlan *pl, int subset, const float *y, float *img, cudaStream_t st, bool sorted_io = false);
+// out[k] = in[perm[k]] (to plan order) or out[perm[k]] = in[k] (to caller order)
+cudaError_t lm_plan_permute(const LmPlan *pl, const float *in, float *out, bool to_plan_order, cudaStream_t st);
 // persistent quad scratch of the plan (allocated on first use): which = 0,1: Q0,Q1; 2,3: B0,B1
 cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
 

@@ -98,6 +98,16 @@ __global__ void k_lm_gather(Lors l, const int16_t *__restrict__ tofbin, const in
     tb[c] = tofbin[j];
 }
 
+__global__ void k_lm_permute(const int *__restrict__ perm, const float *__restrict__ in, float *__restrict__ out, int64_t n,
+                             int to_plan)
+{
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int j = perm[k];
+    if (to_plan) out[k] = in[j];
+    else out[j] = in[k];
+}
+
 // number of runs of consecutive sorted events with the same (canonically ordered) transaxial end points
 __global__ void k_lm_count_runs(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ xe,
                                 const float *__restrict__ ye, int64_t n, unsigned long long *__restrict__ runs)
@@ -244,6 +254,13 @@ cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out)
     }
     *out = pl->quad[which];
     return cudaSuccess;
+}
+
+cudaError_t lm_plan_permute(const LmPlan *pl, const float *in, float *out, bool to_plan_order, cudaStream_t st)
+{
+    if (pl->n == 0) return cudaSuccess;
+    k_lm_permute<<<(unsigned)((pl->n + 255) / 256), 256, 0, st>>>(pl->perm, in, out, pl->n, to_plan_order ? 1 : 0);
+    return cudaGetLastError();
 }
 
 int64_t lm_plan_n(const LmPlan *pl) { return pl->n; }

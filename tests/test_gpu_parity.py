@@ -578,3 +578,34 @@ def test_planned_listmode_when_the_line_tiles_cannot_hold_the_problem(cuda_devic
     bn = jp.jp_back_lm_planned(plan, dev(y, cuda_device))
     assert_back(bn, oracle.back(xs, xe, y, g.n, g.origin, g.voxsize))
     plan.destroy()
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_planned_listmode_in_plan_order(cuda_device, scanner, events, path):
+    """jp_*_tof_lm_planned_sorted take / return per-event arrays in PLAN order: forward == the caller-order result
+    moved to plan order by jp_lm_plan_permute, bit for bit; the adjoint of a permuted y == the caller-order adjoint;
+    the permutation round-trips; per subset as well"""
+    g, ph = scanner
+    if path == 1:
+        xs, xe, tb = _line_events(seed=31)
+    else:
+        xs, xe, tb = (t.numpy()[..., :80_007] for t in events)
+    n = xs.shape[1]
+    tof = jp.make_tof(17.0, 13.6, 3.0, 29)
+    imgd = dev(ph, cuda_device)
+    plan = jp.LmPlan(dev(xs, cuda_device), dev(xe, cuda_device), dev(tb, cuda_device), g.n, g.origin, g.voxsize, tof,
+                     n_subsets=3).set_path(path)
+    p = jp.jp_fwd_tof_lm_planned(plan, imgd)
+    ps = jp.jp_fwd_tof_lm_planned_sorted(plan, imgd)
+    assert torch.equal(ps, jp.jp_lm_plan_permute(plan, p, True))
+    assert torch.equal(jp.jp_lm_plan_permute(plan, ps, False), p)
+    assert_fwd(p, oracle.fwd_tof_lm(xs, xe, tb, ph, g.origin, g.voxsize, 17.0, 13.6, 3.0))
+    y = inputs.uniform_values(n, 0.5, 2.0, seed=19).to(cuda_device)
+    ys = jp.jp_lm_plan_permute(plan, y, True)
+    b = jp.jp_back_tof_lm_planned(plan, y)
+    bs = jp.jp_back_tof_lm_planned_sorted(plan, ys)
+    assert float((b - bs).abs().max()) <= 1e-5 * float(b.abs().max())
+    assert_back(bs, oracle.back_tof_lm(xs, xe, tb, y.cpu().numpy(), g.n, g.origin, g.voxsize, 17.0, 13.6, 3.0))
+    b1 = jp.jp_back_tof_lm_planned_sorted(plan, ys, subset=1)
+    assert float((b1 - jp.jp_back_tof_lm_planned(plan, y, subset=1)).abs().max()) <= 1e-5 * float(b.abs().max())
+    plan.destroy()
