@@ -776,14 +776,21 @@ def run_sharded_osem(jp, dev, rank, world, barrier, steps, warmup):
 def measure_fp32_rate(jp, dev):
     """FFMA lane-instructions per second of jp_fma_burn (148 x 8 CTAs of 256 threads, 8 independent chains per thread),
     best of 5 after a warm-up, CUDA events on the current stream"""
+    import ctypes
+    from paper_2212_12519_b200 import build as jp_build
+    mb = ctypes.CDLL(jp_build.MICROBENCH_LIB)            # bench-only library (csrc/bench/jp_microbench.cu), not the product ABI
+    mb.jp_fma_burn.restype = ctypes.c_int
+    mb.jp_fma_burn.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
     scratch = torch.zeros(4, dtype=torch.float32, device=dev)
     blocks, iters = N_SM * 8, 20000
-    jp.jp_fma_burn(scratch, blocks, iters)
+    n = blocks * 256 * 16 * iters
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    assert mb.jp_fma_burn(scratch.data_ptr(), blocks, iters, st) == 0
     best = 0.0
     for _ in range(5):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        n = jp.jp_fma_burn(scratch, blocks, iters)
+        assert mb.jp_fma_burn(scratch.data_ptr(), blocks, iters, st) == 0
         e1.record()
         torch.cuda.synchronize()
         best = max(best, n / (e0.elapsed_time(e1) * 1e-3))
@@ -895,7 +902,7 @@ def run_ours(args):
         line["sharded_osem"] = sharded
     if world == 1:
         rate = measure_fp32_rate(jp, dev)
-        line["roofline"]["fp32_ffma_measured"] = {"value": rate / 1e12, "unit": "T lane-instr/s (FP32 FFMA, jp_fma_burn)",
+        line["roofline"]["fp32_ffma_measured"] = {"value": rate / 1e12, "unit": "T lane-instr/s (FP32 FFMA, libjp_microbench.so)",
                                                   "frac_of_nominal_peak": rate / (line["roofline"]["peak"] * 1e12)}
     if c == 1 and world == 1 and not args.no_other:
         line["nonaligned_tracks_36_rings"] = w.time_nonaligned_tracks()

@@ -322,11 +322,6 @@ int jp_fwd_tof_lm_host(const jp_lors *lors_host, const int16_t *tofbin_host, con
 int jp_back_tof_lm_host(const jp_lors *lors_host, const int16_t *tofbin_host, const float *y_host, const jp_geom *geom,
                         const jp_tof *tof, float *img_host);
 
-/* FP32 issue-rate microbenchmark for the roofline denominator: enqueues blocks x 256 threads, each
- * running 16 x iters dependent-chain FFMAs (8 independent chains); the caller times the launch.  scratch: device,
- * at least one float (not written in practice). */
-int jp_fma_burn(float *scratch, int blocks, int iters, void *stream);
-
 /* ---- misc ----------------------------------------------------------------------------------------- */
 /* text of the last CUDA error seen by the calling thread ("" if none); valid until the next call */
 const char *jp_last_error(void);

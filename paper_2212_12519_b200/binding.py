@@ -117,7 +117,6 @@ EXPORTS = {
                                      C.c_void_p]),
     "jp_back_tof_lm_host": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.POINTER(jp_tof),
                                       C.c_void_p]),
-    "jp_fma_burn": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
     "jp_last_error": (C.c_char_p, []),
     "jp_version": (C.c_int, []),
 }
@@ -156,6 +155,9 @@ def _dev(t: torch.Tensor, dtype, what: str) -> torch.Tensor:
         raise JosephError(f"{what} must be a CUDA tensor (no CPU fallback)")
     if t.dtype != dtype:
         raise JosephError(f"{what} must be {dtype}, got {t.dtype}")
+    if t.device.index != torch.cuda.current_device():
+        raise JosephError(f"{what} is on cuda:{t.device.index} but the current device is cuda:{torch.cuda.current_device()} "
+                          "(the library launches on the current device)")
     return t
 
 
@@ -182,8 +184,8 @@ def make_lors(xstart: torch.Tensor, xend: torch.Tensor):
     for t in (xstart, xend):
         for a in range(3):
             row = t[a]
-            if not row.is_contiguous():
-                row = row.contiguous()
+            if not row.is_contiguous():    # no hidden copies: a temporary would have to outlive the asynchronous call
+                raise JosephError("every row of xstart / xend must be contiguous (use t.contiguous())")
             rows.append(row)
     l = jp_lors(*[r.data_ptr() for r in rows], int(xstart.shape[1]))
     return l, rows
@@ -887,10 +889,3 @@ def jp_back_tof_lm_host(xstart, xend, tofbin, y, img, origin, voxsize, tof: jp_t
     _check(load().jp_back_tof_lm_host(C.byref(l), tofbin.data_ptr(), y.data_ptr(), C.byref(g), C.byref(tof),
                                       img.data_ptr()), "jp_back_tof_lm_host")
     return img
-
-
-def jp_fma_burn(scratch: torch.Tensor, blocks: int, iters: int, stream=None) -> int:
-    """enqueue the FP32 FFMA microbenchmark; returns the number of lane-instructions (FFMAs) it executes"""
-    _dev(scratch, torch.float32, "scratch")
-    _check(load().jp_fma_burn(scratch.data_ptr(), int(blocks), int(iters), _stream(stream)), "jp_fma_burn")
-    return int(blocks) * 256 * 16 * int(iters)

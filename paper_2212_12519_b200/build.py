@@ -10,6 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libjoseph_b200.so")
+MICROBENCH_SRC = os.path.join(CSRC, "bench", "jp_microbench.cu")      # bench.py's FFMA microbenchmark: NOT in the product library
+MICROBENCH_LIB = os.path.join(HERE, "libjp_microbench.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -27,21 +29,26 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
+    if not os.path.exists(MICROBENCH_LIB) or os.path.getmtime(MICROBENCH_SRC) > os.path.getmtime(MICROBENCH_LIB):
+        return True
     deps = glob.glob(os.path.join(CSRC, "*")) + glob.glob(os.path.join(HERE, "..", "include", "*.h"))
-    return any(os.path.getmtime(d) > t for d in deps)
+    return any(os.path.getmtime(d) > t for d in deps if os.path.isfile(d))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
-    extra = os.environ.get("JP_NVCC_EXTRA", "").split()      # tuning sweeps: -DJP_... overrides of kernel constants
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + sources() + ["-o", LIB]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    # JP_NVCC_EXTRA: a BUILD-time hook for tuning sweeps (-DJP_... overrides of the kernels' compile-time constants,
+    # e.g. JP_SMEM_KB_FWD); nothing in the built library reads the environment
+    extra = os.environ.get("JP_NVCC_EXTRA", "").split()
+    for srcs, out in ((sources(), LIB), ([MICROBENCH_SRC], MICROBENCH_LIB)):
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + srcs + ["-o", out]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
     return LIB
 
 

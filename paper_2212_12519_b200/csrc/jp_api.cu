@@ -1216,13 +1216,4 @@ int jp_osem_update(float *x, float *b, const float *sens, float scale, const jp_
     return JP_OK;
 }
 
-int jp_fma_burn(float *scratch, int blocks, int iters, void *stream)
-{
-    g_err[0] = 0;
-    if (!scratch) return fail(JP_ERR_POINTER, "scratch is NULL");
-    if (blocks < 1 || iters < 1) return fail(JP_ERR_SIZE, "blocks < 1 or iters < 1");
-    JP_CUDA(jp::launch_fma_burn(scratch, blocks, iters, (cudaStream_t)stream), "jp_fma_burn");
-    return JP_OK;
-}
-
 } // extern "C"

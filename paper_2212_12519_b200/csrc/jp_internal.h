@@ -20,9 +20,6 @@ struct Range {
     int64_t io_off = 0;        // compact: per-LOR inputs/outputs are indexed by c + io_off
 };
 
-// FP32 FFMA issue-rate microbenchmark: blocks x 256 threads x 16 x iters FFMAs
-cudaError_t launch_fma_burn(float *out, int blocks, int iters, cudaStream_t st);
-
 cudaError_t launch_classify(const Lors &l, int64_t n, uint8_t *axis, cudaStream_t st);
 
 cudaError_t launch_plane_steps(const Lors &l, int64_t n, const Geom &g, unsigned long long *total, cudaStream_t st);

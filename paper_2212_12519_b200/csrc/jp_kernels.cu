@@ -382,31 +382,3 @@ cudaError_t launch_osem_update(float *x, float *b, const float *sens, float scal
 }
 
 } // namespace jp
-
-// ---- FP32 issue-rate microbenchmark ("measure it with an FMA microbenchmark") ---------------------
-// Every thread runs 8 independent FFMA chains; 8 x iters x 2 FFMA per thread.  bench.py times the launch with CUDA
-// events and reports lane-instructions per second beside the nominal 148 x 128 x clock peak.
-namespace jp {
-namespace {
-__global__ void __launch_bounds__(256) k_fma_burn(float *out, int iters, float a, float b)
-{
-    float x0 = threadIdx.x, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f, x4 = x0 + 4.f, x5 = x0 + 5.f, x6 = x0 + 6.f, x7 = x0 + 7.f;
-#pragma unroll 1
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
-            x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
-        }
-    }
-    const float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
-    if (s == 123.456f) out[0] = s; // never true in practice: keeps the chains alive
-}
-} // namespace
-
-cudaError_t launch_fma_burn(float *out, int blocks, int iters, cudaStream_t st)
-{
-    k_fma_burn<<<blocks, 256, 0, st>>>(out, iters, 0.999f, 0.001f);
-    return cudaGetLastError();
-}
-} // namespace jp

@@ -554,3 +554,44 @@ def test_segment_rule_endpoint_inside_image():
     assert oracle.fwd(e, s, img, o, v)[0] == pytest.approx(5.0, rel=1e-14)
     s, e = _col([2.0001, 1.0, 1.0]), _col([6.0, 1.0, 1.0])
     assert oracle.fwd(s, e, img, o, v)[0] == pytest.approx(4.0, rel=1e-14)
+
+
+def test_O2_osem_subsets_by_composition_of_single_subset_updates():
+    """Pins what test_O only re-types: the subset rule, the order of the subsets and the x n_subsets factor of A14.
+    An OSEM pass over two subsets is two EM updates in a row (Hudson & Larkin, PAPER.md:193 ref. 39).  Each update is
+    computed here through the ONE-subset path -- pinned by the count identity above and by H (sinogram OSEM of the
+    histogrammed list) -- on the events of that subset alone with the sensitivity sens / n_subsets, because
+    x b n / sens = x b / (sens / n).  Interleaving two different event lists A, B makes subset 0 = A, subset 1 = B.
+    Swapping the roles of A and B changes the result (the order is part of the convention); k identical copies of one
+    list make OSEM with k subsets equal to k ML-EM iterations on that list."""
+    rng = np.random.default_rng(12)
+    n = (24, 24, 8)
+    v = np.array([12.0, 12.0, 12.0])
+    o = -(np.array(n) - 1) / 2.0 * v
+    sa, ea = _scanner_like(rng, 1500)
+    sb, eb = _scanner_like(rng, 1500)
+    for a in (sa, ea, sb, eb):
+        a[2] *= 0.25
+    ta, tb = rng.integers(-2, 3, 1500).astype(np.int16), rng.integers(-2, 3, 1500).astype(np.int16)
+    sens = rng.uniform(0.5, 2.0, n)
+    x0 = rng.uniform(0.5, 1.5, n)
+    T = (17.0, 13.6, 3.0)
+    ileave = lambda p, q: np.stack([p, q], axis=-1).reshape(p.shape[:-1] + (-1,))
+    s, e, it = ileave(sa, sb), ileave(ea, eb), ileave(ta, tb)
+    assert np.array_equal(s[:, 0::2], sa) and np.array_equal(s[:, 1::2], sb) and np.array_equal(it[1::2], tb)
+    got = oracle.lm_osem(s, e, it, sens, x0, o, v, *T, n_subsets=2, n_iter=1)
+    step1 = oracle.lm_osem(sa, ea, ta, sens / 2.0, x0, o, v, *T, n_subsets=1, n_iter=1)
+    step2 = oracle.lm_osem(sb, eb, tb, sens / 2.0, step1, o, v, *T, n_subsets=1, n_iter=1)
+    assert np.allclose(got, step2, rtol=1e-12, atol=1e-15)
+    other = oracle.lm_osem(sa, ea, ta, sens / 2.0, oracle.lm_osem(sb, eb, tb, sens / 2.0, x0, o, v, *T, n_subsets=1, n_iter=1),
+                           o, v, *T, n_subsets=1, n_iter=1)
+    assert np.abs(got - other).max() > 1e-6 * np.abs(got).max()          # B-then-A is a different image
+    # two iterations = the same pass twice
+    got2 = oracle.lm_osem(s, e, it, sens, x0, o, v, *T, n_subsets=2, n_iter=2)
+    assert np.allclose(got2, oracle.lm_osem(s, e, it, sens, got, o, v, *T, n_subsets=2, n_iter=1), rtol=1e-12, atol=1e-15)
+    # k interleaved copies of one list: OSEM with k subsets == k ML-EM iterations on the list with sens / k
+    k = 3
+    s3, e3, t3 = np.repeat(sa, k, axis=1), np.repeat(ea, k, axis=1), np.repeat(ta, k)
+    osem = oracle.lm_osem(s3, e3, t3, sens, x0, o, v, *T, n_subsets=k, n_iter=1)
+    mlem = oracle.lm_osem(sa, ea, ta, sens / k, x0, o, v, *T, n_subsets=1, n_iter=k)
+    assert np.allclose(osem, mlem, rtol=1e-12, atol=1e-15)
