@@ -38,21 +38,26 @@ namespace {
 constexpr int kG1K = 512;   // table intervals per TOF bin width
 constexpr int kMinRun = 48; // shorter runs are not worth a row build
 
+// The table runs in the DISTANCE FROM THE SUPPORT EDGE, x' = R - |x| (bin widths, R = n_sigmas sigma / W + 1/2): the two
+// kinks of the truncated kernel (A4: erf argument clamped at +- n_sigmas sigma) sit at x' = 0 and x' = 1, i.e. exactly
+// on table nodes, so the piecewise-linear table never interpolates across one (tabulated in |x| the kinks fall inside
+// an interval and the tail weights are off by up to 2.7e-6 absolute, 10 % of a 1e-5 weight)
 __global__ void k_tof_g1tab(float2 *tab, int n, double W, double m, double isc)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
+    const double R = m / W + 0.5;
     auto E = [&](double y) { return erf(fmin(fmax(y, -m), m) * isc); };
-    auto G = [&](double x) { return 0.5 * (E((x + 0.5) * W) - E((x - 0.5) * W)); };
-    const double g0 = G((double)k / kG1K), g1 = G((double)(k + 1) / kG1K);
-    tab[k] = make_float2((float)(g0 - (double)k * (g1 - g0)), (float)(g1 - g0)); // (intercept, slope): G(x) = .x + x .y
+    auto G = [&](double xp) { const double x = R - xp; return 0.5 * (E((x + 0.5) * W) - E((x - 0.5) * W)); };
+    const double g0 = k == 0 ? 0.0 : G((double)k / kG1K), g1 = G((double)(k + 1) / kG1K);
+    tab[k] = make_float2((float)(g0 - (double)k * (g1 - g0)), (float)(g1 - g0)); // (intercept, slope): G = .x + x' .y
 }
 
 struct G1Tab {
-    const float2 *tab; // device, n entries; entry k = (intercept, slope) of G on [k, k+1] / kG1K; zero beyond R
+    const float2 *tab; // device, n entries; entry k = (intercept, slope) of G on x' in [k, k+1] / kG1K
     int n;
     float scale; // kG1K / W: mm -> table units
-    float xmax;  // n - 1.5
+    float xedge; // R kG1K: table position of the support edge
 };
 
 // canonical orientation of the transaxial end points: start = the lexicographically smaller (x, y)
@@ -62,9 +67,9 @@ __device__ __forceinline__ bool is_swapped(float xs, float ys, float xe, float y
 }
 
 // weight of the event's bin at table position xs (table units, any sign)
-__device__ __forceinline__ float g1_weight(uint32_t gbase, float xmax, float xs)
+__device__ __forceinline__ float g1_weight(uint32_t gbase, float xedge, float xs)
 {
-    const float xa = fminf(fabsf(xs), xmax);
+    const float xa = fmaxf(xedge - fabsf(xs), 0.f);
     const float tt = __fadd_rd(xa, kMagic);
     const float2 v = lds_pair<0>(gbase + (__float_as_uint(tt) << 3));
     return fmaf(xa, v.y, v.x);
@@ -152,7 +157,7 @@ __device__ __forceinline__ float generic_fwd_lm(const Lors &l, int64_t j, float 
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        const float w = TOF ? g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale) : 1.f;
+        const float w = TOF ? g1_weight(gbase, gt.xedge, (centre - tau) * gt.scale) : 1.f;
         acc = fmaf(plane_value(img, r, k, cl), w, acc);
     }
     return r.cf * acc;
@@ -169,7 +174,7 @@ __device__ __forceinline__ void generic_back_lm(const Lors &l, int64_t j, float 
     for (int k = 0; k < r.nk; ++k) {
         const Cell cl = plane_cell(r, k);
         const float tau = fmaf(r.dtau, (float)k, r.tau0);
-        const float w = TOF ? g1_weight(gbase, gt.xmax, (centre - tau) * gt.scale) : 1.f;
+        const float w = TOF ? g1_weight(gbase, gt.xedge, (centre - tau) * gt.scale) : 1.f;
         if (w != 0.f) plane_scatter(img, r, k, cl, x * w);
     }
 }
@@ -236,7 +241,7 @@ __device__ __forceinline__ int64_t out_index(const int *__restrict__ perm, int64
         const float u = fmaf(b2, fk, A2K);                                      \
         const float tt = __fadd_rd(u, kMagic);                                  \
         const float2 v = lds_pair<(K) * P * 8>(row + (__float_as_uint(tt) << 3)); \
-        const float wt = TOF ? g1_weight(gbase, xmax, fmaf(dx, fk, X0K)) : 1.f; \
+        const float wt = TOF ? g1_weight(gbase, xedge, fmaf(dx, fk, X0K)) : 1.f; \
         acc = fmaf(fmaf(u, v.y, v.x), wt, acc);                                 \
     }
 
@@ -260,7 +265,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_FWD)
     if (TOF)
         for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
     const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
-    const float xmax = gt.xmax;
+    const float xedge = gt.xedge;
 
     // ---- canonical transaxial end points of the CTA's events -> runs
     {
@@ -425,7 +430,7 @@ __device__ __forceinline__ void reds_add_lm(uint32_t addr, int q)
         const float tt = __fadd_rd(u, kMagic);                                  \
         const float w = u - (tt - kMagic);                                      \
         const uint32_t a = row + (__float_as_uint(tt) << 2);                    \
-        const float xw = TOF ? xm * g1_weight(gbase, xmax, fmaf(dx, fk, X0K)) : xm; \
+        const float xw = TOF ? xm * g1_weight(gbase, xedge, fmaf(dx, fk, X0K)) : xm; \
         const int qxw = __float_as_int(xw + kMagic);                            \
         const int bits = __float_as_int(fmaf(xw, w, kMagic));                   \
         reds_add_lm<(K) * P * 4>(a, qxw - bits);                                \
@@ -453,7 +458,7 @@ __global__ void __launch_bounds__(kThreads, JP_LMT_MINB_BACK)
     if (TOF)
         for (int i = tid; i < gt.n; i += kThreads) g1[i] = __ldg(gt.tab + i);
     const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
-    const float xmax = gt.xmax;
+    const float xedge = gt.xedge;
     {
         uint4 canon[kPerThread];
 #pragma unroll
@@ -726,7 +731,7 @@ cudaError_t g1tab_create(const Tof &t, int n, cudaStream_t st, G1Tab *out)
     out->tab = tab;
     out->n = n;
     out->scale = (float)((double)kG1K / (double)t.width);
-    out->xmax = (float)n - 1.5f;
+    out->xedge = (float)(((double)t.nsig * (double)t.sigma / (double)t.width + 0.5) * kG1K);
     return cudaSuccess;
 }
 
