@@ -159,6 +159,11 @@ struct SinoPlanView {
     const unsigned char *slot_grp = nullptr; // [T] group of the entry, numbered from 0 inside its slice
     const int *slice_ng = nullptr;         // [ceil(T / kSinoSlice)] groups of the slice; 0: too many, weights per lane
     int slice_len = kSinoSlice;
+    // whole-track kernels (jp_track.cu): a track is cut into t_npieces equal pieces of at most 2304 LORs, a piece has
+    // t_npt x 256 slots; [0] forward lane order, [1] adjoint lane order
+    const float2 *t_zp[2] = {nullptr, nullptr}; // [t_npieces][slots] (zs, ze) of the slot's LOR
+    const int *t_ord[2] = {nullptr, nullptr};   // [t_npieces][slots] its index inside the track, -1: empty slot
+    int t_npieces = 0, t_npt = 0;
     Lors lors{};                  // irregular: the plan's own SoA copy of the list
 };
 cudaError_t sino_plan_create(const Lors &l, int64_t n, cudaStream_t st, SinoPlan **out);
@@ -166,6 +171,10 @@ void sino_plan_destroy(SinoPlan *pl);
 SinoPlanView sino_plan_view(const SinoPlan *pl);
 // regular plan: write the end points of LORs [first, first + count) as SoA arrays into coord6 (6 x count floats)
 cudaError_t sino_plan_expand(const SinoPlanView &pv, int64_t first, int64_t count, float *coord6, cudaStream_t st, Lors *out);
+
+// non-TOF projections of a REGULAR plan, one CTA per track (jp_track.cu); cudaErrorNotSupported: image too wide
+cudaError_t launch_fwd_track(const SinoPlanView &pv, const float *img, const Geom &g, float *p, cudaStream_t st);
+cudaError_t launch_back_track(const SinoPlanView &pv, const float *y, const Geom &g, float *img, cudaStream_t st);
 
 // TOF sinogram kernels on the track tiles of a REGULAR plan (jp_tof_sino_tile.cu), tracks [k0, k0 + nk):
 //   mode 0  p[j][:] = A x            (p, y, epi arrays are indexed by the LOR index j of the plan's list)

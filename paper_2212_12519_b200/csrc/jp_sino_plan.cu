@@ -96,6 +96,8 @@ struct SinoPlan {
     int *order = nullptr;
     unsigned char *slot_grp = nullptr;
     int *slice_ng = nullptr;
+    float2 *t_zp = nullptr; // both lane orders of the whole-track kernels, one allocation each
+    int *t_ord = nullptr;
     float *coord = nullptr;
 };
 
@@ -107,6 +109,8 @@ void sino_plan_destroy(SinoPlan *pl)
     cudaFree(pl->order);
     cudaFree(pl->slot_grp);
     cudaFree(pl->slice_ng);
+    cudaFree(pl->t_zp);
+    cudaFree(pl->t_ord);
     cudaFree(pl->coord);
     delete pl;
 }
@@ -221,7 +225,70 @@ cudaError_t sino_plan_create(const Lors &l, int64_t n, cudaStream_t st, SinoPlan
         JP_SP_TRY(cudaMemcpyAsync(pl->order, order_h.data(), sizeof(int) * (size_t)T, cudaMemcpyHostToDevice, st));
         JP_SP_TRY(cudaMemcpyAsync(pl->slot_grp, grp_h.data(), (size_t)T, cudaMemcpyHostToDevice, st));
         JP_SP_TRY(cudaMemcpyAsync(pl->slice_ng, ng_h.data(), sizeof(int) * (size_t)nsl, cudaMemcpyHostToDevice, st));
+        // ---- lane orders of the whole-track kernels (jp_track.cu; again a performance hint only).  A track is cut into
+        // equal pieces of at most 2304 LORs (9 per thread).  Inside a piece the LORs of a sinogram form a grid (rows: one
+        // axial end point fixed, the other one varies: L columns).  Forward: a half-warp takes a block of 2 rows x 8
+        // columns (at most ~11 axial cells wide: its 64-bit row loads stay conflict-free).  Adjoint: a half-warp takes a
+        // 16-long grid diagonal (lanes one row pitch apart never hit one address), the next half-warp the next diagonal.
+        const int kTrkSlotsMax = 9 * 256;
+        const int npieces = (T + kTrkSlotsMax - 1) / kTrkSlotsMax;
+        const int piece_len = (T + npieces - 1) / npieces;
+        const int npt = piece_len <= 3 * 256 ? 3 : piece_len <= 6 * 256 ? 6 : 9;
+        const int slots = npt * 256;
+        std::vector<float2> tzp((size_t)2 * npieces * slots, make_float2(0.f, 0.f));
+        std::vector<int> tord((size_t)2 * npieces * slots, -1);
+        for (int pc = 0; pc < npieces; ++pc) {
+            const int first = pc * piece_len, cnt = std::min(piece_len, T - first);
+            // row length of the grid: the first entry whose zs (or ze) changes while the other one has been constant
+            int Ls = cnt, Le = cnt;
+            for (int i = 1; i < cnt && Ls == cnt; ++i)
+                if (zp[(size_t)(first + i)].x != zp[(size_t)first].x) Ls = i;
+            for (int i = 1; i < cnt && Le == cnt; ++i)
+                if (zp[(size_t)(first + i)].y != zp[(size_t)first].y) Le = i;
+            int L = 0;
+            if (Ls == 1 && Le < cnt) L = Le;
+            else if (Le == 1 && Ls < cnt) L = Ls;
+            if (L < 2 || cnt % L) L = 0;
+            std::vector<int> of, ob;
+            of.reserve((size_t)cnt);
+            ob.reserve((size_t)cnt);
+            if (L) {
+                const int R = cnt / L;
+                for (int r0 = 0; r0 < R; r0 += 2)
+                    for (int cb = 0; cb < L; cb += 8)
+                        for (int r = r0; r < std::min(R, r0 + 2); ++r)
+                            for (int c = cb; c < std::min(L, cb + 8); ++c) of.push_back(r * L + c);
+                for (int r0 = 0; r0 < R; r0 += 16) {
+                    const int nr = std::min(16, R - r0);
+                    for (int c0 = 0; c0 < L; ++c0)
+                        for (int d = 0; d < nr; ++d) ob.push_back((r0 + d) * L + (c0 + d) % L);
+                }
+            } else {
+                for (int i = 0; i < cnt; ++i) {
+                    of.push_back(i);
+                    ob.push_back(i);
+                }
+            }
+            for (int dir = 0; dir < 2; ++dir) {
+                const std::vector<int> &o = dir ? ob : of;
+                const size_t base = ((size_t)dir * npieces + pc) * slots;
+                for (int i = 0; i < cnt; ++i) {
+                    tord[base + i] = first + o[(size_t)i];
+                    tzp[base + i] = zp[(size_t)(first + o[(size_t)i])];
+                }
+            }
+        }
+        JP_SP_TRY(cudaMalloc((void **)&pl->t_zp, sizeof(float2) * tzp.size()));
+        JP_SP_TRY(cudaMalloc((void **)&pl->t_ord, sizeof(int) * tord.size()));
+        JP_SP_TRY(cudaMemcpyAsync(pl->t_zp, tzp.data(), sizeof(float2) * tzp.size(), cudaMemcpyHostToDevice, st));
+        JP_SP_TRY(cudaMemcpyAsync(pl->t_ord, tord.data(), sizeof(int) * tord.size(), cudaMemcpyHostToDevice, st));
         JP_SP_TRY(cudaStreamSynchronize(st)); // the vectors are host temporaries
+        pl->v.t_npieces = npieces;
+        pl->v.t_npt = npt;
+        for (int dir = 0; dir < 2; ++dir) {
+            pl->v.t_zp[dir] = pl->t_zp + (size_t)dir * npieces * slots;
+            pl->v.t_ord[dir] = pl->t_ord + (size_t)dir * npieces * slots;
+        }
         pl->v.K = K;
         pl->v.T = T;
         pl->v.regular = 1;

@@ -21,6 +21,9 @@
 #include "jp_f32x2.cuh"
 #include "jp_tile_common.cuh"
 
+#ifndef JP_PLAN_TRACKS
+#define JP_PLAN_TRACKS 1 // regular plans: whole-track kernels (jp_track.cu); 0: the tile kernels, dealt per track
+#endif
 #ifndef JP_BACK_MAP
 #define JP_BACK_MAP 0
 #endif // adjoint lane mapping: which neighbouring diagonal the second half-warp takes
@@ -726,6 +729,7 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
 {
     if (n == 0) return cudaSuccess;
     const bool plan = pv && pv->regular;
+    if (plan && JP_PLAN_TRACKS) return launch_fwd_track(*pv, img, g, p, st);
     const TileCfg c = tile_cfg(g, img, sizeof(float2), JP_SMEM_KB_FWD * 1024);
     const PlanSrc ps = plan_src(pv);
     if (!c.P) return plan ? cudaErrorNotSupported : launch_fwd(l, Range{0, 1, n, false, nullptr}, img, g, p, st);
@@ -752,6 +756,7 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
 {
     if (n == 0) return cudaSuccess;
     const bool plan = pv && pv->regular;
+    if (plan && JP_PLAN_TRACKS) return launch_back_track(*pv, y, g, img, st);
     const TileCfg c = tile_cfg(g, img, sizeof(int), JP_SMEM_KB_BACK * 1024);
     const PlanSrc ps = plan_src(pv);
     if (!c.P) return plan ? cudaErrorNotSupported : launch_back(l, Range{0, 1, n, false, nullptr}, y, g, img, st);

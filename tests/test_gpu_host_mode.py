@@ -101,7 +101,8 @@ def test_hybrid_handle_nontof_workers(cuda_device):
     y = inputs.uniform_values(n, 0.0, 1.0, seed=5)
     ref = oracle.fwd(xs.numpy(), xe.numpy(), ph, g.origin, g.voxsize)
     bref = oracle.back(xs.numpy(), xe.numpy(), y.numpy(), g.n, g.origin, g.voxsize)
-    p_dev = jp.jp_fwd(xs.to(cuda_device), xe.to(cuda_device), img.to(cuda_device), g.origin, g.voxsize).cpu()
+    plan = jp.SinoPlan(xs.to(cuda_device), xe.to(cuda_device))
+    p_dev = jp.jp_fwd_planned(plan, img.to(cuda_device), g.origin, g.voxsize).cpu()   # shards are whole tracks: same kernel
     for devs in _devices_variants():
         h = jp.Hybrid(devs)
         assert h.workers == len(devs)

@@ -239,8 +239,9 @@ def test_planned_sino_osem(cuda_device):
 # ---- non-TOF projections of a sinogram plan (per-track tiles, no end-point arrays read) --------------------------------
 def test_planned_nontof_scanner_views(cuda_device):
     """configs[1] structure: views 0, 64 (exact 45 degree ties) and 100 x 14 radial bins (incl. the degenerate
-    r = +-128 and misses) x 2304 ring pairs: planned forward == unplanned forward bit for bit (same arithmetic per
-    LOR), both against the oracle; planned adjoint against the oracle; accumulate semantics"""
+    r = +-128 and misses) x 2304 ring pairs: planned forward (one CTA per track) against the unplanned forward (tiles
+    of 768 LORs: the same arithmetic per LOR up to the rounding of the plane coordinate, which depends on where a
+    chunk of planes starts), both against the oracle; planned adjoint against the oracle; accumulate semantics"""
     g, ph = inputs.GEOM_SCANNER, inputs.phantom()
     radial = [-128, -70, -64, -33, -20, -1, 0, 1, 7, 31, 50, 64, 65, 128]
     xs, xe = inputs.sinogram_lors(views=[0, 64, 100], radial=radial)
@@ -249,7 +250,9 @@ def test_planned_nontof_scanner_views(cuda_device):
     plan = jp.SinoPlan(xsd, xed)
     assert plan.regular and plan.track_length == 2304 and plan.n_tracks == 3 * len(radial)
     p = jp.jp_fwd_planned(plan, imgd, g.origin, g.voxsize)
-    assert torch.equal(p, jp.jp_fwd(xsd, xed, imgd, g.origin, g.voxsize))
+    pu = jp.jp_fwd(xsd, xed, imgd, g.origin, g.voxsize)
+    assert float((p - pu).abs().max()) <= 2e-6 * float(pu.abs().max())
+    assert torch.equal(p == 0, pu == 0)       # LORs that miss the image: exactly zero in both
     ref = oracle.fwd(xs.numpy(), xe.numpy(), ph, g.origin, g.voxsize)
     assert (ref > 0).mean() > 0.3
     assert_fwd(p, ref)
@@ -290,6 +293,28 @@ def test_planned_nontof_tracks_not_a_multiple_of_the_tile(cuda_device):
     y2 = np.random.default_rng(2).uniform(-1, 1, K * T).astype(np.float32)
     b2 = jp.jp_back_planned(plan2, dev(y2, cuda_device), gs.n, gs.origin, gs.voxsize)
     assert_back(b2, oracle.back(sxs, sxe, y2, gs.n, gs.origin, gs.voxsize))
+
+
+@pytest.mark.parametrize("nzs,nze", [(60, 60), (1, 2500), (53, 47)])
+def test_planned_nontof_long_tracks(cuda_device, nzs, nze):
+    """tracks longer than one CTA takes (3600 = 2 pieces of 1800; 2500 LORs with ONE axial start point: no grid, 2
+    pieces of 1250; 2491 = 53 x 47: 2 ragged pieces that cut the grid rows) on the small image, wide axial range
+    (part of every track misses the image, the extra tracks are steep or degenerate)"""
+    gs = inputs.GEOM_SMALL
+    extra = [(-20.0, 3.0, 25.0, 5.0), (-150.0, 0.5, 150.0, -0.5), (-150.0, -150.0, 150.0, 150.0), (30.0, 40.0, 30.0, 40.0)]
+    sxs, sxe, K, T = mini_sinogram(5, np.linspace(-45.0, 45.0, nzs) if nzs > 1 else [3.0], np.linspace(-50.0, 41.0, nze),
+                                   seed=nzs, extra_tracks=extra)
+    img = np.random.default_rng(1).uniform(0, 1, gs.n).astype(np.float32)
+    plan = jp.SinoPlan(dev(sxs, cuda_device), dev(sxe, cuda_device))
+    assert plan.regular and plan.track_length == nzs * nze and T > 2304
+    p = jp.jp_fwd_planned(plan, dev(img, cuda_device), gs.origin, gs.voxsize)
+    ref = oracle.fwd(sxs, sxe, img, gs.origin, gs.voxsize)
+    assert (ref > 0).mean() > 0.3
+    assert_fwd(p, ref)
+    y = np.random.default_rng(2).uniform(-1, 1, K * T).astype(np.float32)
+    b = jp.jp_back_planned(plan, dev(y, cuda_device), gs.n, gs.origin, gs.voxsize)
+    assert_back(b, oracle.back(sxs, sxe, y, gs.n, gs.origin, gs.voxsize))
+    assert adj_gap(p, dev(y, cuda_device), dev(img, cuda_device), b) <= ADJ_GAP
 
 
 @pytest.mark.parametrize("planned", [False, True])
