@@ -141,13 +141,16 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
  * sort, done once per event list: the events of every OSEM subset (subset m = {e : e mod n_subsets == m},
  * the rule of jp_lm_osem) are ordered by principal axis, transaxial line, plane and axial position of
  * their TOF bin, and a sorted copy of the end points / TOF bins is kept on the device together with the
- * permutation.  Planned calls compute exactly what the unplanned calls compute (same arithmetic per
- * event; only the order of the floating-point sums of the back projection changes) and take / return
- * per-event arrays in CALLER order.
+ * permutation.  Planned calls compute the projections the unplanned calls compute (path 2 with the same
+ * arithmetic per event, the other paths within float32 rounding: other TOF weight table, other order of
+ * the floating-point sums) and take / return per-event arrays in CALLER order.
  *   events, tofbin: device arrays, only read during jp_lm_plan_create (not kept).
- *   The plan owns its device buffers (26 + 4 bytes per event) until jp_lm_plan_destroy.
- *   jp_lm_plan_create allocates with cudaMalloc and SYNCHRONISES `stream` twice (it reads the per-subset / per-axis
- *   event counts and the run statistics back to the host); the planned calls are asynchronous.  A plan keeps
+ *   The plan owns its device buffers (26 + 4 bytes per event) until jp_lm_plan_destroy.  When the sorted events do NOT
+ *   come in long runs on one transaxial line (an OSEM subset of a clinical acquisition: ~20 events per line), the plan
+ *   also cuts every event into PIECES per image brick of 32 x 32 x 16 cells (csrc/jp_brick.cu; about 3.5 pieces of
+ *   32 bytes per event + 4 bytes per event), so that the forward projection can run on bricks held in shared memory.
+ *   jp_lm_plan_create allocates with cudaMalloc and SYNCHRONISES `stream` (it reads the per-subset / per-axis event
+ *   counts, the run statistics and the piece counts back to the host); the planned calls are asynchronous.  A plan keeps
  *   image-sized scratch (quad image and accumulators, allocated with cudaMalloc on the first call that needs them)
  *   that the planned calls write: use a plan from ONE stream at a time.
  *   n_subsets in 1..255, fewer than 2^31 events.  subset = -1 in the calls below means all events. */
@@ -155,11 +158,22 @@ typedef struct jp_plan jp_plan;
 int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom, const jp_tof *tof,
                       int n_subsets, void *stream, jp_plan **plan);
 int jp_lm_plan_destroy(jp_plan *plan);
-/* Which kernels the planned listmode projectors use: 0 = chosen from the plan's run statistics (default: line tiles
- * when the sorted events come in runs of >= 512 on one transaxial line, else the quad image), 1 = line tiles,
- * 2 = quad image / per-event kernels.  All paths compute the same projections (tests force each of them); images or
- * TOF kernels too wide for the line tiles take path 2 whatever is asked.  Not to be changed while a call that uses the
- * plan is being issued from another thread. */
+/* Which kernels the planned listmode projectors and the planned OSEM use:
+ *   0  chosen from the plan's run statistics (default): line tiles when the sorted events come in runs of >= 512 on one
+ *      transaxial line, else path 3 when the plan could build its brick pieces, else path 2;
+ *   1  line tiles (csrc/jp_lm_tile.cu): rows shared by the events of a line, adjoint staged in fixed point per run;
+ *   2  quad image (csrc/jp_quad.cu): one 128-bit gather / float atomic add per event and plane;
+ *   3  image bricks for the forward projection (csrc/jp_brick.cu: TMA box loads into shared memory), float atomic adds
+ *      on the quad accumulators for the adjoint -- the same floating-point semantics as path 2;
+ *   4  image bricks both ways: the adjoint is staged per brick in int32 fixed point and flushed with 128-bit REDs.  One
+ *      scale per chunk of <= 4096 pieces, tied to the chunk's MEDIAN |cf y|: a term is rounded to T / lim, T = 16 .. 32 x
+ *      that median, lim >= 2^19 (2^31 / (G(0) x the largest number of pieces of the chunk that touch one voxel), counted by
+ *      the plan; ~2^26 for a clinical subset); values above T, Inf and NaN take float atomic adds.  Back projections meet
+ *      north_star's 1e-4 max|.| bound; an OSEM whose update is ill-conditioned (a sensitivity image with zeros inside the
+ *      object) amplifies the rounding and wants paths 0 / 2 / 3.  Never chosen automatically.
+ * All paths compute the same projections (tests force each of them); images or TOF kernels a path cannot hold fall
+ * back towards path 2.  Paths 3 / 4 build the brick pieces if the plan has none (allocates, synchronises).  Not to be
+ * changed while a call that uses the plan is being issued from another thread. */
 int jp_lm_plan_set_path(jp_plan *plan, int path);
 /* number of events of a subset (subset = -1: all); -1 for an invalid plan or subset */
 int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset);

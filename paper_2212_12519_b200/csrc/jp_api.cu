@@ -149,6 +149,32 @@ static int lm_osem_loop(View view, int n_subsets, int n_iter, const jp::Geom &g,
     return JP_OK;
 }
 
+// Which kernels a planned listmode call uses.  Line tiles (jp_lm_tile.cu) pay when the sorted events come in long runs
+// on one transaxial line (crystal-snapped events, all subsets together: ~2500 per run for configs[3]); sparsely
+// populated lines (one OSEM subset of 20: ~120 per run) take the image bricks (jp_brick.cu), and whatever the bricks
+// cannot hold takes the quad image (jp_quad.cu).  jp_lm_plan_set_path overrides the rule.
+bool lm_tiles_wanted(const jp::LmPlan *lm, bool tof)
+{
+    if (!jp::lm_tile_supported(jp::lm_plan_geom(lm), jp::lm_plan_tof(lm), tof)) return false;
+    const int path = jp::lm_plan_path(lm);
+    if (path == 1) return true;
+    if (path >= 2) return false;
+    const int64_t runs = jp::lm_plan_runs(lm);
+    return runs > 0 && jp::lm_plan_n(lm) / runs >= 512;
+}
+
+// the plan's brick set if the call should use it (path 0 / 3 / 4 and the plan could build one), else null.
+// *staged: the adjoint goes through the bricks too (path 4: fixed-point staging in shared memory); otherwise only the
+// forward projection does and the adjoint keeps float atomics on the quad accumulators (path 0 / 3).
+cudaError_t lm_bricks_wanted(jp::LmPlan *lm, cudaStream_t st, const jp::BrickSet **bs, bool *staged = nullptr)
+{
+    *bs = nullptr;
+    const int path = jp::lm_plan_path(lm);
+    if (staged) *staged = path == 4;
+    if (path == 1 || path == 2) return cudaSuccess;
+    return jp::lm_plan_bricks(lm, st, bs);
+}
+
 } // namespace
 
 extern "C" {
@@ -370,6 +396,14 @@ int jp_lm_plan_create(const jp_lors *events, const int16_t *tofbin, const jp_geo
     JP_CUDA(jp::lm_plan_create(l, tofbin, events->n, g, t, n_subsets, (cudaStream_t)stream, &lm), "jp_lm_plan_create");
     jp_plan *pl = new jp_plan;
     pl->lm = lm;
+    if (!lm_tiles_wanted(lm, true)) { // sparsely populated lines: the planned calls will want the brick pieces
+        const jp::BrickSet *bs;
+        const cudaError_t e = jp::lm_plan_bricks(lm, (cudaStream_t)stream, &bs);
+        if (e != cudaSuccess) {
+            jp_plan_destroy(pl);
+            return fail_cuda(e, "jp_lm_plan_create (bricks)");
+        }
+    }
     *plan = pl;
     return JP_OK;
 }
@@ -393,8 +427,13 @@ int jp_lm_plan_set_path(jp_plan *plan, int path)
 {
     g_err[0] = 0;
     if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "not a listmode plan");
-    if (path < 0 || path > 2) return fail(JP_ERR_SIZE, "path must be 0 (automatic), 1 (line tiles) or 2 (quad image)");
+    if (path < 0 || path > 4)
+        return fail(JP_ERR_SIZE, "path must be 0 (automatic), 1 (line tiles), 2 (quad image), 3 (bricks forward) or 4 (bricks both ways)");
     jp::lm_plan_set_path(plan->lm, path);
+    if (path >= 3) { // builds the pieces now if the plan has none yet (allocates, synchronises the NULL stream)
+        const jp::BrickSet *bs;
+        JP_CUDA(jp::lm_plan_bricks(plan->lm, nullptr, &bs), "jp_lm_plan_set_path (bricks)");
+    }
     return JP_OK;
 }
 
@@ -411,20 +450,6 @@ int64_t jp_lm_plan_subset_count(const jp_plan *plan, int subset)
 
 // ---- planned calls: quad image, axis by axis (jp_quad.cu) --------------------------------------------------------
 namespace {
-
-// line tiles (jp_lm_tile.cu) pay when the sorted events come in long runs on one transaxial line (crystal-snapped
-// events, all subsets together: ~2500 per run for configs[3]); short runs (one OSEM subset of 20: ~120) are
-// faster on the quad image.  jp_lm_plan_set_path overrides the rule; images / TOF kernels the tiles cannot hold
-// always take the other paths.
-bool lm_tiles_wanted(const jp::LmPlan *lm, bool tof)
-{
-    if (!jp::lm_tile_supported(jp::lm_plan_geom(lm), jp::lm_plan_tof(lm), tof)) return false;
-    const int path = jp::lm_plan_path(lm);
-    if (path == 1) return true;
-    if (path == 2) return false;
-    const int64_t runs = jp::lm_plan_runs(lm);
-    return runs > 0 && jp::lm_plan_n(lm) / runs >= 512;
-}
 
 struct PlanCtx {
     jp::LmPlan *lm;
@@ -456,6 +481,15 @@ struct PlanCtx {
     {
         jp::Range rg = seg(m, a, sorted_io);
         if (sorted_io) rg.io_off = rg.first;
+        return rg;
+    }
+    // all events of subset m (a contiguous run of the sorted list), per-event arrays indexed from its start
+    jp::Range subset(int m) const
+    {
+        jp::Lors ll;
+        const int16_t *tt;
+        jp::Range rg;
+        jp::lm_plan_view(lm, m, true, &ll, &tt, &rg);
         return rg;
     }
     bool has_axis2(int subset) const
@@ -491,12 +525,31 @@ cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, 
     TofCtx tc;
     tc.st = st;
     JP_E(jp::tof_lut_create(c.t, st, &tc.lut));
-    float4 *q[2];
-    JP_E(jp::lm_plan_quad(c.lm, 0, &q[0]));
-    JP_E(jp::lm_plan_quad(c.lm, 1, &q[1]));
     const bool tiles = lm_tiles_wanted(c.lm, true);
-    if (!tiles) JP_E(jp::launch_quad_build(img, c.g, q[0], q[1], st));
-    for (int a = 0; a < 2; ++a)
+    const jp::BrickSet *bs = nullptr;
+    if (!tiles) JP_E(lm_bricks_wanted(c.lm, st, &bs));
+    if (bs) { // image bricks: per-event sums of every subset in a stream-ordered scratch array, then p = cf sum
+        float *acc = nullptr;
+        JP_E(cudaMallocAsync((void **)&acc, sizeof(float) * (size_t)jp::lm_plan_n(c.lm), st));
+        cudaError_t e = cudaMemsetAsync(acc, 0, sizeof(float) * (size_t)jp::lm_plan_n(c.lm), st);
+        for (int m = 0; m < c.ns && e == cudaSuccess; ++m)
+            if (subset < 0 || m == subset) {
+                e = jp::launch_brick_fwd(bs, m, img, c.g, c.t, 0, acc, st);
+                for (int a = 0; a < 2 && e == cudaSuccess; ++a) {
+                    const jp::Range rg = c.seg_io(m, a, sorted_io);
+                    e = jp::launch_brick_finish(bs, acc, rg.first, rg.count, 0, rg.perm, rg.io_off, 0, p, st);
+                }
+            }
+        cudaFreeAsync(acc, st);
+        JP_E(e);
+    }
+    float4 *q[2] = {nullptr, nullptr};
+    if (!tiles && !bs) {
+        JP_E(jp::lm_plan_quad(c.lm, 0, &q[0]));
+        JP_E(jp::lm_plan_quad(c.lm, 1, &q[1]));
+        JP_E(jp::launch_quad_build(img, c.g, q[0], q[1], st));
+    }
+    for (int a = 0; a < 2 && !bs; ++a)
         for (int m = 0; m < c.ns; ++m)
             if (subset < 0 || m == subset) {
                 const jp::Range rg = c.seg_io(m, a, sorted_io);
@@ -522,13 +575,22 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
     TofCtx tc;
     tc.st = st;
     JP_E(jp::tof_lut_create(c.t, st, &tc.lut));
-    if (lm_tiles_wanted(c.lm, true)) {
+    const bool tiles = lm_tiles_wanted(c.lm, true);
+    const jp::BrickSet *bs = nullptr;
+    bool staged = false;
+    if (!tiles) JP_E(lm_bricks_wanted(c.lm, st, &bs, &staged));
+    if (!staged) bs = nullptr;
+    if (tiles) {
         for (int a = 0; a < 2; ++a)
             for (int m = 0; m < c.ns; ++m)
                 if (subset < 0 || m == subset) {
                     const jp::Range rg = c.seg_io(m, a, sorted_io);
                     JP_E(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, rg.io_off, y, c.g, c.t, img, st));
                 }
+    } else if (bs) { // image bricks: y indexed by the sorted position (plan order) or through the permutation
+        for (int m = 0; m < c.ns; ++m)
+            if (subset < 0 || m == subset)
+                JP_E(jp::launch_brick_back(bs, m, 0, y, sorted_io ? nullptr : c.all.perm, c.g, c.t, 0, img, st));
     } else {
         float4 *b[2];
         const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
@@ -688,14 +750,19 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
     TofCtx tc;
     tc.st = st;
     JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
-    float4 *q[2], *b[2];
+    // bs: forward sums on the image bricks; staged: the adjoint too (else float atomics on the quad accumulators)
+    const jp::BrickSet *bs = nullptr;
+    bool staged = false;
+    JP_CUDA(lm_bricks_wanted(c.lm, st, &bs, &staged), where);
+    staged = staged && bs;
+    float4 *q[2] = {nullptr, nullptr}, *b[2] = {nullptr, nullptr};
     const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
-    for (int a = 0; a < 2; ++a) {
-        JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
+    for (int a = 0; a < 2 && !staged; ++a) {
+        if (!bs) JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
         JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
     }
     const bool z_events = c.has_axis2(-1);
-    if (z_events) JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
+    if (z_events || staged) JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
     // resolution model: xb = G x feeds the forward projection, G folds the back projection (stream-ordered scratch)
     struct Scratch {
         float *p = nullptr;
@@ -718,10 +785,25 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                 JP_CUDA(jp::launch_gauss3d(img, xb, tmp, c.g, res_sigma, res_nsig, st), where);
                 xin = xb;
             }
-            JP_CUDA(jp::launch_quad_build(xin, c.g, q[0], q[1], st), where);
-            for (int a = 0; a < 2; ++a) { // forward, ratio and back of the subset's events in one pass per axis
-                JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
-                JP_CUDA(jp::launch_osem_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, b[a], st), where);
+            if (bs) { // bricks: forward sums per event; ratio + back projection staged per brick into bz, or with
+                      // float atomics on the quad accumulators
+                const jp::Range sub = c.subset(m);
+                JP_CUDA(cudaMemsetAsync(r, 0, sizeof(float) * (size_t)sub.count, st), where);
+                JP_CUDA(jp::launch_brick_fwd(bs, m, xin, c.g, c.t, sub.first, r, st), where);
+                if (staged) {
+                    JP_CUDA(jp::launch_brick_back(bs, m, 1, r, nullptr, c.g, c.t, sub.first, bz, st), where);
+                } else {
+                    for (int a = 0; a < 2; ++a) {
+                        JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
+                        JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st, 1), where);
+                    }
+                }
+            } else {
+                JP_CUDA(jp::launch_quad_build(xin, c.g, q[0], q[1], st), where);
+                for (int a = 0; a < 2; ++a) { // forward, ratio and back of the subset's events in one pass per axis
+                    JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
+                    JP_CUDA(jp::launch_osem_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, b[a], st), where);
+                }
             }
             if (z_events) {
                 float *px = nullptr, *pb = nullptr;
@@ -734,7 +816,13 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                 jp::padded_destroy(pb, st);
                 JP_CUDA(e, where);
             }
-            if (!res) {
+            if (staged && !res) {
+                JP_CUDA(jp::launch_osem_update(img, bz, sens, (float)c.ns, nvox, st), where); // clears bz
+            } else if (staged) {
+                JP_CUDA(jp::launch_gauss3d(bz, bb, tmp, c.g, res_sigma, res_nsig, st), where);
+                JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
+                JP_CUDA(jp::launch_osem_update(img, bb, sens, (float)c.ns, nvox, st), where);
+            } else if (!res) {
                 JP_CUDA(jp::launch_quad_osem_update(img, b[0], b[1], z_events ? bz : nullptr, sens, (float)c.ns, c.g, st), where);
             } else {
                 JP_CUDA(cudaMemsetAsync(bb, 0, sizeof(float) * (size_t)nvox, st), where);
@@ -1178,19 +1266,40 @@ int jp_lm_osem_planned_backratio(const jp_plan *plan, int subset, const float *x
     TofCtx tc;
     tc.st = st;
     JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
-    float4 *q[2], *qb[2];
-    const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
-    for (int a = 0; a < 2; ++a) {
-        JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
-        JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &qb[a]), where);
-    }
     const int m = subset;
-    JP_CUDA(jp::launch_quad_build(x, c.g, q[0], q[1], st), where);
-    for (int a = 0; a < 2; ++a) {
-        JP_CUDA(cudaMemsetAsync(qb[a], 0, qbytes, st), where);
-        JP_CUDA(jp::launch_osem_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, qb[a], st), where);
+    const jp::BrickSet *bs = nullptr;
+    bool staged = false;
+    JP_CUDA(lm_bricks_wanted(c.lm, st, &bs, &staged), where);
+    if (bs) {
+        const jp::Range sub = c.subset(m);
+        JP_CUDA(cudaMemsetAsync(r, 0, sizeof(float) * (size_t)sub.count, st), where);
+        JP_CUDA(jp::launch_brick_fwd(bs, m, x, c.g, c.t, sub.first, r, st), where);
     }
-    JP_CUDA(jp::launch_quad_merge(qb[0], qb[1], c.g, b, st), where);
+    if (bs && staged) {
+        JP_CUDA(jp::launch_brick_back(bs, m, 1, r, nullptr, c.g, c.t, c.subset(m).first, b, st), where);
+    } else if (bs) {
+        float4 *qb[2];
+        const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+        for (int a = 0; a < 2; ++a) {
+            JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &qb[a]), where);
+            JP_CUDA(cudaMemsetAsync(qb[a], 0, qbytes, st), where);
+            JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, qb[a], st, 1), where);
+        }
+        JP_CUDA(jp::launch_quad_merge(qb[0], qb[1], c.g, b, st), where);
+    } else {
+        float4 *q[2], *qb[2];
+        const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
+        for (int a = 0; a < 2; ++a) {
+            JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
+            JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &qb[a]), where);
+        }
+        JP_CUDA(jp::launch_quad_build(x, c.g, q[0], q[1], st), where);
+        for (int a = 0; a < 2; ++a) {
+            JP_CUDA(cudaMemsetAsync(qb[a], 0, qbytes, st), where);
+            JP_CUDA(jp::launch_osem_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), q[a], c.g, c.t, tc.lut, qb[a], st), where);
+        }
+        JP_CUDA(jp::launch_quad_merge(qb[0], qb[1], c.g, b, st), where);
+    }
     if (c.has_axis2(m)) {
         float *px = nullptr, *pb = nullptr;
         JP_CUDA(jp::padded_create(x, c.g, false, st, &px), where);

@@ -1,0 +1,932 @@
+// jp_brick.cu -- TOF listmode projections of SPARSE event sets on image BRICKS held in shared memory: the kernels
+// behind the planned listmode OSEM (BASELINE.json configs[4]) and the planned projections of sparsely populated lists.
+//
+// An OSEM subset of a listmode acquisition (40e6 events in 20 - 34 subsets) puts ~20 events on a
+// transaxial line, so nothing is shared along a line (the line tiles of jp_lm_tile.cu need hundreds), and a TOF event
+// only touches the ~46 planes around its TOF bin ("only affected by a few voxels"): its 4 gathers / 4 atomic
+// adds per plane land on random sectors of the 15 MB image.  Measured on B200 such a walk runs at the L1 gather rate
+// (one 128-byte line per clock and SM) and at the L2 atomic rate, whatever the order of the events.
+// But every voxel is still touched ~100 times per subset.  The reuse is spatial, not per line, so the image is cut into
+// bricks of kBrP x kBr1 x kBr2 cells (principal axis, other transaxial axis, axial) and every event into PIECES, the
+// maximal runs of consecutive planes whose interpolation cell lies in one brick (3.5 per event for 32 x 32 x 16).  The
+// plan (set-up, "pre-sorting") sorts the pieces of every subset by brick and length and stores, per piece,
+// the affine plane loop in BRICK-LOCAL coordinates (32 bytes, float64 set-up as in jp_ray.cuh).  A CTA takes a chunk of
+// <= kBrChunk pieces of one brick:
+//   forward   brick (+ one column of neighbours) -> shared memory; per piece  acc[event] += sum_k G(k) bilinear(k)
+//   adjoint   per piece  brick[cell] += cf y G(k) hat(k)  with native int32 shared atomics (fixed point, scale from the
+//             chunk's max |cf y|: an event adds to a voxel at most once, so a voxel receives <= kBrChunk terms), then
+//             the brick is flushed once with 128-bit REDs (north_star: shared-memory tile staging before global atomics).
+// Shared-memory gathers of 32 random banks cost ~3.5 wavefronts instead of 32 L1 wavefronts, and the L2 sees one RED per
+// 4 voxels and chunk instead of four per plane step.
+#include <cuda.h> // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked)
+
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
+
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "jp_g1tab.cuh"
+
+namespace jp {
+
+namespace {
+
+#ifndef JP_BR_P
+#define JP_BR_P 32
+#endif
+#ifndef JP_BR_1
+#define JP_BR_1 32
+#endif
+#ifndef JP_BR_2
+#define JP_BR_2 16
+#endif
+#ifndef JP_BR_CHUNK
+#define JP_BR_CHUNK 4096
+#endif
+#ifndef JP_BR_THREADS
+#define JP_BR_THREADS 768
+#endif
+#ifndef JP_BR_MINB
+#define JP_BR_MINB 2
+#endif
+constexpr int kBrP = JP_BR_P, kBr1 = JP_BR_1, kBr2 = JP_BR_2; // cells of a brick along p, q1, q2 (axial)
+// columns held per brick row: the cells, the bilinear neighbour (+1) and one safety column (the float32 plane loop may
+// land one cell above the cell the float64 set-up assigned to the brick; below is excluded by construction)
+constexpr int kBrC1 = kBr1 + 2, kBrC2 = kBr2 + 2;
+// cells are shifted before they are cut into bricks: local column c <-> voxel b kBr - kOff + c.  Along q1 one column of
+// padding is what cell -1 needs; along z four, so that every brick starts at a multiple of 4 voxels (16 bytes: the TMA
+// box of the forward kernel and the 128-bit REDs of the adjoint flush need that alignment)
+constexpr int kOff1 = 1, kOff2 = 4;
+constexpr int kBrRow = kBrC2;                 // elements per (plane, q1) row
+constexpr int kBrPlane = kBrC1 * kBrC2;       // elements per plane
+constexpr int kBrVox = kBrP * kBrPlane;       // elements per brick
+constexpr int kBrChunk = JP_BR_CHUNK;         // pieces per CTA
+constexpr int kBrT = JP_BR_THREADS;
+constexpr int kBrPer = (kBrChunk + kBrT - 1) / kBrT; // pieces per thread
+constexpr int kLenBits = 6;                   // key bits of the piece length (kBrP <= 64)
+static_assert(kBrP <= 64 && kBrP < 256, "piece length must fit its key / record field");
+static_assert(kBr2 % 4 == 0, "vector flush needs bricks aligned to 4 axial voxels");
+
+// one piece: planes k = 0 .. nk-1 of the brick-local loop
+//   u1(k) = a1 + b1 k, u2(k) = a2 + b2 k   cell (floor u1, floor u2) of brick plane pl0 + k, local column c <-> voxel
+//                                          b kBr - kOff + c
+//   x(k)  = x0 + dx k                      position in the G1 table (jp_g1tab.cuh)
+struct __align__(16) BrickPiece {
+    float a1, b1, a2, b2;
+    float x0, dx;
+    int pl_nk; // pl0 << 8 | nk
+    int ev;    // position of the event in the plan's sorted list
+};
+static_assert(sizeof(BrickPiece) == 32, "piece record is two 16-byte loads");
+
+struct __align__(8) BrickChunk {
+    int first, count;   // pieces [first, first + count) of the sorted piece list
+    short bp, b1, b2;   // brick coordinates
+    short axis;         // principal axis (0 or 1)
+    int mcount;         // the largest number of pieces of the chunk that touch one and the same voxel (k_brick_maxcount)
+    int pad;
+};
+
+// brick grid of the image for principal axis a: cells kk = k + kOff in [kOff - 1, n_q + kOff) along q1 / q2, planes [0, n_p)
+struct BrickGrid {
+    int nb[2][3];
+    int NB; // max over the axes of the number of bricks
+};
+
+BrickGrid brick_grid(const Geom &g)
+{
+    BrickGrid bg{};
+    for (int a = 0; a < 2; ++a) {
+        const int q1 = 1 - a;
+        bg.nb[a][0] = (g.n[a] + kBrP - 1) / kBrP;
+        bg.nb[a][1] = (g.n[q1] + kOff1 + kBr1 - 1) / kBr1;
+        bg.nb[a][2] = (g.n[2] + kOff2 + kBr2 - 1) / kBr2;
+        const int nb = bg.nb[a][0] * bg.nb[a][1] * bg.nb[a][2];
+        if (nb > bg.NB) bg.NB = nb;
+    }
+    return bg;
+}
+
+// ---- plan-time set-up of one event in float64 (same formulae and the same discrete decisions as ray_setup_pts) ----
+struct DRay {
+    int p;          // principal axis
+    int ilo, ihi;   // planes visited (closed segment rule, TOF window, crossing point strictly inside (-1, n) x (-1, n))
+    double A1, B1;  // u_q1(i) = A1 + B1 i, i the plane index
+    double A2, B2;
+    double tau0, dtau; // tau(i) = tau0 + dtau i
+    float cf;
+};
+
+__device__ bool dray_setup(const Lors &l, int64_t e, const int16_t *__restrict__ tb, const Geom &g, const Tof &t, DRay &R)
+{
+    const float centre = (float)tb[e] * t.width;
+    const float reach = 0.5f * t.width + t.nsig * t.sigma;
+    const double s[3] = {(double)l.xs[e], (double)l.ys[e], (double)l.zs[e]};
+    const double en[3] = {(double)l.xe[e], (double)l.ye[e], (double)l.ze[e]};
+    Ray r;
+    ray_setup_pts<true>(s, en, g, t.coff, centre - reach, centre + reach, r);
+    R.p = r.p;
+    R.cf = r.cf;
+    R.ilo = 0;
+    R.ihi = -1;
+    if (r.nk == 0 || r.p == 2) return false;
+    const int p = r.p, q1 = 1 - p;
+    const double d[3] = {en[0] - s[0], en[1] - s[1], en[2] - s[2]};
+    const double op = (double)g.o[p], vp = (double)g.v[p];
+    const double inv_dp = drcp(d[p]);
+    const double r1 = d[q1] * inv_dp, r2 = d[2] * inv_dp;
+    const double iv1 = drcp((double)g.v[q1]), iv2 = drcp((double)g.v[2]);
+    R.B1 = r1 * vp * iv1;
+    R.A1 = (s[q1] - (double)g.o[q1] + (op - s[p]) * r1) * iv1;
+    R.B2 = r2 * vp * iv2;
+    R.A2 = (s[2] - (double)g.o[2] + (op - s[p]) * r2) * iv2;
+    const double L = dsqrt_pos(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    R.dtau = vp * inv_dp * L;
+    R.tau0 = ((op - s[p]) * inv_dp - 0.5) * L - (double)t.coff;
+    // the clips of ray_setup are rounded outwards: drop end planes whose crossing point is not strictly inside
+    // (-1, n_q1) x (-1, n_2) (all four neighbours outside the image: they contribute exactly zero, reading A5)
+    const double n1 = (double)g.n[q1], n2 = (double)g.n[2];
+    int ilo = r.i0, ihi = r.i0 + r.nk - 1;
+    auto inside = [&](int i) {
+        const double u1 = fma(R.B1, (double)i, R.A1), u2 = fma(R.B2, (double)i, R.A2);
+        return u1 > -1.0 && u1 < n1 && u2 > -1.0 && u2 < n2;
+    };
+    while (ilo <= ihi && !inside(ilo)) ++ilo;
+    while (ihi >= ilo && !inside(ihi)) --ihi;
+    R.ilo = ilo;
+    R.ihi = ihi;
+    return ihi >= ilo;
+}
+
+__device__ __forceinline__ int dray_brick(const DRay &R, int i, const int (&nb)[3])
+{
+    const int bp = i / kBrP;
+    const int k1 = (int)floor(fma(R.B1, (double)i, R.A1) + (double)kOff1), k2 = (int)floor(fma(R.B2, (double)i, R.A2) + (double)kOff2);
+    return (bp * nb[1] + k1 / kBr1) * nb[2] + k2 / kBr2;
+}
+
+// pieces per event (0 for principal axis z and for events that miss the image / whose TOF window does), cf per event
+__global__ void __launch_bounds__(256) k_brick_count(Lors l, const int16_t *__restrict__ tb, int64_t n, Geom g, Tof t,
+                                                      BrickGrid bg, int *__restrict__ npieces, float *__restrict__ cf,
+                                                      unsigned long long *__restrict__ total)
+{
+    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int cnt = 0;
+    if (e < n) {
+        DRay R;
+        if (dray_setup(l, e, tb, g, t, R)) {
+            int prev = -1;
+            for (int i = R.ilo; i <= R.ihi; ++i) {
+                const int b = dray_brick(R, i, bg.nb[R.p]);
+                cnt += (b != prev);
+                prev = b;
+            }
+        }
+        npieces[e] = cnt;
+        cf[e] = R.cf;
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(total, (unsigned long long)cnt);
+}
+
+// sort key of a piece: ((subset * 2 + axis) * NB + brick) << kLenBits | (nk - 1); payload: (event, first plane, nk)
+__global__ void __launch_bounds__(256) k_brick_emit(Lors l, const int16_t *__restrict__ tb, int64_t first, int64_t count,
+                                                     int subset, Geom g, Tof t, BrickGrid bg, const int *__restrict__ offs,
+                                                     unsigned *__restrict__ keys, int *__restrict__ idx, int2 *__restrict__ payload)
+{
+    const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c >= count) return;
+    const int64_t e = first + c;
+    DRay R;
+    if (!dray_setup(l, e, tb, g, t, R)) return;
+    int at = offs[e];
+    int prev = dray_brick(R, R.ilo, bg.nb[R.p]), i0 = R.ilo;
+    const unsigned sab0 = (unsigned)(subset * 2 + R.p) * (unsigned)bg.NB;
+    for (int i = R.ilo + 1; i <= R.ihi + 1; ++i) {
+        const int b = (i <= R.ihi) ? dray_brick(R, i, bg.nb[R.p]) : -1;
+        if (b != prev) {
+            const int nk = i - i0;
+            keys[at] = ((sab0 + (unsigned)prev) << kLenBits) | (unsigned)(nk - 1);
+            idx[at] = at;
+            payload[at] = make_int2((int)e, (i0 << 8) | nk);
+            ++at;
+            prev = b;
+            i0 = i;
+        }
+    }
+}
+
+// first piece of every (subset, axis, brick) in the sorted list
+__global__ void __launch_bounds__(256) k_brick_bounds(const unsigned *__restrict__ keys, int64_t n, int *__restrict__ firsts)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const unsigned sab = keys[j] >> kLenBits;
+    if (j == 0 || (keys[j - 1] >> kLenBits) != sab) firsts[sab] = (int)j;
+}
+
+// records of the sorted pieces: the event's set-up again (float64), rebased to the piece's brick
+__global__ void __launch_bounds__(256) k_brick_records(Lors l, const int16_t *__restrict__ tb, Geom g, Tof t, BrickGrid bg,
+                                                        const unsigned *__restrict__ keys, const int *__restrict__ idx,
+                                                        const int2 *__restrict__ payload, int64_t n, float scale,
+                                                        BrickPiece *__restrict__ pieces)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const int2 pay = payload[idx[j]];
+    const int e = pay.x, i0 = pay.y >> 8, nk = pay.y & 0xff;
+    DRay R;
+    dray_setup(l, e, tb, g, t, R);
+    const int (&nb)[3] = bg.nb[R.p];
+    const int brick = (int)((keys[j] >> kLenBits) % (unsigned)bg.NB);
+    const int b2 = brick % nb[2], b1 = (brick / nb[2]) % nb[1], bp = brick / (nb[2] * nb[1]);
+    BrickPiece pc;
+    // local coordinates: column c <-> voxel b kBr - kOff + c, so u' = u + kOff - b kBr lies in [0, kBr) for the brick's cells
+    const double a1 = fma(R.B1, (double)i0, R.A1) + (double)kOff1 - (double)(b1 * kBr1);
+    const double a2 = fma(R.B2, (double)i0, R.A2) + (double)kOff2 - (double)(b2 * kBr2);
+    pc.b1 = (float)R.B1;
+    pc.b2 = (float)R.B2;
+    pc.a1 = fmaxf((float)a1, 0.f);
+    pc.a2 = fmaxf((float)a2, 0.f);
+    // the plane loop evaluates fmaf(b, k, a) in float32: keep its last plane (the other extreme of a monotone
+    // sequence) at or above 0 as well; the shift is a few ulp of a (<= 4e-6 voxel)
+    const float kl = (float)(nk - 1);
+    for (int it = 0; it < 64 && fmaf(pc.b1, kl, pc.a1) < 0.f; ++it) pc.a1 = nextafterf(pc.a1, 1e30f);
+    for (int it = 0; it < 64 && fmaf(pc.b2, kl, pc.a2) < 0.f; ++it) pc.a2 = nextafterf(pc.a2, 1e30f);
+    const double centre = (double)((float)tb[e] * t.width);
+    pc.x0 = (float)((centre - fma(R.dtau, (double)i0, R.tau0)) * (double)scale);
+    pc.dx = (float)(-R.dtau * (double)scale);
+    pc.pl_nk = ((i0 - bp * kBrP) << 8) | nk;
+    pc.ev = e;
+    pieces[j] = pc;
+}
+
+// ---- hot kernels ---------------------------------------------------------------------------------------------------
+template <int OFF>
+__device__ __forceinline__ float lds_f32(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(addr), "n"(OFF) : "memory");
+    return v;
+}
+
+template <int OFF>
+__device__ __forceinline__ void reds_add(uint32_t addr, int q)
+{
+    asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(q) : "memory");
+}
+
+struct BrickOrg {
+    int p, q1;
+    int sp, s1;            // element strides of the image along p and q1 (axial stride 1)
+    int i0, k1_0, k2_0;    // image indices of local (plane 0, column 0, column 0)
+    int np, n1, n2;
+};
+
+__device__ __forceinline__ BrickOrg brick_org(const BrickChunk &ch, const Geom &g)
+{
+    BrickOrg o;
+    o.p = ch.axis;
+    o.q1 = 1 - o.p;
+    const int s_x = g.n[1] * g.n[2], s_y = g.n[2];
+    o.sp = o.p == 0 ? s_x : s_y;
+    o.s1 = o.p == 0 ? s_y : s_x;
+    o.i0 = ch.bp * kBrP;
+    o.k1_0 = ch.b1 * kBr1 - kOff1;
+    o.k2_0 = ch.b2 * kBr2 - kOff2;
+    o.np = o.p == 0 ? g.n[0] : g.n[1];
+    o.n1 = o.p == 0 ? g.n[1] : g.n[0];
+    o.n2 = g.n[2];
+    return o;
+}
+
+// ---- forward -------------------------------------------------------------------------------------------------------
+// The brick is a 3-D box of the image: ONE TMA tile load (cp.async.bulk.tensor.3d) brings it into shared memory, the
+// hardware zero-fills whatever lies outside the image (reading A5), and no thread spends instructions or LSU wavefronts
+// on it.  Box rows are kFwRow floats (a multiple of 16 bytes).  The box follows the image's axis order, so the plane /
+// q1 strides of the shared copy depend on the principal axis: axis 0: [plane][q1][z], axis 1: [q1][plane][z].
+constexpr int kFwRow = (kBrC2 + 3) / 4 * 4;
+constexpr int kFwVox = kFwRow * kBrC1 * kBrP;
+
+__device__ __forceinline__ void mbar_init(uint32_t mbar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "JP_MBAR_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra JP_MBAR_WAIT_%=;\n"
+        "}\n" ::"r"(mbar), "r"(parity)
+        : "memory");
+}
+
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tm, int c0, int c1, int c2, uint32_t mbar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+                 "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(mbar)
+                 : "memory");
+}
+
+// the pieces of one chunk on the shared brick; SP / S1: element strides of a plane / a q1 row of the shared copy
+template <int SP, int S1>
+__device__ __forceinline__ void brick_fwd_pieces(const BrickChunk &ch, const BrickPiece *__restrict__ pieces, uint32_t bsm,
+                                                 uint32_t gbase, float xedge, int ev0, float *__restrict__ acc)
+{
+    const uint32_t bbase = bsm - (uint32_t)kMagicI * (uint32_t)((S1 + 1) * 4);
+    for (int j = threadIdx.x; j < ch.count; j += kBrT) {
+        const float4 *rec = reinterpret_cast<const float4 *>(pieces + ch.first + j);
+        const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);
+        const float a1 = r0.x, b1 = r0.y, a2 = r0.z, b2 = r0.w, x0 = r1.x, dx = r1.y;
+        const int pl_nk = __float_as_int(r1.z), ev = __float_as_int(r1.w);
+        const int nk = pl_nk & 0xff;
+        uint32_t row = bbase + (uint32_t)(pl_nk >> 8) * (uint32_t)(SP * 4);
+        float fk = 0.f, sum = 0.f;
+#pragma unroll 2
+        for (int k = 0; k < nk; ++k) {
+            const float u1 = fmaf(b1, fk, a1), u2 = fmaf(b2, fk, a2);
+            const float t1 = __fadd_rd(u1, kMagic), t2 = __fadd_rd(u2, kMagic);
+            const float w1 = u1 - (t1 - kMagic), w2 = u2 - (t2 - kMagic);
+            const uint32_t ad = row + __float_as_uint(t1) * (uint32_t)(S1 * 4) + (__float_as_uint(t2) << 2);
+            const float v00 = lds_f32<0>(ad), v01 = lds_f32<4>(ad);
+            const float v10 = lds_f32<S1 * 4>(ad), v11 = lds_f32<S1 * 4 + 4>(ad);
+            const float lo = fmaf(w2, v01 - v00, v00), hi = fmaf(w2, v11 - v10, v10);
+            const float wt = g1_weight(gbase, xedge, fmaf(dx, fk, x0));
+            sum = fmaf(fmaf(w1, hi - lo, lo), wt, sum);
+            fk += 1.f;
+            row += SP * 4;
+        }
+        atomicAdd(acc + (ev - ev0), sum);
+    }
+}
+
+// forward: acc[ev - ev0] += sum over the piece's planes of  G * bilinear  (the factor cf is applied per event later)
+__global__ void __launch_bounds__(kBrT, JP_BR_MINB)
+    k_brick_fwd(const __grid_constant__ CUtensorMap tm0, const __grid_constant__ CUtensorMap tm1, int use_tma,
+                const BrickChunk *__restrict__ chunks, const BrickPiece *__restrict__ pieces, const float *__restrict__ img,
+                Geom g, G1Tab gt, int ev0, float *__restrict__ acc)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float *B = reinterpret_cast<float *>(smem_raw);
+    float2 *g1 = reinterpret_cast<float2 *>(smem_raw + sizeof(float) * kFwVox);
+    __shared__ __align__(8) unsigned long long mbar_sm;
+    const int tid = threadIdx.x;
+    const BrickChunk ch = chunks[blockIdx.x];
+    const BrickOrg o = brick_org(ch, g);
+    const int SP = (o.p == 0) ? kBrC1 * kFwRow : kFwRow;  // element strides of the shared copy
+    const int S1 = (o.p == 0) ? kFwRow : kBrP * kFwRow;
+    const uint32_t mbar = smem_addr(&mbar_sm);
+    if (use_tma) {
+        if (tid == 0) mbar_init(mbar, 1);
+        __syncthreads();
+        if (tid == 0) {
+            mbar_expect_tx(mbar, (uint32_t)(sizeof(float) * kFwVox));
+            if (o.p == 0) tma_load_3d(smem_addr(B), &tm0, o.k2_0, o.k1_0, o.i0, mbar);
+            else tma_load_3d(smem_addr(B), &tm1, o.k2_0, o.i0, o.k1_0, mbar);
+        }
+    } else { // images the tensor map cannot describe (axial size not a multiple of 4, unaligned base)
+        for (int idx = tid; idx < kBrP * kBrC1 * kBrC2; idx += kBrT) {
+            const int c2 = idx % kBrC2, r = idx / kBrC2;
+            const int c1 = r % kBrC1, pl = r / kBrC1;
+            const int i = o.i0 + pl, k1 = o.k1_0 + c1, k2 = o.k2_0 + c2;
+            float v = 0.f;
+            if (i < o.np && (unsigned)k1 < (unsigned)o.n1 && (unsigned)k2 < (unsigned)o.n2)
+                v = __ldg(img + (int64_t)i * o.sp + (int64_t)k1 * o.s1 + k2);
+            B[pl * SP + c1 * S1 + c2] = v;
+        }
+    }
+    for (int i = tid; i < gt.n; i += kBrT) g1[i] = __ldg(gt.tab + i);
+    __syncthreads();
+    if (use_tma) mbar_wait(mbar, 0);
+    const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
+    // the strides are compile-time constants inside the loop (immediates): one instantiation per principal axis
+    if (o.p == 0) brick_fwd_pieces<kBrC1 * kFwRow, kFwRow>(ch, pieces, smem_addr(B), gbase, gt.xedge, ev0, acc);
+    else brick_fwd_pieces<kFwRow, kBrP * kFwRow>(ch, pieces, smem_addr(B), gbase, gt.xedge, ev0, acc);
+}
+
+// plan time: for every chunk the largest number of terms any voxel of its brick receives (a piece touches the four
+// neighbours of its cell on every plane).  It bounds the fixed-point sums of k_brick_back far below the worst case
+// "every piece of the chunk hits the same voxel", which buys the staging ~6 more bits.
+__global__ void __launch_bounds__(kBrT, JP_BR_MINB)
+    k_brick_maxcount(BrickChunk *__restrict__ chunks, const BrickPiece *__restrict__ pieces)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    int *B = reinterpret_cast<int *>(smem_raw);
+    __shared__ int red[kBrT / 32];
+    const int tid = threadIdx.x;
+    const BrickChunk ch = chunks[blockIdx.x];
+    for (int idx = tid; idx < kBrVox; idx += kBrT) B[idx] = 0;
+    __syncthreads();
+    const uint32_t bbase = smem_addr(B) - (uint32_t)kMagicI * (uint32_t)((kBrRow + 1) * 4);
+    for (int j = tid; j < ch.count; j += kBrT) {
+        const float4 *rec = reinterpret_cast<const float4 *>(pieces + ch.first + j);
+        const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);
+        const int pl_nk = __float_as_int(r1.z);
+        const int nk = pl_nk & 0xff;
+        uint32_t row = bbase + (uint32_t)(pl_nk >> 8) * (uint32_t)(kBrPlane * 4);
+        float fk = 0.f;
+        for (int k = 0; k < nk; ++k) {
+            const float t1 = __fadd_rd(fmaf(r0.y, fk, r0.x), kMagic), t2 = __fadd_rd(fmaf(r0.w, fk, r0.z), kMagic);
+            const uint32_t ad = row + __float_as_uint(t1) * (uint32_t)(kBrRow * 4) + (__float_as_uint(t2) << 2);
+            reds_add<0>(ad, 1);
+            reds_add<4>(ad, 1);
+            reds_add<kBrRow * 4>(ad, 1);
+            reds_add<kBrRow * 4 + 4>(ad, 1);
+            fk += 1.f;
+            row += kBrPlane * 4;
+        }
+    }
+    __syncthreads();
+    int mx = 0;
+    for (int idx = tid; idx < kBrVox; idx += kBrT) mx = max(mx, B[idx]);
+    for (int s = 16; s > 0; s >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+    if ((tid & 31) == 0) red[tid >> 5] = mx;
+    __syncthreads();
+    if (tid == 0) {
+        for (int w = 1; w < kBrT / 32; ++w) mx = max(mx, red[w]);
+        chunks[blockIdx.x].mcount = max(mx, 1);
+    }
+}
+
+// value scattered by event ev:  MODE 0: cf y[io]  (plain adjoint);  MODE 1: cf / (cf acc) if cf acc > 1e-9 else 0 (OSEM, A14)
+template <int MODE>
+__device__ __forceinline__ float brick_x(int ev, int ev0, const float *__restrict__ cf, const float *__restrict__ v,
+                                         const int *__restrict__ perm)
+{
+    const float c = __ldg(cf + ev);
+    if (MODE == 0) return c * __ldg(v + (perm ? (int64_t)__ldg(perm + ev) : (int64_t)(ev - ev0)));
+    const float ybar = c * __ldg(v + (ev - ev0));
+    return (ybar > 1e-9f) ? c * (1.f / ybar) : 0.f;
+}
+
+// Adjoint of one chunk.  The brick is staged in int32 fixed point (native shared atomics).  One scale per chunk must
+// serve every value in it, and OSEM ratios span decades (an event whose TOF window sits outside the activity has a tiny
+// expectation), so the scale is tied to the chunk's MEDIAN |x| (exponent histogram), not to its maximum:
+//   |x| <= T = 2^kBrHead * 2^ceil(log2 median)   fixed point with scale lim / T: quantum T / lim per term
+//   |x| >  T, Inf, NaN                           float atomics on the image, like the per-event path (exact, slow, rare)
+#ifndef JP_BR_HEAD
+#define JP_BR_HEAD 4
+#endif
+constexpr int kBrHead = JP_BR_HEAD;
+
+template <int MODE>
+__global__ void __launch_bounds__(kBrT, JP_BR_MINB)
+    k_brick_back(const BrickChunk *__restrict__ chunks, const BrickPiece *__restrict__ pieces, const float *__restrict__ cf,
+                 const float *__restrict__ v, const int *__restrict__ perm, Geom g, G1Tab gt, int ev0, float gmax, int vec_ok,
+                 float *__restrict__ img)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    int *B = reinterpret_cast<int *>(smem_raw);
+    float2 *g1 = reinterpret_cast<float2 *>(smem_raw + sizeof(int) * kBrVox);
+    __shared__ int hist[256];
+    __shared__ float T_sm;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const BrickChunk ch = chunks[blockIdx.x];
+    const BrickOrg o = brick_org(ch, g);
+    if (tid < 256) hist[tid] = 0;
+    for (int i = tid; i < gt.n; i += kBrT) g1[i] = __ldg(gt.tab + i);
+    for (int idx = tid; idx < kBrVox; idx += kBrT) B[idx] = 0;
+    __syncthreads();
+    // histogram of the float exponents of the chunk's values (zeros left out)
+#pragma unroll 1
+    for (int m = 0; m < kBrPer; ++m) {
+        const int j = tid + m * kBrT;
+        const float xj = (j < ch.count) ? brick_x<MODE>(pieces[ch.first + j].ev, ev0, cf, v, perm) : 0.f;
+        const int ex = (xj != 0.f) ? (int)((__float_as_uint(xj) >> 23) & 0xffu) : -1;
+        const unsigned peers = __match_any_sync(0xffffffffu, ex);
+        if (ex >= 0 && lane == __ffs(peers) - 1) atomicAdd(&hist[ex], __popc(peers));
+    }
+    __syncthreads();
+    if (tid < 32) { // median exponent: 8 bins per lane, scan over the lanes
+        int c[8], tot = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            c[k] = hist[tid * 8 + k];
+            tot += c[k];
+        }
+        int incl = tot;
+        for (int s = 1; s < 32; s <<= 1) {
+            const int up = __shfl_up_sync(0xffffffffu, incl, s);
+            if (tid >= s) incl += up;
+        }
+        const int all = __shfl_sync(0xffffffffu, incl, 31);
+        const int half = (all + 1) >> 1;
+        int run = incl - tot, emed = 256;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            run += c[k];
+            if (emed == 256 && run >= half && c[k] > 0) emed = tid * 8 + k;
+        }
+        for (int s = 16; s > 0; s >>= 1) emed = min(emed, __shfl_xor_sync(0xffffffffu, emed, s));
+        if (tid == 0) {
+            // 2^(emed - 127 + 1) bounds the median from above; an exponent near the top of the range leaves no head room
+            const int et = min(emed + 1 + kBrHead, 254);
+            T_sm = (all > 0 && emed < 255) ? __uint_as_float((unsigned)et << 23) : 0.f;
+        }
+    }
+    __syncthreads();
+    const float T = T_sm;
+    const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
+    const float xedge = gt.xedge;
+    // fixed point: a voxel receives at most ch.mcount terms (counted by the plan), each at most gmax lim in magnitude
+    // (gmax = G(0) >= every TOF weight, |x| <= T), plus one rounding unit per term
+    const float lim = fminf(1073741824.f, (2147483648.f - 2.f * (float)ch.mcount) / ((float)ch.mcount * gmax));
+    const float Sc = (T > 0.f) ? lim / T : 0.f, invS = (T > 0.f) ? T / lim : 0.f;
+    const uint32_t bbase = smem_addr(B) - (uint32_t)kMagicI * (uint32_t)((kBrRow + 1) * 4);
+#pragma unroll 1
+    for (int j = tid; j < ch.count; j += kBrT) {
+        const float4 *rec = reinterpret_cast<const float4 *>(pieces + ch.first + j);
+        const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);
+        const float a1 = r0.x, b1 = r0.y, a2 = r0.z, b2 = r0.w, x0 = r1.x, dx = r1.y;
+        const int pl_nk = __float_as_int(r1.z);
+        const int nk = pl_nk & 0xff, pl0 = pl_nk >> 8;
+        const float xj = brick_x<MODE>(__float_as_int(r1.w), ev0, cf, v, perm); // (again: cheaper than keeping it)
+        if (xj == 0.f) continue;
+        if (fabsf(xj) <= T) {
+            uint32_t row = bbase + (uint32_t)pl0 * (uint32_t)(kBrPlane * 4);
+            const float xs = xj * Sc;
+            float fk = 0.f;
+#pragma unroll 2
+            for (int k = 0; k < nk; ++k) {
+                const float u1 = fmaf(b1, fk, a1), u2 = fmaf(b2, fk, a2);
+                const float t1 = __fadd_rd(u1, kMagic), t2 = __fadd_rd(u2, kMagic);
+                const float w1 = u1 - (t1 - kMagic), w2 = u2 - (t2 - kMagic);
+                const uint32_t ad = row + __float_as_uint(t1) * (uint32_t)(kBrRow * 4) + (__float_as_uint(t2) << 2);
+                const float xw = xs * g1_weight(gbase, xedge, fmaf(dx, fk, x0));
+                const float xb = xw * w1, xa = xw - xb;
+                const float xa1 = xa * w2, xb1 = xb * w2;
+                reds_add<0>(ad, __float2int_rn(xa - xa1));
+                reds_add<4>(ad, __float2int_rn(xa1));
+                reds_add<kBrRow * 4>(ad, __float2int_rn(xb - xb1));
+                reds_add<kBrRow * 4 + 4>(ad, __float2int_rn(xb1));
+                fk += 1.f;
+                row += kBrPlane * 4;
+            }
+        } else { // far above the chunk's median, or not finite: float atomics on the image
+#pragma unroll 1
+            for (int k = 0; k < nk; ++k) {
+                const float fk = (float)k;
+                const float u1 = fmaf(b1, fk, a1), u2 = fmaf(b2, fk, a2);
+                const float f1 = floorf(u1), f2 = floorf(u2);
+                const float w1 = u1 - f1, w2 = u2 - f2;
+                const float w = g1_weight(gbase, xedge, fmaf(dx, fk, x0));
+                if (w == 0.f) continue;
+                const int i = o.i0 + pl0 + k, k1 = o.k1_0 + (int)f1, k2 = o.k2_0 + (int)f2;
+                float *ptr = img + (int64_t)i * o.sp + (int64_t)k1 * o.s1 + k2;
+                const float x = xj * w;
+                const float xa = x * (1.f - w1), xb = x * w1, m2 = 1.f - w2;
+                const bool in1a = (unsigned)k1 < (unsigned)o.n1, in1b = (unsigned)(k1 + 1) < (unsigned)o.n1;
+                const bool in2a = (unsigned)k2 < (unsigned)o.n2, in2b = (unsigned)(k2 + 1) < (unsigned)o.n2;
+                if (in1a && in2a) atomicAdd(ptr, xa * m2);
+                if (in1a && in2b) atomicAdd(ptr + 1, xa * w2);
+                if (in1b && in2a) atomicAdd(ptr + o.s1, xb * m2);
+                if (in1b && in2b) atomicAdd(ptr + o.s1 + 1, xb * w2);
+            }
+        }
+    }
+    __syncthreads();
+    if (!(T > 0.f)) return;
+    // ---- flush: per row kBr2 / 4 aligned groups of four voxels and the two columns beyond them
+    constexpr int kGroups = kBr2 / 4;
+    constexpr int kOps = kGroups + 2;
+    for (int op = tid; op < kBrP * kBrC1 * kOps; op += kBrT) {
+        const int gi = op % kOps, r = op / kOps;
+        const int c1 = r % kBrC1, pl = r / kBrC1;
+        const int i = o.i0 + pl, k1 = o.k1_0 + c1;
+        if (i >= o.np || (unsigned)k1 >= (unsigned)o.n1) continue;
+        const int *src = B + r * kBrRow;
+        float *dst = img + (int64_t)i * o.sp + (int64_t)k1 * o.s1 + o.k2_0;
+        if (gi >= kGroups) { // scalar columns kBr2 and kBr2 + 1
+            const int c2 = kBr2 + (gi - kGroups);
+            const int q = src[c2];
+            if (q != 0 && (unsigned)(o.k2_0 + c2) < (unsigned)o.n2) atomicAdd(dst + c2, (float)q * invS);
+        } else {
+            const int c2 = 4 * gi;
+            const int q0 = src[c2], q1 = src[c2 + 1], q2 = src[c2 + 2], q3 = src[c2 + 3];
+            if ((q0 | q1 | q2 | q3) == 0) continue;
+            const int k2 = o.k2_0 + c2;
+            if (vec_ok && k2 >= 0 && k2 + 3 < o.n2) {
+                atomicAdd(reinterpret_cast<float4 *>(dst + c2),
+                          make_float4((float)q0 * invS, (float)q1 * invS, (float)q2 * invS, (float)q3 * invS));
+            } else {
+                if (q0 != 0 && (unsigned)k2 < (unsigned)o.n2) atomicAdd(dst + c2, (float)q0 * invS);
+                if (q1 != 0 && (unsigned)(k2 + 1) < (unsigned)o.n2) atomicAdd(dst + c2 + 1, (float)q1 * invS);
+                if (q2 != 0 && (unsigned)(k2 + 2) < (unsigned)o.n2) atomicAdd(dst + c2 + 2, (float)q2 * invS);
+                if (q3 != 0 && (unsigned)(k2 + 3) < (unsigned)o.n2) atomicAdd(dst + c2 + 3, (float)q3 * invS);
+            }
+        }
+    }
+}
+
+// p[io] = cf acc  (MODE 0)  or the OSEM ratio 1 / (cf acc)  (MODE 1) for the events [first, first + count) of the sorted
+// list that have pieces (principal axis 0 / 1)
+__global__ void __launch_bounds__(256) k_brick_finish(const float *__restrict__ cf, const float *__restrict__ acc, int64_t first,
+                                                       int64_t count, int ev0, const int *__restrict__ perm, int64_t io_off,
+                                                       int mode, float *__restrict__ p)
+{
+    const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (c >= count) return;
+    const int64_t e = first + c;
+    float out = cf[e] * acc[e - ev0];
+    if (mode == 1) out = (out > 1e-9f) ? 1.f / out : 0.f;
+    p[perm ? (int64_t)perm[e] : c + io_off] = out;
+}
+
+constexpr size_t brick_smem(int g1n) { return sizeof(float) * (size_t)kBrVox + sizeof(float2) * (size_t)g1n; }
+constexpr size_t brick_smem_fwd(int g1n) { return sizeof(float) * (size_t)kFwVox + sizeof(float2) * (size_t)g1n; }
+
+} // namespace
+
+// ---- the brick set of a listmode plan --------------------------------------------------------------------------------
+struct BrickSet {
+    int64_t n_pieces = 0;
+    BrickPiece *pieces = nullptr;
+    BrickChunk *chunks = nullptr;
+    float *cf = nullptr;                       // [n] incidence factor of every sorted event
+    std::vector<int> chunk_first, chunk_count; // per subset
+    int g1n = 0;
+    float gmax = 1.f;
+};
+
+bool brick_supported(const Geom &g, const Tof &t, int n_subsets)
+{
+    const BrickGrid bg = brick_grid(g);
+    if (bg.NB > 32767) return false; // brick coordinates are stored as shorts
+    if ((uint64_t)n_subsets * 2u * (uint64_t)bg.NB >= ((uint64_t)1 << (32 - kLenBits))) return false;
+    if (g.n[0] >= (1 << 23) || g.n[1] >= (1 << 23)) return false;
+    if (brick_smem_fwd(g1tab_entries(t)) > 110 * 1024) return false; // two CTAs per SM
+    return true;
+}
+
+void brick_set_destroy(BrickSet *bs)
+{
+    if (!bs) return;
+    cudaFree(bs->pieces);
+    cudaFree(bs->chunks);
+    cudaFree(bs->cf);
+    delete bs;
+}
+
+int64_t brick_set_pieces(const BrickSet *bs) { return bs->n_pieces; }
+
+// l / tb: the plan's SORTED events (subset-major, then principal axis); sub_first[m], sub_count[m]: events of subset m.
+// Synchronises `st` (piece counts and the per-brick bounds are read back).  cudaErrorNotSupported: too many pieces.
+cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const Geom &g, const Tof &t, int n_subsets,
+                             const int64_t *sub_first, const int64_t *sub_count, cudaStream_t st, BrickSet **out)
+{
+    *out = nullptr;
+    if (!brick_supported(g, t, n_subsets)) return cudaErrorNotSupported;
+    BrickSet *bs = new BrickSet;
+    const BrickGrid bg = brick_grid(g);
+    bs->g1n = g1tab_entries(t);
+    {   // G(0): the largest TOF weight
+        const double m = (double)t.nsig * (double)t.sigma, h = 0.5 * (double)t.width;
+        bs->gmax = (float)(std::erf(std::fmin(h, m) / ((double)t.sigma * 1.4142135623730951)) * 1.0001);
+    }
+    bs->chunk_first.assign((size_t)n_subsets, 0);
+    bs->chunk_count.assign((size_t)n_subsets, 0);
+    *out = bs;
+    if (n == 0) return cudaSuccess;
+    cudaError_t e;
+    int *npieces = nullptr, *idx = nullptr, *idx2 = nullptr, *firsts = nullptr;
+    unsigned *keys = nullptr, *keys2 = nullptr;
+    int2 *payload = nullptr;
+    unsigned long long *total = nullptr;
+    void *tmp = nullptr;
+    size_t tmp_bytes = 0;
+    const size_t n_sab = (size_t)n_subsets * 2 * (size_t)bg.NB;
+    std::vector<int> h_firsts;
+    std::vector<BrickChunk> h_chunks;
+#define JP_BR_TRY(x)                     \
+    do {                                 \
+        e = (x);                         \
+        if (e != cudaSuccess) goto fail; \
+    } while (0)
+    JP_BR_TRY(cudaMalloc((void **)&bs->cf, sizeof(float) * (size_t)n));
+    JP_BR_TRY(cudaMallocAsync((void **)&npieces, sizeof(int) * (size_t)n, st));
+    JP_BR_TRY(cudaMallocAsync((void **)&total, sizeof(unsigned long long), st));
+    JP_BR_TRY(cudaMemsetAsync(total, 0, sizeof(unsigned long long), st));
+    {
+        const unsigned grid = (unsigned)((n + 255) / 256);
+        k_brick_count<<<grid, 256, 0, st>>>(l, tb, n, g, t, bg, npieces, bs->cf, total);
+        JP_BR_TRY(cudaGetLastError());
+        unsigned long long h_total = 0;
+        JP_BR_TRY(cudaMemcpyAsync(&h_total, total, sizeof(h_total), cudaMemcpyDeviceToHost, st));
+        JP_BR_TRY(cudaStreamSynchronize(st));
+        if (h_total >= ((unsigned long long)1 << 31)) {
+            e = cudaErrorNotSupported;
+            goto fail;
+        }
+        bs->n_pieces = (int64_t)h_total;
+    }
+    if (bs->n_pieces > 0) {
+        const int64_t np = bs->n_pieces;
+        JP_BR_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, npieces, npieces, (int)n, st));
+        JP_BR_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
+        JP_BR_TRY(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, npieces, npieces, (int)n, st));
+        JP_BR_TRY(cudaFreeAsync(tmp, st));
+        tmp = nullptr;
+        JP_BR_TRY(cudaMallocAsync((void **)&keys, sizeof(unsigned) * (size_t)np, st));
+        JP_BR_TRY(cudaMallocAsync((void **)&keys2, sizeof(unsigned) * (size_t)np, st));
+        JP_BR_TRY(cudaMallocAsync((void **)&idx, sizeof(int) * (size_t)np, st));
+        JP_BR_TRY(cudaMallocAsync((void **)&idx2, sizeof(int) * (size_t)np, st));
+        JP_BR_TRY(cudaMallocAsync((void **)&payload, sizeof(int2) * (size_t)np, st));
+        for (int m = 0; m < n_subsets; ++m) {
+            if (sub_count[m] == 0) continue;
+            const unsigned grid = (unsigned)((sub_count[m] + 255) / 256);
+            k_brick_emit<<<grid, 256, 0, st>>>(l, tb, sub_first[m], sub_count[m], m, g, t, bg, npieces, keys, idx, payload);
+            JP_BR_TRY(cudaGetLastError());
+        }
+        int key_bits = kLenBits;
+        while (((uint64_t)1 << key_bits) < ((uint64_t)n_sab << kLenBits)) ++key_bits;
+        JP_BR_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, idx2, (int)np, 0, key_bits, st));
+        JP_BR_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
+        JP_BR_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, idx, idx2, (int)np, 0, key_bits, st));
+        JP_BR_TRY(cudaMalloc((void **)&bs->pieces, sizeof(BrickPiece) * (size_t)np));
+        const unsigned pgrid = (unsigned)((np + 255) / 256);
+        k_brick_records<<<pgrid, 256, 0, st>>>(l, tb, g, t, bg, keys2, idx2, payload, np, (float)((double)kG1K / (double)t.width),
+                                               bs->pieces);
+        JP_BR_TRY(cudaGetLastError());
+        JP_BR_TRY(cudaMallocAsync((void **)&firsts, sizeof(int) * n_sab, st));
+        JP_BR_TRY(cudaMemsetAsync(firsts, 0xff, sizeof(int) * n_sab, st));
+        k_brick_bounds<<<pgrid, 256, 0, st>>>(keys2, np, firsts);
+        JP_BR_TRY(cudaGetLastError());
+        h_firsts.resize(n_sab);
+        JP_BR_TRY(cudaMemcpyAsync(h_firsts.data(), firsts, sizeof(int) * n_sab, cudaMemcpyDeviceToHost, st));
+        JP_BR_TRY(cudaStreamSynchronize(st));
+        // chunks: every (subset, axis, brick) run of the sorted pieces, cut into slices of <= kBrChunk pieces
+        int64_t next = np;
+        std::vector<int64_t> h_count(n_sab, 0);
+        for (size_t s = n_sab; s-- > 0;)
+            if (h_firsts[s] >= 0) {
+                h_count[s] = next - h_firsts[s];
+                next = h_firsts[s];
+            }
+        for (int m = 0; m < n_subsets; ++m) {
+            bs->chunk_first[(size_t)m] = (int)h_chunks.size();
+            for (int a = 0; a < 2; ++a)
+                for (int b = 0; b < bg.NB; ++b) {
+                    const size_t s = ((size_t)m * 2 + a) * (size_t)bg.NB + b;
+                    if (h_count[s] == 0) continue;
+                    const int (&nb)[3] = bg.nb[a];
+                    for (int64_t at = 0; at < h_count[s]; at += kBrChunk) {
+                        BrickChunk c;
+                        c.first = (int)(h_firsts[s] + at);
+                        c.count = (int)std::min<int64_t>(kBrChunk, h_count[s] - at);
+                        c.b2 = (short)(b % nb[2]);
+                        c.b1 = (short)((b / nb[2]) % nb[1]);
+                        c.bp = (short)(b / (nb[2] * nb[1]));
+                        c.axis = (short)a;
+                        c.mcount = c.count;
+                        c.pad = 0;
+                        h_chunks.push_back(c);
+                    }
+                }
+            bs->chunk_count[(size_t)m] = (int)h_chunks.size() - bs->chunk_first[(size_t)m];
+        }
+        if (!h_chunks.empty()) {
+            JP_BR_TRY(cudaMalloc((void **)&bs->chunks, sizeof(BrickChunk) * h_chunks.size()));
+            JP_BR_TRY(cudaMemcpyAsync(bs->chunks, h_chunks.data(), sizeof(BrickChunk) * h_chunks.size(), cudaMemcpyHostToDevice, st));
+            JP_BR_TRY(cudaFuncSetAttribute(k_brick_maxcount, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
+            k_brick_maxcount<<<(unsigned)h_chunks.size(), kBrT, sizeof(int) * kBrVox, st>>>(bs->chunks, bs->pieces);
+            JP_BR_TRY(cudaGetLastError());
+            JP_BR_TRY(cudaStreamSynchronize(st)); // h_chunks goes out of scope
+        }
+    }
+    e = cudaSuccess;
+fail:
+    if (tmp) cudaFreeAsync(tmp, st);
+    if (firsts) cudaFreeAsync(firsts, st);
+    if (payload) cudaFreeAsync(payload, st);
+    if (idx2) cudaFreeAsync(idx2, st);
+    if (idx) cudaFreeAsync(idx, st);
+    if (keys2) cudaFreeAsync(keys2, st);
+    if (keys) cudaFreeAsync(keys, st);
+    if (total) cudaFreeAsync(total, st);
+    if (npieces) cudaFreeAsync(npieces, st);
+    if (e != cudaSuccess) {
+        brick_set_destroy(bs);
+        *out = nullptr;
+    }
+    return e;
+#undef JP_BR_TRY
+}
+
+const float *brick_set_cf(const BrickSet *bs) { return bs->cf; }
+
+static cudaError_t brick_attr()
+{
+    static bool done = false; // idempotent; a race only repeats the calls
+    if (done) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_brick_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_brick_back<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_brick_back<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    if (e == cudaSuccess) done = true;
+    return e;
+}
+
+// acc[e - ev0] += sum_k G bilinear over the pieces of subset m (acc: zeroed by the caller, one float per event of the
+// subset, ev0 = position of the subset's first event in the sorted list)
+// tensor maps of the image for the brick boxes of principal axis 0 / 1; false: the image cannot be described (the
+// kernel then loads the brick with plain loads)
+static bool brick_tensor_maps(const float *img, const Geom &g, CUtensorMap *tm0, CUtensorMap *tm1)
+{
+    typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    static bool looked = false;
+    if (!looked) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            encode = reinterpret_cast<EncodeFn>(fn);
+        else
+            (void)cudaGetLastError();
+        looked = true;
+    }
+    if (!encode || g.n[2] % 4 != 0 || (uintptr_t)img % 16 != 0) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)g.n[2], (cuuint64_t)g.n[1], (cuuint64_t)g.n[0]};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.n[2] * 4u, (cuuint64_t)g.n[1] * (cuuint64_t)g.n[2] * 4u};
+    const cuuint32_t es[3] = {1, 1, 1};
+    const cuuint32_t box0[3] = {(cuuint32_t)kFwRow, (cuuint32_t)kBrC1, (cuuint32_t)kBrP}; // principal axis 0: q1 = axis 1
+    const cuuint32_t box1[3] = {(cuuint32_t)kFwRow, (cuuint32_t)kBrP, (cuuint32_t)kBrC1}; // principal axis 1: q1 = axis 0
+    void *base = const_cast<float *>(img);
+    if (encode(tm0, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, dims, strides, box0, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    if (encode(tm1, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, dims, strides, box1, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    return true;
+}
+
+// acc[e - ev0] += sum_k G bilinear over the pieces of subset m (acc: zeroed by the caller, one float per event of the
+// subset, ev0 = position of the subset's first event in the sorted list)
+cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const Geom &g, const Tof &t, int64_t ev0, float *acc,
+                             cudaStream_t st)
+{
+    const int nc = bs->chunk_count[(size_t)m];
+    if (nc == 0) return cudaSuccess;
+    cudaError_t e = brick_attr();
+    if (e != cudaSuccess) return e;
+    G1Tab gt{};
+    e = g1tab_create(t, bs->g1n, st, &gt);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tm0, tm1;
+    memset(&tm0, 0, sizeof(tm0));
+    memset(&tm1, 0, sizeof(tm1));
+    const int use_tma = brick_tensor_maps(img, g, &tm0, &tm1) ? 1 : 0;
+    k_brick_fwd<<<(unsigned)nc, kBrT, brick_smem_fwd(bs->g1n), st>>>(tm0, tm1, use_tma, bs->chunks + bs->chunk_first[(size_t)m],
+                                                                    bs->pieces, img, g, gt, (int)ev0, acc);
+    e = cudaGetLastError();
+    cudaFreeAsync((void *)gt.tab, st);
+    return e;
+}
+
+// img += A_m^T x over the events with pieces.  mode 0: x = cf v[io] (v = y; io = perm[e] or e - ev0);
+// mode 1: v = acc of launch_brick_fwd, x = cf / (cf acc) if cf acc > 1e-9 else 0 (the OSEM ratio, reading A14)
+cudaError_t launch_brick_back(const BrickSet *bs, int m, int mode, const float *v, const int *perm, const Geom &g, const Tof &t,
+                              int64_t ev0, float *img, cudaStream_t st)
+{
+    const int nc = bs->chunk_count[(size_t)m];
+    if (nc == 0) return cudaSuccess;
+    cudaError_t e = brick_attr();
+    if (e != cudaSuccess) return e;
+    G1Tab gt{};
+    e = g1tab_create(t, bs->g1n, st, &gt);
+    if (e != cudaSuccess) return e;
+    const int vec_ok = (g.n[2] % 4 == 0) && ((uintptr_t)img % 16 == 0);
+    const BrickChunk *ch = bs->chunks + bs->chunk_first[(size_t)m];
+    const size_t smem = brick_smem(bs->g1n);
+    if (mode == 1)
+        k_brick_back<1><<<(unsigned)nc, kBrT, smem, st>>>(ch, bs->pieces, bs->cf, v, nullptr, g, gt, (int)ev0, bs->gmax, vec_ok, img);
+    else
+        k_brick_back<0><<<(unsigned)nc, kBrT, smem, st>>>(ch, bs->pieces, bs->cf, v, perm, g, gt, (int)ev0, bs->gmax, vec_ok, img);
+    e = cudaGetLastError();
+    cudaFreeAsync((void *)gt.tab, st);
+    return e;
+}
+
+cudaError_t launch_brick_finish(const BrickSet *bs, const float *acc, int64_t first, int64_t count, int64_t ev0, const int *perm,
+                                int64_t io_off, int mode, float *p, cudaStream_t st)
+{
+    if (count == 0) return cudaSuccess;
+    k_brick_finish<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(bs->cf, acc, first, count, (int)ev0, perm, io_off, mode, p);
+    return cudaGetLastError();
+}
+
+} // namespace jp

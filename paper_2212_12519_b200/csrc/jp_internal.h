@@ -99,8 +99,9 @@ cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range r
 // forward + ratio + back of one OSEM subset in one pass (quad image in, quad accumulator out)
 cudaError_t launch_osem_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float4 *q, const Geom &g,
                                     const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
+// y_mode 1: y holds the forward sums without the factor cf; the OSEM ratio 1 / (cf y) is back projected
 cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
-                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st, int y_mode = 0);
 
 // TOF listmode on line tiles (jp_lm_tile.cu): events [first, first + count) of a SORTED list; outputs / inputs at
 // perm[e] (perm != null) or io_off + e - first; cudaErrorNotSupported: image too wide for the tiled kernels
@@ -137,6 +138,24 @@ cudaError_t lm_plan_back_tof(LmPlan *pl, int subset, const float *y, float *img,
 cudaError_t lm_plan_permute(const LmPlan *pl, const float *in, float *out, bool to_plan_order, cudaStream_t st);
 // persistent quad scratch of the plan (allocated on first use): which = 0,1: Q0,Q1; 2,3: B0,B1
 cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out);
+
+// listmode bricks (jp_brick.cu): the events of every subset cut into pieces per image brick, see the file header
+struct BrickSet;
+bool brick_supported(const Geom &g, const Tof &t, int n_subsets);
+cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const Geom &g, const Tof &t, int n_subsets,
+                             const int64_t *sub_first, const int64_t *sub_count, cudaStream_t st, BrickSet **out);
+void brick_set_destroy(BrickSet *bs);
+int64_t brick_set_pieces(const BrickSet *bs);
+cudaError_t lm_plan_bricks(LmPlan *pl, cudaStream_t st, const BrickSet **out);
+// acc[e - ev0] += sum_k G(k) bilinear(k) over the pieces of subset m (ev0: sorted position of the subset's first event)
+cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const Geom &g, const Tof &t, int64_t ev0, float *acc,
+                             cudaStream_t st);
+// img += A_m^T x.  mode 0: x = cf v[perm ? perm[e] : e - ev0];  mode 1: v = acc, x = cf / (cf acc) if cf acc > 1e-9 else 0
+cudaError_t launch_brick_back(const BrickSet *bs, int m, int mode, const float *v, const int *perm, const Geom &g, const Tof &t,
+                              int64_t ev0, float *img, cudaStream_t st);
+// p[perm ? perm[e] : e - first + io_off] = cf acc[e - ev0] (mode 0) or its OSEM ratio (mode 1), e in [first, first + count)
+cudaError_t launch_brick_finish(const BrickSet *bs, const float *acc, int64_t first, int64_t count, int64_t ev0, const int *perm,
+                                int64_t io_off, int mode, float *p, cudaStream_t st);
 
 // sinogram plan (jp_sino_plan.cu): a LOR list analysed once.  REGULAR = K tracks of T LORs each (a track: identical
 // transaxial end points) that all share ONE axial pattern (zs, ze)[T] -- every sinogram of a ring scanner.  A regular

@@ -18,6 +18,7 @@
 // canonically ordered transaxial end points) and processes run after run; an event given as (e, s) instead of
 // (s, e) is walked in the canonical orientation with its axial end points swapped and its TOF centre negated
 // (the kernel is even).  Runs shorter than kMinRun, and events whose principal axis is z, take the per-LOR path.
+#include "jp_g1tab.cuh"
 #include "jp_tile_common.cuh"
 
 namespace jp {
@@ -35,7 +36,6 @@ namespace {
 #ifndef JP_LMT_MINB_BACK
 #define JP_LMT_MINB_BACK 5
 #endif
-constexpr int kG1K = 512;   // table intervals per TOF bin width
 constexpr int kMinRun = 48; // shorter runs are not worth a row build
 
 // The table runs in the DISTANCE FROM THE SUPPORT EDGE, x' = R - |x| (bin widths, R = n_sigmas sigma / W + 1/2): the two
@@ -53,12 +53,6 @@ __global__ void k_tof_g1tab(float2 *tab, int n, double W, double m, double isc)
     tab[k] = make_float2((float)(g0 - (double)k * (g1 - g0)), (float)(g1 - g0)); // (intercept, slope): G = .x + x' .y
 }
 
-struct G1Tab {
-    const float2 *tab; // device, n entries; entry k = (intercept, slope) of G on x' in [k, k+1] / kG1K
-    int n;
-    float scale; // kG1K / W: mm -> table units
-    float xedge; // R kG1K: table position of the support edge
-};
 
 // canonical orientation of the transaxial end points: start = the lexicographically smaller (x, y)
 __device__ __forceinline__ bool is_swapped(float xs, float ys, float xe, float ye)
@@ -66,14 +60,6 @@ __device__ __forceinline__ bool is_swapped(float xs, float ys, float xe, float y
     return !((xs < xe) || (xs == xe && ys <= ye));
 }
 
-// weight of the event's bin at table position xs (table units, any sign)
-__device__ __forceinline__ float g1_weight(uint32_t gbase, float xedge, float xs)
-{
-    const float xa = fmaxf(xedge - fabsf(xs), 0.f);
-    const float tt = __fadd_rd(xa, kMagic);
-    const float2 v = lds_pair<0>(gbase + (__float_as_uint(tt) << 3));
-    return fmaf(xa, v.y, v.x);
-}
 
 // per-event axial + TOF part on track t (canonical orientation)
 struct LmRay {
@@ -688,8 +674,7 @@ LmTileCfg lm_tile_cfg(const Geom &g, const Tof &t, const void *img, size_t elem,
     for (int P : pitches)
         if (need <= P) { c.P = P; break; }
     if (!c.P) return c;
-    const double R = (double)t.nsig * (double)t.sigma / (double)t.width + 0.5;
-    c.g1n = (int)ceil(R * kG1K) + 3;
+    c.g1n = g1tab_entries(t);
     const int np = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
     const size_t fixed = (size_t)np * sizeof(RowInfo) + (size_t)c.g1n * sizeof(float2);
     const size_t row = (size_t)c.P * elem;
@@ -714,8 +699,6 @@ bool lm_tile_supported(const Geom &g, const Tof &t_in, bool tof)
            lm_tile_cfg(g, t, nullptr, sizeof(int), JP_LMT_SMEM_KB_BACK * 1024).P != 0;
 }
 
-namespace {
-
 cudaError_t g1tab_create(const Tof &t, int n, cudaStream_t st, G1Tab *out)
 {
     float2 *tab = nullptr;
@@ -734,8 +717,6 @@ cudaError_t g1tab_create(const Tof &t, int n, cudaStream_t st, G1Tab *out)
     out->xedge = (float)(((double)t.nsig * (double)t.sigma / (double)t.width + 0.5) * kG1K);
     return cudaSuccess;
 }
-
-} // namespace
 
 #define JP_LM_DISPATCH_P(CFG, ...)                           \
     switch ((CFG).P) {                                       \

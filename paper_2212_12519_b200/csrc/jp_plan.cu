@@ -139,6 +139,8 @@ struct LmPlan {
     int *perm = nullptr;    // sorted position -> caller index
     std::vector<int64_t> seg_first, seg_count; // [n_subsets][4]: run of (subset, principal axis) in the sorted list
     float4 *quad[4] = {nullptr, nullptr, nullptr, nullptr}; // Q0, Q1, B0, B1 (allocated on first use)
+    BrickSet *bricks = nullptr; // pieces of the events per image brick (jp_brick.cu), built by lm_plan_bricks
+    bool bricks_tried = false;  // a failed build is not repeated
 };
 
 static int bits_for(int v)
@@ -237,6 +239,7 @@ void lm_plan_destroy(LmPlan *pl)
     cudaFree(pl->tb);
     cudaFree(pl->perm);
     for (float4 *q : pl->quad) cudaFree(q);
+    brick_set_destroy(pl->bricks);
     delete pl;
 }
 
@@ -253,6 +256,29 @@ cudaError_t lm_plan_quad(LmPlan *pl, int which, float4 **out)
         if (e != cudaSuccess) return e;
     }
     *out = pl->quad[which];
+    return cudaSuccess;
+}
+
+// the plan's brick set, built on first use (allocates and synchronises `st`); *out = null when the image / TOF kernel /
+// event count is outside what the brick kernels take (the callers then use the quad path)
+cudaError_t lm_plan_bricks(LmPlan *pl, cudaStream_t st, const BrickSet **out)
+{
+    *out = nullptr;
+    if (!pl->bricks && !pl->bricks_tried) {
+        pl->bricks_tried = true;
+        std::vector<int64_t> first((size_t)pl->n_subsets), count((size_t)pl->n_subsets);
+        Lors l;
+        const int16_t *tb;
+        Range rg;
+        for (int m = 0; m < pl->n_subsets; ++m) {
+            lm_plan_view(pl, m, true, &l, &tb, &rg);
+            first[(size_t)m] = rg.first;
+            count[(size_t)m] = rg.count;
+        }
+        const cudaError_t e = brick_set_create(l, tb, pl->n, pl->g, pl->t, pl->n_subsets, first.data(), count.data(), st, &pl->bricks);
+        if (e != cudaSuccess && e != cudaErrorNotSupported) return e;
+    }
+    *out = pl->bricks;
     return cudaSuccess;
 }
 

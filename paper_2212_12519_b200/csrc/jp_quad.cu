@@ -144,6 +144,9 @@ __global__ void __launch_bounds__(kQBlock) k_fwd_tof_lm_quad(Lors l, const int16
     p[q_io_index(rg, c)] = out;
 }
 
+// Y_MODE 0: y = the values to back project;  1: y = sum_k G bilinear of every event (the forward projection without
+// its factor cf, e.g. from the brick kernels) and the OSEM ratio 1 / (cf y) if cf y > 1e-9 else 0 is back projected (A14)
+template <int Y_MODE>
 __global__ void __launch_bounds__(kQBlock) k_back_tof_lm_quad(Lors l, const int16_t *__restrict__ tofbin, Range rg,
                                                               const float *__restrict__ y, Geom g, Tof t, TofLut lut,
                                                               float4 *__restrict__ b)
@@ -155,7 +158,7 @@ __global__ void __launch_bounds__(kQBlock) k_back_tof_lm_quad(Lors l, const int1
     const int64_t c = blockIdx.x * (int64_t)kQBlock + threadIdx.x;
     if (c >= rg.count) return;
     const int64_t j = rg.first + c * rg.stride;
-    const float yj = y[q_io_index(rg, c)];
+    float yj = y[q_io_index(rg, c)];
     if (yj == 0.f) return;
     const float half_w = 0.5f * t.width;
     const float centre = (float)tofbin[j] * t.width;
@@ -163,6 +166,11 @@ __global__ void __launch_bounds__(kQBlock) k_back_tof_lm_quad(Lors l, const int1
     Ray r;
     ray_setup<true>(l, j, g, t.coff, centre - reach, centre + reach, r);
     const PRay pr = pray_from(r, g);
+    if (Y_MODE == 1) {
+        const float ybar = pr.cf * yj;
+        if (!(ybar > 1e-9f)) return;
+        yj = 1.f / ybar;
+    }
     const float x = pr.cf * yj;
     float fk = 0.f;
     int po = pr.off;
@@ -260,10 +268,13 @@ cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range r
 }
 
 cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
-                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st)
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st, int y_mode)
 {
     if (rg.count == 0) return cudaSuccess;
-    k_back_tof_lm_quad<<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, b);
+    if (y_mode == 1)
+        k_back_tof_lm_quad<1><<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, b);
+    else
+        k_back_tof_lm_quad<0><<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, b);
     return cudaGetLastError();
 }
 

@@ -272,13 +272,20 @@ def test_config3_plan_sorted_events(cuda_device, scanner, events):
     counts = [plan.subset_count(m) for m in range(7)]
     assert counts == [len(range(m, n, 7)) for m in range(7)] and plan.subset_count(-1) == n
     p_ref = jp.jp_fwd_tof_lm(xsd, xed, tbd, imgd, g.origin, g.voxsize, tof)
-    p_all = jp.jp_fwd_tof_lm_planned(plan, imgd)
-    assert torch.equal(p_all, p_ref)          # same arithmetic per event, only the order differs
-    # one subset: only its events are written
-    p_sub = jp.jp_fwd_tof_lm_planned(plan, imgd, subset=3, out=torch.full((n,), -1.0, device=cuda_device))
     mask = torch.zeros(n, dtype=torch.bool, device=cuda_device)
     mask[3::7] = True
+    # the plan's own choice for this list (sparsely populated lines: image bricks, another TOF table and summation
+    # order than the per-event kernels): equal within float32 rounding
+    p_all = jp.jp_fwd_tof_lm_planned(plan, imgd)
+    assert float((p_all - p_ref).abs().max()) <= 1e-5 * float(p_ref.max())
+    p_sub = jp.jp_fwd_tof_lm_planned(plan, imgd, subset=3, out=torch.full((n,), -1.0, device=cuda_device))
+    assert float((p_sub[mask] - p_ref[mask]).abs().max()) <= 1e-5 * float(p_ref.max()) and bool((p_sub[~mask] == -1.0).all())
+    # quad image: same arithmetic per event as the unplanned kernels, only the order differs -> bit for bit
+    plan.set_path(2)
+    assert torch.equal(jp.jp_fwd_tof_lm_planned(plan, imgd), p_ref)
+    p_sub = jp.jp_fwd_tof_lm_planned(plan, imgd, subset=3, out=torch.full((n,), -1.0, device=cuda_device))
     assert torch.equal(p_sub[mask], p_ref[mask]) and bool((p_sub[~mask] == -1.0).all())
+    plan.set_path(0)
     # adjoint: subsets add up to the whole, and the whole matches the oracle
     y = inputs.uniform_values(n, 0.5, 2.0, seed=13).to(cuda_device)
     b_all = jp.jp_back_tof_lm_planned(plan, y)
@@ -344,7 +351,9 @@ def test_lm_line_tiles(cuda_device, scanner, n_subsets):
     plan.destroy()
 
 
-def test_config4_small_osem_planned(cuda_device, scanner, events):
+@pytest.mark.parametrize("path", [0, 2, 3])
+def test_config4_small_osem_planned(cuda_device, scanner, events, path):
+    """listmode OSEM on a plan: 0 = the plan's own choice, 2 = quad image, 3 = image bricks (jp_brick.cu)"""
     g, ph = scanner
     xs, xe, tb = events
     tofp = inputs.TofParams()
@@ -357,7 +366,7 @@ def test_config4_small_osem_planned(cuda_device, scanner, events):
     ref = oracle.lm_osem(xs.numpy(), xe.numpy(), tb.numpy(), sens32.astype(np.float64), x0, g.origin, g.voxsize,
                          *args, n_subsets=5, n_iter=2)
     plan = jp.LmPlan(xs.to(cuda_device), xe.to(cuda_device), tb.to(cuda_device), g.n, g.origin, g.voxsize, tof,
-                     n_subsets=5)
+                     n_subsets=5).set_path(path)
     img = dev(x0, cuda_device).clone()
     jp.jp_lm_osem_planned(plan, dev(sens32, cuda_device), img, n_iter=2)
     got = img.cpu().numpy().astype(np.float64)
