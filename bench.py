@@ -357,7 +357,8 @@ class Workload:
             else:
                 self.sens = torch.ones(G.n, dtype=torch.float32, device=dev)   # replaced by A^T 1 in setup_sens()
                 self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
-                self.launches = 4 * 20 + 1   # per subset: quad build, fused projector per axis (x, y), update
+                # per subset: TOF weight table, brick forward, float-atomic adjoint per axis (x, y), update; + one edge table
+                self.launches = 5 * 20 + 1
 
     def make_sino_plan(self):
         """sinogram plan of the workload's LOR list (set-up, timed separately: `plan_s`); JP_BENCH_UNPLANNED=1 in the
@@ -515,6 +516,27 @@ class Workload:
             out[name] = {"fwd_ms": fm, "back_ms": bm, "fwd_plane_steps_per_s": steps / fm * 1e3,
                          "back_plane_steps_per_s": steps / bm * 1e3}
         plan.destroy()
+        return out
+
+    def time_osem_paths(self, iters=3):
+        """A/B of the kernels behind one OSEM iteration (jp_lm_plan_set_path): 2 = quad image both ways (round 1),
+        3 = image bricks forward + float atomics back (what the plan chooses, the timed configuration), 4 = bricks both
+        ways (adjoint staged in shared memory in fixed point; opt-in, see include/joseph_b200.h); ms per iteration"""
+        out = {}
+        for path, name in ((2, "quad_both_ways"), (3, "bricks_forward_float_adjoint"), (4, "bricks_both_ways_staged_adjoint")):
+            self.plan.set_path(path)
+            self.x.fill_(1.0)
+            self.jp.jp_lm_osem_planned(self.plan, self.sens, self.x, n_iter=1)
+            ts = []
+            for _ in range(iters):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(self.stream)
+                self.jp.jp_lm_osem_planned(self.plan, self.sens, self.x, n_iter=1)
+                e1.record(self.stream)
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            out[name] = {"ms_per_iteration": float(np.median(ts)), "min_ms": float(min(ts))}
+        self.plan.set_path(0)
         return out
 
     def time_osem_with_resolution_model(self, iters=2):
@@ -726,7 +748,8 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     names = {0: ("k_fwd_tile (per-LOR path: random chords are not tracks)", "k_back_tile (per-LOR path)"),
              1: ("k_fwd_tile<104, plan>", "k_back_tile<104, plan>") if planned else ("k_fwd_tile<104, list>", "k_back_tile<104, list>"),
              2: ("k_tof_sino_tile<6,fwd>", "k_tof_sino_tile<6,back>") if planned else ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
-             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"), 4: ("k_osem_tof_lm_quad (forward + ratio + back per event)", ""),
+             3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"),
+             4: ("k_brick_fwd (forward sums on TMA-loaded image bricks) + k_back_tof_lm_quad<ratio> (float atomics)", ""),
              5: ("k_tof_sino_tile<6,osem> (forward + ratio + back per track slice)" if planned else
                  "k_tof_sino_osem<6> (forward + ratio + back per LOR block)", "")}[w.c]
     src = (f"148 SMs x 128 FP32 lanes x {sm_mhz:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {peak_src})")
@@ -857,7 +880,8 @@ def run_ours(args):
                     "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                     "config": {"workload": SPEC[4]["workload"] + "; events sharded over the ranks (SURVEY.md 8(e))",
                                "parallelism": f"event shards x{world}", "l2": SPEC[4]["l2"]},
-                    "gpu_launches": (4 * 20 + 1 + 20) * args.steps, "s_per_iteration": ms * 1e-3, "sharded": info}
+                    # per subset: 2 tables, brick forward, adjoint per axis, quad merge, update
+                    "gpu_launches": 8 * 20 * args.steps, "s_per_iteration": ms * 1e-3, "sharded": info}
             print(json.dumps(line), flush=True)
         if world > 1:
             dist.destroy_process_group()
@@ -949,6 +973,7 @@ def run_ours(args):
         line["s_per_iteration"] = ms_per_step * 1e-3
     if c == 4:
         line["s_per_iteration_with_resolution_model"] = w.time_osem_with_resolution_model()
+        line["osem_paths"] = w.time_osem_paths()
     if e2e_s is not None:
         line["e2e"] = {"value": world * w.n / e2e_s, "unit": SPEC[c]["unit"], "h2d_bytes_per_step": w.h2d,
                        "d2h_bytes_per_step": w.d2h, "ms_per_step": e2e_s * 1e3, "api": w.e2e_api,
@@ -976,6 +1001,7 @@ def run_ours(args):
             elif oc == 4:
                 d["s_per_iteration"] = t_ms / nb * 1e-3
                 d["s_per_iteration_with_resolution_model"] = ow.time_osem_with_resolution_model()
+                d["osem_paths"] = ow.time_osem_paths()
             else:
                 d["fwd"], d["back"] = r["fwd"], r["back"]
             if oc == 3:

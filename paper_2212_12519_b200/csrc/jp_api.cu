@@ -528,9 +528,8 @@ cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, 
     const bool tiles = lm_tiles_wanted(c.lm, true);
     const jp::BrickSet *bs = nullptr;
     if (!tiles) JP_E(lm_bricks_wanted(c.lm, st, &bs));
-    if (bs) { // image bricks: per-event sums of every subset in a stream-ordered scratch array, then p = cf sum
-        float *acc = nullptr;
-        JP_E(cudaMallocAsync((void **)&acc, sizeof(float) * (size_t)jp::lm_plan_n(c.lm), st));
+    if (bs) { // image bricks: per-event sums of every subset in the plan's scratch array, then p = cf sum
+        float *acc = jp::brick_set_acc(bs); // the plan's scratch (a plan is used from one stream at a time)
         cudaError_t e = cudaMemsetAsync(acc, 0, sizeof(float) * (size_t)jp::lm_plan_n(c.lm), st);
         for (int m = 0; m < c.ns && e == cudaSuccess; ++m)
             if (subset < 0 || m == subset) {
@@ -540,7 +539,6 @@ cudaError_t lm_plan_fwd_tof(LmPlan *lm, int subset, const float *img, float *p, 
                     e = jp::launch_brick_finish(bs, acc, rg.first, rg.count, 0, rg.perm, rg.io_off, 0, p, st);
                 }
             }
-        cudaFreeAsync(acc, st);
         JP_E(e);
     }
     float4 *q[2] = {nullptr, nullptr};

@@ -20,7 +20,6 @@
 // 4 voxels and chunk instead of four per plane step.
 #include <cuda.h> // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked)
 
-#include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
 
 #include <cmath>
@@ -167,82 +166,14 @@ __device__ __forceinline__ int dray_brick(const DRay &R, int i, const int (&nb)[
     return (bp * nb[1] + k1 / kBr1) * nb[2] + k2 / kBr2;
 }
 
-// pieces per event (0 for principal axis z and for events that miss the image / whose TOF window does), cf per event
-__global__ void __launch_bounds__(256) k_brick_count(Lors l, const int16_t *__restrict__ tb, int64_t n, Geom g, Tof t,
-                                                      BrickGrid bg, int *__restrict__ npieces, float *__restrict__ cf,
-                                                      unsigned long long *__restrict__ total)
+// The pieces are ordered by a COUNTING sort on  bin = ((subset * 2 + axis) * NB + brick) << kLenBits | (nk - 1):
+// pass 1 (k_brick_pieces<false>) counts the pieces of every bin, an exclusive scan turns the counts into offsets, and
+// pass 2 (k_brick_pieces<true>) writes every piece's record straight to its final place (one atomic ticket per piece).
+// The order of the pieces inside a bin (same brick, same length) is arbitrary.
+__device__ __forceinline__ void brick_piece_record(const DRay &R, const int16_t *__restrict__ tb, const Tof &t, float scale,
+                                                   const int (&nb)[3], int e, int brick, int i0, int nk, BrickPiece &pc)
 {
-    const int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    int cnt = 0;
-    if (e < n) {
-        DRay R;
-        if (dray_setup(l, e, tb, g, t, R)) {
-            int prev = -1;
-            for (int i = R.ilo; i <= R.ihi; ++i) {
-                const int b = dray_brick(R, i, bg.nb[R.p]);
-                cnt += (b != prev);
-                prev = b;
-            }
-        }
-        npieces[e] = cnt;
-        cf[e] = R.cf;
-    }
-    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(total, (unsigned long long)cnt);
-}
-
-// sort key of a piece: ((subset * 2 + axis) * NB + brick) << kLenBits | (nk - 1); payload: (event, first plane, nk)
-__global__ void __launch_bounds__(256) k_brick_emit(Lors l, const int16_t *__restrict__ tb, int64_t first, int64_t count,
-                                                     int subset, Geom g, Tof t, BrickGrid bg, const int *__restrict__ offs,
-                                                     unsigned *__restrict__ keys, int *__restrict__ idx, int2 *__restrict__ payload)
-{
-    const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (c >= count) return;
-    const int64_t e = first + c;
-    DRay R;
-    if (!dray_setup(l, e, tb, g, t, R)) return;
-    int at = offs[e];
-    int prev = dray_brick(R, R.ilo, bg.nb[R.p]), i0 = R.ilo;
-    const unsigned sab0 = (unsigned)(subset * 2 + R.p) * (unsigned)bg.NB;
-    for (int i = R.ilo + 1; i <= R.ihi + 1; ++i) {
-        const int b = (i <= R.ihi) ? dray_brick(R, i, bg.nb[R.p]) : -1;
-        if (b != prev) {
-            const int nk = i - i0;
-            keys[at] = ((sab0 + (unsigned)prev) << kLenBits) | (unsigned)(nk - 1);
-            idx[at] = at;
-            payload[at] = make_int2((int)e, (i0 << 8) | nk);
-            ++at;
-            prev = b;
-            i0 = i;
-        }
-    }
-}
-
-// first piece of every (subset, axis, brick) in the sorted list
-__global__ void __launch_bounds__(256) k_brick_bounds(const unsigned *__restrict__ keys, int64_t n, int *__restrict__ firsts)
-{
-    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    const unsigned sab = keys[j] >> kLenBits;
-    if (j == 0 || (keys[j - 1] >> kLenBits) != sab) firsts[sab] = (int)j;
-}
-
-// records of the sorted pieces: the event's set-up again (float64), rebased to the piece's brick
-__global__ void __launch_bounds__(256) k_brick_records(Lors l, const int16_t *__restrict__ tb, Geom g, Tof t, BrickGrid bg,
-                                                        const unsigned *__restrict__ keys, const int *__restrict__ idx,
-                                                        const int2 *__restrict__ payload, int64_t n, float scale,
-                                                        BrickPiece *__restrict__ pieces)
-{
-    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    const int2 pay = payload[idx[j]];
-    const int e = pay.x, i0 = pay.y >> 8, nk = pay.y & 0xff;
-    DRay R;
-    dray_setup(l, e, tb, g, t, R);
-    const int (&nb)[3] = bg.nb[R.p];
-    const int brick = (int)((keys[j] >> kLenBits) % (unsigned)bg.NB);
     const int b2 = brick % nb[2], b1 = (brick / nb[2]) % nb[1], bp = brick / (nb[2] * nb[1]);
-    BrickPiece pc;
     // local coordinates: column c <-> voxel b kBr - kOff + c, so u' = u + kOff - b kBr lies in [0, kBr) for the brick's cells
     const double a1 = fma(R.B1, (double)i0, R.A1) + (double)kOff1 - (double)(b1 * kBr1);
     const double a2 = fma(R.B2, (double)i0, R.A2) + (double)kOff2 - (double)(b2 * kBr2);
@@ -260,7 +191,50 @@ __global__ void __launch_bounds__(256) k_brick_records(Lors l, const int16_t *__
     pc.dx = (float)(-R.dtau * (double)scale);
     pc.pl_nk = ((i0 - bp * kBrP) << 8) | nk;
     pc.ev = e;
-    pieces[j] = pc;
+}
+
+// events [first, first + count) of the sorted list = subset `subset`.  EMIT false: bins[bin] += 1 per piece, cf per event,
+// *total += pieces;  EMIT true: bins holds the running offsets (tickets), the records go to pieces[ticket].
+template <bool EMIT>
+__global__ void __launch_bounds__(256) k_brick_pieces(Lors l, const int16_t *__restrict__ tb, int64_t first, int64_t count,
+                                                       int subset, Geom g, Tof t, BrickGrid bg, float scale,
+                                                       int *__restrict__ bins, float *__restrict__ cf,
+                                                       unsigned long long *__restrict__ total, BrickPiece *__restrict__ pieces)
+{
+    const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int cnt = 0;
+    if (c < count) {
+        const int64_t e = first + c;
+        DRay R;
+        const bool hit = dray_setup(l, e, tb, g, t, R);
+        if (!EMIT) cf[e] = R.cf;
+        if (hit) {
+            const int (&nb)[3] = bg.nb[R.p];
+            const unsigned sab0 = (unsigned)(subset * 2 + R.p) * (unsigned)bg.NB;
+            int prev = dray_brick(R, R.ilo, nb), i0 = R.ilo;
+            for (int i = R.ilo + 1; i <= R.ihi + 1; ++i) {
+                const int b = (i <= R.ihi) ? dray_brick(R, i, nb) : -1;
+                if (b != prev) {
+                    const int nk = i - i0;
+                    const unsigned bin = ((sab0 + (unsigned)prev) << kLenBits) | (unsigned)(nk - 1);
+                    if (EMIT) {
+                        BrickPiece pc;
+                        brick_piece_record(R, tb, t, scale, nb, (int)e, prev, i0, nk, pc);
+                        pieces[atomicAdd(&bins[bin], 1)] = pc;
+                    } else {
+                        atomicAdd(&bins[bin], 1);
+                        ++cnt;
+                    }
+                    prev = b;
+                    i0 = i;
+                }
+            }
+        }
+    }
+    if (!EMIT) {
+        for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(total, (unsigned long long)cnt);
+    }
 }
 
 // ---- hot kernels ---------------------------------------------------------------------------------------------------
@@ -655,9 +629,12 @@ struct BrickSet {
     BrickPiece *pieces = nullptr;
     BrickChunk *chunks = nullptr;
     float *cf = nullptr;                       // [n] incidence factor of every sorted event
+    float *acc = nullptr;                      // [n] scratch of the planned forward projection: the events' sums
     std::vector<int> chunk_first, chunk_count; // per subset
     int g1n = 0;
     float gmax = 1.f;
+    int64_t n_chunks = 0;
+    bool counted = false;                      // BrickChunk::mcount holds the counted terms (path 4)
 };
 
 bool brick_supported(const Geom &g, const Tof &t, int n_subsets)
@@ -676,6 +653,7 @@ void brick_set_destroy(BrickSet *bs)
     cudaFree(bs->pieces);
     cudaFree(bs->chunks);
     cudaFree(bs->cf);
+    cudaFree(bs->acc);
     delete bs;
 }
 
@@ -700,14 +678,14 @@ cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const 
     *out = bs;
     if (n == 0) return cudaSuccess;
     cudaError_t e;
-    int *npieces = nullptr, *idx = nullptr, *idx2 = nullptr, *firsts = nullptr;
-    unsigned *keys = nullptr, *keys2 = nullptr;
-    int2 *payload = nullptr;
+    int *bins = nullptr;
     unsigned long long *total = nullptr;
     void *tmp = nullptr;
     size_t tmp_bytes = 0;
     const size_t n_sab = (size_t)n_subsets * 2 * (size_t)bg.NB;
-    std::vector<int> h_firsts;
+    const size_t n_bins = n_sab << kLenBits;
+    const float scale = (float)((double)kG1K / (double)t.width);
+    std::vector<int> h_first(n_sab + 1, 0); // first piece of every (subset, axis, brick)
     std::vector<BrickChunk> h_chunks;
 #define JP_BR_TRY(x)                     \
     do {                                 \
@@ -715,15 +693,26 @@ cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const 
         if (e != cudaSuccess) goto fail; \
     } while (0)
     JP_BR_TRY(cudaMalloc((void **)&bs->cf, sizeof(float) * (size_t)n));
-    JP_BR_TRY(cudaMallocAsync((void **)&npieces, sizeof(int) * (size_t)n, st));
-    JP_BR_TRY(cudaMallocAsync((void **)&total, sizeof(unsigned long long), st));
+    JP_BR_TRY(cudaMalloc((void **)&bs->acc, sizeof(float) * (size_t)n));
+    JP_BR_TRY(cudaMalloc((void **)&bins, sizeof(int) * (n_bins + 1)));
+    JP_BR_TRY(cudaMemsetAsync(bins, 0, sizeof(int) * (n_bins + 1), st));
+    JP_BR_TRY(cudaMalloc((void **)&total, sizeof(unsigned long long)));
     JP_BR_TRY(cudaMemsetAsync(total, 0, sizeof(unsigned long long), st));
-    {
-        const unsigned grid = (unsigned)((n + 255) / 256);
-        k_brick_count<<<grid, 256, 0, st>>>(l, tb, n, g, t, bg, npieces, bs->cf, total);
+    for (int m = 0; m < n_subsets; ++m) {
+        if (sub_count[m] == 0) continue;
+        k_brick_pieces<false><<<(unsigned)((sub_count[m] + 255) / 256), 256, 0, st>>>(l, tb, sub_first[m], sub_count[m], m, g, t, bg,
+                                                                                     scale, bins, bs->cf, total, nullptr);
         JP_BR_TRY(cudaGetLastError());
+    }
+    {
         unsigned long long h_total = 0;
         JP_BR_TRY(cudaMemcpyAsync(&h_total, total, sizeof(h_total), cudaMemcpyDeviceToHost, st));
+        JP_BR_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, bins, bins, (int)(n_bins + 1), st));
+        JP_BR_TRY(cudaMalloc(&tmp, tmp_bytes));
+        JP_BR_TRY(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, bins, bins, (int)(n_bins + 1), st));
+        // offsets of the bricks' first bins (every 2^kLenBits-th entry) and the total, one strided copy
+        JP_BR_TRY(cudaMemcpy2DAsync(h_first.data(), sizeof(int), bins, sizeof(int) << kLenBits, sizeof(int), n_sab + 1,
+                                    cudaMemcpyDeviceToHost, st));
         JP_BR_TRY(cudaStreamSynchronize(st));
         if (h_total >= ((unsigned long long)1 << 31)) {
             e = cudaErrorNotSupported;
@@ -732,64 +721,31 @@ cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const 
         bs->n_pieces = (int64_t)h_total;
     }
     if (bs->n_pieces > 0) {
-        const int64_t np = bs->n_pieces;
-        JP_BR_TRY(cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, npieces, npieces, (int)n, st));
-        JP_BR_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
-        JP_BR_TRY(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, npieces, npieces, (int)n, st));
-        JP_BR_TRY(cudaFreeAsync(tmp, st));
-        tmp = nullptr;
-        JP_BR_TRY(cudaMallocAsync((void **)&keys, sizeof(unsigned) * (size_t)np, st));
-        JP_BR_TRY(cudaMallocAsync((void **)&keys2, sizeof(unsigned) * (size_t)np, st));
-        JP_BR_TRY(cudaMallocAsync((void **)&idx, sizeof(int) * (size_t)np, st));
-        JP_BR_TRY(cudaMallocAsync((void **)&idx2, sizeof(int) * (size_t)np, st));
-        JP_BR_TRY(cudaMallocAsync((void **)&payload, sizeof(int2) * (size_t)np, st));
+        JP_BR_TRY(cudaMalloc((void **)&bs->pieces, sizeof(BrickPiece) * (size_t)bs->n_pieces));
         for (int m = 0; m < n_subsets; ++m) {
             if (sub_count[m] == 0) continue;
-            const unsigned grid = (unsigned)((sub_count[m] + 255) / 256);
-            k_brick_emit<<<grid, 256, 0, st>>>(l, tb, sub_first[m], sub_count[m], m, g, t, bg, npieces, keys, idx, payload);
+            k_brick_pieces<true><<<(unsigned)((sub_count[m] + 255) / 256), 256, 0, st>>>(l, tb, sub_first[m], sub_count[m], m, g, t,
+                                                                                        bg, scale, bins, nullptr, nullptr, bs->pieces);
             JP_BR_TRY(cudaGetLastError());
         }
-        int key_bits = kLenBits;
-        while (((uint64_t)1 << key_bits) < ((uint64_t)n_sab << kLenBits)) ++key_bits;
-        JP_BR_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, idx2, (int)np, 0, key_bits, st));
-        JP_BR_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
-        JP_BR_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, idx, idx2, (int)np, 0, key_bits, st));
-        JP_BR_TRY(cudaMalloc((void **)&bs->pieces, sizeof(BrickPiece) * (size_t)np));
-        const unsigned pgrid = (unsigned)((np + 255) / 256);
-        k_brick_records<<<pgrid, 256, 0, st>>>(l, tb, g, t, bg, keys2, idx2, payload, np, (float)((double)kG1K / (double)t.width),
-                                               bs->pieces);
-        JP_BR_TRY(cudaGetLastError());
-        JP_BR_TRY(cudaMallocAsync((void **)&firsts, sizeof(int) * n_sab, st));
-        JP_BR_TRY(cudaMemsetAsync(firsts, 0xff, sizeof(int) * n_sab, st));
-        k_brick_bounds<<<pgrid, 256, 0, st>>>(keys2, np, firsts);
-        JP_BR_TRY(cudaGetLastError());
-        h_firsts.resize(n_sab);
-        JP_BR_TRY(cudaMemcpyAsync(h_firsts.data(), firsts, sizeof(int) * n_sab, cudaMemcpyDeviceToHost, st));
-        JP_BR_TRY(cudaStreamSynchronize(st));
         // chunks: every (subset, axis, brick) run of the sorted pieces, cut into slices of <= kBrChunk pieces
-        int64_t next = np;
-        std::vector<int64_t> h_count(n_sab, 0);
-        for (size_t s = n_sab; s-- > 0;)
-            if (h_firsts[s] >= 0) {
-                h_count[s] = next - h_firsts[s];
-                next = h_firsts[s];
-            }
         for (int m = 0; m < n_subsets; ++m) {
             bs->chunk_first[(size_t)m] = (int)h_chunks.size();
             for (int a = 0; a < 2; ++a)
                 for (int b = 0; b < bg.NB; ++b) {
                     const size_t s = ((size_t)m * 2 + a) * (size_t)bg.NB + b;
-                    if (h_count[s] == 0) continue;
+                    const int64_t cnt = (int64_t)h_first[s + 1] - h_first[s];
+                    if (cnt == 0) continue;
                     const int (&nb)[3] = bg.nb[a];
-                    for (int64_t at = 0; at < h_count[s]; at += kBrChunk) {
+                    for (int64_t at = 0; at < cnt; at += kBrChunk) {
                         BrickChunk c;
-                        c.first = (int)(h_firsts[s] + at);
-                        c.count = (int)std::min<int64_t>(kBrChunk, h_count[s] - at);
+                        c.first = (int)(h_first[s] + at);
+                        c.count = (int)std::min<int64_t>(kBrChunk, cnt - at);
                         c.b2 = (short)(b % nb[2]);
                         c.b1 = (short)((b / nb[2]) % nb[1]);
                         c.bp = (short)(b / (nb[2] * nb[1]));
                         c.axis = (short)a;
-                        c.mcount = c.count;
+                        c.mcount = c.count; // until brick_set_count_terms() has run
                         c.pad = 0;
                         h_chunks.push_back(c);
                     }
@@ -799,23 +755,16 @@ cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const 
         if (!h_chunks.empty()) {
             JP_BR_TRY(cudaMalloc((void **)&bs->chunks, sizeof(BrickChunk) * h_chunks.size()));
             JP_BR_TRY(cudaMemcpyAsync(bs->chunks, h_chunks.data(), sizeof(BrickChunk) * h_chunks.size(), cudaMemcpyHostToDevice, st));
-            JP_BR_TRY(cudaFuncSetAttribute(k_brick_maxcount, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
-            k_brick_maxcount<<<(unsigned)h_chunks.size(), kBrT, sizeof(int) * kBrVox, st>>>(bs->chunks, bs->pieces);
-            JP_BR_TRY(cudaGetLastError());
             JP_BR_TRY(cudaStreamSynchronize(st)); // h_chunks goes out of scope
         }
+        bs->n_chunks = (int64_t)h_chunks.size();
     }
     e = cudaSuccess;
 fail:
-    if (tmp) cudaFreeAsync(tmp, st);
-    if (firsts) cudaFreeAsync(firsts, st);
-    if (payload) cudaFreeAsync(payload, st);
-    if (idx2) cudaFreeAsync(idx2, st);
-    if (idx) cudaFreeAsync(idx, st);
-    if (keys2) cudaFreeAsync(keys2, st);
-    if (keys) cudaFreeAsync(keys, st);
-    if (total) cudaFreeAsync(total, st);
-    if (npieces) cudaFreeAsync(npieces, st);
+    cudaStreamSynchronize(st); // the temporaries are plain cudaMalloc memory (cheaper than stream-ordered at this size)
+    cudaFree(tmp);
+    cudaFree(total);
+    cudaFree(bins);
     if (e != cudaSuccess) {
         brick_set_destroy(bs);
         *out = nullptr;
@@ -824,7 +773,20 @@ fail:
 #undef JP_BR_TRY
 }
 
+// path 4 only: count, per chunk, the terms the most-hit voxel receives (k_brick_maxcount); once per brick set
+cudaError_t brick_set_count_terms(BrickSet *bs, cudaStream_t st)
+{
+    if (bs->counted || bs->n_chunks == 0) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_brick_maxcount, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    if (e != cudaSuccess) return e;
+    k_brick_maxcount<<<(unsigned)bs->n_chunks, kBrT, sizeof(int) * kBrVox, st>>>(bs->chunks, bs->pieces);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) bs->counted = true;
+    return e;
+}
+
 const float *brick_set_cf(const BrickSet *bs) { return bs->cf; }
+float *brick_set_acc(const BrickSet *bs) { return bs->acc; }
 
 static cudaError_t brick_attr()
 {
@@ -905,6 +867,9 @@ cudaError_t launch_brick_back(const BrickSet *bs, int m, int mode, const float *
     const int nc = bs->chunk_count[(size_t)m];
     if (nc == 0) return cudaSuccess;
     cudaError_t e = brick_attr();
+    // the head room of the fixed-point staging: counted on the first staged adjoint of the plan (stream-ordered; a plan
+    // is used from one stream at a time)
+    if (e == cudaSuccess) e = brick_set_count_terms(const_cast<BrickSet *>(bs), st);
     if (e != cudaSuccess) return e;
     G1Tab gt{};
     e = g1tab_create(t, bs->g1n, st, &gt);

@@ -146,6 +146,7 @@ cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const 
                              const int64_t *sub_first, const int64_t *sub_count, cudaStream_t st, BrickSet **out);
 void brick_set_destroy(BrickSet *bs);
 int64_t brick_set_pieces(const BrickSet *bs);
+float *brick_set_acc(const BrickSet *bs); // one float per event: scratch of the planned forward projection
 cudaError_t lm_plan_bricks(LmPlan *pl, cudaStream_t st, const BrickSet **out);
 // acc[e - ev0] += sum_k G(k) bilinear(k) over the pieces of subset m (ev0: sorted position of the subset's first event)
 cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const Geom &g, const Tof &t, int64_t ev0, float *acc,

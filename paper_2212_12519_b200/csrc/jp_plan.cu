@@ -81,21 +81,32 @@ __global__ void k_lm_keys(Lors l, const int16_t *__restrict__ tofbin, int64_t n,
         if (cnt_sm[i]) atomicAdd(&counts[i], cnt_sm[i]);
 }
 
-__global__ void k_lm_gather(Lors l, const int16_t *__restrict__ tofbin, const int *__restrict__ perm, int64_t n,
+// sorted SoA copy of the events.  A gather of seven arrays through the permutation touches seven 32-byte sectors per
+// event; packing the event into ONE 32-byte record first (coalesced) makes it one sector per event.
+__global__ void k_lm_pack(Lors l, const int16_t *__restrict__ tofbin, int64_t n, float4 *__restrict__ rec)
+{
+    const int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    rec[2 * j] = make_float4(l.xs[j], l.ys[j], l.zs[j], l.xe[j]);
+    rec[2 * j + 1] = make_float4(l.ye[j], l.ze[j], __int_as_float((int)tofbin[j]), 0.f);
+}
+
+__global__ void k_lm_gather(const float4 *__restrict__ rec, const int *__restrict__ perm, int64_t n,
                             float *__restrict__ xs, float *__restrict__ ys, float *__restrict__ zs,
                             float *__restrict__ xe, float *__restrict__ ye, float *__restrict__ ze,
                             int16_t *__restrict__ tb)
 {
     const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (c >= n) return;
-    const int j = perm[c];
-    xs[c] = l.xs[j];
-    ys[c] = l.ys[j];
-    zs[c] = l.zs[j];
-    xe[c] = l.xe[j];
-    ye[c] = l.ye[j];
-    ze[c] = l.ze[j];
-    tb[c] = tofbin[j];
+    const int64_t j = perm[c];
+    const float4 a = __ldg(rec + 2 * j), b = __ldg(rec + 2 * j + 1);
+    xs[c] = a.x;
+    ys[c] = a.y;
+    zs[c] = a.z;
+    xe[c] = a.w;
+    ye[c] = b.x;
+    ze[c] = b.y;
+    tb[c] = (int16_t)__float_as_int(b.z);
 }
 
 __global__ void k_lm_permute(const int *__restrict__ perm, const float *__restrict__ in, float *__restrict__ out, int64_t n,
@@ -165,6 +176,7 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
     cudaError_t e;
     unsigned long long *keys = nullptr, *keys2 = nullptr;
     int *idx = nullptr, *counts = nullptr;
+    float4 *rec = nullptr;
     void *tmp = nullptr;
     size_t tmp_bytes = 0;
 #define JP_PLAN_TRY(x)                  \
@@ -175,10 +187,10 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
     JP_PLAN_TRY(cudaMalloc((void **)&pl->coord, sizeof(float) * 6 * (size_t)n));
     JP_PLAN_TRY(cudaMalloc((void **)&pl->tb, sizeof(int16_t) * (size_t)n));
     JP_PLAN_TRY(cudaMalloc((void **)&pl->perm, sizeof(int) * (size_t)n));
-    JP_PLAN_TRY(cudaMallocAsync((void **)&keys, sizeof(unsigned long long) * (size_t)n, st));
-    JP_PLAN_TRY(cudaMallocAsync((void **)&keys2, sizeof(unsigned long long) * (size_t)n, st));
-    JP_PLAN_TRY(cudaMallocAsync((void **)&idx, sizeof(int) * (size_t)n, st));
-    JP_PLAN_TRY(cudaMallocAsync((void **)&counts, sizeof(int) * (size_t)n_subsets * 4, st));
+    JP_PLAN_TRY(cudaMalloc((void **)&keys, sizeof(unsigned long long) * (size_t)n));
+    JP_PLAN_TRY(cudaMalloc((void **)&keys2, sizeof(unsigned long long) * (size_t)n));
+    JP_PLAN_TRY(cudaMalloc((void **)&idx, sizeof(int) * (size_t)n));
+    JP_PLAN_TRY(cudaMalloc((void **)&counts, sizeof(int) * (size_t)n_subsets * 4));
     JP_PLAN_TRY(cudaMemsetAsync(counts, 0, sizeof(int) * (size_t)n_subsets * 4, st));
     {
         const unsigned grid = (unsigned)((n + 255) / 256);
@@ -197,11 +209,13 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
         }
         const int end_bit = 56 + bits_for(n_subsets);
         JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
-        JP_PLAN_TRY(cudaMallocAsync(&tmp, tmp_bytes, st));
+        JP_PLAN_TRY(cudaMalloc(&tmp, tmp_bytes));
         JP_PLAN_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, idx, pl->perm, (int)n, 0, end_bit, st));
         float *c = pl->coord;
-        k_lm_gather<<<grid, 256, 0, st>>>(l, tofbin, pl->perm, n, c, c + n, c + 2 * n, c + 3 * n, c + 4 * n, c + 5 * n,
-                                           pl->tb);
+        JP_PLAN_TRY(cudaMalloc((void **)&rec, sizeof(float4) * 2 * (size_t)n));
+        k_lm_pack<<<grid, 256, 0, st>>>(l, tofbin, n, rec);
+        JP_PLAN_TRY(cudaGetLastError());
+        k_lm_gather<<<grid, 256, 0, st>>>(rec, pl->perm, n, c, c + n, c + 2 * n, c + 3 * n, c + 4 * n, c + 5 * n, pl->tb);
         JP_PLAN_TRY(cudaGetLastError());
         {   // run statistics of the sorted list: decides between line tiles and the quad kernels
             unsigned long long *runs = reinterpret_cast<unsigned long long *>(keys); // scratch, keys are dead
@@ -214,18 +228,23 @@ cudaError_t lm_plan_create(const Lors &l, const int16_t *tofbin, int64_t n, cons
             pl->n_runs = (int64_t)h;
         }
     }
-    cudaFreeAsync(tmp, st);
-    cudaFreeAsync(counts, st);
-    cudaFreeAsync(idx, st);
-    cudaFreeAsync(keys2, st);
-    cudaFreeAsync(keys, st);
+    // (the stream has just been synchronised: the temporaries are idle.  Plain cudaMalloc / cudaFree on purpose: a
+    // stream-ordered allocation of this size costs ~6 ms per GB to map and as much to trim at the next synchronisation)
+    cudaFree(rec);
+    cudaFree(tmp);
+    cudaFree(counts);
+    cudaFree(idx);
+    cudaFree(keys2);
+    cudaFree(keys);
     return cudaSuccess;
 fail:
-    if (tmp) cudaFreeAsync(tmp, st);
-    if (counts) cudaFreeAsync(counts, st);
-    if (idx) cudaFreeAsync(idx, st);
-    if (keys2) cudaFreeAsync(keys2, st);
-    if (keys) cudaFreeAsync(keys, st);
+    cudaStreamSynchronize(st);
+    cudaFree(rec);
+    cudaFree(tmp);
+    cudaFree(counts);
+    cudaFree(idx);
+    cudaFree(keys2);
+    cudaFree(keys);
     lm_plan_destroy(pl);
     *out = nullptr;
     return e;
