@@ -50,7 +50,7 @@ N_SM = 148
 # ncu figures of the dominant kernels (dram bytes per launch, issue-slot / l1tex / L2 utilisation), read from the text
 # summary of the one `ncu --set full` capture per config committed under profiles/ (the file names its commands and
 # the commit it was taken at); a number measured under the profiler is never a bench value -- these only explain it
-NCU_CSV = os.path.join(ROOT, "profiles", "r02_kernel_metrics.csv")
+NCU_CSV = os.path.join(ROOT, "profiles", "r02b_kernel_metrics.csv")
 
 
 def ncu_metrics():
@@ -69,7 +69,7 @@ def ncu_note(c, direction):
     if not r:
         return None
     f = lambda k: float(r[k]) if r.get(k) not in (None, "") else None
-    return {"source": "profiles/r02_kernel_metrics.csv (ncu --set full, commit %s)" % r.get("commit", "?"), "kernel": r["kernel"],
+    return {"source": "profiles/r02b_kernel_metrics.csv (ncu --set full, commit %s)" % r.get("commit", "?"), "kernel": r["kernel"],
             "duration_ms": f("duration_ms"), "dram_bytes_per_launch": (f("dram_read_bytes") or 0) + (f("dram_write_bytes") or 0),
             "issue_slots_busy_pct": f("issue_pct"), "l1tex_throughput_pct": f("l1tex_pct"), "l2_throughput_pct": f("lts_pct"),
             "fma_pipe_pct": f("fma_pipe_pct"), "l1_hit_pct": f("l1_hit_pct"), "l2_hit_pct": f("l2_hit_pct"),
@@ -704,6 +704,16 @@ def check_parity(w: Workload):
                     "image_max": float(ref.max()), "image_sum": float(ref.sum()), "finite": bool(np.isfinite(got).all()),
                     "oracle_full": {"s_per_iteration": (t1 - t0) / n_iter, "events": int(w.n)}})
         out["pass"] = bool(rel <= tol["osem_rel_l2"] and mx <= tol["osem_max_abs_rel"] and out["finite"])
+        # the same reconstruction through the other kernel paths of the plan (jp_lm_plan_set_path), against the same oracle image
+        out["paths"] = {}
+        for path, name in ((2, "quad_both_ways"), (4, "bricks_both_ways_staged_adjoint")):
+            w.plan.set_path(path)
+            xp = torch.ones(G.n, dtype=torch.float32, device=w.dev)
+            jp.jp_lm_osem_planned(w.plan, w.sens, xp, n_iter=n_iter)
+            gp = f64(xp)
+            out["paths"][name] = {"osem_rel_l2": float(np.linalg.norm(gp - ref) / np.linalg.norm(ref)),
+                                  "osem_max_abs_rel": float(np.abs(gp - ref).max() / np.abs(ref).max())}
+        w.plan.set_path(0)
     else:
         out["skipped"] = "the 40 GB sinogram OSEM workload is checked per subset in tests/test_gpu_fullsize.py"
     return out
