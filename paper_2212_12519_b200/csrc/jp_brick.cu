@@ -13,11 +13,13 @@
 // the affine plane loop in BRICK-LOCAL coordinates (32 bytes, float64 set-up as in jp_ray.cuh).  A CTA takes a chunk of
 // <= kBrChunk pieces of one brick:
 //   forward   brick (+ one column of neighbours) -> shared memory; per piece  acc[event] += sum_k G(k) bilinear(k)
-//   adjoint   per piece  brick[cell] += cf y G(k) hat(k)  with native int32 shared atomics (fixed point, scale from the
-//             chunk's max |cf y|: an event adds to a voxel at most once, so a voxel receives <= kBrChunk terms), then
-//             the brick is flushed once with 128-bit REDs (north_star: shared-memory tile staging before global atomics).
-// Shared-memory gathers of 32 random banks cost ~3.5 wavefronts instead of 32 L1 wavefronts, and the L2 sees one RED per
-// 4 voxels and chunk instead of four per plane step.
+//   adjoint   (opt-in, path 4) per piece  brick[cell] += cf y G(k) hat(k)  with native int32 shared atomics (fixed point;
+//             one scale per chunk, tied to the chunk's median |cf y|, head room from the plan-counted number of terms a
+//             voxel receives; larger and non-finite values take float atomics), then the brick is flushed once with
+//             128-bit REDs (north_star: shared-memory tile staging before global atomics).  The automatic path keeps
+//             float atomics for the adjoint (jp_quad.cu): OSEM ratios need floating-point range, see k_brick_back.
+// Shared-memory gathers of 32 random banks cost ~3.5 wavefronts per load instead of 32 L1 wavefronts per gather, and the
+// L2 sees one RED per 4 voxels and chunk instead of one per plane step.
 #include <cuda.h> // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked)
 
 #include <cub/device/device_scan.cuh>
