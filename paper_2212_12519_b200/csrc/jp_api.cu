@@ -5,7 +5,7 @@
 #include <cstring>
 
 #include "../../include/joseph_b200.h"
-#include "jp_internal.h"
+#include "jp_g1tab.cuh"
 
 namespace jp {
 thread_local char g_err_buf[512] = "";
@@ -87,12 +87,15 @@ inline jp::Range whole(int64_t n) { return jp::Range{0, 1, n, false, nullptr}; }
 // stream-ordered scratch of one TOF call: the edge-function table and a zero-padded image
 struct TofCtx {
     jp::TofLut lut{};
+    jp::G1Tab g1{};       // the brick kernels' TOF table, when the adjoint has to read the same weights (g1_init)
     float *pimg = nullptr;
     cudaStream_t st = nullptr;
+    cudaError_t g1_init(const jp::Tof &t) { return jp::g1tab_create(t, jp::g1tab_entries(t), st, &g1); }
     ~TofCtx()
     {
         jp::tof_lut_destroy(&lut, st);
         jp::padded_destroy(pimg, st);
+        if (g1.tab) cudaFreeAsync((void *)g1.tab, st);
     }
 };
 
@@ -577,6 +580,7 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
     const jp::BrickSet *bs = nullptr;
     bool staged = false;
     if (!tiles) JP_E(lm_bricks_wanted(c.lm, st, &bs, &staged));
+    if (bs && !staged) JP_E(tc.g1_init(c.t)); // float adjoint of the brick forward projection: the same TOF table
     if (!staged) bs = nullptr;
     if (tiles) {
         for (int a = 0; a < 2; ++a)
@@ -597,7 +601,8 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
             JP_E(cudaMemsetAsync(b[a], 0, qbytes, st));
             for (int m = 0; m < c.ns; ++m)
                 if (subset < 0 || m == subset)
-                    JP_E(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg_io(m, a, sorted_io), y, c.g, c.t, tc.lut, b[a], st));
+                    JP_E(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg_io(m, a, sorted_io), y, c.g, c.t, tc.lut, b[a], st, 0,
+                                                     tc.g1.tab ? &tc.g1 : nullptr));
         }
         JP_E(jp::launch_quad_merge(b[0], b[1], c.g, img, st));
     }
@@ -753,6 +758,7 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
     bool staged = false;
     JP_CUDA(lm_bricks_wanted(c.lm, st, &bs, &staged), where);
     staged = staged && bs;
+    if (bs && !staged) JP_CUDA(tc.g1_init(c.t), where); // forward and adjoint must read the same TOF table (jp_quad.cu)
     float4 *q[2] = {nullptr, nullptr}, *b[2] = {nullptr, nullptr};
     const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
     for (int a = 0; a < 2 && !staged; ++a) {
@@ -793,7 +799,7 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                 } else {
                     for (int a = 0; a < 2; ++a) {
                         JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
-                        JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st, 1), where);
+                        JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st, 1, &tc.g1), where);
                     }
                 }
             } else {
@@ -1276,12 +1282,13 @@ int jp_lm_osem_planned_backratio(const jp_plan *plan, int subset, const float *x
     if (bs && staged) {
         JP_CUDA(jp::launch_brick_back(bs, m, 1, r, nullptr, c.g, c.t, c.subset(m).first, b, st), where);
     } else if (bs) {
+        JP_CUDA(tc.g1_init(c.t), where);
         float4 *qb[2];
         const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
         for (int a = 0; a < 2; ++a) {
             JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &qb[a]), where);
             JP_CUDA(cudaMemsetAsync(qb[a], 0, qbytes, st), where);
-            JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, qb[a], st, 1), where);
+            JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, qb[a], st, 1, &tc.g1), where);
         }
         JP_CUDA(jp::launch_quad_merge(qb[0], qb[1], c.g, b, st), where);
     } else {

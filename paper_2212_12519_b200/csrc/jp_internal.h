@@ -100,8 +100,11 @@ cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range r
 cudaError_t launch_osem_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float4 *q, const Geom &g,
                                     const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st);
 // y_mode 1: y holds the forward sums without the factor cf; the OSEM ratio 1 / (cf y) is back projected
+// gt: TOF weights from this G1 table (jp_g1tab.cuh: the table of the brick / line-tile kernels) instead of `lut`
+struct G1Tab;
 cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
-                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st, int y_mode = 0);
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st, int y_mode = 0,
+                                    const G1Tab *gt = nullptr);
 
 // TOF listmode on line tiles (jp_lm_tile.cu): events [first, first + count) of a SORTED list; outputs / inputs at
 // perm[e] (perm != null) or io_off + e - first; cudaErrorNotSupported: image too wide for the tiled kernels

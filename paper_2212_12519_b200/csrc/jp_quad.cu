@@ -14,7 +14,7 @@
 // pass folds the four taps back into the image.  Q_p depends on the principal axis p through q1, so the plan
 // keeps the events of every subset split by axis and the kernels run axis by axis; each array is 4x the
 // image (66.6 MB for 200x200x96), L2-resident on its own (126 MB L2), which is why the axes are not mixed.
-#include "jp_internal.h"
+#include "jp_g1tab.cuh"
 
 namespace jp {
 
@@ -145,16 +145,24 @@ __global__ void __launch_bounds__(kQBlock) k_fwd_tof_lm_quad(Lors l, const int16
 }
 
 // Y_MODE 0: y = the values to back project;  1: y = sum_k G bilinear of every event (the forward projection without
-// its factor cf, e.g. from the brick kernels) and the OSEM ratio 1 / (cf y) if cf y > 1e-9 else 0 is back projected (A14)
-template <int Y_MODE>
+// its factor cf, e.g. from the brick kernels) and the OSEM ratio 1 / (cf y) if cf y > 1e-9 else 0 is back projected (A14).
+// G1W: the TOF weights come from the one-look-up table of jp_g1tab.cuh, the table the brick forward kernel uses, instead
+// of the edge-function table.  An OSEM update divides an event's weights by their own sum: for an event whose expectation
+// is made of a few tail weights the two tables' rounding (1e-7 absolute each) does not cancel unless forward and adjoint
+// read the SAME table (measured: update rel-L2 1.2e-4 -> 2e-6 on a problem with such events).
+template <int Y_MODE, bool G1W>
 __global__ void __launch_bounds__(kQBlock) k_back_tof_lm_quad(Lors l, const int16_t *__restrict__ tofbin, Range rg,
-                                                              const float *__restrict__ y, Geom g, Tof t, TofLut lut,
+                                                              const float *__restrict__ y, Geom g, Tof t, TofLut lut, G1Tab gt,
                                                               float4 *__restrict__ b)
 {
     extern __shared__ __align__(16) float2 lut_sm[];
-    lut_load(lut, lut_sm);
+    if (G1W) {
+        for (int i = threadIdx.x; i < gt.n; i += kQBlock) lut_sm[i] = __ldg(gt.tab + i);
+    } else {
+        lut_load(lut, lut_sm);
+    }
     __syncthreads();
-    const uint32_t lb = lut_base(lut_sm);
+    const uint32_t lb = lut_base(lut_sm); // (the same bias for both tables: entries are float2)
     const int64_t c = blockIdx.x * (int64_t)kQBlock + threadIdx.x;
     if (c >= rg.count) return;
     const int64_t j = rg.first + c * rg.stride;
@@ -172,12 +180,13 @@ __global__ void __launch_bounds__(kQBlock) k_back_tof_lm_quad(Lors l, const int1
         yj = 1.f / ybar;
     }
     const float x = pr.cf * yj;
+    const float x0 = (centre - pr.tau0) * gt.scale, dx = -pr.dtau * gt.scale; // G1W: table position of plane k = x0 + dx k
     float fk = 0.f;
     int po = pr.off;
     for (int k = 0; k < pr.nk; ++k) {
         const PCell cl = pray_cell(pr, fk, po);
-        const float tau = fmaf(pr.dtau, fk, pr.tau0);
-        const float w = tof_weight(lb, lut.inv_h, half_w, tau, centre);
+        const float w = G1W ? g1_weight(lb, gt.xedge, fmaf(dx, fk, x0))
+                            : tof_weight(lb, lut.inv_h, half_w, fmaf(pr.dtau, fk, pr.tau0), centre);
         if (w != 0.f) quad_scatter(b, cl, x * w);
         fk += 1.f;
         po += pr.sp;
@@ -267,14 +276,21 @@ cudaError_t launch_fwd_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range r
     return cudaGetLastError();
 }
 
+// gt != null: TOF weights from that G1 table (the brick forward kernel's), else from the edge-function table `lut`
 cudaError_t launch_back_tof_lm_quad(const Lors &l, const int16_t *tofbin, Range rg, const float *y, const Geom &g,
-                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st, int y_mode)
+                                    const Tof &t, const TofLut &lut, float4 *b, cudaStream_t st, int y_mode, const G1Tab *gt)
 {
     if (rg.count == 0) return cudaSuccess;
-    if (y_mode == 1)
-        k_back_tof_lm_quad<1><<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, b);
-    else
-        k_back_tof_lm_quad<0><<<grid_for(rg.count), kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, b);
+    const unsigned grid = grid_for(rg.count);
+    if (gt && sizeof(float2) * (size_t)gt->n <= 40 * 1024) {
+        const size_t smem = sizeof(float2) * (size_t)gt->n;
+        if (y_mode == 1) k_back_tof_lm_quad<1, true><<<grid, kQBlock, smem, st>>>(l, tofbin, rg, y, g, t, lut, *gt, b);
+        else k_back_tof_lm_quad<0, true><<<grid, kQBlock, smem, st>>>(l, tofbin, rg, y, g, t, lut, *gt, b);
+    } else {
+        const G1Tab none{};
+        if (y_mode == 1) k_back_tof_lm_quad<1, false><<<grid, kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, none, b);
+        else k_back_tof_lm_quad<0, false><<<grid, kQBlock, kLutBytesQ, st>>>(l, tofbin, rg, y, g, t, lut, none, b);
+    }
     return cudaGetLastError();
 }
 
