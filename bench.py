@@ -381,7 +381,7 @@ class Workload:
             self.launches = 2 if c == 1 else 8   # unplanned: c1 one tile kernel per direction; c2: pad/unpad, 2 tables, kernel
             self.make_sino_plan()
             if self.splan is not None:
-                self.launches = 2 if c == 1 else 4   # c1: one track-tile kernel per direction; c2: + the weight table
+                self.launches = 4   # per direction: c1 the track table + the whole-track kernel; c2 the weight table + the tile kernel
             self.hbm_bytes = (self.n * 28 + NVOX * 4) if c == 1 else (self.n * (24 + 4 * TOFP.n_tofbins) + NVOX * 4)
         else:
             nev = int(os.environ.get("JP_BENCH_EVENTS", "40000000"))
@@ -400,12 +400,13 @@ class Workload:
             if c == 3:
                 self.y = inputs.uniform_values(self.n, 0.5, 2.0, seed=inputs.BASE_SEED + 103 + rank, device=dev)
                 self.p = torch.empty(self.n, dtype=torch.float32, device=dev)
-                self.launches = 2 * 2 + 2    # fwd + back line-tile kernels per principal axis (x, y) + their TOF tables
+                # per direction: the edge table, and per principal axis (x, y) the bin-weight table + the line-tile kernel
+                self.launches = 2 * (1 + 2 * 2)
             else:
                 self.sens = torch.ones(G.n, dtype=torch.float32, device=dev)   # replaced by A^T 1 in setup_sens()
                 self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
-                # per subset: TOF weight table, brick forward, float-atomic adjoint per axis (x, y), update; + one edge table
-                self.launches = 5 * 20 + 1
+                # per subset: TOF weight table, brick forward, float-atomic adjoint per axis (x, y), update; + two tables per call
+                self.launches = 5 * 20 + 2
 
     def make_sino_plan(self):
         """sinogram plan of the workload's LOR list (set-up, timed separately: `plan_s`); JP_BENCH_UNPLANNED=1 in the
