@@ -295,7 +295,8 @@ cudaError_t lm_plan_bricks(LmPlan *pl, cudaStream_t st, const BrickSet **out)
             count[(size_t)m] = rg.count;
         }
         const cudaError_t e = brick_set_create(l, tb, pl->n, pl->g, pl->t, pl->n_subsets, first.data(), count.data(), st, &pl->bricks);
-        if (e != cudaSuccess && e != cudaErrorNotSupported) return e;
+        if (e == cudaErrorMemoryAllocation) (void)cudaGetLastError(); // no room for the pieces: the plan works without them
+        else if (e != cudaSuccess && e != cudaErrorNotSupported) return e;
     }
     *out = pl->bricks;
     return cudaSuccess;
