@@ -148,7 +148,8 @@ int jp_lm_osem(const jp_lors *events, const int16_t *tofbin, const jp_geom *geom
  *   The plan owns its device buffers (26 + 4 bytes per event) until jp_lm_plan_destroy.  When the sorted events do NOT
  *   come in long runs on one transaxial line (an OSEM subset of a clinical acquisition: ~20 events per line), the plan
  *   also cuts every event into PIECES per image brick of 32 x 32 x 16 cells (csrc/jp_brick.cu; about 3.5 pieces of
- *   32 bytes per event + 4 bytes per event), so that the forward projection can run on bricks held in shared memory.
+ *   32 bytes per event + 8 bytes per event), so that the forward projection can run on bricks held in shared memory
+ *   (if the device has no room for the pieces the plan is made without them and the planned calls use path 2).
  *   jp_lm_plan_create allocates with cudaMalloc and SYNCHRONISES `stream` (it reads the per-subset / per-axis event
  *   counts, the run statistics and the piece counts back to the host); the planned calls are asynchronous.  A plan keeps
  *   image-sized scratch (quad image and accumulators, allocated with cudaMalloc on the first call that needs them)
