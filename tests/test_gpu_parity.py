@@ -556,6 +556,13 @@ def test_forward_projections_are_deterministic(cuda_device, scanner, events, mon
             assert torch.equal(jp.jp_fwd_tof_lm_planned(plan, img), ref)
             assert torch.equal(jp.jp_fwd_lm_planned(plan, img), refn)
         plan.destroy()
+    # image bricks (path 3): an event's pieces are summed with float atomics, so repeats agree up to the order of a
+    # handful of additions (a race in the TMA-loaded brick would show as a difference orders of magnitude larger)
+    plan = jp.LmPlan(ex, ee, tb, g.n, g.origin, g.voxsize, tof, n_subsets=3).set_path(3)
+    ref = jp.jp_fwd_tof_lm_planned(plan, img).clone()
+    for _ in range(3):
+        assert float((jp.jp_fwd_tof_lm_planned(plan, img) - ref).abs().max()) <= 1e-6 * float(ref.max())
+    plan.destroy()
 
 
 @pytest.mark.parametrize("case", ["wide_image", "wide_tof_kernel"])
