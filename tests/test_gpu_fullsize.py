@@ -157,6 +157,12 @@ def test_config3_full_tof_lm(cuda_device, phantom_dev, events_full):
     assert_back(jp.jp_back_tof_lm_planned(plan, ys), bref)
     bd = jp.jp_back_tof_lm_planned(plan, y)
     assert adj_gap(pp, y, imgd, bd) <= ADJ_GAP
+    # the other kernel paths of the same plan at full size: quad image (2), adjoint staged in the image bricks (4)
+    for path in (2, 4):
+        plan.set_path(path)
+        assert_fwd(jp.jp_fwd_tof_lm_planned(plan, imgd)[idx], ref)
+        assert_back(jp.jp_back_tof_lm_planned(plan, ys), bref)
+        assert adj_gap(pp, y, imgd, jp.jp_back_tof_lm_planned(plan, y)) <= ADJ_GAP
     plan.destroy()
 
 
