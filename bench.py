@@ -405,8 +405,8 @@ class Workload:
             else:
                 self.sens = torch.ones(G.n, dtype=torch.float32, device=dev)   # replaced by A^T 1 in setup_sens()
                 self.x = torch.ones(G.n, dtype=torch.float32, device=dev)
-                # per subset: TOF weight table, brick forward, float-atomic adjoint per axis (x, y), update; + two tables per call
-                self.launches = 5 * 20 + 2
+                # per subset: brick forward, float-atomic adjoint per axis (x, y), update; + two tables per call
+                self.launches = 4 * 20 + 2
 
     def make_sino_plan(self):
         """sinogram plan of the workload's LOR list (set-up, timed separately: `plan_s`); JP_BENCH_UNPLANNED=1 in the

@@ -793,7 +793,7 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                       // float atomics on the quad accumulators
                 const jp::Range sub = c.subset(m);
                 JP_CUDA(cudaMemsetAsync(r, 0, sizeof(float) * (size_t)sub.count, st), where);
-                JP_CUDA(jp::launch_brick_fwd(bs, m, xin, c.g, c.t, sub.first, r, st), where);
+                JP_CUDA(jp::launch_brick_fwd(bs, m, xin, c.g, c.t, sub.first, r, st, tc.g1.tab ? &tc.g1 : nullptr), where);
                 if (staged) {
                     JP_CUDA(jp::launch_brick_back(bs, m, 1, r, nullptr, c.g, c.t, sub.first, bz, st), where);
                 } else {

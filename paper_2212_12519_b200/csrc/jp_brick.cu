@@ -855,14 +855,15 @@ static bool brick_tensor_maps(const float *img, const Geom &g, CUtensorMap *tm0,
 // acc[e - ev0] += sum_k G bilinear over the pieces of subset m (acc: zeroed by the caller, one float per event of the
 // subset, ev0 = position of the subset's first event in the sorted list)
 cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const Geom &g, const Tof &t, int64_t ev0, float *acc,
-                             cudaStream_t st)
+                             cudaStream_t st, const G1Tab *table)
 {
     const int nc = bs->chunk_count[(size_t)m];
     if (nc == 0) return cudaSuccess;
     cudaError_t e = brick_attr();
     if (e != cudaSuccess) return e;
     G1Tab gt{};
-    e = g1tab_create(t, bs->g1n, st, &gt);
+    if (table && table->n == bs->g1n) gt = *table; // the caller's table (a driver that loops over subsets makes it once)
+    else e = g1tab_create(t, bs->g1n, st, &gt);
     if (e != cudaSuccess) return e;
     CUtensorMap tm0, tm1;
     memset(&tm0, 0, sizeof(tm0));
@@ -871,7 +872,7 @@ cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const 
     k_brick_fwd<<<(unsigned)nc, kBrT, brick_smem_fwd(bs->g1n), st>>>(tm0, tm1, use_tma, bs->chunks + bs->chunk_first[(size_t)m],
                                                                     bs->pieces, img, g, gt, (int)ev0, acc);
     e = cudaGetLastError();
-    cudaFreeAsync((void *)gt.tab, st);
+    if (!(table && table->n == bs->g1n)) cudaFreeAsync((void *)gt.tab, st);
     return e;
 }
 

@@ -152,8 +152,9 @@ int64_t brick_set_pieces(const BrickSet *bs);
 float *brick_set_acc(const BrickSet *bs); // one float per event: scratch of the planned forward projection
 cudaError_t lm_plan_bricks(LmPlan *pl, cudaStream_t st, const BrickSet **out);
 // acc[e - ev0] += sum_k G(k) bilinear(k) over the pieces of subset m (ev0: sorted position of the subset's first event)
+// table: the G1 table of t if the caller already has one (else made and freed here, stream-ordered)
 cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const Geom &g, const Tof &t, int64_t ev0, float *acc,
-                             cudaStream_t st);
+                             cudaStream_t st, const G1Tab *table = nullptr);
 // img += A_m^T x.  mode 0: x = cf v[perm ? perm[e] : e - ev0];  mode 1: v = acc, x = cf / (cf acc) if cf acc > 1e-9 else 0
 cudaError_t launch_brick_back(const BrickSet *bs, int m, int mode, const float *v, const int *perm, const Geom &g, const Tof &t,
                               int64_t ev0, float *img, cudaStream_t st);
