@@ -29,11 +29,15 @@ namespace {
 
 constexpr int kTT = 256; // threads per CTA
 
+// Launch settings from sweeps on B200 (configs[1], forward / back ms): 3 CTAs per SM and 72 KB of forward rows 3.53 / 4.08;
+// 4 CTAs (64 registers, ~80 bytes of spills) and 52 KB 3.41 / 4.04; 48 KB 3.32 / 4.04; 40 KB 3.32; 32 KB 3.42; 5 CTAs
+// (48 registers) 3.99 / 4.39.  The forward kernel waits on shared / global loads (24 warps per SM at 3 CTAs): the
+// fourth CTA hides more of that than the spills and the extra row chunks cost.
 #ifndef JP_TRK_MINB9
-#define JP_TRK_MINB9 3 // CTAs per SM with 9 LORs per thread (register budget 85)
+#define JP_TRK_MINB9 4 // CTAs per SM with 9 LORs per thread (register budget 64)
 #endif
 #ifndef JP_TRK_SMEM_KB_FWD
-#define JP_TRK_SMEM_KB_FWD 72
+#define JP_TRK_SMEM_KB_FWD 48
 #endif
 #ifndef JP_TRK_SMEM_KB_BACK
 #define JP_TRK_SMEM_KB_BACK 44
