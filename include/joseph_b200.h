@@ -220,6 +220,28 @@ int jp_osem_update(float *x, float *b, const float *sens, float scale, const jp_
  * stream-ordered.  JP_ERR_SIZE: sigma_mm <= 0, n_sigmas <= 0 or a kernel radius > 16 voxels. */
 int jp_gauss3d(const float *in, float *out, const jp_geom *geom, float sigma_mm, float n_sigmas, void *stream);
 
+/* jp_gauss3d for callers that cannot allocate device memory: same arguments, same kernels, bit-identical result,
+ * and NO cudaMalloc / cudaMallocAsync / cudaFree (or any allocating library routine) anywhere in the call.
+ * Meant for code that runs after all device memory has been handed out (a reconstruction service whose pools were
+ * sized at start-up, a framework that owns the whole GPU), for host threads that may not take the allocator's
+ * device-wide lock or its implicit synchronisation (acquisition / real-time loops), and for set-ups where the
+ * stream-ordered allocator that jp_gauss3d relies on is not available.
+ *   Scratch   the image-sized intermediate of the separable passes lives in a fixed array inside the library's own
+ *             device data: JP_GAUSS3D_STATIC_MAX_VOXELS floats = 16 MiB, held by every GPU that loads the library
+ *             until the process exits.  An image with more voxels than that is refused: JP_ERR_SIZE, text via
+ *             jp_last_error(), nothing enqueued.  (200 x 200 x 96, the paper's image, has 3.84 M voxels.)
+ *   Set-up    the FIRST call on each device looks up that device's address of the array (cudaGetSymbolAddress,
+ *             with the calling thread's current device, which must be the device of `stream`, `in` and `out`);
+ *             later calls on that device reuse it.  Make this first call outside any stream capture.
+ *   Sharing   all calls on one device use the same array.  Calls on one stream are ordered and safe; two calls
+ *             that may overlap on the GPU (different streams, or different host threads on different streams) RACE
+ *             on it and give garbage -- order them with events or use jp_gauss3d for one of them.  Nothing needs
+ *             clearing between calls: every pass overwrites its whole destination before it is read.
+ * in / out: device, caller-owned, geom->n voxels, C order; in may equal out.
+ * Errors as for jp_gauss3d. */
+#define JP_GAUSS3D_STATIC_MAX_VOXELS 4194304
+int jp_gauss3d_static(const float *in, float *out, const jp_geom *geom, float sigma_mm, float n_sigmas, void *stream);
+
 /* jp_lm_osem_planned with the resolution model in every subset (reading R3): ybar = A (G x), b = G (A^T r),
  * x <- x b n_subsets / sens; `sens` is the caller's (it should hold G A^T 1).  Workspace as for
  * jp_lm_osem_planned. */

@@ -79,6 +79,7 @@ EXPORTS = {
                                                C.c_void_p]),
     "jp_osem_update": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.POINTER(jp_geom), C.c_void_p]),
     "jp_gauss3d": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_float, C.c_float, C.c_void_p]),
+    "jp_gauss3d_static": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(jp_geom), C.c_float, C.c_float, C.c_void_p]),
     "jp_sino_osem_tof_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int64, C.POINTER(jp_tof)]),
     "jp_sino_sens_tof": (C.c_int, [C.POINTER(jp_lors), C.c_void_p, C.c_int, C.c_void_p, C.POINTER(jp_geom),
                                    C.POINTER(jp_tof), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
@@ -528,6 +529,24 @@ def jp_gauss3d(img, voxsize, sigma_mm: float, n_sigmas: float = 3.0, out=None, s
     assert out.shape == img.shape and out.is_contiguous()
     _check(load().jp_gauss3d(img.data_ptr(), out.data_ptr(), C.byref(g), float(sigma_mm), float(n_sigmas),
                              _stream(stream)), "jp_gauss3d")
+    return out
+
+
+GAUSS3D_STATIC_MAX_VOXELS = 4194304   # JP_GAUSS3D_STATIC_MAX_VOXELS of joseph_b200.h
+
+
+def jp_gauss3d_static(img, voxsize, sigma_mm: float, n_sigmas: float, out, stream=None) -> torch.Tensor:
+    """out = G img like jp_gauss3d, for callers that cannot allocate device memory (all of it already handed out,
+    an acquisition loop that may not stall on the allocator, no stream-ordered pool): the library's built-in
+    16 MiB scratch serves as the intermediate image, so nothing is allocated -- which is also why `out` must be
+    given here (it may be img).  Images above GAUSS3D_STATIC_MAX_VOXELS voxels raise JosephError.  All calls on a
+    device share the scratch: keep them on one stream, or order them; overlapping calls race."""
+    img = _img(img)
+    g = make_geom(img.shape, (0.0, 0.0, 0.0), voxsize)
+    _dev(out, torch.float32, "out")
+    assert out.shape == img.shape and out.is_contiguous()
+    _check(load().jp_gauss3d_static(img.data_ptr(), out.data_ptr(), C.byref(g), float(sigma_mm), float(n_sigmas),
+                                    _stream(stream)), "jp_gauss3d_static")
     return out
 
 
