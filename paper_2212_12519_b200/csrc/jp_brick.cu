@@ -647,7 +647,9 @@ bool brick_supported(const Geom &g, const Tof &t, int n_subsets)
 {
     const BrickGrid bg = brick_grid(g);
     if (bg.NB > 32767) return false; // brick coordinates are stored as shorts
-    if ((uint64_t)n_subsets * 2u * (uint64_t)bg.NB >= ((uint64_t)1 << (32 - kLenBits))) return false;
+    // the counting sort keeps one int per (subset, axis, brick, length) bin and scans them with an int count: at most
+    // 2^26 bins (256 MB of histogram); larger problems take the line-tile path of the plan
+    if (((uint64_t)n_subsets * 2u * (uint64_t)bg.NB << kLenBits) >= ((uint64_t)1 << 26)) return false;
     if (g.n[0] >= (1 << 23) || g.n[1] >= (1 << 23)) return false;
     if (brick_smem_fwd(g1tab_entries(t)) > 110 * 1024) return false; // two CTAs per SM
     return true;
@@ -804,14 +806,13 @@ cudaError_t brick_set_count_terms(BrickSet *bs, cudaStream_t st)
 const float *brick_set_cf(const BrickSet *bs) { return bs->cf; }
 float *brick_set_acc(const BrickSet *bs) { return bs->acc; }
 
+// function attributes belong to the current device: set on every launch, like the other launchers (a process-wide
+// "done" flag would leave the second GPU of a hybrid handle at the 48 KB default)
 static cudaError_t brick_attr()
 {
-    static bool done = false; // idempotent; a race only repeats the calls
-    if (done) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(k_brick_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_brick_back<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_brick_back<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
-    if (e == cudaSuccess) done = true;
     return e;
 }
 
