@@ -542,6 +542,7 @@ cudaError_t set_smem(K kernel)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
 }
 
+// an unknown P / NPT sets e (a cudaError_t in scope) and falls through: the launchers free their scratch after the switch
 #define JP_TRK_DISPATCH_P(CFG, ...)                          \
     switch ((CFG).P) {                                       \
     case 40: { constexpr int P = 40; __VA_ARGS__; } break;   \
@@ -550,14 +551,14 @@ cudaError_t set_smem(K kernel)
     case 136: { constexpr int P = 136; __VA_ARGS__; } break; \
     case 200: { constexpr int P = 200; __VA_ARGS__; } break; \
     case 264: { constexpr int P = 264; __VA_ARGS__; } break; \
-    default: return cudaErrorInvalidValue;                   \
+    default: e = cudaErrorInvalidValue; break;               \
     }
 #define JP_TRK_DISPATCH_NPT(NPTV, ...)                       \
     switch (NPTV) {                                          \
     case 3: { constexpr int NPT = 3; __VA_ARGS__; } break;   \
     case 6: { constexpr int NPT = 6; __VA_ARGS__; } break;   \
     case 9: { constexpr int NPT = 9; __VA_ARGS__; } break;   \
-    default: return cudaErrorInvalidValue;                   \
+    default: e = cudaErrorInvalidValue; break;               \
     }
 
 // per-call scratch: [K] Track followed by [K] int (stream-ordered allocation)
