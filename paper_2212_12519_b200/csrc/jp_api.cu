@@ -1230,15 +1230,19 @@ int jp_sino_osem_tof_planned(const jp_plan *plan, const int64_t *subset_offsets,
         epi.y_em = y;
         epi.mult = mult;
         epi.contam = contam;
-        bool unsupported = false;
+        // launch_tof_sino_tile decides "not supported" on its first NON-EMPTY subset (an empty one returns at once).
+        // Until then only updates of empty subsets have been enqueued (x <- x 0 / sens = 0, which the unplanned
+        // path repeats with the same result), so the fall-back may still start over from subset 0.
+        bool unsupported = false, launched = false;
         for (int it = 0; it < n_iter && !unsupported; ++it) {
             for (int m = 0; m < n_subsets; ++m) {
                 const int64_t k0 = subset_offsets[m] / v.T, nk = subset_offsets[m + 1] / v.T - k0;
                 const cudaError_t e = jp::launch_tof_sino_tile(2, v, k0, nk, img, b.p, g, t, nullptr, nullptr, &epi, st);
-                if (e == cudaErrorNotSupported && it == 0 && m == 0) { // nothing enqueued yet: take the unplanned path
+                if (e == cudaErrorNotSupported && !launched) { // no projection enqueued yet: take the unplanned path
                     unsupported = true;
                     break;
                 }
+                if (nk > 0) launched = true;
                 JP_CUDA(e, "jp_sino_osem_tof_planned (subset pass)");
                 JP_CUDA(jp::launch_osem_update(img, b.p, sens + (size_t)m * nvox, 1.f, nvox, st),
                         "jp_sino_osem_tof_planned (update)");
