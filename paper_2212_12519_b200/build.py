@@ -39,11 +39,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
-    # JP_NVCC_EXTRA: a BUILD-time hook for tuning sweeps (-DJP_... overrides of the kernels' compile-time constants,
-    # e.g. JP_SMEM_KB_FWD); nothing in the built library reads the environment
-    extra = os.environ.get("JP_NVCC_EXTRA", "").split()
     for srcs, out in ((sources(), LIB), ([MICROBENCH_SRC], MICROBENCH_LIB)):
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + srcs + ["-o", out]
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + srcs + ["-o", out]
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)

@@ -711,6 +711,14 @@ PlanSrc plan_src(const SinoPlanView *pv)
 
 } // namespace
 
+// With JP_PLAN_TRACKS a regular plan never reaches the tile kernels (launch_*_track takes it), so their PLAN = true
+// instantiations are compiled only without it
+#if JP_PLAN_TRACKS
+#define JP_IF_PLAN_TILES(...)
+#else
+#define JP_IF_PLAN_TILES(...) __VA_ARGS__
+#endif
+
 #define JP_DISPATCH_P(CFG, ...)                    \
     switch ((CFG).P) {                             \
     case 40: { constexpr int P = 40; __VA_ARGS__; } break;   \
@@ -737,11 +745,11 @@ cudaError_t launch_fwd_tile(const Lors &l, int64_t n, const float *img, const Ge
     if (tiles >= ((int64_t)1 << 31)) return cudaErrorInvalidValue;
     cudaError_t e = cudaSuccess;
     JP_DISPATCH_P(c, {
-        if (plan) {
+        JP_IF_PLAN_TILES(if (plan) {
             e = set_smem(k_fwd_tile<P, true>);
             if (e == cudaSuccess)
                 k_fwd_tile<P, true><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, img, g, c.rows_cap, c.vec_ok, lane_map, p);
-        } else {
+        } else) {
             e = set_smem(k_fwd_tile<P, false>);
             if (e == cudaSuccess)
                 k_fwd_tile<P, false><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, img, g, c.rows_cap, c.vec_ok, lane_map, p);
@@ -764,11 +772,11 @@ cudaError_t launch_back_tile(const Lors &l, int64_t n, const float *y, const Geo
     if (tiles >= ((int64_t)1 << 31)) return cudaErrorInvalidValue;
     cudaError_t e = cudaSuccess;
     JP_DISPATCH_P(c, {
-        if (plan) {
+        JP_IF_PLAN_TILES(if (plan) {
             e = set_smem(k_back_tile<P, true>);
             if (e == cudaSuccess)
                 k_back_tile<P, true><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, y, g, c.rows_cap, c.vec_ok, lane_map, img);
-        } else {
+        } else) {
             e = set_smem(k_back_tile<P, false>);
             if (e == cudaSuccess)
                 k_back_tile<P, false><<<(unsigned)tiles, kThreads, c.smem, st>>>(l, ps, n, y, g, c.rows_cap, c.vec_ok, lane_map, img);
