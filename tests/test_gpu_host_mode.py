@@ -166,3 +166,30 @@ def test_hybrid_handle_tof(cuda_device):
         with pytest.raises(jp.JosephError):
             jp.Hybrid(devs).fwd(img, g.origin, g.voxsize)   # no list set
         h.destroy()
+
+
+def test_hybrid_tof_listmode_unsnapped_events(cuda_device):
+    """TOF listmode on the handle with end points that are NOT crystal centres (seeded jitter of a few mm, so no two
+    events share a line): every shard's plan is sparse and takes the image-brick kernels, whose > 48 KB dynamic
+    shared memory has to be enabled on EACH device that launches them.  Runs over 1 worker, 3 workers on device 0
+    and, where more than one GPU is visible, one worker per GPU."""
+    g, ph = inputs.GEOM_SCANNER, inputs.phantom()
+    tp = inputs.TofParams()
+    targs = (tp.tofbin_width, tp.sigma_tof, tp.n_sigmas)
+    tof = jp.make_tof(*targs, tp.n_tofbins)
+    n = 40_003
+    ex, ee, tb = inputs.listmode_events(n, seed=inputs.BASE_SEED + 57, img=ph, chunk=200_000)
+    rng = np.random.default_rng(57)
+    ex = (ex + torch.from_numpy(rng.uniform(-2.0, 2.0, size=tuple(ex.shape)).astype(np.float32))).contiguous()
+    ee = (ee + torch.from_numpy(rng.uniform(-2.0, 2.0, size=tuple(ee.shape)).astype(np.float32))).contiguous()
+    img = torch.from_numpy(ph)
+    yl = inputs.uniform_values(n, 0.5, 2.0, seed=58)
+    lref = oracle.fwd_tof_lm(ex.numpy(), ee.numpy(), tb.numpy(), ph, g.origin, g.voxsize, *targs)
+    lbref = oracle.back_tof_lm(ex.numpy(), ee.numpy(), tb.numpy(), yl.numpy(), g.n, g.origin, g.voxsize, *targs)
+    for devs in _devices_variants():
+        h = jp.Hybrid(devs)
+        h.set_lors(ex, ee, tb, g.n, g.origin, g.voxsize, tof)
+        assert_fwd(h.fwd_tof_lm(img), lref)
+        assert_back(h.back_tof_lm(yl, torch.zeros(g.n)), lbref)
+        assert_back(h.back_tof_lm(yl, torch.full(g.n, 1.0)) - 1.0, lbref)     # accumulates
+        h.destroy()
