@@ -804,7 +804,7 @@ def roofline_dict(w: Workload, fwd_ms: float, back_ms: float):
     kf, kb = w.kinds
     planned = getattr(w, "splan", None) is not None
     names = {0: ("k_fwd_tile (per-LOR path: random chords are not tracks)", "k_back_tile (per-LOR path)"),
-             1: ("k_fwd_tile<104, plan>", "k_back_tile<104, plan>") if planned else ("k_fwd_tile<104, list>", "k_back_tile<104, list>"),
+             1: ("k_fwd_track<104, 9>", "k_back_track<104, 9>") if planned else ("k_fwd_tile<104, list>", "k_back_tile<104, list>"),
              2: ("k_tof_sino_tile<6,fwd>", "k_tof_sino_tile<6,back>") if planned else ("k_tof_sino_win<6,fwd>", "k_tof_sino_win<6,back>"),
              3: ("k_fwd_tof_lm_tile", "k_back_tof_lm_tile"),
              4: ("k_brick_fwd (forward sums on TMA-loaded image bricks) + k_back_tof_lm_quad<ratio> (float atomics)", ""),
@@ -1016,6 +1016,11 @@ def run_ours(args):
                                     "is reported as SURVEY.md 8(d) asks, it says nothing about the kernels")
     if w.plan_s is not None:
         line["config"]["plan_s"] = w.plan_s
+    # A/B switches read from the environment change what is timed: the line says so (the driver sets neither)
+    overrides = {k: os.environ[k] for k in ("JP_BENCH_EVENTS", "JP_BENCH_UNPLANNED") if k in os.environ}
+    if overrides:
+        line["config"]["env_overrides"] = overrides
+        line["config"]["workload"] += " [NOT the stated config: environment overrides " + json.dumps(overrides) + "]"
     if sharded:
         line["sharded_osem"] = sharded
     if world == 1:
