@@ -92,8 +92,13 @@ int jp_fwd(const jp_lors *lors, const float *img, const jp_geom *geom, float *p,
    ACCUMULATES into img (the caller zeroes it when a plain back projection is wanted).
    Non-finite y: Inf / NaN on a LOR that crosses the image propagate into the voxels of that LOR exactly as a plain
    atomicAdd of cf y w would (track tiles that hold such a value take the per-LOR float path); y of LORs that miss
-   the image is never used.  Track tiles are staged in shared memory in fixed point with a scale per tile: the
-   rounding error per contribution is <= 3.6e-7 x max |cf y| over the 768 LORs of the tile. */
+   the image is never used.  Tracks are staged in shared memory in int32 fixed point with ONE scale per staged
+   group of LORs, S = lim / max |cf y| over the group, lim = min(2^22 - 2, 2^31 / (2 L) - 1) for a group of up to L LORs:
+     unplanned calls (tiles of 768 consecutive LORs, L = 768):      quantum max|cf y| / lim = 7.2e-7 x the tile's max;
+     planned calls (whole track pieces, L = 768 / 1536 / 2304):      7.2e-7 / 1.4e-6 / 2.1e-6 x the track piece's max
+     (2304 = the 48 x 48 ring pairs of the paper's scanner).
+   Every contribution cf y w is rounded to the nearest multiple of the quantum (error <= half of it); one below half
+   a quantum is dropped.  On configs[1] the image error is 2.6e-6 of its maximum (profiles/r02b_parity.txt). */
 int jp_back(const jp_lors *lors, const float *y, const jp_geom *geom, float *img, void *stream);
 
 /* ---- TOF sinogram: all n_tofbins bins of every LOR ------------------------------ */
