@@ -86,6 +86,44 @@ def test_config1_full_nontof(cuda_device, phantom_dev):
     assert gap <= ADJ_GAP
 
 
+def test_config1_full_nontof_planned(cuda_device, phantom_dev):
+    """configs[1] in the launch configuration bench.py times: a sinogram plan over all 151,584,768 LORs (65,792 tracks
+    of 2304 ring pairs) and the whole-track kernels k_fwd_track / k_back_track on a grid of 65,792 x pieces CTAs, with
+    the 64-bit output offsets and the skipping of the tracks that miss the image (56 % of them) that only this size
+    exercises.  Forward: sampled outputs against the oracle (incl. the tie, rim and degenerate tracks) and EVERY
+    output against the unplanned call (itself oracle-checked in test_config1_full_nontof); back: masked y against
+    the oracle voxel by voxel, dense y through the adjoint identity."""
+    ph, imgd = phantom_dev
+    xs, xe = inputs.sinogram_lors(device=cuda_device)
+    n = xs.shape[1]
+    plan = jp.SinoPlan(xs, xe)
+    assert plan.regular and plan.n == n
+    extra = [_track(64, 0), _track(64, 17), _track(192, -5), _track(10, 64), _track(3, 128), _track(255, -128),
+             _track(0, -128), _track(255, 128)]                             # first and last track of the list
+    idx = _sample(n, 150_000, 2, extra).to(cuda_device)
+    hxs, hxe = xs[:, idx].cpu().numpy(), xe[:, idx].cpu().numpy()
+    p = torch.full((n,), float("nan"), dtype=torch.float32, device=cuda_device)   # every output must be written
+    jp.jp_fwd_planned(plan, imgd, G.origin, G.voxsize, out=p)
+    ref = oracle.fwd(hxs, hxe, ph, G.origin, G.voxsize)
+    assert_fwd(p[idx], ref)
+    pu = jp.jp_fwd(xs, xe, imgd, G.origin, G.voxsize)
+    assert bool(torch.isfinite(p).all())
+    assert float((p - pu).abs().max()) <= 2e-5 * float(pu.abs().max())      # all 151.6 M outputs: track path == tile path
+    del pu, xs, xe                # the planned calls read the plan's track table, not the 3.6 GB of end points
+    y = inputs.uniform_values(n, 0.0, 1.0, seed=inputs.BASE_SEED + 101, device=cuda_device)
+    ys = torch.zeros_like(y)
+    ys[idx] = y[idx]
+    b = jp.jp_back_planned(plan, ys, G.n, G.origin, G.voxsize)
+    assert_back(b, oracle.back(hxs, hxe, ys[idx].cpu().numpy(), G.n, G.origin, G.voxsize))
+    del ys, b
+    bd = jp.jp_back_planned(plan, y, G.n, G.origin, G.voxsize)
+    assert adj_gap(p, y, imgd, bd) <= ADJ_GAP
+    # accumulate semantics at full size: a second pass into the same image doubles it
+    bd2 = jp.jp_back_planned(plan, y, G.n, G.origin, G.voxsize, img=bd.clone())
+    assert float((bd2 - 2 * bd).abs().max()) <= 1e-4 * float(bd.abs().max())
+    plan.destroy()
+
+
 def test_config2_full_tof_sino(cuda_device, phantom_dev):
     ph, imgd = phantom_dev
     xs, xe = inputs.sinogram_lors(views=inputs.SUBSET_VIEWS, device=cuda_device)
@@ -196,6 +234,36 @@ def test_config4_osem_full_image(cuda_device, phantom_dev, events_full):
         mx = np.abs(g - ref).max() / np.abs(ref).max()
         assert rel <= 1e-4, f"OSEM rel-L2 {rel:.3e}"
         assert mx <= 1e-3, f"OSEM max abs / max {mx:.3e}"
+    plan.destroy()
+
+
+def test_config4_full_density_subset(cuda_device, phantom_dev, events_full):
+    """configs[4] at the event density bench.py times (a plan over all 40 M events x 20 subsets: 2 M events per subset,
+    about 20 events per line and subset -- the regime in which the plan picks the image bricks): ONE subset's
+    projection half of the OSEM update, b = A_m^T (1 / A_m x), against the oracle's forward -> ratio -> back over
+    the same 2 M events, every voxel, for each kernel path the plan can pick by itself (0 = its own choice, 1 line
+    tiles, 2 quad image, 3 bricks forward + float adjoint)."""
+    ph, imgd = phantom_dev
+    xs, xe, tb = events_full
+    tof = _tof()
+    m = 7
+    x_h = (ph + 0.25).astype(np.float32)                 # positive everywhere: every event's expectation is > 1e-9
+    x = torch.from_numpy(x_h).to(cuda_device)
+    sub = torch.arange(m, xs.shape[1], 20, device=cuda_device)      # reading A14: subset m = events e with e mod 20 == m
+    hxs, hxe, htb = xs[:, sub].cpu().numpy(), xe[:, sub].cpu().numpy(), tb[sub].cpu().numpy()
+    assert hxs.shape[1] == 2_000_000
+    ybar = oracle.fwd_tof_lm(hxs, hxe, htb, x_h, G.origin, G.voxsize, *TOF_ARGS[:3])
+    r = np.where(ybar > 1e-9, 1.0 / np.maximum(ybar, 1e-300), 0.0)
+    assert (ybar > 1e-3).all()
+    bref = oracle.back_tof_lm(hxs, hxe, htb, r, G.n, G.origin, G.voxsize, *TOF_ARGS[:3])
+    plan = jp.LmPlan(xs, xe, tb, G.n, G.origin, G.voxsize, tof, n_subsets=20)
+    assert plan.subset_count(m) == 2_000_000
+    for path in (0, 1, 2, 3):
+        plan.set_path(path)
+        out = torch.full(G.n, float("nan"), dtype=torch.float32, device=cuda_device)    # the call overwrites b
+        b = jp.jp_lm_osem_planned_backratio(plan, m, x, out=out)
+        err = assert_back(b, bref)
+        assert err <= 1e-4, f"path {path}"
     plan.destroy()
 
 
