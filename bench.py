@@ -568,10 +568,9 @@ class Workload:
 
     def time_osem_paths(self, iters=3):
         """A/B of the kernels behind one OSEM iteration (jp_lm_plan_set_path): 2 = quad image both ways (round 1),
-        3 = image bricks forward + float atomics back (what the plan chooses, the timed configuration), 4 = bricks both
-        ways (adjoint staged in shared memory in fixed point; opt-in, see include/joseph_b200.h); ms per iteration"""
+        3 = image bricks forward + float atomics back (what the plan chooses, the timed configuration); ms per iteration"""
         out = {}
-        for path, name in ((2, "quad_both_ways"), (3, "bricks_forward_float_adjoint"), (4, "bricks_both_ways_staged_adjoint")):
+        for path, name in ((2, "quad_both_ways"), (3, "bricks_forward_float_adjoint")):
             self.plan.set_path(path)
             self.x.fill_(1.0)
             self.jp.jp_lm_osem_planned(self.plan, self.sens, self.x, n_iter=1)
@@ -754,7 +753,7 @@ def check_parity(w: Workload):
         out["pass"] = bool(rel <= tol["osem_rel_l2"] and mx <= tol["osem_max_abs_rel"] and out["finite"])
         # the same reconstruction through the other kernel paths of the plan (jp_lm_plan_set_path), against the same oracle image
         out["paths"] = {}
-        for path, name in ((2, "quad_both_ways"), (4, "bricks_both_ways_staged_adjoint")):
+        for path, name in ((2, "quad_both_ways"),):
             w.plan.set_path(path)
             xp = torch.ones(G.n, dtype=torch.float32, device=w.dev)
             jp.jp_lm_osem_planned(w.plan, w.sens, xp, n_iter=n_iter)

@@ -171,14 +171,8 @@ int jp_lm_plan_destroy(jp_plan *plan);
  *   2  quad image (csrc/jp_quad.cu): one 128-bit gather / float atomic add per event and plane;
  *   3  image bricks for the forward projection (csrc/jp_brick.cu: TMA box loads into shared memory), float atomic adds
  *      on the quad accumulators for the adjoint -- the same floating-point semantics as path 2;
- *   4  image bricks both ways: the adjoint is staged per brick in int32 fixed point and flushed with 128-bit REDs.  One
- *      scale per chunk of <= 4096 pieces, tied to the chunk's MEDIAN |cf y|: a term is rounded to T / lim, T = 16 .. 32 x
- *      that median, lim >= 2^19 (2^31 / (G(0) x the largest number of pieces of the chunk that touch one voxel), counted by
- *      the plan; ~2^26 for a clinical subset); values above T, Inf and NaN take float atomic adds.  Back projections meet
- *      north_star's 1e-4 max|.| bound; an OSEM whose update is ill-conditioned (a sensitivity image with zeros inside the
- *      object) amplifies the rounding and wants paths 0 / 2 / 3.  Never chosen automatically.
  * All paths compute the same projections (tests force each of them); images or TOF kernels a path cannot hold fall
- * back towards path 2.  Paths 3 / 4 build the brick pieces if the plan has none (allocates, synchronises).  Not to be
+ * back towards path 2.  Path 3 builds the brick pieces if the plan has none (allocates, synchronises).  Not to be
  * changed while a call that uses the plan is being issued from another thread. */
 int jp_lm_plan_set_path(jp_plan *plan, int path);
 /* number of events of a subset (subset = -1: all); -1 for an invalid plan or subset */

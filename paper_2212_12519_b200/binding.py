@@ -360,7 +360,7 @@ class LmPlan:
         return int(load().jp_lm_plan_subset_count(self.handle, int(subset)))
 
     def set_path(self, path: int):
-        """0: automatic, 1: line tiles, 2: quad image, 3: image bricks forward + float adjoint, 4: bricks both ways (jp_lm_plan_set_path)"""
+        """0: automatic, 1: line tiles, 2: quad image, 3: image bricks forward + float adjoint (jp_lm_plan_set_path)"""
         _check(load().jp_lm_plan_set_path(self.handle, int(path)), "jp_lm_plan_set_path")
         return self
 

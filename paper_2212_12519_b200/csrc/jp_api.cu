@@ -166,14 +166,12 @@ bool lm_tiles_wanted(const jp::LmPlan *lm, bool tof)
     return runs > 0 && jp::lm_plan_n(lm) / runs >= 512;
 }
 
-// the plan's brick set if the call should use it (path 0 / 3 / 4 and the plan could build one), else null.
-// *staged: the adjoint goes through the bricks too (path 4: fixed-point staging in shared memory); otherwise only the
-// forward projection does and the adjoint keeps float atomics on the quad accumulators (path 0 / 3).
-cudaError_t lm_bricks_wanted(jp::LmPlan *lm, cudaStream_t st, const jp::BrickSet **bs, bool *staged = nullptr)
+// the plan's brick set if the call should use it (path 0 / 3 and the plan could build one), else null.  The forward
+// projection runs on the bricks; the adjoint keeps float atomics on the quad accumulators.
+cudaError_t lm_bricks_wanted(jp::LmPlan *lm, cudaStream_t st, const jp::BrickSet **bs)
 {
     *bs = nullptr;
     const int path = jp::lm_plan_path(lm);
-    if (staged) *staged = path == 4;
     if (path == 1 || path == 2) return cudaSuccess;
     return jp::lm_plan_bricks(lm, st, bs);
 }
@@ -430,10 +428,10 @@ int jp_lm_plan_set_path(jp_plan *plan, int path)
 {
     g_err[0] = 0;
     if (!plan || !plan->lm) return fail(JP_ERR_PLAN, "not a listmode plan");
-    if (path < 0 || path > 4)
-        return fail(JP_ERR_SIZE, "path must be 0 (automatic), 1 (line tiles), 2 (quad image), 3 (bricks forward) or 4 (bricks both ways)");
+    if (path < 0 || path > 3)
+        return fail(JP_ERR_SIZE, "path must be 0 (automatic), 1 (line tiles), 2 (quad image) or 3 (bricks forward, float adjoint)");
     jp::lm_plan_set_path(plan->lm, path);
-    if (path >= 3) { // builds the pieces now if the plan has none yet (allocates, synchronises the NULL stream)
+    if (path == 3) { // builds the pieces now if the plan has none yet (allocates, synchronises the NULL stream)
         const jp::BrickSet *bs;
         JP_CUDA(jp::lm_plan_bricks(plan->lm, nullptr, &bs), "jp_lm_plan_set_path (bricks)");
     }
@@ -578,10 +576,8 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
     JP_E(jp::tof_lut_create(c.t, st, &tc.lut));
     const bool tiles = lm_tiles_wanted(c.lm, true);
     const jp::BrickSet *bs = nullptr;
-    bool staged = false;
-    if (!tiles) JP_E(lm_bricks_wanted(c.lm, st, &bs, &staged));
-    if (bs && !staged) JP_E(tc.g1_init(c.t)); // float adjoint of the brick forward projection: the same TOF table
-    if (!staged) bs = nullptr;
+    if (!tiles) JP_E(lm_bricks_wanted(c.lm, st, &bs));
+    if (bs) JP_E(tc.g1_init(c.t)); // float adjoint of the brick forward projection: the same TOF table
     if (tiles) {
         for (int a = 0; a < 2; ++a)
             for (int m = 0; m < c.ns; ++m)
@@ -589,10 +585,6 @@ cudaError_t lm_plan_back_tof(LmPlan *lm, int subset, const float *y, float *img,
                     const jp::Range rg = c.seg_io(m, a, sorted_io);
                     JP_E(jp::launch_back_tof_lm_tile(c.l, c.tb, rg.first, rg.count, rg.perm, rg.io_off, y, c.g, c.t, img, st));
                 }
-    } else if (bs) { // image bricks: y indexed by the sorted position (plan order) or through the permutation
-        for (int m = 0; m < c.ns; ++m)
-            if (subset < 0 || m == subset)
-                JP_E(jp::launch_brick_back(bs, m, 0, y, sorted_io ? nullptr : c.all.perm, c.g, c.t, 0, img, st));
     } else {
         float4 *b[2];
         const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
@@ -753,20 +745,18 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
     TofCtx tc;
     tc.st = st;
     JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
-    // bs: forward sums on the image bricks; staged: the adjoint too (else float atomics on the quad accumulators)
+    // bs: forward sums on the image bricks (the adjoint: float atomics on the quad accumulators either way)
     const jp::BrickSet *bs = nullptr;
-    bool staged = false;
-    JP_CUDA(lm_bricks_wanted(c.lm, st, &bs, &staged), where);
-    staged = staged && bs;
-    if (bs && !staged) JP_CUDA(tc.g1_init(c.t), where); // forward and adjoint must read the same TOF table (jp_quad.cu)
+    JP_CUDA(lm_bricks_wanted(c.lm, st, &bs), where);
+    if (bs) JP_CUDA(tc.g1_init(c.t), where); // forward and adjoint must read the same TOF table (jp_quad.cu)
     float4 *q[2] = {nullptr, nullptr}, *b[2] = {nullptr, nullptr};
     const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);
-    for (int a = 0; a < 2 && !staged; ++a) {
+    for (int a = 0; a < 2; ++a) {
         if (!bs) JP_CUDA(jp::lm_plan_quad(c.lm, a, &q[a]), where);
         JP_CUDA(jp::lm_plan_quad(c.lm, 2 + a, &b[a]), where);
     }
     const bool z_events = c.has_axis2(-1);
-    if (z_events || staged) JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
+    if (z_events) JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
     // resolution model: xb = G x feeds the forward projection, G folds the back projection (stream-ordered scratch)
     struct Scratch {
         float *p = nullptr;
@@ -789,18 +779,13 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                 JP_CUDA(jp::launch_gauss3d(img, xb, tmp, c.g, res_sigma, res_nsig, st), where);
                 xin = xb;
             }
-            if (bs) { // bricks: forward sums per event; ratio + back projection staged per brick into bz, or with
-                      // float atomics on the quad accumulators
+            if (bs) { // bricks: forward sums per event; ratio + back projection with float atomics on the quad accumulators
                 const jp::Range sub = c.subset(m);
                 JP_CUDA(cudaMemsetAsync(r, 0, sizeof(float) * (size_t)sub.count, st), where);
                 JP_CUDA(jp::launch_brick_fwd(bs, m, xin, c.g, c.t, sub.first, r, st, tc.g1.tab ? &tc.g1 : nullptr), where);
-                if (staged) {
-                    JP_CUDA(jp::launch_brick_back(bs, m, 1, r, nullptr, c.g, c.t, sub.first, bz, st), where);
-                } else {
-                    for (int a = 0; a < 2; ++a) {
-                        JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
-                        JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st, 1, &tc.g1), where);
-                    }
+                for (int a = 0; a < 2; ++a) {
+                    JP_CUDA(cudaMemsetAsync(b[a], 0, qbytes, st), where);
+                    JP_CUDA(jp::launch_back_tof_lm_quad(c.l, c.tb, c.seg(m, a, true), r, c.g, c.t, tc.lut, b[a], st, 1, &tc.g1), where);
                 }
             } else {
                 JP_CUDA(jp::launch_quad_build(xin, c.g, q[0], q[1], st), where);
@@ -820,13 +805,7 @@ static int lm_osem_planned_impl(const jp_plan *plan, const float *sens, float *i
                 jp::padded_destroy(pb, st);
                 JP_CUDA(e, where);
             }
-            if (staged && !res) {
-                JP_CUDA(jp::launch_osem_update(img, bz, sens, (float)c.ns, nvox, st), where); // clears bz
-            } else if (staged) {
-                JP_CUDA(jp::launch_gauss3d(bz, bb, tmp, c.g, res_sigma, res_nsig, st), where);
-                JP_CUDA(cudaMemsetAsync(bz, 0, sizeof(float) * (size_t)nvox, st), where);
-                JP_CUDA(jp::launch_osem_update(img, bb, sens, (float)c.ns, nvox, st), where);
-            } else if (!res) {
+            if (!res) {
                 JP_CUDA(jp::launch_quad_osem_update(img, b[0], b[1], z_events ? bz : nullptr, sens, (float)c.ns, c.g, st), where);
             } else {
                 JP_CUDA(cudaMemsetAsync(bb, 0, sizeof(float) * (size_t)nvox, st), where);
@@ -1276,16 +1255,13 @@ int jp_lm_osem_planned_backratio(const jp_plan *plan, int subset, const float *x
     JP_CUDA(jp::tof_lut_create(c.t, st, &tc.lut), where);
     const int m = subset;
     const jp::BrickSet *bs = nullptr;
-    bool staged = false;
-    JP_CUDA(lm_bricks_wanted(c.lm, st, &bs, &staged), where);
+    JP_CUDA(lm_bricks_wanted(c.lm, st, &bs), where);
     if (bs) {
         const jp::Range sub = c.subset(m);
         JP_CUDA(cudaMemsetAsync(r, 0, sizeof(float) * (size_t)sub.count, st), where);
         JP_CUDA(jp::launch_brick_fwd(bs, m, x, c.g, c.t, sub.first, r, st), where);
     }
-    if (bs && staged) {
-        JP_CUDA(jp::launch_brick_back(bs, m, 1, r, nullptr, c.g, c.t, c.subset(m).first, b, st), where);
-    } else if (bs) {
+    if (bs) {
         JP_CUDA(tc.g1_init(c.t), where);
         float4 *qb[2];
         const size_t qbytes = sizeof(float4) * (size_t)jp::padded_voxels(c.g);

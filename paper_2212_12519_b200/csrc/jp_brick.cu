@@ -13,13 +13,11 @@
 // the affine plane loop in BRICK-LOCAL coordinates (32 bytes, float64 set-up as in jp_ray.cuh).  A CTA takes a chunk of
 // <= kBrChunk pieces of one brick:
 //   forward   brick (+ one column of neighbours) -> shared memory; per piece  acc[event] += sum_k G(k) bilinear(k)
-//   adjoint   (opt-in, path 4) per piece  brick[cell] += cf y G(k) hat(k)  with native int32 shared atomics (fixed point;
-//             one scale per chunk, tied to the chunk's median |cf y|, head room from the plan-counted number of terms a
-//             voxel receives; larger and non-finite values take float atomics), then the brick is flushed once with
-//             128-bit REDs (north_star: shared-memory tile staging before global atomics).  The automatic path keeps
-//             float atomics for the adjoint (jp_quad.cu): OSEM ratios need floating-point range, see k_brick_back.
-// Shared-memory gathers of 32 random banks cost ~3.5 wavefronts per load instead of 32 L1 wavefronts per gather, and the
-// L2 sees one RED per 4 voxels and chunk instead of one per plane step.
+//   adjoint   float atomics on the quad accumulators (jp_quad.cu), reading the same TOF table as the forward kernel.
+//             (Rounds 1-2 also shipped an adjoint staged in the bricks in int32 fixed point, one scale per chunk.  One
+//             scale cannot carry the dynamic range of OSEM ratios: on a low-count reconstruction the update amplified
+//             its rounding to 2e-3 of the image maximum, over the 1e-3 bound, so it was taken out in round 3.)
+// Shared-memory gathers of 32 random banks cost ~3.5 wavefronts per load instead of 32 L1 wavefronts per gather.
 #include <cuda.h> // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, libcuda is not linked)
 
 #include <cub/device/device_scan.cuh>
@@ -62,17 +60,14 @@ constexpr int kBrP = JP_BR_P, kBr1 = JP_BR_1, kBr2 = JP_BR_2; // cells of a bric
 constexpr int kBrC1 = kBr1 + 2, kBrC2 = kBr2 + 2;
 // cells are shifted before they are cut into bricks: local column c <-> voxel b kBr - kOff + c.  Along q1 one column of
 // padding is what cell -1 needs; along z four, so that every brick starts at a multiple of 4 voxels (16 bytes: the TMA
-// box of the forward kernel and the 128-bit REDs of the adjoint flush need that alignment)
+// box of the forward kernel needs that alignment)
 constexpr int kOff1 = 1, kOff2 = 4;
-constexpr int kBrRow = kBrC2;                 // elements per (plane, q1) row
-constexpr int kBrPlane = kBrC1 * kBrC2;       // elements per plane
-constexpr int kBrVox = kBrP * kBrPlane;       // elements per brick
 constexpr int kBrChunk = JP_BR_CHUNK;         // pieces per CTA
 constexpr int kBrT = JP_BR_THREADS;
 constexpr int kBrPer = (kBrChunk + kBrT - 1) / kBrT; // pieces per thread
 constexpr int kLenBits = 6;                   // key bits of the piece length (kBrP <= 64)
 static_assert(kBrP <= 64 && kBrP < 256, "piece length must fit its key / record field");
-static_assert(kBr2 % 4 == 0, "vector flush needs bricks aligned to 4 axial voxels");
+static_assert(kBr2 % 4 == 0, "the TMA box needs bricks aligned to 4 axial voxels");
 
 // one piece: planes k = 0 .. nk-1 of the brick-local loop
 //   u1(k) = a1 + b1 k, u2(k) = a2 + b2 k   cell (floor u1, floor u2) of brick plane pl0 + k, local column c <-> voxel
@@ -90,8 +85,8 @@ struct __align__(8) BrickChunk {
     int first, count;   // pieces [first, first + count) of the sorted piece list
     short bp, b1, b2;   // brick coordinates
     short axis;         // principal axis (0 or 1)
-    int mcount;         // the largest number of pieces of the chunk that touch one and the same voxel (k_brick_maxcount)
-    int pad;
+    int pad;            // host side: slice number of the chunk inside its brick (launch order)
+    int pad2;
 };
 
 // brick grid of the image for principal axis a: cells kk = k + kOff in [kOff - 1, n_q + kOff) along q1 / q2, planes [0, n_p)
@@ -252,12 +247,6 @@ __device__ __forceinline__ float lds_f32(uint32_t addr)
     return v;
 }
 
-template <int OFF>
-__device__ __forceinline__ void reds_add(uint32_t addr, int q)
-{
-    asm volatile("red.shared.add.s32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "r"(q) : "memory");
-}
-
 struct BrickOrg {
     int p, q1;
     int sp, s1;            // element strides of the image along p and q1 (axial stride 1)
@@ -396,220 +385,6 @@ __global__ void __launch_bounds__(kBrT, JP_BR_MINB)
     else brick_fwd_pieces<kFwRow, kBrP * kFwRow>(ch, pieces, smem_addr(B), gbase, gt.xedge, ev0, acc);
 }
 
-// plan time: for every chunk the largest number of terms any voxel of its brick receives (a piece touches the four
-// neighbours of its cell on every plane).  It bounds the fixed-point sums of k_brick_back far below the worst case
-// "every piece of the chunk hits the same voxel", which buys the staging ~6 more bits.
-__global__ void __launch_bounds__(kBrT, JP_BR_MINB)
-    k_brick_maxcount(BrickChunk *__restrict__ chunks, const BrickPiece *__restrict__ pieces)
-{
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    int *B = reinterpret_cast<int *>(smem_raw);
-    __shared__ int red[kBrT / 32];
-    const int tid = threadIdx.x;
-    const BrickChunk ch = chunks[blockIdx.x];
-    for (int idx = tid; idx < kBrVox; idx += kBrT) B[idx] = 0;
-    __syncthreads();
-    const uint32_t bbase = smem_addr(B) - (uint32_t)kMagicI * (uint32_t)((kBrRow + 1) * 4);
-    for (int j = tid; j < ch.count; j += kBrT) {
-        const float4 *rec = reinterpret_cast<const float4 *>(pieces + ch.first + j);
-        const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);
-        const int pl_nk = __float_as_int(r1.z);
-        const int nk = pl_nk & 0xff;
-        uint32_t row = bbase + (uint32_t)(pl_nk >> 8) * (uint32_t)(kBrPlane * 4);
-        float fk = 0.f;
-        for (int k = 0; k < nk; ++k) {
-            const float t1 = __fadd_rd(fmaf(r0.y, fk, r0.x), kMagic), t2 = __fadd_rd(fmaf(r0.w, fk, r0.z), kMagic);
-            const uint32_t ad = row + __float_as_uint(t1) * (uint32_t)(kBrRow * 4) + (__float_as_uint(t2) << 2);
-            reds_add<0>(ad, 1);
-            reds_add<4>(ad, 1);
-            reds_add<kBrRow * 4>(ad, 1);
-            reds_add<kBrRow * 4 + 4>(ad, 1);
-            fk += 1.f;
-            row += kBrPlane * 4;
-        }
-    }
-    __syncthreads();
-    int mx = 0;
-    for (int idx = tid; idx < kBrVox; idx += kBrT) mx = max(mx, B[idx]);
-    for (int s = 16; s > 0; s >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, s));
-    if ((tid & 31) == 0) red[tid >> 5] = mx;
-    __syncthreads();
-    if (tid == 0) {
-        for (int w = 1; w < kBrT / 32; ++w) mx = max(mx, red[w]);
-        chunks[blockIdx.x].mcount = max(mx, 1);
-    }
-}
-
-// value scattered by event ev:  MODE 0: cf y[io]  (plain adjoint);  MODE 1: cf / (cf acc) if cf acc > 1e-9 else 0 (OSEM, A14)
-template <int MODE>
-__device__ __forceinline__ float brick_x(int ev, int ev0, const float *__restrict__ cf, const float *__restrict__ v,
-                                         const int *__restrict__ perm)
-{
-    const float c = __ldg(cf + ev);
-    if (MODE == 0) return c * __ldg(v + (perm ? (int64_t)__ldg(perm + ev) : (int64_t)(ev - ev0)));
-    const float ybar = c * __ldg(v + (ev - ev0));
-    return (ybar > 1e-9f) ? c * (1.f / ybar) : 0.f;
-}
-
-// Adjoint of one chunk.  The brick is staged in int32 fixed point (native shared atomics).  One scale per chunk must
-// serve every value in it, and OSEM ratios span decades (an event whose TOF window sits outside the activity has a tiny
-// expectation), so the scale is tied to the chunk's MEDIAN |x| (exponent histogram), not to its maximum:
-//   |x| <= T = 2^kBrHead * 2^ceil(log2 median)   fixed point with scale lim / T: quantum T / lim per term
-//   |x| >  T, Inf, NaN                           float atomics on the image, like the per-event path (exact, slow, rare)
-#ifndef JP_BR_HEAD
-#define JP_BR_HEAD 4
-#endif
-constexpr int kBrHead = JP_BR_HEAD;
-
-template <int MODE>
-__global__ void __launch_bounds__(kBrT, JP_BR_MINB)
-    k_brick_back(const BrickChunk *__restrict__ chunks, const BrickPiece *__restrict__ pieces, const float *__restrict__ cf,
-                 const float *__restrict__ v, const int *__restrict__ perm, Geom g, G1Tab gt, int ev0, float gmax, int vec_ok,
-                 float *__restrict__ img)
-{
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    int *B = reinterpret_cast<int *>(smem_raw);
-    float2 *g1 = reinterpret_cast<float2 *>(smem_raw + sizeof(int) * kBrVox);
-    __shared__ int hist[256];
-    __shared__ float T_sm;
-    const int tid = threadIdx.x, lane = tid & 31;
-    const BrickChunk ch = chunks[blockIdx.x];
-    const BrickOrg o = brick_org(ch, g);
-    if (tid < 256) hist[tid] = 0;
-    for (int i = tid; i < gt.n; i += kBrT) g1[i] = __ldg(gt.tab + i);
-    for (int idx = tid; idx < kBrVox; idx += kBrT) B[idx] = 0;
-    __syncthreads();
-    // histogram of the float exponents of the chunk's values (zeros left out)
-#pragma unroll 1
-    for (int m = 0; m < kBrPer; ++m) {
-        const int j = tid + m * kBrT;
-        const float xj = (j < ch.count) ? brick_x<MODE>(pieces[ch.first + j].ev, ev0, cf, v, perm) : 0.f;
-        const int ex = (xj != 0.f) ? (int)((__float_as_uint(xj) >> 23) & 0xffu) : -1;
-        const unsigned peers = __match_any_sync(0xffffffffu, ex);
-        if (ex >= 0 && lane == __ffs(peers) - 1) atomicAdd(&hist[ex], __popc(peers));
-    }
-    __syncthreads();
-    if (tid < 32) { // median exponent: 8 bins per lane, scan over the lanes
-        int c[8], tot = 0;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            c[k] = hist[tid * 8 + k];
-            tot += c[k];
-        }
-        int incl = tot;
-        for (int s = 1; s < 32; s <<= 1) {
-            const int up = __shfl_up_sync(0xffffffffu, incl, s);
-            if (tid >= s) incl += up;
-        }
-        const int all = __shfl_sync(0xffffffffu, incl, 31);
-        const int half = (all + 1) >> 1;
-        int run = incl - tot, emed = 256;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            run += c[k];
-            if (emed == 256 && run >= half && c[k] > 0) emed = tid * 8 + k;
-        }
-        for (int s = 16; s > 0; s >>= 1) emed = min(emed, __shfl_xor_sync(0xffffffffu, emed, s));
-        if (tid == 0) {
-            // 2^(emed - 127 + 1) bounds the median from above; an exponent near the top of the range leaves no head room
-            const int et = min(emed + 1 + kBrHead, 254);
-            T_sm = (all > 0 && emed < 255) ? __uint_as_float((unsigned)et << 23) : 0.f;
-        }
-    }
-    __syncthreads();
-    const float T = T_sm;
-    const uint32_t gbase = smem_addr(g1) - ((uint32_t)kMagicI << 3);
-    const float xedge = gt.xedge;
-    // fixed point: a voxel receives at most ch.mcount terms (counted by the plan), each at most gmax lim in magnitude
-    // (gmax = G(0) >= every TOF weight, |x| <= T), plus one rounding unit per term
-    const float lim = fminf(1073741824.f, (2147483648.f - 2.f * (float)ch.mcount) / ((float)ch.mcount * gmax));
-    const float Sc = (T > 0.f) ? lim / T : 0.f, invS = (T > 0.f) ? T / lim : 0.f;
-    const uint32_t bbase = smem_addr(B) - (uint32_t)kMagicI * (uint32_t)((kBrRow + 1) * 4);
-#pragma unroll 1
-    for (int j = tid; j < ch.count; j += kBrT) {
-        const float4 *rec = reinterpret_cast<const float4 *>(pieces + ch.first + j);
-        const float4 r0 = __ldg(rec), r1 = __ldg(rec + 1);
-        const float a1 = r0.x, b1 = r0.y, a2 = r0.z, b2 = r0.w, x0 = r1.x, dx = r1.y;
-        const int pl_nk = __float_as_int(r1.z);
-        const int nk = pl_nk & 0xff, pl0 = pl_nk >> 8;
-        const float xj = brick_x<MODE>(__float_as_int(r1.w), ev0, cf, v, perm); // (again: cheaper than keeping it)
-        if (xj == 0.f) continue;
-        if (fabsf(xj) <= T) {
-            uint32_t row = bbase + (uint32_t)pl0 * (uint32_t)(kBrPlane * 4);
-            const float xs = xj * Sc;
-            float fk = 0.f;
-#pragma unroll 2
-            for (int k = 0; k < nk; ++k) {
-                const float u1 = fmaf(b1, fk, a1), u2 = fmaf(b2, fk, a2);
-                const float t1 = __fadd_rd(u1, kMagic), t2 = __fadd_rd(u2, kMagic);
-                const float w1 = u1 - (t1 - kMagic), w2 = u2 - (t2 - kMagic);
-                const uint32_t ad = row + __float_as_uint(t1) * (uint32_t)(kBrRow * 4) + (__float_as_uint(t2) << 2);
-                const float xw = xs * g1_weight(gbase, xedge, fmaf(dx, fk, x0));
-                const float xb = xw * w1, xa = xw - xb;
-                const float xa1 = xa * w2, xb1 = xb * w2;
-                reds_add<0>(ad, __float2int_rn(xa - xa1));
-                reds_add<4>(ad, __float2int_rn(xa1));
-                reds_add<kBrRow * 4>(ad, __float2int_rn(xb - xb1));
-                reds_add<kBrRow * 4 + 4>(ad, __float2int_rn(xb1));
-                fk += 1.f;
-                row += kBrPlane * 4;
-            }
-        } else { // far above the chunk's median, or not finite: float atomics on the image
-#pragma unroll 1
-            for (int k = 0; k < nk; ++k) {
-                const float fk = (float)k;
-                const float u1 = fmaf(b1, fk, a1), u2 = fmaf(b2, fk, a2);
-                const float f1 = floorf(u1), f2 = floorf(u2);
-                const float w1 = u1 - f1, w2 = u2 - f2;
-                const float w = g1_weight(gbase, xedge, fmaf(dx, fk, x0));
-                if (w == 0.f) continue;
-                const int i = o.i0 + pl0 + k, k1 = o.k1_0 + (int)f1, k2 = o.k2_0 + (int)f2;
-                float *ptr = img + (int64_t)i * o.sp + (int64_t)k1 * o.s1 + k2;
-                const float x = xj * w;
-                const float xa = x * (1.f - w1), xb = x * w1, m2 = 1.f - w2;
-                const bool in1a = (unsigned)k1 < (unsigned)o.n1, in1b = (unsigned)(k1 + 1) < (unsigned)o.n1;
-                const bool in2a = (unsigned)k2 < (unsigned)o.n2, in2b = (unsigned)(k2 + 1) < (unsigned)o.n2;
-                if (in1a && in2a) atomicAdd(ptr, xa * m2);
-                if (in1a && in2b) atomicAdd(ptr + 1, xa * w2);
-                if (in1b && in2a) atomicAdd(ptr + o.s1, xb * m2);
-                if (in1b && in2b) atomicAdd(ptr + o.s1 + 1, xb * w2);
-            }
-        }
-    }
-    __syncthreads();
-    if (!(T > 0.f)) return;
-    // ---- flush: per row kBr2 / 4 aligned groups of four voxels and the two columns beyond them
-    constexpr int kGroups = kBr2 / 4;
-    constexpr int kOps = kGroups + 2;
-    for (int op = tid; op < kBrP * kBrC1 * kOps; op += kBrT) {
-        const int gi = op % kOps, r = op / kOps;
-        const int c1 = r % kBrC1, pl = r / kBrC1;
-        const int i = o.i0 + pl, k1 = o.k1_0 + c1;
-        if (i >= o.np || (unsigned)k1 >= (unsigned)o.n1) continue;
-        const int *src = B + r * kBrRow;
-        float *dst = img + (int64_t)i * o.sp + (int64_t)k1 * o.s1 + o.k2_0;
-        if (gi >= kGroups) { // scalar columns kBr2 and kBr2 + 1
-            const int c2 = kBr2 + (gi - kGroups);
-            const int q = src[c2];
-            if (q != 0 && (unsigned)(o.k2_0 + c2) < (unsigned)o.n2) atomicAdd(dst + c2, (float)q * invS);
-        } else {
-            const int c2 = 4 * gi;
-            const int q0 = src[c2], q1 = src[c2 + 1], q2 = src[c2 + 2], q3 = src[c2 + 3];
-            if ((q0 | q1 | q2 | q3) == 0) continue;
-            const int k2 = o.k2_0 + c2;
-            if (vec_ok && k2 >= 0 && k2 + 3 < o.n2) {
-                atomicAdd(reinterpret_cast<float4 *>(dst + c2),
-                          make_float4((float)q0 * invS, (float)q1 * invS, (float)q2 * invS, (float)q3 * invS));
-            } else {
-                if (q0 != 0 && (unsigned)k2 < (unsigned)o.n2) atomicAdd(dst + c2, (float)q0 * invS);
-                if (q1 != 0 && (unsigned)(k2 + 1) < (unsigned)o.n2) atomicAdd(dst + c2 + 1, (float)q1 * invS);
-                if (q2 != 0 && (unsigned)(k2 + 2) < (unsigned)o.n2) atomicAdd(dst + c2 + 2, (float)q2 * invS);
-                if (q3 != 0 && (unsigned)(k2 + 3) < (unsigned)o.n2) atomicAdd(dst + c2 + 3, (float)q3 * invS);
-            }
-        }
-    }
-}
-
 // p[io] = cf acc  (MODE 0)  or the OSEM ratio 1 / (cf acc)  (MODE 1) for the events [first, first + count) of the sorted
 // list that have pieces (principal axis 0 / 1)
 __global__ void __launch_bounds__(256) k_brick_finish(const float *__restrict__ cf, const float *__restrict__ acc, int64_t first,
@@ -624,7 +399,6 @@ __global__ void __launch_bounds__(256) k_brick_finish(const float *__restrict__ 
     p[perm ? (int64_t)perm[e] : c + io_off] = out;
 }
 
-constexpr size_t brick_smem(int g1n) { return sizeof(float) * (size_t)kBrVox + sizeof(float2) * (size_t)g1n; }
 constexpr size_t brick_smem_fwd(int g1n) { return sizeof(float) * (size_t)kFwVox + sizeof(float2) * (size_t)g1n; }
 
 } // namespace
@@ -640,7 +414,6 @@ struct BrickSet {
     int g1n = 0;
     float gmax = 1.f;
     int64_t n_chunks = 0;
-    bool counted = false;                      // BrickChunk::mcount holds the counted terms (path 4)
 };
 
 bool brick_supported(const Geom &g, const Tof &t, int n_subsets)
@@ -753,16 +526,14 @@ cudaError_t brick_set_create(const Lors &l, const int16_t *tb, int64_t n, const 
                         c.b1 = (short)((b / nb[2]) % nb[1]);
                         c.bp = (short)(b / (nb[2] * nb[1]));
                         c.axis = (short)a;
-                        c.mcount = c.count; // until brick_set_count_terms() has run
                         c.pad = (int)(at / kBrChunk); // slice number inside its brick (launch order, below)
                         h_chunks.push_back(c);
                     }
                 }
             bs->chunk_count[(size_t)m] = (int)h_chunks.size() - bs->chunk_first[(size_t)m];
             // launch order: the k-th slices of all bricks before the (k+1)-th, so that the CTAs in flight at any time
-            // work on different bricks instead of ~40 chunks of one central brick side by side: the flushes of the staged
-            // adjoint and the brick loads do not pile up on one brick's voxels (a small effect: configs[4] iteration
-            // 16.43 -> 16.39 ms, staged 14.35 -> 14.27 ms, A/B in one run)
+            // work on different bricks instead of ~40 chunks of one central brick side by side: the brick loads do not
+            // pile up on one brick's voxels (a small effect: configs[4] iteration 16.43 -> 16.39 ms, A/B in one run)
 #if JP_BR_ROUND_ROBIN
             std::stable_sort(h_chunks.begin() + bs->chunk_first[(size_t)m], h_chunks.end(), [&](const BrickChunk &x, const BrickChunk &y) {
                 return (x.pad < y.pad);
@@ -791,18 +562,6 @@ fail:
 #undef JP_BR_TRY
 }
 
-// path 4 only: count, per chunk, the terms the most-hit voxel receives (k_brick_maxcount); once per brick set
-cudaError_t brick_set_count_terms(BrickSet *bs, cudaStream_t st)
-{
-    if (bs->counted || bs->n_chunks == 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(k_brick_maxcount, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
-    if (e != cudaSuccess) return e;
-    k_brick_maxcount<<<(unsigned)bs->n_chunks, kBrT, sizeof(int) * kBrVox, st>>>(bs->chunks, bs->pieces);
-    e = cudaGetLastError();
-    if (e == cudaSuccess) bs->counted = true;
-    return e;
-}
-
 const float *brick_set_cf(const BrickSet *bs) { return bs->cf; }
 float *brick_set_acc(const BrickSet *bs) { return bs->acc; }
 
@@ -810,10 +569,7 @@ float *brick_set_acc(const BrickSet *bs) { return bs->acc; }
 // "done" flag would leave the second GPU of a hybrid handle at the 48 KB default)
 static cudaError_t brick_attr()
 {
-    cudaError_t e = cudaFuncSetAttribute(k_brick_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_brick_back<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_brick_back<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
-    return e;
+    return cudaFuncSetAttribute(k_brick_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
 }
 
 // acc[e - ev0] += sum_k G bilinear over the pieces of subset m (acc: zeroed by the caller, one float per event of the
@@ -874,33 +630,6 @@ cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const 
                                                                     bs->pieces, img, g, gt, (int)ev0, acc);
     e = cudaGetLastError();
     if (!(table && table->n == bs->g1n)) cudaFreeAsync((void *)gt.tab, st);
-    return e;
-}
-
-// img += A_m^T x over the events with pieces.  mode 0: x = cf v[io] (v = y; io = perm[e] or e - ev0);
-// mode 1: v = acc of launch_brick_fwd, x = cf / (cf acc) if cf acc > 1e-9 else 0 (the OSEM ratio, reading A14)
-cudaError_t launch_brick_back(const BrickSet *bs, int m, int mode, const float *v, const int *perm, const Geom &g, const Tof &t,
-                              int64_t ev0, float *img, cudaStream_t st)
-{
-    const int nc = bs->chunk_count[(size_t)m];
-    if (nc == 0) return cudaSuccess;
-    cudaError_t e = brick_attr();
-    // the head room of the fixed-point staging: counted on the first staged adjoint of the plan (stream-ordered; a plan
-    // is used from one stream at a time)
-    if (e == cudaSuccess) e = brick_set_count_terms(const_cast<BrickSet *>(bs), st);
-    if (e != cudaSuccess) return e;
-    G1Tab gt{};
-    e = g1tab_create(t, bs->g1n, st, &gt);
-    if (e != cudaSuccess) return e;
-    const int vec_ok = (g.n[2] % 4 == 0) && ((uintptr_t)img % 16 == 0);
-    const BrickChunk *ch = bs->chunks + bs->chunk_first[(size_t)m];
-    const size_t smem = brick_smem(bs->g1n);
-    if (mode == 1)
-        k_brick_back<1><<<(unsigned)nc, kBrT, smem, st>>>(ch, bs->pieces, bs->cf, v, nullptr, g, gt, (int)ev0, bs->gmax, vec_ok, img);
-    else
-        k_brick_back<0><<<(unsigned)nc, kBrT, smem, st>>>(ch, bs->pieces, bs->cf, v, perm, g, gt, (int)ev0, bs->gmax, vec_ok, img);
-    e = cudaGetLastError();
-    cudaFreeAsync((void *)gt.tab, st);
     return e;
 }
 

@@ -155,9 +155,6 @@ cudaError_t lm_plan_bricks(LmPlan *pl, cudaStream_t st, const BrickSet **out);
 // table: the G1 table of t if the caller already has one (else made and freed here, stream-ordered)
 cudaError_t launch_brick_fwd(const BrickSet *bs, int m, const float *img, const Geom &g, const Tof &t, int64_t ev0, float *acc,
                              cudaStream_t st, const G1Tab *table = nullptr);
-// img += A_m^T x.  mode 0: x = cf v[perm ? perm[e] : e - ev0];  mode 1: v = acc, x = cf / (cf acc) if cf acc > 1e-9 else 0
-cudaError_t launch_brick_back(const BrickSet *bs, int m, int mode, const float *v, const int *perm, const Geom &g, const Tof &t,
-                              int64_t ev0, float *img, cudaStream_t st);
 // p[perm ? perm[e] : e - first + io_off] = cf acc[e - ev0] (mode 0) or its OSEM ratio (mode 1), e in [first, first + count)
 cudaError_t launch_brick_finish(const BrickSet *bs, const float *acc, int64_t first, int64_t count, int64_t ev0, const int *perm,
                                 int64_t io_off, int mode, float *p, cudaStream_t st);

@@ -195,8 +195,8 @@ def test_config3_full_tof_lm(cuda_device, phantom_dev, events_full):
     assert_back(jp.jp_back_tof_lm_planned(plan, ys), bref)
     bd = jp.jp_back_tof_lm_planned(plan, y)
     assert adj_gap(pp, y, imgd, bd) <= ADJ_GAP
-    # the other kernel paths of the same plan at full size: quad image (2), adjoint staged in the image bricks (4)
-    for path in (2, 4):
+    # the other kernel paths of the same plan at full size: quad image (2), image bricks forward + float adjoint (3)
+    for path in (2, 3):
         plan.set_path(path)
         assert_fwd(jp.jp_fwd_tof_lm_planned(plan, imgd)[idx], ref)
         assert_back(jp.jp_back_tof_lm_planned(plan, ys), bref)
@@ -218,10 +218,6 @@ def test_config4_osem_full_image(cuda_device, phantom_dev, events_full):
     x = torch.ones(G.n, device=cuda_device)
     plan = jp.LmPlan(xs, xe, tb, G.n, G.origin, G.voxsize, tof, n_subsets=20)
     jp.jp_lm_osem_planned(plan, sens, x, n_iter=3)             # the plan's choice: image bricks forward, float adjoint
-    # (the opt-in staged adjoint, path 4, is on record for the whole config: bench.py --config 4 --check, parity.paths in
-    #  profiles/r02b_parity.txt -- rel-L2 3.1e-6 on 40 M events.  On this 4 M-event cut the reconstruction is noisy enough
-    #  (many near-empty voxels after three iterations) for the update to amplify its fixed-point rounding to 2e-3: the
-    #  ill-conditioned case include/joseph_b200.h warns about.)
     x2 = torch.ones(G.n, device=cuda_device)
     jp.jp_lm_osem(xs, xe, tb, sens, x2, G.origin, G.voxsize, tof, n_subsets=20, n_iter=3)
     sens32 = sens.cpu().numpy()
