@@ -50,7 +50,7 @@ N_SM = 148
 # ncu figures of the dominant kernels (dram bytes per launch, issue-slot / l1tex / L2 utilisation), read from the text
 # summary of the one `ncu --set full` capture per config committed under profiles/ (the file names its commands and
 # the commit it was taken at); a number measured under the profiler is never a bench value -- these only explain it
-NCU_CSV = os.path.join(ROOT, "profiles", "r02b_kernel_metrics.csv")
+NCU_CSV = os.path.join(ROOT, "profiles", "r03_kernel_metrics.csv")
 
 
 def ncu_metrics():
@@ -69,7 +69,16 @@ def ncu_note(c, direction):
     if not r:
         return None
     f = lambda k: float(r[k]) if r.get(k) not in (None, "") else None
-    return {"source": "profiles/r02b_kernel_metrics.csv (ncu --set full, commit %s)" % r.get("commit", "?"), "kernel": r["kernel"],
+    dur = (f("duration_ms") or 0.0) * 1e-3
+    rate = lambda k: (f(k) / dur) if (dur > 0 and f(k) is not None) else None
+    atomics = {   # north_star (d) "atomic throughput": counts per launch (profiles/r03_kernel_metrics.md) over ncu's duration
+        "shared_atomic_warp_instr_per_s": rate("shared_atom_inst"), "global_red_warp_instr_per_s": rate("red_inst"),
+        "global_red_sectors_per_s": rate("red_sectors"),
+        "global_red_GBps_at_l2": (rate("red_sectors") * 32 / 1e9) if rate("red_sectors") is not None else None,
+        "shared_wavefronts_per_s": rate("shared_wavefronts"),
+        "shared_bank_conflict_share": (f("shared_bank_conflicts") / f("shared_wavefronts")) if f("shared_wavefronts") else None}
+    return {"source": "profiles/r03_kernel_metrics.csv (ncu --set full, commit %s)" % r.get("commit", "?"), "kernel": r["kernel"],
+            "atomics": atomics,
             "duration_ms": f("duration_ms"), "dram_bytes_per_launch": (f("dram_read_bytes") or 0) + (f("dram_write_bytes") or 0),
             "issue_slots_busy_pct": f("issue_pct"), "l1tex_throughput_pct": f("l1tex_pct"), "l2_throughput_pct": f("lts_pct"),
             "fma_pipe_pct": f("fma_pipe_pct"), "l1_hit_pct": f("l1_hit_pct"), "l2_hit_pct": f("l2_hit_pct"),
